@@ -1,0 +1,168 @@
+"""CPU oracle -- TEST INFRASTRUCTURE, not the product.
+
+ctypes wrapper around `bj_oracle.c` (plain fp64 C written from the paper; see that file's
+header for citations, build flags and the list of pins) plus a dense numpy path (`dense.py`).
+Nothing here imports, links or shares code with the CUDA path.  Allowed callers: `tests/`,
+`__graft_entry__.smoke()`, and `bench.py`'s `cpu_baseline` / `--impl reference` legs.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "bj_oracle.c")
+_LIB = os.path.join(_HERE, "libbj_oracle.so")
+DEFAULT_SEED = 0x2410_02408
+TOL_BREAKDOWN = 1e-12
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-fopenmp", _SRC, "-o", _LIB, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = C.CDLL(_LIB)
+        i64, i32, dbl, vp = C.c_int64, C.c_int, C.c_double, C.c_void_p
+        lib.orc_spmv.argtypes = [i64, vp, vp, vp, vp, vp]
+        lib.orc_extract.argtypes = [i64, vp, vp, vp, i64, vp]
+        lib.orc_factor.argtypes = [i64, i64, vp, C.POINTER(i64)]
+        lib.orc_factor.restype = i32
+        lib.orc_solve_L.argtypes = [i64, i64, vp, vp, vp]
+        lib.orc_solve_Lt.argtypes = [i64, i64, vp, vp, vp]
+        lib.orc_apply.argtypes = [i64, i64, vp, vp, vp, vp]
+        lib.orc_op_apply.argtypes = [i64, vp, vp, vp, i64, vp, vp, vp, vp]
+        lib.orc_seeded_vector.argtypes = [C.c_uint64, i64, vp]
+        lib.orc_lanczos.argtypes = [i64, vp, vp, vp, i64, vp, vp, i32, i32, dbl, vp, vp, C.POINTER(i32)]
+        lib.orc_lanczos.restype = i32
+        lib.orc_tridiag_extremes.argtypes = [i32, vp, vp] + [C.POINTER(dbl)] * 4
+        lib.orc_tridiag_all.argtypes = [i32, vp, vp, vp]
+        lib.orc_num_threads.restype = i32
+        for f in ("orc_spmv", "orc_extract", "orc_solve_L", "orc_solve_Lt", "orc_apply", "orc_op_apply",
+                  "orc_seeded_vector", "orc_tridiag_extremes", "orc_tridiag_all"):
+            getattr(lib, f).restype = None
+        _lib = lib
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+class NotSPD(Exception):
+    def __init__(self, bad_block: int):
+        super().__init__(f"diagonal block {bad_block} is not positive definite")
+        self.bad_block = bad_block
+
+
+def spmv(A, x):
+    x = _f64(x)
+    y = np.empty(A.n)
+    _load().orc_spmv(A.n, _p(A.row_ptr), _p(A.col_idx), _p(A.val), _p(x), _p(y))
+    return y
+
+
+def extract(A, b: int) -> np.ndarray:
+    nblocks = (A.n + b - 1) // b
+    D = np.empty((nblocks, b, b))
+    _load().orc_extract(A.n, _p(A.row_ptr), _p(A.col_idx), _p(A.val), b, _p(D))
+    return D
+
+
+def factor(n: int, b: int, D: np.ndarray) -> np.ndarray:
+    L = _f64(D).copy()
+    bad = C.c_int64(-1)
+    rc = _load().orc_factor(n, b, _p(L), C.byref(bad))
+    if rc != 0:
+        raise NotSPD(int(bad.value))
+    return L
+
+
+class Precond:
+    """setup(A, b): extract + factor.  b == 0: identity (operator = A)."""
+
+    def __init__(self, A, b: int):
+        self.A, self.b, self.n = A, int(b), A.n
+        self.L = factor(A.n, b, extract(A, b)) if b > 0 else None
+        self._tmp = np.empty(2 * A.n)
+
+    def solve_L(self, r):
+        r = _f64(r); y = np.empty(self.n)
+        _load().orc_solve_L(self.n, self.b, _p(self.L), _p(r), _p(y))
+        return y
+
+    def solve_Lt(self, y):
+        y = _f64(y); x = np.empty(self.n)
+        _load().orc_solve_Lt(self.n, self.b, _p(self.L), _p(y), _p(x))
+        return x
+
+    def apply(self, r):
+        r = _f64(r); z = np.empty(self.n)
+        _load().orc_apply(self.n, self.b, _p(self.L), _p(r), _p(z), _p(self._tmp))
+        return z
+
+    def op_apply(self, x):
+        x = _f64(x); y = np.empty(self.n)
+        A = self.A
+        Lp = _p(self.L) if self.L is not None else None
+        _load().orc_op_apply(self.n, _p(A.row_ptr), _p(A.col_idx), _p(A.val), self.b, Lp, _p(x), _p(y), _p(self._tmp))
+        return y
+
+    def lanczos(self, m: int, v0=None, reorth: bool = True, seed: int = DEFAULT_SEED, tol_bd: float = TOL_BREAKDOWN):
+        v0 = seeded_vector(seed, self.n) if v0 is None else _f64(v0)
+        alpha = np.zeros(m); beta = np.zeros(m)
+        m_eff = C.c_int(0)
+        A = self.A
+        Lp = _p(self.L) if self.L is not None else None
+        rc = _load().orc_lanczos(self.n, _p(A.row_ptr), _p(A.col_idx), _p(A.val), self.b, Lp, _p(v0), m,
+                                 int(bool(reorth)), tol_bd, _p(alpha), _p(beta), C.byref(m_eff))
+        if rc != 0:
+            raise MemoryError("oracle lanczos allocation failed")
+        k = m_eff.value
+        return alpha[:k].copy(), beta[:k].copy()
+
+    def cond_estimate(self, m: int, **kw):
+        alpha, beta = self.lanczos(m, **kw)
+        tmin, tmax, rmin, rmax = tridiag_extremes(alpha, beta)
+        return {"lmin": tmin, "lmax": tmax, "kappa": tmax / tmin, "res_min": rmin, "res_max": rmax,
+                "iters_done": len(alpha), "alpha": alpha, "beta": beta}
+
+
+def seeded_vector(seed: int, n: int) -> np.ndarray:
+    v = np.empty(n)
+    _load().orc_seeded_vector(C.c_uint64(seed & 0xFFFFFFFFFFFFFFFF), n, _p(v))
+    return v
+
+
+def tridiag_extremes(alpha, beta):
+    alpha, beta = _f64(alpha), _f64(beta)
+    out = [C.c_double() for _ in range(4)]
+    _load().orc_tridiag_extremes(len(alpha), _p(alpha), _p(beta), *[C.byref(o) for o in out])
+    return tuple(o.value for o in out)
+
+
+def tridiag_all(alpha, beta) -> np.ndarray:
+    alpha, beta = _f64(alpha), _f64(beta)
+    out = np.empty(len(alpha))
+    _load().orc_tridiag_all(len(alpha), _p(alpha), _p(beta), _p(out))
+    return out

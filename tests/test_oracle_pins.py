@@ -1,0 +1,367 @@
+"""Pins for the CPU oracle (CPU only).  Each test checks the oracle against something OTHER than
+itself: closed forms, invariants, library routines on special cases, dense brute force, or the
+few things the paper fixes (cited).  A plausible slip anywhere in oracle/bj_oracle.c (dropped
+term, wrong sign or index, transposed operand) fails at least one of them."""
+import os
+
+import numpy as np
+import pytest
+import scipy.linalg as sla
+
+import oracle
+from oracle import dense as odense
+from paper_2410_02408_b200 import workloads as W
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")) as fh:
+    for line in fh:
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            GOLD[line[0]] = line[1]
+
+
+def mu(n):
+    k = np.arange(1, n + 1)
+    return 2.0 - 2.0 * np.cos(k * np.pi / (n + 1))
+
+
+def dense_precond_spectrum(A, b):
+    """Independent numpy/scipy restatement: L = blockdiag(chol(D_k)), eig(L^-1 A L^-T)."""
+    Ad = A.to_dense()
+    n = A.n
+    Linv = np.zeros((n, n))
+    for lo in range(0, n, b):
+        hi = min(lo + b, n)
+        Lk = np.linalg.cholesky(Ad[lo:hi, lo:hi])
+        Linv[lo:hi, lo:hi] = sla.solve_triangular(Lk, np.eye(hi - lo), lower=True)
+    M = Linv @ Ad @ Linv.T
+    return np.linalg.eigvalsh(0.5 * (M + M.T)), M
+
+
+# ---------------------------------------------------------------- SpMV ------------------------------
+@pytest.mark.parametrize("dims", [(17,), (9, 7), (5, 4, 6)])
+def test_spmv_laplacian_eigenvectors(dims):
+    """A sin-mode = lambda sin-mode with lambda = sum mu_k(n_d)  (closed form)."""
+    A = W.laplacian(dims)
+    rng = np.random.default_rng(1)
+    for _ in range(3):
+        ks = [int(rng.integers(1, s + 1)) for s in dims]
+        grids = np.meshgrid(*[np.arange(1, s + 1) for s in dims], indexing="ij")
+        v = np.ones(dims)
+        lam = 0.0
+        for g, k, s in zip(grids, ks, dims):
+            v = v * np.sin(g * k * np.pi / (s + 1))
+            lam += 2.0 - 2.0 * np.cos(k * np.pi / (s + 1))
+        v = v.ravel(order="F")  # first dimension fastest
+        y = oracle.spmv(A, v)
+        assert np.abs(y - lam * v).max() < 1e-13
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_spmv_matches_scipy_and_is_not_symmetric_blind(cfg):
+    """Library routine (scipy CSR matvec) on every config; plus a nonsymmetric matrix so that a
+    transposed gather (x[row] / val^T) cannot pass."""
+    A = W.build(cfg, "tiny")
+    x = W.seeded_vector(7, A.n)
+    y = oracle.spmv(A, x)
+    assert np.allclose(y, A.to_scipy() @ x, rtol=1e-14, atol=1e-13 * np.abs(y).max())
+    S = A.to_scipy().tolil()
+    S[0, A.n - 1] = 3.5  # break symmetry
+    B = W.from_scipy(S.tocsr())
+    assert np.allclose(oracle.spmv(B, x), B.to_dense() @ x, rtol=1e-13, atol=1e-12)
+
+
+# ---------------------------------------------------------------- extraction ------------------------
+@pytest.mark.parametrize("b", [1, 3, 4, 7, 16])
+def test_extract_is_dense_slicing_like_the_papers_listing(b):
+    """block = A[i:i+bs, j:j+bs]; only the diagonal tiles; ragged last tile."""
+    A = W.build(3, "tiny")
+    Ad = A.to_dense()
+    D = oracle.extract(A, b)
+    n = A.n
+    for k, lo in enumerate(range(0, n, b)):
+        hi = min(lo + b, n)
+        ref = np.zeros((b, b))
+        ref[: hi - lo, : hi - lo] = Ad[lo:hi, lo:hi]
+        assert np.array_equal(D[k], ref)
+
+
+# ---------------------------------------------------------------- Cholesky / solves vs LAPACK --------
+@pytest.mark.parametrize("b", [1, 2, 3, 5, 8, 24, 32])
+def test_cholesky_and_solves_match_library_routines(b):
+    rng = np.random.default_rng(b)
+    nblocks = 5
+    n = nblocks * b - (1 if b > 2 else 0)  # ragged last block when b > 2
+    G = rng.normal(size=(nblocks, b, b))
+    D = np.einsum("kij,klj->kil", G, G) + 0.5 * np.eye(b)
+    if b > 2:
+        D[-1, b - 1, :] = 0.0
+        D[-1, :, b - 1] = 0.0
+    L = oracle.factor(n, b, D)
+    r = rng.normal(size=n)
+    P = oracle.Precond.__new__(oracle.Precond)
+    P.A, P.b, P.n, P.L, P._tmp = None, b, n, L, np.empty(2 * n)
+    y, x, z = P.solve_L(r), P.solve_Lt(r), P.apply(r)
+    for k, lo in enumerate(range(0, n, b)):
+        hi = min(lo + b, n)
+        nb = hi - lo
+        Lref = np.linalg.cholesky(D[k, :nb, :nb])
+        assert np.allclose(L[k, :nb, :nb], Lref, rtol=1e-12, atol=1e-13)
+        assert np.all(np.triu(L[k], 1) == 0.0)
+        assert np.allclose(y[lo:hi], sla.solve_triangular(Lref, r[lo:hi], lower=True), rtol=1e-10, atol=1e-12)
+        assert np.allclose(x[lo:hi], sla.solve_triangular(Lref.T, r[lo:hi], lower=False), rtol=1e-10, atol=1e-12)
+        assert np.allclose(z[lo:hi], np.linalg.solve(D[k, :nb, :nb], r[lo:hi]), rtol=1e-9, atol=1e-11)
+
+
+def test_cholesky_reads_only_lower_triangle_and_flags_non_spd():
+    D = np.array([[[4.0, 99.0], [2.0, 5.0]]])
+    L = oracle.factor(2, 2, D)
+    assert np.allclose(L[0], [[2.0, 0.0], [1.0, 2.0]])
+    bad = np.stack([np.eye(3), np.diag([1.0, -1.0, 1.0]), np.diag([1.0, 0.0, 1.0])])
+    with pytest.raises(oracle.NotSPD) as ei:
+        oracle.factor(9, 3, bad)
+    assert ei.value.bad_block == 1
+    with pytest.raises(oracle.NotSPD):
+        oracle.factor(3, 3, np.array([[[1.0, 0, 0], [0, np.nan, 0], [0, 0, 1.0]]]))
+
+
+# ---------------------------------------------------------------- the paper's own statements ---------
+def test_point_jacobi_is_the_papers_kernel():
+    """PAPER.md:234  M[idx] = 1/A[idx*N+idx]  ==> bj_apply(b=1) on r = 1 returns 1/a_ii."""
+    A = W.build(1, "full")
+    P = oracle.Precond(A, 1)
+    z = P.apply(np.ones(A.n))
+    assert np.allclose(z, 1.0 / A.to_dense().diagonal(), rtol=1e-15)
+
+
+def test_point_jacobi_operator_explicit_formula():
+    """b=1: A^_ij = a_ij / sqrt(a_ii a_jj)  (SURVEY 8(c) reading 1): a SpMV-only restatement."""
+    A = W.build(3, "tiny")
+    Ad = A.to_dense()
+    d = np.sqrt(Ad.diagonal())
+    x = W.seeded_vector(3, A.n)
+    assert np.allclose(oracle.Precond(A, 1).op_apply(x), (Ad / np.outer(d, d)) @ x, rtol=1e-12)
+
+
+@pytest.mark.parametrize("b", [2, 5, 8])
+def test_block_diagonal_model_gives_identity(b):
+    """PAPER.md:80  A = diag(A_1..A_k) with matching b  ==>  L^-1 A L^-T = I, op_apply(x) = x, kappa = 1."""
+    A = W.block_diagonal_spd(6, b)
+    P = oracle.Precond(A, b)
+    x = W.seeded_vector(11, A.n)
+    assert np.abs(P.op_apply(x) - x).max() < 1e-13
+    r = P.cond_estimate(20)
+    assert r["iters_done"] == 1 and abs(r["kappa"] - 1.0) < 1e-13
+
+
+def test_b_equals_N_gives_identity_and_breakdown_at_one():
+    A = W.build(2, "tiny")
+    P = oracle.Precond(A, A.n)
+    x = W.seeded_vector(5, A.n)
+    assert np.linalg.norm(P.op_apply(x) - x) / np.linalg.norm(x) < 1e-10
+    r = P.cond_estimate(30)
+    assert r["iters_done"] == 1
+    assert abs(r["lmin"] - 1.0) < 1e-10 and abs(r["lmax"] - 1.0) < 1e-10
+
+
+# ---------------------------------------------------------------- closed-form spectra ----------------
+def test_laplacian_2d_kappa_closed_form_dense_and_lanczos():
+    n = 32
+    A = W.laplacian((n, n))
+    m = mu(n)
+    lmin, lmax = 2 * m[0], 2 * m[-1]
+    assert abs(lmin - float(GOLD["lap2d_n32_lmin"])) < 1e-11
+    assert abs(lmax - float(GOLD["lap2d_n32_lmax"])) < 1e-11
+    assert abs(lmax / lmin - float(GOLD["lap2d_n32_kappa"])) < 1e-7
+    assert abs(lmax / lmin - 1.0 / np.tan(np.pi / 66) ** 2) < 1e-9
+    P = oracle.Precond(A, 0)
+    ev = odense.spectrum(P)
+    assert abs(ev[0] - lmin) < 1e-12 and abs(ev[-1] - lmax) < 1e-12
+    r = P.cond_estimate(400)  # long run with full reorthogonalisation converges to the true extremes
+    assert abs(r["lmin"] - lmin) < 1e-10 and abs(r["lmax"] - lmax) < 1e-10
+    # point Jacobi with constant diagonal leaves kappa unchanged
+    r1 = oracle.Precond(A, 1).cond_estimate(400)
+    assert abs(r1["kappa"] / (lmax / lmin) - 1.0) < 1e-9
+    assert abs(r1["lmax"] - lmax / 4.0) < 1e-10
+
+
+def test_laplacian_1d_full_lanczos_reproduces_every_eigenvalue():
+    n = 24
+    A = W.laplacian((n,))
+    P = oracle.Precond(A, 0)
+    alpha, beta = P.lanczos(n, reorth=True)
+    assert len(alpha) == n
+    ritz = oracle.tridiag_all(alpha, beta)
+    assert np.abs(ritz - mu(n)).max() < 1e-12
+
+
+def test_laplacian_3d_extremes():
+    dims = (6, 5, 7)
+    A = W.laplacian(dims)
+    lmin = sum(mu(s)[0] for s in dims)
+    lmax = sum(mu(s)[-1] for s in dims)
+    r = oracle.Precond(A, 0).cond_estimate(A.n)
+    assert abs(r["lmin"] - lmin) < 1e-11 and abs(r["lmax"] - lmax) < 1e-11
+
+
+def test_line_block_jacobi_closed_form_2d():
+    """b = n on the x-fastest 2D Laplacian: spectrum {(mu_k + mu_l)/(mu_k + 2)}."""
+    n = 32
+    A = W.laplacian((n, n))
+    m = mu(n)
+    # k = mode ACROSS lines (block index direction), l = mode ALONG the line: block = T_l + 2I ... derived:
+    # A = I (x) T + T (x) I ; M = I (x) (T + 2I) ; M^-1 A has eigenvalues (mu_l + mu_k)/(mu_l + 2)
+    spec = np.sort(((m[:, None] + m[None, :]) / (m[:, None] + 2.0)).ravel())
+    assert abs(spec[0] - float(GOLD["line2d_n32_lmin"])) < 1e-11
+    assert abs(spec[-1] - float(GOLD["line2d_n32_lmax"])) < 1e-11
+    assert abs(spec[-1] / spec[0] - float(GOLD["line2d_n32_kappa"])) < 1e-7
+    P = oracle.Precond(A, n)
+    ev = odense.spectrum(P)
+    assert np.abs(ev - spec).max() < 1e-12
+    r = P.cond_estimate(300)
+    assert abs(r["lmin"] - spec[0]) < 1e-10 and abs(r["lmax"] - spec[-1]) < 1e-10
+
+
+def test_line_and_plane_block_closed_forms_3d():
+    n = 6
+    A = W.laplacian((n, n, n))
+    m = mu(n)
+    a, b_, c = m[:, None, None], m[None, :, None], m[None, None, :]
+    line = np.sort(((a + b_ + c) / (a + 4.0)).ravel())
+    plane = np.sort(((a + b_ + c) / (a + b_ + 2.0)).ravel())
+    assert np.abs(odense.spectrum(oracle.Precond(A, n)) - line).max() < 1e-12
+    assert np.abs(odense.spectrum(oracle.Precond(A, n * n)) - plane).max() < 1e-12
+
+
+def test_anisotropic_closed_forms():
+    """cfg 4 with the cross term off, y fastest: lambda(A) = eps mu_k + mu_l; b = n: (eps mu_k + mu_l)/(mu_l + 2 eps)."""
+    n, eps = 12, 1e-2
+    A = W.config4(n, eps=eps, gamma_over_eps=0.0)
+    m = mu(n)
+    lamA = np.sort((eps * m[:, None] + m[None, :]).ravel())
+    assert np.abs(odense.spectrum(oracle.Precond(A, 0)) - lamA).max() < 1e-12
+    lamP = np.sort(((eps * m[:, None] + m[None, :]) / (m[None, :] + 2 * eps)).ravel())
+    assert np.abs(odense.spectrum(oracle.Precond(A, n)) - lamP).max() < 1e-12
+
+
+# ---------------------------------------------------------------- invariants -------------------------
+@pytest.mark.parametrize("cfg,b", [(1, 1), (1, 4), (2, 1), (2, 8)])
+def test_two_cyclic_spectrum_is_symmetric_about_one(cfg, b):
+    """5-/7-point stencils with b=1 or line-segment blocks: theta_min + theta_max = 2."""
+    A = W.build(cfg, "tiny")
+    ev = odense.spectrum(oracle.Precond(A, b))
+    assert abs(ev[0] + ev[-1] - 2.0) < 1e-11
+    r = oracle.Precond(A, b).cond_estimate(A.n)
+    assert abs(r["lmin"] + r["lmax"] - 2.0) < 1e-9
+
+
+def test_point_jacobi_is_invariant_under_diagonal_scaling_cfg3():
+    N = 512
+    ev_s = odense.spectrum(oracle.Precond(W.config3(N), 1))
+    ev_u = odense.spectrum(oracle.Precond(W.config3_unscaled(N), 1))
+    assert np.abs(ev_s - ev_u).max() < 1e-12
+    assert ev_s[0] > 1 - 1 / 1.01 - 1e-12 and ev_s[-1] < 1 + 1 / 1.01 + 1e-12  # strict diagonal dominance
+
+
+def test_cfg5_smallest_eigenvalue_is_the_shift():
+    """lambda_min(A) = sigma exactly, multiplicity 3 (rigid translations); nnz = 9 (3n-2)^3."""
+    A = W.config5(4)
+    assert A.nnz == 9 * (3 * 4 - 2) ** 3
+    ev = odense.spectrum(oracle.Precond(A, 0))
+    assert np.abs(ev[:3] - 1e-2).max() < 1e-12 and ev[3] > 1e-2 + 1e-6
+
+
+# ---------------------------------------------------------------- dense brute force ------------------
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (3, 32), (4, 16), (5, 3), (5, 24), (3, 7)])
+def test_op_apply_and_spectrum_match_dense_numpy(cfg, b, rel):
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    ev_ref, M = dense_precond_spectrum(A, b)
+    x = W.seeded_vector(13, A.n)
+    e2, ei = rel(P.op_apply(x), M @ x)
+    assert e2 < 1e-11 and ei < 1e-11
+    ev = odense.spectrum(P)
+    assert np.abs(ev - ev_ref).max() < 1e-9 * ev_ref[-1]
+    # apply = (L L^T)^-1 = blockdiag(D_k)^-1
+    Ad = A.to_dense()
+    z_ref = np.empty(A.n)
+    for lo in range(0, A.n, b):
+        hi = min(lo + b, A.n)
+        z_ref[lo:hi] = np.linalg.solve(Ad[lo:hi, lo:hi], x[lo:hi])
+    e2, _ = rel(P.apply(x), z_ref)
+    assert e2 < 1e-10
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (3, 32), (4, 16)])
+def test_lanczos_full_run_equals_dense_spectrum_and_interlaces(cfg, b):
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    ev_ref, _ = dense_precond_spectrum(A, b)
+    alpha, beta = P.lanczos(A.n, reorth=True)
+    if len(alpha) == A.n:
+        assert np.abs(oracle.tridiag_all(alpha, beta) - ev_ref).max() < 1e-9 * ev_ref[-1]
+    prev_min, prev_max = np.inf, -np.inf
+    for m in (2, 5, 10, 20, 40):
+        tmin, tmax, rmin, rmax = oracle.tridiag_extremes(alpha[:m], beta[:m])
+        assert tmin >= ev_ref[0] - 1e-12 and tmax <= ev_ref[-1] + 1e-12       # interlacing
+        assert tmin <= prev_min + 1e-13 and tmax >= prev_max - 1e-13          # monotone in m
+        # Ritz residual bound: an eigenvalue lies within res of each Ritz value
+        assert np.abs(ev_ref - tmin).min() <= rmin + 1e-12
+        assert np.abs(ev_ref - tmax).min() <= rmax + 1e-12
+        prev_min, prev_max = tmin, tmax
+
+
+def test_lanczos_matches_krylov_qr_brute_force():
+    """m-step Ritz values = eigenvalues of Q^T A^ Q with Q an orthonormal basis of the Krylov space."""
+    A = W.build(1, "tiny")
+    b, m = 4, 8
+    P = oracle.Precond(A, b)
+    _, M = dense_precond_spectrum(A, b)
+    v0 = oracle.seeded_vector(oracle.DEFAULT_SEED, A.n)
+    K = np.empty((A.n, m), dtype=np.longdouble)
+    v = v0.astype(np.longdouble)
+    Ml = M.astype(np.longdouble)
+    for j in range(m):
+        v = v / np.sqrt((v * v).sum())
+        K[:, j] = v
+        v = Ml @ v
+    Q, _ = np.linalg.qr(K.astype(np.float64))
+    ritz_ref = np.linalg.eigvalsh(Q.T @ M @ Q)
+    alpha, beta = P.lanczos(m, reorth=True)
+    ritz = oracle.tridiag_all(alpha, beta)
+    assert np.abs(ritz - ritz_ref).max() < 1e-9
+
+
+def test_no_reorth_equals_full_reorth_for_few_steps():
+    A = W.build(2, "tiny")
+    P = oracle.Precond(A, 8)
+    a1, b1 = P.lanczos(6, reorth=True)
+    a0, b0 = P.lanczos(6, reorth=False)
+    assert np.allclose(a1, a0, rtol=1e-10) and np.allclose(b1, b0, rtol=1e-10)
+
+
+def test_tridiag_bisection_matches_lapack():
+    rng = np.random.default_rng(5)
+    for m in (1, 2, 3, 17, 60):
+        d = rng.normal(size=m)
+        e = rng.normal(size=m)  # e[m-1] is the residual norm, not part of T
+        T = np.diag(d) + np.diag(e[: m - 1], 1) + np.diag(e[: m - 1], -1)
+        w, S = np.linalg.eigh(T)
+        assert np.abs(oracle.tridiag_all(d, e) - w).max() < 1e-13
+        tmin, tmax, rmin, rmax = oracle.tridiag_extremes(d, e)
+        assert abs(tmin - w[0]) < 1e-13 and abs(tmax - w[-1]) < 1e-13
+        assert abs(rmin - abs(e[m - 1]) * abs(S[-1, 0])) < 1e-10
+        assert abs(rmax - abs(e[m - 1]) * abs(S[-1, -1])) < 1e-10
+
+
+# ---------------------------------------------------------------- seeded vector ----------------------
+def test_seeded_vector_matches_published_splitmix64_sequence():
+    v = oracle.seeded_vector(0, 3)
+    for i in range(3):
+        z = int(GOLD[f"splitmix64_seed0_out{i}"], 16)
+        assert v[i] == 2.0 * ((z >> 11) / 2.0**53) - 1.0
+    big = oracle.seeded_vector(oracle.DEFAULT_SEED, 200000)
+    assert big.min() >= -1.0 and big.max() < 1.0
+    assert abs(big.mean()) < 5e-3 and abs(big.var() - 1.0 / 3.0) < 5e-3
+    # the input-generator module carries its own copy of the same integer steps
+    assert np.array_equal(big, W.seeded_vector(oracle.DEFAULT_SEED, 200000))
