@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run (contract in the task prompt; details in DESIGN.md section 7).
+
+A "step" is one application of the split-preconditioned operator y = L^-1 A L^-T x (bj_op_apply:
+backward block solve -> CSR SpMV -> forward block solve) on BASELINE.json configs[1]
+(3D 7-point variable-coefficient diffusion on 128^3, block-Jacobi b = 8, fp64), inputs resident in HBM.
+The same run also reports setup ms (extraction + batched Cholesky), bj_apply, the Lanczos kappa
+estimates kappa(A) -> kappa(A^), the roofline of the dominant kernel (CUDA events bracketed around
+each kernel by the library's profiling hooks), the end-to-end rate through the host-buffer entry
+point, and the CPU oracle timed on the host cores as a reported baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--block B] [--impl reference]
+
+N > 1: replicas only -- every rank runs the same problem independently; the
+value is the aggregate applies/s over all ranks with max-over-ranks timing.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2410_02408_b200 import workloads as W  # noqa: E402
+
+METRIC = "precond_operator_applies_per_s"
+UNIT = "applies/s"
+NOMINAL_HBM_GBS = 8000.0  # BASELINE.json north_star "~8 TB/s"
+
+
+def algorithmic_bytes(n: int, nnz: int, b: int) -> dict:
+    """SURVEY.md 8(d) / DESIGN.md section 6: bytes the method itself must move, per launch."""
+    spmv = 12 * nnz + 4 * (n + 1) + 16 * n
+    solve = (4 * n * (b + 1) + 16 * n) if b > 0 else 0
+    return {"spmv": spmv, "solve_L": solve, "solve_Lt": solve, "apply": solve,
+            "spmv_solve_L": spmv + solve, "op_apply": spmv + 2 * solve}
+
+
+def measured_peaks() -> tuple[float, str]:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40,
+                 "sw_thermal_slowdown": 0x20, "hw_power_brake_slowdown": 0x80}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def start(self):
+        if self.nv is not None:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._t:
+            self._t.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def time_oracle(A, b: int, budget_s: float, min_reps: int = 3):
+    import oracle
+    P = oracle.Precond(A, b)
+    x = W.seeded_vector(31, A.n)
+    P.op_apply(x)  # touch
+    reps, t0 = 0, time.perf_counter()
+    while True:
+        P.op_apply(x)
+        reps += 1
+        el = time.perf_counter() - t0
+        if reps >= min_reps and el >= budget_s:
+            break
+        if el > 4 * budget_s:
+            break
+    return reps / el, reps, oracle.num_threads()
+
+
+def run_reference(args, A, b: int):
+    """--impl reference: the CPU oracle, as it stands, on the host cores.  One step = one full operator apply."""
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    P = oracle.Precond(A, b)
+    x = W.seeded_vector(31, A.n)
+    for _ in range(max(1, min(args.warmup, 3))):
+        P.op_apply(x)
+    steps = min(args.steps, 200)  # bounded so the run ends within minutes
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        P.op_apply(x)
+    el = time.perf_counter() - t0
+    v = steps / el
+    cores = oracle.num_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": A.meta.get("name"), "n": A.n, "nnz": A.nnz, "block": b},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{steps} full operator applies (whole vector, N={A.n})"},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def aggregate_max(ms_local: float, world: int) -> float:
+    """max over ranks of the device-timed milliseconds (all_reduce MAX; identity for world == 1)."""
+    if world == 1:
+        return ms_local
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device="cuda" if dist.get_backend() == "nccl" else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2 = configs[1])")
+    ap.add_argument("--block", type=int, default=None)
+    ap.add_argument("--scale", default="full", choices=["full", "small", "tiny"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lanczos-iters", type=int, default=50)
+    ap.add_argument("--cpu-budget-s", type=float, default=10.0)
+    ap.add_argument("--spmv-kernel", type=int, default=-1)
+    ap.add_argument("--fuse", type=int, default=-1)
+    ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e (profiling runs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference" and int(os.environ.get("RANK", "0")) != 0:
+        return  # under torchrun only rank 0 runs the CPU reference arm
+    A = W.build(args.config, args.scale)
+    b = args.block if args.block is not None else W.BLOCK_SIZES[args.config][0]
+    if args.impl == "reference":
+        run_reference(args, A, b)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2410_02408_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    B.lib()  # fail loudly if the CUDA library is missing
+
+    n, nnz = A.n, A.nnz
+    rp = torch.from_numpy(A.row_ptr).cuda()
+    ci = torch.from_numpy(A.col_idx).cuda()
+    val = torch.from_numpy(A.val).cuda()
+
+    # ---- setup (a1-a4): wall-clock ms including allocation, median of 3 -----------------------------
+    setup_ms = []
+    h = None
+    for _ in range(3):
+        if h is not None:
+            B.bj_destroy(h)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h = B.bj_setup(rp, ci, val, b)
+        torch.cuda.synchronize()
+        setup_ms.append(1e3 * (time.perf_counter() - t0))
+    if args.spmv_kernel >= 0:
+        B.bj_set_option(h, B.BJ_OPT_SPMV_KERNEL, args.spmv_kernel)
+    if args.fuse >= 0:
+        B.bj_set_option(h, B.BJ_OPT_FUSE_FORWARD, args.fuse)
+    info = B.bj_get_info(h)
+
+    x = B.bj_seeded_vector(h, 31)
+    y = torch.empty_like(x)
+    ab = algorithmic_bytes(n, nnz, b)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: K operator applies, inputs resident in HBM ------------------------------------
+    for _ in range(args.warmup):
+        B.bj_op_apply(h, x, y)
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    launches0 = B.bj_get_info(h)["kernel_launches"]
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        B.bj_op_apply(h, x, y)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = B.bj_get_info(h)["kernel_launches"] - launches0
+    ms = aggregate_max(e0.elapsed_time(e1), world)
+    value = world * args.steps / (ms * 1e-3)
+    ms_per_step = ms / args.steps
+
+    # ---- per-kernel durations (CUDA events around every kernel, on the launching stream) --------------
+    B.bj_profile_enable(h, True)
+    prof_steps = min(args.steps, 500)
+    for _ in range(prof_steps):
+        B.bj_op_apply(h, x, y)
+    kinds = {B.KERNEL_KIND_NAMES[k]: B.bj_profile_get(h, k) for k in range(B.BJ_K_COUNT)}
+    B.bj_profile_enable(h, False)
+    kern = {k: {"avg_us": 1e3 * v[0] / v[1], "launches": v[1], "alg_bytes": ab[k],
+                "gbs": ab[k] / (1e-3 * v[0] / v[1]) / 1e9} for k, v in kinds.items() if v[1] > 0}
+    peak, peak_src = measured_peaks()
+    dom = max(kern, key=lambda k: kern[k]["avg_us"])
+    total_us = sum(v["avg_us"] for v in kern.values())
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kern[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                "share_of_step": kern[dom]["avg_us"] / total_us,
+                "frac_of_nominal_8TBs": kern[dom]["gbs"] / NOMINAL_HBM_GBS}
+    op_gbs = ab["op_apply"] / (ms_per_step * 1e-3) / 1e9
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": A.meta.get("name"), "baseline_config": args.config, "n": n, "nnz": nnz, "block": b,
+                       "l2": "inputs larger than L2 (%.0f MB per apply)" % (ab["op_apply"] / 1e6),
+                       "parallelism": "replicas" if world > 1 else "single",
+                       "spmv_kernel": info["spmv_kernel"], "fused_forward": info["fused_forward"],
+                       "spmv_lanes": info["spmv_lanes"]},
+            "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
+            "op_apply": {"alg_bytes": ab["op_apply"], "gbs": op_gbs, "frac_of_measured": op_gbs / peak,
+                         "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
+            "kernels": kern, "setup_ms": float(np.median(setup_ms)),
+            "factor_bytes": info["factor_bytes"]}
+
+    if not args.no_extras:
+        # ---- bj_apply (a5) -----------------------------------------------------------------------------
+        if b > 0:
+            for _ in range(10):
+                B.bj_apply(h, x, y)
+            k_apply = max(50, args.steps // 10)
+            e0.record()
+            for _ in range(k_apply):
+                B.bj_apply(h, x, y)
+            e1.record()
+            torch.cuda.synchronize()
+            ams = e0.elapsed_time(e1) / k_apply
+            line["apply"] = {"applies_per_s": 1e3 / ams, "gbs": ab["apply"] / (ams * 1e-3) / 1e9}
+
+        # ---- end to end through the host-buffer entry point (pinned host memory) -----------------------
+        xh = torch.from_numpy(W.seeded_vector(31, n)).pin_memory()
+        yh = torch.empty(n, dtype=torch.float64).pin_memory()
+        for _ in range(3):
+            B.bj_op_apply_host(h, xh, yh)
+        k_e2e = max(10, min(args.steps, 200))
+        barrier()
+        e0.record()
+        for _ in range(k_e2e):
+            B.bj_op_apply_host(h, xh, yh)
+        e1.record()
+        barrier()
+        e2e_ms = aggregate_max(e0.elapsed_time(e1), world)
+        line["e2e"] = {"value": world * k_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * n,
+                       "d2h_bytes_per_step": 8 * n, "steps": k_e2e}
+
+        if rank == 0:
+            # ---- kappa(A) -> kappa(A^) (a8-a10), parity mode (full reorthogonalisation) ------------------
+            m = args.lanczos_iters
+            kap = {}
+            h0 = B.bj_setup(rp, ci, val, 0)
+            for name, hh in (("A", h0), (f"bj{b}", h)):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                r = B.bj_cond_estimate_ex(hh, m, reorth=True)
+                dt = time.perf_counter() - t0
+                kap[name] = {"kappa_est": r["kappa"], "lmin": r["lmin"], "lmax": r["lmax"], "iters": r["iters_done"],
+                             "res_min": r["res_min"], "res_max": r["res_max"], "seconds": dt}
+            r = B.bj_cond_estimate_ex(h, m, reorth=False)
+            t0 = time.perf_counter()
+            r = B.bj_cond_estimate_ex(h, m, reorth=False)
+            dt = time.perf_counter() - t0
+            kap["fast_mode"] = {"kappa_est": r["kappa"], "iters": r["iters_done"], "seconds": dt,
+                                "lanczos_iters_per_s": r["iters_done"] / dt}
+            kap["predicted_hhl_gain_kappa_sq"] = (kap["A"]["kappa_est"] / kap[f"bj{b}"]["kappa_est"]) ** 2
+            line["kappa"] = kap
+            B.bj_destroy(h0)
+
+            # ---- CPU oracle on the host cores (reported baseline, not the target) -------------------------
+            v, reps, cores = time_oracle(A, b, args.cpu_budget_s)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{reps} full operator applies (whole vector, N={n}) in ~{args.cpu_budget_s:.0f} s"}
+
+    B.bj_destroy(h)
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,155 @@
+/*
+ * bj.h -- C ABI of the B200-native block-Jacobi preconditioning path of arxiv 2410.02408.
+ *
+ * What the library computes (citations: PAPER.md line numbers of /root/reference/PAPER.md,
+ * and the readings fixed in DESIGN.md section 3):
+ *   - A is a sparse symmetric positive-definite matrix (sec 3.1), here fp64 CSR.
+ *   - It is partitioned into contiguous index blocks of size b (sec 3.2; the
+ *     listing at 160-208 slices A[i:i+bs, j:j+bs], ragged at the edge).  Only the DIAGONAL tiles
+ *     D_k enter the preconditioner M = blockdiag(D_k).
+ *   - The paper's Jacobi preconditioner M_i = diag(A_i)^-1, A~ = M A, b~ = M b (PAPER.md:84-90,
+ *     sec 3.3; kernel M[idx] = 1/A[idx*N+idx] at 214-235) is the case b = 1.  For general b each
+ *     D_k = L_k L_k^T is factored by Cholesky and the preconditioned operator is taken in the
+ *     symmetric split form  A^ = L^-1 A L^-T  (same spectrum as M^-1 A; HHL needs Hermitian input,
+ *     PAPER.md:68).
+ *   - kappa(A) = ||A|| ||A^-1|| = lambda_max / lambda_min is estimated by Lanczos
+ *     on A (b = 0) and on A^; the paper's cost argument is O(log N kappa^2).
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless the parameter name ends in `_host` or the comment
+ *     says "host".  The library never frees or reallocates caller memory.
+ *   - CSR arrays passed to bj_setup are BORROWED and must outlive the handle.  They must be
+ *     canonical: row_ptr[0] = 0, row_ptr[n] = nnz, row_ptr non-decreasing, 0 <= col < n, columns
+ *     strictly increasing within each row, both triangles stored.  Symmetry is a precondition
+ *     and is not checked.  Only the lower triangle of each diagonal block is read
+ *     by the factorisation.
+ *   - Vector arguments are length-n fp64 arrays.  In-place calls (output == input) are allowed
+ *     for bj_apply, bj_solve_L, bj_solve_Lt and bj_op_apply; bj_spmv requires y != x.
+ *   - bj_apply / bj_op_apply / bj_spmv / bj_solve_* only ENQUEUE work on the handle's stream and
+ *     return without synchronising.  bj_setup, bj_cond_estimate*, bj_*_host synchronise.
+ *   - All functions return BJ_OK (0) or a negative bj_status code; bj_strerror gives text.  A
+ *     CUDA runtime failure returns BJ_ERR_CUDA and leaves the CUDA error string in bj_strerror.
+ *   - No CPU fallback exists: without a CUDA device every compute entry point fails with BJ_ERR_CUDA.
+ */
+#ifndef BJ_H_
+#define BJ_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BJ_B_MAX 32                        /* largest supported block size on the GPU path      */
+#define BJ_DEFAULT_SEED 0x241002408ull      /* default Lanczos start-vector seed                  */
+#define BJ_DEFAULT_BREAKDOWN_TOL 1e-12      /* beta_{j+1} <= tol * max|alpha_i| ends the run      */
+
+typedef enum {
+    BJ_OK = 0,
+    BJ_ERR_INVALID_ARG = -1,   /* null pointer, n <= 0, b < 0, b > BJ_B_MAX, iters < 1, y == x in bj_spmv */
+    BJ_ERR_NOT_CANONICAL = -2, /* CSR validation failed (see Conventions)                                  */
+    BJ_ERR_TOO_LARGE = -3,     /* n or nnz >= 2^31                                                         */
+    BJ_ERR_NOT_SPD = -4,       /* a diagonal block has a pivot <= 0 or non-finite; see bj_info_t.bad_block  */
+    BJ_ERR_ALLOC = -5,         /* device or host allocation failed                                         */
+    BJ_ERR_CUDA = -6           /* CUDA runtime error (sticky text in bj_strerror)                           */
+} bj_status;
+
+typedef struct bj_handle_s* bj_handle_t;
+
+typedef struct {
+    int64_t n, nnz;
+    const int32_t* row_ptr; /* device, n+1 */
+    const int32_t* col_idx; /* device, nnz */
+    const double* val;      /* device, nnz */
+} bj_csr_t;
+
+typedef struct {
+    int32_t iters;        /* number of Lanczos steps = operator applies = dim of T (>= 1)           */
+    int32_t reorth;       /* 0: none (fused fast mode), 1: full reorthogonalisation, twice (parity)  */
+    uint64_t seed;        /* start vector v0[i] = 2 u_i - 1, u_i = (mix64(seed,i) >> 11) 2^-53       */
+    const double* v0;     /* device, optional: caller-supplied start vector (overrides seed)         */
+    double breakdown_tol; /* <= 0 selects BJ_DEFAULT_BREAKDOWN_TOL                                   */
+} bj_lanczos_opts_t;
+
+typedef struct {
+    int32_t iters_done;   /* m_eff <= iters (smaller after a breakdown; not an error)                */
+    double lmin, lmax;    /* extreme Ritz values of T_{m_eff}                                        */
+    double res_min, res_max; /* Ritz residual bounds beta_{m+1} |s_{m,i}| for both ends               */
+    double* alpha_host;   /* host, optional, caller-allocated, >= iters doubles: alpha_1..           */
+    double* beta_host;    /* host, optional, caller-allocated, >= iters doubles: beta_2..beta_{m+1}   */
+} bj_lanczos_result_t;
+
+typedef struct {
+    int64_t n, nnz;
+    int32_t b;
+    int64_t nblocks;
+    int64_t bad_block;        /* first non-SPD block after BJ_ERR_NOT_SPD, else -1                   */
+    int64_t factor_bytes;     /* device bytes held for the factors                                   */
+    int64_t workspace_bytes;  /* device bytes held for temporaries and Lanczos workspace             */
+    int64_t kernel_launches;  /* number of kernels this handle has launched so far                   */
+    int32_t spmv_kernel;      /* 0: row-per-subwarp CSR-vector kernel, 1: TMA-streamed tile kernel    */
+    int32_t spmv_lanes;       /* lanes per row chosen at setup                                       */
+    int32_t solve_kernel;     /* 0: none (b=0), 1: thread-per-block (b<=8), 2: subwarp-per-block      */
+    int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
+} bj_info_t;
+
+/* kernel-kind indices for bj_profile_get */
+enum { BJ_K_SOLVE_LT = 0, BJ_K_SPMV = 1, BJ_K_SOLVE_L = 2, BJ_K_APPLY = 3, BJ_K_SPMV_SOLVE_L = 4, BJ_K_COUNT = 5 };
+
+/* options for bj_set_option */
+enum {
+    BJ_OPT_SPMV_KERNEL = 1,   /* 0 / 1 as in bj_info_t.spmv_kernel; -1 = automatic (default)          */
+    BJ_OPT_FUSE_FORWARD = 2   /* 0: three kernels, 1: fuse forward solve into SpMV, -1 = automatic    */
+};
+
+/* a1-a4. Validate the CSR, extract the diagonal b x b blocks, factor each
+ * by Cholesky (b = 1: PAPER.md:234) and build the launch plan.  b >= 1; b == 0 builds an identity
+ * preconditioner (A^ = A) used to estimate kappa(A).  The last block is ragged when b does not divide n.
+ * On BJ_ERR_NOT_SPD a handle is still returned in *out so that bj_get_info can report bad_block; it
+ * accepts only bj_get_info and bj_destroy.  Uses the default stream until bj_set_stream.  Synchronises. */
+int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out);
+
+/* Same as bj_setup but enqueues on `cuda_stream` (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream) and keeps it as the handle's stream. */
+int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_t* out);
+
+int bj_set_stream(bj_handle_t h, void* cuda_stream);
+int bj_set_option(bj_handle_t h, int option, int value);
+int bj_destroy(bj_handle_t h);
+int bj_get_info(bj_handle_t h, bj_info_t* info_host);
+const char* bj_strerror(int code);
+
+/* a5. z = M^-1 r = L^-T (L^-1 r), M = blockdiag(D_k)  (b~ = M b of PAPER.md:88-90).  b = 0: z = r. */
+int bj_apply(bj_handle_t h, const double* r, double* z);
+/* a6. y = A x (CSR SpMV). */
+int bj_spmv(bj_handle_t h, const double* x, double* y);
+/* y = L^-1 r (forward substitution per block) and x = L^-T y (backward). b = 0: copy. */
+int bj_solve_L(bj_handle_t h, const double* r, double* y);
+int bj_solve_Lt(bj_handle_t h, const double* y, double* x);
+/* a7. y = L^-1 A L^-T x, the split-preconditioned operator (symmetric form of A~ = M A). */
+int bj_op_apply(bj_handle_t h, const double* x, double* y);
+
+/* a8-a9. Lanczos on A^ with the default options (full reorthogonalisation when the basis fits in
+ * free device memory, else none; default seed); extreme Ritz values to host out-pointers.  Synchronises. */
+int bj_cond_estimate(bj_handle_t h, int iters, double* lmin_host, double* lmax_host);
+int bj_cond_estimate_ex(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_lanczos_result_t* res_host);
+
+/* Fill a device vector with the seeded start-vector sequence (see bj_lanczos_opts_t.seed). */
+int bj_seeded_vector(bj_handle_t h, uint64_t seed, double* v);
+
+/* End-to-end variants with HOST buffers (pinned or pageable): copy x to the device, run the device
+ * path, copy the result back, synchronise.  Staging buffers belong to the handle. */
+int bj_op_apply_host(bj_handle_t h, const double* x_host, double* y_host);
+int bj_apply_host(bj_handle_t h, const double* r_host, double* z_host);
+
+/* Per-kernel timing: when enabled, every kernel launched by the calls above is bracketed by CUDA
+ * events on the handle's stream; bj_profile_get synchronises and returns the accumulated device
+ * milliseconds and launch count of one kernel kind (BJ_K_*), then leaves the totals unchanged;
+ * enabling again resets them. */
+int bj_profile_enable(bj_handle_t h, int on);
+int bj_profile_get(bj_handle_t h, int kind, double* ms_total_host, int64_t* launches_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BJ_H_ */

@@ -1,0 +1,401 @@
+// C ABI of the bj library (include/bj.h): handle life cycle, setup orchestration (a1-a4),
+// operator composition (a7) and the host-buffer / profiling helpers.  All arithmetic lives in
+// the kernels of the sibling .cu files; there is no CPU fallback.
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "bj_internal.cuh"
+
+namespace bj {
+
+static thread_local char g_cuda_msg[512] = "no CUDA error recorded";
+
+void set_cuda_error(cudaError_t e, const char* where)
+{
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), where);
+    cudaGetLastError();  // clear the non-sticky error state
+}
+
+KernelScope::KernelScope(bj_handle_s* h_, int kind_) : h(h_), kind(kind_)
+{
+    h->launches++;
+    if (!h->prof_on) return;
+    auto get = [&]() {
+        cudaEvent_t e = nullptr;
+        if (!h->event_pool.empty()) { e = h->event_pool.back(); h->event_pool.pop_back(); }
+        else cudaEventCreate(&e);
+        return e;
+    };
+    a = get();
+    b = get();
+    cudaEventRecord(a, h->stream);
+}
+
+KernelScope::~KernelScope()
+{
+    if (!a) return;
+    cudaEventRecord(b, h->stream);
+    h->spans.push_back(ProfSpan{kind, a, b});
+}
+
+static int resolve_spans(bj_handle_s* h)
+{
+    if (h->spans.empty()) return BJ_OK;
+    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    for (auto& s : h->spans) {
+        float ms = 0.f;
+        BJ_CUDA(cudaEventElapsedTime(&ms, s.a, s.b));
+        h->prof_ms[s.kind] += ms;
+        h->prof_cnt[s.kind] += 1;
+        h->event_pool.push_back(s.a);
+        h->event_pool.push_back(s.b);
+    }
+    h->spans.clear();
+    return BJ_OK;
+}
+
+// y = L^-1 A L^-T x.  x == y allowed.
+int op_apply_device(bj_handle_s* h, const double* x, double* y)
+{
+    int rc;
+    if (h->solve_kind == 0) {  // identity preconditioner: A^ = A
+        if (x == y) {
+            BJ_CUDA(cudaMemcpyAsync(h->t, x, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+            x = h->t;
+        }
+        return h->spmv_kernel == 1 ? launch_spmv_stream(h, x, y, false) : launch_spmv_vector(h, x, y);
+    }
+    rc = launch_solve(h, 1, x, h->t);  // t = L^-T x
+    if (rc != BJ_OK) return rc;
+    const bool fuse = h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0;
+    if (fuse) return launch_spmv_stream(h, h->t, y, true);  // y = L^-1 (A t) in one kernel
+    rc = h->spmv_kernel == 1 ? launch_spmv_stream(h, h->t, h->u, false) : launch_spmv_vector(h, h->t, h->u);
+    if (rc != BJ_OK) return rc;
+    return launch_solve(h, 0, h->u, y);  // y = L^-1 u
+}
+
+static void free_handle(bj_handle_s* h)
+{
+    if (!h) return;
+    lanczos_free(h);
+    cudaFree(h->fac_small); cudaFree(h->fac_fwd); cudaFree(h->fac_bwd);
+    cudaFree(h->t); cudaFree(h->u); cudaFree(h->status);
+    cudaFree(h->stage_in); cudaFree(h->stage_out);
+    for (auto& s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+    for (auto e : h->event_pool) cudaEventDestroy(e);
+    delete h;
+}
+
+static void choose_spmv(bj_handle_s* h)
+{
+    int k = 0;
+    if (h->stream_ok) k = 1;
+    if (h->opt_spmv_kernel == 0) k = 0;
+    if (h->opt_spmv_kernel == 1 && h->stream_ok) k = 1;
+    h->spmv_kernel = k;
+}
+
+}  // namespace bj
+
+using namespace bj;
+
+extern "C" {
+
+const char* bj_strerror(int code)
+{
+    switch (code) {
+        case BJ_OK: return "ok";
+        case BJ_ERR_INVALID_ARG: return "invalid argument";
+        case BJ_ERR_NOT_CANONICAL: return "CSR is not canonical (row_ptr not monotone from 0 to nnz, column out of range, or columns not strictly increasing in a row)";
+        case BJ_ERR_TOO_LARGE: return "n or nnz does not fit 32-bit indices";
+        case BJ_ERR_NOT_SPD: return "a diagonal block is not positive definite (see bj_get_info bad_block)";
+        case BJ_ERR_ALLOC: return "allocation failed";
+        case BJ_ERR_CUDA: return g_cuda_msg;
+        default: return "unknown bj status";
+    }
+}
+
+int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_t* out)
+{
+    if (!out) return BJ_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!csr || !csr->row_ptr || csr->n <= 0 || csr->nnz < 0 || b < 0 || b > BJ_B_MAX) return BJ_ERR_INVALID_ARG;
+    if (csr->nnz > 0 && (!csr->col_idx || !csr->val)) return BJ_ERR_INVALID_ARG;
+    if (csr->n >= (1ll << 31) - 64 || csr->nnz >= (1ll << 31) - 64) return BJ_ERR_TOO_LARGE;
+
+    int dev = 0;
+    BJ_CUDA(cudaGetDevice(&dev));
+    bj_handle_s* h = new (std::nothrow) bj_handle_s();
+    if (!h) return BJ_ERR_ALLOC;
+    h->n = csr->n; h->nnz = csr->nnz; h->b = b;
+    h->row_ptr = csr->row_ptr; h->col_idx = csr->col_idx; h->val = csr->val;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->nblocks = b > 0 ? (csr->n + b - 1) / b : 0;
+    h->packed = b * (b + 1) / 2;
+    cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+
+    auto fail = [&](int code) { free_handle(h); return code; };
+    auto dmalloc = [&](void** p, size_t sz, int64_t* acct) {
+        cudaError_t e = cudaMalloc(p, sz ? sz : 8);
+        if (e != cudaSuccess) { cudaGetLastError(); return false; }
+        *acct += (int64_t)sz;
+        return true;
+    };
+
+    const size_t vb = (size_t)h->n * sizeof(double);
+    if (!dmalloc((void**)&h->t, vb, &h->workspace_bytes) || !dmalloc((void**)&h->u, vb, &h->workspace_bytes) ||
+        !dmalloc((void**)&h->status, sizeof(Status), &h->workspace_bytes))
+        return fail(BJ_ERR_ALLOC);
+    Status init;
+    memset(&init, 0, sizeof(init));
+    init.bad_block = 0x7fffffffffffffffll;
+    cudaError_t ce = cudaMemcpyAsync(h->status, &init, sizeof(init), cudaMemcpyHostToDevice, h->stream);
+    if (ce != cudaSuccess) { set_cuda_error(ce, "status init"); return fail(BJ_ERR_CUDA); }
+
+    // a1 validate (also longest row)
+    int rc = launch_validate(h);
+    if (rc != BJ_OK) return fail(rc);
+    Status stt;
+    ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+    if (ce != cudaSuccess) { set_cuda_error(ce, "validate"); return fail(BJ_ERR_CUDA); }
+    if (stt.flags & (ST_BAD_ROWPTR | ST_BAD_COL | ST_UNSORTED)) return fail(BJ_ERR_NOT_CANONICAL);
+
+    // lanes per row for the SpMV kernels: power of two near the mean row length
+    {
+        const double mean = (double)h->nnz / (double)h->n;
+        int l = 1;
+        while (l < 32 && (double)l * 1.15 < mean) l *= 2;
+        h->spmv_lanes = l;
+    }
+
+    // a2-a4 extract + factor
+    if (b > 0) {
+        if (b <= kSmallMax) {
+            h->solve_kind = 1;
+            const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;
+            const size_t sz = (size_t)groups * h->packed * kInterleave * sizeof(double);
+            if (!dmalloc((void**)&h->fac_small, sz, &h->factor_bytes)) return fail(BJ_ERR_ALLOC);
+            ce = cudaMemsetAsync(h->fac_small, 0, sz, h->stream);
+        } else {
+            h->solve_kind = 2;
+            h->lanes = b <= 16 ? 16 : 32;
+            const size_t sz = (size_t)h->nblocks * h->packed * sizeof(double);
+            if (!dmalloc((void**)&h->fac_fwd, sz, &h->factor_bytes) || !dmalloc((void**)&h->fac_bwd, sz, &h->factor_bytes))
+                return fail(BJ_ERR_ALLOC);
+        }
+        if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
+        rc = launch_extract_factor(h);
+        if (rc != BJ_OK) return fail(rc);
+    }
+
+    // SpMV plan for the streamed kernel
+    rc = spmv_stream_configure(h);
+    if (rc != BJ_OK) return fail(rc);
+
+    ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+    if (ce != cudaSuccess) { set_cuda_error(ce, "setup"); return fail(BJ_ERR_CUDA); }
+    choose_spmv(h);
+    *out = h;
+    if (stt.flags & ST_NOT_SPD) {
+        h->failed = true;
+        h->bad_block = (int64_t)stt.bad_block;
+        return BJ_ERR_NOT_SPD;
+    }
+    return BJ_OK;
+}
+
+int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out) { return bj_setup_on_stream(csr, b, nullptr, out); }
+
+int bj_set_stream(bj_handle_t h, void* cuda_stream)
+{
+    if (!h) return BJ_ERR_INVALID_ARG;
+    h->stream = (cudaStream_t)cuda_stream;
+    return BJ_OK;
+}
+
+int bj_set_option(bj_handle_t h, int option, int value)
+{
+    if (!h || h->failed) return BJ_ERR_INVALID_ARG;
+    switch (option) {
+        case BJ_OPT_SPMV_KERNEL:
+            if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
+            h->opt_spmv_kernel = value;
+            choose_spmv(h);
+            return BJ_OK;
+        case BJ_OPT_FUSE_FORWARD:
+            if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
+            h->opt_fuse = value;
+            return BJ_OK;
+        default: return BJ_ERR_INVALID_ARG;
+    }
+}
+
+int bj_destroy(bj_handle_t h)
+{
+    if (!h) return BJ_ERR_INVALID_ARG;
+    cudaStreamSynchronize(h->stream);
+    free_handle(h);
+    return BJ_OK;
+}
+
+int bj_get_info(bj_handle_t h, bj_info_t* info)
+{
+    if (!h || !info) return BJ_ERR_INVALID_ARG;
+    memset(info, 0, sizeof(*info));
+    info->n = h->n; info->nnz = h->nnz; info->b = h->b; info->nblocks = h->nblocks;
+    info->bad_block = h->bad_block;
+    info->factor_bytes = h->factor_bytes;
+    info->workspace_bytes = h->workspace_bytes;
+    info->kernel_launches = h->launches;
+    info->spmv_kernel = h->spmv_kernel;
+    info->spmv_lanes = h->spmv_lanes;
+    info->solve_kernel = h->solve_kind;
+    info->fused_forward = (h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0 && h->solve_kind != 0) ? 1 : 0;
+    return BJ_OK;
+}
+
+#define BJ_CHECK_H(h) do { if (!(h) || (h)->failed) return BJ_ERR_INVALID_ARG; } while (0)
+
+int bj_apply(bj_handle_t h, const double* r, double* z)
+{
+    BJ_CHECK_H(h);
+    if (!r || !z) return BJ_ERR_INVALID_ARG;
+    return launch_solve(h, 2, r, z);
+}
+
+int bj_solve_L(bj_handle_t h, const double* r, double* y)
+{
+    BJ_CHECK_H(h);
+    if (!r || !y) return BJ_ERR_INVALID_ARG;
+    return launch_solve(h, 0, r, y);
+}
+
+int bj_solve_Lt(bj_handle_t h, const double* y, double* x)
+{
+    BJ_CHECK_H(h);
+    if (!y || !x) return BJ_ERR_INVALID_ARG;
+    return launch_solve(h, 1, y, x);
+}
+
+int bj_spmv(bj_handle_t h, const double* x, double* y)
+{
+    BJ_CHECK_H(h);
+    if (!x || !y || x == y) return BJ_ERR_INVALID_ARG;
+    return h->spmv_kernel == 1 ? launch_spmv_stream(h, x, y, false) : launch_spmv_vector(h, x, y);
+}
+
+int bj_op_apply(bj_handle_t h, const double* x, double* y)
+{
+    BJ_CHECK_H(h);
+    if (!x || !y) return BJ_ERR_INVALID_ARG;
+    return op_apply_device(h, x, y);
+}
+
+int bj_seeded_vector(bj_handle_t h, uint64_t seed, double* v)
+{
+    BJ_CHECK_H(h);
+    if (!v) return BJ_ERR_INVALID_ARG;
+    return launch_seeded_vector(h, seed, v);
+}
+
+int bj_cond_estimate_ex(bj_handle_t h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res)
+{
+    BJ_CHECK_H(h);
+    if (!o || !res || o->iters < 1 || o->iters > (1 << 20)) return BJ_ERR_INVALID_ARG;
+    return lanczos_run(h, o, res);
+}
+
+int bj_cond_estimate(bj_handle_t h, int iters, double* lmin, double* lmax)
+{
+    BJ_CHECK_H(h);
+    if (iters < 1 || !lmin || !lmax) return BJ_ERR_INVALID_ARG;
+    bj_lanczos_opts_t o;
+    memset(&o, 0, sizeof(o));
+    o.iters = iters;
+    o.seed = BJ_DEFAULT_SEED;
+    size_t free_b = 0, total_b = 0;
+    BJ_CUDA(cudaMemGetInfo(&free_b, &total_b));
+    const double need = ((double)iters + 2.0) * (double)h->n * 8.0;
+    o.reorth = (h->lz.cap_vectors >= iters || need < 0.8 * (double)free_b) ? 1 : 0;
+    bj_lanczos_result_t r;
+    memset(&r, 0, sizeof(r));
+    int rc = lanczos_run(h, &o, &r);
+    if (rc != BJ_OK) return rc;
+    *lmin = r.lmin;
+    *lmax = r.lmax;
+    return BJ_OK;
+}
+
+static int ensure_staging(bj_handle_s* h)
+{
+    if (h->stage_in) return BJ_OK;
+    const size_t vb = (size_t)h->n * sizeof(double);
+    if (cudaMalloc((void**)&h->stage_in, vb) != cudaSuccess || cudaMalloc((void**)&h->stage_out, vb) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(h->stage_in);
+        h->stage_in = nullptr;
+        return BJ_ERR_ALLOC;
+    }
+    h->workspace_bytes += 2 * (int64_t)vb;
+    return BJ_OK;
+}
+
+int bj_op_apply_host(bj_handle_t h, const double* x_host, double* y_host)
+{
+    BJ_CHECK_H(h);
+    if (!x_host || !y_host) return BJ_ERR_INVALID_ARG;
+    int rc = ensure_staging(h);
+    if (rc != BJ_OK) return rc;
+    const size_t vb = (size_t)h->n * sizeof(double);
+    BJ_CUDA(cudaMemcpyAsync(h->stage_in, x_host, vb, cudaMemcpyHostToDevice, h->stream));
+    rc = op_apply_device(h, h->stage_in, h->stage_out);
+    if (rc != BJ_OK) return rc;
+    BJ_CUDA(cudaMemcpyAsync(y_host, h->stage_out, vb, cudaMemcpyDeviceToHost, h->stream));
+    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    return BJ_OK;
+}
+
+int bj_apply_host(bj_handle_t h, const double* r_host, double* z_host)
+{
+    BJ_CHECK_H(h);
+    if (!r_host || !z_host) return BJ_ERR_INVALID_ARG;
+    int rc = ensure_staging(h);
+    if (rc != BJ_OK) return rc;
+    const size_t vb = (size_t)h->n * sizeof(double);
+    BJ_CUDA(cudaMemcpyAsync(h->stage_in, r_host, vb, cudaMemcpyHostToDevice, h->stream));
+    rc = launch_solve(h, 2, h->stage_in, h->stage_out);
+    if (rc != BJ_OK) return rc;
+    BJ_CUDA(cudaMemcpyAsync(z_host, h->stage_out, vb, cudaMemcpyDeviceToHost, h->stream));
+    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    return BJ_OK;
+}
+
+int bj_profile_enable(bj_handle_t h, int on)
+{
+    BJ_CHECK_H(h);
+    int rc = resolve_spans(h);
+    if (rc != BJ_OK) return rc;
+    h->prof_on = on != 0;
+    if (on) {
+        for (int k = 0; k < BJ_K_COUNT; ++k) { h->prof_ms[k] = 0.0; h->prof_cnt[k] = 0; }
+    }
+    return BJ_OK;
+}
+
+int bj_profile_get(bj_handle_t h, int kind, double* ms_total, int64_t* launches)
+{
+    BJ_CHECK_H(h);
+    if (kind < 0 || kind >= BJ_K_COUNT) return BJ_ERR_INVALID_ARG;
+    int rc = resolve_spans(h);
+    if (rc != BJ_OK) return rc;
+    if (ms_total) *ms_total = h->prof_ms[kind];
+    if (launches) *launches = h->prof_cnt[kind];
+    return BJ_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,150 @@
+// Internal declarations of the bj CUDA library (sm_100a only).  Not installed; the public
+// boundary is include/bj.h.  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "bj.h"
+
+namespace bj {
+
+constexpr int kSmallMax = 8;        // b <= kSmallMax: one thread per block, factor in registers
+constexpr int kInterleave = 32;     // blocks per interleave group in the small layout
+constexpr int kReduceThreads = 256;
+constexpr int kMaxPartials = 1184;  // 148 SMs x 8: upper bound on reduction grids
+
+// status word bits written by the setup kernels
+enum : int { ST_BAD_ROWPTR = 1, ST_BAD_COL = 2, ST_UNSORTED = 4, ST_NOT_SPD = 8 };
+
+struct Status {
+    int flags;
+    int pad;
+    long long bad_block;  // atomicMin target
+    int max_tile_nnz;     // SpMV plan
+    int max_row_nnz;
+};
+
+struct ProfSpan {
+    int kind;
+    cudaEvent_t a, b;
+};
+
+struct LanczosWs {
+    int64_t cap_vectors = 0;  // vectors of length n held in V
+    double* V = nullptr;      // basis (reorth) or 2 rotating vectors
+    double* w = nullptr;
+    double* partial = nullptr;  // kMaxPartials x (cap+1)
+    double* coef = nullptr;     // reorth coefficients c[0..cap)
+    double* alpha = nullptr;    // device alpha[iters]
+    double* beta = nullptr;
+    double* scal = nullptr;     // [0]=beta_j (current), [1]=amax, [2]=1/||v0||, [3]=alpha_j
+    int* done = nullptr;        // [0]=stop flag, [1]=m_eff
+    int cap_iters = 0;
+    int64_t bytes = 0;
+};
+
+}  // namespace bj
+
+struct bj_handle_s {
+    // problem
+    int64_t n = 0, nnz = 0;
+    int b = 0;
+    int64_t nblocks = 0;
+    const int32_t* row_ptr = nullptr;
+    const int32_t* col_idx = nullptr;
+    const double* val = nullptr;
+    cudaStream_t stream = nullptr;
+    bool failed = false;  // NOT_SPD: only get_info / destroy allowed
+    int64_t bad_block = -1;
+
+    // factors
+    int solve_kind = 0;  // 0 none, 1 small (interleaved), 2 warp (fwd + bwd packed copies)
+    int lanes = 0;       // lanes per block for kind 2 (8, 16 or 32)
+    int packed = 0;      // b(b+1)/2
+    double* fac_small = nullptr;
+    double* fac_fwd = nullptr;
+    double* fac_bwd = nullptr;
+    int64_t factor_bytes = 0;
+
+    // temporaries
+    double* t = nullptr;
+    double* u = nullptr;
+    bj::Status* status = nullptr;  // device
+    int64_t workspace_bytes = 0;
+
+    // SpMV plan
+    int spmv_lanes = 8;       // lanes per row, CSR-vector kernel and tile reduce phase
+    int spmv_kernel = 0;      // chosen kernel
+    int opt_spmv_kernel = -1; // user override
+    int opt_fuse = -1;
+    int tile_rows = 0;        // rows per tile of the streamed kernel (multiple of b)
+    int tile_cap = 0;         // nnz capacity per stage
+    int tile_stages = 0;
+    int64_t ntiles = 0;
+    bool stream_ok = false;   // streamed kernel usable (alignment, capacity)
+    bool fuse_ok = false;
+    int num_sms = 148;
+
+    // Lanczos
+    bj::LanczosWs lz;
+
+    // e2e staging
+    double* stage_in = nullptr;
+    double* stage_out = nullptr;
+
+    // accounting
+    int64_t launches = 0;
+    bool prof_on = false;
+    std::vector<bj::ProfSpan> spans;
+    std::vector<cudaEvent_t> event_pool;
+    double prof_ms[BJ_K_COUNT] = {0};
+    int64_t prof_cnt[BJ_K_COUNT] = {0};
+};
+
+namespace bj {
+
+// error plumbing -------------------------------------------------------------------------------
+void set_cuda_error(cudaError_t e, const char* where);
+#define BJ_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e__ = (call);                       \
+        if (e__ != cudaSuccess) {                       \
+            bj::set_cuda_error(e__, #call);             \
+            return BJ_ERR_CUDA;                         \
+        }                                               \
+    } while (0)
+
+// profiling brackets: RAII around one kernel launch
+struct KernelScope {
+    bj_handle_s* h;
+    int kind;
+    cudaEvent_t a = nullptr, b = nullptr;
+    KernelScope(bj_handle_s* h_, int kind_);
+    ~KernelScope();
+};
+
+// setup (bj_setup_kernels.cu)
+int launch_validate(bj_handle_s* h);
+int launch_extract_factor(bj_handle_s* h);
+int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nnz
+
+// solves (bj_solve_kernels.cu): dir 0 = forward (L^-1), 1 = backward (L^-T), 2 = both (apply)
+int launch_solve(bj_handle_s* h, int dir, const double* in, double* out);
+
+// SpMV (bj_spmv_kernels.cu)
+int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);
+int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward);
+int spmv_stream_configure(bj_handle_s* h);  // decide tile geometry, set stream_ok / fuse_ok
+
+// Lanczos (bj_lanczos.cu)
+int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* r);
+void lanczos_free(bj_handle_s* h);
+int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
+
+// operator (bj_api.cu)
+int op_apply_device(bj_handle_s* h, const double* x, double* y);
+
+}  // namespace bj

@@ -24,8 +24,8 @@ def main():
         P = oracle.Precond(A, b)
         y = P.op_apply(x)
         r = P.cond_estimate(50)
-        out.append(f"b{b}_op_apply_norm2 {np.linalg.norm(y)!r}")
-        out.append(f"b{b}_op_apply_y0 {y[0]!r}")
+        out.append(f"b{b}_op_apply_norm2 {float(np.linalg.norm(y))!r}")
+        out.append(f"b{b}_op_apply_y0 {float(y[0])!r}")
         out.append(f"b{b}_lmin_m50 {r['lmin']!r}")
         out.append(f"b{b}_lmax_m50 {r['lmax']!r}")
         out.append(f"b{b}_kappa_m50 {r['kappa']!r}")

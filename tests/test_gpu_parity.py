@@ -1,0 +1,319 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances are BASELINE.json's: normwise relative
+error <= 1e-12 on apply outputs (2-norm and inf-norm, reading 14) and <= 1e-6 on
+kappa estimates, fp64."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2410_02408_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = 1e-12
+TOL_KAPPA = 1e-6
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2410_02408_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+_MATS = {}
+
+
+def mat(cfg, scale):
+    key = (cfg, scale)
+    if key not in _MATS:
+        _MATS[key] = W.build(cfg, scale)
+    return _MATS[key]
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def check_all_ops(B, torch, A, b, rel, seeds=(101, 202), tol=TOL_APPLY, kernels=(None,)):
+    h, keep = B.setup_from_host(A, b)
+    try:
+        P = oracle.Precond(A, b)
+        for kern in kernels:
+            if kern is not None:
+                B.bj_set_option(h, B.BJ_OPT_SPMV_KERNEL, kern[0])
+                B.bj_set_option(h, B.BJ_OPT_FUSE_FORWARD, kern[1])
+            for seed in seeds:
+                x = W.seeded_vector(seed, A.n)
+                xd = dev(torch, x)
+                got = {
+                    "spmv": B.bj_spmv(h, xd).cpu().numpy(),
+                    "op_apply": B.bj_op_apply(h, xd).cpu().numpy(),
+                }
+                ref = {"spmv": oracle.spmv(A, x), "op_apply": P.op_apply(x)}
+                if b > 0:
+                    got.update(solve_L=B.bj_solve_L(h, xd).cpu().numpy(), solve_Lt=B.bj_solve_Lt(h, xd).cpu().numpy(),
+                               apply=B.bj_apply(h, xd).cpu().numpy())
+                    ref.update(solve_L=P.solve_L(x), solve_Lt=P.solve_Lt(x), apply=P.apply(x))
+                for name in got:
+                    e2, ei = rel(got[name], ref[name])
+                    assert e2 <= tol and ei <= tol, f"{name} b={b} kern={kern}: rel2={e2:.3e} relinf={ei:.3e}"
+                # in-place operator apply
+                y = xd.clone()
+                B.bj_op_apply(h, y, y)
+                e2, ei = rel(y.cpu().numpy(), ref["op_apply"])
+                assert e2 <= tol and ei <= tol
+    finally:
+        B.bj_destroy(h)
+
+
+KERNELS = ((0, 0), (1, 0), (1, 1))
+
+
+# ------------------------------------------------------------------ small configs, every op -----------
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_ops_match_oracle_on_small_configs(B, torch_, rel, cfg):
+    A = mat(cfg, "small")
+    for b in W.BLOCK_SIZES[cfg]:
+        check_all_ops(B, torch_, A, b, rel, kernels=KERNELS)
+
+
+@pytest.mark.parametrize("b", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 12, 16, 20, 24, 31, 32])
+def test_every_block_size_including_ragged_last_block(B, torch_, rel, b):
+    A = mat(3, "small") if b % 2 else mat(2, "small")   # 16384 and 13824 rows: ragged for 5,7,9,20,31 / 5,7,..
+    check_all_ops(B, torch_, A, b, rel, seeds=(7,), kernels=KERNELS)
+
+
+def test_ragged_tail_sizes(B, torch_, rel):
+    """n not a multiple of anything: 1D Laplacian + diagonal, n = 100003 rows spans many tiles and a tail."""
+    n = 100003
+    A = W.laplacian((n,))
+    for b in (3, 8, 16, 32):
+        check_all_ops(B, torch_, A, b, rel, seeds=(5,), kernels=KERNELS)
+
+
+def test_config1_exact(B, torch_, rel):
+    A = mat(1, "full")
+    check_all_ops(B, torch_, A, 4, rel, kernels=KERNELS)
+    h, keep = B.setup_from_host(A, 4)
+    P = oracle.Precond(A, 4)
+    r_gpu = B.bj_cond_estimate_ex(h, 50, reorth=True)
+    r_cpu = P.cond_estimate(50)
+    assert r_gpu["iters_done"] == r_cpu["iters_done"] == 50
+    assert abs(r_gpu["kappa"] / r_cpu["kappa"] - 1) <= TOL_KAPPA
+    assert abs(r_gpu["lmin"] / r_cpu["lmin"] - 1) <= TOL_KAPPA and abs(r_gpu["lmax"] / r_cpu["lmax"] - 1) <= TOL_KAPPA
+    lmin, lmax = B.bj_cond_estimate(h, 50)      # the 4-argument call of the north star
+    assert abs((lmax / lmin) / r_cpu["kappa"] - 1) <= TOL_KAPPA
+    B.bj_destroy(h)
+
+
+# ------------------------------------------------------------------ Lanczos ------------------------------
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_kappa_estimates_match_oracle_small(B, torch_, cfg):
+    A = mat(cfg, "small")
+    for b in [0] + W.BLOCK_SIZES[cfg]:
+        h, keep = B.setup_from_host(A, b)
+        P = oracle.Precond(A, b)
+        g = B.bj_cond_estimate_ex(h, 50, reorth=True)
+        c = P.cond_estimate(50, reorth=True)
+        assert g["iters_done"] == c["iters_done"]
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (cfg, b, g["kappa"], c["kappa"])
+        assert np.allclose(g["alpha"], c["alpha"], rtol=1e-8, atol=1e-10 * abs(c["alpha"]).max())
+        assert abs(g["res_min"] - c["res_min"]) <= 1e-6 * c["lmax"] and abs(g["res_max"] - c["res_max"]) <= 1e-6 * c["lmax"]
+        if b > 0:
+            # fused fast mode (no reorthogonalisation) is safe on the preconditioned operators
+            g0 = B.bj_cond_estimate_ex(h, 50, reorth=False)
+            c0 = P.cond_estimate(50, reorth=False)
+            assert abs(g0["kappa"] / c0["kappa"] - 1) <= TOL_KAPPA
+        B.bj_destroy(h)
+
+
+def test_caller_supplied_start_vector_and_seed(B, torch_):
+    A = mat(2, "small")
+    h, keep = B.setup_from_host(A, 8)
+    P = oracle.Precond(A, 8)
+    v0 = W.seeded_vector(999, A.n)
+    g = B.bj_cond_estimate_ex(h, 30, reorth=True, v0=dev(torch_, v0))
+    c = P.cond_estimate(30, v0=v0)
+    assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+    g2 = B.bj_cond_estimate_ex(h, 30, reorth=True, seed=999)
+    assert abs(g2["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+    sv = B.bj_seeded_vector(h, 999).cpu().numpy()
+    assert np.array_equal(sv, oracle.seeded_vector(999, A.n))   # integer mixer: bit-exact
+    B.bj_destroy(h)
+
+
+def test_breakdown_is_not_an_error(B, torch_, rel):
+    """b = N (<= B_MAX) and the paper's block-diagonal model: A^ = I, m_eff = 1, kappa = 1."""
+    A = W.block_diagonal_spd(1, 24)
+    h, keep = B.setup_from_host(A, 24)
+    g = B.bj_cond_estimate_ex(h, 20, reorth=True)
+    assert g["iters_done"] == 1 and abs(g["kappa"] - 1) < 1e-12
+    B.bj_destroy(h)
+    for b in (2, 5, 8, 16, 32):
+        A = W.block_diagonal_spd(257, b)
+        h, keep = B.setup_from_host(A, b)
+        x = W.seeded_vector(3, A.n)
+        y = B.bj_op_apply(h, dev(torch_, x)).cpu().numpy()
+        e2, ei = rel(y, x)
+        assert e2 < 1e-13 and ei < 1e-13
+        g = B.bj_cond_estimate_ex(h, 20, reorth=False)
+        assert g["iters_done"] == 1 and abs(g["kappa"] - 1) < 1e-12
+        B.bj_destroy(h)
+
+
+def test_point_jacobi_is_the_papers_kernel(B, torch_):
+    """M[idx] = 1/A[idx*N+idx]."""
+    A = mat(1, "full")
+    h, keep = B.setup_from_host(A, 1)
+    z = B.bj_apply(h, torch_.ones(A.n, dtype=torch_.float64, device="cuda")).cpu().numpy()
+    assert np.allclose(z, 1.0 / A.to_dense().diagonal(), rtol=1e-15)
+    B.bj_destroy(h)
+
+
+# ------------------------------------------------------------------ errors and edge cases ----------------
+def test_error_codes(B, torch_):
+    A = mat(1, "full")
+    rp, ci, val = dev(torch_, A.row_ptr), dev(torch_, A.col_idx), dev(torch_, A.val)
+    with pytest.raises(B.BJError) as e:
+        B.bj_setup(rp, ci, val, 33)
+    assert e.value.code == B.BJ_ERR_INVALID_ARG
+    with pytest.raises(B.BJError) as e:
+        B.bj_setup(rp, ci, val, -1)
+    assert e.value.code == B.BJ_ERR_INVALID_ARG
+    # unsorted columns
+    ci2 = A.col_idx.copy()
+    s = A.row_ptr[10]
+    ci2[s], ci2[s + 1] = ci2[s + 1], ci2[s]
+    with pytest.raises(B.BJError) as e:
+        B.bj_setup(rp, dev(torch_, ci2), val, 4)
+    assert e.value.code == B.BJ_ERR_NOT_CANONICAL
+    # column out of range
+    ci3 = A.col_idx.copy()
+    ci3[-1] = A.n
+    with pytest.raises(B.BJError) as e:
+        B.bj_setup(rp, dev(torch_, ci3), val, 4)
+    assert e.value.code == B.BJ_ERR_NOT_CANONICAL
+    # row_ptr not ending at nnz
+    rp2 = A.row_ptr.copy()
+    rp2[-1] -= 1
+    with pytest.raises(B.BJError) as e:
+        B.bj_setup(dev(torch_, rp2), ci, val, 4)
+    assert e.value.code == B.BJ_ERR_NOT_CANONICAL
+    # non-SPD block: first bad block index is reported, same as the oracle
+    v2 = A.val.copy()
+    rows = np.repeat(np.arange(A.n), np.diff(A.row_ptr))
+    for r in (41, 333):
+        v2[(rows == r) & (A.col_idx == r)] = -1.0
+    A2 = W.CSR(A.n, A.row_ptr, A.col_idx, v2)
+    with pytest.raises(B.BJError) as e:
+        B.bj_setup(rp, ci, dev(torch_, v2), 4)
+    assert e.value.code == B.BJ_ERR_NOT_SPD and e.value.bad_block == 41 // 4
+    with pytest.raises(oracle.NotSPD) as eo:
+        oracle.Precond(A2, 4)
+    assert eo.value.bad_block == e.value.bad_block
+    # spmv must not alias
+    h = B.bj_setup(rp, ci, val, 4)
+    x = torch_.ones(A.n, dtype=torch_.float64, device="cuda")
+    with pytest.raises(B.BJError):
+        B.bj_spmv(h, x, x)
+    info = B.bj_get_info(h)
+    assert info["n"] == A.n and info["nnz"] == A.nnz and info["b"] == 4 and info["nblocks"] == 256 and info["bad_block"] == -1
+    B.bj_destroy(h)
+
+
+def test_tiny_and_degenerate_shapes(B, torch_, rel):
+    # n = 1
+    A = W.CSR(1, np.array([0, 1], np.int32), np.array([0], np.int32), np.array([4.0]))
+    for b in (0, 1, 2):
+        check_all_ops(B, torch_, A, b, rel, seeds=(1,), kernels=KERNELS)
+    # empty rows are fine for SpMV (b = 0); with b >= 1 their zero diagonal is not SPD
+    S = mat(3, "tiny").to_scipy().tolil()
+    S[5, :] = 0
+    S[:, 5] = 0
+    A = W.from_scipy(S.tocsr())
+    assert A.row_ptr[5] == A.row_ptr[6]
+    check_all_ops(B, torch_, A, 0, rel, seeds=(1,), kernels=KERNELS)
+    with pytest.raises(B.BJError) as e:
+        B.setup_from_host(A, 4)
+    assert e.value.code == B.BJ_ERR_NOT_SPD and e.value.bad_block == 1
+    # one very long row (arrow matrix): exercises the long-row path of the SpMV kernels
+    import scipy.sparse as sp
+    n = 5000
+    M = sp.lil_matrix((n, n))
+    M.setdiag(np.full(n, 10.0 * n))
+    M[0, :] = 1.0
+    M[:, 0] = 1.0
+    M[0, 0] = 10.0 * n
+    A = W.from_scipy(M.tocsr())
+    check_all_ops(B, torch_, A, 8, rel, seeds=(1,), kernels=KERNELS)
+
+
+def test_host_buffer_entry_points(B, torch_, rel):
+    A = mat(2, "small")
+    h, keep = B.setup_from_host(A, 8)
+    P = oracle.Precond(A, 8)
+    x = W.seeded_vector(77, A.n)
+    xh = torch_.from_numpy(x).pin_memory()
+    yh = torch_.empty(A.n, dtype=torch_.float64).pin_memory()
+    B.bj_op_apply_host(h, xh, yh)
+    e2, ei = rel(yh.numpy(), P.op_apply(x))
+    assert e2 <= TOL_APPLY and ei <= TOL_APPLY
+    B.bj_apply_host(h, xh, yh)
+    e2, ei = rel(yh.numpy(), P.apply(x))
+    assert e2 <= TOL_APPLY and ei <= TOL_APPLY
+    B.bj_destroy(h)
+
+
+def test_runs_on_a_side_stream_and_profiling_counts(B, torch_, rel):
+    A = mat(4, "small")
+    s = torch_.cuda.Stream()
+    with torch_.cuda.stream(s):
+        h, keep = B.setup_from_host(A, 16)
+        x = dev(torch_, W.seeded_vector(8, A.n))
+        B.bj_profile_enable(h, True)
+        for _ in range(5):
+            y = B.bj_op_apply(h, x)
+        s.synchronize()
+        fused = B.bj_get_info(h)["fused_forward"]
+        kinds = [B.bj_profile_get(h, k) for k in range(B.BJ_K_COUNT)]
+        B.bj_profile_enable(h, False)
+    assert kinds[B.BJ_K_SOLVE_LT][1] == 5
+    if fused:
+        assert kinds[B.BJ_K_SPMV_SOLVE_L][1] == 5
+    else:
+        assert kinds[B.BJ_K_SPMV][1] == 5 and kinds[B.BJ_K_SOLVE_L][1] == 5
+    assert all(ms >= 0 for ms, _ in kinds)
+    e2, _ = rel(y.cpu().numpy(), oracle.Precond(A, 16).op_apply(W.seeded_vector(8, A.n)))
+    assert e2 <= TOL_APPLY
+    B.bj_destroy(h)
+
+
+# ------------------------------------------------------------------ BASELINE.json full sizes -------------
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_configs(B, torch_, rel, cfg):
+    """Full-size matrices in the launch configuration bench.py times: whole-vector parity of every op
+    (the oracle finishes one apply in well under a second), kappa parity at a reduced step count for
+    the preconditioned operator, and the 2-cyclic invariant where it holds."""
+    A = mat(cfg, "full")
+    for b in W.BLOCK_SIZES[cfg]:
+        check_all_ops(B, torch_, A, b, rel, seeds=(31,))
+        h, keep = B.setup_from_host(A, b)
+        P = oracle.Precond(A, b)
+        m = 50 if cfg == 2 else 16
+        g = B.bj_cond_estimate_ex(h, m, reorth=True)
+        c = P.cond_estimate(m, reorth=True)
+        assert g["iters_done"] == c["iters_done"] == m
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (cfg, b, g["kappa"], c["kappa"])
+        B.bj_destroy(h)
+        del h, keep
+    _MATS.pop((cfg, "full"), None)
+    torch_.cuda.empty_cache()
