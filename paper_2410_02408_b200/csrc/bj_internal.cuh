@@ -76,7 +76,8 @@ struct bj_handle_s {
     int64_t workspace_bytes = 0;
 
     // SpMV plan
-    int spmv_lanes = 8;       // lanes per row, CSR-vector kernel and tile reduce phase
+    int spmv_lanes = 8;       // lanes per row, CSR-vector kernel
+    int stream_lanes = 1;     // lanes per row, reduce phase of the tile kernel
     int spmv_kernel = 0;      // chosen kernel
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;

@@ -9,6 +9,10 @@
 //   (cp.async.bulk + mbarrier, i.e. the TMA engine: no registers staged, deep memory-level
 //   parallelism), consumer warps reduce rows out of shared memory, gather t through L1/L2, and can
 //   run the forward block solve y = L^-1 u on the tile before y is written (fuses a7's last factor).
+#include <stdlib.h>
+
+#include <algorithm>
+
 #include "bj_internal.cuh"
 
 namespace bj {
@@ -71,16 +75,392 @@ int launch_spmv_vector(bj_handle_s* h, const double* x, double* y)
 }
 
 // ------------------------------------------------------------------------------------------------
-// Kernel 1: placeholder until the streamed kernel lands (never selected while stream_ok is false)
+// Kernel 1: persistent, TMA-streamed tiles
+//
+// A tile is `R` consecutive rows.  Its column indices, values, row pointers and (when fused) the
+// packed factors of its diagonal blocks are each ONE contiguous byte range, so one elected
+// producer thread moves them with four 1-D bulk async copies (cp.async.bulk -> UBLKCP) into one
+// stage of a shared-memory ring; completion is tracked by an mbarrier transaction count.  Bulk
+// copies need 16-byte aligned addresses and sizes: ranges are widened to multiples of four
+// elements, and the (at most three) elements that would fall past the end of a caller array are
+// copied by the producer with plain loads instead.
+// Eight consumer warps then (A) reduce the rows out of shared memory, LPR lanes per row, gathering
+// t[col] through L1/L2, and (B, fused) run the forward substitution of the tile's diagonal blocks
+// from the staged factors, one thread per block, before y is written.  The stage is handed back
+// through a second mbarrier.  Tiles are dealt round-robin to the CTAs, so the CTAs resident at any
+// time stream neighbouring tiles (DRAM page and gather locality).
 // ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kConsumerThreads = 256;
+constexpr int kStreamThreads = kConsumerThreads + 32;
+
+struct StreamParams {
+    int64_t n, nnz;
+    const int32_t* rp;
+    const int32_t* ci;
+    const double* val;
+    const double* x;
+    double* y;
+    const double* fac;   // fac_small (fused) or null
+    int b, P, bs;        // block size, packed size, padded block stride in su
+    int R, cap, stages;
+    int64_t ntiles;
+    int rp_ints;         // ints reserved per stage for row pointers (R + 4)
+    int fac_bytes;       // bytes reserved per stage for factors
+    int stage_bytes;
+    int su_doubles;      // doubles per su buffer
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+        : "memory");
+}
+__device__ __forceinline__ void consumer_bar_sync()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+}
+
+template <int LPR, int FUSE>
+__global__ void __launch_bounds__(kStreamThreads)
+spmv_stream_kernel(const StreamParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    uint64_t* empty = full + p.stages;
+    double* su = reinterpret_cast<double*>(smem_raw + 128);               // 2 x su_doubles (fused only)
+    unsigned char* stage0 = smem_raw + 128 + (size_t)2 * p.su_doubles * sizeof(double);
+    // per stage: val[cap] | fac[fac_bytes] | col[cap] | rp[rp_ints]
+    auto s_val = [&](int s) { return reinterpret_cast<double*>(stage0 + (size_t)s * p.stage_bytes); };
+    auto s_fac = [&](int s) { return reinterpret_cast<double*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 8); };
+    auto s_col = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 8 + p.fac_bytes); };
+    auto s_rp = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 12 + p.fac_bytes); };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kConsumerThreads / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int R = p.R;
+    if (warp == 0) {
+        // ------------------------------ producer ------------------------------------------------
+        const uint64_t pol = policy_evict_first();
+        const int nnz4 = (int)(p.nnz & ~3ll);
+        int pb0 = 0, pb1 = 0;
+        int it = 0;
+        for (int64_t tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
+            if ((it & 31) == 0) {  // each lane fetches the nnz bounds of one of the next 32 tiles
+                const int64_t tl = tile + (int64_t)lane * gridDim.x;
+                if (tl < p.ntiles) {
+                    const int64_t q0 = tl * R;
+                    const int64_t q1 = q0 + R < p.n ? q0 + R : p.n;
+                    pb0 = __ldg(p.rp + q0);
+                    pb1 = __ldg(p.rp + q1);
+                }
+            }
+            const int p0 = __shfl_sync(0xffffffffu, pb0, it & 31);
+            const int p1 = __shfl_sync(0xffffffffu, pb1, it & 31);
+            if (lane == 0) {
+                const int s = it % p.stages;
+                const uint32_t ph = (uint32_t)((it / p.stages) & 1);
+                mbar_wait(&empty[s], ph ^ 1u);
+                const int64_t r0 = tile * R;
+                const int rows = (int)(r0 + R <= p.n ? R : p.n - r0);
+                // nnz range widened to multiples of 4, clamped to the last whole quad of the arrays
+                const int a0 = p0 & ~3;
+                int a1 = (p1 + 3) & ~3;
+                if (a1 > nnz4) a1 = nnz4;
+                if (a1 < a0) a1 = a0;
+                double* dv = s_val(s);
+                int* dc = s_col(s);
+                int* dr = s_rp(s);
+                for (int q = (a1 > p0 ? a1 : p0); q < p1; ++q) {  // tail past the last whole quad
+                    dv[q - a0] = p.val[q];
+                    dc[q - a0] = p.ci[q];
+                }
+                // row pointers r0 .. r0+rows (rows+1 ints), whole quads by bulk copy, rest by hand
+                const int64_t np1 = p.n + 1;
+                int want = rows + 1;
+                int rq = (want + 3) & ~3;
+                if (r0 + rq > np1) rq = (int)((np1 - r0) & ~3ll);
+                for (int q = rq; q < want; ++q) dr[q] = p.rp[r0 + q];
+                uint32_t bytes = (uint32_t)(a1 - a0) * 12u + (uint32_t)rq * 4u;
+                uint32_t fbytes = 0;
+                const double* fsrc = nullptr;
+                if (FUSE) {
+                    const int nblk = (rows + p.b - 1) / p.b;
+                    const int groups = (nblk + kInterleave - 1) / kInterleave;
+                    fbytes = (uint32_t)groups * (uint32_t)p.P * kInterleave * 8u;
+                    fsrc = p.fac + (r0 / p.b / kInterleave) * (int64_t)p.P * kInterleave;
+                    bytes += fbytes;
+                }
+                mbar_expect_tx(&full[s], bytes);
+                if (a1 > a0) {
+                    bulk_g2s(dv, p.val + a0, (uint32_t)(a1 - a0) * 8u, &full[s], pol);
+                    bulk_g2s(dc, p.ci + a0, (uint32_t)(a1 - a0) * 4u, &full[s], pol);
+                }
+                if (rq > 0) bulk_g2s(dr, p.rp + r0, (uint32_t)rq * 4u, &full[s], pol);
+                if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], pol);
+            }
+        }
+    } else {
+        // ------------------------------ consumers -----------------------------------------------
+        const int ctid = threadIdx.x - 32;
+        const int sub = ctid & (LPR - 1);
+        constexpr int kRowsPerPass = kConsumerThreads / LPR;
+        int it = 0;
+        for (int64_t tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
+            const int s = it % p.stages;
+            const uint32_t ph = (uint32_t)((it / p.stages) & 1);
+            const int64_t r0 = tile * R;
+            const int rows = (int)(r0 + R <= p.n ? R : p.n - r0);
+            double* sub_u = su + (size_t)(it & 1) * p.su_doubles;
+            mbar_wait(&full[s], ph);
+            const double* sv = s_val(s);
+            const int* sc = s_col(s);
+            const int* sr = s_rp(s);
+            const int a0 = sr[0] & ~3;
+            // (A) rows out of shared memory
+            for (int base = 0; base < rows; base += kRowsPerPass) {
+                const int i = base + ctid / LPR;
+                const bool valid = i < rows;
+                double acc = 0.0;
+                if (valid) {
+                    // batches of four entries per lane: all four gathers are in flight together
+                    const int e = sr[i + 1] - a0;
+                    for (int q = sr[i] - a0 + sub; q < e; q += 4 * LPR) {
+                        int c[4];
+                        double xv[4], av[4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const int qq = q + k * LPR;
+                            c[k] = sc[qq < e ? qq : q];
+                        }
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) xv[k] = __ldg(p.x + c[k]);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const int qq = q + k * LPR;
+                            av[k] = qq < e ? sv[qq] : 0.0;
+                        }
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) acc = fma(av[k], xv[k], acc);
+                    }
+                }
+#pragma unroll
+                for (int off = LPR / 2; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off, LPR);
+                if (valid && sub == 0) {
+                    if (FUSE) {
+                        const int k = i / p.b;
+                        sub_u[k * p.bs + (i - k * p.b)] = acc;
+                    } else {
+                        p.y[r0 + i] = acc;
+                    }
+                }
+            }
+            if (FUSE) {
+                // (B) forward substitution y = L^-1 u on the tile's diagonal blocks, one thread per block
+                consumer_bar_sync();
+                const int nblk = (rows + p.b - 1) / p.b;
+                const int b = p.b;
+                const double* sf = s_fac(s);
+                const int rot = (ctid + 32 * (it & 7)) & (kConsumerThreads - 1);  // spread the work over warps
+                for (int k = rot; k < nblk; k += kConsumerThreads) {
+                    const double* f = sf + (size_t)(k >> 5) * p.P * kInterleave + (k & 31);
+                    double* uk = sub_u + k * p.bs;
+                    const int64_t lo = r0 + (int64_t)k * b;
+                    double v[kSmallMax];
+#pragma unroll
+                    for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < p.n) ? uk[i] : 0.0;
+#pragma unroll
+                    for (int i = 0; i < kSmallMax; ++i) {
+                        if (i < b) {
+                            double acc = v[i];
+#pragma unroll
+                            for (int j = 0; j < i; ++j) acc -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
+                            v[i] = acc * f[(i * (i + 1) / 2 + i) * kInterleave];
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < kSmallMax; ++i)
+                        if (i < b && lo + i < p.n) p.y[lo + i] = v[i];
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+    }
+}
+
+template <int LPR, int FUSE>
+int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int grid, size_t smem)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
+        configured = true;
+    }
+    spmv_stream_kernel<LPR, FUSE><<<grid, kStreamThreads, smem, h->stream>>>(sp);
+    return BJ_OK;
+}
+
+int env_int(const char* name, int dflt)
+{
+    const char* v = getenv(name);
+    return v && *v ? atoi(v) : dflt;
+}
+
+}  // namespace
+
+namespace {
+// shared-memory layout of one launch; the single source of truth for configure and launch
+void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem)
+{
+    sp.b = h->b > 0 ? h->b : 1;
+    sp.P = h->packed;
+    sp.bs = (sp.b % 2) ? sp.b : sp.b + 1;
+    sp.R = h->tile_rows;
+    sp.cap = h->tile_cap;
+    sp.stages = h->tile_stages;
+    sp.ntiles = h->ntiles;
+    sp.rp_ints = sp.R + 4;
+    sp.fac_bytes = fuse ? (sp.R / sp.b) * sp.P * 8 : 0;
+    sp.stage_bytes = (sp.cap * 12 + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
+    sp.su_doubles = fuse ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : 0;
+    smem = 128 + (size_t)2 * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
+}
+constexpr size_t kSmemTwoPerSm = 110 * 1024;
+constexpr size_t kSmemOnePerSm = 224 * 1024;
+}  // namespace
+
+// Decide the tile geometry.  Called by bj_setup after validation (max_row_nnz known) and, a second
+// time, after tile_nnz_kernel has measured the fullest tile.
 int spmv_stream_configure(bj_handle_s* h)
 {
     h->stream_ok = false;
     h->fuse_ok = false;
     h->ntiles = 0;
+    if (h->nnz == 0) return BJ_OK;
+    if (((uintptr_t)h->val & 15) || ((uintptr_t)h->col_idx & 15) || ((uintptr_t)h->row_ptr & 15)) return BJ_OK;
+    const double mean = (double)h->nnz / (double)h->n;
+    {
+        // lanes per row in the tile kernel: rows come out of shared memory, so one thread per row
+        // (coalesced gathers for banded matrices, oracle summation order) up to ~12 entries per row
+        int l = 1;
+        while (l < 32 && (double)l * 12.0 < mean) l *= 2;
+        h->stream_lanes = env_int("BJ_STREAM_LANES", l);
+    }
+    const int target_nnz = env_int("BJ_TILE_NNZ", 2048);
+    int R = (int)((double)target_nnz / (mean > 1.0 ? mean : 1.0));
+    R = std::max(32, std::min(R, 1024));
+    bool fuse = false;
+    if (h->solve_kind == 1) {
+        const int unit = kInterleave * h->b;  // fused tiles must hold whole interleave groups
+        int Rf = ((R + unit / 2) / unit) * unit;
+        if (Rf < unit) Rf = unit;
+        if ((double)Rf * mean <= 1.6 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
+    }
+    if (!fuse) R = ((R + 31) / 32) * 32;
+    R = env_int("BJ_TILE_ROWS", R);
+    if (fuse && (R % (kInterleave * h->b)) != 0) fuse = false;
+    if (R % 4) return BJ_OK;
+    h->tile_rows = R;
+    h->ntiles = (h->n + R - 1) / R;
+    h->fuse_ok = fuse;
+    // measure the fullest tile
+    BJ_CUDA(cudaMemsetAsync(&h->status->max_tile_nnz, 0, sizeof(int), h->stream));
+    int rc = launch_spmv_plan(h);
+    if (rc != BJ_OK) return rc;
+    int max_tile = 0;
+    BJ_CUDA(cudaMemcpyAsync(&max_tile, &h->status->max_tile_nnz, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    h->tile_cap = ((max_tile + 8) + 3) & ~3;
+    int stages = env_int("BJ_STAGES", 3);
+    StreamParams sp;
+    size_t smem = 0;
+    h->tile_stages = stages;
+    fill_layout(h, fuse, sp, smem);
+    if (smem > kSmemTwoPerSm) {
+        // one CTA per SM: as many stages as fit, at least two
+        while (stages > 2 && smem > kSmemOnePerSm) { h->tile_stages = --stages; fill_layout(h, fuse, sp, smem); }
+        if (smem > kSmemOnePerSm) { h->ntiles = 0; h->fuse_ok = false; return BJ_OK; }
+    }
+    h->tile_stages = stages;
+    h->stream_ok = true;
     return BJ_OK;
 }
 
-int launch_spmv_stream(bj_handle_s*, const double*, double*, bool) { return BJ_ERR_INVALID_ARG; }
+int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward)
+{
+    if (!h->stream_ok) return BJ_ERR_INVALID_ARG;
+    const bool fuse = fuse_forward && h->fuse_ok;
+    if (fuse_forward && !fuse) return BJ_ERR_INVALID_ARG;
+    StreamParams sp;
+    size_t smem = 0;
+    fill_layout(h, fuse, sp, smem);
+    sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
+    sp.x = x; sp.y = y;
+    sp.fac = fuse ? h->fac_small : nullptr;
+    const int per_sm = smem <= kSmemTwoPerSm ? 2 : 1;
+    const int grid = (int)std::min<int64_t>(h->ntiles, (int64_t)h->num_sms * env_int("BJ_CTAS_PER_SM", per_sm));
+    int rc = BJ_OK;
+    {
+        KernelScope scope(h, fuse ? BJ_K_SPMV_SOLVE_L : BJ_K_SPMV);
+#define BJ_CASE(L)                                                                                     \
+    case L:                                                                                            \
+        rc = fuse ? launch_stream_t<L, 1>(h, sp, grid, smem) : launch_stream_t<L, 0>(h, sp, grid, smem); \
+        break;
+        switch (h->stream_lanes) {
+            BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
+            default: rc = BJ_ERR_INVALID_ARG;
+        }
+#undef BJ_CASE
+    }
+    if (rc != BJ_OK) return rc;
+    BJ_CUDA(cudaGetLastError());
+    return BJ_OK;
+}
 
 }  // namespace bj
