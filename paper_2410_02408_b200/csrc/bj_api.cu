@@ -136,6 +136,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     h->nblocks = b > 0 ? (csr->n + b - 1) / b : 0;
     h->packed = b * (b + 1) / 2;
     cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    h->pdl = env_int("BJ_PDL", 1) != 0;
 
     auto fail = [&](int code) { free_handle(h); return code; };
     auto dmalloc = [&](void** p, size_t sz, int64_t* acct) {

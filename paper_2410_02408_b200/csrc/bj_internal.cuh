@@ -88,6 +88,7 @@ struct bj_handle_s {
     bool stream_ok = false;   // streamed kernel usable (alignment, capacity)
     bool fuse_ok = false;
     int num_sms = 148;
+    bool pdl = true;          // chain the library's kernels with programmatic dependent launch
 
     // Lanczos
     bj::LanczosWs lz;
@@ -144,6 +145,8 @@ int spmv_stream_configure(bj_handle_s* h);  // decide tile geometry, set stream_
 int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* r);
 void lanczos_free(bj_handle_s* h);
 int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
+
+int env_int(const char* name, int dflt);  // tuning knobs BJ_* (read at setup / launch)
 
 // operator (bj_api.cu)
 int op_apply_device(bj_handle_s* h, const double* x, double* y);

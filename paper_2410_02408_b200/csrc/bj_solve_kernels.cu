@@ -11,37 +11,42 @@
 //            subtract L_ij y_j.  Column j of L is contiguous in the column-major packed copy, so the
 //            lanes' loads coalesce; the backward solve reads the row-major packed copy the same way.
 //            All b column loads of a lane are issued before the dependent chain starts.
+#include "bj_device.cuh"
 #include "bj_internal.cuh"
 
 namespace bj {
 
-__device__ __forceinline__ double ld_stream(const double* p)
-{
-    double v;
-    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
-    return v;
-}
-
 // ------------------------------------------------------------------------------------------------
 // thread per block, compile-time B.  DIR: 0 forward, 1 backward, 2 both.
 // ------------------------------------------------------------------------------------------------
-template <int B, int DIR>
+template <int B, int DIR, bool VEC>
 __global__ void __launch_bounds__(128)
 solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                    const double* in, double* out)  // in == out allowed: a thread touches only its own block
 {
     constexpr int P = B * (B + 1) / 2;
+    pdl_trigger();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nblocks) return;
     const double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
     double l[P];
 #pragma unroll
-    for (int e = 0; e < P; ++e) l[e] = ld_stream(f + e * kInterleave);
+    for (int e = 0; e < P; ++e) l[e] = ld_stream(f + e * kInterleave);   // factors never change after setup
+    pdl_wait();                                                          // `in` may come from the previous kernel
     const int64_t lo = k * B;
     double v[B];
-    if (lo + B <= n) {
+    const bool whole = lo + B <= n;
+    if (whole) {
+        if constexpr (VEC && B % 4 == 0) {
 #pragma unroll
-        for (int i = 0; i < B; ++i) v[i] = in[lo + i];
+            for (int i = 0; i < B; i += 4) ld_v4(in + lo + i, v + i);
+        } else if constexpr (VEC && B % 2 == 0) {
+#pragma unroll
+            for (int i = 0; i < B; i += 2) ld_v2(in + lo + i, v + i);
+        } else {
+#pragma unroll
+            for (int i = 0; i < B; ++i) v[i] = in[lo + i];
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < B; ++i) v[i] = (lo + i < n) ? in[lo + i] : 0.0;
@@ -64,9 +69,17 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
             v[i] = s * l[i * (i + 1) / 2 + i];
         }
     }
-    if (lo + B <= n) {
+    if (whole) {
+        if constexpr (VEC && B % 4 == 0) {
 #pragma unroll
-        for (int i = 0; i < B; ++i) out[lo + i] = v[i];
+            for (int i = 0; i < B; i += 4) st_v4(out + lo + i, v + i);
+        } else if constexpr (VEC && B % 2 == 0) {
+#pragma unroll
+            for (int i = 0; i < B; i += 2) st_v2(out + lo + i, v + i);
+        } else {
+#pragma unroll
+            for (int i = 0; i < B; ++i) out[lo + i] = v[i];
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < B; ++i)
@@ -82,6 +95,7 @@ __global__ void __launch_bounds__(256)
 solve_warp_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ fwd,
                   const double* __restrict__ bwd, const double* in, double* out)  // in == out allowed
 {
+    pdl_trigger();
     const int i = threadIdx.x & (W - 1);
     int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / W;
     const bool act = k < nblocks;  // no early return: the full-mask shuffles below need every lane
@@ -90,7 +104,7 @@ solve_warp_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
     const int P = b * (b + 1) / 2;
     const int64_t row = k * b + i;
     const bool live = act && (i < b) && (row < n);
-    double r = live ? in[row] : 0.0;
+    double r = 0.0;
     double l[W];
 
     if (DIR == 0 || DIR == 2) {
@@ -100,6 +114,8 @@ solve_warp_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
             // column j: rows j..b-1 at offset j*b - j(j-1)/2
             l[j] = (act && j < b && i >= j && i < b) ? ld_stream(f + (j * b - j * (j - 1) / 2) + (i - j)) : 0.0;
         }
+        pdl_wait();
+        r = live ? in[row] : 0.0;
 #pragma unroll
         for (int j = 0; j < W; ++j) {
             if (j < b) {
@@ -115,6 +131,10 @@ solve_warp_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
         for (int j = 0; j < W; ++j) {
             // row j: columns 0..j at offset j(j+1)/2
             l[j] = (act && j < b && i <= j) ? ld_stream(f + j * (j + 1) / 2 + i) : 0.0;
+        }
+        if (DIR == 1) {
+            pdl_wait();
+            r = live ? in[row] : 0.0;
         }
 #pragma unroll
         for (int jj = 0; jj < W; ++jj) {
@@ -136,15 +156,22 @@ static int launch_small(bj_handle_s* h, const double* in, double* out)
 {
     const int threads = 128;
     const unsigned blocks = (unsigned)((h->nblocks + threads - 1) / threads);
-#define BJ_CASE(B)                                                                                             \
-    case B:                                                                                                    \
-        solve_small_kernel<B, DIR><<<blocks, threads, 0, h->stream>>>(h->n, h->nblocks, h->fac_small, in, out); \
+    const bool vec = ((((uintptr_t)in) | ((uintptr_t)out)) & 31) == 0;
+    const bool pdl = h->pdl && !h->prof_on;
+    cudaError_t e = cudaSuccess;
+#define BJ_CASE(B)                                                                                                   \
+    case B:                                                                                                          \
+        e = vec ? launch_kernel(solve_small_kernel<B, DIR, true>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,  \
+                                (const double*)h->fac_small, in, out)                                                \
+                : launch_kernel(solve_small_kernel<B, DIR, false>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks, \
+                                (const double*)h->fac_small, in, out);                                               \
         break;
     switch (h->b) {
         BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
         default: return BJ_ERR_INVALID_ARG;
     }
 #undef BJ_CASE
+    if (e != cudaSuccess) { set_cuda_error(e, "solve_small_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
 
@@ -152,13 +179,18 @@ template <int DIR>
 static int launch_warp(bj_handle_s* h, const double* in, double* out)
 {
     const int threads = 256;
+    const bool pdl = h->pdl && !h->prof_on;
+    cudaError_t e;
     if (h->lanes == 16) {
         const unsigned blocks = (unsigned)((h->nblocks * 16 + threads - 1) / threads);
-        solve_warp_kernel<16, DIR><<<blocks, threads, 0, h->stream>>>(h->n, h->b, h->nblocks, h->fac_fwd, h->fac_bwd, in, out);
+        e = launch_kernel(solve_warp_kernel<16, DIR>, blocks, threads, 0, h->stream, pdl, h->n, h->b, h->nblocks,
+                          (const double*)h->fac_fwd, (const double*)h->fac_bwd, in, out);
     } else {
         const unsigned blocks = (unsigned)((h->nblocks * 32 + threads - 1) / threads);
-        solve_warp_kernel<32, DIR><<<blocks, threads, 0, h->stream>>>(h->n, h->b, h->nblocks, h->fac_fwd, h->fac_bwd, in, out);
+        e = launch_kernel(solve_warp_kernel<32, DIR>, blocks, threads, 0, h->stream, pdl, h->n, h->b, h->nblocks,
+                          (const double*)h->fac_fwd, (const double*)h->fac_bwd, in, out);
     }
+    if (e != cudaSuccess) { set_cuda_error(e, "solve_warp_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
 

@@ -13,21 +13,15 @@
 
 #include <algorithm>
 
+#include "bj_device.cuh"
 #include "bj_internal.cuh"
 
 namespace bj {
 
-__device__ __forceinline__ double ldg_stream_f64(const double* p)
+int env_int(const char* name, int dflt)
 {
-    double v;
-    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
-    return v;
-}
-__device__ __forceinline__ int ldg_stream_s32(const int* p)
-{
-    int v;
-    asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
-    return v;
+    const char* v = getenv(name);
+    return v && *v ? atoi(v) : dflt;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -38,6 +32,8 @@ __global__ void __launch_bounds__(256)
 spmv_vector_kernel(int64_t n, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
                    const double* __restrict__ val, const double* __restrict__ x, double* __restrict__ y)
 {
+    pdl_trigger();
+    pdl_wait();
     const int64_t gtid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = gtid / LPR;
     const int lane = threadIdx.x & (LPR - 1);
@@ -45,8 +41,8 @@ spmv_vector_kernel(int64_t n, const int32_t* __restrict__ rp, const int32_t* __r
     if (row < n) {
         const int s = rp[row], e = rp[row + 1];
         for (int p = s + lane; p < e; p += LPR) {
-            const int c = ldg_stream_s32(ci + p);
-            const double v = ldg_stream_f64(val + p);
+            const int c = ld_stream(ci + p);
+            const double v = ld_stream(val + p);
             acc = fma(v, __ldg(x + c), acc);
         }
     }
@@ -61,16 +57,19 @@ int launch_spmv_vector(bj_handle_s* h, const double* x, double* y)
     const int lpr = h->spmv_lanes;
     const unsigned blocks = (unsigned)((h->n * lpr + threads - 1) / threads);
     KernelScope scope(h, BJ_K_SPMV);
-#define BJ_CASE(L)                                                                                              \
-    case L:                                                                                                     \
-        spmv_vector_kernel<L><<<blocks, threads, 0, h->stream>>>(h->n, h->row_ptr, h->col_idx, h->val, x, y);  \
+    const bool pdl = h->pdl && !h->prof_on;
+    cudaError_t e = cudaSuccess;
+#define BJ_CASE(L)                                                                                            \
+    case L:                                                                                                   \
+        e = launch_kernel(spmv_vector_kernel<L>, blocks, threads, 0, h->stream, pdl, h->n, h->row_ptr, h->col_idx, \
+                          h->val, x, y);                                                                      \
         break;
     switch (lpr) {
         BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
         default: return BJ_ERR_INVALID_ARG;
     }
 #undef BJ_CASE
-    BJ_CUDA(cudaGetLastError());
+    if (e != cudaSuccess) { set_cuda_error(e, "spmv_vector_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
 
@@ -92,8 +91,8 @@ int launch_spmv_vector(bj_handle_s* h, const double* x, double* y)
 // ------------------------------------------------------------------------------------------------
 namespace {
 
-constexpr int kConsumerThreads = 256;
-constexpr int kStreamThreads = kConsumerThreads + 32;
+constexpr int kMaxConsumerThreads = 512;
+constexpr int kMaxStreamThreads = kMaxConsumerThreads + 32;
 
 struct StreamParams {
     int64_t n, nnz;
@@ -110,6 +109,7 @@ struct StreamParams {
     int fac_bytes;       // bytes reserved per stage for factors
     int stage_bytes;
     int su_doubles;      // doubles per su buffer
+    unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -152,13 +152,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
         "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
         : "memory");
 }
-__device__ __forceinline__ void consumer_bar_sync()
+__device__ __forceinline__ void consumer_bar_sync(int nthreads)
 {
-    asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+    asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
 
-template <int LPR, int FUSE>
-__global__ void __launch_bounds__(kStreamThreads)
+// LPR lanes per row; BATCH entries per lane in flight per round; FUSE: forward solve in the epilogue
+template <int LPR, int BATCH, int FUSE>
+__global__ void __launch_bounds__(kMaxStreamThreads)
 spmv_stream_kernel(const StreamParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -173,10 +174,11 @@ spmv_stream_kernel(const StreamParams p)
     auto s_rp = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 12 + p.fac_bytes); };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_trigger();
     if (threadIdx.x == 0) {
         for (int s = 0; s < p.stages; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], kConsumerThreads / 32);
+            mbar_init(&empty[s], (blockDim.x - 32) / 32);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -247,8 +249,10 @@ spmv_stream_kernel(const StreamParams p)
     } else {
         // ------------------------------ consumers -----------------------------------------------
         const int ctid = threadIdx.x - 32;
+        const int nct = blockDim.x - 32;
         const int sub = ctid & (LPR - 1);
-        constexpr int kRowsPerPass = kConsumerThreads / LPR;
+        const int kRowsPerPass = nct / LPR;
+        pdl_wait();  // x (= t) comes from the previous kernel; the producer streams only setup-time constants
         int it = 0;
         for (int64_t tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
             const int s = it % p.stages;
@@ -267,32 +271,32 @@ spmv_stream_kernel(const StreamParams p)
                 const bool valid = i < rows;
                 double acc = 0.0;
                 if (valid) {
-                    // batches of four entries per lane: all four gathers are in flight together
+                    // BATCH entries per lane per round: all their gathers are in flight together
                     const int e = sr[i + 1] - a0;
-                    for (int q = sr[i] - a0 + sub; q < e; q += 4 * LPR) {
-                        int c[4];
-                        double xv[4], av[4];
+                    for (int q = sr[i] - a0 + sub; q < e; q += BATCH * LPR) {
+                        int c[BATCH];
+                        double xv[BATCH], av[BATCH];
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
+                        for (int k = 0; k < BATCH; ++k) {
                             const int qq = q + k * LPR;
                             c[k] = sc[qq < e ? qq : q];
                         }
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) xv[k] = __ldg(p.x + c[k]);
+                        for (int k = 0; k < BATCH; ++k) xv[k] = __ldg(p.x + c[k]);
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
+                        for (int k = 0; k < BATCH; ++k) {
                             const int qq = q + k * LPR;
                             av[k] = qq < e ? sv[qq] : 0.0;
                         }
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) acc = fma(av[k], xv[k], acc);
+                        for (int k = 0; k < BATCH; ++k) acc = fma(av[k], xv[k], acc);
                     }
                 }
 #pragma unroll
                 for (int off = LPR / 2; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off, LPR);
                 if (valid && sub == 0) {
                     if (FUSE) {
-                        const int k = i / p.b;
+                        const int k = (int)__umulhi((unsigned)i, p.b_magic);
                         sub_u[k * p.bs + (i - k * p.b)] = acc;
                     } else {
                         p.y[r0 + i] = acc;
@@ -301,12 +305,13 @@ spmv_stream_kernel(const StreamParams p)
             }
             if (FUSE) {
                 // (B) forward substitution y = L^-1 u on the tile's diagonal blocks, one thread per block
-                consumer_bar_sync();
+                consumer_bar_sync(nct);
                 const int nblk = (rows + p.b - 1) / p.b;
                 const int b = p.b;
                 const double* sf = s_fac(s);
-                const int rot = (ctid + 32 * (it & 7)) & (kConsumerThreads - 1);  // spread the work over warps
-                for (int k = rot; k < nblk; k += kConsumerThreads) {
+                int rot = ctid - 32 * (it & 7);  // rotate the solving warps from tile to tile
+                if (rot < 0) rot += nct;
+                for (int k = rot; k < nblk; k += nct) {
                     const double* f = sf + (size_t)(k >> 5) * p.P * kInterleave + (k & 31);
                     double* uk = sub_u + k * p.bs;
                     const int64_t lo = r0 + (int64_t)k * b;
@@ -333,24 +338,21 @@ spmv_stream_kernel(const StreamParams p)
     }
 }
 
-template <int LPR, int FUSE>
-int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int grid, size_t smem)
+template <int LPR, int BATCH, int FUSE>
+int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int grid, int threads, size_t smem)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, BATCH, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
-    spmv_stream_kernel<LPR, FUSE><<<grid, kStreamThreads, smem, h->stream>>>(sp);
+    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, BATCH, FUSE>, grid, threads, smem, h->stream,
+                                  h->pdl && !h->prof_on, sp);
+    if (e != cudaSuccess) { set_cuda_error(e, "spmv_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
 
-int env_int(const char* name, int dflt)
-{
-    const char* v = getenv(name);
-    return v && *v ? atoi(v) : dflt;
-}
 
 }  // namespace
 
@@ -369,6 +371,7 @@ void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem
     sp.fac_bytes = fuse ? (sp.R / sp.b) * sp.P * 8 : 0;
     sp.stage_bytes = (sp.cap * 12 + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
     sp.su_doubles = fuse ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : 0;
+    sp.b_magic = (unsigned)(((1ull << 32) + sp.b - 1) / sp.b);
     smem = 128 + (size_t)2 * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
 }
 constexpr size_t kSmemTwoPerSm = 110 * 1024;
@@ -417,7 +420,7 @@ int spmv_stream_configure(bj_handle_s* h)
     BJ_CUDA(cudaMemcpyAsync(&max_tile, &h->status->max_tile_nnz, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     BJ_CUDA(cudaStreamSynchronize(h->stream));
     h->tile_cap = ((max_tile + 8) + 3) & ~3;
-    int stages = env_int("BJ_STAGES", 3);
+    int stages = env_int("BJ_STAGES", 2);
     StreamParams sp;
     size_t smem = 0;
     h->tile_stages = stages;
@@ -443,14 +446,20 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
     sp.fac = fuse ? h->fac_small : nullptr;
-    const int per_sm = smem <= kSmemTwoPerSm ? 2 : 1;
-    const int grid = (int)std::min<int64_t>(h->ntiles, (int64_t)h->num_sms * env_int("BJ_CTAS_PER_SM", per_sm));
+    const int threads = 32 + 32 * std::max(1, std::min(env_int("BJ_CONSUMER_WARPS", 8), kMaxConsumerThreads / 32));
+    int per_sm = (int)((size_t)(227 * 1024) / (smem + 1024));
+    per_sm = std::max(1, std::min(per_sm, std::min(env_int("BJ_CTAS_PER_SM", 4), 2048 / threads)));
+    const int grid = (int)std::min<int64_t>(h->ntiles, (int64_t)h->num_sms * per_sm);
+    const int batch = env_int("BJ_BATCH", 8);
     int rc = BJ_OK;
     {
         KernelScope scope(h, fuse ? BJ_K_SPMV_SOLVE_L : BJ_K_SPMV);
-#define BJ_CASE(L)                                                                                     \
-    case L:                                                                                            \
-        rc = fuse ? launch_stream_t<L, 1>(h, sp, grid, smem) : launch_stream_t<L, 0>(h, sp, grid, smem); \
+#define BJ_CASE(L)                                                                                                 \
+    case L:                                                                                                        \
+        if (batch >= 8)                                                                                            \
+            rc = fuse ? launch_stream_t<L, 8, 1>(h, sp, grid, threads, smem) : launch_stream_t<L, 8, 0>(h, sp, grid, threads, smem); \
+        else                                                                                                       \
+            rc = fuse ? launch_stream_t<L, 4, 1>(h, sp, grid, threads, smem) : launch_stream_t<L, 4, 0>(h, sp, grid, threads, smem); \
         break;
         switch (h->stream_lanes) {
             BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
