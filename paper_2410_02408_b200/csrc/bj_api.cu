@@ -184,9 +184,11 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         } else {
             h->solve_kind = 2;
             h->lanes = b <= 16 ? 16 : 32;
-            const size_t sz = (size_t)h->nblocks * h->packed * sizeof(double);
+            const size_t sz = (size_t)h->nblocks * h->packed * sizeof(double) + 16;  // 16 B slack: bulk copies round up
             if (!dmalloc((void**)&h->fac_fwd, sz, &h->factor_bytes) || !dmalloc((void**)&h->fac_bwd, sz, &h->factor_bytes))
                 return fail(BJ_ERR_ALLOC);
+            ce = cudaMemsetAsync(h->fac_fwd, 0, sz, h->stream);
+            if (ce == cudaSuccess) ce = cudaMemsetAsync(h->fac_bwd, 0, sz, h->stream);
         }
         if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
         rc = launch_extract_factor(h);

@@ -39,6 +39,77 @@ __device__ __forceinline__ void st_v2(double* p, const double* v)
     asm volatile("st.global.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(v[0]), "d"(v[1]) : "memory");
 }
 
+// mbarrier + 1-D bulk async copy (TMA engine) primitives ------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+        : "memory");
+}
+
+// the shared solve of one diagonal block by a sub-warp of W lanes (lane i owns row i), factor read from
+// `f` (shared or global memory).  DIR 0: forward, f = column-major packed lower, rows scaled by 1/l_ii;
+// DIR 1: backward, f = row-major packed lower, columns scaled by 1/l_ii; diagonal slots hold 1/l_ii.
+//   forward : y_i = r_i/l_ii - sum_{j<i} (l_ij/l_ii) y_j      backward: x_i = y_i/l_ii - sum_{j>i} (l_ji/l_ii) x_j
+// Column oriented: at step j lane j's value is final and is broadcast by shuffle; one SHFL + one DFMA
+// per step on the dependent chain.  All W lanes must call (full-mask shuffles); lanes >= b return 0.
+template <int W, int DIR>
+__device__ __forceinline__ double subwarp_block_solve(const double* f, int b, int i, double r)
+{
+    // 1/l_ii sits in the diagonal slot of row/column i
+    const int dslot = DIR == 0 ? i * b - i * (i - 1) / 2 : i * (i + 1) / 2 + i;
+    r *= (i < b) ? f[dslot] : 0.0;
+#pragma unroll
+    for (int jj = 0; jj < W; ++jj) {
+        const int j = DIR == 0 ? jj : W - 1 - jj;
+        if (j < b) {
+            double lij = 0.0;  // off the dependent chain: the address does not depend on r
+            if (DIR == 0) {
+                if (i > j && i < b) lij = f[j * b - j * (j - 1) / 2 + (i - j)];
+            } else {
+                if (i < j) lij = f[j * (j + 1) / 2 + i];
+            }
+            const double vj = __shfl_sync(0xffffffffu, r, j, W);
+            r = fma(-lij, vj, r);
+        }
+    }
+    return r;
+}
+
 // Programmatic dependent launch.  Every kernel of the library calls pdl_trigger() first (lets the
 // next kernel in the stream start its independent prologue while this grid drains) and pdl_wait()
 // before its first access to memory that an earlier kernel in the stream may have written, and

@@ -83,8 +83,8 @@ int launch_spmv_plan(bj_handle_s* h)
 // Rows past the end of a ragged last block are treated as identity rows.
 // Output layouts (diagonal entries stored as RECIPROCALS so the solves multiply instead of divide):
 //   KIND 1 (b <= 8)  fac_small[(k/32) * P * 32 + e * 32 + k % 32],  e = i(i+1)/2 + j  (row-major packed)
-//   KIND 2 (b  > 8)  fac_fwd[k * P + j*b - j(j-1)/2 + (i-j)]        (column-major packed lower, forward solve)
-//                    fac_bwd[k * P + i(i+1)/2 + j]                  (row-major packed lower, backward solve)
+//   KIND 2 (b  > 8)  fac_fwd[k * P + j*b - j(j-1)/2 + (i-j)] = l_ij / l_ii  (column-major packed lower, forward)
+//                    fac_bwd[k * P + i(i+1)/2 + j]           = l_ij / l_jj  (row-major packed lower, backward)
 // ------------------------------------------------------------------------------------------------
 constexpr int kSetupWarps = 4;
 
@@ -149,13 +149,14 @@ extract_factor_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restri
     for (int idx = lane; idx < b * b; idx += 32) {
         const int i = idx / b, j = idx - i * b;
         if (j > i) continue;
-        double v = D[i * ld + j];
-        if (i == j) v = 1.0 / v;
+        const double v = D[i * ld + j];
         if (KIND == 1) {
-            out0[(k >> 5) * (int64_t)P * kInterleave + (int64_t)(i * (i + 1) / 2 + j) * kInterleave + (k & 31)] = v;
+            out0[(k >> 5) * (int64_t)P * kInterleave + (int64_t)(i * (i + 1) / 2 + j) * kInterleave + (k & 31)] =
+                (i == j) ? 1.0 / v : v;
         } else {
-            out0[k * P + (j * b - j * (j - 1) / 2 + (i - j))] = v;
-            out1[k * P + (i * (i + 1) / 2 + j)] = v;
+            // forward copy: row i scaled by 1/l_ii; backward copy: column j scaled by 1/l_jj
+            out0[k * P + (j * b - j * (j - 1) / 2 + (i - j))] = (i == j) ? 1.0 / v : v / D[i * ld + i];
+            out1[k * P + (i * (i + 1) / 2 + j)] = (i == j) ? 1.0 / v : v / D[j * ld + j];
         }
     }
 }

@@ -7,10 +7,12 @@
 //            element e of blocks 32g..32g+31 is one 256-byte line: every load of the warp is fully
 //            coalesced and all P = b(b+1)/2 loads of a thread are independent (deep MLP).
 //   b  > 8 : one SUB-WARP (16 or 32 lanes) per block, lane i owns row i.  Forward substitution is
-//            column oriented: at step j lane j finalises y_j, broadcasts it by shuffle, lanes i > j
-//            subtract L_ij y_j.  Column j of L is contiguous in the column-major packed copy, so the
-//            lanes' loads coalesce; the backward solve reads the row-major packed copy the same way.
-//            All b column loads of a lane are issued before the dependent chain starts.
+//            column oriented: at step j lane j's y_j is final, is broadcast by shuffle, lanes i > j
+//            subtract L_ij y_j.  The packed factors are streamed into shared memory by bulk async
+//            copies (TMA) in a persistent producer/consumer ring, so HBM streaming never waits for
+//            a block's dependent chain.
+#include <algorithm>
+
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
 
@@ -88,65 +90,113 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
 }
 
 // ------------------------------------------------------------------------------------------------
-// sub-warp per block, W lanes (b <= W), lane i owns row i.
+// b > 8: persistent CTAs, factors streamed through a shared-memory ring by the TMA engine.
+// A tile is G consecutive blocks; their packed factors are one contiguous byte range, moved by ONE
+// bulk async copy per stage (two when DIR == 2 needs both copies).  Each consumer sub-warp (W = 16
+// or 32 lanes, lane i owns row i) takes blocks of the tile round-robin: its right-hand sides are
+// fetched from global memory before it waits for the stage, the substitution runs out of shared
+// memory (subwarp_block_solve), results go straight back to global memory.  HBM streaming is thereby
+// decoupled from the b-step dependent chain of each block.
 // ------------------------------------------------------------------------------------------------
-template <int W, int DIR>
-__global__ void __launch_bounds__(256)
-solve_warp_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ fwd,
-                  const double* __restrict__ bwd, const double* in, double* out)  // in == out allowed
-{
-    pdl_trigger();
-    const int i = threadIdx.x & (W - 1);
-    int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / W;
-    const bool act = k < nblocks;  // no early return: the full-mask shuffles below need every lane
-    if (!act) k = 0;
-    const unsigned full = 0xffffffffu;
-    const int P = b * (b + 1) / 2;
-    const int64_t row = k * b + i;
-    const bool live = act && (i < b) && (row < n);
-    double r = 0.0;
-    double l[W];
+constexpr int kMaxBlocksPerSub = 4;
 
-    if (DIR == 0 || DIR == 2) {
-        const double* f = fwd + k * (int64_t)P;
-#pragma unroll
-        for (int j = 0; j < W; ++j) {
-            // column j: rows j..b-1 at offset j*b - j(j-1)/2
-            l[j] = (act && j < b && i >= j && i < b) ? ld_stream(f + (j * b - j * (j - 1) / 2) + (i - j)) : 0.0;
+struct SolveStreamParams {
+    int64_t n, nblocks, ntiles;
+    const double* fac0;  // forward copy (DIR 0, 2) or backward copy (DIR 1)
+    const double* fac1;  // backward copy (DIR 2 only)
+    const double* in;
+    double* out;
+    int b, P, G, stages;
+    int copy_doubles;    // doubles reserved per copy per stage (G * P rounded to even)
+};
+
+template <int W, int DIR>
+__global__ void __launch_bounds__(32 + 256)
+solve_stream_kernel(const SolveStreamParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    uint64_t* empty = full + p.stages;
+    double* stage0 = reinterpret_cast<double*>(smem_raw + 128);
+    constexpr int kCopies = DIR == 2 ? 2 : 1;
+    const int stage_doubles = kCopies * p.copy_doubles;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_trigger();
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], (blockDim.x - 32) / 32);
         }
-        pdl_wait();
-        r = live ? in[row] : 0.0;
-#pragma unroll
-        for (int j = 0; j < W; ++j) {
-            if (j < b) {
-                const double cand = r * l[j];                      // lane j: y_j = r_j / l_jj
-                const double yj = __shfl_sync(full, cand, j, W);
-                r = (i == j) ? yj : fma(-l[j], yj, r);             // lanes i < j hold l[j] = 0
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == 0) {
+        if (lane == 0) {
+            const uint64_t pol = policy_evict_first();
+            int it = 0;
+            for (int64_t tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
+                const int s = it % p.stages;
+                const uint32_t ph = (uint32_t)((it / p.stages) & 1);
+                mbar_wait(&empty[s], ph ^ 1u);
+                const int64_t k0 = tile * p.G;
+                const int nb = (int)(k0 + p.G <= p.nblocks ? p.G : p.nblocks - k0);
+                const uint32_t bytes = (uint32_t)(((size_t)nb * p.P * 8 + 15) & ~(size_t)15);  // arrays carry 16 B of slack
+                double* dst = stage0 + (size_t)s * stage_doubles;
+                mbar_expect_tx(&full[s], bytes * kCopies);
+                bulk_g2s(dst, p.fac0 + k0 * p.P, bytes, &full[s], pol);
+                if (DIR == 2) bulk_g2s(dst + p.copy_doubles, p.fac1 + k0 * p.P, bytes, &full[s], pol);
             }
         }
-    }
-    if (DIR == 1 || DIR == 2) {
-        const double* f = bwd + k * (int64_t)P;
+    } else {
+        const int ctid = threadIdx.x - 32;
+        const int nsub = (blockDim.x - 32) / W;
+        const int sub = ctid / W;
+        const int i = ctid & (W - 1);
+        const int b = p.b;
+        pdl_wait();  // `in` may come from the previous kernel
+        // right-hand sides are fetched one tile ahead: their HBM latency hides behind the current tile's solves
+        auto fetch_rhs = [&](int64_t tile, double* dst) {
+            const int64_t k0 = tile * p.G;
 #pragma unroll
-        for (int j = 0; j < W; ++j) {
-            // row j: columns 0..j at offset j(j+1)/2
-            l[j] = (act && j < b && i <= j) ? ld_stream(f + j * (j + 1) / 2 + i) : 0.0;
-        }
-        if (DIR == 1) {
-            pdl_wait();
-            r = live ? in[row] : 0.0;
-        }
-#pragma unroll
-        for (int jj = 0; jj < W; ++jj) {
-            const int j = W - 1 - jj;
-            if (j < b) {
-                const double cand = r * l[j];                      // lane j: x_j = r_j / l_jj
-                const double xj = __shfl_sync(full, cand, j, W);
-                r = (i == j) ? xj : fma(-l[j], xj, r);             // lanes i > j hold l[j] = 0
+            for (int q = 0; q < kMaxBlocksPerSub; ++q) {
+                const int64_t kb = k0 + sub + q * nsub;
+                const int64_t row = kb * b + i;
+                dst[q] = (tile < p.ntiles && q * nsub < p.G && kb < p.nblocks && i < b && row < p.n) ? p.in[row] : 0.0;
             }
+        };
+        double rn[kMaxBlocksPerSub];
+        fetch_rhs(blockIdx.x, rn);
+        int it = 0;
+        for (int64_t tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
+            const int s = it % p.stages;
+            const uint32_t ph = (uint32_t)((it / p.stages) & 1);
+            const int64_t k0 = tile * p.G;
+            const int nb = (int)(k0 + p.G <= p.nblocks ? p.G : p.nblocks - k0);
+            double r[kMaxBlocksPerSub];
+#pragma unroll
+            for (int q = 0; q < kMaxBlocksPerSub; ++q) r[q] = rn[q];
+            fetch_rhs(tile + gridDim.x, rn);
+            mbar_wait(&full[s], ph);
+            const double* f = stage0 + (size_t)s * stage_doubles;
+#pragma unroll
+            for (int q = 0; q < kMaxBlocksPerSub; ++q) {
+                const int kb = sub + q * nsub;
+                if (q * nsub < p.G) {  // uniform over the CTA
+                    const int kc = kb < nb ? kb : 0;  // idle sub-warps read block 0 (valid memory), result dropped
+                    double v = r[q];
+                    if (DIR == 0 || DIR == 2) v = subwarp_block_solve<W, 0>(f + (size_t)kc * p.P, b, i, v);
+                    if (DIR == 1) v = subwarp_block_solve<W, 1>(f + (size_t)kc * p.P, b, i, v);
+                    if (DIR == 2) v = subwarp_block_solve<W, 1>(f + p.copy_doubles + (size_t)kc * p.P, b, i, v);
+                    const int64_t row = (k0 + kb) * b + i;
+                    if (kb < nb && i < b && row < p.n) p.out[row] = v;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
         }
     }
-    if (live) out[row] = r;
 }
 
 // b == 1 fast path is just the B = 1 instance of solve_small_kernel.
@@ -175,23 +225,53 @@ static int launch_small(bj_handle_s* h, const double* in, double* out)
     return BJ_OK;
 }
 
+template <int W, int DIR>
+static int launch_stream_solve(bj_handle_s* h, const SolveStreamParams& sp, int want_per_sm, int threads, size_t smem)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_stream_kernel)"); return BJ_ERR_CUDA; }
+        configured = true;
+    }
+    int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR>, threads, smem);
+    const int per_sm = std::max(1, std::min(occ, want_per_sm));
+    const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
+    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
+    if (e != cudaSuccess) { set_cuda_error(e, "solve_stream_kernel launch"); return BJ_ERR_CUDA; }
+    return BJ_OK;
+}
+
 template <int DIR>
 static int launch_warp(bj_handle_s* h, const double* in, double* out)
 {
-    const int threads = 256;
-    const bool pdl = h->pdl && !h->prof_on;
-    cudaError_t e;
-    if (h->lanes == 16) {
-        const unsigned blocks = (unsigned)((h->nblocks * 16 + threads - 1) / threads);
-        e = launch_kernel(solve_warp_kernel<16, DIR>, blocks, threads, 0, h->stream, pdl, h->n, h->b, h->nblocks,
-                          (const double*)h->fac_fwd, (const double*)h->fac_bwd, in, out);
-    } else {
-        const unsigned blocks = (unsigned)((h->nblocks * 32 + threads - 1) / threads);
-        e = launch_kernel(solve_warp_kernel<32, DIR>, blocks, threads, 0, h->stream, pdl, h->n, h->b, h->nblocks,
-                          (const double*)h->fac_fwd, (const double*)h->fac_bwd, in, out);
-    }
-    if (e != cudaSuccess) { set_cuda_error(e, "solve_warp_kernel launch"); return BJ_ERR_CUDA; }
-    return BJ_OK;
+    const int W = h->lanes;
+    const int cwarps = std::max(1, std::min(env_int("BJ_SOLVE_WARPS", 8), 8));
+    const int threads = 32 + 32 * cwarps;
+    const int nsub = cwarps * 32 / W;
+    const int copies = DIR == 2 ? 2 : 1;
+    const size_t block_bytes = (size_t)h->packed * 8;
+    const int target = env_int("BJ_SOLVE_STAGE_KB", 32) * 1024;
+    int bps = (int)((target / copies + nsub * block_bytes / 2) / (nsub * block_bytes));
+    bps = std::max(1, std::min(bps, kMaxBlocksPerSub));
+    SolveStreamParams sp;
+    sp.n = h->n; sp.nblocks = h->nblocks; sp.b = h->b; sp.P = h->packed;
+    sp.G = nsub * bps;
+    if (sp.G % 2) sp.G += 1;  // keeps every tile's byte offset 16-byte aligned when P is odd
+    sp.ntiles = (h->nblocks + sp.G - 1) / sp.G;
+    sp.copy_doubles = (sp.G * sp.P + 1) & ~1;
+    sp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
+    sp.fac1 = h->fac_bwd;
+    sp.in = in; sp.out = out;
+    const size_t stage_bytes = (size_t)copies * sp.copy_doubles * 8;
+    int stages = std::max(2, env_int("BJ_SOLVE_STAGES", 2));
+    while (stages > 2 && 128 + stages * stage_bytes > 110 * 1024) --stages;
+    sp.stages = stages;
+    const size_t smem = 128 + stages * stage_bytes;
+    const int per_sm = env_int("BJ_SOLVE_CTAS", 4);
+    return W == 16 ? launch_stream_solve<16, DIR>(h, sp, per_sm, threads, smem)
+                   : launch_stream_solve<32, DIR>(h, sp, per_sm, threads, smem);
 }
 
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)

@@ -112,53 +112,14 @@ struct StreamParams {
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ uint64_t policy_evict_first()
-{
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
-            smem_u32(dst)),
-        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
-        : "memory");
-}
 __device__ __forceinline__ void consumer_bar_sync(int nthreads)
 {
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
 
-// LPR lanes per row; BATCH entries per lane in flight per round; FUSE: forward solve in the epilogue
-template <int LPR, int BATCH, int FUSE>
+// LPR lanes per row; BATCH entries per lane in flight per round;
+// FUSE: 0 = SpMV only, 1 = + forward solve, thread per block (b <= 8), 2 = + forward solve, sub-warp of W lanes per block
+template <int LPR, int BATCH, int FUSE, int W>
 __global__ void __launch_bounds__(kMaxStreamThreads)
 spmv_stream_kernel(const StreamParams p)
 {
@@ -230,11 +191,17 @@ spmv_stream_kernel(const StreamParams p)
                 uint32_t bytes = (uint32_t)(a1 - a0) * 12u + (uint32_t)rq * 4u;
                 uint32_t fbytes = 0;
                 const double* fsrc = nullptr;
-                if (FUSE) {
+                if (FUSE == 1) {
                     const int nblk = (rows + p.b - 1) / p.b;
                     const int groups = (nblk + kInterleave - 1) / kInterleave;
                     fbytes = (uint32_t)groups * (uint32_t)p.P * kInterleave * 8u;
                     fsrc = p.fac + (r0 / p.b / kInterleave) * (int64_t)p.P * kInterleave;
+                    bytes += fbytes;
+                }
+                if (FUSE == 2) {
+                    const int nblk = (rows + p.b - 1) / p.b;
+                    fbytes = (uint32_t)(((size_t)nblk * p.P * 8 + 15) & ~(size_t)15);  // factor arrays carry 16 B of slack
+                    fsrc = p.fac + (r0 / p.b) * (int64_t)p.P;
                     bytes += fbytes;
                 }
                 mbar_expect_tx(&full[s], bytes);
@@ -295,15 +262,38 @@ spmv_stream_kernel(const StreamParams p)
 #pragma unroll
                 for (int off = LPR / 2; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off, LPR);
                 if (valid && sub == 0) {
-                    if (FUSE) {
+                    if (FUSE == 1) {
                         const int k = (int)__umulhi((unsigned)i, p.b_magic);
                         sub_u[k * p.bs + (i - k * p.b)] = acc;
+                    } else if (FUSE == 2) {
+                        sub_u[i] = acc;
                     } else {
                         p.y[r0 + i] = acc;
                     }
                 }
             }
-            if (FUSE) {
+            if (FUSE == 2) {
+                // (B) forward substitution y = L^-1 u, one sub-warp of W lanes per diagonal block
+                consumer_bar_sync(nct);
+                const int b = p.b;
+                const int nblk = (rows + b - 1) / b;
+                const int G = R / b;
+                const int nsub = nct / W;
+                const int sw = ctid / W;
+                const int li = ctid & (W - 1);
+                const double* sf = s_fac(s);
+                for (int q = 0; q * nsub < G; ++q) {
+                    const int kb = sw + q * nsub;
+                    const bool act = kb < nblk;
+                    const int kc = act ? kb : 0;  // idle sub-warps redo block 0, result dropped
+                    const int64_t row = r0 + (int64_t)kc * b + li;
+                    const bool live = act && li < b && row < p.n;
+                    double v = live ? sub_u[kc * b + li] : 0.0;
+                    v = subwarp_block_solve<W, 0>(sf + (size_t)kc * p.P, b, li, v);
+                    if (live) p.y[row] = v;
+                }
+            }
+            if (FUSE == 1) {
                 // (B) forward substitution y = L^-1 u on the tile's diagonal blocks, one thread per block
                 consumer_bar_sync(nct);
                 const int nblk = (rows + p.b - 1) / p.b;
@@ -338,16 +328,20 @@ spmv_stream_kernel(const StreamParams p)
     }
 }
 
-template <int LPR, int BATCH, int FUSE>
-int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int grid, int threads, size_t smem)
+template <int LPR, int BATCH, int FUSE, int W>
+int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, BATCH, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, BATCH, FUSE, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
-    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, BATCH, FUSE>, grid, threads, smem, h->stream,
+    int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_stream_kernel<LPR, BATCH, FUSE, W>, threads, smem);
+    const int per_sm = std::max(1, std::min(occ, want_per_sm));
+    const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
+    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, BATCH, FUSE, W>, grid, threads, smem, h->stream,
                                   h->pdl && !h->prof_on, sp);
     if (e != cudaSuccess) { set_cuda_error(e, "spmv_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
@@ -368,9 +362,9 @@ void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem
     sp.stages = h->tile_stages;
     sp.ntiles = h->ntiles;
     sp.rp_ints = sp.R + 4;
-    sp.fac_bytes = fuse ? (sp.R / sp.b) * sp.P * 8 : 0;
+    sp.fac_bytes = fuse ? (((sp.R / sp.b) * sp.P * 8 + 15) & ~15) : 0;
     sp.stage_bytes = (sp.cap * 12 + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
-    sp.su_doubles = fuse ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : 0;
+    sp.su_doubles = !fuse ? 0 : (h->solve_kind == 1 ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : ((sp.R + 1) & ~1));
     sp.b_magic = (unsigned)(((1ull << 32) + sp.b - 1) / sp.b);
     smem = 128 + (size_t)2 * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
 }
@@ -405,9 +399,17 @@ int spmv_stream_configure(bj_handle_s* h)
         if (Rf < unit) Rf = unit;
         if ((double)Rf * mean <= 1.6 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
     }
+    if (h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 1)) {
+        // fused tiles hold whole blocks; an even block count keeps every tile's factor range 16-byte aligned
+        const int unit = 4 * h->b;
+        int Rf = ((R + unit / 2) / unit) * unit;
+        if (Rf < unit) Rf = unit;
+        if ((double)Rf * mean <= 2.0 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
+    }
     if (!fuse) R = ((R + 31) / 32) * 32;
     R = env_int("BJ_TILE_ROWS", R);
-    if (fuse && (R % (kInterleave * h->b)) != 0) fuse = false;
+    if (fuse && h->solve_kind == 1 && (R % (kInterleave * h->b)) != 0) fuse = false;
+    if (fuse && h->solve_kind == 2 && (R % (4 * h->b)) != 0) fuse = false;
     if (R % 4) return BJ_OK;
     h->tile_rows = R;
     h->ntiles = (h->n + R - 1) / R;
@@ -445,21 +447,19 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     fill_layout(h, fuse, sp, smem);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
-    sp.fac = fuse ? h->fac_small : nullptr;
+    sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
     const int threads = 32 + 32 * std::max(1, std::min(env_int("BJ_CONSUMER_WARPS", 8), kMaxConsumerThreads / 32));
-    int per_sm = (int)((size_t)(227 * 1024) / (smem + 1024));
-    per_sm = std::max(1, std::min(per_sm, std::min(env_int("BJ_CTAS_PER_SM", 4), 2048 / threads)));
-    const int grid = (int)std::min<int64_t>(h->ntiles, (int64_t)h->num_sms * per_sm);
-    const int batch = env_int("BJ_BATCH", 8);
+    const int grid = env_int("BJ_CTAS_PER_SM", 4);  // wanted CTAs per SM; clipped to the real occupancy at launch
     int rc = BJ_OK;
     {
         KernelScope scope(h, fuse ? BJ_K_SPMV_SOLVE_L : BJ_K_SPMV);
-#define BJ_CASE(L)                                                                                                 \
-    case L:                                                                                                        \
-        if (batch >= 8)                                                                                            \
-            rc = fuse ? launch_stream_t<L, 8, 1>(h, sp, grid, threads, smem) : launch_stream_t<L, 8, 0>(h, sp, grid, threads, smem); \
-        else                                                                                                       \
-            rc = fuse ? launch_stream_t<L, 4, 1>(h, sp, grid, threads, smem) : launch_stream_t<L, 4, 0>(h, sp, grid, threads, smem); \
+        const int mode = !fuse ? 0 : (h->solve_kind == 1 ? 1 : (h->lanes == 16 ? 2 : 3));
+#define BJ_CASE(L)                                                                               \
+    case L:                                                                                      \
+        rc = mode == 0   ? launch_stream_t<L, 8, 0, 32>(h, sp, grid, threads, smem)               \
+             : mode == 1 ? launch_stream_t<L, 8, 1, 32>(h, sp, grid, threads, smem)               \
+             : mode == 2 ? launch_stream_t<L, 8, 2, 16>(h, sp, grid, threads, smem)               \
+                         : launch_stream_t<L, 8, 2, 32>(h, sp, grid, threads, smem);              \
         break;
         switch (h->stream_lanes) {
             BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
