@@ -43,6 +43,16 @@ def algorithmic_bytes(n: int, nnz: int, b: int) -> dict:
             "spmv_solve_L": spmv + solve, "op_apply": spmv + 2 * solve}
 
 
+def ncu_traffic(cfg: int, b: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary
+    (profiles/traffic.json, written by hand from profiles/*.md); None if that kernel was not captured."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return json.load(fh).get(f"cfg{cfg}_b{b}", {}).get(kernel)
+    except Exception:
+        return None
+
+
 def measured_peaks() -> tuple[float, str]:
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -256,7 +266,8 @@ def main():
     dom = max(kern, key=lambda k: kern[k]["avg_us"])
     total_us = sum(v["avg_us"] for v in kern.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kern[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                "frac": kern[dom]["gbs"] / peak, "traffic": ncu_traffic(args.config, b, dom), "peak_source": peak_src,
+                "algorithmic_bytes": kern[dom]["alg_bytes"],
                 "share_of_step": kern[dom]["avg_us"] / total_us,
                 "frac_of_nominal_8TBs": kern[dom]["gbs"] / NOMINAL_HBM_GBS}
     op_gbs = ab["op_apply"] / (ms_per_step * 1e-3) / 1e9

@@ -165,6 +165,8 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     if (ce != cudaSuccess) { set_cuda_error(ce, "validate"); return fail(BJ_ERR_CUDA); }
     if (stt.flags & (ST_BAD_ROWPTR | ST_BAD_COL | ST_UNSORTED)) return fail(BJ_ERR_NOT_CANONICAL);
 
+    h->coherence = stt.compared ? (double)stt.coherent / (double)stt.compared : 1.0;
+
     // lanes per row for the SpMV kernels: power of two near the mean row length
     {
         const double mean = (double)h->nnz / (double)h->n;

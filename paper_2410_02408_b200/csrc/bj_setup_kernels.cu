@@ -17,26 +17,35 @@ validate_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ rp, const in
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int flags = 0;
     int len = 0;
+    unsigned coh = 0, cmp = 0;
     if (i < n) {
         int64_t s = rp[i], e = rp[i + 1];
         if (s > e || s < 0 || e > nnz || (i == 0 && s != 0) || (i == n - 1 && e != nnz)) {
             flags |= ST_BAD_ROWPTR;
         } else {
             len = (int)(e - s);
+            // next row, only if its pointers are sane (it validates itself): used for the coherence statistic
+            int64_t s2 = 0, e2 = 0;
+            if (i + 1 < n) { s2 = e; e2 = rp[i + 2]; if (e2 < s2 || e2 > nnz) e2 = s2; }
             int prev = -1;
             for (int64_t p = s; p < e; ++p) {
                 int c = ci[p];
                 if (c < 0 || c >= n) flags |= ST_BAD_COL;
                 if (c <= prev) flags |= ST_UNSORTED;
                 prev = c;
+                if (s2 + (p - s) < e2) { ++cmp; coh += (ci[s2 + (p - s)] == c + 1); }
             }
         }
     }
     flags = __reduce_or_sync(0xffffffffu, flags);
     len = __reduce_max_sync(0xffffffffu, len);
+    coh = __reduce_add_sync(0xffffffffu, coh);
+    cmp = __reduce_add_sync(0xffffffffu, cmp);
     if ((threadIdx.x & 31) == 0) {
         if (flags) atomicOr(&st->flags, flags);
         atomicMax(&st->max_row_nnz, len);
+        atomicAdd(&st->coherent, (unsigned long long)coh);
+        atomicAdd(&st->compared, (unsigned long long)cmp);
     }
 }
 

@@ -387,19 +387,25 @@ int spmv_stream_configure(bj_handle_s* h)
         // (coalesced gathers for banded matrices, oracle summation order) up to ~12 entries per row
         int l = 1;
         while (l < 32 && (double)l * 12.0 < mean) l *= 2;
+        // Random column structure (no coherence between neighbouring rows): the kernel is bound by the
+        // L1/LSU gather rate, not by HBM; what helps is many warps with gathers in flight, one row per thread.
+        const bool random_cols = h->coherence < 0.25;
+        if (random_cols && mean <= 48.0) l = 1;
         h->stream_lanes = env_int("BJ_STREAM_LANES", l);
+        h->stream_warps = std::max(1, std::min(env_int("BJ_CONSUMER_WARPS", random_cols ? 16 : 8), kMaxConsumerThreads / 32));
     }
     const int target_nnz = env_int("BJ_TILE_NNZ", 2048);
     int R = (int)((double)target_nnz / (mean > 1.0 ? mean : 1.0));
     R = std::max(32, std::min(R, 1024));
     bool fuse = false;
-    if (h->solve_kind == 1) {
+    const bool random_cols = h->coherence < 0.25;
+    if (h->solve_kind == 1 && !random_cols) {
         const int unit = kInterleave * h->b;  // fused tiles must hold whole interleave groups
         int Rf = ((R + unit / 2) / unit) * unit;
         if (Rf < unit) Rf = unit;
         if ((double)Rf * mean <= 1.6 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
     }
-    if (h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 1)) {
+    if (h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 0)) {
         // fused tiles hold whole blocks; an even block count keeps every tile's factor range 16-byte aligned
         const int unit = 4 * h->b;
         int Rf = ((R + unit / 2) / unit) * unit;
@@ -448,7 +454,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
     sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
-    const int threads = 32 + 32 * std::max(1, std::min(env_int("BJ_CONSUMER_WARPS", 8), kMaxConsumerThreads / 32));
+    const int threads = 32 + 32 * h->stream_warps;
     const int grid = env_int("BJ_CTAS_PER_SM", 4);  // wanted CTAs per SM; clipped to the real occupancy at launch
     int rc = BJ_OK;
     {

@@ -297,6 +297,33 @@ def test_runs_on_a_side_stream_and_profiling_counts(B, torch_, rel):
     B.bj_destroy(h)
 
 
+def test_fused_subwarp_forward_solve_path(B, torch_, rel, monkeypatch):
+    """The SpMV tile kernel can also run the b > 8 forward solve in its epilogue (off by default: not faster yet)."""
+    monkeypatch.setenv("BJ_FUSE_WARP", "1")
+    for cfg, b in ((4, 16), (3, 32), (5, 24), (2, 12)):
+        A = mat(cfg, "small")
+        h, keep = B.setup_from_host(A, b)
+        assert B.bj_get_info(h)["fused_forward"] == 1
+        B.bj_destroy(h)
+        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
+
+
+def test_block_size_sweep_runs_the_real_path(B, torch_):
+    """a11: host-side sweep over b; kappa estimates agree with the oracle at the chosen b; b = N/.. ordering sane."""
+    from paper_2410_02408_b200 import sweep
+    A = mat(1, "full")
+    rp, ci, val = dev(torch_, A.row_ptr), dev(torch_, A.col_idx), dev(torch_, A.val)
+    res = sweep.sweep(rp, ci, val, blocks=(1, 4, 32), iters=50, apply_steps=20)
+    assert [r["b"] for r in res["rows"]] == [1, 4, 32]
+    for r in res["rows"]:
+        c = oracle.Precond(A, r["b"]).cond_estimate(50)
+        assert abs(r["kappa_est"] / c["kappa"] - 1) <= TOL_KAPPA
+        assert r["applies_per_s"] > 0 and r["setup_ms"] > 0
+    c0 = oracle.Precond(A, 0).cond_estimate(50)
+    assert abs(res["kappa_A"]["kappa_est"] / c0["kappa"] - 1) <= TOL_KAPPA
+    assert res["best_b"] == min(res["rows"], key=lambda r: r["kappa_est"])["b"]
+
+
 # ------------------------------------------------------------------ BASELINE.json full sizes -------------
 @pytest.mark.parametrize("cfg", [2, 3, 4, 5])
 def test_full_size_configs(B, torch_, rel, cfg):
