@@ -25,7 +25,7 @@ struct Status {
     long long bad_block;  // atomicMin target
     int max_tile_nnz;     // SpMV plan
     int max_row_nnz;
-    unsigned long long coherent;  // entries whose column is the upper neighbour row's column + 1 (banded structure)
+    unsigned long long coherent;  // entries whose column is within 16 of the same-position column of the next row
     unsigned long long compared;  // entries compared
 };
 
@@ -81,7 +81,7 @@ struct bj_handle_s {
     int spmv_lanes = 8;       // lanes per row, CSR-vector kernel
     int stream_lanes = 1;     // lanes per row, reduce phase of the tile kernel
     int stream_warps = 8;     // consumer warps of the tile kernel
-    double coherence = 1.0;   // fraction of entries with col(i+1, j) == col(i, j) + 1: ~1 banded, ~0 random
+    double coherence = 1.0;   // fraction of entries with |col(i+1, j) - col(i, j)| <= 16: ~1 banded/stencil, ~0 random
     int spmv_kernel = 0;      // chosen kernel
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;

@@ -33,7 +33,7 @@ validate_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ rp, const in
                 if (c < 0 || c >= n) flags |= ST_BAD_COL;
                 if (c <= prev) flags |= ST_UNSORTED;
                 prev = c;
-                if (s2 + (p - s) < e2) { ++cmp; coh += (ci[s2 + (p - s)] == c + 1); }
+                if (s2 + (p - s) < e2) { ++cmp; const int d = ci[s2 + (p - s)] - c; coh += (d >= -16 && d <= 16); }
             }
         }
     }

@@ -406,8 +406,10 @@ int spmv_stream_configure(bj_handle_s* h)
         if ((double)Rf * mean <= 1.6 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
     }
     if (h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 0)) {
-        // fused tiles hold whole blocks; an even block count keeps every tile's factor range 16-byte aligned
-        const int unit = 4 * h->b;
+        // fused tiles hold whole blocks; with an odd packed size an even block count keeps every tile's factor
+        // range 16-byte aligned; row pointers need the tile start to be a multiple of 4 rows
+        int unit = h->b * ((h->packed % 2) ? 2 : 1);
+        while (unit % 4) unit += h->b * ((h->packed % 2) ? 2 : 1);
         int Rf = ((R + unit / 2) / unit) * unit;
         if (Rf < unit) Rf = unit;
         if ((double)Rf * mean <= 2.0 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
@@ -415,7 +417,7 @@ int spmv_stream_configure(bj_handle_s* h)
     if (!fuse) R = ((R + 31) / 32) * 32;
     R = env_int("BJ_TILE_ROWS", R);
     if (fuse && h->solve_kind == 1 && (R % (kInterleave * h->b)) != 0) fuse = false;
-    if (fuse && h->solve_kind == 2 && (R % (4 * h->b)) != 0) fuse = false;
+    if (fuse && h->solve_kind == 2 && ((R % h->b) != 0 || (((R / h->b) * h->packed) % 2) != 0)) fuse = false;
     if (R % 4) return BJ_OK;
     h->tile_rows = R;
     h->ntiles = (h->n + R - 1) / R;
