@@ -12,6 +12,7 @@
 
 #include <algorithm>
 
+#include "bj_device.cuh"
 #include "bj_internal.cuh"
 
 namespace bj {
@@ -60,62 +61,113 @@ __device__ __forceinline__ Chunk my_chunk(int64_t n)
     return c;
 }
 
-// partial[blockIdx.x * stride + slot] = sum over the CTA's chunk of a[i] * b[i]
+// Every CTA of a consumer kernel re-sums the producer's per-CTA partials in the same fixed order, so all
+// CTAs hold the identical scalar without a separate finalize launch (deterministic, no atomics).
+__device__ __forceinline__ double reduce_partials(const double* __restrict__ part, int nparts, double* sh)
+{
+    double s = 0.0;
+    for (int p = threadIdx.x; p < nparts; p += blockDim.x) s += part[p];
+    s = block_sum(s, sh);
+    __syncthreads();
+    if (threadIdx.x == 0) sh[0] = s;
+    __syncthreads();
+    return sh[0];
+}
+
+// P[cta] = sum over the CTA's chunk of a[i] * b[i]
 __global__ void __launch_bounds__(kReduceThreads)
-dot_partial_kernel(int64_t n, const double* __restrict__ a, const double* __restrict__ b,
-                   double* __restrict__ partial, int stride, const int* __restrict__ done)
+dot_partial_kernel(int64_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ P)
 {
     __shared__ double sh[kReduceThreads / 32];
-    if (done && done[0]) return;
+    pdl_trigger();
+    pdl_wait();
     const Chunk c = my_chunk(n);
     double s = 0.0;
     for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) s = fma(a[i], b[i], s);
     s = block_sum(s, sh);
-    if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * stride] = s;
+    if (threadIdx.x == 0) P[blockIdx.x] = s;
 }
 
-// w -= beta_j * vprev (when vprev != null);  partial of v . w
+// Closes step j_prev and opens the next one:  beta = sqrt(sum PB);  out = in / beta.
+//   mode 0: start vector, v_1 = v0 / ||v0||, no bookkeeping.
+//   mode 1: beta_{j_prev+2} = ||w||: CTA 0 records beta[j_prev], max|alpha|, m_eff and the breakdown flag
+//           (beta <= tol max|alpha|); on breakdown nothing is written.  out == nullptr: bookkeeping only.
 __global__ void __launch_bounds__(kReduceThreads)
-alpha_partial_kernel(int64_t n, double* __restrict__ w, const double* __restrict__ vprev,
-                     const double* __restrict__ v, const double* __restrict__ scal,
-                     double* __restrict__ partial, int stride, const int* __restrict__ done)
+scale_kernel(int64_t n, const double* __restrict__ in, double* __restrict__ out, const double* __restrict__ PB,
+             int nparts, int mode, int j_prev, double tol, const double* __restrict__ alpha,
+             double* __restrict__ beta, double* __restrict__ amax_buf, int* __restrict__ done)
 {
     __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    if (done[0]) return;
+    const double bn = sqrt(reduce_partials(PB, nparts, sh));
+    if (mode == 1) {
+        const double a = fabs(alpha[j_prev]);
+        const double prev = amax_buf[j_prev & 1];
+        const double amax = a > prev ? a : prev;
+        const bool brk = !(bn > tol * amax);
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            beta[j_prev] = bn;
+            amax_buf[(j_prev + 1) & 1] = amax;
+            done[1] = j_prev + 1;
+            if (brk) done[0] = 1;
+        }
+        if (brk) return;
+    }
+    if (!out) return;
+    const Chunk c = my_chunk(n);
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) out[i] = in[i] / bn;
+}
+
+// w -= beta_j v_{j-1} (j > 0);  PA[cta] = partial of v_j . w
+__global__ void __launch_bounds__(kReduceThreads)
+alpha_partial_kernel(int64_t n, double* __restrict__ w, const double* __restrict__ vprev,
+                     const double* __restrict__ v, const double* __restrict__ beta, int j,
+                     double* __restrict__ PA, const int* __restrict__ done)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
     if (done[0]) return;
     const Chunk c = my_chunk(n);
-    const double beta = scal[0];
+    const double bj = j > 0 ? beta[j - 1] : 0.0;
     double s = 0.0;
     for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
         double wi = w[i];
-        if (vprev) {
-            wi -= beta * vprev[i];
+        if (j > 0) {
+            wi -= bj * vprev[i];
             w[i] = wi;
         }
         s = fma(v[i], wi, s);
     }
     s = block_sum(s, sh);
-    if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * stride] = s;
+    if (threadIdx.x == 0) PA[blockIdx.x] = s;
 }
 
-// w -= alpha * v;  optional partial of w . w
+// alpha_j = sum PA (CTA 0 records it);  w -= alpha_j v_j;  optional PB[cta] = partial of w . w
 __global__ void __launch_bounds__(kReduceThreads)
-axpy_norm_kernel(int64_t n, double* __restrict__ w, const double* __restrict__ v,
-                 const double* __restrict__ scal, double* __restrict__ partial, int stride,
-                 int want_norm, const int* __restrict__ done)
+axpy_norm_kernel(int64_t n, double* __restrict__ w, const double* __restrict__ v, const double* __restrict__ PA,
+                 int nparts, int j, double* __restrict__ alpha, double* __restrict__ PB, int want_norm,
+                 const int* __restrict__ done)
 {
     __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
     if (done[0]) return;
+    const double a = reduce_partials(PA, nparts, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) alpha[j] = a;
     const Chunk c = my_chunk(n);
-    const double alpha = scal[3];
     double s = 0.0;
     for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
-        const double wi = w[i] - alpha * v[i];
+        const double wi = w[i] - a * v[i];
         w[i] = wi;
         s = fma(wi, wi, s);
     }
     if (want_norm) {
+        __syncthreads();
         s = block_sum(s, sh);
-        if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * stride] = s;
+        if (threadIdx.x == 0) PB[blockIdx.x] = s;
     }
 }
 
@@ -125,6 +177,8 @@ multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const d
                         double* __restrict__ partial, int stride, const int* __restrict__ done)
 {
     __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
     if (done[0]) return;
     const Chunk c = my_chunk(n);
     for (int q0 = 0; q0 < nv; q0 += 4) {
@@ -148,10 +202,12 @@ multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const d
 // w[i] -= c_0 V_0[i]; w[i] -= c_1 V_1[i]; ... in that order; optional partial of w . w
 __global__ void __launch_bounds__(kReduceThreads)
 multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w,
-                 const double* __restrict__ coef, double* __restrict__ partial, int stride, int want_norm,
+                 const double* __restrict__ coef, double* __restrict__ PB, int want_norm,
                  const int* __restrict__ done)
 {
     __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
     if (done[0]) return;
     const Chunk c = my_chunk(n);
     double s = 0.0;
@@ -163,7 +219,7 @@ multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __rest
     }
     if (want_norm) {
         s = block_sum(s, sh);
-        if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * stride] = s;
+        if (threadIdx.x == 0) PB[blockIdx.x] = s;
     }
 }
 
@@ -172,55 +228,14 @@ __global__ void __launch_bounds__(256)
 finalize_multi_kernel(int nparts, int nv, const double* __restrict__ partial, int stride,
                       double* __restrict__ out, const int* __restrict__ done)
 {
+    pdl_trigger();
+    pdl_wait();
     if (done[0]) return;
     for (int q = threadIdx.x; q < nv; q += blockDim.x) {
         double s = 0.0;
         for (int p = 0; p < nparts; ++p) s += partial[(int64_t)p * stride + q];
         out[q] = s;
     }
-}
-
-// one CTA reduces `nparts` partials (slot 0) and applies the scalar step `what`:
-//   0: scal[2] = sqrt(sum)                       (||v0||)
-//   1: alpha[j] = scal[3] = sum
-//   2: beta[j] = scal[0] = sqrt(sum); amax; m_eff = j+1; breakdown flag
-__global__ void __launch_bounds__(256)
-finalize_scalar_kernel(int nparts, const double* __restrict__ partial, int stride, int what, int j,
-                       double tol, double* __restrict__ scal, double* __restrict__ alpha,
-                       double* __restrict__ beta, int* __restrict__ done)
-{
-    __shared__ double sh[8];
-    if (done[0]) return;
-    double s = 0.0;
-    for (int p = threadIdx.x; p < nparts; p += blockDim.x) s += partial[(int64_t)p * stride];
-    s = block_sum(s, sh);
-    if (threadIdx.x != 0) return;
-    if (what == 0) {
-        scal[2] = sqrt(s);
-    } else if (what == 1) {
-        alpha[j] = s;
-        scal[3] = s;
-    } else {
-        const double bn = sqrt(s);
-        beta[j] = bn;
-        scal[0] = bn;
-        const double a = fabs(scal[3]);
-        const double amax = a > scal[1] ? a : scal[1];
-        scal[1] = amax;
-        done[1] = j + 1;
-        if (!(bn > tol * amax)) done[0] = 1;
-    }
-}
-
-// out[i] = in[i] / scal[slot]
-__global__ void __launch_bounds__(256)
-scale_div_kernel(int64_t n, const double* __restrict__ in, double* __restrict__ out,
-                 const double* __restrict__ scal, int slot, const int* __restrict__ done)
-{
-    if (done[0]) return;
-    const double d = scal[slot];
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        out[i] = in[i] / d;
 }
 
 int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v)
@@ -253,7 +268,7 @@ static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec)
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = A((void**)&z.V, vb * nvec);
     if (e == cudaSuccess) e = A((void**)&z.w, vb);
-    if (e == cudaSuccess) e = A((void**)&z.partial, sizeof(double) * kMaxPartials * (size_t)(iters + 1));
+    if (e == cudaSuccess) e = A((void**)&z.partial, sizeof(double) * kMaxPartials * (size_t)(iters + 3));
     if (e == cudaSuccess) e = A((void**)&z.coef, sizeof(double) * (size_t)(iters + 1));
     if (e == cudaSuccess) e = A((void**)&z.alpha, sizeof(double) * (size_t)iters);
     if (e == cudaSuccess) e = A((void**)&z.beta, sizeof(double) * (size_t)iters);
@@ -340,7 +355,6 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     cudaStream_t st = h->stream;
     const int stride = m + 1;
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
-    const unsigned EG = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
 
     BJ_CUDA(cudaMemsetAsync(z.scal, 0, sizeof(double) * 8, st));
     BJ_CUDA(cudaMemsetAsync(z.done, 0, sizeof(int) * 4, st));
@@ -348,6 +362,18 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     BJ_CUDA(cudaMemsetAsync(z.beta, 0, sizeof(double) * m, st));
 
     auto vcol = [&](int j) { return z.V + (size_t)(reorth ? j : (j & 1)) * (size_t)n; };
+    double* PA = z.partial;                 // per-CTA partials of v_j . w
+    double* PB = z.partial + kMaxPartials;  // per-CTA partials of w . w
+    double* PM = z.partial + 2 * kMaxPartials;  // reorthogonalisation partials, G x stride
+    double* amax_buf = z.scal;              // two slots, ping-pong
+    const bool pdl = h->pdl;
+    cudaError_t e = cudaSuccess;
+#define BJ_LAUNCH(kernel, grid, block, ...)                                          \
+    do {                                                                             \
+        e = launch_kernel(kernel, dim3(grid), dim3(block), 0, st, pdl, __VA_ARGS__); \
+        if (e != cudaSuccess) { set_cuda_error(e, #kernel); return BJ_ERR_CUDA; }    \
+        h->launches++;                                                               \
+    } while (0)
 
     // v_1 = v0 / ||v0||
     const double* v0 = o->v0;
@@ -356,38 +382,33 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         if (rc != BJ_OK) return rc;
         v0 = z.w;
     }
-    dot_partial_kernel<<<G, kReduceThreads, 0, st>>>(n, v0, v0, z.partial, stride, nullptr);
-    finalize_scalar_kernel<<<1, 256, 0, st>>>(G, z.partial, stride, 0, 0, tol, z.scal, z.alpha, z.beta, z.done);
-    scale_div_kernel<<<EG, 256, 0, st>>>(n, v0, vcol(0), z.scal, 2, z.done);
-    h->launches += 3;
-    BJ_CUDA(cudaGetLastError());
+    BJ_LAUNCH(dot_partial_kernel, G, kReduceThreads, n, v0, v0, PB);
+    BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, v0, vcol(0), (const double*)PB, G, 0, 0, tol,
+              (const double*)z.alpha, z.beta, amax_buf, z.done);
 
     for (int j = 0; j < m; ++j) {
         double* vj = vcol(j);
-        rc = op_apply_device(h, vj, z.w);
+        rc = op_apply_device(h, vj, z.w);  // w = A^ v_j
         if (rc != BJ_OK) return rc;
-        alpha_partial_kernel<<<G, kReduceThreads, 0, st>>>(n, z.w, j > 0 ? vcol(j - 1) : nullptr, vj, z.scal,
-                                                           z.partial, stride, z.done);
-        finalize_scalar_kernel<<<1, 256, 0, st>>>(G, z.partial, stride, 1, j, tol, z.scal, z.alpha, z.beta, z.done);
-        axpy_norm_kernel<<<G, kReduceThreads, 0, st>>>(n, z.w, vj, z.scal, z.partial, stride, reorth ? 0 : 1, z.done);
-        h->launches += 3;
+        BJ_LAUNCH(alpha_partial_kernel, G, kReduceThreads, n, z.w, (const double*)(j > 0 ? vcol(j - 1) : vj),
+                  (const double*)vj, (const double*)z.beta, j, PA, (const int*)z.done);
+        BJ_LAUNCH(axpy_norm_kernel, G, kReduceThreads, n, z.w, (const double*)vj, (const double*)PA, G, j, z.alpha,
+                  PB, reorth ? 0 : 1, (const int*)z.done);
         if (reorth) {
             for (int pass = 0; pass < 2; ++pass) {
-                multidot_partial_kernel<<<G, kReduceThreads, 0, st>>>(n, j + 1, z.V, z.w, z.partial, stride, z.done);
-                finalize_multi_kernel<<<1, 256, 0, st>>>(G, j + 1, z.partial, stride, z.coef, z.done);
-                multiaxpy_kernel<<<G, kReduceThreads, 0, st>>>(n, j + 1, z.V, z.w, z.coef, z.partial, stride,
-                                                               pass == 1 ? 1 : 0, z.done);
-                h->launches += 3;
+                BJ_LAUNCH(multidot_partial_kernel, G, kReduceThreads, n, j + 1, (const double*)z.V,
+                          (const double*)z.w, PM, stride, (const int*)z.done);
+                BJ_LAUNCH(finalize_multi_kernel, 1, 256, G, j + 1, (const double*)PM, stride, z.coef,
+                          (const int*)z.done);
+                BJ_LAUNCH(multiaxpy_kernel, G, kReduceThreads, n, j + 1, (const double*)z.V, z.w,
+                          (const double*)z.coef, PB, pass == 1 ? 1 : 0, (const int*)z.done);
             }
         }
-        finalize_scalar_kernel<<<1, 256, 0, st>>>(G, z.partial, stride, 2, j, tol, z.scal, z.alpha, z.beta, z.done);
-        h->launches += 1;
-        if (j + 1 < m) {
-            scale_div_kernel<<<EG, 256, 0, st>>>(n, z.w, vcol(j + 1), z.scal, 0, z.done);
-            h->launches += 1;
-        }
-        BJ_CUDA(cudaGetLastError());
+        // beta_{j+2} = ||w||, bookkeeping, and v_{j+2} = w / beta (not needed after the last step)
+        BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, (const double*)z.w, j + 1 < m ? vcol(j + 1) : (double*)nullptr,
+                  (const double*)PB, G, 1, j, tol, (const double*)z.alpha, z.beta, amax_buf, z.done);
     }
+#undef BJ_LAUNCH
 
     std::vector<double> a(m), b(m);
     int done[4] = {0, 0, 0, 0};
