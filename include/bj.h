@@ -113,6 +113,10 @@ int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out);
  * torch.cuda.current_stream().cuda_stream) and keeps it as the handle's stream. */
 int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_t* out);
 
+/* Handle memory comes from a private stream-ordered pool that keeps freed slabs cached for the next
+ * bj_setup (block-size sweeps); this returns the cache to the driver.  Synchronises the device. */
+int bj_release_cached_memory(void);
+
 int bj_set_stream(bj_handle_t h, void* cuda_stream);
 int bj_set_option(bj_handle_t h, int option, int value);
 int bj_destroy(bj_handle_t h);

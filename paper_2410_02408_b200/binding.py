@@ -22,7 +22,7 @@ KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
 EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
-           "bj_profile_get"]
+           "bj_profile_get", "bj_release_cached_memory"]
 
 
 class bj_csr_t(C.Structure):
@@ -79,6 +79,7 @@ def lib():
         L.bj_cond_estimate.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.bj_cond_estimate_ex.argtypes = [vp, C.POINTER(bj_lanczos_opts_t), C.POINTER(bj_lanczos_result_t)]
         L.bj_seeded_vector.argtypes = [vp, C.c_uint64, vp]
+        L.bj_release_cached_memory.argtypes = []
         L.bj_profile_enable.argtypes = [vp, i32]
         L.bj_profile_get.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
         for f in EXPORTS:
@@ -233,6 +234,10 @@ def bj_seeded_vector(h, seed: int, v=None):
         v = torch.empty(h.n, dtype=torch.float64, device="cuda")
     _check(lib().bj_seeded_vector(h.ptr, seed & 0xFFFFFFFFFFFFFFFF, _dptr(v, torch.float64, h.n)))
     return v
+
+
+def bj_release_cached_memory():
+    _check(lib().bj_release_cached_memory())
 
 
 def bj_profile_enable(h, on: bool):

@@ -77,12 +77,56 @@ int op_apply_device(bj_handle_s* h, const double* x, double* y)
     return launch_solve(h, 0, h->u, y);  // y = L^-1 u
 }
 
+// Device memory for a handle comes from a private stream-ordered pool (cudaMallocFromPoolAsync) whose
+// release threshold keeps freed slabs cached: repeated setups (block-size sweeps) then cost microseconds
+// instead of a cudaMalloc each.  bj_release_cached_memory() returns the cache to the driver.
+// BJ_POOL=0 selects plain cudaMalloc.
+static cudaMemPool_t g_pool[64] = {};
+static bool g_pool_tried[64] = {};
+
+static cudaMemPool_t get_pool(int dev)
+{
+    if (dev < 0 || dev >= 64 || env_int("BJ_POOL", 1) == 0) return nullptr;
+    if (!g_pool_tried[dev]) {
+        g_pool_tried[dev] = true;
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) == cudaSuccess) {
+            uint64_t keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            g_pool[dev] = pool;
+        } else {
+            cudaGetLastError();
+        }
+    }
+    return g_pool[dev];
+}
+
+static void* slab_alloc(size_t bytes, int dev, cudaStream_t stream, bool* pooled)
+{
+    void* p = nullptr;
+    *pooled = false;
+    if (cudaMemPool_t pool = get_pool(dev)) {
+        if (cudaMallocFromPoolAsync(&p, bytes, pool, stream) == cudaSuccess) { *pooled = true; return p; }
+        cudaGetLastError();
+    }
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+
 static void free_handle(bj_handle_s* h)
 {
     if (!h) return;
     lanczos_free(h);
-    cudaFree(h->fac_small); cudaFree(h->fac_fwd); cudaFree(h->fac_bwd);
-    cudaFree(h->t); cudaFree(h->u); cudaFree(h->status);
+    if (h->slab) {
+        if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
+        else cudaFree(h->slab);
+    }
     cudaFree(h->stage_in); cudaFree(h->stage_out);
     for (auto& s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
     for (auto e : h->event_pool) cudaEventDestroy(e);
@@ -139,24 +183,41 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     h->pdl = env_int("BJ_PDL", 1) != 0;
 
     auto fail = [&](int code) { free_handle(h); return code; };
-    auto dmalloc = [&](void** p, size_t sz, int64_t* acct) {
-        cudaError_t e = cudaMalloc(p, sz ? sz : 8);
-        if (e != cudaSuccess) { cudaGetLastError(); return false; }
-        *acct += (int64_t)sz;
-        return true;
-    };
 
-    const size_t vb = (size_t)h->n * sizeof(double);
-    if (!dmalloc((void**)&h->t, vb, &h->workspace_bytes) || !dmalloc((void**)&h->u, vb, &h->workspace_bytes) ||
-        !dmalloc((void**)&h->status, sizeof(Status), &h->workspace_bytes))
-        return fail(BJ_ERR_ALLOC);
+    // one slab holds t, u, the status words and the factors (one allocation instead of five)
+    auto up256 = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t vb = up256((size_t)h->n * sizeof(double));
+    size_t fac_a = 0, fac_b = 0;
+    if (b > 0 && b <= kSmallMax) {
+        h->solve_kind = 1;
+        const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;
+        fac_a = (size_t)groups * h->packed * kInterleave * sizeof(double);
+    } else if (b > 0) {
+        h->solve_kind = 2;
+        h->lanes = b <= 16 ? 16 : 32;
+        fac_a = fac_b = (size_t)h->nblocks * h->packed * sizeof(double) + 16;  // 16 B slack: bulk copies round up
+    }
+    const size_t total = 2 * vb + 256 + up256(fac_a) + up256(fac_b);
+    h->slab = slab_alloc(total, dev, h->stream, &h->slab_pooled);
+    if (!h->slab) return fail(BJ_ERR_ALLOC);
+    {
+        char* base = (char*)h->slab;
+        h->t = (double*)base;
+        h->u = (double*)(base + vb);
+        h->status = (Status*)(base + 2 * vb);
+        char* f = base + 2 * vb + 256;
+        if (h->solve_kind == 1) h->fac_small = (double*)f;
+        if (h->solve_kind == 2) { h->fac_fwd = (double*)f; h->fac_bwd = (double*)(f + up256(fac_a)); }
+        h->workspace_bytes = (int64_t)(2 * vb + 256);
+        h->factor_bytes = (int64_t)(fac_a + fac_b);
+    }
     Status init;
     memset(&init, 0, sizeof(init));
     init.bad_block = 0x7fffffffffffffffll;
     cudaError_t ce = cudaMemcpyAsync(h->status, &init, sizeof(init), cudaMemcpyHostToDevice, h->stream);
     if (ce != cudaSuccess) { set_cuda_error(ce, "status init"); return fail(BJ_ERR_CUDA); }
 
-    // a1 validate (also longest row)
+    // a1 validate (also longest row and the column-coherence statistic)
     int rc = launch_validate(h);
     if (rc != BJ_OK) return fail(rc);
     Status stt;
@@ -164,10 +225,11 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
     if (ce != cudaSuccess) { set_cuda_error(ce, "validate"); return fail(BJ_ERR_CUDA); }
     if (stt.flags & (ST_BAD_ROWPTR | ST_BAD_COL | ST_UNSORTED)) return fail(BJ_ERR_NOT_CANONICAL);
+    if (stt.descents != stt.legal_descents) return fail(BJ_ERR_NOT_CANONICAL);  // a descent inside a row
 
     h->coherence = stt.compared ? (double)stt.coherent / (double)stt.compared : 1.0;
 
-    // lanes per row for the SpMV kernels: power of two near the mean row length
+    // lanes per row for the CSR-vector kernel: power of two near the mean row length
     {
         const double mean = (double)h->nnz / (double)h->n;
         int l = 1;
@@ -175,35 +237,29 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         h->spmv_lanes = l;
     }
 
-    // a2-a4 extract + factor
+    // a2-a4 extract + factor; only the padding the kernels do not write needs zeroing
+    if (h->solve_kind == 1) {
+        const size_t group_bytes = (size_t)h->packed * kInterleave * sizeof(double);
+        if (h->nblocks % kInterleave) ce = cudaMemsetAsync((char*)h->fac_small + fac_a - group_bytes, 0, group_bytes, h->stream);
+    } else if (h->solve_kind == 2) {
+        ce = cudaMemsetAsync((char*)h->fac_fwd + fac_a - 16, 0, 16, h->stream);
+        if (ce == cudaSuccess) ce = cudaMemsetAsync((char*)h->fac_bwd + fac_b - 16, 0, 16, h->stream);
+    }
+    if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
     if (b > 0) {
-        if (b <= kSmallMax) {
-            h->solve_kind = 1;
-            const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;
-            const size_t sz = (size_t)groups * h->packed * kInterleave * sizeof(double);
-            if (!dmalloc((void**)&h->fac_small, sz, &h->factor_bytes)) return fail(BJ_ERR_ALLOC);
-            ce = cudaMemsetAsync(h->fac_small, 0, sz, h->stream);
-        } else {
-            h->solve_kind = 2;
-            h->lanes = b <= 16 ? 16 : 32;
-            const size_t sz = (size_t)h->nblocks * h->packed * sizeof(double) + 16;  // 16 B slack: bulk copies round up
-            if (!dmalloc((void**)&h->fac_fwd, sz, &h->factor_bytes) || !dmalloc((void**)&h->fac_bwd, sz, &h->factor_bytes))
-                return fail(BJ_ERR_ALLOC);
-            ce = cudaMemsetAsync(h->fac_fwd, 0, sz, h->stream);
-            if (ce == cudaSuccess) ce = cudaMemsetAsync(h->fac_bwd, 0, sz, h->stream);
-        }
-        if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
         rc = launch_extract_factor(h);
         if (rc != BJ_OK) return fail(rc);
     }
 
-    // SpMV plan for the streamed kernel
+    // SpMV plan for the streamed kernel: tile rows now, stage capacity once the fullest tile is known
     rc = spmv_stream_configure(h);
     if (rc != BJ_OK) return fail(rc);
 
     ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
     if (ce != cudaSuccess) { set_cuda_error(ce, "setup"); return fail(BJ_ERR_CUDA); }
+    rc = spmv_stream_finish(h, stt.max_tile_nnz);
+    if (rc != BJ_OK) return fail(rc);
     choose_spmv(h);
     *out = h;
     if (stt.flags & ST_NOT_SPD) {
@@ -215,6 +271,17 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
 }
 
 int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out) { return bj_setup_on_stream(csr, b, nullptr, out); }
+
+int bj_release_cached_memory(void)
+{
+    int dev = 0;
+    BJ_CUDA(cudaGetDevice(&dev));
+    if (dev >= 0 && dev < 64 && g_pool[dev]) {
+        BJ_CUDA(cudaDeviceSynchronize());
+        BJ_CUDA(cudaMemPoolTrimTo(g_pool[dev], 0));
+    }
+    return BJ_OK;
+}
 
 int bj_set_stream(bj_handle_t h, void* cuda_stream)
 {

@@ -27,6 +27,8 @@ struct Status {
     int max_row_nnz;
     unsigned long long coherent;  // entries whose column is within 16 of the same-position column of the next row
     unsigned long long compared;  // entries compared
+    unsigned long long descents;        // entries with col[p] <= col[p-1]
+    unsigned long long legal_descents;  // ... of which at the start of a non-empty row
 };
 
 struct ProfSpan {
@@ -72,6 +74,8 @@ struct bj_handle_s {
     int64_t factor_bytes = 0;
 
     // temporaries
+    void* slab = nullptr;     // one allocation holds t, u, status and the factors
+    bool slab_pooled = false;
     double* t = nullptr;
     double* u = nullptr;
     bj::Status* status = nullptr;  // device
@@ -143,7 +147,8 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out);
 // SpMV (bj_spmv_kernels.cu)
 int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);
 int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward);
-int spmv_stream_configure(bj_handle_s* h);  // decide tile geometry, set stream_ok / fuse_ok
+int spmv_stream_configure(bj_handle_s* h);  // decide tile rows / fusion, launch tile_nnz_kernel (async)
+int spmv_stream_finish(bj_handle_s* h, int max_tile);  // stage capacity and count, sets stream_ok
 
 // Lanczos (bj_lanczos.cu)
 int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* r);

@@ -3,37 +3,45 @@
 // in split form).  One warp owns one block: the block's CSR range is contiguous, so the warp
 // streams its column indices with coalesced loads, drops in-block entries into a dense tile in
 // shared memory, factors it there and writes the layouts the solve kernels want.
+#include <algorithm>
+
 #include "bj_internal.cuh"
 
 namespace bj {
 
 // ------------------------------------------------------------------------------------------------
-// a1: one thread per row.  Also records the longest row (for the SpMV plan).
+// a1, two coalesced passes, no per-entry search and almost no atomics.
+//   entries pass : grid-stride over the entries -- 0 <= col < n; counts the DESCENTS col[p] <= col[p-1].
+//   rows pass    : one thread per row -- row_ptr monotone, starts at 0, ends at nnz; longest row; counts the
+//                  descents that sit at the start of a non-empty row (the only legal ones).
+//   Columns are strictly increasing inside every row  <=>  both counts agree (checked on the host).
+//   Every 8th CTA of the rows pass also gathers the column-coherence statistic that steers the SpMV shape.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-validate_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
-                Status* st)
+validate_rows_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
+                     Status* st)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    int flags = 0;
-    int len = 0;
-    unsigned coh = 0, cmp = 0;
+    __shared__ unsigned sh[3][8];
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int flags = 0, len = 0;
+    unsigned coh = 0, cmp = 0, legal = 0;
     if (i < n) {
-        int64_t s = rp[i], e = rp[i + 1];
+        const int64_t s = rp[i], e = rp[i + 1];
         if (s > e || s < 0 || e > nnz || (i == 0 && s != 0) || (i == n - 1 && e != nnz)) {
             flags |= ST_BAD_ROWPTR;
         } else {
             len = (int)(e - s);
-            // next row, only if its pointers are sane (it validates itself): used for the coherence statistic
-            int64_t s2 = 0, e2 = 0;
-            if (i + 1 < n) { s2 = e; e2 = rp[i + 2]; if (e2 < s2 || e2 > nnz) e2 = s2; }
-            int prev = -1;
-            for (int64_t p = s; p < e; ++p) {
-                int c = ci[p];
-                if (c < 0 || c >= n) flags |= ST_BAD_COL;
-                if (c <= prev) flags |= ST_UNSORTED;
-                prev = c;
-                if (s2 + (p - s) < e2) { ++cmp; const int d = ci[s2 + (p - s)] - c; coh += (d >= -16 && d <= 16); }
+            if (len > 0 && s > 0) legal = ci[s] <= ci[s - 1];
+            if ((blockIdx.x & 7) == 0 && i + 1 < n) {
+                const int64_t e2 = rp[i + 2];
+                if (e2 >= e && e2 <= nnz) {
+                    const int64_t m = (e2 - e) < (e - s) ? (e2 - e) : (e - s);
+                    for (int64_t q = 0; q < m; ++q) {
+                        const int d = ci[e + q] - ci[s + q];
+                        ++cmp;
+                        coh += (d >= -16 && d <= 16);
+                    }
+                }
             }
         }
     }
@@ -41,19 +49,58 @@ validate_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ rp, const in
     len = __reduce_max_sync(0xffffffffu, len);
     coh = __reduce_add_sync(0xffffffffu, coh);
     cmp = __reduce_add_sync(0xffffffffu, cmp);
+    legal = __reduce_add_sync(0xffffffffu, legal);
+    const int warp = threadIdx.x >> 5;
     if ((threadIdx.x & 31) == 0) {
         if (flags) atomicOr(&st->flags, flags);
-        atomicMax(&st->max_row_nnz, len);
-        atomicAdd(&st->coherent, (unsigned long long)coh);
-        atomicAdd(&st->compared, (unsigned long long)cmp);
+        if (len > *(volatile int*)&st->max_row_nnz) atomicMax(&st->max_row_nnz, len);
+        sh[0][warp] = coh; sh[1][warp] = cmp; sh[2][warp] = legal;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned a = 0, c = 0, l = 0;
+        for (int w = 0; w < 8; ++w) { a += sh[0][w]; c += sh[1][w]; l += sh[2][w]; }
+        if (c) { atomicAdd(&st->coherent, (unsigned long long)a); atomicAdd(&st->compared, (unsigned long long)c); }
+        if (l) atomicAdd(&st->legal_descents, (unsigned long long)l);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+validate_entries_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ ci, Status* st)
+{
+    __shared__ unsigned sh[8];
+    int flags = 0;
+    unsigned desc = 0;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < nnz; p += (int64_t)gridDim.x * blockDim.x) {
+        const int c = ci[p];
+        if (c < 0 || c >= n) flags |= ST_BAD_COL;
+        if (p > 0) desc += (c <= ci[p - 1]);
+    }
+    flags = __reduce_or_sync(0xffffffffu, flags);
+    desc = __reduce_add_sync(0xffffffffu, desc);
+    if ((threadIdx.x & 31) == 0) {
+        if (flags) atomicOr(&st->flags, flags);
+        sh[threadIdx.x >> 5] = desc;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned d = 0;
+        for (int w = 0; w < 8; ++w) d += sh[w];
+        if (d) atomicAdd(&st->descents, (unsigned long long)d);
     }
 }
 
 int launch_validate(bj_handle_s* h)
 {
-    int64_t blocks = (h->n + 255) / 256;
-    validate_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->n, h->nnz, h->row_ptr, h->col_idx, h->status);
+    const int64_t blocks = (h->n + 255) / 256;
+    validate_rows_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->n, h->nnz, h->row_ptr, h->col_idx, h->status);
     h->launches++;
+    if (h->nnz > 0) {
+        const int64_t want = (h->nnz + 256 * 8 - 1) / (256 * 8);
+        const unsigned eb = (unsigned)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * 32));
+        validate_entries_kernel<<<eb, 256, 0, h->stream>>>(h->n, h->nnz, h->col_idx, h->status);
+        h->launches++;
+    }
     BJ_CUDA(cudaGetLastError());
     return BJ_OK;
 }
@@ -170,15 +217,212 @@ extract_factor_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restri
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// a2 + a3 for b <= 8: one THREAD per diagonal block, the block in registers (compile-time B).
+// A warp covers 32 consecutive blocks = 32 B consecutive rows, so its CSR reads stay inside one
+// contiguous range (L1 absorbs the per-thread strides) and its interleaved factor writes are whole
+// 256-byte lines.  Same left-looking Cholesky order as above.
+// ------------------------------------------------------------------------------------------------
+template <int B>
+__global__ void __launch_bounds__(128)
+extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restrict__ rp,
+                            const int32_t* __restrict__ ci, const double* __restrict__ val,
+                            double* __restrict__ fac, Status* st)
+{
+    constexpr int P = B * (B + 1) / 2;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nblocks) return;
+    const int64_t lo = k * B;
+    double d[P];  // packed lower triangle, e = i(i+1)/2 + j
+#pragma unroll
+    for (int e = 0; e < P; ++e) d[e] = 0.0;
+#pragma unroll
+    for (int i = 0; i < B; ++i) {
+        const int64_t row = lo + i;
+        if (row < n) {
+            int s = rp[row];
+            const int e_ = rp[row + 1];
+            if (e_ - s > 16) {                 // long row: binary search for the first column >= lo
+                int hi = e_;
+                while (s < hi) {
+                    const int mid = (s + hi) >> 1;
+                    if (ci[mid] < lo) s = mid + 1; else hi = mid;
+                }
+            }
+            for (int p = s; p < e_; ++p) {
+                const int64_t c = ci[p];
+                if (c > row) break;            // columns ascend: nothing of the lower triangle is left
+                if (c >= lo) {
+                    const double v = val[p];
+                    const int j = (int)(c - lo);
+#pragma unroll
+                    for (int jj = 0; jj <= i; ++jj)
+                        if (jj == j) d[i * (i + 1) / 2 + jj] = v;
+                }
+            }
+        } else {
+            d[i * (i + 1) / 2 + i] = 1.0;      // identity rows pad a ragged last block
+        }
+    }
+    bool bad = false;
+#pragma unroll
+    for (int j = 0; j < B; ++j) {
+        double sjj = d[j * (j + 1) / 2 + j];
+#pragma unroll
+        for (int p = 0; p < j; ++p) sjj -= d[j * (j + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
+        if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
+        const double ljj = sqrt(sjj);
+        d[j * (j + 1) / 2 + j] = ljj;
+#pragma unroll
+        for (int i = j + 1; i < B; ++i) {
+            double t = d[i * (i + 1) / 2 + j];
+#pragma unroll
+            for (int p = 0; p < j; ++p) t -= d[i * (i + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
+            d[i * (i + 1) / 2 + j] = t / ljj;
+        }
+    }
+    if (bad) {
+        atomicOr(&st->flags, ST_NOT_SPD);
+        atomicMin(&st->bad_block, (long long)k);
+    }
+    double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
+#pragma unroll
+    for (int i = 0; i < B; ++i)
+#pragma unroll
+        for (int j = 0; j <= i; ++j) {
+            const double v = d[i * (i + 1) / 2 + j];
+            f[(i * (i + 1) / 2 + j) * kInterleave] = (i == j) ? 1.0 / v : v;
+        }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2 + a3 for b > 8: one SUB-WARP of W lanes per diagonal block, lane i owns row i IN REGISTERS.
+//   extraction : each lane binary-searches its (sorted) row for the first column >= kb and copies the
+//                entries up to the diagonal into its row of a small shared-memory tile;
+//   Cholesky   : right-looking in registers -- column j: l_jj = sqrt(a_jj) (broadcast from lane j),
+//                l_ij = a_ij / l_jj, then a_ik -= l_ij l_kj for k in (j, i] with l_kj fetched by shuffle.
+//                Updates hit a_ik in the order j = 0, 1, ..: the same subtraction order as the oracle's
+//                left-looking sum.  No shared memory, no barriers inside the factorisation.
+//   output     : both scaled packed copies, written with consecutive lanes on consecutive addresses.
+// ------------------------------------------------------------------------------------------------
+template <int W>
+__global__ void __launch_bounds__(128)
+extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restrict__ rp,
+                              const int32_t* __restrict__ ci, const double* __restrict__ val,
+                              double* __restrict__ out0, double* __restrict__ out1, Status* st)
+{
+    extern __shared__ double smem[];
+    constexpr int LD = W + 1;
+    const int nsub = blockDim.x / W;
+    const int sub = threadIdx.x / W;
+    const int i = threadIdx.x & (W - 1);
+    double* D = smem + (size_t)sub * (W * LD);
+    int64_t k = (int64_t)blockIdx.x * nsub + sub;
+    const bool act = k < nblocks;
+    if (!act) k = nblocks - 1;  // redundant work, nothing written: the shuffles below need every lane
+    const int64_t lo = k * b;
+    const int64_t row = lo + i;
+    const bool rowlive = i < b && row < n;
+
+#pragma unroll
+    for (int c = 0; c < W; ++c) D[i * LD + c] = 0.0;
+    if (!rowlive) D[i * LD + i] = 1.0;  // identity rows pad ragged blocks and idle lanes
+    if (rowlive) {
+        int s = rp[row];
+        const int e = rp[row + 1];
+        int hi = e;
+        while (s < hi) {  // first entry with column >= lo
+            const int mid = (s + hi) >> 1;
+            if (ci[mid] < lo) s = mid + 1; else hi = mid;
+        }
+        // entries up to the diagonal, eight loads in flight at a time
+        for (int p = s; p < e; p += 8) {
+            int cc[8];
+            double vv[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) cc[q] = (p + q < e) ? ci[p + q] : 0x7fffffff;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) vv[q] = (p + q < e && cc[q] <= row) ? val[p + q] : 0.0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+                if (cc[q] <= row) D[i * LD + (int)(cc[q] - lo)] = vv[q];
+            if (cc[7] > row) break;  // columns ascend: the lower triangle is done
+        }
+    }
+    __syncwarp();
+    double a[W];
+#pragma unroll
+    for (int c = 0; c < W; ++c) a[c] = D[i * LD + c];
+
+    bool bad = false;
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        if (j < b) {
+            double ajj = __shfl_sync(0xffffffffu, a[j], j, W);
+            if (!(ajj > 0.0) || isinf(ajj)) { bad = true; ajj = 1.0; }
+            const double ljj = sqrt(ajj);
+            const double lij = (i > j) ? a[j] / ljj : (i == j ? ljj : 0.0);
+            a[j] = lij;
+#pragma unroll
+            for (int k2 = j + 1; k2 < W; ++k2) {
+                if (k2 < b) {
+                    const double lkj = __shfl_sync(0xffffffffu, lij, k2, W);
+                    if (i >= k2) a[k2] = fma(-lij, lkj, a[k2]);
+                }
+            }
+        }
+    }
+    if (bad && act && i == 0) {
+        atomicOr(&st->flags, ST_NOT_SPD);
+        atomicMin(&st->bad_block, (long long)k);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int c = 0; c < W; ++c) D[i * LD + c] = a[c];
+    __syncwarp();
+    if (!act) return;
+    const int P = b * (b + 1) / 2;
+    const double inv = 1.0 / D[i * LD + i];  // one division per lane; the scalings below multiply by it
+    // forward copy: column-major packed, row i scaled by 1/l_ii
+    for (int j = 0; j < b; ++j)
+        if (i >= j && i < b) out0[k * P + (j * b - j * (j - 1) / 2) + (i - j)] = (i == j) ? inv : D[i * LD + j] * inv;
+    // backward copy: row-major packed, column i scaled by 1/l_ii
+    for (int r = 0; r < b; ++r)
+        if (i <= r) out1[k * P + r * (r + 1) / 2 + i] = (i == r) ? inv : D[r * LD + i] * inv;
+}
+
 int launch_extract_factor(bj_handle_s* h)
 {
     const int b = h->b;
     const int per_warp = b * (b + 1) + ((b + 2 + 1) / 2);
     const size_t smem = (size_t)kSetupWarps * per_warp * sizeof(double);
     const int64_t blocks = (h->nblocks + kSetupWarps - 1) / kSetupWarps;
-    if (h->solve_kind == 1) {
+    if (h->solve_kind == 1 && env_int("BJ_SETUP_WARP", 0) == 0) {
+        const unsigned tb = (unsigned)((h->nblocks + 127) / 128);
+#define BJ_CASE(B)                                                                                          \
+    case B:                                                                                                 \
+        extract_factor_small_kernel<B><<<tb, 128, 0, h->stream>>>(h->n, h->nblocks, h->row_ptr, h->col_idx,  \
+                                                                  h->val, h->fac_small, h->status);         \
+        break;
+        switch (b) {
+            BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
+            default: return BJ_ERR_INVALID_ARG;
+        }
+#undef BJ_CASE
+    } else if (h->solve_kind == 1) {
         extract_factor_kernel<1><<<(unsigned)blocks, kSetupWarps * 32, smem, h->stream>>>(
             h->n, b, h->nblocks, h->row_ptr, h->col_idx, h->val, h->fac_small, nullptr, h->status);
+    } else if (env_int("BJ_SETUP_WARP", 0) == 0) {
+        const int W = h->lanes;
+        const int nsub = 128 / W;
+        const size_t sm = (size_t)nsub * W * (W + 1) * sizeof(double);
+        const unsigned sb = (unsigned)((h->nblocks + nsub - 1) / nsub);
+        if (W == 16)
+            extract_factor_subwarp_kernel<16><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
+                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status);
+        else
+            extract_factor_subwarp_kernel<32><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
+                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status);
     } else {
         extract_factor_kernel<2><<<(unsigned)blocks, kSetupWarps * 32, smem, h->stream>>>(
             h->n, b, h->nblocks, h->row_ptr, h->col_idx, h->val, h->fac_fwd, h->fac_bwd, h->status);

@@ -372,8 +372,7 @@ constexpr size_t kSmemTwoPerSm = 110 * 1024;
 constexpr size_t kSmemOnePerSm = 224 * 1024;
 }  // namespace
 
-// Decide the tile geometry.  Called by bj_setup after validation (max_row_nnz known) and, a second
-// time, after tile_nnz_kernel has measured the fullest tile.
+// Decide the tile geometry (rows per tile, fusion) and launch the kernel that measures the fullest tile.
 int spmv_stream_configure(bj_handle_s* h)
 {
     h->stream_ok = false;
@@ -422,13 +421,15 @@ int spmv_stream_configure(bj_handle_s* h)
     h->tile_rows = R;
     h->ntiles = (h->n + R - 1) / R;
     h->fuse_ok = fuse;
-    // measure the fullest tile
-    BJ_CUDA(cudaMemsetAsync(&h->status->max_tile_nnz, 0, sizeof(int), h->stream));
-    int rc = launch_spmv_plan(h);
-    if (rc != BJ_OK) return rc;
-    int max_tile = 0;
-    BJ_CUDA(cudaMemcpyAsync(&max_tile, &h->status->max_tile_nnz, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    // measure the fullest tile (result is read back with the rest of the setup status)
+    return launch_spmv_plan(h);
+}
+
+// second half of the plan, once the fullest tile is known
+int spmv_stream_finish(bj_handle_s* h, int max_tile)
+{
+    if (h->ntiles <= 0) return BJ_OK;
+    const bool fuse = h->fuse_ok;
     h->tile_cap = ((max_tile + 8) + 3) & ~3;
     int stages = env_int("BJ_STAGES", 2);
     StreamParams sp;
