@@ -108,9 +108,10 @@ struct SolveStreamParams {
     double* out;
     int b, P, G, stages;
     int copy_doubles;    // doubles reserved per copy per stage (G * P rounded to even)
+    int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
 };
 
-template <int W, int DIR>
+template <int W, int DIR, int B>  // B: compile-time block size, 0 = runtime p.b
 __global__ void __launch_bounds__(32 + 256)
 solve_stream_kernel(const SolveStreamParams p)
 {
@@ -122,7 +123,7 @@ solve_stream_kernel(const SolveStreamParams p)
     const int stage_doubles = kCopies * p.copy_doubles;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    pdl_trigger();
+    if (p.early_trigger) pdl_trigger();
     if (threadIdx.x == 0) {
         for (int s = 0; s < p.stages; ++s) {
             mbar_init(&full[s], 1);
@@ -154,7 +155,7 @@ solve_stream_kernel(const SolveStreamParams p)
         const int nsub = (blockDim.x - 32) / W;
         const int sub = ctid / W;
         const int i = ctid & (W - 1);
-        const int b = p.b;
+        const int b = B > 0 ? B : p.b;
         pdl_wait();  // `in` may come from the previous kernel
         // right-hand sides are fetched one tile ahead: their HBM latency hides behind the current tile's solves
         auto fetch_rhs = [&](int64_t tile, double* dst) {
@@ -186,9 +187,9 @@ solve_stream_kernel(const SolveStreamParams p)
                 if (q * nsub < p.G) {  // uniform over the CTA
                     const int kc = kb < nb ? kb : 0;  // idle sub-warps read block 0 (valid memory), result dropped
                     double v = r[q];
-                    if (DIR == 0 || DIR == 2) v = subwarp_block_solve<W, 0>(f + (size_t)kc * p.P, b, i, v);
-                    if (DIR == 1) v = subwarp_block_solve<W, 1>(f + (size_t)kc * p.P, b, i, v);
-                    if (DIR == 2) v = subwarp_block_solve<W, 1>(f + p.copy_doubles + (size_t)kc * p.P, b, i, v);
+                    if (DIR == 0 || DIR == 2) v = subwarp_solve<W, 0, B>(f + (size_t)kc * p.P, b, i, v);
+                    if (DIR == 1) v = subwarp_solve<W, 1, B>(f + (size_t)kc * p.P, b, i, v);
+                    if (DIR == 2) v = subwarp_solve<W, 1, B>(f + p.copy_doubles + (size_t)kc * p.P, b, i, v);
                     const int64_t row = (k0 + kb) * b + i;
                     if (kb < nb && i < b && row < p.n) p.out[row] = v;
                 }
@@ -225,20 +226,20 @@ static int launch_small(bj_handle_s* h, const double* in, double* out)
     return BJ_OK;
 }
 
-template <int W, int DIR>
+template <int W, int DIR, int B>
 static int launch_stream_solve(bj_handle_s* h, const SolveStreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_stream_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR>, threads, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR, B>, threads, smem);
     const int per_sm = std::max(1, std::min(occ, want_per_sm));
     const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
-    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
+    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR, B>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
@@ -264,14 +265,21 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
     sp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
     sp.fac1 = h->fac_bwd;
     sp.in = in; sp.out = out;
+    sp.early_trigger = env_int("BJ_PDL_EARLY", 0) & 1;
     const size_t stage_bytes = (size_t)copies * sp.copy_doubles * 8;
     int stages = std::max(2, env_int("BJ_SOLVE_STAGES", 2));
     while (stages > 2 && 128 + stages * stage_bytes > 110 * 1024) --stages;
     sp.stages = stages;
     const size_t smem = 128 + stages * stage_bytes;
     const int per_sm = env_int("BJ_SOLVE_CTAS", 4);
-    return W == 16 ? launch_stream_solve<16, DIR>(h, sp, per_sm, threads, smem)
-                   : launch_stream_solve<32, DIR>(h, sp, per_sm, threads, smem);
+    switch (h->b) {  // compile-time instances for the workloads' block sizes
+        case 16: return launch_stream_solve<16, DIR, 16>(h, sp, per_sm, threads, smem);
+        case 24: return launch_stream_solve<32, DIR, 24>(h, sp, per_sm, threads, smem);
+        case 32: return launch_stream_solve<32, DIR, 32>(h, sp, per_sm, threads, smem);
+        default: break;
+    }
+    return W == 16 ? launch_stream_solve<16, DIR, 0>(h, sp, per_sm, threads, smem)
+                   : launch_stream_solve<32, DIR, 0>(h, sp, per_sm, threads, smem);
 }
 
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)

@@ -110,6 +110,7 @@ struct StreamParams {
     int stage_bytes;
     int su_doubles;      // doubles per su buffer
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
+    int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
 };
 
 __device__ __forceinline__ void consumer_bar_sync(int nthreads)
@@ -135,7 +136,7 @@ spmv_stream_kernel(const StreamParams p)
     auto s_rp = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 12 + p.fac_bytes); };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    pdl_trigger();
+    if (p.early_trigger) pdl_trigger();
     if (threadIdx.x == 0) {
         for (int s = 0; s < p.stages; ++s) {
             mbar_init(&full[s], 1);
@@ -249,7 +250,8 @@ spmv_stream_kernel(const StreamParams p)
                             c[k] = sc[qq < e ? qq : q];
                         }
 #pragma unroll
-                        for (int k = 0; k < BATCH; ++k) xv[k] = __ldg(p.x + c[k]);
+                        for (int k = 0; k < BATCH; ++k)  // predicated: a masked lane costs no L1 wavefront
+                            xv[k] = (q + k * LPR < e) ? __ldg(p.x + c[k]) : 0.0;
 #pragma unroll
                         for (int k = 0; k < BATCH; ++k) {
                             const int qq = q + k * LPR;
@@ -456,6 +458,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     fill_layout(h, fuse, sp, smem);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
+    sp.early_trigger = (env_int("BJ_PDL_EARLY", 0) >> 1) & 1;
     sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
     const int threads = 32 + 32 * h->stream_warps;
     const int grid = env_int("BJ_CTAS_PER_SM", 4);  // wanted CTAs per SM; clipped to the real occupancy at launch
