@@ -111,36 +111,40 @@ __device__ __forceinline__ double subwarp_block_solve(const double* f, int b, in
 }
 
 // Same solve with the block size known at compile time (B <= W): every factor address is the lane's base
-// plus an immediate, the step loop has no branches, and one step is LDS + 2 SHFL + DFMA.
-template <int W, int DIR, int B>
-__device__ __forceinline__ double subwarp_block_solve_ct(const double* f, int i, double r)
+// plus an immediate and the step loop has no branches.  NB independent blocks are solved together: their
+// dependent chains (SHFL -> DFMA per step) interleave, and the step's lane predicate is shared.
+template <int W, int DIR, int B, int NB>
+__device__ __forceinline__ void subwarp_block_solve_ct(const double* const (&f)[NB], int i, double (&r)[NB])
 {
     static_assert(B >= 2 && B <= W, "block size must fit the sub-warp");
     const bool in = i < B;
     const int dslot = DIR == 0 ? i * B - i * (i - 1) / 2 : i * (i + 1) / 2 + i;
-    r *= in ? f[dslot] : 0.0;
-    const double* fi = f + i;
+#pragma unroll
+    for (int q = 0; q < NB; ++q) r[q] *= in ? f[q][dslot] : 0.0;
 #pragma unroll
     for (int jj = 0; jj < B - 1; ++jj) {
         const int j = DIR == 0 ? jj : B - 1 - jj;
-        double lij = 0.0;
-        if (DIR == 0) {
-            if (i > j && in) lij = fi[j * B - j * (j - 1) / 2 - j];
-        } else {
-            if (i < j) lij = fi[j * (j + 1) / 2];
+        const bool on = DIR == 0 ? (i > j && in) : (i < j);
+        const int off = DIR == 0 ? j * B - j * (j - 1) / 2 - j : j * (j + 1) / 2;
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const double lij = on ? f[q][i + off] : 0.0;
+            const double vj = __shfl_sync(0xffffffffu, r[q], j, W);
+            r[q] = fma(-lij, vj, r[q]);
         }
-        const double vj = __shfl_sync(0xffffffffu, r, j, W);
-        r = fma(-lij, vj, r);
     }
-    return r;
 }
 
 // dispatch: compile-time instance for the block sizes of the paper-shaped workloads, runtime loop otherwise
-template <int W, int DIR, int B>
-__device__ __forceinline__ double subwarp_solve(const double* f, int b, int i, double r)
+template <int W, int DIR, int B, int NB>
+__device__ __forceinline__ void subwarp_solve(const double* const (&f)[NB], int b, int i, double (&r)[NB])
 {
-    if constexpr (B > 0) return subwarp_block_solve_ct<W, DIR, B>(f, i, r);
-    else return subwarp_block_solve<W, DIR>(f, b, i, r);
+    if constexpr (B > 0) {
+        subwarp_block_solve_ct<W, DIR, B, NB>(f, i, r);
+    } else {
+#pragma unroll
+        for (int q = 0; q < NB; ++q) r[q] = subwarp_block_solve<W, DIR>(f[q], b, i, r[q]);
+    }
 }
 
 // Programmatic dependent launch.  Every kernel of the library calls pdl_trigger() first (lets the

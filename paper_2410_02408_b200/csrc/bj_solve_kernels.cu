@@ -99,6 +99,9 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
 // decoupled from the b-step dependent chain of each block.
 // ------------------------------------------------------------------------------------------------
 constexpr int kMaxBlocksPerSub = 4;
+#ifndef BJ_SOLVE_MINB
+#define BJ_SOLVE_MINB 3  // registers capped so that three CTAs fit one SM
+#endif
 
 struct SolveStreamParams {
     int64_t n, nblocks, ntiles;
@@ -111,8 +114,8 @@ struct SolveStreamParams {
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
 };
 
-template <int W, int DIR, int B>  // B: compile-time block size, 0 = runtime p.b
-__global__ void __launch_bounds__(32 + 256)
+template <int W, int DIR, int B, int NB>  // B: compile-time block size, 0 = runtime p.b; NB: blocks a sub-warp solves together
+__global__ void __launch_bounds__(32 + 256, BJ_SOLVE_MINB)
 solve_stream_kernel(const SolveStreamParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -182,16 +185,28 @@ solve_stream_kernel(const SolveStreamParams p)
             mbar_wait(&full[s], ph);
             const double* f = stage0 + (size_t)s * stage_doubles;
 #pragma unroll
-            for (int q = 0; q < kMaxBlocksPerSub; ++q) {
-                const int kb = sub + q * nsub;
-                if (q * nsub < p.G) {  // uniform over the CTA
-                    const int kc = kb < nb ? kb : 0;  // idle sub-warps read block 0 (valid memory), result dropped
-                    double v = r[q];
-                    if (DIR == 0 || DIR == 2) v = subwarp_solve<W, 0, B>(f + (size_t)kc * p.P, b, i, v);
-                    if (DIR == 1) v = subwarp_solve<W, 1, B>(f + (size_t)kc * p.P, b, i, v);
-                    if (DIR == 2) v = subwarp_solve<W, 1, B>(f + p.copy_doubles + (size_t)kc * p.P, b, i, v);
-                    const int64_t row = (k0 + kb) * b + i;
-                    if (kb < nb && i < b && row < p.n) p.out[row] = v;
+            for (int q0 = 0; q0 < kMaxBlocksPerSub; q0 += NB) {
+                if (q0 * nsub < p.G) {  // uniform over the CTA
+                    const double* fq[NB];
+                    const double* gq[NB];
+                    double v[NB];
+#pragma unroll
+                    for (int d = 0; d < NB; ++d) {
+                        const int kb = sub + (q0 + d) * nsub;
+                        const int kc = kb < nb ? kb : 0;  // idle sub-warps read block 0 (valid memory), result dropped
+                        fq[d] = f + (size_t)kc * p.P;
+                        gq[d] = fq[d] + p.copy_doubles;
+                        v[d] = r[q0 + d];
+                    }
+                    if (DIR == 0 || DIR == 2) subwarp_solve<W, 0, B, NB>(fq, b, i, v);
+                    if (DIR == 1) subwarp_solve<W, 1, B, NB>(fq, b, i, v);
+                    if (DIR == 2) subwarp_solve<W, 1, B, NB>(gq, b, i, v);
+#pragma unroll
+                    for (int d = 0; d < NB; ++d) {
+                        const int kb = sub + (q0 + d) * nsub;
+                        const int64_t row = (k0 + kb) * b + i;
+                        if (kb < nb && i < b && row < p.n) p.out[row] = v[d];
+                    }
                 }
             }
             __syncwarp();
@@ -226,20 +241,20 @@ static int launch_small(bj_handle_s* h, const double* in, double* out)
     return BJ_OK;
 }
 
-template <int W, int DIR, int B>
+template <int W, int DIR, int B, int NB>
 static int launch_stream_solve(bj_handle_s* h, const SolveStreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR, B, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_stream_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR, B>, threads, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR, B, NB>, threads, smem);
     const int per_sm = std::max(1, std::min(occ, want_per_sm));
     const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
-    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR, B>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
+    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR, B, NB>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
@@ -272,14 +287,18 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
     sp.stages = stages;
     const size_t smem = 128 + stages * stage_bytes;
     const int per_sm = env_int("BJ_SOLVE_CTAS", 4);
+    const bool pair = bps % 2 == 0 && env_int("BJ_SOLVE_PAIR", 1) != 0;  // two blocks per sub-warp at a time
     switch (h->b) {  // compile-time instances for the workloads' block sizes
-        case 16: return launch_stream_solve<16, DIR, 16>(h, sp, per_sm, threads, smem);
-        case 24: return launch_stream_solve<32, DIR, 24>(h, sp, per_sm, threads, smem);
-        case 32: return launch_stream_solve<32, DIR, 32>(h, sp, per_sm, threads, smem);
+        case 16: return pair ? launch_stream_solve<16, DIR, 16, 2>(h, sp, per_sm, threads, smem)
+                             : launch_stream_solve<16, DIR, 16, 1>(h, sp, per_sm, threads, smem);
+        case 24: return pair ? launch_stream_solve<32, DIR, 24, 2>(h, sp, per_sm, threads, smem)
+                             : launch_stream_solve<32, DIR, 24, 1>(h, sp, per_sm, threads, smem);
+        case 32: return pair ? launch_stream_solve<32, DIR, 32, 2>(h, sp, per_sm, threads, smem)
+                             : launch_stream_solve<32, DIR, 32, 1>(h, sp, per_sm, threads, smem);
         default: break;
     }
-    return W == 16 ? launch_stream_solve<16, DIR, 0>(h, sp, per_sm, threads, smem)
-                   : launch_stream_solve<32, DIR, 0>(h, sp, per_sm, threads, smem);
+    return W == 16 ? launch_stream_solve<16, DIR, 0, 1>(h, sp, per_sm, threads, smem)
+                   : launch_stream_solve<32, DIR, 0, 1>(h, sp, per_sm, threads, smem);
 }
 
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)

@@ -9,6 +9,7 @@
 //   (cp.async.bulk + mbarrier, i.e. the TMA engine: no registers staged, deep memory-level
 //   parallelism), consumer warps reduce rows out of shared memory, gather t through L1/L2, and can
 //   run the forward block solve y = L^-1 u on the tile before y is written (fuses a7's last factor).
+#include <stdio.h>
 #include <stdlib.h>
 
 #include <algorithm>
@@ -445,6 +446,9 @@ int spmv_stream_finish(bj_handle_s* h, int max_tile)
     }
     h->tile_stages = stages;
     h->stream_ok = true;
+    if (env_int("BJ_VERBOSE", 0))
+        fprintf(stderr, "[bj] spmv plan: rows/tile %d cap %d stages %d smem %zu B lanes/row %d consumer warps %d fuse %d coherence %.3f\n",
+                h->tile_rows, h->tile_cap, h->tile_stages, smem, h->stream_lanes, h->stream_warps, (int)h->fuse_ok, h->coherence);
     return BJ_OK;
 }
 
