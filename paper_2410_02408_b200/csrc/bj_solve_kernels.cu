@@ -215,6 +215,176 @@ solve_stream_kernel(const SolveStreamParams p)
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// b in {16, 24, 32}: a GROUP of LPB = 4 lanes per block, each lane owning the b / 4 rows i = 4k + l in
+// registers, eight blocks per warp.  At step j the owner of row j broadcasts its finished value inside
+// the group (one 64-bit shuffle serves b / 4 rows of eight blocks), every lane updates its rows below
+// (above) j with one LDS + one DFMA each; which rows take part is known at compile time except in the
+// one register row that holds row j.  About 2 instructions per block and step instead of 9 with one lane
+// per row, no idle lanes for b = 24: the solve is HBM-bound again instead of issue-bound.
+// Each warp owns a private ring of shared-memory stages; lane 0 refills a stage right after the warp
+// has consumed it (one bulk async copy per block, blocks padded to a stride of 32 mod 128 bytes so the
+// eight groups of a warp read different banks).  No producer warp, no CTA-wide barrier.
+// ------------------------------------------------------------------------------------------------
+template <int B, int LPB>
+struct GroupGeom {
+    static constexpr int P = B * (B + 1) / 2;
+    static constexpr int RPL = B / LPB;   // rows per lane
+    static constexpr int NBW = 32 / LPB;  // blocks per warp
+    // per-block stride in shared memory: packed size padded so that consecutive blocks start LPB * 8 bytes
+    // (mod 128) apart -- the groups of a warp then read different banks
+    static constexpr int target = (LPB * 8) % 128;
+    static constexpr int pad_bytes = ((target - (P * 8) % 128) + 128) % 128;
+    static constexpr int STRIDE = P + pad_bytes / 8;
+    static_assert(B % LPB == 0 && (P * 8) % 16 == 0 && pad_bytes % 16 == 0, "bulk copies need 16-byte granules");
+};
+
+// forward substitution on the staged forward copy (column-major packed lower, rows scaled by 1/l_ii)
+template <int B, int LPB>
+__device__ __forceinline__ void group_forward(const double* f, int l, double (&r)[B / LPB])
+{
+    constexpr int RPL = B / LPB;
+#pragma unroll
+    for (int k = 0; k < RPL; ++k) {
+        const int i = k * LPB + l;
+        r[k] *= f[i * B - i * (i - 1) / 2];
+    }
+#pragma unroll
+    for (int j = 0; j < B - 1; ++j) {
+        const int kj = j / LPB, lj = j % LPB;
+        const double vj = __shfl_sync(0xffffffffu, r[kj], lj, LPB);
+        const double* col = f + (j * B - j * (j - 1) / 2 - j) + l;  // element (i, j) at col[i - l]
+#pragma unroll
+        for (int k = kj; k < RPL; ++k) {
+            if (k == kj && lj == LPB - 1) continue;  // no row of this register row lies below j
+            double lij = col[k * LPB];
+            if (k == kj) lij = (l > lj) ? lij : 0.0;
+            r[k] = fma(-lij, vj, r[k]);
+        }
+    }
+}
+
+// backward substitution on the staged backward copy (row-major packed lower, columns scaled by 1/l_jj)
+template <int B, int LPB>
+__device__ __forceinline__ void group_backward(const double* f, int l, double (&r)[B / LPB])
+{
+    constexpr int RPL = B / LPB;
+#pragma unroll
+    for (int k = 0; k < RPL; ++k) {
+        const int i = k * LPB + l;
+        r[k] *= f[i * (i + 1) / 2 + i];
+    }
+#pragma unroll
+    for (int j = B - 1; j >= 1; --j) {
+        const int kj = j / LPB, lj = j % LPB;
+        const double vj = __shfl_sync(0xffffffffu, r[kj], lj, LPB);
+        const double* row = f + j * (j + 1) / 2 + l;  // element (j, i) at row[i - l]
+#pragma unroll
+        for (int k = 0; k <= kj; ++k) {
+            if (k == kj && lj == 0) continue;  // no row of this register row lies above j
+            double lji = (k < kj || l < lj) ? row[k * LPB] : 0.0;  // the guard also keeps the read inside row j
+            r[k] = fma(-lji, vj, r[k]);
+        }
+    }
+}
+
+struct GroupParams {
+    int64_t n, nblocks, ntiles;  // a tile = the eight consecutive blocks one warp solves together
+    const double* fac0;          // forward copy (DIR 0, 2) or backward copy (DIR 1)
+    const double* fac1;          // backward copy (DIR 2 only)
+    const double* in;
+    double* out;
+    int stages;
+};
+
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+template <int B, int LPB, int DIR>
+__global__ void __launch_bounds__(384)
+solve_group_kernel(const GroupParams p)
+{
+    using Geo = GroupGeom<B, LPB>;
+    constexpr int RPL = Geo::RPL;
+    constexpr int NBW = Geo::NBW;
+    constexpr int kCopies = DIR == 2 ? 2 : 1;
+    constexpr int kStageDoubles = kCopies * NBW * Geo::STRIDE;
+    constexpr uint32_t kBlockBytes = Geo::P * 8;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nwarps = blockDim.x >> 5;
+    // per warp: `stages` mbarriers (64 bytes reserved), then its ring
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw) + warp * 8;
+    double* ring = reinterpret_cast<double*>(smem_raw + (size_t)nwarps * 64) + (size_t)warp * p.stages * kStageDoubles;
+
+    if (lane == 0) {
+        for (int s = 0; s < p.stages; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    const int64_t stride = (int64_t)gridDim.x * nwarps;
+    const int64_t first = (int64_t)blockIdx.x * nwarps + warp;
+    const uint64_t pol = policy_evict_first();
+    auto issue = [&](int64_t tile, int s) {  // lane 0 only: one bulk copy per block and copy
+        if (tile >= p.ntiles) return;
+        const int64_t k0 = tile * NBW;
+        const int nb = (int)(k0 + NBW <= p.nblocks ? NBW : p.nblocks - k0);
+        double* dst = ring + (size_t)s * kStageDoubles;
+        mbar_expect_tx(&full[s], (uint32_t)nb * kBlockBytes * kCopies);
+        for (int q = 0; q < nb; ++q) {
+            bulk_g2s(dst + q * Geo::STRIDE, p.fac0 + (k0 + q) * Geo::P, kBlockBytes, &full[s], pol);
+            if (DIR == 2) bulk_g2s(dst + (NBW + q) * Geo::STRIDE, p.fac1 + (k0 + q) * Geo::P, kBlockBytes, &full[s], pol);
+        }
+    };
+    if (lane == 0)
+        for (int s = 0; s < p.stages; ++s) issue(first + s * stride, s);  // factors are setup-time constants: no wait
+
+    const int g = lane / LPB, l = lane % LPB;
+    pdl_wait();  // `in` may come from the previous kernel
+    auto fetch = [&](int64_t tile, double (&dst)[RPL]) {
+        const int64_t kb = tile * NBW + g;
+        const int64_t base = kb * B + l;
+#pragma unroll
+        for (int k = 0; k < RPL; ++k) {
+            const int64_t row = base + k * LPB;
+            dst[k] = (tile < p.ntiles && kb < p.nblocks && row < p.n) ? p.in[row] : 0.0;
+        }
+    };
+    double rn[RPL];
+    fetch(first, rn);
+    int it = 0;
+    for (int64_t tile = first; tile < p.ntiles; tile += stride, ++it) {
+        const int s = it % p.stages;
+        const uint32_t ph = (uint32_t)((it / p.stages) & 1);
+        double r[RPL];
+#pragma unroll
+        for (int k = 0; k < RPL; ++k) r[k] = rn[k];
+        fetch(tile + stride, rn);  // one tile ahead: its latency hides behind this tile's solve
+        mbar_wait(&full[s], ph);
+        const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
+        if (DIR == 0 || DIR == 2) group_forward<B, LPB>(f, l, r);
+        if (DIR == 1) group_backward<B, LPB>(f, l, r);
+        if (DIR == 2) group_backward<B, LPB>(f + NBW * Geo::STRIDE, l, r);
+        const int64_t kb = tile * NBW + g;
+        const int64_t base = kb * B + l;
+        if (kb < p.nblocks) {
+#pragma unroll
+            for (int k = 0; k < RPL; ++k) {
+                const int64_t row = base + k * LPB;
+                if (row < p.n) p.out[row] = r[k];
+            }
+        }
+        __syncwarp();
+        if (lane == 0) {
+            fence_proxy_async();  // the warp's generic reads of this stage precede the async refill
+            issue(tile + (int64_t)p.stages * stride, s);
+        }
+    }
+}
+
 // b == 1 fast path is just the B = 1 instance of solve_small_kernel.
 
 template <int DIR>
@@ -301,6 +471,61 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
                    : launch_stream_solve<32, DIR, 0, 1>(h, sp, per_sm, threads, smem);
 }
 
+template <int B, int LPB, int DIR>
+static int launch_group_t(bj_handle_s* h, const double* in, double* out)
+{
+    using Geo = GroupGeom<B, LPB>;
+    constexpr int kGroupBlocksPerWarp = Geo::NBW;
+    constexpr int kCopies = DIR == 2 ? 2 : 1;
+    const size_t stage_bytes = (size_t)kCopies * kGroupBlocksPerWarp * Geo::STRIDE * 8;
+    const int stages = std::max(2, std::min(8, env_int("BJ_GROUP_STAGES", 2)));
+    // as many warps as fit one SM's shared memory (one CTA per SM), at most 12: the bytes in flight per SM are
+    // what hides the ~2 us loaded DRAM latency (throughput ~ ring bytes / (latency + one tile's solve))
+    const size_t budget = (size_t)env_int("BJ_GROUP_SMEM_KB", 222) * 1024;
+    int warps = (int)(budget / (stages * stage_bytes + 64));
+    warps = std::max(1, std::min(warps, env_int("BJ_GROUP_WARPS", 12)));
+    const size_t smem = (size_t)warps * (64 + stages * stage_bytes);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(solve_group_kernel<B, LPB, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_group_kernel)"); return BJ_ERR_CUDA; }
+        configured = true;
+    }
+    GroupParams gp;
+    gp.n = h->n; gp.nblocks = h->nblocks;
+    gp.ntiles = (h->nblocks + kGroupBlocksPerWarp - 1) / kGroupBlocksPerWarp;
+    gp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
+    gp.fac1 = h->fac_bwd;
+    gp.in = in; gp.out = out; gp.stages = stages;
+    int occ = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_group_kernel<B, LPB, DIR>, warps * 32, smem);
+    const int64_t want = (gp.ntiles + warps - 1) / warps;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * std::max(1, occ)));
+    cudaError_t e = launch_kernel(solve_group_kernel<B, LPB, DIR>, grid, warps * 32, smem, h->stream, h->pdl && !h->prof_on, gp);
+    if (e != cudaSuccess) { set_cuda_error(e, "solve_group_kernel launch"); return BJ_ERR_CUDA; }
+    return BJ_OK;
+}
+
+template <int DIR>
+static int launch_group(bj_handle_s* h, const double* in, double* out)
+{
+    // lanes per block: small enough tiles that many warps fit one SM's shared memory (latency hiding)
+    const int lpb = env_int("BJ_GROUP_LANES", h->b == 32 ? 8 : 4);
+    switch (h->b) {
+        case 16: return lpb == 8 ? launch_group_t<16, 8, DIR>(h, in, out) : launch_group_t<16, 4, DIR>(h, in, out);
+        case 24: return lpb == 8 ? launch_group_t<24, 8, DIR>(h, in, out) : launch_group_t<24, 4, DIR>(h, in, out);
+        case 32: return lpb == 16 ? launch_group_t<32, 16, DIR>(h, in, out)
+                      : lpb == 8 ? launch_group_t<32, 8, DIR>(h, in, out) : launch_group_t<32, 4, DIR>(h, in, out);
+        default: return BJ_ERR_INVALID_ARG;
+    }
+}
+
+static bool use_group_kernel(const bj_handle_s* h)
+{
+    return (h->b == 16 || h->b == 24 || h->b == 32) && env_int("BJ_SOLVE_GROUP", 1) != 0 &&
+           (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0;
+}
+
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)
 {
     int rc = BJ_OK;
@@ -313,6 +538,8 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)
         KernelScope scope(h, kind);
         if (h->solve_kind == 1) {
             rc = dir == 0 ? launch_small<0>(h, in, out) : dir == 1 ? launch_small<1>(h, in, out) : launch_small<2>(h, in, out);
+        } else if (use_group_kernel(h)) {
+            rc = dir == 0 ? launch_group<0>(h, in, out) : dir == 1 ? launch_group<1>(h, in, out) : launch_group<2>(h, in, out);
         } else {
             rc = dir == 0 ? launch_warp<0>(h, in, out) : dir == 1 ? launch_warp<1>(h, in, out) : launch_warp<2>(h, in, out);
         }
