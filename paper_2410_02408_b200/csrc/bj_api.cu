@@ -8,6 +8,7 @@
 #include <new>
 
 #include "bj_internal.cuh"
+#include "bj_lanczos_fuse.cuh"
 
 namespace bj {
 
@@ -75,6 +76,18 @@ int op_apply_device(bj_handle_s* h, const double* x, double* y)
     rc = h->spmv_kernel == 1 ? launch_spmv_stream(h, h->t, h->u, false) : launch_spmv_vector(h, h->t, h->u);
     if (rc != BJ_OK) return rc;
     return launch_solve(h, 0, h->u, y);  // y = L^-1 u
+}
+
+int op_apply_lanczos(bj_handle_s* h, const LzPrologue* pro, const LzEpilogue* epi, double* w)
+{
+    if (!lanczos_fusable(h)) return BJ_ERR_INVALID_ARG;
+    int rc = launch_solve(h, 1, nullptr, h->t, pro, nullptr);  // v_next on the fly, t = L^-T v_next
+    if (rc != BJ_OK) return rc;
+    const bool fuse = h->solve_kind == 1 && h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0;
+    if (fuse) return launch_spmv_stream(h, h->t, w, true, epi);  // w' and the dot partials in the SpMV's epilogue
+    rc = h->spmv_kernel == 1 ? launch_spmv_stream(h, h->t, h->u, false) : launch_spmv_vector(h, h->t, h->u);
+    if (rc != BJ_OK) return rc;
+    return launch_solve(h, 0, h->u, w, nullptr, epi);
 }
 
 // Device memory for a handle comes from a private stream-ordered pool (cudaMallocFromPoolAsync) whose

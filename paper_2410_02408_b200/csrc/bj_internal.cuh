@@ -46,6 +46,10 @@ struct LanczosWs {
     double* beta = nullptr;
     double* scal = nullptr;     // [0]=beta_j (current), [1]=amax, [2]=1/||v0||, [3]=alpha_j
     int* done = nullptr;        // [0]=stop flag, [1]=m_eff
+    double* lz_part = nullptr;  // fused fast mode: [2][lz_cap] per-CTA partials of the epilogue kernel
+    double* lz_sums = nullptr;  // [0] = v.w', [1] = w'.w'
+    unsigned* lz_ticket = nullptr;
+    int lz_cap = 0;
     int cap_iters = 0;
     int64_t bytes = 0;
 };
@@ -136,17 +140,23 @@ struct KernelScope {
     ~KernelScope();
 };
 
+struct LzPrologue;
+struct LzEpilogue;
+
 // setup (bj_setup_kernels.cu)
 int launch_validate(bj_handle_s* h);
 int launch_extract_factor(bj_handle_s* h);
 int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nnz
 
 // solves (bj_solve_kernels.cu): dir 0 = forward (L^-1), 1 = backward (L^-T), 2 = both (apply)
-int launch_solve(bj_handle_s* h, int dir, const double* in, double* out);
+// pro (dir 1 only) / epi (dir 0 only): fused Lanczos hooks of bj_lanczos_fuse.cuh, null for a plain solve
+int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro = nullptr,
+                 const LzEpilogue* epi = nullptr);
+bool lanczos_fusable(const bj_handle_s* h);  // the handle's solve / SpMV kernels carry the fused Lanczos hooks
 
 // SpMV (bj_spmv_kernels.cu)
 int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);
-int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward);
+int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi = nullptr);
 int spmv_stream_configure(bj_handle_s* h);  // decide tile rows / fusion, launch tile_nnz_kernel (async)
 int spmv_stream_finish(bj_handle_s* h, int max_tile);  // stage capacity and count, sets stream_ok
 
@@ -159,5 +169,7 @@ int env_int(const char* name, int dflt);  // tuning knobs BJ_* (read at setup / 
 
 // operator (bj_api.cu)
 int op_apply_device(bj_handle_s* h, const double* x, double* y);
+// one fused Lanczos step: t = L^-T v_next (v_next built by the prologue), w = L^-1 A t - beta v_cur with the dot partials
+int op_apply_lanczos(bj_handle_s* h, const LzPrologue* pro, const LzEpilogue* epi, double* w);
 
 }  // namespace bj

@@ -14,6 +14,7 @@
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
+#include "bj_lanczos_fuse.cuh"
 
 namespace bj {
 
@@ -253,6 +254,7 @@ void lanczos_free(bj_handle_s* h)
     LanczosWs& z = h->lz;
     cudaFree(z.V); cudaFree(z.w); cudaFree(z.partial); cudaFree(z.coef);
     cudaFree(z.alpha); cudaFree(z.beta); cudaFree(z.scal); cudaFree(z.done);
+    cudaFree(z.lz_part); cudaFree(z.lz_sums); cudaFree(z.lz_ticket);
     h->workspace_bytes -= z.bytes;
     z = LanczosWs();
 }
@@ -274,6 +276,11 @@ static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec)
     if (e == cudaSuccess) e = A((void**)&z.beta, sizeof(double) * (size_t)iters);
     if (e == cudaSuccess) e = A((void**)&z.scal, sizeof(double) * 8);
     if (e == cudaSuccess) e = A((void**)&z.done, sizeof(int) * 4);
+    // fused fast mode: the epilogue kernel with the largest grid is the thread-per-block solve (nblocks / 128 CTAs)
+    z.lz_cap = (int)std::max<int64_t>(kMaxPartials, (h->nblocks + 127) / 128 + 1);
+    if (e == cudaSuccess) e = A((void**)&z.lz_part, sizeof(double) * 2 * (size_t)z.lz_cap);
+    if (e == cudaSuccess) e = A((void**)&z.lz_sums, sizeof(double) * 4);
+    if (e == cudaSuccess) e = A((void**)&z.lz_ticket, sizeof(unsigned) * 4);
     z.bytes = bytes;
     h->workspace_bytes += bytes;
     if (e != cudaSuccess) {
@@ -382,11 +389,42 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         if (rc != BJ_OK) return rc;
         v0 = z.w;
     }
-    BJ_LAUNCH(dot_partial_kernel, G, kReduceThreads, n, v0, v0, PB);
-    BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, v0, vcol(0), (const double*)PB, G, 0, 0, tol,
-              (const double*)z.alpha, z.beta, amax_buf, z.done);
+    const bool fused_mode = !reorth && lanczos_fusable(h) && env_int("BJ_LANCZOS_FUSE", 1) != 0;
+    if (!fused_mode) BJ_LAUNCH(dot_partial_kernel, G, kReduceThreads, n, v0, v0, PB);
+    if (!fused_mode)
+        BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, v0, vcol(0), (const double*)PB, G, 0, 0, tol,
+                  (const double*)z.alpha, z.beta, amax_buf, z.done);
 
-    for (int j = 0; j < m; ++j) {
+    const bool fused = fused_mode;
+    if (fused) {
+        // Fast mode, fused: an iteration is exactly the kernels of one operator apply (bj_lanczos_fuse.cuh).
+        BJ_CUDA(cudaMemsetAsync(z.lz_ticket, 0, sizeof(unsigned) * 4, st));
+        LzPrologue pro;
+        LzEpilogue epi;
+        pro.w = z.w; pro.sum_a = z.lz_sums; pro.alpha = z.alpha; pro.done = z.done;
+        pro.red.part = z.lz_part; pro.red.out = z.lz_sums + 1; pro.red.ticket = z.lz_ticket; pro.red.cap = z.lz_cap;
+        epi.w = z.w; epi.sum_b = z.lz_sums + 1; epi.alpha = z.alpha; epi.beta = z.beta; epi.amax = amax_buf;
+        epi.done = z.done; epi.tol = tol;
+        epi.red.part = z.lz_part; epi.red.out = z.lz_sums; epi.red.ticket = z.lz_ticket; epi.red.cap = z.lz_cap;
+        for (int j = 0; j < m; ++j) {
+            pro.w0 = j == 0 ? v0 : nullptr;
+            pro.vcur = j > 0 ? vcol(j - 1) : nullptr;
+            pro.j = j - 1;
+            pro.first = j == 0;
+            epi.vprev = j > 0 ? vcol(j - 1) : nullptr;
+            epi.vnew = vcol(j);
+            epi.j = j - 1;
+            epi.first = j == 0;
+            rc = op_apply_lanczos(h, &pro, &epi, z.w);
+            if (rc != BJ_OK) return rc;
+        }
+        // close the last step with the unfused kernels: alpha_m, w = w' - alpha_m v_m, beta_{m+1} = ||w||
+        BJ_LAUNCH(axpy_norm_kernel, G, kReduceThreads, n, z.w, (const double*)vcol(m - 1), (const double*)z.lz_sums, 1, m - 1,
+                  z.alpha, PB, 1, (const int*)z.done);
+        BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, (const double*)z.w, (double*)nullptr, (const double*)PB, G, 1, m - 1, tol,
+                  (const double*)z.alpha, z.beta, amax_buf, z.done);
+    }
+    for (int j = 0; j < m && !fused; ++j) {
         double* vj = vcol(j);
         rc = op_apply_device(h, vj, z.w);  // w = A^ v_j
         if (rc != BJ_OK) return rc;

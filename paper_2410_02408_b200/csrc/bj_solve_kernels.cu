@@ -15,43 +15,97 @@
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
+#include "bj_lanczos_fuse.cuh"
 
 namespace bj {
 
 // ------------------------------------------------------------------------------------------------
 // thread per block, compile-time B.  DIR: 0 forward, 1 backward, 2 both.
 // ------------------------------------------------------------------------------------------------
-template <int B, int DIR, bool VEC>
+template <int B, bool VEC>
+__device__ __forceinline__ void load_rows(const double* src, int64_t lo, int64_t n, bool whole, double (&v)[B])
+{
+    if (whole) {
+        if constexpr (VEC && B % 4 == 0) {
+#pragma unroll
+            for (int i = 0; i < B; i += 4) ld_v4(src + lo + i, v + i);
+        } else if constexpr (VEC && B % 2 == 0) {
+#pragma unroll
+            for (int i = 0; i < B; i += 2) ld_v2(src + lo + i, v + i);
+        } else {
+#pragma unroll
+            for (int i = 0; i < B; ++i) v[i] = src[lo + i];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < B; ++i) v[i] = (lo + i < n) ? src[lo + i] : 0.0;
+    }
+}
+
+template <int B, bool VEC>
+__device__ __forceinline__ void store_rows(double* dst, int64_t lo, int64_t n, bool whole, const double (&v)[B])
+{
+    if (whole) {
+        if constexpr (VEC && B % 4 == 0) {
+#pragma unroll
+            for (int i = 0; i < B; i += 4) st_v4(dst + lo + i, v + i);
+        } else if constexpr (VEC && B % 2 == 0) {
+#pragma unroll
+            for (int i = 0; i < B; i += 2) st_v2(dst + lo + i, v + i);
+        } else {
+#pragma unroll
+            for (int i = 0; i < B; ++i) dst[lo + i] = v[i];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < B; ++i)
+            if (lo + i < n) dst[lo + i] = v[i];
+    }
+}
+
+// LZ: 0 plain, 1 Lanczos prologue (DIR 1: the input is w built on the fly), 2 Lanczos epilogue (DIR 0)
+template <int B, int DIR, bool VEC, int LZ>
 __global__ void __launch_bounds__(128)
 solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
-                   const double* in, double* out)  // in == out allowed: a thread touches only its own block
+                   const double* in, double* out,  // in == out allowed: a thread touches only its own block
+                   const LzPrologue pro, const LzEpilogue epi)
 {
     constexpr int P = B * (B + 1) / 2;
+    __shared__ double lz_sh[4];
     pdl_trigger();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= nblocks) return;
-    const double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
+    const bool act = k < nblocks;
+    if (LZ == 0 && !act) return;
+    const int64_t kc = act ? k : 0;
+    const double* f = fac + (kc >> 5) * (int64_t)(P * kInterleave) + (kc & 31);
     double l[P];
 #pragma unroll
     for (int e = 0; e < P; ++e) l[e] = ld_stream(f + e * kInterleave);   // factors never change after setup
     pdl_wait();                                                          // `in` may come from the previous kernel
-    const int64_t lo = k * B;
+    const int64_t lo = kc * B;
     double v[B];
     const bool whole = lo + B <= n;
-    if (whole) {
-        if constexpr (VEC && B % 4 == 0) {
+    double acc = 0.0, beta = 0.0, inv_beta = 0.0;  // Lanczos: running dot product of this thread
+    if (LZ == 1) {
+        double alpha;
+        if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
+        if (act) {
+            if (pro.first) {
+                load_rows<B, VEC>(pro.w0, lo, n, whole, v);
+            } else {
+                double c[B];
+                load_rows<B, VEC>(pro.w, lo, n, whole, v);
+                load_rows<B, VEC>(pro.vcur, lo, n, whole, c);
 #pragma unroll
-            for (int i = 0; i < B; i += 4) ld_v4(in + lo + i, v + i);
-        } else if constexpr (VEC && B % 2 == 0) {
+                for (int i = 0; i < B; ++i) v[i] -= alpha * c[i];
+            }
 #pragma unroll
-            for (int i = 0; i < B; i += 2) ld_v2(in + lo + i, v + i);
-        } else {
-#pragma unroll
-            for (int i = 0; i < B; ++i) v[i] = in[lo + i];
+            for (int i = 0; i < B; ++i) acc = fma(v[i], v[i], acc);  // rows past n were loaded as zeros
+            store_rows<B, VEC>(pro.w, lo, n, whole, v);
         }
     } else {
-#pragma unroll
-        for (int i = 0; i < B; ++i) v[i] = (lo + i < n) ? in[lo + i] : 0.0;
+        if (LZ == 2 && lz_epilogue_begin(epi, beta, inv_beta)) return;  // uniform over the grid
+        load_rows<B, VEC>(in, lo, n, whole, v);
     }
     if (DIR == 0 || DIR == 2) {
 #pragma unroll
@@ -71,21 +125,25 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
             v[i] = s * l[i * (i + 1) / 2 + i];
         }
     }
-    if (whole) {
-        if constexpr (VEC && B % 4 == 0) {
+    if (LZ == 2) {
+        if (act) {
+            double c[B], d[B];  // w and v_j
+            load_rows<B, VEC>(epi.w, lo, n, whole, c);
+            if (epi.vprev) load_rows<B, VEC>(epi.vprev, lo, n, whole, d);
 #pragma unroll
-            for (int i = 0; i < B; i += 4) st_v4(out + lo + i, v + i);
-        } else if constexpr (VEC && B % 2 == 0) {
-#pragma unroll
-            for (int i = 0; i < B; i += 2) st_v2(out + lo + i, v + i);
-        } else {
-#pragma unroll
-            for (int i = 0; i < B; ++i) out[lo + i] = v[i];
+            for (int i = 0; i < B; ++i) {
+                c[i] *= inv_beta;                       // v_{j+1}
+                v[i] *= inv_beta;
+                if (epi.vprev) v[i] -= beta * d[i];     // w'_new
+                acc = fma(c[i], v[i], acc);             // rows past n: c = 0
+            }
+            store_rows<B, VEC>(epi.vnew, lo, n, whole, c);
+            store_rows<B, VEC>(epi.w, lo, n, whole, v);
         }
+        lz_reduce_finish(epi.red, acc, lz_sh);
     } else {
-#pragma unroll
-        for (int i = 0; i < B; ++i)
-            if (lo + i < n) out[lo + i] = v[i];
+        if (act) store_rows<B, VEC>(out, lo, n, whole, v);
+        if (LZ == 1) lz_reduce_finish(pro.red, acc, lz_sh);
     }
 }
 
@@ -295,6 +353,9 @@ struct GroupParams {
     const double* in;
     double* out;
     int stages;
+    int lz;              // 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0)
+    LzPrologue pro;
+    LzEpilogue epi;
 };
 
 __device__ __forceinline__ void fence_proxy_async()
@@ -315,9 +376,13 @@ solve_group_kernel(const GroupParams p)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nwarps = blockDim.x >> 5;
-    // per warp: `stages` mbarriers (64 bytes reserved), then its ring
+    // per warp: `stages` mbarriers (64 bytes reserved), an exchange buffer for the tile's vector rows, then its ring
+    constexpr int XB = B + 2;          // padded row of the exchange buffer (one block), in doubles
+    constexpr int kXchg = NBW * XB;    // NBW * B = 32 * RPL rows per tile
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw) + warp * 8;
-    double* ring = reinterpret_cast<double*>(smem_raw + (size_t)nwarps * 64) + (size_t)warp * p.stages * kStageDoubles;
+    double* xchg = reinterpret_cast<double*>(smem_raw + (size_t)nwarps * 64) + (size_t)warp * kXchg;
+    double* ring = reinterpret_cast<double*>(smem_raw + (size_t)nwarps * 64) + (size_t)nwarps * kXchg +
+                   (size_t)warp * p.stages * kStageDoubles;
 
     if (lane == 0) {
         for (int s = 0; s < p.stages; ++s) mbar_init(&full[s], 1);
@@ -344,37 +409,96 @@ solve_group_kernel(const GroupParams p)
 
     const int g = lane / LPB, l = lane % LPB;
     pdl_wait();  // `in` may come from the previous kernel
-    auto fetch = [&](int64_t tile, double (&dst)[RPL]) {
-        const int64_t kb = tile * NBW + g;
-        const int64_t base = kb * B + l;
+    __shared__ double lz_sh[12];
+    double alpha = 0.0, beta = 0.0, inv_beta = 0.0, acc = 0.0;  // Lanczos scalars and this thread's dot product
+    bool stop = false;
+    if (DIR == 1 && p.lz == 1) stop = lz_prologue_begin(p.pro, alpha);
+    if (DIR == 0 && p.lz == 2) stop = lz_epilogue_begin(p.epi, beta, inv_beta);
+    if (stop) {  // uniform over the grid; the bulk copies already issued must land before the CTA may exit
+        for (int s = 0; s < p.stages; ++s)
+            if (first + s * stride < p.ntiles) mbar_wait(&full[s], 0u);
+        return;
+    }
+    // Vector rows move COALESCED: the tile's NBW * B = 32 * RPL rows are contiguous in memory, lane q takes rows
+    // k * 32 + q; the exchange buffer turns that into the solve's (block g, row k * LPB + l) ownership and back.
+    // Loads of one tile are issued together (all rows, all vectors) before anything is stored: the Lanczos
+    // vectors may alias as far as the compiler knows, so interleaved stores would serialise the loads.
+    auto fetch = [&](int64_t tile, double (&dst)[RPL], double (&ew)[RPL], double (&ev)[RPL]) {
+        const int64_t row0 = tile * (NBW * B) + lane;
+        double a[RPL], c[RPL];
 #pragma unroll
         for (int k = 0; k < RPL; ++k) {
-            const int64_t row = base + k * LPB;
-            dst[k] = (tile < p.ntiles && kb < p.nblocks && row < p.n) ? p.in[row] : 0.0;
+            const int64_t row = row0 + k * 32;
+            const bool live = tile < p.ntiles && row < p.n;
+            a[k] = c[k] = 0.0;
+            if (DIR == 1 && p.lz == 1) {
+                if (live) a[k] = p.pro.first ? p.pro.w0[row] : p.pro.w[row];
+                if (live && !p.pro.first) c[k] = p.pro.vcur[row];
+            } else {
+                if (live) a[k] = p.in[row];
+                if (DIR == 0 && p.lz == 2) {  // the epilogue's own operands ride along one tile ahead
+                    ew[k] = live ? p.epi.w[row] : 0.0;
+                    ev[k] = (live && p.epi.vprev) ? p.epi.vprev[row] : 0.0;
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < RPL; ++k) {
+            if (DIR == 1 && p.lz == 1) {  // the solve's input is w = w' - alpha v_j, built here and stored once
+                const int64_t row = row0 + k * 32;
+                const double wi = a[k] - alpha * c[k];
+                if (tile < p.ntiles && row < p.n) p.pro.w[row] = wi;
+                acc = fma(wi, wi, acc);
+                dst[k] = wi;
+            } else {
+                dst[k] = a[k];
+            }
         }
     };
-    double rn[RPL];
-    fetch(first, rn);
+    double rn[RPL], ewn[RPL], evn[RPL];
+    fetch(first, rn, ewn, evn);
     int it = 0;
     for (int64_t tile = first; tile < p.ntiles; tile += stride, ++it) {
         const int s = it % p.stages;
         const uint32_t ph = (uint32_t)((it / p.stages) & 1);
         double r[RPL];
 #pragma unroll
-        for (int k = 0; k < RPL; ++k) r[k] = rn[k];
-        fetch(tile + stride, rn);  // one tile ahead: its latency hides behind this tile's solve
+        for (int k = 0; k < RPL; ++k) {
+            const int e = k * 32 + lane;
+            xchg[(e / B) * XB + e % B] = rn[k];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < RPL; ++k) r[k] = xchg[g * XB + k * LPB + l];
+        double ew[RPL], ev[RPL];
+#pragma unroll
+        for (int k = 0; k < RPL; ++k) { ew[k] = ewn[k]; ev[k] = evn[k]; }
+        fetch(tile + stride, rn, ewn, evn);  // one tile ahead: its latency hides behind this tile's solve
         mbar_wait(&full[s], ph);
         const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
         if (DIR == 0 || DIR == 2) group_forward<B, LPB>(f, l, r);
         if (DIR == 1) group_backward<B, LPB>(f, l, r);
         if (DIR == 2) group_backward<B, LPB>(f + NBW * Geo::STRIDE, l, r);
-        const int64_t kb = tile * NBW + g;
-        const int64_t base = kb * B + l;
-        if (kb < p.nblocks) {
+        __syncwarp();
 #pragma unroll
-            for (int k = 0; k < RPL; ++k) {
-                const int64_t row = base + k * LPB;
-                if (row < p.n) p.out[row] = r[k];
+        for (int k = 0; k < RPL; ++k) xchg[g * XB + k * LPB + l] = r[k];
+        __syncwarp();
+        const int64_t row0 = tile * (NBW * B) + lane;
+#pragma unroll
+        for (int k = 0; k < RPL; ++k) {
+            const int e = k * 32 + lane;
+            const int64_t row = row0 + k * 32;
+            const double y = xchg[(e / B) * XB + e % B];
+            if (row < p.n) {
+                if (DIR == 0 && p.lz == 2) {
+                    const double vn = ew[k] * inv_beta;              // v_{j+1}
+                    const double wi = y * inv_beta - beta * ev[k];   // w'_new (ev = 0 on the first step)
+                    p.epi.vnew[row] = vn;
+                    p.epi.w[row] = wi;
+                    acc = fma(vn, wi, acc);
+                } else {
+                    p.out[row] = y;
+                }
             }
         }
         __syncwarp();
@@ -383,24 +507,32 @@ solve_group_kernel(const GroupParams p)
             issue(tile + (int64_t)p.stages * stride, s);
         }
     }
+    if (DIR == 1 && p.lz == 1) lz_reduce_finish(p.pro.red, acc, lz_sh);
+    if (DIR == 0 && p.lz == 2) lz_reduce_finish(p.epi.red, acc, lz_sh);
 }
 
 // b == 1 fast path is just the B = 1 instance of solve_small_kernel.
 
-template <int DIR>
-static int launch_small(bj_handle_s* h, const double* in, double* out)
+template <int DIR, int LZ>
+static int launch_small(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
 {
     const int threads = 128;
     const unsigned blocks = (unsigned)((h->nblocks + threads - 1) / threads);
-    const bool vec = ((((uintptr_t)in) | ((uintptr_t)out)) & 31) == 0;
+    uintptr_t al = (uintptr_t)in | (uintptr_t)out;
+    if (pro) al |= (uintptr_t)pro->w0 | (uintptr_t)pro->w | (uintptr_t)pro->vcur;
+    if (epi) al |= (uintptr_t)epi->w | (uintptr_t)epi->vprev | (uintptr_t)epi->vnew;
+    const bool vec = (al & 31) == 0;
     const bool pdl = h->pdl && !h->prof_on;
+    const LzPrologue pr = pro ? *pro : LzPrologue{};
+    const LzEpilogue ep = epi ? *epi : LzEpilogue{};
+    if ((epi && (int)blocks > epi->red.cap) || (pro && (int)blocks > pro->red.cap)) return BJ_ERR_INVALID_ARG;
     cudaError_t e = cudaSuccess;
-#define BJ_CASE(B)                                                                                                   \
-    case B:                                                                                                          \
-        e = vec ? launch_kernel(solve_small_kernel<B, DIR, true>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,  \
-                                (const double*)h->fac_small, in, out)                                                \
-                : launch_kernel(solve_small_kernel<B, DIR, false>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks, \
-                                (const double*)h->fac_small, in, out);                                               \
+#define BJ_CASE(B)                                                                                                          \
+    case B:                                                                                                                 \
+        e = vec ? launch_kernel(solve_small_kernel<B, DIR, true, LZ>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,  \
+                                (const double*)h->fac_small, in, out, pr, ep)                                               \
+                : launch_kernel(solve_small_kernel<B, DIR, false, LZ>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks, \
+                                (const double*)h->fac_small, in, out, pr, ep);                                              \
         break;
     switch (h->b) {
         BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
@@ -416,7 +548,7 @@ static int launch_stream_solve(bj_handle_s* h, const SolveStreamParams& sp, int 
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR, B, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR, B, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_stream_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
@@ -472,7 +604,7 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
 }
 
 template <int B, int LPB, int DIR>
-static int launch_group_t(bj_handle_s* h, const double* in, double* out)
+static int launch_group_t(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
 {
     using Geo = GroupGeom<B, LPB>;
     constexpr int kGroupBlocksPerWarp = Geo::NBW;
@@ -481,13 +613,14 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out)
     const int stages = std::max(2, std::min(8, env_int("BJ_GROUP_STAGES", 2)));
     // as many warps as fit one SM's shared memory (one CTA per SM), at most 12: the bytes in flight per SM are
     // what hides the ~2 us loaded DRAM latency (throughput ~ ring bytes / (latency + one tile's solve))
-    const size_t budget = (size_t)env_int("BJ_GROUP_SMEM_KB", 222) * 1024;
-    int warps = (int)(budget / (stages * stage_bytes + 64));
+    const size_t budget = (size_t)env_int("BJ_GROUP_SMEM_KB", 220) * 1024;
+    const size_t xchg_bytes = (size_t)kGroupBlocksPerWarp * (B + 2) * 8;
+    int warps = (int)(budget / (stages * stage_bytes + 64 + xchg_bytes));
     warps = std::max(1, std::min(warps, env_int("BJ_GROUP_WARPS", 12)));
-    const size_t smem = (size_t)warps * (64 + stages * stage_bytes);
+    const size_t smem = (size_t)warps * (64 + xchg_bytes + stages * stage_bytes);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(solve_group_kernel<B, LPB, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(solve_group_kernel<B, LPB, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_group_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
@@ -497,25 +630,29 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out)
     gp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
     gp.fac1 = h->fac_bwd;
     gp.in = in; gp.out = out; gp.stages = stages;
+    gp.lz = (DIR == 1 && pro) ? 1 : (DIR == 0 && epi) ? 2 : 0;
+    gp.pro = pro ? *pro : LzPrologue{};
+    gp.epi = epi ? *epi : LzEpilogue{};
     int occ = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_group_kernel<B, LPB, DIR>, warps * 32, smem);
     const int64_t want = (gp.ntiles + warps - 1) / warps;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * std::max(1, occ)));
+    if ((gp.lz == 2 && grid > gp.epi.red.cap) || (gp.lz == 1 && grid > gp.pro.red.cap)) return BJ_ERR_INVALID_ARG;
     cudaError_t e = launch_kernel(solve_group_kernel<B, LPB, DIR>, grid, warps * 32, smem, h->stream, h->pdl && !h->prof_on, gp);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_group_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
 
 template <int DIR>
-static int launch_group(bj_handle_s* h, const double* in, double* out)
+static int launch_group(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
 {
     // lanes per block: small enough tiles that many warps fit one SM's shared memory (latency hiding)
     const int lpb = env_int("BJ_GROUP_LANES", h->b == 32 ? 8 : 4);
     switch (h->b) {
-        case 16: return lpb == 8 ? launch_group_t<16, 8, DIR>(h, in, out) : launch_group_t<16, 4, DIR>(h, in, out);
-        case 24: return lpb == 8 ? launch_group_t<24, 8, DIR>(h, in, out) : launch_group_t<24, 4, DIR>(h, in, out);
-        case 32: return lpb == 16 ? launch_group_t<32, 16, DIR>(h, in, out)
-                      : lpb == 8 ? launch_group_t<32, 8, DIR>(h, in, out) : launch_group_t<32, 4, DIR>(h, in, out);
+        case 16: return lpb == 8 ? launch_group_t<16, 8, DIR>(h, in, out, pro, epi) : launch_group_t<16, 4, DIR>(h, in, out, pro, epi);
+        case 24: return lpb == 8 ? launch_group_t<24, 8, DIR>(h, in, out, pro, epi) : launch_group_t<24, 4, DIR>(h, in, out, pro, epi);
+        case 32: return lpb == 16 ? launch_group_t<32, 16, DIR>(h, in, out, pro, epi)
+                      : lpb == 8 ? launch_group_t<32, 8, DIR>(h, in, out, pro, epi) : launch_group_t<32, 4, DIR>(h, in, out, pro, epi);
         default: return BJ_ERR_INVALID_ARG;
     }
 }
@@ -526,8 +663,15 @@ static bool use_group_kernel(const bj_handle_s* h)
            (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0;
 }
 
-int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)
+// kind 1 always carries the hooks; kind 2 only in the group kernel (b = 16, 24, 32); b = 0 has no solve to ride on
+bool lanczos_fusable(const bj_handle_s* h)
 {
+    return h->solve_kind == 1 || (h->solve_kind == 2 && use_group_kernel(h));
+}
+
+int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
+{
+    if ((pro || epi) && !lanczos_fusable(h)) return BJ_ERR_INVALID_ARG;
     int rc = BJ_OK;
     if (h->solve_kind == 0) {
         if (in != out) BJ_CUDA(cudaMemcpyAsync(out, in, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
@@ -537,9 +681,12 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out)
     {
         KernelScope scope(h, kind);
         if (h->solve_kind == 1) {
-            rc = dir == 0 ? launch_small<0>(h, in, out) : dir == 1 ? launch_small<1>(h, in, out) : launch_small<2>(h, in, out);
+            rc = dir == 0   ? (epi ? launch_small<0, 2>(h, in, out, nullptr, epi) : launch_small<0, 0>(h, in, out, nullptr, nullptr))
+                 : dir == 1 ? (pro ? launch_small<1, 1>(h, in, out, pro, nullptr) : launch_small<1, 0>(h, in, out, nullptr, nullptr))
+                            : launch_small<2, 0>(h, in, out, nullptr, nullptr);
         } else if (use_group_kernel(h)) {
-            rc = dir == 0 ? launch_group<0>(h, in, out) : dir == 1 ? launch_group<1>(h, in, out) : launch_group<2>(h, in, out);
+            rc = dir == 0 ? launch_group<0>(h, in, out, pro, epi) : dir == 1 ? launch_group<1>(h, in, out, pro, epi)
+                          : launch_group<2>(h, in, out, nullptr, nullptr);
         } else {
             rc = dir == 0 ? launch_warp<0>(h, in, out) : dir == 1 ? launch_warp<1>(h, in, out) : launch_warp<2>(h, in, out);
         }

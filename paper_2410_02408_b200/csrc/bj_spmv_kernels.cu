@@ -16,6 +16,7 @@
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
+#include "bj_lanczos_fuse.cuh"
 
 namespace bj {
 
@@ -112,6 +113,8 @@ struct StreamParams {
     int su_doubles;      // doubles per su buffer
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
+    int lz;              // 1: fused Lanczos epilogue on the rows this kernel writes (FUSE 0 and 1)
+    LzEpilogue epi;
 };
 
 __device__ __forceinline__ void consumer_bar_sync(int nthreads)
@@ -148,6 +151,12 @@ spmv_stream_kernel(const StreamParams p)
     __syncthreads();
 
     const int R = p.R;
+    __shared__ double lz_sh[kMaxStreamThreads / 32];
+    double pa = 0.0, beta = 0.0, inv_beta = 0.0;
+    if (p.lz) {  // beta and the stop flag come from the previous kernel: every thread waits for it
+        pdl_wait();
+        if (lz_epilogue_begin(p.epi, beta, inv_beta)) return;  // uniform over the grid, nothing in flight yet
+    }
     if (warp == 0) {
         // ------------------------------ producer ------------------------------------------------
         const uint64_t pol = policy_evict_first();
@@ -271,7 +280,8 @@ spmv_stream_kernel(const StreamParams p)
                     } else if (FUSE == 2) {
                         sub_u[i] = acc;
                     } else {
-                        p.y[r0 + i] = acc;
+                        if (p.lz) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, acc, pa);
+                        else p.y[r0 + i] = acc;
                     }
                 }
             }
@@ -322,13 +332,23 @@ spmv_stream_kernel(const StreamParams p)
                     }
 #pragma unroll
                     for (int i = 0; i < kSmallMax; ++i)
-                        if (i < b && lo + i < p.n) p.y[lo + i] = v[i];
+                        if (i < b) uk[i] = v[i];
+                }
+                // (C) rows leave COALESCED: thread q takes rows q, q + nct, .. of the tile (and, inside a Lanczos
+                // step, their w / v_j / v_{j+1} elements)
+                consumer_bar_sync(nct);
+                for (int i = ctid; i < rows; i += nct) {
+                    const int k = (int)__umulhi((unsigned)i, p.b_magic);
+                    const double yv = sub_u[k * p.bs + (i - k * b)];
+                    if (p.lz) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, yv, pa);
+                    else p.y[r0 + i] = yv;
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[s]);
         }
     }
+    if (p.lz) lz_reduce_finish(p.epi.red, pa, lz_sh);
 }
 
 template <int LPR, int BATCH, int FUSE, int W>
@@ -336,7 +356,7 @@ int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int want_per_sm, int
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, BATCH, FUSE, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, BATCH, FUSE, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
         configured = true;
     }
@@ -452,7 +472,7 @@ int spmv_stream_finish(bj_handle_s* h, int max_tile)
     return BJ_OK;
 }
 
-int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward)
+int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi)
 {
     if (!h->stream_ok) return BJ_ERR_INVALID_ARG;
     const bool fuse = fuse_forward && h->fuse_ok;
@@ -463,6 +483,10 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
     sp.early_trigger = (env_int("BJ_PDL_EARLY", 0) >> 1) & 1;
+    sp.lz = epi ? 1 : 0;
+    sp.epi = epi ? *epi : LzEpilogue{};
+    if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the sub-warp fused path has no hook
+    if (epi && h->num_sms * 4 > epi->red.cap) return BJ_ERR_INVALID_ARG;
     sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
     const int threads = 32 + 32 * h->stream_warps;
     const int grid = env_int("BJ_CTAS_PER_SM", 4);  // wanted CTAs per SM; clipped to the real occupancy at launch
