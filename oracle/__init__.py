@@ -50,6 +50,8 @@ def _load():
         lib.orc_tridiag_extremes.argtypes = [i32, vp, vp] + [C.POINTER(dbl)] * 4
         lib.orc_tridiag_all.argtypes = [i32, vp, vp, vp]
         lib.orc_num_threads.restype = i32
+        lib.orc_pcg.argtypes = [i64, vp, vp, vp, i64, vp, vp, vp, i32, dbl, vp, vp, vp, C.POINTER(i32), C.POINTER(dbl)]
+        lib.orc_pcg.restype = i32
         for f in ("orc_spmv", "orc_extract", "orc_solve_L", "orc_solve_Lt", "orc_apply", "orc_op_apply",
                   "orc_seeded_vector", "orc_tridiag_extremes", "orc_tridiag_all"):
             getattr(lib, f).restype = None
@@ -141,11 +143,40 @@ class Precond:
         k = m_eff.value
         return alpha[:k].copy(), beta[:k].copy()
 
+    def pcg(self, rhs, max_iters: int, rtol: float):
+        """Preconditioned CG from x0 = 0; returns x and the iteration record."""
+        rhs = _f64(rhs)
+        x = np.empty(self.n)
+        alpha = np.zeros(max_iters); beta = np.zeros(max_iters); relres = np.zeros(max_iters)
+        it = C.c_int(0); tr = C.c_double(0.0)
+        A = self.A
+        Lp = _p(self.L) if self.L is not None else None
+        rc = _load().orc_pcg(self.n, _p(A.row_ptr), _p(A.col_idx), _p(A.val), self.b, Lp, _p(rhs), _p(x), int(max_iters),
+                             float(rtol), _p(alpha), _p(beta), _p(relres), C.byref(it), C.byref(tr))
+        if rc != 0:
+            raise MemoryError("oracle pcg allocation failed")
+        k = it.value
+        nb = k - 1 if (k > 0 and relres[k - 1] <= rtol) else k
+        return {"x": x, "iters": k, "alpha": alpha[:k].copy(), "beta": beta[:max(nb, 0)].copy(),
+                "relres": relres[:k].copy(), "true_relres": tr.value}
+
     def cond_estimate(self, m: int, **kw):
         alpha, beta = self.lanczos(m, **kw)
         tmin, tmax, rmin, rmax = tridiag_extremes(alpha, beta)
         return {"lmin": tmin, "lmax": tmax, "kappa": tmax / tmin, "res_min": rmin, "res_max": rmax,
                 "iters_done": len(alpha), "alpha": alpha, "beta": beta}
+
+
+def cg_tridiag(alpha, beta):
+    """Lanczos tridiagonal of M^-1 A implied by k CG steps (CG-Lanczos equivalence): diagonal
+    d_0 = 1/a_0, d_j = 1/a_j + bt_{j-1}/a_{j-1}; off-diagonal e_j = sqrt(bt_j)/a_j, j = 0..k-2."""
+    a, bt = _f64(alpha), _f64(beta)
+    k = len(a)
+    d = np.empty(k)
+    for j in range(k):
+        d[j] = 1.0 / a[j] + (bt[j - 1] / a[j - 1] if j > 0 else 0.0)
+    e = np.array([np.sqrt(bt[j]) / a[j] for j in range(k - 1)])
+    return d, e
 
 
 def seeded_vector(seed: int, n: int) -> np.ndarray:

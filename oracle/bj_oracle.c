@@ -16,6 +16,7 @@
  * Pins (tests/test_oracle_pins.py): closed-form Laplacian spectra, line-block spectra,
  * b=N => identity, block-diagonal model of PAPER.md:80, numpy/scipy library routines on
  * random SPD blocks, dense eigensolves for N<=1024, m=N Lanczos == dense spectrum.
+ * PCG (orc_pcg): numpy dense solve, scipy.sparse.linalg.cg iterates, M = A => one step, CG-Lanczos Ritz values.
  * Unpinned against truth: kappa estimates of the five full-size configs (no closed form);
  * those are pinned only by the invariants above.  See DESIGN.md section 3.
  */
@@ -324,6 +325,58 @@ void orc_tridiag_extremes(int m, const double* alpha, const double* beta,
 void orc_tridiag_all(int m, const double* alpha, const double* beta, double* out)
 {
     for (int k = 0; k < m; ++k) out[k] = kth_eigenvalue(m, alpha, beta, k);
+}
+
+/* ---- NEXT-1: preconditioned conjugate gradients, the classical stand-in for the solve
+ * stage that follows the preconditioning path, with M = blockdiag(D_k) = L L^T applied
+ * as z = M^-1 r (b~ = M b) and the paper's accuracy metric ||Ax - b|| / ||b||
+ * (threshold 1e-3 at PAPER.md:388).  Textbook Hestenes-Stiefel ordering, x_0 = 0:
+ *   r = b; z = M^-1 r; p = z; rho = r.z
+ *   repeat: q = A p; a = rho / (p.q); x += a p; r -= a q; stop if ||r|| / ||b|| <= rtol;
+ *           z = M^-1 r; rho' = r.z; bt = rho' / rho; p = z + bt p; rho = rho'
+ * alpha[k] = a_k, beta[k] = bt_k (one fewer than alpha when the loop stops on rtol), relres[k] = ||r_{k+1}|| / ||b||
+ * from the recurrence; *true_relres = ||A x - b|| / ||b|| recomputed from x.  b == 0: M = I.                   */
+int orc_pcg(int64_t n, const int32_t* rp, const int32_t* ci, const double* val, int64_t b, const double* L,
+            const double* rhs, double* x, int max_iters, double rtol, double* alpha, double* beta,
+            double* relres, int* iters, double* true_relres)
+{
+    double* r = (double*)malloc((size_t)n * sizeof(double));
+    double* z = (double*)malloc((size_t)n * sizeof(double));
+    double* p = (double*)malloc((size_t)n * sizeof(double));
+    double* q = (double*)malloc((size_t)n * sizeof(double));
+    double* tmp = (double*)malloc((size_t)2 * (size_t)n * sizeof(double));
+    if (!r || !z || !p || !q || !tmp) { free(r); free(z); free(p); free(q); free(tmp); return ORC_ALLOC; }
+    const double bnorm = sqrt(dot(n, rhs, rhs));
+    for (int64_t i = 0; i < n; ++i) { x[i] = 0.0; r[i] = rhs[i]; }
+    *iters = 0;
+    *true_relres = 0.0;
+    if (bnorm > 0.0) {
+        if (b > 0) orc_apply(n, b, L, r, z, tmp); else memcpy(z, r, (size_t)n * sizeof(double));
+        memcpy(p, z, (size_t)n * sizeof(double));
+        double rho = dot(n, r, z);
+        for (int k = 0; k < max_iters; ++k) {
+            orc_spmv(n, rp, ci, val, p, q);
+            const double a = rho / dot(n, p, q);
+            for (int64_t i = 0; i < n; ++i) x[i] += a * p[i];
+            for (int64_t i = 0; i < n; ++i) r[i] -= a * q[i];
+            alpha[k] = a;
+            relres[k] = sqrt(dot(n, r, r)) / bnorm;
+            *iters = k + 1;
+            if (relres[k] <= rtol) break;
+            if (b > 0) orc_apply(n, b, L, r, z, tmp); else memcpy(z, r, (size_t)n * sizeof(double));
+            const double rho_new = dot(n, r, z);
+            const double bt = rho_new / rho;
+            beta[k] = bt;
+            for (int64_t i = 0; i < n; ++i) p[i] = z[i] + bt * p[i];
+            rho = rho_new;
+        }
+        orc_spmv(n, rp, ci, val, x, q);
+        double s = 0.0;
+        for (int64_t i = 0; i < n; ++i) { const double d = q[i] - rhs[i]; s += d * d; }
+        *true_relres = sqrt(s) / bnorm;
+    }
+    free(r); free(z); free(p); free(q); free(tmp);
+    return ORC_OK;
 }
 
 int orc_num_threads(void)

@@ -365,3 +365,100 @@ def test_seeded_vector_matches_published_splitmix64_sequence():
     assert abs(big.mean()) < 5e-3 and abs(big.var() - 1.0 / 3.0) < 5e-3
     # the input-generator module carries its own copy of the same integer steps
     assert np.array_equal(big, W.seeded_vector(oracle.DEFAULT_SEED, 200000))
+
+
+# ---------------------------------------------------------------- PCG -----------
+def _scipy_csr(A):
+    import scipy.sparse as sp
+    return sp.csr_matrix((A.val, A.col_idx, A.row_ptr), shape=(A.n, A.n))
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (3, 32), (4, 16), (5, 3), (1, 0)])
+def test_pcg_solves_the_system_dense_numpy(cfg, b):
+    """x from the oracle PCG = numpy dense solve; reported true residual = ||Ax - b|| / ||b||
+    recomputed here with scipy; the recurrence residual agrees with it; A-norm error decreases monotonically."""
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    xs = W.seeded_vector(11, A.n)
+    S = _scipy_csr(A)
+    rhs = S @ xs
+    r = P.pcg(rhs, 4 * A.n, 1e-13)
+    xd = np.linalg.solve(A.to_dense(), rhs)
+    kap = np.linalg.cond(A.to_dense())
+    assert np.linalg.norm(r["x"] - xd) <= 1e-12 * kap * np.linalg.norm(xd)
+    tr = np.linalg.norm(S @ r["x"] - rhs) / np.linalg.norm(rhs)
+    assert abs(tr - r["true_relres"]) <= 1e-14 + 1e-6 * tr
+    assert r["relres"][-1] <= 1e-13 and tr <= 1e-11
+    # monotone A-norm error (a property of CG, not of the residual norm): re-run with growing iteration caps
+    errs = []
+    for k in (1, 2, 3, 5, 8):
+        xk = P.pcg(rhs, k, 0.0)["x"]
+        e = xk - xd
+        errs.append(float(e @ (S @ e)))
+    assert all(errs[i + 1] <= errs[i] * (1 + 1e-12) for i in range(len(errs) - 1))
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (4, 16)])
+def test_pcg_iterates_match_scipy_cg(cfg, b):
+    """Library special case: scipy.sparse.linalg.cg with M = (L L^T)^-1 built from numpy Cholesky factors
+    runs the same recurrence; after k steps the iterates agree to rounding."""
+    import scipy.sparse.linalg as spla
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    S = _scipy_csr(A)
+    Ad = A.to_dense()
+    blocks = [np.linalg.inv(Ad[lo:min(lo + b, A.n), lo:min(lo + b, A.n)]) for lo in range(0, A.n, b)]
+
+    def minv(r):
+        out = np.empty_like(r)
+        for q, lo in enumerate(range(0, A.n, b)):
+            hi = min(lo + b, A.n)
+            out[lo:hi] = blocks[q] @ r[lo:hi]
+        return out
+
+    M = spla.LinearOperator((A.n, A.n), matvec=minv, dtype=np.float64)
+    rhs = W.seeded_vector(5, A.n)
+    for k in (1, 4, 9):
+        xs, _ = spla.cg(S, rhs, rtol=0.0, atol=0.0, maxiter=k, M=M)
+        xo = P.pcg(rhs, k, 0.0)["x"]
+        assert np.linalg.norm(xs - xo) <= 1e-10 * np.linalg.norm(xs), (cfg, b, k)
+
+
+def test_pcg_with_exact_preconditioner_takes_one_step():
+    """b = N: M = A, so x_1 = A^-1 b exactly (alpha_0 = 1) -- the paper's literal block-diagonal model."""
+    A = W.build(1, "tiny")
+    P = oracle.Precond(A, A.n)
+    rhs = W.seeded_vector(2, A.n)
+    r = P.pcg(rhs, 10, 1e-12)
+    assert r["iters"] == 1 and abs(r["alpha"][0] - 1.0) <= 1e-12 and r["true_relres"] <= 1e-13
+    Ab = W.block_diagonal_spd(9, 6)
+    r = oracle.Precond(Ab, 6).pcg(W.seeded_vector(3, Ab.n), 10, 1e-12)
+    assert r["iters"] == 1
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (3, 32)])
+def test_pcg_coefficients_give_the_lanczos_ritz_values(cfg, b):
+    """CG-Lanczos equivalence: the tridiagonal built from (alpha_k, beta_k) has the Ritz values of k-step Lanczos
+    on A^ = L^-1 A L^-T started from L^-1 b -- computed by the oracle's separate Lanczos routine."""
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    rhs = W.seeded_vector(8, A.n)
+    k = 12
+    r = P.pcg(rhs, k, 0.0)
+    d, e = oracle.cg_tridiag(r["alpha"], r["beta"])
+    T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+    ritz_cg = np.linalg.eigvalsh(T)
+    al, be = P.lanczos(k, v0=P.solve_L(rhs), reorth=True)
+    ritz_lz = oracle.tridiag_all(al, be)
+    assert np.allclose(ritz_cg, np.sort(ritz_lz), rtol=1e-9, atol=1e-12)
+
+
+def test_pcg_zero_rhs_and_residual_threshold():
+    A = W.build(2, "tiny")
+    P = oracle.Precond(A, 8)
+    r = P.pcg(np.zeros(A.n), 5, 1e-3)
+    assert r["iters"] == 0 and not r["x"].any()
+    rhs = W.seeded_vector(4, A.n)
+    r = P.pcg(rhs, 500, 1e-3)          # the paper's accuracy bar, PAPER.md:388
+    assert r["true_relres"] <= 1.05e-3 and r["relres"][-1] <= 1e-3
+    assert len(r["relres"]) == r["iters"] and (r["iters"] == 1 or r["relres"][-2] > 1e-3)
