@@ -93,6 +93,23 @@ typedef struct {
     int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
 } bj_info_t;
 
+typedef struct {
+    int32_t max_iters;    /* >= 1                                                                     */
+    int32_t check_every;  /* the host reads the device stop flag every this many iterations; <= 0: 16 */
+    double rtol;          /* stop when ||r_k|| / ||b|| <= rtol (recurrence residual); 0: run max_iters */
+} bj_pcg_opts_t;
+
+typedef struct {
+    int32_t iters;        /* iterations done                                                          */
+    int32_t converged;    /* 1 if the rtol test stopped the run                                       */
+    double relres;        /* ||r_k|| / ||b|| from the recurrence at exit                              */
+    double true_relres;   /* ||A x - b|| / ||b|| recomputed from x: the paper's accuracy metric */
+    double lmin, lmax;    /* extreme Ritz values of M^-1 A from the CG coefficients (CG-Lanczos); 0 if iters < 1 */
+    double* alpha_host;   /* host, optional, caller-allocated, >= max_iters doubles: step lengths a_k  */
+    double* beta_host;    /* host, optional, >= max_iters doubles: bt_k                                */
+    double* relres_host;  /* host, optional, >= max_iters doubles: ||r_{k+1}|| / ||b||                 */
+} bj_pcg_result_t;
+
 /* kernel-kind indices for bj_profile_get */
 enum { BJ_K_SOLVE_LT = 0, BJ_K_SPMV = 1, BJ_K_SOLVE_L = 2, BJ_K_APPLY = 3, BJ_K_SPMV_SOLVE_L = 4, BJ_K_COUNT = 5 };
 
@@ -137,6 +154,15 @@ int bj_op_apply(bj_handle_t h, const double* x, double* y);
  * free device memory, else none; default seed); extreme Ritz values to host out-pointers.  Synchronises. */
 int bj_cond_estimate(bj_handle_t h, int iters, double* lmin_host, double* lmax_host);
 int bj_cond_estimate_ex(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_lanczos_result_t* res_host);
+
+/* preconditioned conjugate gradients for A x = b from x_0 = 0 with M = blockdiag(D_k)
+ * (z = M^-1 r is bj_apply; b = 0 handle: plain CG), the classical stand-in for the solve stage that follows
+ * the preconditioning path.  b_dev and x_dev are device vectors of length n (x_dev out).
+ * Textbook Hestenes-Stiefel ordering; every scalar stays on the device, the host only polls the stop flag every
+ * check_every iterations.  Reports the paper's residual ||Ax-b||/||b|| (its bar is 1e-3,
+ * PAPER.md:388) and a second estimate of the spectrum of M^-1 A from the CG coefficients.  Synchronises.
+ * Workspace (4 n doubles) is allocated by the first call and kept by the handle.  b_dev = 0 returns x = 0, iters = 0. */
+int bj_pcg_solve(bj_handle_t h, const double* b_dev, double* x_dev, const bj_pcg_opts_t* opts_host, bj_pcg_result_t* res_host);
 
 /* Fill a device vector with the seeded start-vector sequence (see bj_lanczos_opts_t.seed). */
 int bj_seeded_vector(bj_handle_t h, uint64_t seed, double* v);

@@ -22,7 +22,7 @@ KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
 EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
-           "bj_profile_get", "bj_release_cached_memory"]
+           "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve"]
 
 
 class bj_csr_t(C.Structure):
@@ -38,6 +38,16 @@ class bj_lanczos_opts_t(C.Structure):
 class bj_lanczos_result_t(C.Structure):
     _fields_ = [("iters_done", C.c_int32), ("lmin", C.c_double), ("lmax", C.c_double), ("res_min", C.c_double),
                 ("res_max", C.c_double), ("alpha_host", C.c_void_p), ("beta_host", C.c_void_p)]
+
+
+class bj_pcg_opts_t(C.Structure):
+    _fields_ = [("max_iters", C.c_int32), ("check_every", C.c_int32), ("rtol", C.c_double)]
+
+
+class bj_pcg_result_t(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("relres", C.c_double), ("true_relres", C.c_double),
+                ("lmin", C.c_double), ("lmax", C.c_double), ("alpha_host", C.c_void_p), ("beta_host", C.c_void_p),
+                ("relres_host", C.c_void_p)]
 
 
 class bj_info_t(C.Structure):
@@ -79,6 +89,7 @@ def lib():
         L.bj_cond_estimate.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.bj_cond_estimate_ex.argtypes = [vp, C.POINTER(bj_lanczos_opts_t), C.POINTER(bj_lanczos_result_t)]
         L.bj_seeded_vector.argtypes = [vp, C.c_uint64, vp]
+        L.bj_pcg_solve.argtypes = [vp, vp, vp, C.POINTER(bj_pcg_opts_t), C.POINTER(bj_pcg_result_t)]
         L.bj_release_cached_memory.argtypes = []
         L.bj_profile_enable.argtypes = [vp, i32]
         L.bj_profile_get.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
@@ -226,6 +237,24 @@ def bj_cond_estimate_ex(h, iters: int, reorth: bool = True, seed: int = BJ_DEFAU
     k = r.iters_done
     return {"iters_done": k, "lmin": r.lmin, "lmax": r.lmax, "kappa": r.lmax / r.lmin, "res_min": r.res_min,
             "res_max": r.res_max, "alpha": alpha[:k].copy(), "beta": beta[:k].copy()}
+
+
+def bj_pcg_solve(h, b, x=None, max_iters: int = 1000, rtol: float = 1e-3, check_every: int = 0) -> dict:
+    """Preconditioned CG for A x = b from x0 = 0 (rtol defaults to the paper's accuracy bar)."""
+    import numpy as np
+    import torch
+    if x is None:
+        x = torch.empty(h.n, dtype=torch.float64, device=b.device)
+    alpha, beta, rel = np.zeros(max_iters), np.zeros(max_iters), np.zeros(max_iters)
+    o = bj_pcg_opts_t(int(max_iters), int(check_every), float(rtol))
+    r = bj_pcg_result_t(0, 0, 0.0, 0.0, 0.0, 0.0, alpha.ctypes.data_as(C.c_void_p), beta.ctypes.data_as(C.c_void_p),
+                        rel.ctypes.data_as(C.c_void_p))
+    _check(lib().bj_pcg_solve(h.ptr, _dptr(b, torch.float64, h.n), _dptr(x, torch.float64, h.n), C.byref(o), C.byref(r)))
+    k = r.iters
+    nb = k - 1 if (k > 0 and r.converged) else k
+    return {"x": x, "iters": k, "converged": bool(r.converged), "relres": r.relres, "true_relres": r.true_relres,
+            "lmin": r.lmin, "lmax": r.lmax, "alpha": alpha[:k].copy(), "beta": beta[:max(nb, 0)].copy(),
+            "relres_hist": rel[:k].copy()}
 
 
 def bj_seeded_vector(h, seed: int, v=None):

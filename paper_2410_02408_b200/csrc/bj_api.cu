@@ -136,6 +136,7 @@ static void free_handle(bj_handle_s* h)
 {
     if (!h) return;
     lanczos_free(h);
+    pcg_free(h);
     if (h->slab) {
         if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
         else cudaFree(h->slab);
@@ -379,6 +380,14 @@ int bj_op_apply(bj_handle_t h, const double* x, double* y)
     BJ_CHECK_H(h);
     if (!x || !y) return BJ_ERR_INVALID_ARG;
     return op_apply_device(h, x, y);
+}
+
+int bj_pcg_solve(bj_handle_t h, const double* b_dev, double* x_dev, const bj_pcg_opts_t* o, bj_pcg_result_t* res)
+{
+    if (!h || h->failed || !b_dev || !x_dev || !o || !res || o->max_iters < 1 || b_dev == x_dev) return BJ_ERR_INVALID_ARG;
+    const int rc = pcg_run(h, b_dev, x_dev, o, res);
+    if (rc != BJ_OK) return rc;
+    return resolve_spans(h);
 }
 
 int bj_seeded_vector(bj_handle_t h, uint64_t seed, double* v)

@@ -105,6 +105,11 @@ struct bj_handle_s {
     // Lanczos
     bj::LanczosWs lz;
 
+    // PCG workspace (bj_pcg.cu): r, z, p, q and the device scalars, allocated by the first bj_pcg_solve
+    double* pcg_vec = nullptr;
+    double* pcg_scal = nullptr;
+    int pcg_cap_iters = 0;
+
     // e2e staging
     double* stage_in = nullptr;
     double* stage_out = nullptr;
@@ -164,6 +169,12 @@ int spmv_stream_finish(bj_handle_s* h, int max_tile);  // stage capacity and cou
 int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* r);
 void lanczos_free(bj_handle_s* h);
 int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
+// k-th smallest eigenvalue (k = 0 .. m-1) of the symmetric tridiagonal (diag a[0..m-1], off-diagonal e[0..m-2]), bisection
+double tridiag_eig_k(int m, const double* a, const double* e, int k);
+
+// preconditioned CG (bj_pcg.cu)
+int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* r);
+void pcg_free(bj_handle_s* h);
 
 int env_int(const char* name, int dflt);  // tuning knobs BJ_* (read at setup / launch)
 

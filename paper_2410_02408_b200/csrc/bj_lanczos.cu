@@ -15,6 +15,7 @@
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
 #include "bj_lanczos_fuse.cuh"
+#include "bj_reduce.cuh"
 
 namespace bj {
 
@@ -32,47 +33,6 @@ __global__ void seeded_vector_kernel(uint64_t seed, int64_t n, double* __restric
         const double u = (double)(mix64(seed, (uint64_t)i) >> 11) * (1.0 / 9007199254740992.0);
         v[i] = 2.0 * u - 1.0;
     }
-}
-
-// fixed-order block reduction: shuffle tree inside each warp, then warp 0 adds the warp sums in order
-__device__ __forceinline__ double block_sum(double v, double* sh)
-{
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    __syncthreads();
-    if (lane == 0) sh[warp] = v;
-    __syncthreads();
-    double s = 0.0;
-    if (threadIdx.x == 0)
-        for (int q = 0; q < (int)(blockDim.x >> 5); ++q) s += sh[q];
-    return s;  // valid on thread 0
-}
-
-struct Chunk {
-    int64_t lo, hi;
-};
-__device__ __forceinline__ Chunk my_chunk(int64_t n)
-{
-    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
-    Chunk c;
-    c.lo = (int64_t)blockIdx.x * per;
-    c.hi = c.lo + per < n ? c.lo + per : n;
-    if (c.lo > n) c.lo = n;
-    return c;
-}
-
-// Every CTA of a consumer kernel re-sums the producer's per-CTA partials in the same fixed order, so all
-// CTAs hold the identical scalar without a separate finalize launch (deterministic, no atomics).
-__device__ __forceinline__ double reduce_partials(const double* __restrict__ part, int nparts, double* sh)
-{
-    double s = 0.0;
-    for (int p = threadIdx.x; p < nparts; p += blockDim.x) s += part[p];
-    s = block_sum(s, sh);
-    __syncthreads();
-    if (threadIdx.x == 0) sh[0] = s;
-    __syncthreads();
-    return sh[0];
 }
 
 // P[cta] = sum over the CTA's chunk of a[i] * b[i]
@@ -310,7 +270,7 @@ static int negcount(int m, const double* a, const double* e, double x)
     return cnt;
 }
 
-static double eig_k(int m, const double* a, const double* e, int k)
+double tridiag_eig_k(int m, const double* a, const double* e, int k)
 {
     double lo = a[0], hi = a[0];
     for (int i = 0; i < m; ++i) {
@@ -457,8 +417,8 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     const int me = done[1];
     if (me < 1) return BJ_ERR_CUDA;
     res->iters_done = me;
-    res->lmin = eig_k(me, a.data(), b.data(), 0);
-    res->lmax = eig_k(me, a.data(), b.data(), me - 1);
+    res->lmin = tridiag_eig_k(me, a.data(), b.data(), 0);
+    res->lmax = tridiag_eig_k(me, a.data(), b.data(), me - 1);
     res->res_min = fabs(b[me - 1]) * last_comp(me, a.data(), b.data(), res->lmin);
     res->res_max = fabs(b[me - 1]) * last_comp(me, a.data(), b.data(), res->lmax);
     if (res->alpha_host) std::copy(a.begin(), a.begin() + me, res->alpha_host);

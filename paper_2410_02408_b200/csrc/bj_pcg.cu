@@ -1,0 +1,312 @@
+// Preconditioned conjugate gradients: the classical stand-in for the solve stage
+// that follows the preconditioning path, built from the path's own kernels --
+// q = A p is the CSR SpMV (a6), z = M^-1 r is the batched block solve pair (a5) -- plus the vector
+// kernels below.  Textbook Hestenes-Stiefel ordering from x_0 = 0:
+//   r = b; z = M^-1 r; p = z; rho = r.z
+//   repeat: q = A p; a = rho / (p.q); x += a p; r -= a q; stop if ||r|| / ||b|| <= rtol;
+//           z = M^-1 r; rho' = r.z; bt = rho' / rho; p = z + bt p; rho = rho'
+// Every scalar (rho, p.q, ||r||^2, a, bt, the stop flag) stays in device memory: a kernel that needs one
+// re-sums the producer's per-CTA partials in a fixed order (bj_reduce.cuh), so the loop has no host
+// synchronisation except a poll of the stop flag every `check_every` iterations.
+// Reported: the paper's accuracy metric ||Ax - b|| / ||b|| recomputed from x, and the
+// extreme Ritz values of M^-1 A from the CG coefficients (CG-Lanczos equivalence).
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "bj_device.cuh"
+#include "bj_internal.cuh"
+#include "bj_reduce.cuh"
+
+namespace bj {
+
+namespace {
+
+// device scalar slots
+enum { S_BB = 0, S_COUNT = 8 };
+// int flags: [0] stop, [1] iterations done, [2] converged
+
+// r = b; x = 0; P0[cta] = partial of b.b
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_init_kernel(int64_t n, const double* __restrict__ b, double* __restrict__ r, double* __restrict__ x,
+                double* __restrict__ P0)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const Chunk c = my_chunk(n);
+    double s = 0.0;
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
+        const double bi = b[i];
+        r[i] = bi;
+        x[i] = 0.0;
+        s = fma(bi, bi, s);
+    }
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) P0[blockIdx.x] = s;
+}
+
+// bb = sum P0 (kept in scal[S_BB]); zero right-hand side stops the run; p = z; PR[cta] = partial of r.z
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_start_kernel(int64_t n, const double* __restrict__ r, const double* __restrict__ z, double* __restrict__ p,
+                 const double* __restrict__ P0, int nparts, double* __restrict__ scal, double* __restrict__ PR,
+                 int* __restrict__ flags)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const double bb = reduce_partials(P0, nparts, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        scal[S_BB] = bb;
+        if (!(bb > 0.0)) flags[0] = 1;
+    }
+    if (!(bb > 0.0)) return;
+    const Chunk c = my_chunk(n);
+    double s = 0.0;
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
+        const double zi = z[i];
+        p[i] = zi;
+        s = fma(r[i], zi, s);
+    }
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) PR[blockIdx.x] = s;
+}
+
+// PQ[cta] = partial of p.q
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_pq_kernel(int64_t n, const double* __restrict__ p, const double* __restrict__ q, double* __restrict__ PQ,
+              const int* __restrict__ flags)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    if (flags[0]) return;
+    const Chunk c = my_chunk(n);
+    double s = 0.0;
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) s = fma(p[i], q[i], s);
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) PQ[blockIdx.x] = s;
+}
+
+// a = (sum PR) / (sum PQ); x += a p; r -= a q; PRR[cta] = partial of r.r; CTA 0 records alpha[k]
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_update_kernel(int64_t n, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ p,
+                  const double* __restrict__ q, const double* __restrict__ PR, const double* __restrict__ PQ,
+                  int nparts, int k, double* __restrict__ alpha, double* __restrict__ PRR, const int* __restrict__ flags)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    if (flags[0]) return;
+    const double rho = reduce_partials(PR, nparts, sh);
+    const double pq = reduce_partials(PQ, nparts, sh);
+    const double a = rho / pq;
+    if (blockIdx.x == 0 && threadIdx.x == 0) alpha[k] = a;
+    const Chunk c = my_chunk(n);
+    double s = 0.0;
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
+        x[i] = fma(a, p[i], x[i]);
+        const double ri = r[i] - a * q[i];
+        r[i] = ri;
+        s = fma(ri, ri, s);
+    }
+    __syncthreads();
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) PRR[blockIdx.x] = s;
+}
+
+// relres_k = sqrt(sum PRR / bb): CTA 0 records it and the iteration count; all CTAs stop together when it is
+// <= rtol.  Otherwise PR2[cta] = partial of r.z (z = M^-1 r of the updated residual).
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_rz_kernel(int64_t n, const double* __restrict__ r, const double* __restrict__ z, const double* __restrict__ PRR,
+              int nparts, const double* __restrict__ scal, double rtol, int k, double* __restrict__ relres,
+              double* __restrict__ PR2, int* __restrict__ flags)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    if (flags[0]) return;
+    const double rr = reduce_partials(PRR, nparts, sh);
+    const double rel = sqrt(rr / scal[S_BB]);
+    const bool stop = rel <= rtol;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        relres[k] = rel;
+        flags[1] = k + 1;
+        if (stop) { flags[0] = 1; flags[2] = 1; }
+    }
+    if (stop) return;
+    const Chunk c = my_chunk(n);
+    double s = 0.0;
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) s = fma(r[i], z[i], s);
+    __syncthreads();
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) PR2[blockIdx.x] = s;
+}
+
+// bt = (sum PR2) / (sum PR); p = z + bt p; CTA 0 records beta[k]
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_direction_kernel(int64_t n, double* __restrict__ p, const double* __restrict__ z, const double* __restrict__ PR,
+                     const double* __restrict__ PR2, int nparts, int k, double* __restrict__ beta,
+                     const int* __restrict__ flags)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    if (flags[0]) return;
+    const double rho = reduce_partials(PR, nparts, sh);
+    const double rho_new = reduce_partials(PR2, nparts, sh);
+    const double bt = rho_new / rho;
+    if (blockIdx.x == 0 && threadIdx.x == 0) beta[k] = bt;
+    const Chunk c = my_chunk(n);
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) p[i] = fma(bt, p[i], z[i]);
+}
+
+// PD[cta] = partial of ||q - b||^2  (q = A x)
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_residual_kernel(int64_t n, const double* __restrict__ q, const double* __restrict__ b, double* __restrict__ PD)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const Chunk c = my_chunk(n);
+    double s = 0.0;
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
+        const double d = q[i] - b[i];
+        s = fma(d, d, s);
+    }
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) PD[blockIdx.x] = s;
+}
+
+}  // namespace
+
+void pcg_free(bj_handle_s* h)
+{
+    if (h->pcg_vec) { h->workspace_bytes -= (int64_t)4 * h->n * (int64_t)sizeof(double); cudaFree(h->pcg_vec); }
+    cudaFree(h->pcg_scal);
+    h->pcg_vec = nullptr;
+    h->pcg_scal = nullptr;
+    h->pcg_cap_iters = 0;
+}
+
+int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* res)
+{
+    const int64_t n = h->n;
+    const int m = o->max_iters;
+    const int check = o->check_every > 0 ? o->check_every : 16;
+    const double rtol = o->rtol > 0.0 ? o->rtol : 0.0;
+    cudaStream_t st = h->stream;
+
+    // workspace: r, z, p, q; scalars, six partial arrays, alpha / beta / relres, flags
+    if (!h->pcg_vec) {
+        BJ_CUDA(cudaMalloc((void**)&h->pcg_vec, (size_t)4 * n * sizeof(double)));
+        h->workspace_bytes += (int64_t)4 * n * (int64_t)sizeof(double);
+    }
+    if (h->pcg_cap_iters < m) {
+        cudaFree(h->pcg_scal);
+        h->pcg_scal = nullptr;
+        h->pcg_cap_iters = 0;
+        BJ_CUDA(cudaMalloc((void**)&h->pcg_scal, sizeof(double) * (S_COUNT + 6 * (size_t)kMaxPartials + 3 * (size_t)m + 8)));
+        h->pcg_cap_iters = m;
+    }
+    double* r = h->pcg_vec;
+    double* z = r + n;
+    double* p = z + n;
+    double* q = p + n;
+    double* scal = h->pcg_scal;
+    double* P0 = scal + S_COUNT;
+    double* PRa = P0 + kMaxPartials;
+    double* PRb = PRa + kMaxPartials;
+    double* PQ = PRb + kMaxPartials;
+    double* PRR = PQ + kMaxPartials;
+    double* PD = PRR + kMaxPartials;
+    double* alpha = PD + kMaxPartials;
+    double* beta = alpha + h->pcg_cap_iters;
+    double* relres = beta + h->pcg_cap_iters;
+    int* flags = reinterpret_cast<int*>(relres + h->pcg_cap_iters);
+    BJ_CUDA(cudaMemsetAsync(scal, 0, sizeof(double) * S_COUNT, st));
+    BJ_CUDA(cudaMemsetAsync(alpha, 0, sizeof(double) * (3 * (size_t)h->pcg_cap_iters + 8), st));
+
+    const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
+    const bool pdl = h->pdl;
+    cudaError_t e = cudaSuccess;
+    int rc = BJ_OK;
+#define BJ_LAUNCH(kernel, ...)                                                                  \
+    do {                                                                                        \
+        e = launch_kernel(kernel, dim3(G), dim3(kReduceThreads), 0, st, pdl, __VA_ARGS__);      \
+        if (e != cudaSuccess) { set_cuda_error(e, #kernel); return BJ_ERR_CUDA; }               \
+        h->launches++;                                                                          \
+    } while (0)
+    auto spmv = [&](const double* in, double* out) {
+        return h->spmv_kernel == 1 ? launch_spmv_stream(h, in, out, false) : launch_spmv_vector(h, in, out);
+    };
+
+    BJ_LAUNCH(pcg_init_kernel, n, b, r, x, P0);
+    rc = launch_solve(h, 2, r, z);  // z = M^-1 r  (b = 0: copy)
+    if (rc != BJ_OK) return rc;
+    BJ_LAUNCH(pcg_start_kernel, n, (const double*)r, (const double*)z, p, (const double*)P0, G, scal, PRa, flags);
+
+    int hflags[4] = {0, 0, 0, 0};
+    double* PR = PRa;   // partials of the current rho = r.z
+    double* PR2 = PRb;  // partials of the next one
+    for (int k = 0; k < m; ++k) {
+        rc = spmv(p, q);  // q = A p
+        if (rc != BJ_OK) return rc;
+        BJ_LAUNCH(pcg_pq_kernel, n, (const double*)p, (const double*)q, PQ, (const int*)flags);
+        BJ_LAUNCH(pcg_update_kernel, n, x, r, (const double*)p, (const double*)q, (const double*)PR, (const double*)PQ, G, k,
+                  alpha, PRR, (const int*)flags);
+        rc = launch_solve(h, 2, r, z);  // z = M^-1 r
+        if (rc != BJ_OK) return rc;
+        BJ_LAUNCH(pcg_rz_kernel, n, (const double*)r, (const double*)z, (const double*)PRR, G, (const double*)scal, rtol, k,
+                  relres, PR2, flags);
+        BJ_LAUNCH(pcg_direction_kernel, n, p, (const double*)z, (const double*)PR, (const double*)PR2, G, k, beta,
+                  (const int*)flags);
+        std::swap(PR, PR2);
+        if ((k + 1) % check == 0 && k + 1 < m) {
+            BJ_CUDA(cudaMemcpyAsync(hflags, flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+            BJ_CUDA(cudaStreamSynchronize(st));
+            if (hflags[0]) break;
+        }
+    }
+    // the paper's metric from x itself: ||A x - b|| / ||b||
+    rc = spmv(x, q);
+    if (rc != BJ_OK) return rc;
+    BJ_LAUNCH(pcg_residual_kernel, n, (const double*)q, b, PD);
+#undef BJ_LAUNCH
+
+    std::vector<double> ha(m), hb(m), hr(m), hpd(G);
+    double hscal[S_COUNT];
+    BJ_CUDA(cudaMemcpyAsync(ha.data(), alpha, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hb.data(), beta, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hr.data(), relres, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hpd.data(), PD, sizeof(double) * G, cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hscal, scal, sizeof(hscal), cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hflags, flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaStreamSynchronize(st));
+
+    const int it = hflags[1];
+    res->iters = it;
+    res->converged = hflags[2];
+    res->relres = it > 0 ? hr[it - 1] : 0.0;
+    double dd = 0.0;
+    for (int g = 0; g < G; ++g) dd += hpd[g];
+    res->true_relres = hscal[S_BB] > 0.0 ? sqrt(dd / hscal[S_BB]) : 0.0;
+    res->lmin = res->lmax = 0.0;
+    // CG-Lanczos: T = tridiag(e; d) with d_0 = 1/a_0, d_j = 1/a_j + bt_{j-1}/a_{j-1}, e_j = sqrt(bt_j)/a_j
+    const int nb = (it > 0 && hflags[2]) ? it - 1 : it;  // a run stopped by rtol has one beta fewer
+    const int kt = std::min(it, nb + 1);
+    if (kt >= 1) {
+        std::vector<double> d(kt), off(kt > 1 ? kt - 1 : 1);
+        for (int j = 0; j < kt; ++j) d[j] = 1.0 / ha[j] + (j > 0 ? hb[j - 1] / ha[j - 1] : 0.0);
+        for (int j = 0; j + 1 < kt; ++j) off[j] = sqrt(hb[j] > 0.0 ? hb[j] : 0.0) / ha[j];
+        res->lmin = tridiag_eig_k(kt, d.data(), off.data(), 0);
+        res->lmax = tridiag_eig_k(kt, d.data(), off.data(), kt - 1);
+    }
+    if (res->alpha_host) std::copy(ha.begin(), ha.begin() + it, res->alpha_host);
+    if (res->beta_host) std::copy(hb.begin(), hb.begin() + std::max(nb, 0), res->beta_host);
+    if (res->relres_host) std::copy(hr.begin(), hr.begin() + it, res->relres_host);
+    return BJ_OK;
+}
+
+}  // namespace bj
