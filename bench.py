@@ -328,15 +328,35 @@ def main():
                 dt = time.perf_counter() - t0
                 kap[name] = {"kappa_est": r["kappa"], "lmin": r["lmin"], "lmax": r["lmax"], "iters": r["iters_done"],
                              "res_min": r["res_min"], "res_max": r["res_max"], "seconds": dt}
-            r = B.bj_cond_estimate_ex(h, m, reorth=False)
+            mf = max(m, 200)  # long enough that the one host synchronisation at the end does not matter
+            r = B.bj_cond_estimate_ex(h, mf, reorth=False)
+            torch.cuda.synchronize()
             t0 = time.perf_counter()
-            r = B.bj_cond_estimate_ex(h, m, reorth=False)
+            r = B.bj_cond_estimate_ex(h, mf, reorth=False)
             dt = time.perf_counter() - t0
             kap["fast_mode"] = {"kappa_est": r["kappa"], "iters": r["iters_done"], "seconds": dt,
                                 "lanczos_iters_per_s": r["iters_done"] / dt}
             kap["predicted_hhl_gain_kappa_sq"] = (kap["A"]["kappa_est"] / kap[f"bj{b}"]["kappa_est"]) ** 2
             line["kappa"] = kap
             B.bj_destroy(h0)
+
+            # ---- PCG to the paper's residual bar 1e-3 --------------
+            rhs = B.bj_seeded_vector(h, 17)
+            pcg = {"rtol": 1e-3}
+            h0 = B.bj_setup(rp, ci, val, 0)
+            for name, hh, cap in ((f"bj{b}", h, 3000), ("A", h0, 1000)):
+                B.bj_pcg_solve(hh, rhs, max_iters=4, rtol=0.0)  # workspace allocation outside the timed call
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                pr = B.bj_pcg_solve(hh, rhs, max_iters=cap, rtol=1e-3)
+                torch.cuda.synchronize()
+                dt = time.perf_counter() - t0
+                pcg[name] = {"iters": pr["iters"], "converged": pr["converged"], "ms": 1e3 * dt,
+                             "us_per_iter": 1e6 * dt / max(pr["iters"], 1), "true_relres": pr["true_relres"],
+                             "relres": pr["relres"], "max_iters": cap,
+                             "kappa_cg": (pr["lmax"] / pr["lmin"]) if pr["lmin"] > 0 else None}
+            B.bj_destroy(h0)
+            line["pcg"] = pcg
 
             # ---- CPU oracle on the host cores (reported baseline, not the target) -------------------------
             v, reps, cores = time_oracle(A, b, args.cpu_budget_s)

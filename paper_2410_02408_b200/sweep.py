@@ -6,7 +6,7 @@ bj_op_apply, bj_cond_estimate_ex -- and picks the b that minimises the predicted
 kappa_est(b)^2 (the paper's O(log n_b kappa^2)), ties broken by the cheaper apply.
 Everything runs through the C ABI; nothing here touches the oracle.
 
-    python -m paper_2410_02408_b200.sweep --config 2 [--scale full] [--iters 50] [--long-iters 0]
+    python -m paper_2410_02408_b200.sweep --config 2 [--scale full] [--iters 50] [--long-iters 0] [--pcg-rtol 1e-3]
 """
 from __future__ import annotations
 
@@ -18,7 +18,7 @@ DEFAULT_BLOCKS = (1, 2, 3, 4, 8, 16, 24, 32)
 
 
 def sweep(rp, ci, val, blocks=DEFAULT_BLOCKS, iters: int = 50, reorth: bool = True, apply_steps: int = 200,
-          long_iters: int = 0) -> dict:
+          long_iters: int = 0, pcg_rtol: float = 0.0, pcg_max_iters: int = 2000) -> dict:
     """rp/ci/val: CUDA CSR tensors.  Returns {"rows": [...], "kappa_A": ..., "best_b": ...}."""
     import torch
     from . import binding as B
@@ -65,6 +65,16 @@ def sweep(rp, ci, val, blocks=DEFAULT_BLOCKS, iters: int = 50, reorth: bool = Tr
                "factor_bytes": B.bj_get_info(h)["factor_bytes"]}
         if long_iters:
             row["kappa_est_long"] = B.bj_cond_estimate_ex(h, long_iters, reorth=False)["kappa"]
+        if pcg_rtol > 0.0:
+            # the classical stand-in for the solve stage (bj_pcg_solve): iterations and time to the residual bar
+            rhs = B.bj_seeded_vector(h, 17)
+            B.bj_pcg_solve(h, rhs, max_iters=8, rtol=0.0)  # allocate the workspace outside the timed call
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            pr = B.bj_pcg_solve(h, rhs, max_iters=pcg_max_iters, rtol=pcg_rtol)
+            torch.cuda.synchronize()
+            row.update({"pcg_iters": pr["iters"], "pcg_ms": 1e3 * (time.perf_counter() - t0), "pcg_converged": pr["converged"],
+                        "pcg_true_relres": pr["true_relres"]})
         out["rows"].append(row)
         B.bj_destroy(h)
     ok = [r for r in out["rows"] if "error" not in r]
@@ -83,12 +93,14 @@ def main():
     ap.add_argument("--iters", type=int, default=50)
     ap.add_argument("--long-iters", type=int, default=0)
     ap.add_argument("--blocks", default=",".join(map(str, DEFAULT_BLOCKS)))
+    ap.add_argument("--pcg-rtol", type=float, default=0.0, help="> 0: also solve A x = b by PCG to this residual (paper: 1e-3)")
     args = ap.parse_args()
     import torch
     from . import workloads as W
     A = W.build(args.config, args.scale)
     rp, ci, val = (torch.from_numpy(a).cuda() for a in (A.row_ptr, A.col_idx, A.val))
-    res = sweep(rp, ci, val, tuple(int(b) for b in args.blocks.split(",")), iters=args.iters, long_iters=args.long_iters)
+    res = sweep(rp, ci, val, tuple(int(b) for b in args.blocks.split(",")), iters=args.iters, long_iters=args.long_iters,
+                pcg_rtol=args.pcg_rtol)
     res["workload"] = A.meta.get("name")
     print(json.dumps(res))
 
