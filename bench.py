@@ -179,6 +179,8 @@ def main():
     ap.add_argument("--spmv-kernel", type=int, default=-1)
     ap.add_argument("--fuse", type=int, default=-1)
     ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e (profiling runs)")
+    ap.add_argument("--gather-envelope", type=int, default=-1,
+                    help="1: also measure the machine's gather+stream envelope for this matrix (default: only config 3)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -285,6 +287,17 @@ def main():
                          "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
             "kernels": kern, "setup_ms": float(np.median(setup_ms)),
             "factor_bytes": info["factor_bytes"]}
+
+    if args.gather_envelope == 1 or (args.gather_envelope < 0 and args.config == 3):
+        # The SpMV of a matrix with random column structure is bound by one L1 wavefront per 8-byte gather plus the
+        # matrix stream sharing the SM <-> L2 path, not by HBM: measure that envelope on this device for this mix.
+        env = B.bj_probe_gather_stream(n, nnz, 12 * nnz + 4 * (n + 1))
+        sp_us = kern.get("spmv", kern.get("spmv_solve_L", {})).get("avg_us")
+        env.update({"gathers": nnz, "stream_bytes": 12 * nnz + 4 * (n + 1), "vec_len": n, "spmv_us": sp_us,
+                    "spmv_frac_of_envelope": (env["us_both"] / sp_us) if sp_us else None,
+                    "gathers_per_clk_per_sm": nnz / (env["us_gather"] * 1e-6) / (clocks["sm_mhz"] * 1e6) / 148
+                    if clocks.get("sm_mhz") else None})
+        line["gather_envelope"] = env
 
     if not args.no_extras:
         # ---- bj_apply (a5) -----------------------------------------------------------------------------

@@ -179,6 +179,14 @@ int bj_apply_host(bj_handle_t h, const double* r_host, double* z_host);
 int bj_profile_enable(bj_handle_t h, int on);
 int bj_profile_get(bj_handle_t h, int kind, double* ms_total_host, int64_t* launches_host);
 
+/* Diagnostic (not on the operator path): the machine envelope that bounds the SpMV of matrices with random column
+ * structure (config 3), which is limited by one L1 wavefront per 8-byte gather and not by HBM.  Measures, on the
+ * current device, the microseconds of (a) `gathers` random 8-byte loads from an L2-resident vector of `vec_len`
+ * doubles, (b) `stream_bytes` streamed HBM -> shared memory by bulk async copies, (c) both in one kernel.
+ * Host out-pointers; allocates and frees its own buffers; synchronises. */
+int bj_probe_gather_stream(int64_t vec_len, int64_t gathers, int64_t stream_bytes, double* us_gather_host,
+                           double* us_stream_host, double* us_both_host);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,8 @@ KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
 EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
-           "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve"]
+           "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve",
+           "bj_probe_gather_stream"]
 
 
 class bj_csr_t(C.Structure):
@@ -91,6 +92,7 @@ def lib():
         L.bj_seeded_vector.argtypes = [vp, C.c_uint64, vp]
         L.bj_pcg_solve.argtypes = [vp, vp, vp, C.POINTER(bj_pcg_opts_t), C.POINTER(bj_pcg_result_t)]
         L.bj_release_cached_memory.argtypes = []
+        L.bj_probe_gather_stream.argtypes = [i64, i64, i64] + [C.POINTER(C.c_double)] * 3
         L.bj_profile_enable.argtypes = [vp, i32]
         L.bj_profile_get.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
         for f in EXPORTS:
@@ -263,6 +265,13 @@ def bj_seeded_vector(h, seed: int, v=None):
         v = torch.empty(h.n, dtype=torch.float64, device="cuda")
     _check(lib().bj_seeded_vector(h.ptr, seed & 0xFFFFFFFFFFFFFFFF, _dptr(v, torch.float64, h.n)))
     return v
+
+
+def bj_probe_gather_stream(vec_len: int, gathers: int, stream_bytes: int) -> dict:
+    """Microseconds of random 8-byte gathers, of a TMA stream, and of both at once (see include/bj.h)."""
+    g, s_, b = C.c_double(), C.c_double(), C.c_double()
+    _check(lib().bj_probe_gather_stream(int(vec_len), int(gathers), int(stream_bytes), C.byref(g), C.byref(s_), C.byref(b)))
+    return {"us_gather": g.value, "us_stream": s_.value, "us_both": b.value}
 
 
 def bj_release_cached_memory():
