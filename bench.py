@@ -179,6 +179,8 @@ def main():
     ap.add_argument("--spmv-kernel", type=int, default=-1)
     ap.add_argument("--fuse", type=int, default=-1)
     ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e (profiling runs)")
+    ap.add_argument("--graph", type=int, default=-1,
+                    help="1: also time the operator apply replayed from a CUDA graph (default: only config 1, launch-bound)")
     ap.add_argument("--gather-envelope", type=int, default=-1,
                     help="1: also measure the machine's gather+stream envelope for this matrix (default: only config 3)")
     args = ap.parse_args()
@@ -287,6 +289,35 @@ def main():
                          "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
             "kernels": kern, "setup_ms": float(np.median(setup_ms)),
             "factor_bytes": info["factor_bytes"]}
+
+    if args.graph == 1 or (args.graph < 0 and args.config == 1):
+        # Launch-bound sizes (config 1: 0.15 MB per apply): capture G back-to-back applies in a CUDA graph on a side
+        # stream and replay it -- the kernels, their PDL chaining and their arguments are the library's own launches.
+        G = 64
+        side = torch.cuda.Stream()
+        B.bj_set_stream(h, side)
+        with torch.cuda.stream(side):
+            for _ in range(3):
+                B.bj_op_apply(h, x, y)
+            side.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                for _ in range(G):
+                    B.bj_op_apply(h, x, y)
+            graph.replay()
+            side.synchronize()
+            reps = max(1, args.steps // G)
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(side)
+            for _ in range(reps):
+                graph.replay()
+            g1.record(side)
+            side.synchronize()
+            gus = 1e3 * g0.elapsed_time(g1) / (reps * G)
+        B.bj_set_stream(h, torch.cuda.current_stream())
+        line["graph"] = {"applies_per_graph": G, "replays": reps, "us_per_apply": gus, "applies_per_s": 1e6 / gus,
+                         "eager_us_per_apply": 1e3 * ms_per_step}
+        del graph
 
     if args.gather_envelope == 1 or (args.gather_envelope < 0 and args.config == 3):
         # The SpMV of a matrix with random column structure is bound by one L1 wavefront per 8-byte gather plus the

@@ -99,6 +99,7 @@ struct bj_handle_s {
     int64_t ntiles = 0;
     bool stream_ok = false;   // streamed kernel usable (alignment, capacity)
     bool fuse_ok = false;
+    bool fuse_group = false;  // the fused forward solve is the group-per-block one (b = 16, 24, 32)
     int num_sms = 148;
     bool pdl = true;          // chain the library's kernels with programmatic dependent launch
 

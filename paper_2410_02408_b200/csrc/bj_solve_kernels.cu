@@ -284,68 +284,6 @@ solve_stream_kernel(const SolveStreamParams p)
 // has consumed it (one bulk async copy per block, blocks padded to a stride of 32 mod 128 bytes so the
 // eight groups of a warp read different banks).  No producer warp, no CTA-wide barrier.
 // ------------------------------------------------------------------------------------------------
-template <int B, int LPB>
-struct GroupGeom {
-    static constexpr int P = B * (B + 1) / 2;
-    static constexpr int RPL = B / LPB;   // rows per lane
-    static constexpr int NBW = 32 / LPB;  // blocks per warp
-    // per-block stride in shared memory: packed size padded so that consecutive blocks start LPB * 8 bytes
-    // (mod 128) apart -- the groups of a warp then read different banks
-    static constexpr int target = (LPB * 8) % 128;
-    static constexpr int pad_bytes = ((target - (P * 8) % 128) + 128) % 128;
-    static constexpr int STRIDE = P + pad_bytes / 8;
-    static_assert(B % LPB == 0 && (P * 8) % 16 == 0 && pad_bytes % 16 == 0, "bulk copies need 16-byte granules");
-};
-
-// forward substitution on the staged forward copy (column-major packed lower, rows scaled by 1/l_ii)
-template <int B, int LPB>
-__device__ __forceinline__ void group_forward(const double* f, int l, double (&r)[B / LPB])
-{
-    constexpr int RPL = B / LPB;
-#pragma unroll
-    for (int k = 0; k < RPL; ++k) {
-        const int i = k * LPB + l;
-        r[k] *= f[i * B - i * (i - 1) / 2];
-    }
-#pragma unroll
-    for (int j = 0; j < B - 1; ++j) {
-        const int kj = j / LPB, lj = j % LPB;
-        const double vj = __shfl_sync(0xffffffffu, r[kj], lj, LPB);
-        const double* col = f + (j * B - j * (j - 1) / 2 - j) + l;  // element (i, j) at col[i - l]
-#pragma unroll
-        for (int k = kj; k < RPL; ++k) {
-            if (k == kj && lj == LPB - 1) continue;  // no row of this register row lies below j
-            double lij = col[k * LPB];
-            if (k == kj) lij = (l > lj) ? lij : 0.0;
-            r[k] = fma(-lij, vj, r[k]);
-        }
-    }
-}
-
-// backward substitution on the staged backward copy (row-major packed lower, columns scaled by 1/l_jj)
-template <int B, int LPB>
-__device__ __forceinline__ void group_backward(const double* f, int l, double (&r)[B / LPB])
-{
-    constexpr int RPL = B / LPB;
-#pragma unroll
-    for (int k = 0; k < RPL; ++k) {
-        const int i = k * LPB + l;
-        r[k] *= f[i * (i + 1) / 2 + i];
-    }
-#pragma unroll
-    for (int j = B - 1; j >= 1; --j) {
-        const int kj = j / LPB, lj = j % LPB;
-        const double vj = __shfl_sync(0xffffffffu, r[kj], lj, LPB);
-        const double* row = f + j * (j + 1) / 2 + l;  // element (j, i) at row[i - l]
-#pragma unroll
-        for (int k = 0; k <= kj; ++k) {
-            if (k == kj && lj == 0) continue;  // no row of this register row lies above j
-            double lji = (k < kj || l < lj) ? row[k * LPB] : 0.0;  // the guard also keeps the read inside row j
-            r[k] = fma(-lji, vj, r[k]);
-        }
-    }
-}
-
 struct GroupParams {
     int64_t n, nblocks, ntiles;  // a tile = the eight consecutive blocks one warp solves together
     const double* fac0;          // forward copy (DIR 0, 2) or backward copy (DIR 1)

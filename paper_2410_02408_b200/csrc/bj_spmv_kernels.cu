@@ -111,6 +111,7 @@ struct StreamParams {
     int fac_bytes;       // bytes reserved per stage for factors
     int stage_bytes;
     int su_doubles;      // doubles per su buffer
+    int su_bufs;         // number of su buffers (2; FUSE 3: one per stage)
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
     int lz;              // 1: fused Lanczos epilogue on the rows this kernel writes (FUSE 0 and 1)
@@ -123,7 +124,9 @@ __device__ __forceinline__ void consumer_bar_sync(int nthreads)
 }
 
 // LPR lanes per row; BATCH entries per lane in flight per round;
-// FUSE: 0 = SpMV only, 1 = + forward solve, thread per block (b <= 8), 2 = + forward solve, sub-warp of W lanes per block
+// FUSE: 0 = SpMV only, 1 = + forward solve, thread per block (b <= 8), 2 = + forward solve, sub-warp of W lanes per block,
+//       3 = + forward solve, group of lanes per block (bj_device.cuh), W = the compile-time block size (16, 24, 32):
+//           the solving warps rotate from tile to tile and the other warps go on to the next tile meanwhile
 template <int LPR, int BATCH, int FUSE, int W>
 __global__ void __launch_bounds__(kMaxStreamThreads)
 spmv_stream_kernel(const StreamParams p)
@@ -131,8 +134,13 @@ spmv_stream_kernel(const StreamParams p)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
     uint64_t* empty = full + p.stages;
-    double* su = reinterpret_cast<double*>(smem_raw + 128);               // 2 x su_doubles (fused only)
-    unsigned char* stage0 = smem_raw + 128 + (size_t)2 * p.su_doubles * sizeof(double);
+    // FUSE 3 geometry (unused otherwise): block size GB, GLPB lanes per block, NBW blocks per solving warp
+    constexpr int GB = FUSE == 3 ? W : 32;
+    constexpr int GLPB = GB == 32 ? 8 : 4;
+    using Geo = GroupGeom<GB, GLPB>;
+    constexpr int XB = GB + 2;  // padded block row of the su buffer
+    double* su = reinterpret_cast<double*>(smem_raw + 128);               // su_bufs x su_doubles (fused only)
+    unsigned char* stage0 = smem_raw + 128 + (size_t)p.su_bufs * p.su_doubles * sizeof(double);
     // per stage: val[cap] | fac[fac_bytes] | col[cap] | rp[rp_ints]
     auto s_val = [&](int s) { return reinterpret_cast<double*>(stage0 + (size_t)s * p.stage_bytes); };
     auto s_fac = [&](int s) { return reinterpret_cast<double*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 8); };
@@ -215,6 +223,11 @@ spmv_stream_kernel(const StreamParams p)
                     fsrc = p.fac + (r0 / p.b) * (int64_t)p.P;
                     bytes += fbytes;
                 }
+                int gblk = 0;
+                if (FUSE == 3) {
+                    gblk = (rows + GB - 1) / GB;
+                    bytes += (uint32_t)gblk * (uint32_t)(Geo::P * 8);
+                }
                 mbar_expect_tx(&full[s], bytes);
                 if (a1 > a0) {
                     bulk_g2s(dv, p.val + a0, (uint32_t)(a1 - a0) * 8u, &full[s], pol);
@@ -222,6 +235,10 @@ spmv_stream_kernel(const StreamParams p)
                 }
                 if (rq > 0) bulk_g2s(dr, p.rp + r0, (uint32_t)rq * 4u, &full[s], pol);
                 if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], pol);
+                if (FUSE == 3)  // one copy per block, padded stride: the groups of a solving warp read different banks
+                    for (int q = 0; q < gblk; ++q)
+                        bulk_g2s(s_fac(s) + (size_t)q * Geo::STRIDE, p.fac + (r0 / GB + q) * (int64_t)Geo::P, (uint32_t)(Geo::P * 8),
+                                 &full[s], pol);
             }
         }
     } else {
@@ -237,7 +254,7 @@ spmv_stream_kernel(const StreamParams p)
             const uint32_t ph = (uint32_t)((it / p.stages) & 1);
             const int64_t r0 = tile * R;
             const int rows = (int)(r0 + R <= p.n ? R : p.n - r0);
-            double* sub_u = su + (size_t)(it & 1) * p.su_doubles;
+            double* sub_u = su + (size_t)(FUSE == 3 ? it % p.su_bufs : (it & 1)) * p.su_doubles;
             mbar_wait(&full[s], ph);
             const double* sv = s_val(s);
             const int* sc = s_col(s);
@@ -279,9 +296,49 @@ spmv_stream_kernel(const StreamParams p)
                         sub_u[k * p.bs + (i - k * p.b)] = acc;
                     } else if (FUSE == 2) {
                         sub_u[i] = acc;
+                    } else if (FUSE == 3) {
+                        const int kb = i / GB;
+                        sub_u[kb * XB + (i - kb * GB)] = acc;
                     } else {
                         if (p.lz) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, acc, pa);
                         else p.y[r0 + i] = acc;
+                    }
+                }
+            }
+            if (FUSE == 3) {
+                // (B) forward substitution y = L^-1 u by ROTATING solver warps: group gq (NBW blocks) of tile `it` belongs to
+                // consumer warp (it * ngmax + gq) mod ncw.  The other warps only signal that their rows are in the su
+                // buffer (bar.arrive) and go on to the next tile; a solver waits for all rows (bar.sync), solves, writes y
+                // coalesced, and only then hands the stage back.  The stage ring orders the reuse of the su buffers.
+                constexpr int NBW = Geo::NBW;
+                constexpr int RPL = Geo::RPL;
+                const int ncw = nct >> 5, cw = warp - 1;
+                const int nblk = (rows + GB - 1) / GB;
+                const int ngroups = (nblk + NBW - 1) / NBW;
+                const int ngmax = (R / GB + NBW - 1) / NBW;
+                int myg = -1;
+                for (int gq = 0; gq < ngroups; ++gq)
+                    if ((it * ngmax + gq) % ncw == cw) myg = gq;
+                const int bar_id = 2 + it % p.su_bufs;
+                if (myg < 0) {
+                    asm volatile("bar.arrive %0, %1;" ::"r"(bar_id), "r"(nct) : "memory");
+                } else {
+                    asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nct) : "memory");
+                    const int g = lane / GLPB, l = lane % GLPB;
+                    const int blk0 = myg * NBW;
+                    double* xu = sub_u + (blk0 + g) * XB;
+                    double r[RPL];
+#pragma unroll
+                    for (int k = 0; k < RPL; ++k) r[k] = xu[k * GLPB + l];
+                    group_forward<GB, GLPB>(s_fac(s) + (size_t)(blk0 + g) * Geo::STRIDE, l, r);
+#pragma unroll
+                    for (int k = 0; k < RPL; ++k) xu[k * GLPB + l] = r[k];
+                    __syncwarp();
+#pragma unroll
+                    for (int k = 0; k < RPL; ++k) {
+                        const int e = k * 32 + lane;
+                        const int i = blk0 * GB + e;
+                        if (i < rows) p.y[r0 + i] = sub_u[(blk0 + e / GB) * XB + e % GB];
                     }
                 }
             }
@@ -385,11 +442,23 @@ void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem
     sp.stages = h->tile_stages;
     sp.ntiles = h->ntiles;
     sp.rp_ints = sp.R + 4;
-    sp.fac_bytes = fuse ? (((sp.R / sp.b) * sp.P * 8 + 15) & ~15) : 0;
+    const bool group = fuse && h->fuse_group;
+    sp.su_bufs = group ? sp.stages : 2;
+    if (group) {
+        // whole solver groups (NBW blocks of b rows, padded) so that idle lanes stay inside the buffers
+        const int lpb = sp.b == 32 ? 8 : 4, nbw = 32 / lpb;
+        const int pbytes = sp.P * 8, target = (lpb * 8) % 128;
+        const int stride = sp.P + (((target - pbytes % 128) + 128) % 128) / 8;  // GroupGeom<b, lpb>::STRIDE
+        const int slots = ((sp.R / sp.b + nbw - 1) / nbw) * nbw;
+        sp.fac_bytes = slots * stride * 8;
+        sp.su_doubles = slots * (sp.b + 2);
+    } else {
+        sp.fac_bytes = fuse ? (((sp.R / sp.b) * sp.P * 8 + 15) & ~15) : 0;
+        sp.su_doubles = !fuse ? 0 : (h->solve_kind == 1 ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : ((sp.R + 1) & ~1));
+    }
     sp.stage_bytes = (sp.cap * 12 + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
-    sp.su_doubles = !fuse ? 0 : (h->solve_kind == 1 ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : ((sp.R + 1) & ~1));
     sp.b_magic = (unsigned)(((1ull << 32) + sp.b - 1) / sp.b);
-    smem = 128 + (size_t)2 * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
+    smem = 128 + (size_t)sp.su_bufs * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
 }
 constexpr size_t kSmemTwoPerSm = 110 * 1024;
 constexpr size_t kSmemOnePerSm = 224 * 1024;
@@ -427,7 +496,19 @@ int spmv_stream_configure(bj_handle_s* h)
         if (Rf < unit) Rf = unit;
         if ((double)Rf * mean <= 1.6 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
     }
-    if (h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 0)) {
+    h->fuse_group = false;
+    const bool group_ok = h->solve_kind == 2 && (h->b == 16 || h->b == 24 || h->b == 32) && h->stream_lanes <= 4 &&
+                          (((uintptr_t)h->fac_fwd) & 15) == 0 && env_int("BJ_FUSE_GROUP", 0) != 0;
+    if (group_ok) {
+        // fused tiles hold whole solver groups (NBW blocks): the forward solve then rides on the SpMV kernel.
+        // Off by default: measured within 1 % of the unfused kernels on configs 3 and 4 (the stage is held for the
+        // solve, which costs the streaming what the saved u round trip gains).
+        const int unit = h->b * (h->b == 32 ? 4 : 8);
+        int Rf = ((R + unit / 2) / unit) * unit;
+        if (Rf < unit) Rf = unit;
+        if ((double)Rf * mean <= 2.0 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; h->fuse_group = true; }
+    }
+    if (!fuse && h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 0)) {
         // fused tiles hold whole blocks; with an odd packed size an even block count keeps every tile's factor
         // range 16-byte aligned; row pointers need the tile start to be a multiple of 4 rows
         int unit = h->b * ((h->packed % 2) ? 2 : 1);
@@ -439,7 +520,8 @@ int spmv_stream_configure(bj_handle_s* h)
     if (!fuse) R = ((R + 31) / 32) * 32;
     R = env_int("BJ_TILE_ROWS", R);
     if (fuse && h->solve_kind == 1 && (R % (kInterleave * h->b)) != 0) fuse = false;
-    if (fuse && h->solve_kind == 2 && ((R % h->b) != 0 || (((R / h->b) * h->packed) % 2) != 0)) fuse = false;
+    if (fuse && h->solve_kind == 2 && !h->fuse_group && ((R % h->b) != 0 || (((R / h->b) * h->packed) % 2) != 0)) fuse = false;
+    if (fuse && h->fuse_group && (R % h->b) != 0) { fuse = false; h->fuse_group = false; }
     if (R % 4) return BJ_OK;
     h->tile_rows = R;
     h->ntiles = (h->n + R - 1) / R;
@@ -485,7 +567,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.early_trigger = (env_int("BJ_PDL_EARLY", 0) >> 1) & 1;
     sp.lz = epi ? 1 : 0;
     sp.epi = epi ? *epi : LzEpilogue{};
-    if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the sub-warp fused path has no hook
+    if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the b > 8 fused paths have no hook
     if (epi && h->num_sms * 4 > epi->red.cap) return BJ_ERR_INVALID_ARG;
     sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
     const int threads = 32 + 32 * h->stream_warps;
@@ -493,7 +575,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     int rc = BJ_OK;
     {
         KernelScope scope(h, fuse ? BJ_K_SPMV_SOLVE_L : BJ_K_SPMV);
-        const int mode = !fuse ? 0 : (h->solve_kind == 1 ? 1 : (h->lanes == 16 ? 2 : 3));
+        const int mode = !fuse ? 0 : (h->solve_kind == 1 ? 1 : h->fuse_group ? (h->b == 16 ? 4 : h->b == 24 ? 5 : 6) : (h->lanes == 16 ? 2 : 3));
 #define BJ_CASE(L)                                                                               \
     case L:                                                                                      \
         rc = mode == 0   ? launch_stream_t<L, 8, 0, 32>(h, sp, grid, threads, smem)               \
@@ -501,10 +583,24 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
              : mode == 2 ? launch_stream_t<L, 8, 2, 16>(h, sp, grid, threads, smem)               \
                          : launch_stream_t<L, 8, 2, 32>(h, sp, grid, threads, smem);              \
         break;
-        switch (h->stream_lanes) {
-            BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
-            default: rc = BJ_ERR_INVALID_ARG;
+#define BJ_GCASE(L)                                                                              \
+    case L:                                                                                      \
+        rc = mode == 4   ? launch_stream_t<L, 8, 3, 16>(h, sp, grid, threads, smem)               \
+             : mode == 5 ? launch_stream_t<L, 8, 3, 24>(h, sp, grid, threads, smem)               \
+                         : launch_stream_t<L, 8, 3, 32>(h, sp, grid, threads, smem);              \
+        break;
+        if (mode >= 4) {
+            switch (h->stream_lanes) {
+                BJ_GCASE(1) BJ_GCASE(2) BJ_GCASE(4)
+                default: rc = BJ_ERR_INVALID_ARG;
+            }
+        } else {
+            switch (h->stream_lanes) {
+                BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
+                default: rc = BJ_ERR_INVALID_ARG;
+            }
         }
+#undef BJ_GCASE
 #undef BJ_CASE
     }
     if (rc != BJ_OK) return rc;

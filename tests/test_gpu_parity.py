@@ -308,6 +308,46 @@ def test_fused_subwarp_forward_solve_path(B, torch_, rel, monkeypatch):
         check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
 
 
+def test_operator_apply_replays_from_a_cuda_graph(B, torch_, rel):
+    """The library's launches (PDL-chained) can be captured on a side stream and replayed: bitwise the eager result."""
+    for cfg, b in ((1, 4), (4, 16)):
+        A = mat(cfg, "small")
+        h, keep = B.setup_from_host(A, b)
+        x = dev(torch_, W.seeded_vector(9, A.n))
+        y_eager = B.bj_op_apply(h, x).clone()
+        side = torch_.cuda.Stream()
+        B.bj_set_stream(h, side)
+        y = torch_.zeros_like(x)
+        with torch_.cuda.stream(side):
+            B.bj_op_apply(h, x, y)
+            side.synchronize()
+            y.zero_()
+            g = torch_.cuda.CUDAGraph()
+            with torch_.cuda.graph(g, stream=side):
+                B.bj_op_apply(h, x, y)
+                B.bj_op_apply(h, x, y)
+            side.synchronize()
+            assert not y.cpu().numpy().any()      # capture does not execute
+            g.replay()
+            side.synchronize()
+        assert np.array_equal(y.cpu().numpy(), y_eager.cpu().numpy())
+        B.bj_set_stream(h, torch_.cuda.current_stream())
+        del g
+        B.bj_destroy(h)
+
+
+def test_fused_group_forward_solve_path(B, torch_, rel, monkeypatch):
+    """b = 16 / 24 / 32: the group-per-block forward solve can ride on the SpMV tile kernel with rotating solver warps
+    (off by default: within 1 % of the unfused kernels)."""
+    monkeypatch.setenv("BJ_FUSE_GROUP", "1")
+    for cfg, b in ((4, 16), (3, 32), (2, 24), (1, 16)):
+        A = mat(cfg, "small")
+        h, keep = B.setup_from_host(A, b)
+        assert B.bj_get_info(h)["fused_forward"] == 1
+        B.bj_destroy(h)
+        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
+
+
 def test_block_size_sweep_runs_the_real_path(B, torch_):
     """a11: host-side sweep over b; kappa estimates agree with the oracle at the chosen b; b = N/.. ordering sane."""
     from paper_2410_02408_b200 import sweep
