@@ -195,6 +195,22 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     h->packed = b * (b + 1) / 2;
     cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
     h->pdl = env_int("BJ_PDL", 1) != 0;
+    {
+        Tuning& t = h->tune;
+        t.solve_warps = env_int("BJ_SOLVE_WARPS", t.solve_warps);
+        t.solve_stage_kb = env_int("BJ_SOLVE_STAGE_KB", t.solve_stage_kb);
+        t.solve_stages = env_int("BJ_SOLVE_STAGES", t.solve_stages);
+        t.solve_ctas = env_int("BJ_SOLVE_CTAS", t.solve_ctas);
+        t.solve_pair = env_int("BJ_SOLVE_PAIR", t.solve_pair);
+        t.solve_group = env_int("BJ_SOLVE_GROUP", t.solve_group);
+        t.group_stages = env_int("BJ_GROUP_STAGES", t.group_stages);
+        t.group_smem_kb = env_int("BJ_GROUP_SMEM_KB", t.group_smem_kb);
+        t.group_warps = env_int("BJ_GROUP_WARPS", t.group_warps);
+        t.group_lanes = env_int("BJ_GROUP_LANES", t.group_lanes);
+        t.pdl_early = env_int("BJ_PDL_EARLY", t.pdl_early);
+        t.ctas_per_sm = env_int("BJ_CTAS_PER_SM", t.ctas_per_sm);
+        t.lanczos_fuse = env_int("BJ_LANCZOS_FUSE", t.lanczos_fuse);
+    }
 
     auto fail = [&](int code) { free_handle(h); return code; };
 

@@ -219,6 +219,20 @@ __device__ __forceinline__ void group_backward(const double* f, int l, double (&
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Opt-in to more than 48 KB of dynamic shared memory, once per kernel AND per device (the attribute is per device).
+template <typename K>
+inline cudaError_t ensure_big_smem(K kernel, bool (&done)[64])
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (done[dev]) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+    if (e == cudaSuccess) done[dev] = true;
+    return e;
+}
+
 // launch with the programmatic-stream-serialization attribute when `pdl` is set
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,

@@ -31,6 +31,16 @@ struct Status {
     unsigned long long legal_descents;  // ... of which at the start of a non-empty row
 };
 
+// Launch-shape knobs: defaults are the measured best on B200; each can be overridden by the environment variable
+// BJ_<NAME>, read ONCE by bj_setup (sweeps re-run the setup).
+struct Tuning {
+    int solve_warps = 8, solve_stage_kb = 32, solve_stages = 2, solve_ctas = 4, solve_pair = 1;  // solve_stream_kernel
+    int solve_group = 1, group_stages = 2, group_smem_kb = 220, group_warps = 12, group_lanes = 0;  // solve_group_kernel
+    int pdl_early = 0;      // bit 0: stream solves, bit 1: stream SpMV release their dependents at entry
+    int ctas_per_sm = 4;    // wanted CTAs per SM of the SpMV tile kernel
+    int lanczos_fuse = 1;   // fast-mode Lanczos rides on the operator's kernels
+};
+
 struct ProfSpan {
     int kind;
     cudaEvent_t a, b;
@@ -102,6 +112,7 @@ struct bj_handle_s {
     bool fuse_group = false;  // the fused forward solve is the group-per-block one (b = 16, 24, 32)
     int num_sms = 148;
     bool pdl = true;          // chain the library's kernels with programmatic dependent launch
+    bj::Tuning tune;
 
     // Lanczos
     bj::LanczosWs lz;

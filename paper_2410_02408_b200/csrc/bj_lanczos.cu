@@ -349,7 +349,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         if (rc != BJ_OK) return rc;
         v0 = z.w;
     }
-    const bool fused_mode = !reorth && lanczos_fusable(h) && env_int("BJ_LANCZOS_FUSE", 1) != 0;
+    const bool fused_mode = !reorth && lanczos_fusable(h) && h->tune.lanczos_fuse != 0;
     if (!fused_mode) BJ_LAUNCH(dot_partial_kernel, G, kReduceThreads, n, v0, v0, PB);
     if (!fused_mode)
         BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, v0, vcol(0), (const double*)PB, G, 0, 0, tol,

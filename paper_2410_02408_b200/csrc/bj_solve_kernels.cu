@@ -484,11 +484,10 @@ static int launch_small(bj_handle_s* h, const double* in, double* out, const LzP
 template <int W, int DIR, int B, int NB>
 static int launch_stream_solve(bj_handle_s* h, const SolveStreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(solve_stream_kernel<W, DIR, B, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+    static bool configured[64] = {};
+    {
+        cudaError_t e = ensure_big_smem(solve_stream_kernel<W, DIR, B, NB>, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_stream_kernel)"); return BJ_ERR_CUDA; }
-        configured = true;
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR, B, NB>, threads, smem);
@@ -503,12 +502,12 @@ template <int DIR>
 static int launch_warp(bj_handle_s* h, const double* in, double* out)
 {
     const int W = h->lanes;
-    const int cwarps = std::max(1, std::min(env_int("BJ_SOLVE_WARPS", 8), 8));
+    const int cwarps = std::max(1, std::min(h->tune.solve_warps, 8));
     const int threads = 32 + 32 * cwarps;
     const int nsub = cwarps * 32 / W;
     const int copies = DIR == 2 ? 2 : 1;
     const size_t block_bytes = (size_t)h->packed * 8;
-    const int target = env_int("BJ_SOLVE_STAGE_KB", 32) * 1024;
+    const int target = h->tune.solve_stage_kb * 1024;
     int bps = (int)((target / copies + nsub * block_bytes / 2) / (nsub * block_bytes));
     bps = std::max(1, std::min(bps, kMaxBlocksPerSub));
     SolveStreamParams sp;
@@ -520,14 +519,14 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
     sp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
     sp.fac1 = h->fac_bwd;
     sp.in = in; sp.out = out;
-    sp.early_trigger = env_int("BJ_PDL_EARLY", 0) & 1;
+    sp.early_trigger = h->tune.pdl_early & 1;
     const size_t stage_bytes = (size_t)copies * sp.copy_doubles * 8;
-    int stages = std::max(2, env_int("BJ_SOLVE_STAGES", 2));
+    int stages = std::max(2, h->tune.solve_stages);
     while (stages > 2 && 128 + stages * stage_bytes > 110 * 1024) --stages;
     sp.stages = stages;
     const size_t smem = 128 + stages * stage_bytes;
-    const int per_sm = env_int("BJ_SOLVE_CTAS", 4);
-    const bool pair = bps % 2 == 0 && env_int("BJ_SOLVE_PAIR", 1) != 0;  // two blocks per sub-warp at a time
+    const int per_sm = h->tune.solve_ctas;
+    const bool pair = bps % 2 == 0 && h->tune.solve_pair != 0;  // two blocks per sub-warp at a time
     switch (h->b) {  // compile-time instances for the workloads' block sizes
         case 16: return pair ? launch_stream_solve<16, DIR, 16, 2>(h, sp, per_sm, threads, smem)
                              : launch_stream_solve<16, DIR, 16, 1>(h, sp, per_sm, threads, smem);
@@ -548,19 +547,18 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     constexpr int kGroupBlocksPerWarp = Geo::NBW;
     constexpr int kCopies = DIR == 2 ? 2 : 1;
     const size_t stage_bytes = (size_t)kCopies * kGroupBlocksPerWarp * Geo::STRIDE * 8;
-    const int stages = std::max(2, std::min(8, env_int("BJ_GROUP_STAGES", 2)));
+    const int stages = std::max(2, std::min(8, h->tune.group_stages));
     // as many warps as fit one SM's shared memory (one CTA per SM), at most 12: the bytes in flight per SM are
     // what hides the ~2 us loaded DRAM latency (throughput ~ ring bytes / (latency + one tile's solve))
-    const size_t budget = (size_t)env_int("BJ_GROUP_SMEM_KB", 220) * 1024;
+    const size_t budget = (size_t)h->tune.group_smem_kb * 1024;
     const size_t xchg_bytes = (size_t)kGroupBlocksPerWarp * (B + 2) * 8;
     int warps = (int)(budget / (stages * stage_bytes + 64 + xchg_bytes));
-    warps = std::max(1, std::min(warps, env_int("BJ_GROUP_WARPS", 12)));
+    warps = std::max(1, std::min(warps, h->tune.group_warps));
     const size_t smem = (size_t)warps * (64 + xchg_bytes + stages * stage_bytes);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(solve_group_kernel<B, LPB, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+    static bool configured[64] = {};
+    {
+        cudaError_t e = ensure_big_smem(solve_group_kernel<B, LPB, DIR>, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_group_kernel)"); return BJ_ERR_CUDA; }
-        configured = true;
     }
     GroupParams gp;
     gp.n = h->n; gp.nblocks = h->nblocks;
@@ -585,7 +583,7 @@ template <int DIR>
 static int launch_group(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
 {
     // lanes per block: small enough tiles that many warps fit one SM's shared memory (latency hiding)
-    const int lpb = env_int("BJ_GROUP_LANES", h->b == 32 ? 8 : 4);
+    const int lpb = (h->tune.group_lanes > 0 ? h->tune.group_lanes : (h->b == 32 ? 8 : 4));
     switch (h->b) {
         case 16: return lpb == 8 ? launch_group_t<16, 8, DIR>(h, in, out, pro, epi) : launch_group_t<16, 4, DIR>(h, in, out, pro, epi);
         case 24: return lpb == 8 ? launch_group_t<24, 8, DIR>(h, in, out, pro, epi) : launch_group_t<24, 4, DIR>(h, in, out, pro, epi);
@@ -597,7 +595,7 @@ static int launch_group(bj_handle_s* h, const double* in, double* out, const LzP
 
 static bool use_group_kernel(const bj_handle_s* h)
 {
-    return (h->b == 16 || h->b == 24 || h->b == 32) && env_int("BJ_SOLVE_GROUP", 1) != 0 &&
+    return (h->b == 16 || h->b == 24 || h->b == 32) && h->tune.solve_group != 0 &&
            (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0;
 }
 

@@ -411,11 +411,10 @@ spmv_stream_kernel(const StreamParams p)
 template <int LPR, int BATCH, int FUSE, int W>
 int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(spmv_stream_kernel<LPR, BATCH, FUSE, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+    static bool configured[64] = {};
+    {
+        cudaError_t e = ensure_big_smem(spmv_stream_kernel<LPR, BATCH, FUSE, W>, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
-        configured = true;
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_stream_kernel<LPR, BATCH, FUSE, W>, threads, smem);
@@ -564,14 +563,14 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     fill_layout(h, fuse, sp, smem);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
-    sp.early_trigger = (env_int("BJ_PDL_EARLY", 0) >> 1) & 1;
+    sp.early_trigger = (h->tune.pdl_early >> 1) & 1;
     sp.lz = epi ? 1 : 0;
     sp.epi = epi ? *epi : LzEpilogue{};
     if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the b > 8 fused paths have no hook
     if (epi && h->num_sms * 4 > epi->red.cap) return BJ_ERR_INVALID_ARG;
     sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
     const int threads = 32 + 32 * h->stream_warps;
-    const int grid = env_int("BJ_CTAS_PER_SM", 4);  // wanted CTAs per SM; clipped to the real occupancy at launch
+    const int grid = h->tune.ctas_per_sm;  // wanted CTAs per SM; clipped to the real occupancy at launch
     int rc = BJ_OK;
     {
         KernelScope scope(h, fuse ? BJ_K_SPMV_SOLVE_L : BJ_K_SPMV);
