@@ -159,6 +159,7 @@ struct KernelScope {
 
 struct LzPrologue;
 struct LzEpilogue;
+struct PcgHook;
 
 // setup (bj_setup_kernels.cu)
 int launch_validate(bj_handle_s* h);
@@ -168,12 +169,15 @@ int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nn
 // solves (bj_solve_kernels.cu): dir 0 = forward (L^-1), 1 = backward (L^-T), 2 = both (apply)
 // pro (dir 1 only) / epi (dir 0 only): fused Lanczos hooks of bj_lanczos_fuse.cuh, null for a plain solve
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro = nullptr,
-                 const LzEpilogue* epi = nullptr);
+                 const LzEpilogue* epi = nullptr, const PcgHook* pcg = nullptr);  // pcg: dir 2 only (bj_pcg_fuse.cuh)
 bool lanczos_fusable(const bj_handle_s* h);  // the handle's solve / SpMV kernels carry the fused Lanczos hooks
 
 // SpMV (bj_spmv_kernels.cu)
 int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);
-int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi = nullptr);
+struct LzReduce;
+// epi: fused Lanczos epilogue; dot_with / dot_red: per-CTA partials of dot_with . y finished into *dot_red->out (unfused only)
+int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi = nullptr,
+                       const double* dot_with = nullptr, const LzReduce* dot_red = nullptr);
 int spmv_stream_configure(bj_handle_s* h);  // decide tile rows / fusion, launch tile_nnz_kernel (async)
 int spmv_stream_finish(bj_handle_s* h, int max_tile);  // stage capacity and count, sets stream_ok
 

@@ -17,6 +17,7 @@
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
+#include "bj_pcg_fuse.cuh"
 #include "bj_reduce.cuh"
 
 namespace bj {
@@ -24,7 +25,7 @@ namespace bj {
 namespace {
 
 // device scalar slots
-enum { S_BB = 0, S_COUNT = 8 };
+enum { S_BB = 0, S_RHO_A = 1, S_RHO_B = 2, S_PQ = 3, S_RR = 4, S_COUNT = 8 };
 // int flags: [0] stop, [1] iterations done, [2] converged
 
 // r = b; x = 0; P0[cta] = partial of b.b
@@ -179,6 +180,42 @@ pcg_residual_kernel(int64_t n, const double* __restrict__ q, const double* __res
     if (threadIdx.x == 0) PD[blockIdx.x] = s;
 }
 
+// fused path: out[0] = sum PR (one CTA): the first rho as a finished scalar
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_scalar_kernel(const double* __restrict__ PR, int nparts, double* __restrict__ out, const int* __restrict__ flags)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    if (flags[0]) return;
+    const double s = reduce_partials(PR, nparts, sh);
+    if (threadIdx.x == 0) out[0] = s;
+}
+
+// fused path, K3: stopping test on sqrt(rr / bb) (CTA 0 records relres[k] and the iteration count), then
+// bt = rho_new / rho, p = z + bt p (CTA 0 records beta[k]).  All scalars are finished sums in scal[].
+__global__ void __launch_bounds__(kReduceThreads)
+pcg_direction_fused_kernel(int64_t n, double* __restrict__ p, const double* __restrict__ z, const double* __restrict__ scal,
+                           int rho_cur, int rho_new, double rtol, int k, double* __restrict__ relres,
+                           double* __restrict__ beta, int* __restrict__ flags)
+{
+    pdl_trigger();
+    pdl_wait();
+    if (flags[0]) return;
+    const double rel = sqrt(scal[S_RR] / scal[S_BB]);
+    const bool stop = rel <= rtol;
+    const double bt = scal[rho_new] / scal[rho_cur];
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        relres[k] = rel;
+        flags[1] = k + 1;
+        if (stop) { flags[0] = 1; flags[2] = 1; }
+        else beta[k] = bt;
+    }
+    if (stop) return;
+    const Chunk c = my_chunk(n);
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) p[i] = fma(bt, p[i], z[i]);
+}
+
 }  // namespace
 
 void pcg_free(bj_handle_s* h)
@@ -198,7 +235,8 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     const double rtol = o->rtol > 0.0 ? o->rtol : 0.0;
     cudaStream_t st = h->stream;
 
-    // workspace: r, z, p, q; scalars, six partial arrays, alpha / beta / relres, flags
+    // workspace: r, z, p, q; scalars, six partial arrays, alpha / beta / relres, flags, three partial arrays of the fused path
+    const size_t fcap = (size_t)std::max<int64_t>(kMaxPartials, (h->nblocks + 127) / 128 + 1);
     if (!h->pcg_vec) {
         BJ_CUDA(cudaMalloc((void**)&h->pcg_vec, (size_t)4 * n * sizeof(double)));
         h->workspace_bytes += (int64_t)4 * n * (int64_t)sizeof(double);
@@ -207,7 +245,7 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
         cudaFree(h->pcg_scal);
         h->pcg_scal = nullptr;
         h->pcg_cap_iters = 0;
-        BJ_CUDA(cudaMalloc((void**)&h->pcg_scal, sizeof(double) * (S_COUNT + 6 * (size_t)kMaxPartials + 3 * (size_t)m + 8)));
+        BJ_CUDA(cudaMalloc((void**)&h->pcg_scal, sizeof(double) * (S_COUNT + 6 * (size_t)kMaxPartials + 3 * (size_t)m + 8 + 3 * fcap)));
         h->pcg_cap_iters = m;
     }
     double* r = h->pcg_vec;
@@ -224,7 +262,8 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     double* alpha = PD + kMaxPartials;
     double* beta = alpha + h->pcg_cap_iters;
     double* relres = beta + h->pcg_cap_iters;
-    int* flags = reinterpret_cast<int*>(relres + h->pcg_cap_iters);
+    int* flags = reinterpret_cast<int*>(relres + h->pcg_cap_iters);  // 16 ints: [0..2] flags, [4..6] tickets of the fused path
+    double* FP = relres + h->pcg_cap_iters + 8;                    // 3 x fcap partials of the fused path
     BJ_CUDA(cudaMemsetAsync(scal, 0, sizeof(double) * S_COUNT, st));
     BJ_CUDA(cudaMemsetAsync(alpha, 0, sizeof(double) * (3 * (size_t)h->pcg_cap_iters + 8), st));
 
@@ -248,9 +287,40 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     BJ_LAUNCH(pcg_start_kernel, n, (const double*)r, (const double*)z, p, (const double*)P0, G, scal, PRa, flags);
 
     int hflags[4] = {0, 0, 0, 0};
+    // Fused iteration (bj_pcg_fuse.cuh): needs the tile SpMV (dot hook) and a solve kernel that carries the PCG hook
+    const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && env_int("BJ_PCG_FUSE", 1) != 0;
+    if (fused) {
+        unsigned* tickets = reinterpret_cast<unsigned*>(flags + 4);
+        LzReduce red_pq{FP, scal + S_PQ, tickets + 0, (int)fcap};
+        PcgHook hook;
+        hook.x = x; hook.p = p; hook.r = r; hook.q = q; hook.pq = scal + S_PQ; hook.alpha = alpha; hook.flags = flags;
+        hook.red_rr = LzReduce{FP + fcap, scal + S_RR, tickets + 1, (int)fcap};
+        int rho_cur = S_RHO_A, rho_new = S_RHO_B;
+        e = launch_kernel(pcg_scalar_kernel, dim3(1), dim3(kReduceThreads), 0, st, pdl, (const double*)PRa, G, scal + rho_cur,
+                          (const int*)flags);
+        if (e != cudaSuccess) { set_cuda_error(e, "pcg_scalar_kernel"); return BJ_ERR_CUDA; }
+        h->launches++;
+        for (int k = 0; k < m; ++k) {
+            rc = launch_spmv_stream(h, p, q, false, nullptr, p, &red_pq);  // K1: q = A p, p.q
+            if (rc != BJ_OK) return rc;
+            hook.rho = scal + rho_cur;
+            hook.red_rz = LzReduce{FP + 2 * fcap, scal + rho_new, tickets + 2, (int)fcap};
+            hook.k = k;
+            rc = launch_solve(h, 2, nullptr, z, nullptr, nullptr, &hook);  // K2: x, r updates, z = M^-1 r, r.r, r.z
+            if (rc != BJ_OK) return rc;
+            BJ_LAUNCH(pcg_direction_fused_kernel, n, p, (const double*)z, (const double*)scal, rho_cur, rho_new, rtol, k, relres,
+                      beta, flags);  // K3
+            std::swap(rho_cur, rho_new);
+            if ((k + 1) % check == 0 && k + 1 < m) {
+                BJ_CUDA(cudaMemcpyAsync(hflags, flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+                BJ_CUDA(cudaStreamSynchronize(st));
+                if (hflags[0]) break;
+            }
+        }
+    }
     double* PR = PRa;   // partials of the current rho = r.z
     double* PR2 = PRb;  // partials of the next one
-    for (int k = 0; k < m; ++k) {
+    for (int k = 0; k < m && !fused; ++k) {
         rc = spmv(p, q);  // q = A p
         if (rc != BJ_OK) return rc;
         BJ_LAUNCH(pcg_pq_kernel, n, (const double*)p, (const double*)q, PQ, (const int*)flags);

@@ -16,6 +16,7 @@
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
 #include "bj_lanczos_fuse.cuh"
+#include "bj_pcg_fuse.cuh"
 
 namespace bj {
 
@@ -63,12 +64,13 @@ __device__ __forceinline__ void store_rows(double* dst, int64_t lo, int64_t n, b
     }
 }
 
-// LZ: 0 plain, 1 Lanczos prologue (DIR 1: the input is w built on the fly), 2 Lanczos epilogue (DIR 0)
+// LZ: 0 plain, 1 Lanczos prologue (DIR 1: the input is w built on the fly), 2 Lanczos epilogue (DIR 0),
+//     3 PCG update + apply (DIR 2: x += a p, r -= a q on the fly, z = M^-1 r, partials of r.r and r.z)
 template <int B, int DIR, bool VEC, int LZ>
 __global__ void __launch_bounds__(128)
 solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                    const double* in, double* out,  // in == out allowed: a thread touches only its own block
-                   const LzPrologue pro, const LzEpilogue epi)
+                   const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg)
 {
     constexpr int P = B * (B + 1) / 2;
     __shared__ double lz_sh[4];
@@ -85,7 +87,9 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
     const int64_t lo = kc * B;
     double v[B];
     const bool whole = lo + B <= n;
-    double acc = 0.0, beta = 0.0, inv_beta = 0.0;  // Lanczos: running dot product of this thread
+    double acc = 0.0, beta = 0.0, inv_beta = 0.0;  // Lanczos / PCG: running dot product of this thread
+    double rin[LZ == 3 ? B : 1];                   // PCG: the residual rows, kept for r.z
+    double acc2 = 0.0;
     if (LZ == 1) {
         double alpha;
         if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
@@ -102,6 +106,27 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
 #pragma unroll
             for (int i = 0; i < B; ++i) acc = fma(v[i], v[i], acc);  // rows past n were loaded as zeros
             store_rows<B, VEC>(pro.w, lo, n, whole, v);
+        }
+    } else if (LZ == 3) {
+        double a;
+        if (pcg_hook_begin(pcg, a)) return;  // uniform over the grid
+        if (act) {
+            double c[B];
+            load_rows<B, VEC>(pcg.r, lo, n, whole, v);
+            load_rows<B, VEC>(pcg.q, lo, n, whole, c);
+#pragma unroll
+            for (int i = 0; i < B; ++i) {
+                v[i] = v[i] - a * c[i];             // r_new
+                acc = fma(v[i], v[i], acc);
+                rin[i] = v[i];
+            }
+            store_rows<B, VEC>(pcg.r, lo, n, whole, v);
+            double xs[B];
+            load_rows<B, VEC>(pcg.x, lo, n, whole, xs);
+            load_rows<B, VEC>(pcg.p, lo, n, whole, c);
+#pragma unroll
+            for (int i = 0; i < B; ++i) xs[i] = fma(a, c[i], xs[i]);
+            store_rows<B, VEC>(pcg.x, lo, n, whole, xs);
         }
     } else {
         if (LZ == 2 && lz_epilogue_begin(epi, beta, inv_beta)) return;  // uniform over the grid
@@ -144,6 +169,15 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
     } else {
         if (act) store_rows<B, VEC>(out, lo, n, whole, v);
         if (LZ == 1) lz_reduce_finish(pro.red, acc, lz_sh);
+        if (LZ == 3) {
+            if (act) {
+#pragma unroll
+                for (int i = 0; i < B; ++i) acc2 = fma(rin[i], v[i], acc2);
+            }
+            lz_reduce_finish(pcg.red_rr, acc, lz_sh);
+            __syncthreads();
+            lz_reduce_finish(pcg.red_rz, acc2, lz_sh);
+        }
     }
 }
 
@@ -291,9 +325,10 @@ struct GroupParams {
     const double* in;
     double* out;
     int stages;
-    int lz;              // 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0)
+    int lz;              // 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0), 3 PCG update + apply (DIR 2)
     LzPrologue pro;
     LzEpilogue epi;
+    PcgHook pcg;
 };
 
 __device__ __forceinline__ void fence_proxy_async()
@@ -352,6 +387,8 @@ solve_group_kernel(const GroupParams p)
     bool stop = false;
     if (DIR == 1 && p.lz == 1) stop = lz_prologue_begin(p.pro, alpha);
     if (DIR == 0 && p.lz == 2) stop = lz_epilogue_begin(p.epi, beta, inv_beta);
+    double acc2 = 0.0;  // PCG: r.z
+    if (DIR == 2 && p.lz == 3) stop = pcg_hook_begin(p.pcg, alpha);  // alpha = the CG step length here
     if (stop) {  // uniform over the grid; the bulk copies already issued must land before the CTA may exit
         for (int s = 0; s < p.stages; ++s)
             if (first + s * stride < p.ntiles) mbar_wait(&full[s], 0u);
@@ -372,6 +409,8 @@ solve_group_kernel(const GroupParams p)
             if (DIR == 1 && p.lz == 1) {
                 if (live) a[k] = p.pro.first ? p.pro.w0[row] : p.pro.w[row];
                 if (live && !p.pro.first) c[k] = p.pro.vcur[row];
+            } else if (DIR == 2 && p.lz == 3) {
+                if (live) { a[k] = p.pcg.r[row]; c[k] = p.pcg.q[row]; ew[k] = p.pcg.x[row]; ev[k] = p.pcg.p[row]; }
             } else {
                 if (live) a[k] = p.in[row];
                 if (DIR == 0 && p.lz == 2) {  // the epilogue's own operands ride along one tile ahead
@@ -388,6 +427,15 @@ solve_group_kernel(const GroupParams p)
                 if (tile < p.ntiles && row < p.n) p.pro.w[row] = wi;
                 acc = fma(wi, wi, acc);
                 dst[k] = wi;
+            } else if (DIR == 2 && p.lz == 3) {  // r_new = r - a q (the solve's input, stored once), x += a p
+                const int64_t row = row0 + k * 32;
+                const double ri = a[k] - alpha * c[k];
+                if (tile < p.ntiles && row < p.n) {
+                    p.pcg.r[row] = ri;
+                    p.pcg.x[row] = fma(alpha, ev[k], ew[k]);
+                    acc = fma(ri, ri, acc);
+                }
+                dst[k] = (tile < p.ntiles && row < p.n) ? ri : 0.0;
             } else {
                 dst[k] = a[k];
             }
@@ -410,7 +458,7 @@ solve_group_kernel(const GroupParams p)
         for (int k = 0; k < RPL; ++k) r[k] = xchg[g * XB + k * LPB + l];
         double ew[RPL], ev[RPL];
 #pragma unroll
-        for (int k = 0; k < RPL; ++k) { ew[k] = ewn[k]; ev[k] = evn[k]; }
+        for (int k = 0; k < RPL; ++k) { ew[k] = (DIR == 2 && p.lz == 3) ? rn[k] : ewn[k]; ev[k] = evn[k]; }  // PCG: ew = r_new rows
         fetch(tile + stride, rn, ewn, evn);  // one tile ahead: its latency hides behind this tile's solve
         mbar_wait(&full[s], ph);
         const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
@@ -435,6 +483,7 @@ solve_group_kernel(const GroupParams p)
                     p.epi.w[row] = wi;
                     acc = fma(vn, wi, acc);
                 } else {
+                    if (DIR == 2 && p.lz == 3) acc2 = fma(ew[k], y, acc2);  // r_new . z
                     p.out[row] = y;
                 }
             }
@@ -447,30 +496,39 @@ solve_group_kernel(const GroupParams p)
     }
     if (DIR == 1 && p.lz == 1) lz_reduce_finish(p.pro.red, acc, lz_sh);
     if (DIR == 0 && p.lz == 2) lz_reduce_finish(p.epi.red, acc, lz_sh);
+    if (DIR == 2 && p.lz == 3) {
+        lz_reduce_finish(p.pcg.red_rr, acc, lz_sh);
+        __syncthreads();
+        lz_reduce_finish(p.pcg.red_rz, acc2, lz_sh);
+    }
 }
 
 // b == 1 fast path is just the B = 1 instance of solve_small_kernel.
 
 template <int DIR, int LZ>
-static int launch_small(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
+static int launch_small(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                        const PcgHook* pcg = nullptr)
 {
     const int threads = 128;
     const unsigned blocks = (unsigned)((h->nblocks + threads - 1) / threads);
     uintptr_t al = (uintptr_t)in | (uintptr_t)out;
     if (pro) al |= (uintptr_t)pro->w0 | (uintptr_t)pro->w | (uintptr_t)pro->vcur;
     if (epi) al |= (uintptr_t)epi->w | (uintptr_t)epi->vprev | (uintptr_t)epi->vnew;
+    if (pcg) al |= (uintptr_t)pcg->x | (uintptr_t)pcg->p | (uintptr_t)pcg->r | (uintptr_t)pcg->q;
     const bool vec = (al & 31) == 0;
     const bool pdl = h->pdl && !h->prof_on;
     const LzPrologue pr = pro ? *pro : LzPrologue{};
     const LzEpilogue ep = epi ? *epi : LzEpilogue{};
+    const PcgHook pc = pcg ? *pcg : PcgHook{};
+    if (pcg && ((int)blocks > pcg->red_rr.cap || (int)blocks > pcg->red_rz.cap)) return BJ_ERR_INVALID_ARG;
     if ((epi && (int)blocks > epi->red.cap) || (pro && (int)blocks > pro->red.cap)) return BJ_ERR_INVALID_ARG;
     cudaError_t e = cudaSuccess;
 #define BJ_CASE(B)                                                                                                          \
     case B:                                                                                                                 \
         e = vec ? launch_kernel(solve_small_kernel<B, DIR, true, LZ>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,  \
-                                (const double*)h->fac_small, in, out, pr, ep)                                               \
+                                (const double*)h->fac_small, in, out, pr, ep, pc)                                           \
                 : launch_kernel(solve_small_kernel<B, DIR, false, LZ>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks, \
-                                (const double*)h->fac_small, in, out, pr, ep);                                              \
+                                (const double*)h->fac_small, in, out, pr, ep, pc);                                           \
         break;
     switch (h->b) {
         BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
@@ -541,7 +599,8 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
 }
 
 template <int B, int LPB, int DIR>
-static int launch_group_t(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
+static int launch_group_t(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                          const PcgHook* pcg)
 {
     using Geo = GroupGeom<B, LPB>;
     constexpr int kGroupBlocksPerWarp = Geo::NBW;
@@ -566,7 +625,8 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     gp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
     gp.fac1 = h->fac_bwd;
     gp.in = in; gp.out = out; gp.stages = stages;
-    gp.lz = (DIR == 1 && pro) ? 1 : (DIR == 0 && epi) ? 2 : 0;
+    gp.lz = (DIR == 1 && pro) ? 1 : (DIR == 0 && epi) ? 2 : (DIR == 2 && pcg) ? 3 : 0;
+    gp.pcg = pcg ? *pcg : PcgHook{};
     gp.pro = pro ? *pro : LzPrologue{};
     gp.epi = epi ? *epi : LzEpilogue{};
     int occ = 1;
@@ -574,21 +634,23 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     const int64_t want = (gp.ntiles + warps - 1) / warps;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * std::max(1, occ)));
     if ((gp.lz == 2 && grid > gp.epi.red.cap) || (gp.lz == 1 && grid > gp.pro.red.cap)) return BJ_ERR_INVALID_ARG;
+    if (gp.lz == 3 && (grid > gp.pcg.red_rr.cap || grid > gp.pcg.red_rz.cap)) return BJ_ERR_INVALID_ARG;
     cudaError_t e = launch_kernel(solve_group_kernel<B, LPB, DIR>, grid, warps * 32, smem, h->stream, h->pdl && !h->prof_on, gp);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_group_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
 
 template <int DIR>
-static int launch_group(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
+static int launch_group(bj_handle_s* h, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                        const PcgHook* pcg = nullptr)
 {
     // lanes per block: small enough tiles that many warps fit one SM's shared memory (latency hiding)
     const int lpb = (h->tune.group_lanes > 0 ? h->tune.group_lanes : (h->b == 32 ? 8 : 4));
     switch (h->b) {
-        case 16: return lpb == 8 ? launch_group_t<16, 8, DIR>(h, in, out, pro, epi) : launch_group_t<16, 4, DIR>(h, in, out, pro, epi);
-        case 24: return lpb == 8 ? launch_group_t<24, 8, DIR>(h, in, out, pro, epi) : launch_group_t<24, 4, DIR>(h, in, out, pro, epi);
-        case 32: return lpb == 16 ? launch_group_t<32, 16, DIR>(h, in, out, pro, epi)
-                      : lpb == 8 ? launch_group_t<32, 8, DIR>(h, in, out, pro, epi) : launch_group_t<32, 4, DIR>(h, in, out, pro, epi);
+        case 16: return lpb == 8 ? launch_group_t<16, 8, DIR>(h, in, out, pro, epi, pcg) : launch_group_t<16, 4, DIR>(h, in, out, pro, epi, pcg);
+        case 24: return lpb == 8 ? launch_group_t<24, 8, DIR>(h, in, out, pro, epi, pcg) : launch_group_t<24, 4, DIR>(h, in, out, pro, epi, pcg);
+        case 32: return lpb == 16 ? launch_group_t<32, 16, DIR>(h, in, out, pro, epi, pcg)
+                      : lpb == 8 ? launch_group_t<32, 8, DIR>(h, in, out, pro, epi, pcg) : launch_group_t<32, 4, DIR>(h, in, out, pro, epi, pcg);
         default: return BJ_ERR_INVALID_ARG;
     }
 }
@@ -605,9 +667,11 @@ bool lanczos_fusable(const bj_handle_s* h)
     return h->solve_kind == 1 || (h->solve_kind == 2 && use_group_kernel(h));
 }
 
-int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi)
+int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                 const PcgHook* pcg)
 {
-    if ((pro || epi) && !lanczos_fusable(h)) return BJ_ERR_INVALID_ARG;
+    if ((pro || epi || pcg) && !lanczos_fusable(h)) return BJ_ERR_INVALID_ARG;
+    if (pcg && dir != 2) return BJ_ERR_INVALID_ARG;
     int rc = BJ_OK;
     if (h->solve_kind == 0) {
         if (in != out) BJ_CUDA(cudaMemcpyAsync(out, in, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
@@ -619,10 +683,10 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const L
         if (h->solve_kind == 1) {
             rc = dir == 0   ? (epi ? launch_small<0, 2>(h, in, out, nullptr, epi) : launch_small<0, 0>(h, in, out, nullptr, nullptr))
                  : dir == 1 ? (pro ? launch_small<1, 1>(h, in, out, pro, nullptr) : launch_small<1, 0>(h, in, out, nullptr, nullptr))
-                            : launch_small<2, 0>(h, in, out, nullptr, nullptr);
+                            : (pcg ? launch_small<2, 3>(h, in, out, nullptr, nullptr, pcg) : launch_small<2, 0>(h, in, out, nullptr, nullptr));
         } else if (use_group_kernel(h)) {
             rc = dir == 0 ? launch_group<0>(h, in, out, pro, epi) : dir == 1 ? launch_group<1>(h, in, out, pro, epi)
-                          : launch_group<2>(h, in, out, nullptr, nullptr);
+                          : launch_group<2>(h, in, out, nullptr, nullptr, pcg);
         } else {
             rc = dir == 0 ? launch_warp<0>(h, in, out) : dir == 1 ? launch_warp<1>(h, in, out) : launch_warp<2>(h, in, out);
         }

@@ -114,8 +114,10 @@ struct StreamParams {
     int su_bufs;         // number of su buffers (2; FUSE 3: one per stage)
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
-    int lz;              // 1: fused Lanczos epilogue on the rows this kernel writes (FUSE 0 and 1)
+    int lz;              // 1: fused Lanczos epilogue on the rows this kernel writes (FUSE 0 and 1); 2: dot hook (FUSE 0)
     LzEpilogue epi;
+    const double* dot_with;  // lz == 2: per-CTA partials of dot_with . y go to dot_red (PCG: p . A p)
+    LzReduce dot_red;
 };
 
 __device__ __forceinline__ void consumer_bar_sync(int nthreads)
@@ -161,7 +163,7 @@ spmv_stream_kernel(const StreamParams p)
     const int R = p.R;
     __shared__ double lz_sh[kMaxStreamThreads / 32];
     double pa = 0.0, beta = 0.0, inv_beta = 0.0;
-    if (p.lz) {  // beta and the stop flag come from the previous kernel: every thread waits for it
+    if (p.lz == 1) {  // beta and the stop flag come from the previous kernel: every thread waits for it
         pdl_wait();
         if (lz_epilogue_begin(p.epi, beta, inv_beta)) return;  // uniform over the grid, nothing in flight yet
     }
@@ -300,8 +302,12 @@ spmv_stream_kernel(const StreamParams p)
                         const int kb = i / GB;
                         sub_u[kb * XB + (i - kb * GB)] = acc;
                     } else {
-                        if (p.lz) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, acc, pa);
-                        else p.y[r0 + i] = acc;
+                        if (p.lz == 1) {
+                            lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, acc, pa);
+                        } else {
+                            if (p.lz == 2) pa = fma(p.dot_with[r0 + i], acc, pa);
+                            p.y[r0 + i] = acc;
+                        }
                     }
                 }
             }
@@ -397,7 +403,7 @@ spmv_stream_kernel(const StreamParams p)
                 for (int i = ctid; i < rows; i += nct) {
                     const int k = (int)__umulhi((unsigned)i, p.b_magic);
                     const double yv = sub_u[k * p.bs + (i - k * b)];
-                    if (p.lz) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, yv, pa);
+                    if (p.lz == 1) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, yv, pa);
                     else p.y[r0 + i] = yv;
                 }
             }
@@ -405,7 +411,8 @@ spmv_stream_kernel(const StreamParams p)
             if (lane == 0) mbar_arrive(&empty[s]);
         }
     }
-    if (p.lz) lz_reduce_finish(p.epi.red, pa, lz_sh);
+    if (p.lz == 1) lz_reduce_finish(p.epi.red, pa, lz_sh);
+    if (p.lz == 2) lz_reduce_finish(p.dot_red, pa, lz_sh);
 }
 
 template <int LPR, int BATCH, int FUSE, int W>
@@ -553,7 +560,8 @@ int spmv_stream_finish(bj_handle_s* h, int max_tile)
     return BJ_OK;
 }
 
-int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi)
+int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi,
+                       const double* dot_with, const LzReduce* dot_red)
 {
     if (!h->stream_ok) return BJ_ERR_INVALID_ARG;
     const bool fuse = fuse_forward && h->fuse_ok;
@@ -564,7 +572,10 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
     sp.early_trigger = (h->tune.pdl_early >> 1) & 1;
-    sp.lz = epi ? 1 : 0;
+    sp.lz = epi ? 1 : (dot_with && dot_red) ? 2 : 0;
+    sp.dot_with = dot_with;
+    sp.dot_red = dot_red ? *dot_red : LzReduce{};
+    if (sp.lz == 2 && (fuse || h->num_sms * 4 > dot_red->cap)) return BJ_ERR_INVALID_ARG;
     sp.epi = epi ? *epi : LzEpilogue{};
     if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the b > 8 fused paths have no hook
     if (epi && h->num_sms * 4 > epi->red.cap) return BJ_ERR_INVALID_ARG;

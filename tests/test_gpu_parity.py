@@ -431,6 +431,29 @@ def test_pcg_matches_oracle_small(B, torch_, rel, cfg):
         B.bj_destroy(h)
 
 
+@pytest.mark.parametrize("fuse", ["0", "1"])
+def test_pcg_fused_and_unfused_iterations_agree(B, torch_, rel, monkeypatch, fuse):
+    """BJ_PCG_FUSE=0 runs the seven-kernel iteration of bj_pcg.cu, the default rides on the SpMV and solve kernels
+    (three kernels per iteration): both follow the oracle, for every solve kernel (b = 3, 8: thread per block; 16, 24, 32:
+    group per block; 12: no hook -> unfused either way)."""
+    monkeypatch.setenv("BJ_PCG_FUSE", fuse)
+    A = mat(2, "small")
+    rhs = W.seeded_vector(23, A.n)
+    for b in (3, 8, 12, 16, 24, 32):
+        h, keep = B.setup_from_host(A, b)
+        g = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=10, rtol=0.0, check_every=4)
+        c = oracle.Precond(A, b).pcg(rhs, 10, 0.0)
+        assert g["iters"] == 10
+        assert np.allclose(g["alpha"], c["alpha"], rtol=1e-9, atol=0) and np.allclose(g["beta"], c["beta"], rtol=1e-9, atol=0), b
+        assert np.allclose(g["relres_hist"], c["relres"], rtol=1e-9, atol=0)
+        e2, ei = rel(g["x"].cpu().numpy(), c["x"])
+        assert e2 <= 1e-9, (b, e2)
+        g = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=500, rtol=1e-6, check_every=16)
+        c = oracle.Precond(A, b).pcg(rhs, 500, 1e-6)
+        assert g["converged"] and abs(g["iters"] - c["iters"]) <= max(2, c["iters"] // 50) and g["true_relres"] <= 2e-6
+        B.bj_destroy(h)
+
+
 def test_pcg_degenerate_cases(B, torch_, rel):
     A = W.block_diagonal_spd(65, 8)     # M = A: one step (PAPER.md:80)
     h, keep = B.setup_from_host(A, 8)
