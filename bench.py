@@ -175,6 +175,7 @@ def main():
     ap.add_argument("--scale", default="full", choices=["full", "small", "tiny"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--lanczos-iters", type=int, default=50)
+    ap.add_argument("--long-iters", type=int, default=2000, help="iterations of the long fast-mode kappa runs (0: skip)")
     ap.add_argument("--cpu-budget-s", type=float, default=10.0)
     ap.add_argument("--spmv-kernel", type=int, default=-1)
     ap.add_argument("--fuse", type=int, default=-1)
@@ -380,6 +381,20 @@ def main():
             dt = time.perf_counter() - t0
             kap["fast_mode"] = {"kappa_est": r["kappa"], "iters": r["iters_done"], "seconds": dt,
                                 "lanczos_iters_per_s": r["iters_done"] / dt}
+            # long runs (fast mode: the extreme Ritz values keep converging, ghosts only repeat them) so that
+            # kappa(A) -> kappa(A^) is meaningful beyond the m-step lower bounds above (SURVEY 8(c) reading 13)
+            ml = args.long_iters
+            if ml > 0:
+                h0l = B.bj_setup(rp, ci, val, 0)
+                long_run = {"iters": ml}
+                for name, hh in (("A", h0l), (f"bj{b}", h)):
+                    t0 = time.perf_counter()
+                    r = B.bj_cond_estimate_ex(hh, ml, reorth=False)
+                    long_run[name] = {"kappa_est": r["kappa"], "lmin": r["lmin"], "lmax": r["lmax"], "res_min": r["res_min"],
+                                      "res_max": r["res_max"], "iters": r["iters_done"], "seconds": time.perf_counter() - t0}
+                long_run["predicted_hhl_gain_kappa_sq"] = (long_run["A"]["kappa_est"] / long_run[f"bj{b}"]["kappa_est"]) ** 2
+                kap["long_run"] = long_run
+                B.bj_destroy(h0l)
             kap["predicted_hhl_gain_kappa_sq"] = (kap["A"]["kappa_est"] / kap[f"bj{b}"]["kappa_est"]) ** 2
             line["kappa"] = kap
             B.bj_destroy(h0)
