@@ -35,10 +35,13 @@ UNIT = "applies/s"
 NOMINAL_HBM_GBS = 8000.0  # BASELINE.json north_star "~8 TB/s"
 
 
-def algorithmic_bytes(n: int, nnz: int, b: int) -> dict:
-    """SURVEY.md 8(d) / DESIGN.md section 6: bytes the method itself must move, per launch."""
+def algorithmic_bytes(n: int, nnz: int, b: int, band: int = -1) -> dict:
+    """SURVEY.md 8(d) / DESIGN.md section 6: bytes the method itself must move, per launch.  band >= 0 (banded block
+    factors, opt-in): a solve pass reads (band + 1) b doubles per block instead of b(b+1)/2."""
     spmv = 12 * nnz + 4 * (n + 1) + 16 * n
     solve = (4 * n * (b + 1) + 16 * n) if b > 0 else 0
+    if band >= 0:
+        solve = 8 * n * (band + 1) + 16 * n
     return {"spmv": spmv, "solve_L": solve, "solve_Lt": solve, "apply": solve,
             "spmv_solve_L": spmv + solve, "op_apply": spmv + 2 * solve}
 
@@ -180,6 +183,9 @@ def main():
     ap.add_argument("--spmv-kernel", type=int, default=-1)
     ap.add_argument("--fuse", type=int, default=-1)
     ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e (profiling runs)")
+    ap.add_argument("--band", type=int, default=0,
+                    help="1: banded block factors where the diagonal blocks are banded (b > 8; SURVEY 8(f) NEXT-2); "
+                         "the byte model of the roofline then counts the band, the dense-packed count is given beside it")
     ap.add_argument("--graph", type=int, default=-1,
                     help="1: also time the operator apply replayed from a CUDA graph (default: only config 1, launch-bound)")
     ap.add_argument("--gather-envelope", type=int, default=-1,
@@ -206,6 +212,8 @@ def main():
     if world > 1:
         dist.init_process_group("nccl")
     B.lib()  # fail loudly if the CUDA library is missing
+    if args.band:
+        os.environ["BJ_BAND"] = "1"  # read by bj_setup
 
     n, nnz = A.n, A.nnz
     rp = torch.from_numpy(A.row_ptr).cuda()
@@ -231,7 +239,8 @@ def main():
 
     x = B.bj_seeded_vector(h, 31)
     y = torch.empty_like(x)
-    ab = algorithmic_bytes(n, nnz, b)
+    ab = algorithmic_bytes(n, nnz, b, info.get("band_width", -1))
+    ab_dense = algorithmic_bytes(n, nnz, b)
 
     def barrier():
         torch.cuda.synchronize()
@@ -288,6 +297,8 @@ def main():
             "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
             "op_apply": {"alg_bytes": ab["op_apply"], "gbs": op_gbs, "frac_of_measured": op_gbs / peak,
                          "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
+            "band": {"width": info.get("band_width", -1), "op_apply_bytes_dense_packed": ab_dense["op_apply"],
+                     "gbs_vs_dense_packed_count": ab_dense["op_apply"] / (ms_per_step * 1e-3) / 1e9},
             "kernels": kern, "setup_ms": float(np.median(setup_ms)),
             "factor_bytes": info["factor_bytes"]}
 

@@ -89,8 +89,10 @@ typedef struct {
     int64_t kernel_launches;  /* number of kernels this handle has launched so far                   */
     int32_t spmv_kernel;      /* 0: row-per-subwarp CSR-vector kernel, 1: TMA-streamed tile kernel    */
     int32_t spmv_lanes;       /* lanes per row chosen at setup                                       */
-    int32_t solve_kernel;     /* 0: none (b=0), 1: thread-per-block (b<=8), 2: subwarp-per-block      */
+    int32_t solve_kernel;     /* 0: none (b=0), 1: thread-per-block (b<=8), 2: group/subwarp-per-block, 3: banded */
     int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
+    int32_t band_width;       /* >= 0: banded factors in use (BJ_BAND=1 at setup, solve_kernel 3), the lower
+                                 bandwidth of every diagonal block; -1: dense packed factors              */
 } bj_info_t;
 
 typedef struct {

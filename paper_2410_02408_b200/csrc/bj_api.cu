@@ -259,6 +259,22 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
 
     h->coherence = stt.compared ? (double)stt.coherent / (double)stt.compared : 1.0;
 
+    // NEXT-2, opt-in: banded diagonal blocks keep banded factors -- (w+1) b doubles per block instead of b(b+1)/2.
+    // Only for b > 8 (the b <= 8 path fuses the forward solve into the SpMV kernel, which the band path does not).
+    if (h->solve_kind == 2 && h->nblocks >= 64 && env_int("BJ_BAND", 0) != 0) {
+        rc = launch_band_width(h);
+        if (rc != BJ_OK) return fail(rc);
+        ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+        if (ce != cudaSuccess) { set_cuda_error(ce, "band width"); return fail(BJ_ERR_CUDA); }
+        if (stt.max_band >= 0 && stt.max_band <= 2) {
+            h->solve_kind = 3;
+            h->band = stt.max_band;
+            h->fac_band = h->fac_fwd;  // (w+1) b <= 3 b < b(b+1)/2 for b > 8: fits the forward copy's storage
+            h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * kInterleave * (h->band + 1) * b * (int64_t)sizeof(double);
+        }
+    }
+
     // lanes per row for the CSR-vector kernel: power of two near the mean row length
     {
         const double mean = (double)h->nnz / (double)h->n;
@@ -271,13 +287,18 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     if (h->solve_kind == 1) {
         const size_t group_bytes = (size_t)h->packed * kInterleave * sizeof(double);
         if (h->nblocks % kInterleave) ce = cudaMemsetAsync((char*)h->fac_small + fac_a - group_bytes, 0, group_bytes, h->stream);
+    } else if (h->solve_kind == 3) {
+        // the last interleave group may be partly unused: zero it so that no lane ever reads an uninitialised factor
+        const size_t group_bytes = (size_t)(h->band + 1) * b * kInterleave * sizeof(double);
+        if (h->nblocks % kInterleave)
+            ce = cudaMemsetAsync((char*)h->fac_band + (size_t)(h->nblocks / kInterleave) * group_bytes, 0, group_bytes, h->stream);
     } else if (h->solve_kind == 2) {
         ce = cudaMemsetAsync((char*)h->fac_fwd + fac_a - 16, 0, 16, h->stream);
         if (ce == cudaSuccess) ce = cudaMemsetAsync((char*)h->fac_bwd + fac_b - 16, 0, 16, h->stream);
     }
     if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
     if (b > 0) {
-        rc = launch_extract_factor(h);
+        rc = h->solve_kind == 3 ? launch_extract_factor_band(h) : launch_extract_factor(h);
         if (rc != BJ_OK) return fail(rc);
     }
 
@@ -357,6 +378,7 @@ int bj_get_info(bj_handle_t h, bj_info_t* info)
     info->spmv_kernel = h->spmv_kernel;
     info->spmv_lanes = h->spmv_lanes;
     info->solve_kernel = h->solve_kind;
+    info->band_width = h->solve_kind == 3 ? h->band : -1;
     info->fused_forward = (h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0 && h->solve_kind != 0) ? 1 : 0;
     return BJ_OK;
 }

@@ -1,0 +1,239 @@
+// Banded block factors (opt-in with BJ_BAND=1 at setup, b > 8).
+//
+// When every diagonal block D_k is banded with lower bandwidth w <= 2 (stencil matrices whose blocks follow a grid
+// line are tridiagonal: configs 2 and 4), its Cholesky factor has the same band (no fill outside it), so the
+// packed-dense factor stream of b(b+1)/2 doubles per block shrinks to (w+1) b.  This moves FEWER bytes than the
+// dense-block count of SURVEY.md 8(d) and therefore carries its own byte accounting:
+//   one solve pass = 8 N (w+1) + 16 N bytes  instead of  4 N (b+1) + 16 N.
+// Arithmetic: exactly the oracle's left-looking Cholesky and substitutions with the structurally zero terms
+// skipped (adding a zero product changes nothing), so the parity bar is unchanged.
+//
+// Layout: element (i, d) = l_{i, i-d}, d = 0..w (d = 0 holds 1 / l_ii), of blocks 32 g .. 32 g + 31 is one 256-byte
+// line: fac_band[g * 32 E + (i (w+1) + d) * 32 + k % 32], E = (w+1) b.  One THREAD per block: every load of a warp
+// is one coalesced line and no load depends on the substitution chain.
+#include <algorithm>
+
+#include "bj_device.cuh"
+#include "bj_internal.cuh"
+
+namespace bj {
+
+namespace {
+
+// lower bandwidth of the diagonal blocks: max over rows of (row - first in-block column of the row)
+__global__ void __launch_bounds__(256)
+band_width_kernel(int64_t n, int b, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci, Status* st)
+{
+    const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int d = 0;
+    if (row < n) {
+        const int64_t lo = (row / b) * b;
+        int s = rp[row], hi = rp[row + 1];
+        const int e = hi;
+        while (s < hi) {  // first entry with column >= lo
+            const int mid = (s + hi) >> 1;
+            if (ci[mid] < lo) s = mid + 1; else hi = mid;
+        }
+        if (s < e && ci[s] < row) d = (int)(row - ci[s]);
+    }
+    d = __reduce_max_sync(0xffffffffu, d);
+    if ((threadIdx.x & 31) == 0 && d > *(volatile int*)&st->max_band) atomicMax(&st->max_band, d);
+}
+
+// a2 + a3 for banded blocks: one thread per block, rows in order, a window of the last W factor rows in registers
+template <int W>
+__global__ void __launch_bounds__(128)
+extract_factor_band_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restrict__ rp,
+                           const int32_t* __restrict__ ci, const double* __restrict__ val, double* __restrict__ fac,
+                           Status* st)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nblocks) return;
+    const int E = (W + 1) * b;
+    double* f = fac + (k >> 5) * (int64_t)E * kInterleave + (k & 31);
+    const int64_t lo = k * b;
+    double prev[W > 0 ? W : 1][W + 1];  // prev[r][d] = l_{i-1-r, i-1-r-d}
+#pragma unroll
+    for (int r = 0; r < (W > 0 ? W : 1); ++r)
+#pragma unroll
+        for (int d = 0; d <= W; ++d) prev[r][d] = 0.0;
+    bool bad = false;
+    for (int i = 0; i < b; ++i) {
+        const int64_t row = lo + i;
+        double a[W + 1];
+#pragma unroll
+        for (int d = 0; d <= W; ++d) a[d] = 0.0;
+        if (row < n) {
+            const int64_t first = row - W > lo ? row - W : lo;
+            int s = rp[row], hi = rp[row + 1];
+            const int e = hi;
+            while (s < hi) {
+                const int mid = (s + hi) >> 1;
+                if (ci[mid] < first) s = mid + 1; else hi = mid;
+            }
+#pragma unroll
+            for (int q = 0; q <= W; ++q) {
+                if (s + q < e) {
+                    const int64_t c = ci[s + q];
+                    if (c <= row) {
+                        const int d = (int)(row - c);
+#pragma unroll
+                        for (int dd = 0; dd <= W; ++dd)
+                            if (dd == d) a[dd] = val[s + q];
+                    }
+                }
+            }
+        } else {
+            a[0] = 1.0;  // identity rows pad the ragged last block
+        }
+        // row i of the factor: l_{i,j} = (a_ij - sum_{p<j} l_ip l_jp) / l_jj for j = i-W .. i-1, then the diagonal
+        double cur[W + 1];
+#pragma unroll
+        for (int d = W; d >= 1; --d) {
+            double sres = a[d];
+            // p runs over i-W .. i-d-1 (ascending): offsets i-p = W .. d+1 in this row, (i-d)-p = W-d .. 1 in row i-d
+#pragma unroll
+            for (int o = W; o > d; --o) sres -= cur[o] * prev[d - 1][o - d];
+            cur[d] = (i - d >= 0) ? sres / prev[d - 1][0] : 0.0;
+        }
+        double dg = a[0];
+#pragma unroll
+        for (int d = W; d >= 1; --d) dg -= cur[d] * cur[d];
+        if (!(dg > 0.0) || isinf(dg)) { bad = true; dg = 1.0; }
+        cur[0] = sqrt(dg);
+        f[(i * (W + 1)) * kInterleave] = 1.0 / cur[0];
+#pragma unroll
+        for (int d = 1; d <= W; ++d) f[(i * (W + 1) + d) * kInterleave] = cur[d];
+        // slide the window
+#pragma unroll
+        for (int r = W - 1; r >= 1; --r)
+#pragma unroll
+            for (int d = 0; d <= W; ++d) prev[r][d] = prev[r - 1][d];
+        if (W > 0) {
+#pragma unroll
+            for (int d = 0; d <= W; ++d) prev[0][d] = cur[d];
+        }
+    }
+    if (bad) {
+        atomicOr(&st->flags, ST_NOT_SPD);
+        atomicMin(&st->bad_block, (long long)k);
+    }
+}
+
+// thread per block; BMAX bounds the register arrays (b <= BMAX); DIR 0 forward, 1 backward, 2 both
+template <int BMAX, int W, int DIR>
+__global__ void __launch_bounds__(128)
+solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ fac, const double* in, double* out)
+{
+    pdl_trigger();
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nblocks) return;
+    const int E = (W + 1) * b;
+    const double* f = fac + (k >> 5) * (int64_t)E * kInterleave + (k & 31);
+    const int64_t lo = k * b;
+    const bool vec = (b % 4 == 0) && lo + b <= n && (((uintptr_t)in | (uintptr_t)out) & 31) == 0;
+    // the whole band goes to registers first: (W+1) b independent, coalesced loads in flight per thread
+    double l[(W + 1) * BMAX];
+#pragma unroll
+    for (int e = 0; e < (W + 1) * BMAX; ++e) l[e] = (e < E) ? ld_const_stream(f + e * kInterleave) : 0.0;
+    pdl_wait();  // `in` may come from the previous kernel
+    double v[BMAX];
+    if (vec) {
+#pragma unroll
+        for (int i = 0; i < BMAX; i += 4)
+            if (i < b) ld_v4(in + lo + i, v + i);
+    } else {
+#pragma unroll
+        for (int i = 0; i < BMAX; ++i) v[i] = (i < b && lo + i < n) ? in[lo + i] : 0.0;
+    }
+    if (DIR == 0 || DIR == 2) {
+#pragma unroll
+        for (int i = 0; i < BMAX; ++i) {
+            if (i < b) {
+                double s = v[i];
+#pragma unroll
+                for (int d = W; d >= 1; --d)
+                    if (i - d >= 0) s -= l[i * (W + 1) + d] * v[i - d];
+                v[i] = s * l[i * (W + 1)];
+            }
+        }
+    }
+    if (DIR == 1 || DIR == 2) {
+#pragma unroll
+        for (int i = BMAX - 1; i >= 0; --i) {
+            if (i < b) {
+                double s = v[i];
+#pragma unroll
+                for (int d = 1; d <= W; ++d)
+                    if (i + d < BMAX && i + d < b) s -= l[(i + d) * (W + 1) + d] * v[i + d];
+                v[i] = s * l[i * (W + 1)];
+            }
+        }
+    }
+    if (vec) {
+#pragma unroll
+        for (int i = 0; i < BMAX; i += 4)
+            if (i < b) st_v4(out + lo + i, v + i);
+    } else {
+#pragma unroll
+        for (int i = 0; i < BMAX; ++i)
+            if (i < b && lo + i < n) out[lo + i] = v[i];
+    }
+}
+
+template <int BMAX, int W>
+int launch_band_t(bj_handle_s* h, int dir, const double* in, double* out)
+{
+    const unsigned blocks = (unsigned)((h->nblocks + 127) / 128);
+    const bool pdl = h->pdl && !h->prof_on;
+    cudaError_t e = dir == 0   ? launch_kernel(solve_band_kernel<BMAX, W, 0>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,
+                                               (const double*)h->fac_band, in, out)
+                    : dir == 1 ? launch_kernel(solve_band_kernel<BMAX, W, 1>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,
+                                               (const double*)h->fac_band, in, out)
+                               : launch_kernel(solve_band_kernel<BMAX, W, 2>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,
+                                               (const double*)h->fac_band, in, out);
+    if (e != cudaSuccess) { set_cuda_error(e, "solve_band_kernel launch"); return BJ_ERR_CUDA; }
+    return BJ_OK;
+}
+
+}  // namespace
+
+int launch_band_width(bj_handle_s* h)
+{
+    const unsigned blocks = (unsigned)((h->n + 255) / 256);
+    band_width_kernel<<<blocks, 256, 0, h->stream>>>(h->n, h->b, h->row_ptr, h->col_idx, h->status);
+    h->launches++;
+    BJ_CUDA(cudaGetLastError());
+    return BJ_OK;
+}
+
+int launch_extract_factor_band(bj_handle_s* h)
+{
+    const unsigned blocks = (unsigned)((h->nblocks + 127) / 128);
+#define BJ_CASE(W)                                                                                                      \
+    case W:                                                                                                             \
+        extract_factor_band_kernel<W><<<blocks, 128, 0, h->stream>>>(h->n, h->b, h->nblocks, h->row_ptr, h->col_idx, h->val, \
+                                                                     h->fac_band, h->status);                          \
+        break;
+    switch (h->band) {
+        BJ_CASE(0) BJ_CASE(1) BJ_CASE(2)
+        default: return BJ_ERR_INVALID_ARG;
+    }
+#undef BJ_CASE
+    h->launches++;
+    BJ_CUDA(cudaGetLastError());
+    return BJ_OK;
+}
+
+int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out)
+{
+    const bool small = h->b <= 16;
+    switch (h->band) {
+        case 0: return small ? launch_band_t<16, 0>(h, dir, in, out) : launch_band_t<32, 0>(h, dir, in, out);
+        case 1: return small ? launch_band_t<16, 1>(h, dir, in, out) : launch_band_t<32, 1>(h, dir, in, out);
+        case 2: return small ? launch_band_t<16, 2>(h, dir, in, out) : launch_band_t<32, 2>(h, dir, in, out);
+        default: return BJ_ERR_INVALID_ARG;
+    }
+}
+
+}  // namespace bj

@@ -14,6 +14,13 @@ __device__ __forceinline__ double ld_stream(const double* p)
     asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
+// same load, but schedulable: the compiler may hoist it above unrelated arithmetic (the data never changes after setup)
+__device__ __forceinline__ double ld_const_stream(const double* p)
+{
+    double v;
+    asm("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ int ld_stream(const int* p)
 {
     int v;

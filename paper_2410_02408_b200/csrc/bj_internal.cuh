@@ -29,6 +29,8 @@ struct Status {
     unsigned long long compared;  // entries compared
     unsigned long long descents;        // entries with col[p] <= col[p-1]
     unsigned long long legal_descents;  // ... of which at the start of a non-empty row
+    int max_band;                       // largest lower bandwidth of a diagonal block (band_width_kernel, BJ_BAND=1)
+    int pad2;
 };
 
 // Launch-shape knobs: defaults are the measured best on B200; each can be overridden by the environment variable
@@ -79,7 +81,9 @@ struct bj_handle_s {
     int64_t bad_block = -1;
 
     // factors
-    int solve_kind = 0;  // 0 none, 1 small (interleaved), 2 warp (fwd + bwd packed copies)
+    int solve_kind = 0;  // 0 none, 1 small (interleaved), 2 warp (fwd + bwd packed copies), 3 banded (interleaved band)
+    int band = -1;       // kind 3: lower bandwidth w of every diagonal block (0..2)
+    double* fac_band = nullptr;  // kind 3: aliases the dense factor storage of the slab
     int lanes = 0;       // lanes per block for kind 2 (8, 16 or 32)
     int packed = 0;      // b(b+1)/2
     double* fac_small = nullptr;
@@ -165,6 +169,11 @@ struct PcgHook;
 int launch_validate(bj_handle_s* h);
 int launch_extract_factor(bj_handle_s* h);
 int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nnz
+
+// banded block factors (bj_band_kernels.cu), opt-in
+int launch_band_width(bj_handle_s* h);            // Status.max_band
+int launch_extract_factor_band(bj_handle_s* h);   // a2 + a3 into fac_band
+int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out);
 
 // solves (bj_solve_kernels.cu): dir 0 = forward (L^-1), 1 = backward (L^-T), 2 = both (apply)
 // pro (dir 1 only) / epi (dir 0 only): fused Lanczos hooks of bj_lanczos_fuse.cuh, null for a plain solve

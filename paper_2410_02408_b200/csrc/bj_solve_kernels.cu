@@ -680,7 +680,9 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const L
     const int kind = dir == 0 ? BJ_K_SOLVE_L : (dir == 1 ? BJ_K_SOLVE_LT : BJ_K_APPLY);
     {
         KernelScope scope(h, kind);
-        if (h->solve_kind == 1) {
+        if (h->solve_kind == 3) {
+            rc = launch_solve_band(h, dir, in, out);
+        } else if (h->solve_kind == 1) {
             rc = dir == 0   ? (epi ? launch_small<0, 2>(h, in, out, nullptr, epi) : launch_small<0, 0>(h, in, out, nullptr, nullptr))
                  : dir == 1 ? (pro ? launch_small<1, 1>(h, in, out, pro, nullptr) : launch_small<1, 0>(h, in, out, nullptr, nullptr))
                             : (pcg ? launch_small<2, 3>(h, in, out, nullptr, nullptr, pcg) : launch_small<2, 0>(h, in, out, nullptr, nullptr));

@@ -348,6 +348,45 @@ def test_fused_group_forward_solve_path(B, torch_, rel, monkeypatch):
         check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
 
 
+def test_banded_factor_path(B, torch_, rel, monkeypatch):
+    """SURVEY 8(f) NEXT-2, opt-in (BJ_BAND=1): when every diagonal block is banded (w <= 2) the factor keeps the band and
+    only (w+1) b doubles per block are stored and streamed.  Same parity bar as the dense-packed path; blocks that are
+    not banded fall back to it."""
+    import scipy.sparse as sp
+    monkeypatch.setenv("BJ_BAND", "1")
+    n = 5000
+    T = sp.diags([-np.ones(n - 1), 2.5 * np.ones(n), -np.ones(n - 1)], [-1, 0, 1], format="csr")
+    penta = W.from_scipy((T @ T).tocsr(), {"name": "pentadiagonal"})        # w = 2 inside every block
+    cases = [(mat(4, "small"), 16, 1), (mat(2, "small"), 16, 1), (mat(4, "small"), 32, 1), (penta, 24, 2), (penta, 9, 2),
+             (W.block_diagonal_spd(2000, 1), 16, 0), (mat(3, "small"), 32, None), (mat(5, "small"), 24, None)]
+    for A, b, w in cases:
+        h, keep = B.setup_from_host(A, b)
+        info = B.bj_get_info(h)
+        if w is None:
+            assert info["solve_kernel"] == 2 and info["band_width"] == -1     # not banded: dense packed factors
+        else:
+            assert info["solve_kernel"] == 3 and info["band_width"] == w, (b, info)
+            assert info["factor_bytes"] < 8 * A.n * (w + 1) + 8 * 32 * (w + 1) * b + 1
+        B.bj_destroy(h)
+        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 0),))
+        h, keep = B.setup_from_host(A, b)
+        P = oracle.Precond(A, b)
+        g = B.bj_cond_estimate_ex(h, 20, reorth=True)
+        c = P.cond_estimate(20, reorth=True)
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+        rhs = W.seeded_vector(5, A.n)
+        gp = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=8, rtol=0.0)
+        cp = P.pcg(rhs, 8, 0.0)
+        assert np.allclose(gp["alpha"], cp["alpha"], rtol=1e-9, atol=0)
+        B.bj_destroy(h)
+    # a banded block that is not positive definite is reported like any other
+    bad = sp.diags([-np.ones(n - 1), np.r_[2.5 * np.ones(n - 40), -1.0, 2.5 * np.ones(39)], -np.ones(n - 1)], [-1, 0, 1], format="csr")
+    Ab = W.from_scipy(bad, {"name": "indefinite tridiagonal"})
+    with pytest.raises(B.BJError) as ei:
+        B.setup_from_host(Ab, 16)
+    assert ei.value.code == B.BJ_ERR_NOT_SPD and ei.value.bad_block == (n - 40) // 16
+
+
 def test_block_size_sweep_runs_the_real_path(B, torch_):
     """a11: host-side sweep over b; kappa estimates agree with the oracle at the chosen b; b = N/.. ordering sane."""
     from paper_2410_02408_b200 import sweep
