@@ -261,6 +261,21 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
 
     // NEXT-2, opt-in: banded diagonal blocks keep banded factors -- (w+1) b doubles per block instead of b(b+1)/2.
     // Only for b > 8 (the b <= 8 path fuses the forward solve into the SpMV kernel, which the band path does not).
+    if (h->solve_kind == 1 && b >= 4 && env_int("BJ_BAND", 0) != 0 && env_int("BJ_SETUP_WARP", 0) == 0) {
+        // b <= 8: tridiagonal blocks keep bidiagonal factors, 2b - 1 doubles per block instead of b(b+1)/2; same kernels
+        // (thread per block, fused into the SpMV tile kernel, Lanczos / PCG hooks), compile-time / uniform index switch
+        rc = launch_band_width(h);
+        if (rc != BJ_OK) return fail(rc);
+        ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+        if (ce != cudaSuccess) { set_cuda_error(ce, "band width"); return fail(BJ_ERR_CUDA); }
+        if (stt.max_band >= 0 && stt.max_band <= 1) {
+            h->tri = true;
+            h->band = stt.max_band;
+            h->packed = 2 * b - 1;
+            h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * h->packed * kInterleave * (int64_t)sizeof(double);
+        }
+    }
     if (h->solve_kind == 2 && h->nblocks >= 64 && env_int("BJ_BAND", 0) != 0) {
         rc = launch_band_width(h);
         if (rc != BJ_OK) return fail(rc);
@@ -286,7 +301,8 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     // a2-a4 extract + factor; only the padding the kernels do not write needs zeroing
     if (h->solve_kind == 1) {
         const size_t group_bytes = (size_t)h->packed * kInterleave * sizeof(double);
-        if (h->nblocks % kInterleave) ce = cudaMemsetAsync((char*)h->fac_small + fac_a - group_bytes, 0, group_bytes, h->stream);
+        const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;  // (packed may be the compact tridiagonal size)
+        if (h->nblocks % kInterleave) ce = cudaMemsetAsync((char*)h->fac_small + (size_t)(groups - 1) * group_bytes, 0, group_bytes, h->stream);
     } else if (h->solve_kind == 3) {
         // the last interleave group may be partly unused: zero it so that no lane ever reads an uninitialised factor
         const size_t group_bytes = (size_t)(h->band + 1) * b * kInterleave * sizeof(double);
@@ -378,7 +394,7 @@ int bj_get_info(bj_handle_t h, bj_info_t* info)
     info->spmv_kernel = h->spmv_kernel;
     info->spmv_lanes = h->spmv_lanes;
     info->solve_kernel = h->solve_kind;
-    info->band_width = h->solve_kind == 3 ? h->band : -1;
+    info->band_width = (h->solve_kind == 3 || h->tri) ? h->band : -1;
     info->fused_forward = (h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0 && h->solve_kind != 0) ? 1 : 0;
     return BJ_OK;
 }

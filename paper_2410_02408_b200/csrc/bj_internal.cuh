@@ -84,6 +84,7 @@ struct bj_handle_s {
     int solve_kind = 0;  // 0 none, 1 small (interleaved), 2 warp (fwd + bwd packed copies), 3 banded (interleaved band)
     int band = -1;       // kind 3: lower bandwidth w of every diagonal block (0..2)
     double* fac_band = nullptr;  // kind 3: aliases the dense factor storage of the slab
+    bool tri = false;    // kind 1 with BJ_BAND=1: every block is (at most) tridiagonal, compact bidiagonal factors, packed = 2b - 1
     int lanes = 0;       // lanes per block for kind 2 (8, 16 or 32)
     int packed = 0;      // b(b+1)/2
     double* fac_small = nullptr;

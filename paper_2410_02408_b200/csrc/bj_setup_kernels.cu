@@ -227,7 +227,7 @@ template <int B>
 __global__ void __launch_bounds__(128)
 extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restrict__ rp,
                             const int32_t* __restrict__ ci, const double* __restrict__ val,
-                            double* __restrict__ fac, Status* st)
+                            double* __restrict__ fac, Status* st, int tri)
 {
     constexpr int P = B * (B + 1) / 2;
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -284,6 +284,17 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
     if (bad) {
         atomicOr(&st->flags, ST_NOT_SPD);
         atomicMin(&st->bad_block, (long long)k);
+    }
+    if (tri) {
+        // tridiagonal blocks (BJ_BAND=1): the factor is bidiagonal, only the 2B - 1 elements (i, i-1), (i, i) are kept,
+        // element (i, j) at slot i + j
+        double* f = fac + (k >> 5) * (int64_t)((2 * B - 1) * kInterleave) + (k & 31);
+#pragma unroll
+        for (int i = 0; i < B; ++i) {
+            if (i > 0) f[(2 * i - 1) * kInterleave] = d[i * (i + 1) / 2 + i - 1];
+            f[(2 * i) * kInterleave] = 1.0 / d[i * (i + 1) / 2 + i];
+        }
+        return;
     }
     double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
 #pragma unroll
@@ -402,7 +413,8 @@ int launch_extract_factor(bj_handle_s* h)
 #define BJ_CASE(B)                                                                                          \
     case B:                                                                                                 \
         extract_factor_small_kernel<B><<<tb, 128, 0, h->stream>>>(h->n, h->nblocks, h->row_ptr, h->col_idx,  \
-                                                                  h->val, h->fac_small, h->status);         \
+                                                                  h->val, h->fac_small, h->status,          \
+                                                                  h->tri ? 1 : 0);                          \
         break;
         switch (b) {
             BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)

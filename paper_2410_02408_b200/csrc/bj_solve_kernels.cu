@@ -66,13 +66,14 @@ __device__ __forceinline__ void store_rows(double* dst, int64_t lo, int64_t n, b
 
 // LZ: 0 plain, 1 Lanczos prologue (DIR 1: the input is w built on the fly), 2 Lanczos epilogue (DIR 0),
 //     3 PCG update + apply (DIR 2: x += a p, r -= a q on the fly, z = M^-1 r, partials of r.r and r.z)
-template <int B, int DIR, bool VEC, int LZ>
+//     TRI: tridiagonal blocks, compact bidiagonal factor of 2B - 1 elements, element (i, j) at slot i + j
+template <int B, int DIR, bool VEC, int LZ, bool TRI>
 __global__ void __launch_bounds__(128)
 solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                    const double* in, double* out,  // in == out allowed: a thread touches only its own block
                    const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg)
 {
-    constexpr int P = B * (B + 1) / 2;
+    constexpr int P = TRI ? 2 * B - 1 : B * (B + 1) / 2;
     __shared__ double lz_sh[4];
     pdl_trigger();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -136,18 +137,28 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
 #pragma unroll
         for (int i = 0; i < B; ++i) {
             double s = v[i];
+            if (TRI) {
+                if (i > 0) s -= l[2 * i - 1] * v[i - 1];
+                v[i] = s * l[2 * i];
+            } else {
 #pragma unroll
-            for (int j = 0; j < i; ++j) s -= l[i * (i + 1) / 2 + j] * v[j];
-            v[i] = s * l[i * (i + 1) / 2 + i];
+                for (int j = 0; j < i; ++j) s -= l[i * (i + 1) / 2 + j] * v[j];
+                v[i] = s * l[i * (i + 1) / 2 + i];
+            }
         }
     }
     if (DIR == 1 || DIR == 2) {
 #pragma unroll
         for (int i = B - 1; i >= 0; --i) {
             double s = v[i];
+            if (TRI) {
+                if (i + 1 < B) s -= l[2 * i + 1] * v[i + 1];
+                v[i] = s * l[2 * i];
+            } else {
 #pragma unroll
-            for (int j = i + 1; j < B; ++j) s -= l[j * (j + 1) / 2 + i] * v[j];
-            v[i] = s * l[i * (i + 1) / 2 + i];
+                for (int j = i + 1; j < B; ++j) s -= l[j * (j + 1) / 2 + i] * v[j];
+                v[i] = s * l[i * (i + 1) / 2 + i];
+            }
         }
     }
     if (LZ == 2) {
@@ -523,18 +534,25 @@ static int launch_small(bj_handle_s* h, const double* in, double* out, const LzP
     if (pcg && ((int)blocks > pcg->red_rr.cap || (int)blocks > pcg->red_rz.cap)) return BJ_ERR_INVALID_ARG;
     if ((epi && (int)blocks > epi->red.cap) || (pro && (int)blocks > pro->red.cap)) return BJ_ERR_INVALID_ARG;
     cudaError_t e = cudaSuccess;
-#define BJ_CASE(B)                                                                                                          \
-    case B:                                                                                                                 \
-        e = vec ? launch_kernel(solve_small_kernel<B, DIR, true, LZ>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,  \
-                                (const double*)h->fac_small, in, out, pr, ep, pc)                                           \
-                : launch_kernel(solve_small_kernel<B, DIR, false, LZ>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks, \
-                                (const double*)h->fac_small, in, out, pr, ep, pc);                                           \
+#define BJ_LAUNCH_SMALL(B, V, T)                                                                                  \
+    launch_kernel(solve_small_kernel<B, DIR, V, LZ, T>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,     \
+                  (const double*)h->fac_small, in, out, pr, ep, pc)
+#define BJ_CASE(B)                                                                         \
+    case B:                                                                                \
+        e = vec ? BJ_LAUNCH_SMALL(B, true, false) : BJ_LAUNCH_SMALL(B, false, false);      \
+        break;
+#define BJ_CASE_T(B)                                                                       \
+    case B:                                                                                \
+        e = h->tri ? (vec ? BJ_LAUNCH_SMALL(B, true, true) : BJ_LAUNCH_SMALL(B, false, true)) \
+                   : (vec ? BJ_LAUNCH_SMALL(B, true, false) : BJ_LAUNCH_SMALL(B, false, false)); \
         break;
     switch (h->b) {
-        BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
+        BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE_T(4) BJ_CASE_T(5) BJ_CASE_T(6) BJ_CASE_T(7) BJ_CASE_T(8)
         default: return BJ_ERR_INVALID_ARG;
     }
+#undef BJ_CASE_T
 #undef BJ_CASE
+#undef BJ_LAUNCH_SMALL
     if (e != cudaSuccess) { set_cuda_error(e, "solve_small_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }

@@ -112,6 +112,7 @@ struct StreamParams {
     int stage_bytes;
     int su_doubles;      // doubles per su buffer
     int su_bufs;         // number of su buffers (2; FUSE 3: one per stage)
+    int tri;             // FUSE 1: compact bidiagonal factors (tridiagonal blocks), element (i, j) at slot i + j
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
     int lz;              // 1: fused Lanczos epilogue on the rows this kernel writes (FUSE 0 and 1); 2: dot hook (FUSE 0)
@@ -388,9 +389,14 @@ spmv_stream_kernel(const StreamParams p)
                     for (int i = 0; i < kSmallMax; ++i) {
                         if (i < b) {
                             double acc = v[i];
+                            if (p.tri) {  // uniform over the grid
+                                if (i > 0) acc -= f[(2 * i - 1) * kInterleave] * v[i - 1];
+                                v[i] = acc * f[(2 * i) * kInterleave];
+                            } else {
 #pragma unroll
-                            for (int j = 0; j < i; ++j) acc -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
-                            v[i] = acc * f[(i * (i + 1) / 2 + i) * kInterleave];
+                                for (int j = 0; j < i; ++j) acc -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
+                                v[i] = acc * f[(i * (i + 1) / 2 + i) * kInterleave];
+                            }
                         }
                     }
 #pragma unroll
@@ -571,6 +577,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     fill_layout(h, fuse, sp, smem);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
+    sp.tri = h->tri ? 1 : 0;
     sp.early_trigger = (h->tune.pdl_early >> 1) & 1;
     sp.lz = epi ? 1 : (dot_with && dot_red) ? 2 : 0;
     sp.dot_with = dot_with;

@@ -387,6 +387,34 @@ def test_banded_factor_path(B, torch_, rel, monkeypatch):
     assert ei.value.code == B.BJ_ERR_NOT_SPD and ei.value.bad_block == (n - 40) // 16
 
 
+def test_tridiagonal_compact_factors_small_blocks(B, torch_, rel, monkeypatch):
+    """BJ_BAND=1 with b <= 8: tridiagonal blocks keep 2b - 1 factor elements; the same kernels run (thread per block,
+    fused SpMV + solve, fused Lanczos and PCG hooks) with a compact index map."""
+    import scipy.sparse as sp
+    monkeypatch.setenv("BJ_BAND", "1")
+    n = 3001
+    T = sp.diags([-np.ones(n - 1), 2.5 * np.ones(n), -np.ones(n - 1)], [-1, 0, 1], format="csr")
+    penta = W.from_scipy((T @ T).tocsr(), {"name": "pentadiagonal"})
+    for A, b, tri in ((mat(2, "small"), 8, True), (mat(4, "small"), 8, True), (mat(1, "small"), 4, True),
+                      (mat(2, "small"), 5, True), (penta, 8, False), (mat(5, "small"), 3, False)):
+        h, keep = B.setup_from_host(A, b)
+        info = B.bj_get_info(h)
+        assert info["solve_kernel"] == 1
+        assert (info["band_width"] == 1) == tri, (b, info)
+        if tri:
+            assert info["factor_bytes"] == ((A.n + b - 1) // b + 31) // 32 * 32 * (2 * b - 1) * 8
+        P = oracle.Precond(A, b)
+        g = B.bj_cond_estimate_ex(h, 30, reorth=False)      # fused Lanczos step on the compact factors
+        c = P.cond_estimate(30, reorth=False)
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+        rhs = W.seeded_vector(5, A.n)
+        gp = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=8, rtol=0.0)   # fused PCG iteration
+        cp = P.pcg(rhs, 8, 0.0)
+        assert np.allclose(gp["alpha"], cp["alpha"], rtol=1e-9, atol=0)
+        B.bj_destroy(h)
+        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=KERNELS)
+
+
 def test_block_size_sweep_runs_the_real_path(B, torch_):
     """a11: host-side sweep over b; kappa estimates agree with the oracle at the chosen b; b = N/.. ordering sane."""
     from paper_2410_02408_b200 import sweep
