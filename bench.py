@@ -428,6 +428,29 @@ def main():
             B.bj_destroy(h0)
             line["pcg"] = pcg
 
+            # ---- NEXT-2 variant beside the headline: banded / compact factors (own byte model), same matrix and b ----
+            if not args.band and b >= 4:
+                os.environ["BJ_BAND"] = "1"
+                hb = B.bj_setup(rp, ci, val, b)
+                os.environ.pop("BJ_BAND", None)
+                ib = B.bj_get_info(hb)
+                if ib.get("band_width", -1) >= 0:
+                    for _ in range(10):
+                        B.bj_op_apply(hb, x, y)
+                    kb = max(100, args.steps // 10)
+                    e0.record()
+                    for _ in range(kb):
+                        B.bj_op_apply(hb, x, y)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    bus = 1e3 * e0.elapsed_time(e1) / kb
+                    abb = algorithmic_bytes(n, nnz, b, ib["band_width"])
+                    line["banded_variant"] = {"band_width": ib["band_width"], "us_per_apply": bus, "applies_per_s": 1e6 / bus,
+                                              "band_model_bytes": abb["op_apply"], "gbs_band_model": abb["op_apply"] / bus / 1e3,
+                                              "factor_bytes": ib["factor_bytes"], "note": "opt-in (--band 1 / BJ_BAND=1); "
+                                              "fewer bytes than the dense-block count of SURVEY 8(d), own accounting"}
+                B.bj_destroy(hb)
+
             # ---- CPU oracle on the host cores (reported baseline, not the target) -------------------------
             v, reps, cores = time_oracle(A, b, args.cpu_budget_s)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",

@@ -132,30 +132,57 @@ axpy_norm_kernel(int64_t n, double* __restrict__ w, const double* __restrict__ v
     }
 }
 
-// partial[cta * stride + q] = sum over chunk of V_q[i] * w[i],  q = 0..nv-1
+// partial[cta * stride + q] = sum over chunk of V_q[i] * w[i],  q = 0..nv-1.
+// Eight columns per sweep of the chunk (w is read once per eight columns, eight independent load streams per thread),
+// one combined block reduction per sweep: shuffle tree per value, then thread d adds the warp sums of value d in order.
+constexpr int kDotCols = 8;
 __global__ void __launch_bounds__(kReduceThreads)
 multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const double* __restrict__ w,
                         double* __restrict__ partial, int stride, const int* __restrict__ done)
 {
-    __shared__ double sh[kReduceThreads / 32];
+    __shared__ double sh[kReduceThreads / 32][kDotCols];
     pdl_trigger();
     pdl_wait();
     if (done[0]) return;
     const Chunk c = my_chunk(n);
-    for (int q0 = 0; q0 < nv; q0 += 4) {
-        double s[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
-            const double wi = w[i];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int q0 = 0; q0 < nv; q0 += kDotCols) {
+        double s[kDotCols];
 #pragma unroll
-            for (int d = 0; d < 4; ++d)
-                if (q0 + d < nv) s[d] = fma(V[(int64_t)(q0 + d) * n + i], wi, s[d]);
+        for (int d = 0; d < kDotCols; ++d) s[d] = 0.0;
+        const int live = nv - q0 < kDotCols ? nv - q0 : kDotCols;
+        if (live == kDotCols) {
+            for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
+                const double wi = w[i];
+                double vq[kDotCols];
+#pragma unroll
+                for (int d = 0; d < kDotCols; ++d) vq[d] = V[(int64_t)(q0 + d) * n + i];
+#pragma unroll
+                for (int d = 0; d < kDotCols; ++d) s[d] = fma(vq[d], wi, s[d]);
+            }
+        } else {
+            for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
+                const double wi = w[i];
+#pragma unroll
+                for (int d = 0; d < kDotCols; ++d)
+                    if (d < live) s[d] = fma(V[(int64_t)(q0 + d) * n + i], wi, s[d]);
+            }
         }
 #pragma unroll
-        for (int d = 0; d < 4; ++d) {
-            if (q0 + d < nv) {
-                const double r = block_sum(s[d], sh);
-                if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * stride + q0 + d] = r;
-            }
+        for (int d = 0; d < kDotCols; ++d) {
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) s[d] += __shfl_down_sync(0xffffffffu, s[d], off);
+        }
+        __syncthreads();  // the previous sweep's readers are done with sh
+        if (lane == 0) {
+#pragma unroll
+            for (int d = 0; d < kDotCols; ++d) sh[warp][d] = s[d];
+        }
+        __syncthreads();
+        if (threadIdx.x < live) {
+            double r = 0.0;
+            for (int q = 0; q < (int)(blockDim.x >> 5); ++q) r += sh[q][threadIdx.x];
+            partial[(int64_t)blockIdx.x * stride + q0 + threadIdx.x] = r;
         }
     }
 }
@@ -174,7 +201,15 @@ multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __rest
     double s = 0.0;
     for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
         double wi = w[i];
-        for (int q = 0; q < nv; ++q) wi -= coef[q] * V[(int64_t)q * n + i];
+        int q = 0;
+        for (; q + kDotCols <= nv; q += kDotCols) {  // eight loads in flight, subtraction order unchanged
+            double vq[kDotCols];
+#pragma unroll
+            for (int d = 0; d < kDotCols; ++d) vq[d] = V[(int64_t)(q + d) * n + i];
+#pragma unroll
+            for (int d = 0; d < kDotCols; ++d) wi -= coef[q + d] * vq[d];
+        }
+        for (; q < nv; ++q) wi -= coef[q] * V[(int64_t)q * n + i];
         w[i] = wi;
         s = fma(wi, wi, s);
     }
@@ -184,7 +219,8 @@ multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __rest
     }
 }
 
-// one CTA: out[q] = sum_cta partial[cta * stride + q]  (sequential over cta: fixed order)
+// one CTA: out[q] = sum_cta partial[cta * stride + q].  One WARP per coefficient: lane l adds the partials of CTAs
+// l, l + 32, .. (independent loads in flight), then a fixed shuffle tree -- a fixed order, bitwise reproducible.
 __global__ void __launch_bounds__(256)
 finalize_multi_kernel(int nparts, int nv, const double* __restrict__ partial, int stride,
                       double* __restrict__ out, const int* __restrict__ done)
@@ -192,10 +228,13 @@ finalize_multi_kernel(int nparts, int nv, const double* __restrict__ partial, in
     pdl_trigger();
     pdl_wait();
     if (done[0]) return;
-    for (int q = threadIdx.x; q < nv; q += blockDim.x) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int q = warp; q < nv; q += nw) {
         double s = 0.0;
-        for (int p = 0; p < nparts; ++p) s += partial[(int64_t)p * stride + q];
-        out[q] = s;
+        for (int p = lane; p < nparts; p += 32) s += partial[(int64_t)p * stride + q];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+        if (lane == 0) out[q] = s;
     }
 }
 
