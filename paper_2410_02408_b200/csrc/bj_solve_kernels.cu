@@ -347,7 +347,9 @@ __device__ __forceinline__ void fence_proxy_async()
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
-template <int B, int LPB, int DIR>
+// LZ (compile time: the plain solves carry none of the hooks): 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue
+// (DIR 0), 3 PCG update + apply (DIR 2)
+template <int B, int LPB, int DIR, int LZ>
 __global__ void __launch_bounds__(384)
 solve_group_kernel(const GroupParams p)
 {
@@ -396,10 +398,10 @@ solve_group_kernel(const GroupParams p)
     __shared__ double lz_sh[12];
     double alpha = 0.0, beta = 0.0, inv_beta = 0.0, acc = 0.0;  // Lanczos scalars and this thread's dot product
     bool stop = false;
-    if (DIR == 1 && p.lz == 1) stop = lz_prologue_begin(p.pro, alpha);
-    if (DIR == 0 && p.lz == 2) stop = lz_epilogue_begin(p.epi, beta, inv_beta);
+    if (DIR == 1 && LZ == 1) stop = lz_prologue_begin(p.pro, alpha);
+    if (DIR == 0 && LZ == 2) stop = lz_epilogue_begin(p.epi, beta, inv_beta);
     double acc2 = 0.0;  // PCG: r.z
-    if (DIR == 2 && p.lz == 3) stop = pcg_hook_begin(p.pcg, alpha);  // alpha = the CG step length here
+    if (DIR == 2 && LZ == 3) stop = pcg_hook_begin(p.pcg, alpha);  // alpha = the CG step length here
     if (stop) {  // uniform over the grid; the bulk copies already issued must land before the CTA may exit
         for (int s = 0; s < p.stages; ++s)
             if (first + s * stride < p.ntiles) mbar_wait(&full[s], 0u);
@@ -417,14 +419,14 @@ solve_group_kernel(const GroupParams p)
             const int64_t row = row0 + k * 32;
             const bool live = tile < p.ntiles && row < p.n;
             a[k] = c[k] = 0.0;
-            if (DIR == 1 && p.lz == 1) {
+            if (DIR == 1 && LZ == 1) {
                 if (live) a[k] = p.pro.first ? p.pro.w0[row] : p.pro.w[row];
                 if (live && !p.pro.first) c[k] = p.pro.vcur[row];
-            } else if (DIR == 2 && p.lz == 3) {
+            } else if (DIR == 2 && LZ == 3) {
                 if (live) { a[k] = p.pcg.r[row]; c[k] = p.pcg.q[row]; ew[k] = p.pcg.x[row]; ev[k] = p.pcg.p[row]; }
             } else {
                 if (live) a[k] = p.in[row];
-                if (DIR == 0 && p.lz == 2) {  // the epilogue's own operands ride along one tile ahead
+                if (DIR == 0 && LZ == 2) {  // the epilogue's own operands ride along one tile ahead
                     ew[k] = live ? p.epi.w[row] : 0.0;
                     ev[k] = (live && p.epi.vprev) ? p.epi.vprev[row] : 0.0;
                 }
@@ -432,13 +434,13 @@ solve_group_kernel(const GroupParams p)
         }
 #pragma unroll
         for (int k = 0; k < RPL; ++k) {
-            if (DIR == 1 && p.lz == 1) {  // the solve's input is w = w' - alpha v_j, built here and stored once
+            if (DIR == 1 && LZ == 1) {  // the solve's input is w = w' - alpha v_j, built here and stored once
                 const int64_t row = row0 + k * 32;
                 const double wi = a[k] - alpha * c[k];
                 if (tile < p.ntiles && row < p.n) p.pro.w[row] = wi;
                 acc = fma(wi, wi, acc);
                 dst[k] = wi;
-            } else if (DIR == 2 && p.lz == 3) {  // r_new = r - a q (the solve's input, stored once), x += a p
+            } else if (DIR == 2 && LZ == 3) {  // r_new = r - a q (the solve's input, stored once), x += a p
                 const int64_t row = row0 + k * 32;
                 const double ri = a[k] - alpha * c[k];
                 if (tile < p.ntiles && row < p.n) {
@@ -469,7 +471,7 @@ solve_group_kernel(const GroupParams p)
         for (int k = 0; k < RPL; ++k) r[k] = xchg[g * XB + k * LPB + l];
         double ew[RPL], ev[RPL];
 #pragma unroll
-        for (int k = 0; k < RPL; ++k) { ew[k] = (DIR == 2 && p.lz == 3) ? rn[k] : ewn[k]; ev[k] = evn[k]; }  // PCG: ew = r_new rows
+        for (int k = 0; k < RPL; ++k) { ew[k] = (DIR == 2 && LZ == 3) ? rn[k] : ewn[k]; ev[k] = evn[k]; }  // PCG: ew = r_new rows
         fetch(tile + stride, rn, ewn, evn);  // one tile ahead: its latency hides behind this tile's solve
         mbar_wait(&full[s], ph);
         const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
@@ -487,14 +489,14 @@ solve_group_kernel(const GroupParams p)
             const int64_t row = row0 + k * 32;
             const double y = xchg[(e / B) * XB + e % B];
             if (row < p.n) {
-                if (DIR == 0 && p.lz == 2) {
+                if (DIR == 0 && LZ == 2) {
                     const double vn = ew[k] * inv_beta;              // v_{j+1}
                     const double wi = y * inv_beta - beta * ev[k];   // w'_new (ev = 0 on the first step)
                     p.epi.vnew[row] = vn;
                     p.epi.w[row] = wi;
                     acc = fma(vn, wi, acc);
                 } else {
-                    if (DIR == 2 && p.lz == 3) acc2 = fma(ew[k], y, acc2);  // r_new . z
+                    if (DIR == 2 && LZ == 3) acc2 = fma(ew[k], y, acc2);  // r_new . z
                     p.out[row] = y;
                 }
             }
@@ -505,9 +507,9 @@ solve_group_kernel(const GroupParams p)
             issue(tile + (int64_t)p.stages * stride, s);
         }
     }
-    if (DIR == 1 && p.lz == 1) lz_reduce_finish(p.pro.red, acc, lz_sh);
-    if (DIR == 0 && p.lz == 2) lz_reduce_finish(p.epi.red, acc, lz_sh);
-    if (DIR == 2 && p.lz == 3) {
+    if (DIR == 1 && LZ == 1) lz_reduce_finish(p.pro.red, acc, lz_sh);
+    if (DIR == 0 && LZ == 2) lz_reduce_finish(p.epi.red, acc, lz_sh);
+    if (DIR == 2 && LZ == 3) {
         lz_reduce_finish(p.pcg.red_rr, acc, lz_sh);
         __syncthreads();
         lz_reduce_finish(p.pcg.red_rz, acc2, lz_sh);
@@ -633,8 +635,10 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     warps = std::max(1, std::min(warps, h->tune.group_warps));
     const size_t smem = (size_t)warps * (64 + xchg_bytes + stages * stage_bytes);
     static bool configured[64] = {};
+    static bool configured_hook[64] = {};
     {
-        cudaError_t e = ensure_big_smem(solve_group_kernel<B, LPB, DIR>, configured);
+        cudaError_t e = ensure_big_smem(solve_group_kernel<B, LPB, DIR, 0>, configured);
+        if (e == cudaSuccess) e = ensure_big_smem(solve_group_kernel<B, LPB, DIR, (DIR == 1 ? 1 : DIR == 0 ? 2 : 3)>, configured_hook);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_group_kernel)"); return BJ_ERR_CUDA; }
     }
     GroupParams gp;
@@ -647,13 +651,15 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     gp.pcg = pcg ? *pcg : PcgHook{};
     gp.pro = pro ? *pro : LzPrologue{};
     gp.epi = epi ? *epi : LzEpilogue{};
+    constexpr int kLz = DIR == 1 ? 1 : DIR == 0 ? 2 : 3;  // the one hook this direction can carry
     int occ = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_group_kernel<B, LPB, DIR>, warps * 32, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_group_kernel<B, LPB, DIR, 0>, warps * 32, smem);
     const int64_t want = (gp.ntiles + warps - 1) / warps;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * std::max(1, occ)));
     if ((gp.lz == 2 && grid > gp.epi.red.cap) || (gp.lz == 1 && grid > gp.pro.red.cap)) return BJ_ERR_INVALID_ARG;
     if (gp.lz == 3 && (grid > gp.pcg.red_rr.cap || grid > gp.pcg.red_rz.cap)) return BJ_ERR_INVALID_ARG;
-    cudaError_t e = launch_kernel(solve_group_kernel<B, LPB, DIR>, grid, warps * 32, smem, h->stream, h->pdl && !h->prof_on, gp);
+    cudaError_t e = gp.lz ? launch_kernel(solve_group_kernel<B, LPB, DIR, kLz>, grid, warps * 32, smem, h->stream, h->pdl && !h->prof_on, gp)
+                          : launch_kernel(solve_group_kernel<B, LPB, DIR, 0>, grid, warps * 32, smem, h->stream, h->pdl && !h->prof_on, gp);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_group_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }

@@ -112,7 +112,6 @@ struct StreamParams {
     int stage_bytes;
     int su_doubles;      // doubles per su buffer
     int su_bufs;         // number of su buffers (2; FUSE 3: one per stage)
-    int tri;             // FUSE 1: compact bidiagonal factors (tridiagonal blocks), element (i, j) at slot i + j
     unsigned b_magic;    // ceil(2^32 / b): i / b == (i * b_magic) >> 32 for 0 <= i < 65536
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
     int lz;              // 1: fused Lanczos epilogue on the rows this kernel writes (FUSE 0 and 1); 2: dot hook (FUSE 0)
@@ -128,9 +127,11 @@ __device__ __forceinline__ void consumer_bar_sync(int nthreads)
 
 // LPR lanes per row; BATCH entries per lane in flight per round;
 // FUSE: 0 = SpMV only, 1 = + forward solve, thread per block (b <= 8), 2 = + forward solve, sub-warp of W lanes per block,
+//           (W == 1 with FUSE 1: the blocks are tridiagonal and the factors compact, element (i, j) at slot i + j)
 //       3 = + forward solve, group of lanes per block (bj_device.cuh), W = the compile-time block size (16, 24, 32):
 //           the solving warps rotate from tile to tile and the other warps go on to the next tile meanwhile
-template <int LPR, int BATCH, int FUSE, int W>
+// LZ (compile time, so that the plain operator kernel carries none of it): 0 plain, 1 fused Lanczos epilogue, 2 dot hook
+template <int LPR, int BATCH, int FUSE, int W, int LZ>
 __global__ void __launch_bounds__(kMaxStreamThreads)
 spmv_stream_kernel(const StreamParams p)
 {
@@ -164,7 +165,7 @@ spmv_stream_kernel(const StreamParams p)
     const int R = p.R;
     __shared__ double lz_sh[kMaxStreamThreads / 32];
     double pa = 0.0, beta = 0.0, inv_beta = 0.0;
-    if (p.lz == 1) {  // beta and the stop flag come from the previous kernel: every thread waits for it
+    if (LZ == 1) {  // beta and the stop flag come from the previous kernel: every thread waits for it
         pdl_wait();
         if (lz_epilogue_begin(p.epi, beta, inv_beta)) return;  // uniform over the grid, nothing in flight yet
     }
@@ -303,10 +304,10 @@ spmv_stream_kernel(const StreamParams p)
                         const int kb = i / GB;
                         sub_u[kb * XB + (i - kb * GB)] = acc;
                     } else {
-                        if (p.lz == 1) {
+                        if (LZ == 1) {
                             lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, acc, pa);
                         } else {
-                            if (p.lz == 2) pa = fma(p.dot_with[r0 + i], acc, pa);
+                            if (LZ == 2) pa = fma(p.dot_with[r0 + i], acc, pa);
                             p.y[r0 + i] = acc;
                         }
                     }
@@ -385,19 +386,25 @@ spmv_stream_kernel(const StreamParams p)
                     double v[kSmallMax];
 #pragma unroll
                     for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < p.n) ? uk[i] : 0.0;
+                    if (FUSE == 1 && W == 1) {  // compact bidiagonal factors (tridiagonal blocks): compile-time variant, W == 1 marks it
+#pragma unroll
+                        for (int i = 0; i < kSmallMax; ++i) {
+                            if (i < b) {
+                                double acc = v[i];
+                                if (i > 0) acc -= f[(2 * i - 1) * kInterleave] * v[i - 1];
+                                v[i] = acc * f[(2 * i) * kInterleave];
+                            }
+                        }
+                    } else {
 #pragma unroll
                     for (int i = 0; i < kSmallMax; ++i) {
                         if (i < b) {
                             double acc = v[i];
-                            if (p.tri) {  // uniform over the grid
-                                if (i > 0) acc -= f[(2 * i - 1) * kInterleave] * v[i - 1];
-                                v[i] = acc * f[(2 * i) * kInterleave];
-                            } else {
 #pragma unroll
-                                for (int j = 0; j < i; ++j) acc -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
-                                v[i] = acc * f[(i * (i + 1) / 2 + i) * kInterleave];
-                            }
+                            for (int j = 0; j < i; ++j) acc -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
+                            v[i] = acc * f[(i * (i + 1) / 2 + i) * kInterleave];
                         }
+                    }
                     }
 #pragma unroll
                     for (int i = 0; i < kSmallMax; ++i)
@@ -409,7 +416,7 @@ spmv_stream_kernel(const StreamParams p)
                 for (int i = ctid; i < rows; i += nct) {
                     const int k = (int)__umulhi((unsigned)i, p.b_magic);
                     const double yv = sub_u[k * p.bs + (i - k * b)];
-                    if (p.lz == 1) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, yv, pa);
+                    if (LZ == 1) lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, yv, pa);
                     else p.y[r0 + i] = yv;
                 }
             }
@@ -417,23 +424,23 @@ spmv_stream_kernel(const StreamParams p)
             if (lane == 0) mbar_arrive(&empty[s]);
         }
     }
-    if (p.lz == 1) lz_reduce_finish(p.epi.red, pa, lz_sh);
-    if (p.lz == 2) lz_reduce_finish(p.dot_red, pa, lz_sh);
+    if (LZ == 1) lz_reduce_finish(p.epi.red, pa, lz_sh);
+    if (LZ == 2) lz_reduce_finish(p.dot_red, pa, lz_sh);
 }
 
-template <int LPR, int BATCH, int FUSE, int W>
+template <int LPR, int BATCH, int FUSE, int W, int LZ = 0>
 int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
     static bool configured[64] = {};
     {
-        cudaError_t e = ensure_big_smem(spmv_stream_kernel<LPR, BATCH, FUSE, W>, configured);
+        cudaError_t e = ensure_big_smem(spmv_stream_kernel<LPR, BATCH, FUSE, W, LZ>, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_stream_kernel<LPR, BATCH, FUSE, W>, threads, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_stream_kernel<LPR, BATCH, FUSE, W, LZ>, threads, smem);
     const int per_sm = std::max(1, std::min(occ, want_per_sm));
     const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
-    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, BATCH, FUSE, W>, grid, threads, smem, h->stream,
+    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, BATCH, FUSE, W, LZ>, grid, threads, smem, h->stream,
                                   h->pdl && !h->prof_on, sp);
     if (e != cudaSuccess) { set_cuda_error(e, "spmv_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
@@ -577,7 +584,6 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     fill_layout(h, fuse, sp, smem);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.x = x; sp.y = y;
-    sp.tri = h->tri ? 1 : 0;
     sp.early_trigger = (h->tune.pdl_early >> 1) & 1;
     sp.lz = epi ? 1 : (dot_with && dot_red) ? 2 : 0;
     sp.dot_with = dot_with;
@@ -595,8 +601,13 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
         const int mode = !fuse ? 0 : (h->solve_kind == 1 ? 1 : h->fuse_group ? (h->b == 16 ? 4 : h->b == 24 ? 5 : 6) : (h->lanes == 16 ? 2 : 3));
 #define BJ_CASE(L)                                                                               \
     case L:                                                                                      \
-        rc = mode == 0   ? launch_stream_t<L, 8, 0, 32>(h, sp, grid, threads, smem)               \
-             : mode == 1 ? launch_stream_t<L, 8, 1, 32>(h, sp, grid, threads, smem)               \
+        rc = mode == 0   ? (sp.lz == 1   ? launch_stream_t<L, 8, 0, 32, 1>(h, sp, grid, threads, smem)  \
+                            : sp.lz == 2 ? launch_stream_t<L, 8, 0, 32, 2>(h, sp, grid, threads, smem)  \
+                                         : launch_stream_t<L, 8, 0, 32, 0>(h, sp, grid, threads, smem)) \
+             : mode == 1 ? (h->tri ? (sp.lz == 1 ? launch_stream_t<L, 8, 1, 1, 1>(h, sp, grid, threads, smem)    \
+                                                 : launch_stream_t<L, 8, 1, 1, 0>(h, sp, grid, threads, smem))   \
+                                   : (sp.lz == 1 ? launch_stream_t<L, 8, 1, 32, 1>(h, sp, grid, threads, smem)   \
+                                                 : launch_stream_t<L, 8, 1, 32, 0>(h, sp, grid, threads, smem))) \
              : mode == 2 ? launch_stream_t<L, 8, 2, 16>(h, sp, grid, threads, smem)               \
                          : launch_stream_t<L, 8, 2, 32>(h, sp, grid, threads, smem);              \
         break;
