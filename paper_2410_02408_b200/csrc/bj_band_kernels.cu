@@ -16,6 +16,7 @@
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
+#include "bj_pcg_fuse.cuh"
 
 namespace bj {
 
@@ -121,31 +122,109 @@ extract_factor_band_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __r
     }
 }
 
-// thread per block; BMAX bounds the register arrays (b <= BMAX); DIR 0 forward, 1 backward, 2 both
-template <int BMAX, int W, int DIR>
-__global__ void __launch_bounds__(128)
-solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ fac, const double* in, double* out)
+// rows lo .. lo + b - 1 of a vector <-> registers (b <= BMAX at run time); 256-bit accesses when `vec`
+template <int BMAX>
+__device__ __forceinline__ void load_rows_rt(const double* src, int64_t lo, int64_t n, int b, bool vec, double (&v)[BMAX])
 {
+    if (vec) {
+#pragma unroll
+        for (int i = 0; i < BMAX; i += 4)
+            if (i < b) ld_v4(src + lo + i, v + i);
+    } else {
+#pragma unroll
+        for (int i = 0; i < BMAX; ++i) v[i] = (i < b && lo + i < n) ? src[lo + i] : 0.0;
+    }
+}
+template <int BMAX>
+__device__ __forceinline__ void store_rows_rt(double* dst, int64_t lo, int64_t n, int b, bool vec, const double (&v)[BMAX])
+{
+    if (vec) {
+#pragma unroll
+        for (int i = 0; i < BMAX; i += 4)
+            if (i < b) st_v4(dst + lo + i, v + i);
+    } else {
+#pragma unroll
+        for (int i = 0; i < BMAX; ++i)
+            if (i < b && lo + i < n) dst[lo + i] = v[i];
+    }
+}
+
+// thread per block; BMAX bounds the register arrays (b <= BMAX); DIR 0 forward, 1 backward, 2 both.
+// LZ (compile time): 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0), 3 PCG update + apply (DIR 2) --
+// the same hooks, in the same order of operations, as solve_small_kernel (bj_solve_kernels.cu).
+template <int BMAX, int W, int DIR, int LZ>
+__global__ void __launch_bounds__(128)
+solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ fac, const double* in, double* out,
+                  const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg)
+{
+    __shared__ double lz_sh[4];
     pdl_trigger();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= nblocks) return;
+    const bool act = k < nblocks;
+    if (LZ == 0 && !act) return;
+    const int64_t kc = act ? k : 0;
     const int E = (W + 1) * b;
-    const double* f = fac + (k >> 5) * (int64_t)E * kInterleave + (k & 31);
-    const int64_t lo = k * b;
-    const bool vec = (b % 4 == 0) && lo + b <= n && (((uintptr_t)in | (uintptr_t)out) & 31) == 0;
+    const double* f = fac + (kc >> 5) * (int64_t)E * kInterleave + (kc & 31);
+    const int64_t lo = kc * b;
+    uintptr_t al = (uintptr_t)in | (uintptr_t)out;
+    if (LZ == 1) al = (uintptr_t)pro.w0 | (uintptr_t)pro.w | (uintptr_t)pro.vcur;
+    if (LZ == 2) al |= (uintptr_t)epi.w | (uintptr_t)epi.vprev | (uintptr_t)epi.vnew;
+    if (LZ == 3) al = (uintptr_t)out | (uintptr_t)pcg.x | (uintptr_t)pcg.p | (uintptr_t)pcg.r | (uintptr_t)pcg.q;
+    const bool vec = (b % 4 == 0) && lo + b <= n && (al & 31) == 0;
     // the whole band goes to registers first: (W+1) b independent, coalesced loads in flight per thread
     double l[(W + 1) * BMAX];
 #pragma unroll
     for (int e = 0; e < (W + 1) * BMAX; ++e) l[e] = (e < E) ? ld_const_stream(f + e * kInterleave) : 0.0;
     pdl_wait();  // `in` may come from the previous kernel
     double v[BMAX];
-    if (vec) {
+    double acc = 0.0, acc2 = 0.0, beta = 0.0, inv_beta = 0.0;
+    double rin[LZ == 3 ? BMAX : 1];
+    if (LZ == 1) {
+        double alpha;
+        if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
+        if (act) {
+            if (pro.first) {
+                load_rows_rt<BMAX>(pro.w0, lo, n, b, vec, v);
+            } else {
+                double c[BMAX];
+                load_rows_rt<BMAX>(pro.w, lo, n, b, vec, v);
+                load_rows_rt<BMAX>(pro.vcur, lo, n, b, vec, c);
 #pragma unroll
-        for (int i = 0; i < BMAX; i += 4)
-            if (i < b) ld_v4(in + lo + i, v + i);
+                for (int i = 0; i < BMAX; ++i)
+                    if (i < b) v[i] -= alpha * c[i];
+            }
+#pragma unroll
+            for (int i = 0; i < BMAX; ++i)
+                if (i < b && lo + i < n) acc = fma(v[i], v[i], acc);
+            store_rows_rt<BMAX>(pro.w, lo, n, b, vec, v);
+        }
+    } else if (LZ == 3) {
+        double a;
+        if (pcg_hook_begin(pcg, a)) return;  // uniform over the grid
+        if (act) {
+            double c[BMAX];
+            load_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
+            load_rows_rt<BMAX>(pcg.q, lo, n, b, vec, c);
+#pragma unroll
+            for (int i = 0; i < BMAX; ++i) {
+                if (i < b) {
+                    v[i] = v[i] - a * c[i];
+                    if (lo + i < n) acc = fma(v[i], v[i], acc);
+                    rin[i] = v[i];
+                }
+            }
+            store_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
+            double xs[BMAX];
+            load_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
+            load_rows_rt<BMAX>(pcg.p, lo, n, b, vec, c);
+#pragma unroll
+            for (int i = 0; i < BMAX; ++i)
+                if (i < b) xs[i] = fma(a, c[i], xs[i]);
+            store_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
+        }
     } else {
-#pragma unroll
-        for (int i = 0; i < BMAX; ++i) v[i] = (i < b && lo + i < n) ? in[lo + i] : 0.0;
+        if (LZ == 2 && lz_epilogue_begin(epi, beta, inv_beta)) return;  // uniform over the grid
+        load_rows_rt<BMAX>(in, lo, n, b, vec, v);
     }
     if (DIR == 0 || DIR == 2) {
 #pragma unroll
@@ -171,28 +250,59 @@ solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
             }
         }
     }
-    if (vec) {
+    if (LZ == 2) {
+        if (act) {
+            double c[BMAX], d[BMAX];  // w and v_j
+            load_rows_rt<BMAX>(epi.w, lo, n, b, vec, c);
+            if (epi.vprev) load_rows_rt<BMAX>(epi.vprev, lo, n, b, vec, d);
 #pragma unroll
-        for (int i = 0; i < BMAX; i += 4)
-            if (i < b) st_v4(out + lo + i, v + i);
+            for (int i = 0; i < BMAX; ++i) {
+                if (i < b) {
+                    c[i] *= inv_beta;                       // v_{j+1}
+                    v[i] *= inv_beta;
+                    if (epi.vprev) v[i] -= beta * d[i];     // w'_new
+                    if (lo + i < n) acc = fma(c[i], v[i], acc);
+                }
+            }
+            store_rows_rt<BMAX>(epi.vnew, lo, n, b, vec, c);
+            store_rows_rt<BMAX>(epi.w, lo, n, b, vec, v);
+        }
+        lz_reduce_finish(epi.red, acc, lz_sh);
     } else {
+        if (act) store_rows_rt<BMAX>(out, lo, n, b, vec, v);
+        if (LZ == 1) lz_reduce_finish(pro.red, acc, lz_sh);
+        if (LZ == 3) {
+            if (act) {
 #pragma unroll
-        for (int i = 0; i < BMAX; ++i)
-            if (i < b && lo + i < n) out[lo + i] = v[i];
+                for (int i = 0; i < BMAX; ++i)
+                    if (i < b && lo + i < n) acc2 = fma(rin[i], v[i], acc2);
+            }
+            lz_reduce_finish(pcg.red_rr, acc, lz_sh);
+            __syncthreads();
+            lz_reduce_finish(pcg.red_rz, acc2, lz_sh);
+        }
     }
 }
 
 template <int BMAX, int W>
-int launch_band_t(bj_handle_s* h, int dir, const double* in, double* out)
+int launch_band_t(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                  const PcgHook* pcg)
 {
     const unsigned blocks = (unsigned)((h->nblocks + 127) / 128);
     const bool pdl = h->pdl && !h->prof_on;
-    cudaError_t e = dir == 0   ? launch_kernel(solve_band_kernel<BMAX, W, 0>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,
-                                               (const double*)h->fac_band, in, out)
-                    : dir == 1 ? launch_kernel(solve_band_kernel<BMAX, W, 1>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,
-                                               (const double*)h->fac_band, in, out)
-                               : launch_kernel(solve_band_kernel<BMAX, W, 2>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,
-                                               (const double*)h->fac_band, in, out);
+    const LzPrologue pr = pro ? *pro : LzPrologue{};
+    const LzEpilogue ep = epi ? *epi : LzEpilogue{};
+    const PcgHook pc = pcg ? *pcg : PcgHook{};
+    if ((pro && (int)blocks > pro->red.cap) || (epi && (int)blocks > epi->red.cap) ||
+        (pcg && ((int)blocks > pcg->red_rr.cap || (int)blocks > pcg->red_rz.cap)))
+        return BJ_ERR_INVALID_ARG;
+#define BJ_BAND_LAUNCH(D, L)                                                                                          \
+    launch_kernel(solve_band_kernel<BMAX, W, D, L>, blocks, 128, 0, h->stream, pdl, h->n, h->b, h->nblocks,             \
+                  (const double*)h->fac_band, in, out, pr, ep, pc)
+    cudaError_t e = dir == 0   ? (epi ? BJ_BAND_LAUNCH(0, 2) : BJ_BAND_LAUNCH(0, 0))
+                    : dir == 1 ? (pro ? BJ_BAND_LAUNCH(1, 1) : BJ_BAND_LAUNCH(1, 0))
+                               : (pcg ? BJ_BAND_LAUNCH(2, 3) : BJ_BAND_LAUNCH(2, 0));
+#undef BJ_BAND_LAUNCH
     if (e != cudaSuccess) { set_cuda_error(e, "solve_band_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
@@ -226,13 +336,14 @@ int launch_extract_factor_band(bj_handle_s* h)
     return BJ_OK;
 }
 
-int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out)
+int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                      const PcgHook* pcg)
 {
     const bool small = h->b <= 16;
     switch (h->band) {
-        case 0: return small ? launch_band_t<16, 0>(h, dir, in, out) : launch_band_t<32, 0>(h, dir, in, out);
-        case 1: return small ? launch_band_t<16, 1>(h, dir, in, out) : launch_band_t<32, 1>(h, dir, in, out);
-        case 2: return small ? launch_band_t<16, 2>(h, dir, in, out) : launch_band_t<32, 2>(h, dir, in, out);
+        case 0: return small ? launch_band_t<16, 0>(h, dir, in, out, pro, epi, pcg) : launch_band_t<32, 0>(h, dir, in, out, pro, epi, pcg);
+        case 1: return small ? launch_band_t<16, 1>(h, dir, in, out, pro, epi, pcg) : launch_band_t<32, 1>(h, dir, in, out, pro, epi, pcg);
+        case 2: return small ? launch_band_t<16, 2>(h, dir, in, out, pro, epi, pcg) : launch_band_t<32, 2>(h, dir, in, out, pro, epi, pcg);
         default: return BJ_ERR_INVALID_ARG;
     }
 }

@@ -162,19 +162,21 @@ struct KernelScope {
     ~KernelScope();
 };
 
-struct LzPrologue;
-struct LzEpilogue;
-struct PcgHook;
 
 // setup (bj_setup_kernels.cu)
 int launch_validate(bj_handle_s* h);
 int launch_extract_factor(bj_handle_s* h);
 int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nnz
 
+struct LzPrologue;
+struct LzEpilogue;
+struct PcgHook;
+
 // banded block factors (bj_band_kernels.cu), opt-in
 int launch_band_width(bj_handle_s* h);            // Status.max_band
 int launch_extract_factor_band(bj_handle_s* h);   // a2 + a3 into fac_band
-int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out);
+int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
+                      const PcgHook* pcg);
 
 // solves (bj_solve_kernels.cu): dir 0 = forward (L^-1), 1 = backward (L^-T), 2 = both (apply)
 // pro (dir 1 only) / epi (dir 0 only): fused Lanczos hooks of bj_lanczos_fuse.cuh, null for a plain solve

@@ -688,7 +688,7 @@ static bool use_group_kernel(const bj_handle_s* h)
 // kind 1 always carries the hooks; kind 2 only in the group kernel (b = 16, 24, 32); b = 0 has no solve to ride on
 bool lanczos_fusable(const bj_handle_s* h)
 {
-    return h->solve_kind == 1 || (h->solve_kind == 2 && use_group_kernel(h));
+    return h->solve_kind == 1 || h->solve_kind == 3 || (h->solve_kind == 2 && use_group_kernel(h));
 }
 
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro, const LzEpilogue* epi,
@@ -705,7 +705,7 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const L
     {
         KernelScope scope(h, kind);
         if (h->solve_kind == 3) {
-            rc = launch_solve_band(h, dir, in, out);
+            rc = launch_solve_band(h, dir, in, out, pro, epi, pcg);
         } else if (h->solve_kind == 1) {
             rc = dir == 0   ? (epi ? launch_small<0, 2>(h, in, out, nullptr, epi) : launch_small<0, 0>(h, in, out, nullptr, nullptr))
                  : dir == 1 ? (pro ? launch_small<1, 1>(h, in, out, pro, nullptr) : launch_small<1, 0>(h, in, out, nullptr, nullptr))
