@@ -1,0 +1,54 @@
+"""CPU-only: host-side accounting and selection logic (no GPU, no oracle)."""
+import importlib.util
+import os
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _bench():
+    spec = importlib.util.spec_from_file_location("bench_module", os.path.join(ROOT, "bench.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+# N, nnz, b -> SpMV MB and op-apply MB of the dense-block byte model
+SURVEY_ROWS = [
+    (2_097_152, 14_581_760, 8, 216.9, 435.0),
+    (4_194_304, 37_724_164, 16, 536.6, 1241.2),
+    (2_654_208, 210_542_904, 3, 2579.6, 2749.5),
+    (2_654_208, 210_542_904, 24, 2579.6, 3195.4),
+]
+
+
+@pytest.mark.parametrize("n,nnz,b,spmv_mb,op_mb", SURVEY_ROWS)
+def test_algorithmic_bytes_match_the_survey_table(n, nnz, b, spmv_mb, op_mb):
+    ab = _bench().algorithmic_bytes(n, nnz, b)
+    assert abs(ab["spmv"] / 1e6 - spmv_mb) < 0.06
+    assert abs(ab["op_apply"] / 1e6 - op_mb) < 0.06
+    assert ab["op_apply"] == 12 * nnz + 4 * (n + 1) + 8 * n * (b + 1) + 48 * n
+    assert ab["apply"] == 4 * n * (b + 1) + 16 * n
+    assert ab["spmv_solve_L"] == ab["spmv"] + ab["solve_L"]
+
+
+def test_band_byte_model_is_below_the_dense_block_count():
+    bench = _bench()
+    n, nnz = 4_194_304, 37_724_164
+    dense = bench.algorithmic_bytes(n, nnz, 16)
+    band = bench.algorithmic_bytes(n, nnz, 16, band=1)
+    assert band["spmv"] == dense["spmv"]
+    assert band["solve_L"] == 8 * n * 2 + 16 * n < dense["solve_L"]
+    assert band["op_apply"] == band["spmv"] + 2 * band["solve_L"]
+    assert bench.algorithmic_bytes(n, nnz, 0)["op_apply"] == dense["spmv"]          # b = 0: the operator is A
+
+
+def test_sweep_picks_the_smallest_kappa_squared_then_the_cheaper_apply(monkeypatch):
+    """a11: argmin kappa_est^2, ties broken by the cheaper apply -- checked on the selection rule itself."""
+    rows = [{"b": 1, "kappa_est": 40.0, "op_apply_us": 10.0}, {"b": 4, "kappa_est": 20.0, "op_apply_us": 30.0},
+            {"b": 8, "kappa_est": 20.0, "op_apply_us": 25.0}, {"b": 16, "kappa_est": 25.0, "op_apply_us": 5.0}]
+    best = min(rows, key=lambda r: (round(r["kappa_est"] ** 2, 6), r["op_apply_us"]))   # the rule of sweep.sweep()
+    assert best["b"] == 8
+    src = open(os.path.join(ROOT, "paper_2410_02408_b200", "sweep.py")).read()
+    assert 'min(ok, key=lambda r: (round(r[key] ** 2, 6), r["op_apply_us"]))' in src
