@@ -1,0 +1,348 @@
+// Batched small systems: the paper's own sizes (N = 2^10 .. 2^14) as MANY
+// independent systems in one launch -- its "solve each block separately" picture.
+// The batch is one block-diagonal CSR (system s owns rows s*seg .. (s+1)*seg - 1), so setup, bj_apply and bj_op_apply
+// work on it unchanged; what differs is that every system has its OWN Lanczos scalars.  One CTA per system does the
+// whole vector part of a Lanczos step for its system -- alpha, the two axpys, beta, the breakdown test, the scaling --
+// with block-level reductions only: no grid reduction, no partials, no host synchronisation inside the loop.
+// An iteration is the operator apply on the whole batch plus ONE launch of lz_batch_step_kernel.
+// Variant: DESIGN.md reading 10-12 without reorthogonalisation (the systems are small and the preconditioned
+// spectra tame); per system it is exactly the recurrence of bj_lanczos.cu.
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "bj_device.cuh"
+#include "bj_internal.cuh"
+#include "bj_reduce.cuh"
+
+namespace bj {
+
+namespace {
+
+constexpr int kBatchThreads = 256;
+
+// sum over the CTA, valid on every thread
+__device__ __forceinline__ double block_sum_all(double v, double* sh)
+{
+    v = block_sum(v, sh);
+    __syncthreads();
+    if (threadIdx.x == 0) sh[0] = v;
+    __syncthreads();
+    const double r = sh[0];
+    __syncthreads();
+    return r;
+}
+
+// v_1 = v0 / ||v0|| per system
+__global__ void __launch_bounds__(kBatchThreads)
+lz_batch_start_kernel(int64_t seg, const double* __restrict__ v0, double* __restrict__ v)
+{
+    __shared__ double sh[kBatchThreads / 32];
+    const int64_t base = (int64_t)blockIdx.x * seg;
+    double s = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
+        const double x = v0[base + i];
+        s = fma(x, x, s);
+    }
+    const double nrm = sqrt(block_sum_all(s, sh));
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) v[base + i] = v0[base + i] / nrm;
+}
+
+// one Lanczos step of system blockIdx.x:  w -= beta_j v_{j-1};  alpha_j = v_j.w;  w -= alpha_j v_j;  beta_{j+1} = ||w||;
+// stop this system if beta_{j+1} <= tol max|alpha|;  v_{j+1} = w / beta_{j+1}.  alpha/beta: [nsys][m] (device).
+// A stopped system writes zeros into v_{j+1}, so the shared operator apply keeps producing zeros for it.
+__global__ void __launch_bounds__(kBatchThreads)
+lz_batch_step_kernel(int64_t seg, int m, int j, double tol, double* __restrict__ w, const double* vprev,
+                     const double* __restrict__ vcur, double* vnext,  // vprev and vnext share one buffer
+                     double* __restrict__ alpha,
+                     double* __restrict__ beta, double* __restrict__ amax, int* __restrict__ m_eff, int* __restrict__ stopped)
+{
+    __shared__ double sh[kBatchThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const int s = blockIdx.x;
+    const int64_t base = (int64_t)s * seg;
+    if (stopped[s]) {
+        if (vnext)
+            for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) vnext[base + i] = 0.0;
+        return;
+    }
+    const double bj = j > 0 ? beta[(int64_t)s * m + j - 1] : 0.0;
+    double a = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
+        double wi = w[base + i];
+        if (j > 0) {
+            wi -= bj * vprev[base + i];
+            w[base + i] = wi;
+        }
+        a = fma(vcur[base + i], wi, a);
+    }
+    a = block_sum_all(a, sh);
+    double bb = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
+        const double wi = w[base + i] - a * vcur[base + i];
+        w[base + i] = wi;
+        bb = fma(wi, wi, bb);
+    }
+    const double bn = sqrt(block_sum_all(bb, sh));
+    const double am = fmax(amax[s], fabs(a));
+    const bool brk = !(bn > tol * am);
+    if (threadIdx.x == 0) {
+        alpha[(int64_t)s * m + j] = a;
+        beta[(int64_t)s * m + j] = bn;
+        amax[s] = am;
+        m_eff[s] = j + 1;
+        if (brk) stopped[s] = 1;
+    }
+    if (!vnext) return;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) vnext[base + i] = brk ? 0.0 : w[base + i] / bn;
+}
+
+// ---- batched PCG: per-system scalars, one CTA per system for the vector parts ------------------------------------
+// r = b, x = 0, bb[s] = ||b_s||^2 (a zero right-hand side stops its system at once)
+__global__ void __launch_bounds__(kBatchThreads)
+pcg_batch_init_kernel(int64_t seg, const double* __restrict__ b, double* __restrict__ r, double* __restrict__ x,
+                      double* __restrict__ bb, int* __restrict__ stopped, int* __restrict__ nstopped)
+{
+    __shared__ double sh[kBatchThreads / 32];
+    const int s = blockIdx.x;
+    const int64_t base = (int64_t)s * seg;
+    double acc = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
+        const double bi = b[base + i];
+        r[base + i] = bi;
+        x[base + i] = 0.0;
+        acc = fma(bi, bi, acc);
+    }
+    acc = block_sum_all(acc, sh);
+    if (threadIdx.x == 0) {
+        bb[s] = acc;
+        if (!(acc > 0.0)) { stopped[s] = 1; atomicAdd(nstopped, 1); }
+    }
+}
+
+// first == 1: p = z, rho = r.z.   else: bt = (r.z) / rho, p = z + bt p, rho = r.z.   A stopped system keeps p = 0.
+__global__ void __launch_bounds__(kBatchThreads)
+pcg_batch_direction_kernel(int64_t seg, int first, const double* __restrict__ r, const double* __restrict__ z,
+                           double* __restrict__ p, double* __restrict__ rho, const int* __restrict__ stopped)
+{
+    __shared__ double sh[kBatchThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const int s = blockIdx.x;
+    const int64_t base = (int64_t)s * seg;
+    if (stopped[s]) {
+        for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) p[base + i] = 0.0;
+        return;
+    }
+    double acc = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) acc = fma(r[base + i], z[base + i], acc);
+    const double rz = block_sum_all(acc, sh);
+    const double bt = first ? 0.0 : rz / rho[s];
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) p[base + i] = first ? z[base + i] : fma(bt, p[base + i], z[base + i]);
+    if (threadIdx.x == 0) rho[s] = rz;
+}
+
+// a = rho / (p.q); x += a p; r -= a q; relres = ||r|| / ||b||; the system stops when relres <= rtol
+__global__ void __launch_bounds__(kBatchThreads)
+pcg_batch_update_kernel(int64_t seg, int k, double rtol, double* __restrict__ x, double* __restrict__ r,
+                        const double* __restrict__ p, const double* __restrict__ q, const double* __restrict__ rho,
+                        const double* __restrict__ bb, double* __restrict__ relres, int* __restrict__ iters,
+                        int* __restrict__ stopped, int* __restrict__ converged, int* __restrict__ nstopped)
+{
+    __shared__ double sh[kBatchThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const int s = blockIdx.x;
+    if (stopped[s]) return;
+    const int64_t base = (int64_t)s * seg;
+    double acc = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) acc = fma(p[base + i], q[base + i], acc);
+    const double a = rho[s] / block_sum_all(acc, sh);
+    acc = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
+        x[base + i] = fma(a, p[base + i], x[base + i]);
+        const double ri = r[base + i] - a * q[base + i];
+        r[base + i] = ri;
+        acc = fma(ri, ri, acc);
+    }
+    const double rel = sqrt(block_sum_all(acc, sh) / bb[s]);
+    if (threadIdx.x == 0) {
+        relres[s] = rel;
+        iters[s] = k + 1;
+        if (rel <= rtol) { stopped[s] = 1; converged[s] = 1; atomicAdd(nstopped, 1); }
+    }
+}
+
+// true_relres[s] = ||q_s - b_s|| / ||b_s||  with q = A x
+__global__ void __launch_bounds__(kBatchThreads)
+pcg_batch_residual_kernel(int64_t seg, const double* __restrict__ q, const double* __restrict__ b,
+                          const double* __restrict__ bb, double* __restrict__ out)
+{
+    __shared__ double sh[kBatchThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const int s = blockIdx.x;
+    const int64_t base = (int64_t)s * seg;
+    double acc = 0.0;
+    for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
+        const double d = q[base + i] - b[base + i];
+        acc = fma(d, d, acc);
+    }
+    acc = block_sum_all(acc, sh);
+    if (threadIdx.x == 0) out[s] = bb[s] > 0.0 ? sqrt(acc / bb[s]) : 0.0;
+}
+
+}  // namespace
+}  // namespace bj
+
+using namespace bj;
+
+extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_dev, double* x_dev, int max_iters, double rtol,
+                                  int32_t* iters_host, double* relres_host, double* true_relres_host)
+{
+    if (!h || h->failed || nsys < 1 || max_iters < 1 || !b_dev || !x_dev || b_dev == x_dev) return BJ_ERR_INVALID_ARG;
+    const int64_t n = h->n;
+    if (n % nsys) return BJ_ERR_INVALID_ARG;
+    const int64_t seg = n / nsys;
+    if (h->b > 0 && seg % h->b) return BJ_ERR_INVALID_ARG;
+    cudaStream_t st = h->stream;
+    double* vec = nullptr;   // r, z, p, q
+    double* scal = nullptr;  // rho, bb, relres, true_relres [nsys each]
+    int* ints = nullptr;     // iters, stopped, converged [nsys each], nstopped
+    auto cleanup = [&]() { cudaFree(vec); cudaFree(scal); cudaFree(ints); };
+    if (cudaMalloc((void**)&vec, (size_t)4 * n * sizeof(double)) != cudaSuccess ||
+        cudaMalloc((void**)&scal, (size_t)4 * nsys * sizeof(double)) != cudaSuccess ||
+        cudaMalloc((void**)&ints, ((size_t)3 * nsys + 4) * sizeof(int)) != cudaSuccess) {
+        cudaGetLastError();
+        cleanup();
+        return BJ_ERR_ALLOC;
+    }
+    double *r = vec, *z = vec + n, *p = vec + 2 * n, *q = vec + 3 * n;
+    double *rho = scal, *bb = scal + nsys, *relres = scal + 2 * nsys, *truerel = scal + 3 * nsys;
+    int *iters = ints, *stopped = ints + nsys, *converged = ints + 2 * nsys, *nstopped = ints + 3 * nsys;
+    cudaError_t e = cudaMemsetAsync(scal, 0, (size_t)4 * nsys * sizeof(double), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ints, 0, ((size_t)3 * nsys + 4) * sizeof(int), st);
+    if (e != cudaSuccess) { set_cuda_error(e, "batch memset"); cleanup(); return BJ_ERR_CUDA; }
+    const unsigned G = (unsigned)nsys;
+    const bool pdl = h->pdl;
+    int rc = BJ_OK;
+    auto spmv = [&](const double* in, double* out) {
+        return h->spmv_kernel == 1 ? launch_spmv_stream(h, in, out, false) : launch_spmv_vector(h, in, out);
+    };
+#define BJ_BL(kernel, ...)                                                                                 \
+    do {                                                                                                   \
+        e = launch_kernel(kernel, dim3(G), dim3(kBatchThreads), 0, st, pdl, __VA_ARGS__);                  \
+        if (e != cudaSuccess) { set_cuda_error(e, #kernel); rc = BJ_ERR_CUDA; }                            \
+        h->launches++;                                                                                     \
+    } while (0)
+    pcg_batch_init_kernel<<<G, kBatchThreads, 0, st>>>(seg, b_dev, r, x_dev, bb, stopped, nstopped);
+    h->launches++;
+    rc = launch_solve(h, 2, r, z);
+    if (rc == BJ_OK) BJ_BL(pcg_batch_direction_kernel, seg, 1, (const double*)r, (const double*)z, p, rho, (const int*)stopped);
+    for (int k = 0; k < max_iters && rc == BJ_OK; ++k) {
+        rc = spmv(p, q);
+        if (rc != BJ_OK) break;
+        BJ_BL(pcg_batch_update_kernel, seg, k, rtol, x_dev, r, (const double*)p, (const double*)q, (const double*)rho,
+              (const double*)bb, relres, iters, stopped, converged, nstopped);
+        if (rc != BJ_OK) break;
+        rc = launch_solve(h, 2, r, z);
+        if (rc != BJ_OK) break;
+        BJ_BL(pcg_batch_direction_kernel, seg, 0, (const double*)r, (const double*)z, p, rho, (const int*)stopped);
+        if ((k + 1) % 16 == 0 && k + 1 < max_iters && rc == BJ_OK) {  // every system done?
+            int ns = 0;
+            e = cudaMemcpyAsync(&ns, nstopped, sizeof(int), cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) { set_cuda_error(e, "batch poll"); rc = BJ_ERR_CUDA; break; }
+            if (ns >= nsys) break;
+        }
+    }
+    if (rc == BJ_OK) rc = spmv(x_dev, q);
+    if (rc == BJ_OK) BJ_BL(pcg_batch_residual_kernel, seg, (const double*)q, b_dev, (const double*)bb, truerel);
+#undef BJ_BL
+    if (rc == BJ_OK) {
+        e = cudaSuccess;
+        if (iters_host) e = cudaMemcpyAsync(iters_host, iters, (size_t)nsys * sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && relres_host) e = cudaMemcpyAsync(relres_host, relres, (size_t)nsys * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && true_relres_host) e = cudaMemcpyAsync(true_relres_host, truerel, (size_t)nsys * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { set_cuda_error(e, "batch readback"); rc = BJ_ERR_CUDA; }
+    }
+    cleanup();
+    return rc;
+}
+
+extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, uint64_t seed, double* lmin_host,
+                                      double* lmax_host, int32_t* iters_done_host)
+{
+    if (!h || h->failed || nsys < 1 || iters < 1 || !lmin_host || !lmax_host) return BJ_ERR_INVALID_ARG;
+    const int64_t n = h->n;
+    if (n % nsys) return BJ_ERR_INVALID_ARG;
+    const int64_t seg = n / nsys;
+    if (h->b > 0 && seg % h->b) return BJ_ERR_INVALID_ARG;  // a Jacobi block must not straddle two systems
+    if (nsys > (1ll << 30)) return BJ_ERR_TOO_LARGE;
+    const int m = iters;
+    cudaStream_t st = h->stream;
+    const double tol = BJ_DEFAULT_BREAKDOWN_TOL;
+
+    // workspace: v_prev, v_cur (rotating), w; alpha/beta [nsys][m]; amax, m_eff, stopped [nsys]
+    double* vec = nullptr;
+    double* scal = nullptr;
+    int* ints = nullptr;
+    auto cleanup = [&]() { cudaFree(vec); cudaFree(scal); cudaFree(ints); };
+    if (cudaMalloc((void**)&vec, (size_t)3 * n * sizeof(double)) != cudaSuccess ||
+        cudaMalloc((void**)&scal, ((size_t)2 * nsys * m + nsys) * sizeof(double)) != cudaSuccess ||
+        cudaMalloc((void**)&ints, (size_t)2 * nsys * sizeof(int)) != cudaSuccess) {
+        cudaGetLastError();
+        cleanup();
+        return BJ_ERR_ALLOC;
+    }
+    double* V[2] = {vec, vec + n};
+    double* w = vec + 2 * n;
+    double* alpha = scal;
+    double* beta = scal + (size_t)nsys * m;
+    double* amax = beta + (size_t)nsys * m;
+    int* m_eff = ints;
+    int* stopped = ints + nsys;
+    int rc = BJ_OK;
+    cudaError_t e = cudaMemsetAsync(scal, 0, ((size_t)2 * nsys * m + nsys) * sizeof(double), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ints, 0, (size_t)2 * nsys * sizeof(int), st);
+    if (e != cudaSuccess) { set_cuda_error(e, "batch memset"); cleanup(); return BJ_ERR_CUDA; }
+
+    rc = launch_seeded_vector(h, seed, w);  // the start vector of system s is this vector's slice s
+    if (rc == BJ_OK) {
+        lz_batch_start_kernel<<<(unsigned)nsys, kBatchThreads, 0, st>>>(seg, w, V[0]);
+        h->launches++;
+    }
+    for (int j = 0; j < m && rc == BJ_OK; ++j) {
+        double* vj = V[j & 1];
+        double* vn = V[(j + 1) & 1];
+        rc = op_apply_device(h, vj, w);  // the whole batch at once: the matrix is block diagonal
+        if (rc != BJ_OK) break;
+        e = launch_kernel(lz_batch_step_kernel, dim3((unsigned)nsys), dim3(kBatchThreads), 0, st, h->pdl, seg, m, j, tol, w,
+                          (const double*)vn, (const double*)vj, j + 1 < m ? vn : (double*)nullptr, alpha, beta, amax, m_eff,
+                          stopped);
+        if (e != cudaSuccess) { set_cuda_error(e, "lz_batch_step_kernel"); rc = BJ_ERR_CUDA; break; }
+        h->launches++;
+    }
+    std::vector<double> ha((size_t)nsys * m), hb((size_t)nsys * m);
+    std::vector<int> hm((size_t)nsys);
+    if (rc == BJ_OK) {
+        e = cudaMemcpyAsync(ha.data(), alpha, ha.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(hb.data(), beta, hb.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(hm.data(), m_eff, hm.size() * sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { set_cuda_error(e, "batch readback"); rc = BJ_ERR_CUDA; }
+    }
+    cleanup();
+    if (rc != BJ_OK) return rc;
+    for (int64_t s = 0; s < nsys; ++s) {
+        const int me = hm[s];
+        if (me < 1) return BJ_ERR_CUDA;
+        lmin_host[s] = tridiag_eig_k(me, ha.data() + s * m, hb.data() + s * m, 0);
+        lmax_host[s] = tridiag_eig_k(me, ha.data() + s * m, hb.data() + s * m, me - 1);
+        if (iters_done_host) iters_done_host[s] = me;
+    }
+    return BJ_OK;
+}

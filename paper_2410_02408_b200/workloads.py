@@ -364,3 +364,33 @@ def block_diagonal_spd(nblocks: int, b: int, seed: int = SEED) -> CSR:
     col = (np.arange(nblocks)[:, None, None] * b + np.arange(b)[None, None, :] + np.zeros((1, b, 1), dtype=np.int64))
     return CSR(n, row_ptr, col.ravel().astype(np.int32), np.ascontiguousarray(blocks.ravel()),
                {"kind": "block_diagonal", "b": b})
+
+
+def batch_poisson(nsys: int, n: int = 32, seed: int = SEED) -> CSR:
+    """the paper's own problem sizes (N = 2^10, 2^12, 2^14) as a BATCH of `nsys`
+    independent systems in one block-diagonal CSR (the paper's "solve each block separately" picture, PAPER.md:76-82,
+    126-130).  System s is config 1's construction on an n x n grid (N = n^2 = 1024 for n = 32) with its own diagonal
+    draw u ~ U[0,1) from Philox(key = seed + 1, counter offset by s): rows s N .. (s+1) N - 1."""
+    a = laplacian((n, n))
+    N = a.n
+    u = _rng(1, seed).random(nsys * N)
+    rp = a.row_ptr.astype(np.int64)
+    rows = np.repeat(np.arange(N), np.diff(rp))
+    diag = a.col_idx == rows
+    nnz = int(rp[-1])
+    val = np.tile(a.val, nsys)
+    dmask = np.tile(diag, nsys)
+    val[dmask] = 4.0 + u
+    col = (np.tile(a.col_idx.astype(np.int64), nsys) + np.repeat(np.arange(nsys, dtype=np.int64) * N, nnz)).astype(np.int32)
+    row_ptr = (np.tile(rp[:-1], nsys) + np.repeat(np.arange(nsys, dtype=np.int64) * nnz, N))
+    row_ptr = np.concatenate([row_ptr, [nsys * nnz]]).astype(np.int32)
+    return CSR(nsys * N, row_ptr, col, val, {"kind": "batch", "nsys": nsys, "seg": N, "name": f"batch{nsys}xpoisson2d_{n}x{n}"})
+
+
+def batch_system(A: CSR, s: int) -> CSR:
+    """System s of a batch built by batch_poisson, as a CSR of its own (for the per-system oracle runs)."""
+    seg = A.meta["seg"]
+    r0, r1 = s * seg, (s + 1) * seg
+    p0, p1 = int(A.row_ptr[r0]), int(A.row_ptr[r1])
+    return CSR(seg, (A.row_ptr[r0:r1 + 1] - p0).astype(np.int32), (A.col_idx[p0:p1] - r0).astype(np.int32),
+               A.val[p0:p1].copy(), {"kind": "batch_member", "s": s})

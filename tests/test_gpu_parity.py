@@ -422,6 +422,55 @@ def test_tridiagonal_compact_factors_small_blocks(B, torch_, rel, monkeypatch):
         check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=KERNELS)
 
 
+def test_batched_small_systems(B, torch_, rel):
+    """a batch of independent N = 1024 systems (the paper's smallest size) in one
+    block-diagonal CSR.  Per system the kappa estimate equals the oracle's Lanczos on that system alone with the same
+    start-vector slice; the operator apply equals the per-system applies."""
+    nsys, m = 12, 30
+    A = W.batch_poisson(nsys, 32)
+    seg = A.meta["seg"]
+    v0 = W.seeded_vector(B.BJ_DEFAULT_SEED, A.n)
+    for b in (0, 1, 4, 16):
+        h, keep = B.setup_from_host(A, b)
+        g = B.bj_cond_estimate_batch(h, nsys, m)
+        x = W.seeded_vector(7, A.n)
+        y = B.bj_op_apply(h, dev(torch_, x)).cpu().numpy()
+        for s in range(nsys):
+            As = W.batch_system(A, s)
+            P = oracle.Precond(As, b)
+            c = P.cond_estimate(m, v0=v0[s * seg:(s + 1) * seg], reorth=False)
+            assert g["iters_done"][s] == c["iters_done"]
+            assert abs(g["kappa"][s] / c["kappa"] - 1) <= TOL_KAPPA, (b, s, g["kappa"][s], c["kappa"])
+            e2, ei = rel(y[s * seg:(s + 1) * seg], P.op_apply(x[s * seg:(s + 1) * seg]))
+            assert e2 <= TOL_APPLY and ei <= TOL_APPLY
+        assert len(set(np.round(g["kappa"], 6))) == nsys          # every system has its own spectrum
+        B.bj_destroy(h)
+    # the solve side: per-system PCG, each system with its own stopping iteration
+    h, keep = B.setup_from_host(A, 4)
+    rhs = W.seeded_vector(17, A.n)
+    rhs[3 * seg:4 * seg] = 0.0                                    # one system has nothing to solve
+    g = B.bj_pcg_solve_batch(h, nsys, dev(torch_, rhs), max_iters=200, rtol=1e-8)
+    xg = g["x"].cpu().numpy()
+    for s in range(nsys):
+        c = oracle.Precond(W.batch_system(A, s), 4).pcg(rhs[s * seg:(s + 1) * seg], 200, 1e-8)
+        assert abs(int(g["iters"][s]) - c["iters"]) <= 1, (s, g["iters"][s], c["iters"])
+        if s == 3:
+            assert g["iters"][s] == 0 and not xg[s * seg:(s + 1) * seg].any()
+            continue
+        e2, ei = rel(xg[s * seg:(s + 1) * seg], c["x"])
+        assert e2 <= 1e-7 and g["relres"][s] <= 1e-8 and g["true_relres"][s] <= 2e-8, (s, e2)
+    assert len(set(g["iters"].tolist())) > 1                      # the systems really stop at different steps
+    B.bj_destroy(h)
+    # a system whose preconditioner is exact breaks down at step 1 while the others go on
+    Ab = W.block_diagonal_spd(64, 8)
+    h, keep = B.setup_from_host(Ab, 8)
+    g = B.bj_cond_estimate_batch(h, 4, 10)
+    assert (g["iters_done"] == 1).all() and np.allclose(g["kappa"], 1.0, atol=1e-12)
+    with pytest.raises(B.BJError):
+        B.bj_cond_estimate_batch(h, 5, 10)       # 512 rows do not split into 5 systems
+    B.bj_destroy(h)
+
+
 def test_block_size_sweep_runs_the_real_path(B, torch_):
     """a11: host-side sweep over b; kappa estimates agree with the oracle at the chosen b; b = N/.. ordering sane."""
     from paper_2410_02408_b200 import sweep
