@@ -157,6 +157,68 @@ def run_reference(args, A, b: int):
     print(json.dumps(line))
 
 
+def run_batch(args):
+    """Second workload (NEXT-4): many small systems per launch.  Metric: systems/s for the per-system kappa estimate
+    (m Lanczos steps each) and for the per-system PCG to the paper's bar 1e-3; plus the CPU oracle on a sample."""
+    import torch
+    from paper_2410_02408_b200 import binding as B
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    nsys, m = args.batch, args.lanczos_iters
+    b = args.block if args.block is not None else 4
+    A = W.batch_poisson(nsys, 32)
+    rp, ci, val = (torch.from_numpy(a).cuda() for a in (A.row_ptr, A.col_idx, A.val))
+    h = B.bj_setup(rp, ci, val, b)
+    x = B.bj_seeded_vector(h, 31)
+    y = torch.empty_like(x)
+    for _ in range(max(args.warmup, 3)):
+        B.bj_op_apply(h, x, y)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        B.bj_op_apply(h, x, y)
+    e1.record()
+    torch.cuda.synchronize()
+    us = 1e3 * e0.elapsed_time(e1) / args.steps
+    B.bj_cond_estimate_batch(h, nsys, m)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    g = B.bj_cond_estimate_batch(h, nsys, m)
+    t_k = time.perf_counter() - t0
+    rhs = B.bj_seeded_vector(h, 17)
+    B.bj_pcg_solve_batch(h, nsys, rhs, max_iters=4, rtol=0.0)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    pr = B.bj_pcg_solve_batch(h, nsys, rhs, max_iters=500, rtol=1e-3)
+    t_p = time.perf_counter() - t0
+    # CPU oracle on a sample of the systems (reported baseline)
+    import oracle
+    v0 = W.seeded_vector(B.BJ_DEFAULT_SEED, A.n)
+    seg, ns = A.meta["seg"], min(nsys, 64)
+    t0 = time.perf_counter()
+    worst = 0.0
+    for s in range(ns):
+        c = oracle.Precond(W.batch_system(A, s), b).cond_estimate(m, v0=v0[s * seg:(s + 1) * seg], reorth=False)
+        worst = max(worst, abs(g["kappa"][s] / c["kappa"] - 1))
+    t_o = time.perf_counter() - t0
+    n, nnz = A.n, A.nnz
+    ab = algorithmic_bytes(n, nnz, b)
+    line = {"metric": "batched_systems_kappa_per_s", "value": nsys / t_k, "unit": "systems/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_k, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": A.meta["name"], "systems": nsys, "system_size": seg, "n": n, "nnz": nnz, "block": b,
+                       "lanczos_iters": m, "paper_size": "N = 2^10 (PAPER.md:365)"},
+            "op_apply": {"us": us, "applies_per_s": 1e6 / us, "alg_bytes": ab["op_apply"], "gbs": ab["op_apply"] / us / 1e3},
+            "kappa": {"seconds": t_k, "min": float(g["kappa"].min()), "median": float(np.median(g["kappa"])),
+                      "max": float(g["kappa"].max()), "max_rel_dev_vs_oracle_sample": worst},
+            "pcg": {"rtol": 1e-3, "seconds": t_p, "systems_per_s": nsys / t_p, "iters_min": int(pr["iters"].min()),
+                    "iters_max": int(pr["iters"].max()), "true_relres_max": float(pr["true_relres"].max())},
+            "cpu_baseline": {"value": ns / t_o, "unit": "systems/s", "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": f"kappa estimate ({m} Lanczos steps) of {ns} of the {nsys} systems"},
+            "gpu_launches": B.bj_get_info(h)["kernel_launches"]}
+    B.bj_destroy(h)
+    print(json.dumps(line))
+
+
 def aggregate_max(ms_local: float, world: int) -> float:
     """max over ranks of the device-timed milliseconds (all_reduce MAX; identity for world == 1)."""
     if world == 1:
@@ -183,6 +245,9 @@ def main():
     ap.add_argument("--spmv-kernel", type=int, default=-1)
     ap.add_argument("--fuse", type=int, default=-1)
     ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e (profiling runs)")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="N > 0: second workload (SURVEY 8(f) NEXT-4): N independent 32x32 Poisson systems (the paper's N = 2^10) "
+                         "in one block-diagonal CSR; prints one JSON line for it and exits")
     ap.add_argument("--band", type=int, default=0,
                     help="1: banded block factors where the diagonal blocks are banded (b > 8; SURVEY 8(f) NEXT-2); "
                          "the byte model of the roofline then counts the band, the dense-packed count is given beside it")
@@ -195,6 +260,9 @@ def main():
 
     if args.impl == "reference" and int(os.environ.get("RANK", "0")) != 0:
         return  # under torchrun only rank 0 runs the CPU reference arm
+    if args.batch > 0 and args.impl != "reference":
+        run_batch(args)
+        return
     A = W.build(args.config, args.scale)
     b = args.block if args.block is not None else W.BLOCK_SIZES[args.config][0]
     if args.impl == "reference":

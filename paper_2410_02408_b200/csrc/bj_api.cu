@@ -137,6 +137,7 @@ static void free_handle(bj_handle_s* h)
     if (!h) return;
     lanczos_free(h);
     pcg_free(h);
+    batch_free(h);
     if (h->slab) {
         if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
         else cudaFree(h->slab);

@@ -99,6 +99,47 @@ lz_batch_step_kernel(int64_t seg, int m, int j, double tol, double* __restrict__
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) vnext[base + i] = brk ? 0.0 : w[base + i] / bn;
 }
 
+// extreme eigenvalues of every system's Lanczos tridiagonal by bisection on the inertia of T - x I (the algorithm of
+// tridiag_eig_k in bj_lanczos.cu), one THREAD per system: thousands of tiny tridiagonals are a device job, not a host loop
+__device__ __forceinline__ int batch_negcount(int m, const double* a, const double* e, double x)
+{
+    int cnt = 0;
+    double piv = a[0] - x;
+    cnt += piv < 0.0;
+    for (int i = 1; i < m; ++i) {
+        if (piv == 0.0) piv = 1e-300;
+        piv = (a[i] - x) - (e[i - 1] * e[i - 1]) / piv;
+        cnt += piv < 0.0;
+    }
+    return cnt;
+}
+__device__ __forceinline__ double batch_eig_k(int m, const double* a, const double* e, int k)
+{
+    double lo = a[0], hi = a[0];
+    for (int i = 0; i < m; ++i) {
+        const double r = (i ? fabs(e[i - 1]) : 0.0) + (i + 1 < m ? fabs(e[i]) : 0.0);
+        lo = fmin(lo, a[i] - r);
+        hi = fmax(hi, a[i] + r);
+    }
+    for (int it = 0; it < 4000; ++it) {
+        const double mid = 0.5 * lo + 0.5 * hi;
+        if (!(mid > lo) || !(mid < hi)) break;
+        if (batch_negcount(m, a, e, mid) >= k + 1) hi = mid; else lo = mid;
+    }
+    return 0.5 * lo + 0.5 * hi;
+}
+__global__ void __launch_bounds__(128)
+batch_extremes_kernel(int64_t nsys, int m, const double* __restrict__ alpha, const double* __restrict__ beta,
+                      const int* __restrict__ m_eff, double* __restrict__ lmin, double* __restrict__ lmax)
+{
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsys) return;
+    const int me = m_eff[s];
+    if (me < 1) { lmin[s] = lmax[s] = 0.0; return; }
+    lmin[s] = batch_eig_k(me, alpha + s * m, beta + s * m, 0);
+    lmax[s] = batch_eig_k(me, alpha + s * m, beta + s * m, me - 1);
+}
+
 // ---- batched PCG: per-system scalars, one CTA per system for the vector parts ------------------------------------
 // r = b, x = 0, bb[s] = ||b_s||^2 (a zero right-hand side stops its system at once)
 __global__ void __launch_bounds__(kBatchThreads)
@@ -197,6 +238,25 @@ pcg_batch_residual_kernel(int64_t seg, const double* __restrict__ q, const doubl
 }  // namespace
 }  // namespace bj
 
+namespace bj {
+void batch_free(bj_handle_s* h)
+{
+    if (h->batch_ws) { cudaFree(h->batch_ws); h->workspace_bytes -= (int64_t)h->batch_ws_bytes; }
+    h->batch_ws = nullptr;
+    h->batch_ws_bytes = 0;
+}
+// one allocation kept by the handle (a cudaMalloc of ~100 MB per call costs up to 0.2 s on a cold heap)
+static void* batch_workspace(bj_handle_s* h, size_t bytes)
+{
+    if (h->batch_ws_bytes >= bytes) return h->batch_ws;
+    batch_free(h);
+    if (cudaMalloc(&h->batch_ws, bytes) != cudaSuccess) { cudaGetLastError(); h->batch_ws = nullptr; return nullptr; }
+    h->batch_ws_bytes = bytes;
+    h->workspace_bytes += (int64_t)bytes;
+    return h->batch_ws;
+}
+}  // namespace bj
+
 using namespace bj;
 
 extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_dev, double* x_dev, int max_iters, double rtol,
@@ -208,17 +268,16 @@ extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_d
     const int64_t seg = n / nsys;
     if (h->b > 0 && seg % h->b) return BJ_ERR_INVALID_ARG;
     cudaStream_t st = h->stream;
-    double* vec = nullptr;   // r, z, p, q
-    double* scal = nullptr;  // rho, bb, relres, true_relres [nsys each]
-    int* ints = nullptr;     // iters, stopped, converged [nsys each], nstopped
-    auto cleanup = [&]() { cudaFree(vec); cudaFree(scal); cudaFree(ints); };
-    if (cudaMalloc((void**)&vec, (size_t)4 * n * sizeof(double)) != cudaSuccess ||
-        cudaMalloc((void**)&scal, (size_t)4 * nsys * sizeof(double)) != cudaSuccess ||
-        cudaMalloc((void**)&ints, ((size_t)3 * nsys + 4) * sizeof(int)) != cudaSuccess) {
-        cudaGetLastError();
-        cleanup();
-        return BJ_ERR_ALLOC;
-    }
+    // workspace: r, z, p, q; rho, bb, relres, true_relres [nsys each]; iters, stopped, converged [nsys each], nstopped
+    const size_t vec_b = (size_t)4 * n * sizeof(double);
+    const size_t scal_b = (size_t)4 * nsys * sizeof(double);
+    const size_t int_b = ((size_t)3 * nsys + 4) * sizeof(int);
+    char* ws = (char*)batch_workspace(h, vec_b + scal_b + int_b);
+    if (!ws) return BJ_ERR_ALLOC;
+    double* vec = (double*)ws;
+    double* scal = (double*)(ws + vec_b);
+    int* ints = (int*)(ws + vec_b + scal_b);
+    auto cleanup = [&]() {};
     double *r = vec, *z = vec + n, *p = vec + 2 * n, *q = vec + 3 * n;
     double *rho = scal, *bb = scal + nsys, *relres = scal + 2 * nsys, *truerel = scal + 3 * nsys;
     int *iters = ints, *stopped = ints + nsys, *converged = ints + 2 * nsys, *nstopped = ints + 3 * nsys;
@@ -286,18 +345,16 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
     cudaStream_t st = h->stream;
     const double tol = BJ_DEFAULT_BREAKDOWN_TOL;
 
-    // workspace: v_prev, v_cur (rotating), w; alpha/beta [nsys][m]; amax, m_eff, stopped [nsys]
-    double* vec = nullptr;
-    double* scal = nullptr;
-    int* ints = nullptr;
-    auto cleanup = [&]() { cudaFree(vec); cudaFree(scal); cudaFree(ints); };
-    if (cudaMalloc((void**)&vec, (size_t)3 * n * sizeof(double)) != cudaSuccess ||
-        cudaMalloc((void**)&scal, ((size_t)2 * nsys * m + nsys) * sizeof(double)) != cudaSuccess ||
-        cudaMalloc((void**)&ints, (size_t)2 * nsys * sizeof(int)) != cudaSuccess) {
-        cudaGetLastError();
-        cleanup();
-        return BJ_ERR_ALLOC;
-    }
+    // workspace: v_prev, v_cur (rotating), w; alpha/beta [nsys][m]; amax, lmin, lmax [nsys]; m_eff, stopped [nsys]
+    const size_t vec_b = (size_t)3 * n * sizeof(double);
+    const size_t scal_b = ((size_t)2 * nsys * m + 3 * nsys) * sizeof(double);
+    const size_t int_b = (size_t)2 * nsys * sizeof(int);
+    char* ws = (char*)batch_workspace(h, vec_b + scal_b + int_b);
+    if (!ws) return BJ_ERR_ALLOC;
+    double* vec = (double*)ws;
+    double* scal = (double*)(ws + vec_b);
+    int* ints = (int*)(ws + vec_b + scal_b);
+    auto cleanup = [&]() {};
     double* V[2] = {vec, vec + n};
     double* w = vec + 2 * n;
     double* alpha = scal;
@@ -306,7 +363,9 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
     int* m_eff = ints;
     int* stopped = ints + nsys;
     int rc = BJ_OK;
-    cudaError_t e = cudaMemsetAsync(scal, 0, ((size_t)2 * nsys * m + nsys) * sizeof(double), st);
+    double* dlmin = amax + nsys;
+    double* dlmax = dlmin + nsys;
+    cudaError_t e = cudaMemsetAsync(scal, 0, ((size_t)2 * nsys * m + 3 * nsys) * sizeof(double), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(ints, 0, (size_t)2 * nsys * sizeof(int), st);
     if (e != cudaSuccess) { set_cuda_error(e, "batch memset"); cleanup(); return BJ_ERR_CUDA; }
 
@@ -326,11 +385,12 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
         if (e != cudaSuccess) { set_cuda_error(e, "lz_batch_step_kernel"); rc = BJ_ERR_CUDA; break; }
         h->launches++;
     }
-    std::vector<double> ha((size_t)nsys * m), hb((size_t)nsys * m);
     std::vector<int> hm((size_t)nsys);
     if (rc == BJ_OK) {
-        e = cudaMemcpyAsync(ha.data(), alpha, ha.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(hb.data(), beta, hb.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
+        batch_extremes_kernel<<<(unsigned)((nsys + 127) / 128), 128, 0, st>>>(nsys, m, alpha, beta, m_eff, dlmin, dlmax);
+        h->launches++;
+        e = cudaMemcpyAsync(lmin_host, dlmin, (size_t)nsys * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(lmax_host, dlmax, (size_t)nsys * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(hm.data(), m_eff, hm.size() * sizeof(int), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { set_cuda_error(e, "batch readback"); rc = BJ_ERR_CUDA; }
@@ -338,11 +398,8 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
     cleanup();
     if (rc != BJ_OK) return rc;
     for (int64_t s = 0; s < nsys; ++s) {
-        const int me = hm[s];
-        if (me < 1) return BJ_ERR_CUDA;
-        lmin_host[s] = tridiag_eig_k(me, ha.data() + s * m, hb.data() + s * m, 0);
-        lmax_host[s] = tridiag_eig_k(me, ha.data() + s * m, hb.data() + s * m, me - 1);
-        if (iters_done_host) iters_done_host[s] = me;
+        if (hm[s] < 1) return BJ_ERR_CUDA;
+        if (iters_done_host) iters_done_host[s] = hm[s];
     }
     return BJ_OK;
 }

@@ -127,6 +127,10 @@ struct bj_handle_s {
     double* pcg_scal = nullptr;
     int pcg_cap_iters = 0;
 
+    // batched-systems workspace (bj_batch.cu): one allocation kept by the handle, grown on demand
+    void* batch_ws = nullptr;
+    size_t batch_ws_bytes = 0;
+
     // e2e staging
     double* stage_in = nullptr;
     double* stage_out = nullptr;
@@ -203,6 +207,7 @@ double tridiag_eig_k(int m, const double* a, const double* e, int k);
 // preconditioned CG (bj_pcg.cu)
 int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* r);
 void pcg_free(bj_handle_s* h);
+void batch_free(bj_handle_s* h);
 
 int env_int(const char* name, int dflt);  // tuning knobs BJ_* (read at setup / launch)
 

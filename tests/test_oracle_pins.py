@@ -462,3 +462,23 @@ def test_pcg_zero_rhs_and_residual_threshold():
     r = P.pcg(rhs, 500, 1e-3)          # the paper's accuracy bar
     assert r["true_relres"] <= 1.05e-3 and r["relres"][-1] <= 1e-3
     assert len(r["relres"]) == r["iters"] and (r["iters"] == 1 or r["relres"][-2] > 1e-3)
+
+
+# ---------------------------------------------------------------- batch workload ----
+def test_batch_generator_is_block_diagonal_and_members_match():
+    """The batch CSR is exactly the direct sum of its members (input generator, no method arithmetic): dense comparison
+    on a tiny batch, and every member is config 1's construction (diagonal 4 + U[0,1), off-diagonals -1)."""
+    A = W.batch_poisson(5, 8)
+    D = A.to_dense()
+    assert np.array_equal(D, D.T)
+    seg = A.meta["seg"]
+    rebuilt = np.zeros_like(D)
+    for s in range(5):
+        M = W.batch_system(A, s).to_dense()
+        rebuilt[s * seg:(s + 1) * seg, s * seg:(s + 1) * seg] = M
+        d = np.diag(M)
+        assert (d >= 4.0).all() and (d < 5.0).all()
+        off = M - np.diag(d)
+        assert set(np.unique(off)) <= {-1.0, 0.0} and (off.sum(axis=1) >= -4).all()
+    assert np.array_equal(rebuilt, D)
+    assert len({tuple(np.diag(W.batch_system(A, s).to_dense())) for s in range(5)}) == 5   # each system has its own draw
