@@ -102,6 +102,10 @@ def main():
     res = sweep(rp, ci, val, tuple(int(b) for b in args.blocks.split(",")), iters=args.iters, long_iters=args.long_iters,
                 pcg_rtol=args.pcg_rtol)
     res["workload"] = A.meta.get("name")
+    from . import predict  # NEXT-3: the structural suggestion beside the measured choice
+    sug = predict.suggest_block(A, tuple(int(b) for b in args.blocks.split(",")))
+    res["suggested_b"] = sug["suggested_b"]
+    res["captured_coupling"] = sug["captured"]
     print(json.dumps(res))
 
 
