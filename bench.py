@@ -251,6 +251,9 @@ def main():
     ap.add_argument("--band", type=int, default=0,
                     help="1: banded block factors where the diagonal blocks are banded (b > 8; SURVEY 8(f) NEXT-2); "
                          "the byte model of the roofline then counts the band, the dense-packed count is given beside it")
+    ap.add_argument("--bsr", type=int, default=0,
+                    help="1: keep a 3x3-blocked (BSR) copy of the matrix when its structure allows (config 5; SURVEY 8(f) NEXT-2); "
+                         "the SpMV byte model then counts 8 nnz + 4 nnz/9, the CSR count is given beside it")
     ap.add_argument("--graph", type=int, default=-1,
                     help="1: also time the operator apply replayed from a CUDA graph (default: only config 1, launch-bound)")
     ap.add_argument("--gather-envelope", type=int, default=-1,
@@ -282,6 +285,8 @@ def main():
     B.lib()  # fail loudly if the CUDA library is missing
     if args.band:
         os.environ["BJ_BAND"] = "1"  # read by bj_setup
+    if args.bsr:
+        os.environ["BJ_BSR"] = "1"   # read by bj_setup
 
     n, nnz = A.n, A.nnz
     rp = torch.from_numpy(A.row_ptr).cuda()
@@ -309,6 +314,9 @@ def main():
     y = torch.empty_like(x)
     ab = algorithmic_bytes(n, nnz, b, info.get("band_width", -1))
     ab_dense = algorithmic_bytes(n, nnz, b)
+    if info["spmv_kernel"] == 2:  # BSR(3) copy: values + one block column per nine entries + block row pointers
+        spmv_bsr = 8 * nnz + 4 * (nnz // 9) + 4 * (n // 3 + 1) + 16 * n
+        ab = dict(ab, spmv=spmv_bsr, spmv_solve_L=spmv_bsr + ab["solve_L"], op_apply=spmv_bsr + 2 * ab["solve_L"])
 
     def barrier():
         torch.cuda.synchronize()
@@ -365,7 +373,7 @@ def main():
             "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
             "op_apply": {"alg_bytes": ab["op_apply"], "gbs": op_gbs, "frac_of_measured": op_gbs / peak,
                          "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
-            "band": {"width": info.get("band_width", -1), "op_apply_bytes_dense_packed": ab_dense["op_apply"],
+            "band": {"width": info.get("band_width", -1), "bsr3": info["spmv_kernel"] == 2, "op_apply_bytes_dense_packed": ab_dense["op_apply"],
                      "gbs_vs_dense_packed_count": ab_dense["op_apply"] / (ms_per_step * 1e-3) / 1e9},
             "kernels": kern, "setup_ms": float(np.median(setup_ms)),
             "factor_bytes": info["factor_bytes"]}

@@ -58,6 +58,12 @@ static int resolve_spans(bj_handle_s* h)
     return BJ_OK;
 }
 
+int launch_spmv(bj_handle_s* h, const double* x, double* y)
+{
+    if (h->spmv_kernel == 2) return launch_spmv_bsr(h, x, y);
+    return h->spmv_kernel == 1 ? launch_spmv_stream(h, x, y, false) : launch_spmv_vector(h, x, y);
+}
+
 // y = L^-1 A L^-T x.  x == y allowed.
 int op_apply_device(bj_handle_s* h, const double* x, double* y)
 {
@@ -67,13 +73,13 @@ int op_apply_device(bj_handle_s* h, const double* x, double* y)
             BJ_CUDA(cudaMemcpyAsync(h->t, x, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
             x = h->t;
         }
-        return h->spmv_kernel == 1 ? launch_spmv_stream(h, x, y, false) : launch_spmv_vector(h, x, y);
+        return launch_spmv(h, x, y);
     }
     rc = launch_solve(h, 1, x, h->t);  // t = L^-T x
     if (rc != BJ_OK) return rc;
     const bool fuse = h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0;
     if (fuse) return launch_spmv_stream(h, h->t, y, true);  // y = L^-1 (A t) in one kernel
-    rc = h->spmv_kernel == 1 ? launch_spmv_stream(h, h->t, h->u, false) : launch_spmv_vector(h, h->t, h->u);
+    rc = launch_spmv(h, h->t, h->u);
     if (rc != BJ_OK) return rc;
     return launch_solve(h, 0, h->u, y);  // y = L^-1 u
 }
@@ -85,7 +91,7 @@ int op_apply_lanczos(bj_handle_s* h, const LzPrologue* pro, const LzEpilogue* ep
     if (rc != BJ_OK) return rc;
     const bool fuse = h->solve_kind == 1 && h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0;
     if (fuse) return launch_spmv_stream(h, h->t, w, true, epi);  // w' and the dot partials in the SpMV's epilogue
-    rc = h->spmv_kernel == 1 ? launch_spmv_stream(h, h->t, h->u, false) : launch_spmv_vector(h, h->t, h->u);
+    rc = launch_spmv(h, h->t, h->u);
     if (rc != BJ_OK) return rc;
     return launch_solve(h, 0, h->u, w, nullptr, epi);
 }
@@ -138,6 +144,7 @@ static void free_handle(bj_handle_s* h)
     lanczos_free(h);
     pcg_free(h);
     batch_free(h);
+    bsr_free(h);
     if (h->slab) {
         if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
         else cudaFree(h->slab);
@@ -152,6 +159,7 @@ static void choose_spmv(bj_handle_s* h)
 {
     int k = 0;
     if (h->stream_ok) k = 1;
+    if (h->bsr_ok) k = 2;  // opt-in (BJ_BSR=1) and the matrix is 3x3-blocked: fewer bytes than either CSR kernel
     if (h->opt_spmv_kernel == 0) k = 0;
     if (h->opt_spmv_kernel == 1 && h->stream_ok) k = 1;
     h->spmv_kernel = k;
@@ -328,6 +336,11 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     if (ce != cudaSuccess) { set_cuda_error(ce, "setup"); return fail(BJ_ERR_CUDA); }
     rc = spmv_stream_finish(h, stt.max_tile_nnz);
     if (rc != BJ_OK) return fail(rc);
+    if (env_int("BJ_BSR", 0) != 0) {  // NEXT-2, opt-in: 3x3-blocked copy of the matrix when its structure allows
+        h->bsr_max_row_nnz = stt.max_row_nnz;
+        rc = bsr_build(h);
+        if (rc != BJ_OK) return fail(rc);
+    }
     choose_spmv(h);
     *out = h;
     if (stt.flags & ST_NOT_SPD) {
@@ -427,7 +440,7 @@ int bj_spmv(bj_handle_t h, const double* x, double* y)
 {
     BJ_CHECK_H(h);
     if (!x || !y || x == y) return BJ_ERR_INVALID_ARG;
-    return h->spmv_kernel == 1 ? launch_spmv_stream(h, x, y, false) : launch_spmv_vector(h, x, y);
+    return launch_spmv(h, x, y);
 }
 
 int bj_op_apply(bj_handle_t h, const double* x, double* y)

@@ -288,7 +288,7 @@ extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_d
     const bool pdl = h->pdl;
     int rc = BJ_OK;
     auto spmv = [&](const double* in, double* out) {
-        return h->spmv_kernel == 1 ? launch_spmv_stream(h, in, out, false) : launch_spmv_vector(h, in, out);
+        return launch_spmv(h, in, out);
     };
 #define BJ_BL(kernel, ...)                                                                                 \
     do {                                                                                                   \

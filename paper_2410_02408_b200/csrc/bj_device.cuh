@@ -21,6 +21,20 @@ __device__ __forceinline__ double ld_const_stream(const double* p)
     asm("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
+// read-once stream with an L2 evict-first policy (createpolicy, see policy_evict_first): small reused arrays (row
+// pointers, the gathered vector) stay L2-resident
+__device__ __forceinline__ double ld_once(const double* p, uint64_t pol)
+{
+    double v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ int ld_once(const int* p, uint64_t pol)
+{
+    int v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
+    return v;
+}
 __device__ __forceinline__ int ld_stream(const int* p)
 {
     int v;

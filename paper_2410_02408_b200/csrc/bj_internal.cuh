@@ -105,7 +105,7 @@ struct bj_handle_s {
     int stream_lanes = 1;     // lanes per row, reduce phase of the tile kernel
     int stream_warps = 8;     // consumer warps of the tile kernel
     double coherence = 1.0;   // fraction of entries with |col(i+1, j) - col(i, j)| <= 16: ~1 banded/stencil, ~0 random
-    int spmv_kernel = 0;      // chosen kernel
+    int spmv_kernel = 0;      // chosen kernel: 0 CSR-vector, 1 TMA tile kernel, 2 BSR(3) copy
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;
     int tile_rows = 0;        // rows per tile of the streamed kernel (multiple of b)
@@ -126,6 +126,14 @@ struct bj_handle_s {
     double* pcg_vec = nullptr;
     double* pcg_scal = nullptr;
     int pcg_cap_iters = 0;
+
+    // BSR(3) copy of the matrix (bj_bsr.cu), opt-in BJ_BSR=1: owned by the handle
+    double* bsr_val = nullptr;
+    int32_t* bsr_col = nullptr;
+    int32_t* bsr_rp = nullptr;
+    bool bsr_ok = false;
+    int64_t bsr_bytes = 0;
+    int bsr_tile_rows = 0, bsr_tile_cap = 0, bsr_max_row_nnz = 0;
 
     // batched-systems workspace (bj_batch.cu): one allocation kept by the handle, grown on demand
     void* batch_ws = nullptr;
@@ -190,6 +198,11 @@ bool lanczos_fusable(const bj_handle_s* h);  // the handle's solve / SpMV kernel
 
 // SpMV (bj_spmv_kernels.cu)
 int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);
+int launch_spmv_bsr(bj_handle_s* h, const double* x, double* y);  // bj_bsr.cu
+int bsr_build(bj_handle_s* h);
+void bsr_free(bj_handle_s* h);
+// plain y = A x with the handle's chosen kernel (0 CSR-vector, 1 TMA tile kernel, 2 BSR(3))
+int launch_spmv(bj_handle_s* h, const double* x, double* y);
 struct LzReduce;
 // epi: fused Lanczos epilogue; dot_with / dot_red: per-CTA partials of dot_with . y finished into *dot_red->out (unfused only)
 int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi = nullptr,

@@ -278,7 +278,7 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
         h->launches++;                                                                          \
     } while (0)
     auto spmv = [&](const double* in, double* out) {
-        return h->spmv_kernel == 1 ? launch_spmv_stream(h, in, out, false) : launch_spmv_vector(h, in, out);
+        return launch_spmv(h, in, out);
     };
 
     BJ_LAUNCH(pcg_init_kernel, n, b, r, x, P0);

@@ -471,6 +471,50 @@ def test_batched_small_systems(B, torch_, rel):
     B.bj_destroy(h)
 
 
+def test_bsr3_matrix_copy(B, torch_, rel, monkeypatch):
+    """SURVEY 8(f) NEXT-2, opt-in (BJ_BSR=1): a 3x3-blocked matrix (config 5: three dofs per node) is also kept as BSR(3)
+    -- 8.44 bytes per entry instead of 12 -- and every product of the path runs from that copy; a matrix without the block
+    structure keeps the CSR kernels."""
+    monkeypatch.setenv("BJ_BSR", "1")
+    A = mat(5, "small")
+    for b in (0, 3, 24, 6):
+        h, keep = B.setup_from_host(A, b)
+        assert B.bj_get_info(h)["spmv_kernel"] == 2
+        P = oracle.Precond(A, b)
+        for seed in (3, 4):
+            x = W.seeded_vector(seed, A.n)
+            xd = dev(torch_, x)
+            for name, got, ref in (("spmv", B.bj_spmv(h, xd), oracle.spmv(A, x)), ("op_apply", B.bj_op_apply(h, xd), P.op_apply(x))):
+                e2, ei = rel(got.cpu().numpy(), ref)
+                assert e2 <= TOL_APPLY and ei <= TOL_APPLY, (b, name, e2, ei)
+        g = B.bj_cond_estimate_ex(h, 20, reorth=True)
+        c = P.cond_estimate(20, reorth=True)
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+        if b:
+            g = B.bj_cond_estimate_ex(h, 20, reorth=False)
+            c = P.cond_estimate(20, reorth=False)
+            assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+        rhs = W.seeded_vector(5, A.n)
+        gp = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=8, rtol=0.0)
+        cp = P.pcg(rhs, 8, 0.0)
+        assert np.allclose(gp["alpha"], cp["alpha"], rtol=1e-9, atol=0)
+        B.bj_set_option(h, B.BJ_OPT_SPMV_KERNEL, 1)            # the CSR kernels stay selectable
+        assert B.bj_get_info(h)["spmv_kernel"] in (0, 1)
+        B.bj_destroy(h)
+    for cfg in (2, 3):                                         # no 3x3 block structure: CSR kernels
+        h, keep = B.setup_from_host(mat(cfg, "small"), 3)
+        assert B.bj_get_info(h)["spmv_kernel"] in (0, 1)
+        B.bj_destroy(h)
+    # a matrix whose size and entry count are multiples of 3 and 9 but whose pattern is not blocked
+    h, keep = B.setup_from_host(W.block_diagonal_spd(27, 9), 3)
+    info = B.bj_get_info(h)
+    B.bj_destroy(h)
+    assert info["spmv_kernel"] == 2                            # 9x9 dense blocks ARE 3x3-blocked
+    h, keep = B.setup_from_host(W.laplacian((9, 9, 9)), 3)
+    assert B.bj_get_info(h)["spmv_kernel"] in (0, 1)
+    B.bj_destroy(h)
+
+
 def test_block_size_sweep_runs_the_real_path(B, torch_):
     """a11: host-side sweep over b; kappa estimates agree with the oracle at the chosen b; b = N/.. ordering sane."""
     from paper_2410_02408_b200 import sweep
