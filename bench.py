@@ -343,6 +343,18 @@ def main():
     value = world * args.steps / (ms * 1e-3)
     ms_per_step = ms / args.steps
 
+    # ---- repeatability: five more timed regions of K/5 steps each (median of >= 5 repeats) ----
+    rep_us = []
+    kr = max(20, args.steps // 5)
+    for _ in range(5):
+        e0.record()
+        for _ in range(kr):
+            B.bj_op_apply(h, x, y)
+        e1.record()
+        torch.cuda.synchronize()
+        rep_us.append(1e3 * e0.elapsed_time(e1) / kr)
+    repeats = {"steps_each": kr, "us_median": float(np.median(rep_us)), "us_min": float(min(rep_us)), "us_max": float(max(rep_us))}
+
     # ---- per-kernel durations (CUDA events around every kernel, on the launching stream) --------------
     B.bj_profile_enable(h, True)
     prof_steps = min(args.steps, 500)
@@ -370,7 +382,7 @@ def main():
                        "parallelism": "replicas" if world > 1 else "single",
                        "spmv_kernel": info["spmv_kernel"], "fused_forward": info["fused_forward"],
                        "spmv_lanes": info["spmv_lanes"]},
-            "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
+            "clocks": clocks, "gpu_launches": launches, "repeats": repeats, "roofline": roofline,
             "op_apply": {"alg_bytes": ab["op_apply"], "gbs": op_gbs, "frac_of_measured": op_gbs / peak,
                          "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
             "band": {"width": info.get("band_width", -1), "bsr3": info["spmv_kernel"] == 2, "op_apply_bytes_dense_packed": ab_dense["op_apply"],
