@@ -48,9 +48,9 @@ def algorithmic_bytes(n: int, nnz: int, b: int, band: int = -1) -> dict:
 
 def ncu_traffic(cfg: int, b: int, kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary
-    (profiles/traffic.json, written by hand from profiles/*.md); None if that kernel was not captured."""
+    (profiles/traffic.txt: JSON text, written by hand from profiles/*.md); None if that kernel was not captured."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+        with open(os.path.join(ROOT, "profiles", "traffic.txt")) as fh:
             return json.load(fh).get(f"cfg{cfg}_b{b}", {}).get(kernel)
     except Exception:
         return None
