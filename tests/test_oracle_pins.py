@@ -482,3 +482,26 @@ def test_batch_generator_is_block_diagonal_and_members_match():
         assert set(np.unique(off)) <= {-1.0, 0.0} and (off.sum(axis=1) >= -4).all()
     assert np.array_equal(rebuilt, D)
     assert len({tuple(np.diag(W.batch_system(A, s).to_dense())) for s in range(5)}) == 5   # each system has its own draw
+
+
+def test_pcg_terminates_in_as_many_steps_as_distinct_eigenvalues():
+    """Textbook property of CG: with k distinct eigenvalues of M^-1 A the residual vanishes after k steps.  A diagonal
+    matrix with the values {1, 2, 5} (b = 0: M = I) needs exactly 3; with b = 1 (M = diag A) the preconditioned operator
+    is the identity and one step is enough.  Pins the recurrence without any library."""
+    import scipy.sparse as sp
+    n = 60
+    d = np.array([1.0, 2.0, 5.0])[np.arange(n) % 3]
+    A = W.from_scipy(sp.diags([d], [0], format="csr"))
+    rhs = W.seeded_vector(9, n)
+    r = oracle.Precond(A, 0).pcg(rhs, 10, 1e-13)
+    assert r["iters"] == 3 and r["relres"][1] > 1e-6 and r["true_relres"] <= 1e-13
+    assert np.allclose(r["x"], rhs / d, rtol=1e-13, atol=0)
+    r1 = oracle.Precond(A, 1).pcg(rhs, 10, 1e-13)
+    assert r1["iters"] == 1 and abs(r1["alpha"][0] - 1.0) <= 1e-15
+    # 1D Dirichlet Laplacian, n = 12: exact termination in at most n steps, and the CG-Lanczos tridiagonal of the FULL run
+    # reproduces the closed-form spectrum mu_k = 2 - 2 cos(k pi / (n + 1))
+    L = W.laplacian((12,))
+    rl = oracle.Precond(L, 0).pcg(W.seeded_vector(4, 12), 12, 0.0)
+    dd, ee = oracle.cg_tridiag(rl["alpha"], rl["beta"][:11])
+    ev = np.linalg.eigvalsh(np.diag(dd) + np.diag(ee, 1) + np.diag(ee, -1))
+    assert np.allclose(ev, mu(12), rtol=1e-8, atol=0)
