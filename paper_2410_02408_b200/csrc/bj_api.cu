@@ -68,6 +68,7 @@ int launch_spmv(bj_handle_s* h, const double* x, double* y)
 int op_apply_device(bj_handle_s* h, const double* x, double* y)
 {
     int rc;
+    if (tiny_op_usable(h)) return launch_tiny_op_apply(h, x, y);  // launch-bound sizes: one kernel
     if (h->solve_kind == 0) {  // identity preconditioner: A^ = A
         if (x == y) {
             BJ_CUDA(cudaMemcpyAsync(h->t, x, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
@@ -219,6 +220,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         t.pdl_early = env_int("BJ_PDL_EARLY", t.pdl_early);
         t.ctas_per_sm = env_int("BJ_CTAS_PER_SM", t.ctas_per_sm);
         t.lanczos_fuse = env_int("BJ_LANCZOS_FUSE", t.lanczos_fuse);
+        t.tiny = env_int("BJ_TINY", t.tiny);
     }
 
     auto fail = [&](int code) { free_handle(h); return code; };

@@ -41,6 +41,8 @@ struct Tuning {
     int pdl_early = 0;      // bit 0: stream solves, bit 1: stream SpMV release their dependents at entry
     int ctas_per_sm = 4;    // wanted CTAs per SM of the SpMV tile kernel
     int lanczos_fuse = 1;   // fast-mode Lanczos rides on the operator's kernels
+    int tiny = 0;           // BJ_TINY=1: launch-bound sizes run the whole operator apply in one single-CTA kernel
+                            // (eager 7.2 -> 5.9 us on config 1, but 5.2 vs 3.9 us when replayed from a CUDA graph: off)
 };
 
 struct ProfSpan {
@@ -194,7 +196,9 @@ int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out, co
 // pro (dir 1 only) / epi (dir 0 only): fused Lanczos hooks of bj_lanczos_fuse.cuh, null for a plain solve
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro = nullptr,
                  const LzEpilogue* epi = nullptr, const PcgHook* pcg = nullptr);  // pcg: dir 2 only (bj_pcg_fuse.cuh)
-bool lanczos_fusable(const bj_handle_s* h);  // the handle's solve / SpMV kernels carry the fused Lanczos hooks
+bool lanczos_fusable(const bj_handle_s* h);
+bool tiny_op_usable(const bj_handle_s* h);                          // n <= 8192, b <= 8: one-kernel operator apply
+int launch_tiny_op_apply(bj_handle_s* h, const double* x, double* y);  // the handle's solve / SpMV kernels carry the fused Lanczos hooks
 
 // SpMV (bj_spmv_kernels.cu)
 int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);

@@ -685,6 +685,141 @@ static bool use_group_kernel(const bj_handle_s* h)
            (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Launch-bound sizes (config 1: N = 1024, 0.15 MB per apply): the WHOLE operator y = L^-1 A L^-T x in ONE kernel of
+// one CTA -- backward block solves into shared memory, barrier, CSR rows out of shared memory, barrier, forward block
+// solves -- instead of two launches.  b <= 8 (thread per block, interleaved factors, same arithmetic and order as
+// solve_small_kernel and the CSR-vector kernel with one lane per row) or b = 0; n <= kTinyMaxN.
+// ------------------------------------------------------------------------------------------------
+constexpr int kTinyMaxN = 8192;
+constexpr int kTinyThreads = 1024;
+
+__global__ void __launch_bounds__(kTinyThreads)
+tiny_op_apply_kernel(int n, int b, int P, int tri, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
+                     const double* __restrict__ val, const double* __restrict__ fac, const double* x, double* y)
+{
+    extern __shared__ double tiny_sm[];
+    double* t = tiny_sm;
+    double* u = tiny_sm + n;
+    pdl_trigger();
+    pdl_wait();
+    const int nblocks = b > 0 ? (n + b - 1) / b : 0;
+    // the thread's first row: bounds and first eight entries, issued now so that their latency hides behind the solves
+    int pre_s = 0, pre_e = 0, pre_c[8];
+    double pre_a[8];
+    if ((int)threadIdx.x < n) {
+        pre_s = rp[threadIdx.x];
+        pre_e = rp[threadIdx.x + 1];
+    }
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const bool live = pre_s + k < pre_e;
+        pre_c[k] = live ? ci[pre_s + k] : 0;
+        pre_a[k] = live ? val[pre_s + k] : 0.0;
+    }
+    // t = L^-T x
+    if (b == 0) {
+        for (int i = threadIdx.x; i < n; i += blockDim.x) t[i] = x[i];
+    }
+    for (int k = threadIdx.x; k < nblocks; k += blockDim.x) {
+        const double* f = fac + (size_t)(k >> 5) * P * kInterleave + (k & 31);
+        const int lo = k * b;
+        double v[kSmallMax];
+#pragma unroll
+        for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < n) ? x[lo + i] : 0.0;
+#pragma unroll
+        for (int i = kSmallMax - 1; i >= 0; --i) {
+            if (i < b) {
+                double s = v[i];
+                if (tri) {
+                    if (i + 1 < b) s -= f[(2 * i + 1) * kInterleave] * v[i + 1];
+                    v[i] = s * f[(2 * i) * kInterleave];
+                } else {
+#pragma unroll
+                    for (int j = i + 1; j < kSmallMax; ++j)
+                        if (j < b) s -= f[(j * (j + 1) / 2 + i) * kInterleave] * v[j];
+                    v[i] = s * f[(i * (i + 1) / 2 + i) * kInterleave];
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < kSmallMax; ++i)
+            if (i < b && lo + i < n) t[lo + i] = v[i];
+    }
+    __syncthreads();
+    // u = A t, left to right within a row (the oracle's order); eight entries per round, their loads in flight together;
+    // the first round of the thread's first row was loaded before the barrier (pre_*): it does not depend on t
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        double acc = 0.0;
+        const bool first_row = i == (int)threadIdx.x;
+        const int s0 = first_row ? pre_s : rp[i];
+        const int e = first_row ? pre_e : rp[i + 1];
+        for (int q = s0; q < e; q += 8) {
+            int c[8];
+            double a[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const bool live = q + k < e;
+                const bool pre = first_row && q == s0;
+                c[k] = pre ? pre_c[k] : (live ? ci[q + k] : 0);
+                a[k] = pre ? pre_a[k] : (live ? val[q + k] : 0.0);
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) acc = fma(a[k], t[c[k]], acc);  // padded entries: a = 0, c = 0
+        }
+        u[i] = acc;
+    }
+    __syncthreads();
+    // y = L^-1 u
+    if (b == 0) {
+        for (int i = threadIdx.x; i < n; i += blockDim.x) y[i] = u[i];
+    }
+    for (int k = threadIdx.x; k < nblocks; k += blockDim.x) {
+        const double* f = fac + (size_t)(k >> 5) * P * kInterleave + (k & 31);
+        const int lo = k * b;
+        double v[kSmallMax];
+#pragma unroll
+        for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < n) ? u[lo + i] : 0.0;
+#pragma unroll
+        for (int i = 0; i < kSmallMax; ++i) {
+            if (i < b) {
+                double s = v[i];
+                if (tri) {
+                    if (i > 0) s -= f[(2 * i - 1) * kInterleave] * v[i - 1];
+                    v[i] = s * f[(2 * i) * kInterleave];
+                } else {
+#pragma unroll
+                    for (int j = 0; j < i; ++j) s -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
+                    v[i] = s * f[(i * (i + 1) / 2 + i) * kInterleave];
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < kSmallMax; ++i)
+            if (i < b && lo + i < n) y[lo + i] = v[i];
+    }
+}
+
+bool tiny_op_usable(const bj_handle_s* h)
+{
+    return h->n <= kTinyMaxN && h->solve_kind <= 1 && h->opt_spmv_kernel < 0 && h->opt_fuse < 0 && h->tune.tiny != 0;
+}
+
+int launch_tiny_op_apply(bj_handle_s* h, const double* x, double* y)
+{
+    KernelScope scope(h, h->solve_kind == 0 ? BJ_K_SPMV : BJ_K_SPMV_SOLVE_L);
+    const size_t smem = (size_t)2 * h->n * sizeof(double);
+    static bool configured[64] = {};
+    if (smem > 48 * 1024) {
+        cudaError_t e = ensure_big_smem(tiny_op_apply_kernel, configured);
+        if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(tiny_op_apply_kernel)"); return BJ_ERR_CUDA; }
+    }
+    cudaError_t e = launch_kernel(tiny_op_apply_kernel, 1, kTinyThreads, smem, h->stream, h->pdl && !h->prof_on, (int)h->n, h->b,
+                                  h->packed, h->tri ? 1 : 0, h->row_ptr, h->col_idx, h->val, (const double*)h->fac_small, x, y);
+    if (e != cudaSuccess) { set_cuda_error(e, "tiny_op_apply_kernel launch"); return BJ_ERR_CUDA; }
+    return BJ_OK;
+}
+
 // kind 1 always carries the hooks; kind 2 only in the group kernel (b = 16, 24, 32); b = 0 has no solve to ride on
 bool lanczos_fusable(const bj_handle_s* h)
 {

@@ -308,6 +308,26 @@ def test_fused_subwarp_forward_solve_path(B, torch_, rel, monkeypatch):
         check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
 
 
+def test_single_kernel_operator_apply_for_tiny_sizes(B, torch_, rel, monkeypatch):
+    """BJ_TINY=1: n <= 8192 and b <= 8 run the whole operator in one single-CTA kernel (off by default: faster eagerly,
+    slower than the two PDL-chained kernels when replayed from a CUDA graph)."""
+    monkeypatch.setenv("BJ_TINY", "1")
+    for cfg, bs in ((1, (0, 1, 4, 7)), (5, (3, 8))):
+        A = mat(cfg, "small")
+        for b in bs:
+            h, keep = B.setup_from_host(A, b)
+            launches0 = B.bj_get_info(h)["kernel_launches"]
+            x = W.seeded_vector(11, A.n)
+            y = B.bj_op_apply(h, dev(torch_, x))
+            assert B.bj_get_info(h)["kernel_launches"] == launches0 + 1      # one kernel, not two or three
+            e2, ei = rel(y.cpu().numpy(), oracle.Precond(A, b).op_apply(x))
+            assert e2 <= TOL_APPLY and ei <= TOL_APPLY, (cfg, b, e2, ei)
+            z = dev(torch_, x).clone()
+            B.bj_op_apply(h, z, z)                                            # in place
+            assert np.array_equal(z.cpu().numpy(), y.cpu().numpy())
+            B.bj_destroy(h)
+
+
 def test_operator_apply_replays_from_a_cuda_graph(B, torch_, rel):
     """The library's launches (PDL-chained) can be captured on a side stream and replayed: bitwise the eager result."""
     for cfg, b in ((1, 4), (4, 16)):
