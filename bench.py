@@ -251,6 +251,8 @@ def main():
     ap.add_argument("--band", type=int, default=0,
                     help="1: banded block factors where the diagonal blocks are banded (b > 8; SURVEY 8(f) NEXT-2); "
                          "the byte model of the roofline then counts the band, the dense-packed count is given beside it")
+    ap.add_argument("--col16", type=int, default=0,
+                    help="1: 16-bit column deltas in the tile SpMV when the bandwidth allows (SURVEY 8(f) NEXT-2): 10 bytes per entry")
     ap.add_argument("--bsr", type=int, default=0,
                     help="1: keep a 3x3-blocked (BSR) copy of the matrix when its structure allows (config 5; SURVEY 8(f) NEXT-2); "
                          "the SpMV byte model then counts 8 nnz + 4 nnz/9, the CSR count is given beside it")
@@ -287,6 +289,8 @@ def main():
         os.environ["BJ_BAND"] = "1"  # read by bj_setup
     if args.bsr:
         os.environ["BJ_BSR"] = "1"   # read by bj_setup
+    if args.col16:
+        os.environ["BJ_COL16"] = "1"
 
     n, nnz = A.n, A.nnz
     rp = torch.from_numpy(A.row_ptr).cuda()
@@ -314,6 +318,9 @@ def main():
     y = torch.empty_like(x)
     ab = algorithmic_bytes(n, nnz, b, info.get("band_width", -1))
     ab_dense = algorithmic_bytes(n, nnz, b)
+    if info.get("col16") and info["spmv_kernel"] == 1:  # 16-bit column deltas: 10 bytes per entry
+        spmv16 = ab["spmv"] - 2 * nnz
+        ab = dict(ab, spmv=spmv16, spmv_solve_L=spmv16 + ab["solve_L"], op_apply=spmv16 + 2 * ab["solve_L"])
     if info["spmv_kernel"] == 2:  # BSR(3) copy: values + one block column per nine entries + block row pointers
         spmv_bsr = 8 * nnz + 4 * (nnz // 9) + 4 * (n // 3 + 1) + 16 * n
         ab = dict(ab, spmv=spmv_bsr, spmv_solve_L=spmv_bsr + ab["solve_L"], op_apply=spmv_bsr + 2 * ab["solve_L"])
@@ -385,7 +392,7 @@ def main():
             "clocks": clocks, "gpu_launches": launches, "repeats": repeats, "roofline": roofline,
             "op_apply": {"alg_bytes": ab["op_apply"], "gbs": op_gbs, "frac_of_measured": op_gbs / peak,
                          "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
-            "band": {"width": info.get("band_width", -1), "bsr3": info["spmv_kernel"] == 2, "op_apply_bytes_dense_packed": ab_dense["op_apply"],
+            "band": {"width": info.get("band_width", -1), "bsr3": info["spmv_kernel"] == 2, "col16": bool(info.get("col16")), "op_apply_bytes_dense_packed": ab_dense["op_apply"],
                      "gbs_vs_dense_packed_count": ab_dense["op_apply"] / (ms_per_step * 1e-3) / 1e9},
             "kernels": kern, "setup_ms": float(np.median(setup_ms)),
             "factor_bytes": info["factor_bytes"]}

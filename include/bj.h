@@ -93,6 +93,7 @@ typedef struct {
     int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
     int32_t band_width;       /* >= 0: banded factors in use (BJ_BAND=1 at setup, solve_kernel 3), the lower
                                  bandwidth of every diagonal block; -1: dense packed factors              */
+    int32_t col16;            /* 1: the tile SpMV streams 16-bit column deltas (BJ_COL16=1 at setup)          */
 } bj_info_t;
 
 typedef struct {

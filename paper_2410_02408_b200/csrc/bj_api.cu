@@ -146,6 +146,7 @@ static void free_handle(bj_handle_s* h)
     pcg_free(h);
     batch_free(h);
     bsr_free(h);
+    col16_free(h);
     if (h->slab) {
         if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
         else cudaFree(h->slab);
@@ -338,6 +339,10 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     if (ce != cudaSuccess) { set_cuda_error(ce, "setup"); return fail(BJ_ERR_CUDA); }
     rc = spmv_stream_finish(h, stt.max_tile_nnz);
     if (rc != BJ_OK) return fail(rc);
+    if (env_int("BJ_COL16", 0) != 0 && h->stream_ok) {  // NEXT-2, opt-in: 16-bit column deltas for the tile kernel
+        rc = col16_build(h);
+        if (rc != BJ_OK) return fail(rc);
+    }
     if (env_int("BJ_BSR", 0) != 0) {  // NEXT-2, opt-in: 3x3-blocked copy of the matrix when its structure allows
         h->bsr_max_row_nnz = stt.max_row_nnz;
         rc = bsr_build(h);
@@ -411,6 +416,7 @@ int bj_get_info(bj_handle_t h, bj_info_t* info)
     info->spmv_lanes = h->spmv_lanes;
     info->solve_kernel = h->solve_kind;
     info->band_width = (h->solve_kind == 3 || h->tri) ? h->band : -1;
+    info->col16 = h->col16 ? 1 : 0;
     info->fused_forward = (h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0 && h->solve_kind != 0) ? 1 : 0;
     return BJ_OK;
 }

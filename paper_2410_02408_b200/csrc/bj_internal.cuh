@@ -129,6 +129,8 @@ struct bj_handle_s {
     double* pcg_scal = nullptr;
     int pcg_cap_iters = 0;
 
+    int16_t* col16 = nullptr;  // opt-in BJ_COL16=1: column stream as 16-bit deltas col - row (owned by the handle)
+
     // BSR(3) copy of the matrix (bj_bsr.cu), opt-in BJ_BSR=1: owned by the handle
     double* bsr_val = nullptr;
     int32_t* bsr_col = nullptr;
@@ -181,6 +183,8 @@ struct KernelScope {
 int launch_validate(bj_handle_s* h);
 int launch_extract_factor(bj_handle_s* h);
 int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nnz
+int col16_build(bj_handle_s* h);       // 16-bit column deltas when every |col - row| < 32768
+void col16_free(bj_handle_s* h);
 
 struct LzPrologue;
 struct LzEpilogue;

@@ -402,6 +402,64 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
         if (i <= r) out1[k * P + r * (r + 1) / 2 + i] = (i == r) ? inv : D[r * LD + i] * inv;
 }
 
+// ------------------------------------------------------------------------------------------------
+// 16-bit column deltas (opt-in BJ_COL16=1): col - row fits int16 for stencil matrices whose bandwidth
+// is below 32768 (configs 2 and 4); the handle then owns a 2-byte-per-entry copy of the column stream.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+col16_check_kernel(int64_t n, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci, int* __restrict__ flag)
+{
+    const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 3;  // eight lanes per row
+    const int sub = threadIdx.x & 7;
+    bool bad = false;
+    if (row < n) {
+        const int e = rp[row + 1];
+        for (int p = rp[row] + sub; p < e; p += 8) {
+            const int64_t d = (int64_t)ci[p] - row;
+            if (d < -32768 || d > 32767) bad = true;
+        }
+    }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1);
+}
+
+__global__ void __launch_bounds__(256)
+col16_build_kernel(int64_t n, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci, int16_t* __restrict__ out)
+{
+    const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 3;
+    const int sub = threadIdx.x & 7;
+    if (row >= n) return;
+    const int e = rp[row + 1];
+    for (int p = rp[row] + sub; p < e; p += 8) out[p] = (int16_t)((int64_t)ci[p] - row);
+}
+
+void col16_free(bj_handle_s* h)
+{
+    if (h->col16) h->workspace_bytes -= (int64_t)h->nnz * 2;
+    cudaFree(h->col16);
+    h->col16 = nullptr;
+}
+
+// checks the bandwidth, builds the copy; leaves col16 null (no error) when a delta does not fit.  Synchronises once.
+int col16_build(bj_handle_s* h)
+{
+    if (h->nnz == 0) return BJ_OK;
+    int* flag = &h->status->pad;
+    BJ_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), h->stream));
+    const unsigned grid = (unsigned)((h->n * 8 + 255) / 256);
+    col16_check_kernel<<<grid, 256, 0, h->stream>>>(h->n, h->row_ptr, h->col_idx, flag);
+    h->launches++;
+    int bad = 1;
+    BJ_CUDA(cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    if (bad) return BJ_OK;
+    if (cudaMalloc((void**)&h->col16, (size_t)h->nnz * 2 + 16) != cudaSuccess) { cudaGetLastError(); h->col16 = nullptr; return BJ_ERR_ALLOC; }
+    h->workspace_bytes += (int64_t)h->nnz * 2;
+    col16_build_kernel<<<grid, 256, 0, h->stream>>>(h->n, h->row_ptr, h->col_idx, h->col16);
+    h->launches++;
+    BJ_CUDA(cudaGetLastError());
+    return BJ_OK;
+}
+
 int launch_extract_factor(bj_handle_s* h)
 {
     const int b = h->b;

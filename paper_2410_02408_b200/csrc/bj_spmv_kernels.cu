@@ -100,6 +100,7 @@ struct StreamParams {
     int64_t n, nnz;
     const int32_t* rp;
     const int32_t* ci;
+    const int16_t* ci16;  // LZ == 3: 16-bit column deltas col - row (handle-owned copy)
     const double* val;
     const double* x;
     double* y;
@@ -130,7 +131,8 @@ __device__ __forceinline__ void consumer_bar_sync(int nthreads)
 //           (W == 1 with FUSE 1: the blocks are tridiagonal and the factors compact, element (i, j) at slot i + j)
 //       3 = + forward solve, group of lanes per block (bj_device.cuh), W = the compile-time block size (16, 24, 32):
 //           the solving warps rotate from tile to tile and the other warps go on to the next tile meanwhile
-// LZ (compile time, so that the plain operator kernel carries none of it): 0 plain, 1 fused Lanczos epilogue, 2 dot hook
+// LZ (compile time, so that the plain operator kernel carries none of it): 0 plain, 1 fused Lanczos epilogue, 2 dot hook,
+// 3 plain with 16-bit column deltas (BJ_COL16=1: the column stream is col - row in int16, 10 bytes per entry instead of 12)
 template <int LPR, int BATCH, int FUSE, int W, int LZ>
 __global__ void __launch_bounds__(kMaxStreamThreads)
 spmv_stream_kernel(const StreamParams p)
@@ -148,8 +150,12 @@ spmv_stream_kernel(const StreamParams p)
     // per stage: val[cap] | fac[fac_bytes] | col[cap] | rp[rp_ints]
     auto s_val = [&](int s) { return reinterpret_cast<double*>(stage0 + (size_t)s * p.stage_bytes); };
     auto s_fac = [&](int s) { return reinterpret_cast<double*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 8); };
+    constexpr bool C16 = LZ == 3;
+    constexpr int Q = C16 ? 8 : 4;            // ranges are widened to whole groups of Q entries (16-byte bulk copies)
+    constexpr int kColBytes = C16 ? 2 : 4;
     auto s_col = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 8 + p.fac_bytes); };
-    auto s_rp = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 12 + p.fac_bytes); };
+    auto s_col16 = [&](int s) { return reinterpret_cast<int16_t*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * 8 + p.fac_bytes); };
+    auto s_rp = [&](int s) { return reinterpret_cast<int*>(stage0 + (size_t)s * p.stage_bytes + (size_t)p.cap * (8 + kColBytes) + p.fac_bytes); };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (p.early_trigger) pdl_trigger();
@@ -172,7 +178,7 @@ spmv_stream_kernel(const StreamParams p)
     if (warp == 0) {
         // ------------------------------ producer ------------------------------------------------
         const uint64_t pol = policy_evict_first();
-        const int nnz4 = (int)(p.nnz & ~3ll);
+        const int nnz4 = (int)(p.nnz & ~(long long)(Q - 1));
         int pb0 = 0, pb1 = 0;
         int it = 0;
         for (int64_t tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
@@ -194,16 +200,17 @@ spmv_stream_kernel(const StreamParams p)
                 const int64_t r0 = tile * R;
                 const int rows = (int)(r0 + R <= p.n ? R : p.n - r0);
                 // nnz range widened to multiples of 4, clamped to the last whole quad of the arrays
-                const int a0 = p0 & ~3;
-                int a1 = (p1 + 3) & ~3;
+                const int a0 = p0 & ~(Q - 1);
+                int a1 = (p1 + Q - 1) & ~(Q - 1);
                 if (a1 > nnz4) a1 = nnz4;
                 if (a1 < a0) a1 = a0;
                 double* dv = s_val(s);
                 int* dc = s_col(s);
+                int16_t* dc16 = s_col16(s);
                 int* dr = s_rp(s);
-                for (int q = (a1 > p0 ? a1 : p0); q < p1; ++q) {  // tail past the last whole quad
+                for (int q = (a1 > p0 ? a1 : p0); q < p1; ++q) {  // tail past the last whole group of the arrays
                     dv[q - a0] = p.val[q];
-                    dc[q - a0] = p.ci[q];
+                    if (C16) dc16[q - a0] = p.ci16[q]; else dc[q - a0] = p.ci[q];
                 }
                 // row pointers r0 .. r0+rows (rows+1 ints), whole quads by bulk copy, rest by hand
                 const int64_t np1 = p.n + 1;
@@ -211,7 +218,7 @@ spmv_stream_kernel(const StreamParams p)
                 int rq = (want + 3) & ~3;
                 if (r0 + rq > np1) rq = (int)((np1 - r0) & ~3ll);
                 for (int q = rq; q < want; ++q) dr[q] = p.rp[r0 + q];
-                uint32_t bytes = (uint32_t)(a1 - a0) * 12u + (uint32_t)rq * 4u;
+                uint32_t bytes = (uint32_t)(a1 - a0) * (uint32_t)(8 + kColBytes) + (uint32_t)rq * 4u;
                 uint32_t fbytes = 0;
                 const double* fsrc = nullptr;
                 if (FUSE == 1) {
@@ -235,7 +242,8 @@ spmv_stream_kernel(const StreamParams p)
                 mbar_expect_tx(&full[s], bytes);
                 if (a1 > a0) {
                     bulk_g2s(dv, p.val + a0, (uint32_t)(a1 - a0) * 8u, &full[s], pol);
-                    bulk_g2s(dc, p.ci + a0, (uint32_t)(a1 - a0) * 4u, &full[s], pol);
+                    if (C16) bulk_g2s(dc16, p.ci16 + a0, (uint32_t)(a1 - a0) * 2u, &full[s], pol);
+                    else bulk_g2s(dc, p.ci + a0, (uint32_t)(a1 - a0) * 4u, &full[s], pol);
                 }
                 if (rq > 0) bulk_g2s(dr, p.rp + r0, (uint32_t)rq * 4u, &full[s], pol);
                 if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], pol);
@@ -262,8 +270,9 @@ spmv_stream_kernel(const StreamParams p)
             mbar_wait(&full[s], ph);
             const double* sv = s_val(s);
             const int* sc = s_col(s);
+            const int16_t* sc16 = s_col16(s);
             const int* sr = s_rp(s);
-            const int a0 = sr[0] & ~3;
+            const int a0 = sr[0] & ~(Q - 1);
             // (A) rows out of shared memory
             for (int base = 0; base < rows; base += kRowsPerPass) {
                 const int i = base + ctid / LPR;
@@ -278,7 +287,7 @@ spmv_stream_kernel(const StreamParams p)
 #pragma unroll
                         for (int k = 0; k < BATCH; ++k) {
                             const int qq = q + k * LPR;
-                            c[k] = sc[qq < e ? qq : q];
+                            c[k] = C16 ? (int)(r0 + i) + (int)sc16[qq < e ? qq : q] : sc[qq < e ? qq : q];
                         }
 #pragma unroll
                         for (int k = 0; k < BATCH; ++k)  // predicated: a masked lane costs no L1 wavefront
@@ -451,7 +460,7 @@ int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int want_per_sm, int
 
 namespace {
 // shared-memory layout of one launch; the single source of truth for configure and launch
-void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem)
+void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem, bool c16 = false)
 {
     sp.b = h->b > 0 ? h->b : 1;
     sp.P = h->packed;
@@ -475,7 +484,7 @@ void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem
         sp.fac_bytes = fuse ? (((sp.R / sp.b) * sp.P * 8 + 15) & ~15) : 0;
         sp.su_doubles = !fuse ? 0 : (h->solve_kind == 1 ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : ((sp.R + 1) & ~1));
     }
-    sp.stage_bytes = (sp.cap * 12 + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
+    sp.stage_bytes = (sp.cap * (c16 ? 10 : 12) + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
     sp.b_magic = (unsigned)(((1ull << 32) + sp.b - 1) / sp.b);
     smem = 128 + (size_t)sp.su_bufs * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
 }
@@ -554,7 +563,7 @@ int spmv_stream_finish(bj_handle_s* h, int max_tile)
 {
     if (h->ntiles <= 0) return BJ_OK;
     const bool fuse = h->fuse_ok;
-    h->tile_cap = ((max_tile + 8) + 3) & ~3;
+    h->tile_cap = ((max_tile + 16) + 7) & ~7;  // ranges are widened to groups of up to 8 entries on both sides
     int stages = env_int("BJ_STAGES", 2);
     StreamParams sp;
     size_t smem = 0;
@@ -581,8 +590,11 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     if (fuse_forward && !fuse) return BJ_ERR_INVALID_ARG;
     StreamParams sp;
     size_t smem = 0;
-    fill_layout(h, fuse, sp, smem);
+    // 16-bit column deltas: plain operator kernels only (no hooks), thread-per-block fusion or none
+    const bool c16 = h->col16 != nullptr && !epi && !dot_with && (!fuse || h->solve_kind == 1);
+    fill_layout(h, fuse, sp, smem, c16);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
+    sp.ci16 = h->col16;
     sp.x = x; sp.y = y;
     sp.early_trigger = (h->tune.pdl_early >> 1) & 1;
     sp.lz = epi ? 1 : (dot_with && dot_red) ? 2 : 0;
@@ -603,10 +615,13 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     case L:                                                                                      \
         rc = mode == 0   ? (sp.lz == 1   ? launch_stream_t<L, 8, 0, 32, 1>(h, sp, grid, threads, smem)  \
                             : sp.lz == 2 ? launch_stream_t<L, 8, 0, 32, 2>(h, sp, grid, threads, smem)  \
+                            : c16        ? launch_stream_t<L, 8, 0, 32, 3>(h, sp, grid, threads, smem)  \
                                          : launch_stream_t<L, 8, 0, 32, 0>(h, sp, grid, threads, smem)) \
              : mode == 1 ? (h->tri ? (sp.lz == 1 ? launch_stream_t<L, 8, 1, 1, 1>(h, sp, grid, threads, smem)    \
+                                      : c16      ? launch_stream_t<L, 8, 1, 1, 3>(h, sp, grid, threads, smem)    \
                                                  : launch_stream_t<L, 8, 1, 1, 0>(h, sp, grid, threads, smem))   \
                                    : (sp.lz == 1 ? launch_stream_t<L, 8, 1, 32, 1>(h, sp, grid, threads, smem)   \
+                                      : c16      ? launch_stream_t<L, 8, 1, 32, 3>(h, sp, grid, threads, smem)   \
                                                  : launch_stream_t<L, 8, 1, 32, 0>(h, sp, grid, threads, smem))) \
              : mode == 2 ? launch_stream_t<L, 8, 2, 16>(h, sp, grid, threads, smem)               \
                          : launch_stream_t<L, 8, 2, 32>(h, sp, grid, threads, smem);              \

@@ -491,6 +491,35 @@ def test_batched_small_systems(B, torch_, rel):
     B.bj_destroy(h)
 
 
+def test_16_bit_column_deltas(B, torch_, rel, monkeypatch):
+    """SURVEY 8(f) NEXT-2, opt-in (BJ_COL16=1): when every |col - row| < 32768 the tile kernel streams the columns as
+    int16 deltas (10 bytes per entry instead of 12); bit-identical products (same values, same order)."""
+    for cfg, b in ((2, 8), (4, 8), (1, 4), (3, 4), (4, 16), (5, 3)):
+        A = mat(cfg, "small")
+        x = dev(torch_, W.seeded_vector(6, A.n))
+        monkeypatch.delenv("BJ_COL16", raising=False)
+        h, keep = B.setup_from_host(A, b)
+        ref_spmv, ref_op = B.bj_spmv(h, x).clone(), B.bj_op_apply(h, x).clone()
+        B.bj_destroy(h)
+        monkeypatch.setenv("BJ_COL16", "1")
+        h, keep = B.setup_from_host(A, b)
+        assert B.bj_get_info(h)["col16"] == 1
+        assert np.array_equal(B.bj_spmv(h, x).cpu().numpy(), ref_spmv.cpu().numpy())
+        assert np.array_equal(B.bj_op_apply(h, x).cpu().numpy(), ref_op.cpu().numpy())
+        P = oracle.Precond(A, b)
+        g = B.bj_cond_estimate_ex(h, 15, reorth=False)       # the hooked kernels keep the 32-bit columns
+        assert abs(g["kappa"] / P.cond_estimate(15, reorth=False)["kappa"] - 1) <= TOL_KAPPA
+        B.bj_destroy(h)
+    # a matrix with a far off-diagonal keeps the 32-bit stream
+    import scipy.sparse as sp
+    n = 70000
+    far = sp.diags([np.full(n, 4.0), np.full(n - 40000, -1.0), np.full(n - 40000, -1.0)], [0, 40000, -40000], format="csr")
+    h, keep = B.setup_from_host(W.from_scipy(far), 4)
+    assert B.bj_get_info(h)["col16"] == 0
+    B.bj_destroy(h)
+    check_all_ops(B, torch_, mat(2, "small"), 8, rel, seeds=(3,), kernels=KERNELS)
+
+
 def test_bsr3_matrix_copy(B, torch_, rel, monkeypatch):
     """SURVEY 8(f) NEXT-2, opt-in (BJ_BSR=1): a 3x3-blocked matrix (config 5: three dofs per node) is also kept as BSR(3)
     -- 8.44 bytes per entry instead of 12 -- and every product of the path runs from that copy; a matrix without the block
