@@ -30,6 +30,15 @@
  *   - All functions return BJ_OK (0) or a negative bj_status code; bj_strerror gives text.  A
  *     CUDA runtime failure returns BJ_ERR_CUDA and leaves the CUDA error string in bj_strerror.
  *   - No CPU fallback exists: without a CUDA device every compute entry point fails with BJ_ERR_CUDA.
+ *   - A handle is not thread-safe; different handles may be used concurrently on different streams.
+ *
+ * Opt-in storage variants, selected by environment variables that bj_setup reads ONCE (each moves fewer bytes than
+ * the CSR / dense-block counts of SURVEY.md 8(d) and has its own byte accounting; each falls back
+ * silently to the default layout when the matrix does not have the structure; results stay within the same tolerances):
+ *     BJ_BAND=1   banded diagonal blocks (lower bandwidth <= 2; b <= 8: tridiagonal) keep banded Cholesky factors;
+ *     BJ_COL16=1  the column stream of the tile SpMV as 16-bit deltas col - row when every |col - row| < 32768;
+ *     BJ_BSR=1    a handle-owned BSR(3) copy of a 3x3-blocked matrix (three unknowns per node).
+ * bj_get_info reports which are in use (band_width, col16, spmv_kernel == 2).  Launch-shape knobs: DESIGN.md section 5.
  */
 #ifndef BJ_H_
 #define BJ_H_
@@ -87,7 +96,8 @@ typedef struct {
     int64_t factor_bytes;     /* device bytes held for the factors                                   */
     int64_t workspace_bytes;  /* device bytes held for temporaries and Lanczos workspace             */
     int64_t kernel_launches;  /* number of kernels this handle has launched so far                   */
-    int32_t spmv_kernel;      /* 0: row-per-subwarp CSR-vector kernel, 1: TMA-streamed tile kernel    */
+    int32_t spmv_kernel;      /* 0: row-per-subwarp CSR-vector kernel, 1: TMA-streamed tile kernel,
+                                 2: TMA-streamed BSR(3) kernel (BJ_BSR=1)                              */
     int32_t spmv_lanes;       /* lanes per row chosen at setup                                       */
     int32_t solve_kernel;     /* 0: none (b=0), 1: thread-per-block (b<=8), 2: group/subwarp-per-block, 3: banded */
     int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
