@@ -232,6 +232,38 @@ __device__ __forceinline__ void group_backward(const double* f, int l, double (&
     }
 }
 
+// backward substitution on the FORWARD copy (column-major packed lower, rows scaled: f_ji = l_ji / l_jj, diagonal slot
+// 1 / l_jj): with x~_j = l_jj x_j the recurrence is  x~_i = y_i - sum_{j > i} f_ji x~_j,  x_i = x~_i / l_ii.  bj_apply can
+// therefore run both substitutions from ONE staged copy: its factor traffic is the algorithmic 4 N (b+1) bytes, not twice
+// that.  Lane (row i) walks down its own column: element (j, i) at colbase_i + j.
+template <int B, int LPB>
+__device__ __forceinline__ void group_backward_fwdcopy(const double* f, int l, double (&r)[B / LPB])
+{
+    constexpr int RPL = B / LPB;
+    int colbase[RPL];  // i B - i (i - 1) / 2 - i: start of column i minus i
+#pragma unroll
+    for (int k = 0; k < RPL; ++k) {
+        const int i = k * LPB + l;
+        colbase[k] = i * B - i * (i - 1) / 2 - i;
+    }
+#pragma unroll
+    for (int j = B - 1; j >= 1; --j) {
+        const int kj = j / LPB, lj = j % LPB;
+        const double vj = __shfl_sync(0xffffffffu, r[kj], lj, LPB);
+#pragma unroll
+        for (int k = 0; k <= kj; ++k) {
+            if (k == kj && lj == 0) continue;
+            const double fji = (k < kj || l < lj) ? f[colbase[k] + j] : 0.0;
+            r[k] = fma(-fji, vj, r[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < RPL; ++k) {
+        const int i = k * LPB + l;
+        r[k] *= f[colbase[k] + i];  // the diagonal slot holds 1 / l_ii
+    }
+}
+
 // Programmatic dependent launch.  Every kernel of the library calls pdl_trigger() first (lets the
 // next kernel in the stream start its independent prologue while this grid drains) and pdl_wait()
 // before its first access to memory that an earlier kernel in the stream may have written, and

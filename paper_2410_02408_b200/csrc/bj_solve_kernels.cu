@@ -356,7 +356,7 @@ solve_group_kernel(const GroupParams p)
     using Geo = GroupGeom<B, LPB>;
     constexpr int RPL = Geo::RPL;
     constexpr int NBW = Geo::NBW;
-    constexpr int kCopies = DIR == 2 ? 2 : 1;
+    constexpr int kCopies = 1;  // bj_apply (DIR 2) runs both substitutions from the forward copy
     constexpr int kStageDoubles = kCopies * NBW * Geo::STRIDE;
     constexpr uint32_t kBlockBytes = Geo::P * 8;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -387,7 +387,6 @@ solve_group_kernel(const GroupParams p)
         mbar_expect_tx(&full[s], (uint32_t)nb * kBlockBytes * kCopies);
         for (int q = 0; q < nb; ++q) {
             bulk_g2s(dst + q * Geo::STRIDE, p.fac0 + (k0 + q) * Geo::P, kBlockBytes, &full[s], pol);
-            if (DIR == 2) bulk_g2s(dst + (NBW + q) * Geo::STRIDE, p.fac1 + (k0 + q) * Geo::P, kBlockBytes, &full[s], pol);
         }
     };
     if (lane == 0)
@@ -477,7 +476,7 @@ solve_group_kernel(const GroupParams p)
         const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
         if (DIR == 0 || DIR == 2) group_forward<B, LPB>(f, l, r);
         if (DIR == 1) group_backward<B, LPB>(f, l, r);
-        if (DIR == 2) group_backward<B, LPB>(f + NBW * Geo::STRIDE, l, r);
+        if (DIR == 2) group_backward_fwdcopy<B, LPB>(f, l, r);
         __syncwarp();
 #pragma unroll
         for (int k = 0; k < RPL; ++k) xchg[g * XB + k * LPB + l] = r[k];
@@ -624,7 +623,7 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
 {
     using Geo = GroupGeom<B, LPB>;
     constexpr int kGroupBlocksPerWarp = Geo::NBW;
-    constexpr int kCopies = DIR == 2 ? 2 : 1;
+    constexpr int kCopies = 1;  // DIR 2 uses the forward copy for both substitutions
     const size_t stage_bytes = (size_t)kCopies * kGroupBlocksPerWarp * Geo::STRIDE * 8;
     const int stages = std::max(2, std::min(8, h->tune.group_stages));
     // as many warps as fit one SM's shared memory (one CTA per SM), at most 12: the bytes in flight per SM are
