@@ -238,6 +238,10 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         h->solve_kind = 2;
         h->lanes = b <= 16 ? 16 : 32;
         fac_a = fac_b = (size_t)h->nblocks * h->packed * sizeof(double) + 16;  // 16 B slack: bulk copies round up
+        // the group kernel (b = 16, 24, 32) runs the backward substitution from the forward copy too: one copy is kept
+        h->single_copy = (b == 16 || b == 24 || b == 32) && h->tune.solve_group != 0 && env_int("BJ_SINGLE_COPY", 1) != 0 &&
+                         env_int("BJ_SETUP_WARP", 0) == 0;
+        if (h->single_copy) fac_b = 0;
     }
     const size_t total = 2 * vb + 256 + up256(fac_a) + up256(fac_b);
     h->slab = slab_alloc(total, dev, h->stream, &h->slab_pooled);
@@ -249,7 +253,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         h->status = (Status*)(base + 2 * vb);
         char* f = base + 2 * vb + 256;
         if (h->solve_kind == 1) h->fac_small = (double*)f;
-        if (h->solve_kind == 2) { h->fac_fwd = (double*)f; h->fac_bwd = (double*)(f + up256(fac_a)); }
+        if (h->solve_kind == 2) { h->fac_fwd = (double*)f; h->fac_bwd = h->single_copy ? nullptr : (double*)(f + up256(fac_a)); }
         h->workspace_bytes = (int64_t)(2 * vb + 256);
         h->factor_bytes = (int64_t)(fac_a + fac_b);
     }
@@ -322,7 +326,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
             ce = cudaMemsetAsync((char*)h->fac_band + (size_t)(h->nblocks / kInterleave) * group_bytes, 0, group_bytes, h->stream);
     } else if (h->solve_kind == 2) {
         ce = cudaMemsetAsync((char*)h->fac_fwd + fac_a - 16, 0, 16, h->stream);
-        if (ce == cudaSuccess) ce = cudaMemsetAsync((char*)h->fac_bwd + fac_b - 16, 0, 16, h->stream);
+        if (ce == cudaSuccess && h->fac_bwd) ce = cudaMemsetAsync((char*)h->fac_bwd + fac_b - 16, 0, 16, h->stream);
     }
     if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
     if (b > 0) {

@@ -91,7 +91,8 @@ struct bj_handle_s {
     int packed = 0;      // b(b+1)/2
     double* fac_small = nullptr;
     double* fac_fwd = nullptr;
-    double* fac_bwd = nullptr;
+    double* fac_bwd = nullptr;   // null when single_copy
+    bool single_copy = false;    // b = 16, 24, 32 with the group kernel: both substitutions run from the forward copy
     int64_t factor_bytes = 0;
 
     // temporaries

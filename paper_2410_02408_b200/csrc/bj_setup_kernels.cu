@@ -397,9 +397,10 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
     // forward copy: column-major packed, row i scaled by 1/l_ii
     for (int j = 0; j < b; ++j)
         if (i >= j && i < b) out0[k * P + (j * b - j * (j - 1) / 2) + (i - j)] = (i == j) ? inv : D[i * LD + j] * inv;
-    // backward copy: row-major packed, column i scaled by 1/l_ii
-    for (int r = 0; r < b; ++r)
-        if (i <= r) out1[k * P + r * (r + 1) / 2 + i] = (i == r) ? inv : D[r * LD + i] * inv;
+    // backward copy: row-major packed, column i scaled by 1/l_ii (not kept when the solves use the forward copy for both)
+    if (out1)
+        for (int r = 0; r < b; ++r)
+            if (i <= r) out1[k * P + r * (r + 1) / 2 + i] = (i == r) ? inv : D[r * LD + i] * inv;
 }
 
 // ------------------------------------------------------------------------------------------------

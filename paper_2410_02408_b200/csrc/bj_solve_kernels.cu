@@ -337,6 +337,7 @@ struct GroupParams {
     double* out;
     int stages;
     int lz;              // 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0), 3 PCG update + apply (DIR 2)
+    int bwd_from_fwd;    // DIR 1: run the backward substitution from the forward copy (fac0 = forward copy)
     LzPrologue pro;
     LzEpilogue epi;
     PcgHook pcg;
@@ -475,7 +476,9 @@ solve_group_kernel(const GroupParams p)
         mbar_wait(&full[s], ph);
         const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
         if (DIR == 0 || DIR == 2) group_forward<B, LPB>(f, l, r);
-        if (DIR == 1) group_backward<B, LPB>(f, l, r);
+        if (DIR == 1) {
+            if (p.bwd_from_fwd) group_backward_fwdcopy<B, LPB>(f, l, r); else group_backward<B, LPB>(f, l, r);
+        }
         if (DIR == 2) group_backward_fwdcopy<B, LPB>(f, l, r);
         __syncwarp();
 #pragma unroll
@@ -643,7 +646,8 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     GroupParams gp;
     gp.n = h->n; gp.nblocks = h->nblocks;
     gp.ntiles = (h->nblocks + kGroupBlocksPerWarp - 1) / kGroupBlocksPerWarp;
-    gp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
+    gp.bwd_from_fwd = h->single_copy ? 1 : 0;
+    gp.fac0 = (DIR == 1 && !gp.bwd_from_fwd) ? h->fac_bwd : h->fac_fwd;
     gp.fac1 = h->fac_bwd;
     gp.in = in; gp.out = out; gp.stages = stages;
     gp.lz = (DIR == 1 && pro) ? 1 : (DIR == 0 && epi) ? 2 : (DIR == 2 && pcg) ? 3 : 0;
@@ -681,7 +685,7 @@ static int launch_group(bj_handle_s* h, const double* in, double* out, const LzP
 static bool use_group_kernel(const bj_handle_s* h)
 {
     return (h->b == 16 || h->b == 24 || h->b == 32) && h->tune.solve_group != 0 &&
-           (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0;
+           (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0 && (h->single_copy || h->fac_bwd != nullptr);
 }
 
 // ------------------------------------------------------------------------------------------------
