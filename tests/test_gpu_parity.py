@@ -706,3 +706,28 @@ def test_pcg_full_size(B, torch_, rel, cfg):
     del h, keep
     _MATS.pop((cfg, "full"), None)
     torch_.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("cfg,b,env", [(2, 8, {"BJ_BAND": "1", "BJ_COL16": "1"}), (4, 16, {"BJ_BAND": "1", "BJ_COL16": "1"}),
+                                       (5, 3, {"BJ_BSR": "1"})])
+def test_full_size_opt_in_variants(B, torch_, rel, monkeypatch, cfg, b, env):
+    """The byte-reducing variants at BASELINE.json's full sizes, in the launch configuration
+    `bench.py --band 1 --col16 1` / `--bsr 1` times: whole-vector parity of every op with the oracle, and a short kappa run."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    A = mat(cfg, "full")
+    h, keep = B.setup_from_host(A, b)
+    info = B.bj_get_info(h)
+    if "BJ_BAND" in env:
+        assert info["band_width"] == 1 and info["col16"] == 1
+    if "BJ_BSR" in env:
+        assert info["spmv_kernel"] == 2
+    P = oracle.Precond(A, b)
+    g = B.bj_cond_estimate_ex(h, 12, reorth=False)
+    c = P.cond_estimate(12, reorth=False)
+    assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+    B.bj_destroy(h)
+    del h, keep
+    check_all_ops(B, torch_, A, b, rel, seeds=(31,))
+    _MATS.pop((cfg, "full"), None)
+    torch_.cuda.empty_cache()
