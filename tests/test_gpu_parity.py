@@ -731,3 +731,32 @@ def test_full_size_opt_in_variants(B, torch_, rel, monkeypatch, cfg, b, env):
     check_all_ops(B, torch_, A, b, rel, seeds=(31,))
     _MATS.pop((cfg, "full"), None)
     torch_.cuda.empty_cache()
+
+
+def test_handles_release_their_device_memory(B, torch_, monkeypatch):
+    """Setup / Lanczos / PCG / batch / BSR / 16-bit-column workspaces all belong to the handle: after destroy and
+    bj_release_cached_memory the free device memory is back where it started."""
+    A = mat(5, "small")
+    rp, ci, val = (torch_.from_numpy(a).cuda() for a in (A.row_ptr, A.col_idx, A.val))
+    x = dev(torch_, W.seeded_vector(1, A.n))
+    torch_.cuda.synchronize()
+    B.bj_release_cached_memory()
+    free0, _ = torch_.cuda.mem_get_info()
+    monkeypatch.setenv("BJ_BSR", "1")
+    monkeypatch.setenv("BJ_COL16", "1")
+    monkeypatch.setenv("BJ_BAND", "1")
+    for rep in range(12):
+        for b in (0, 3, 8, 24):
+            h = B.bj_setup(rp, ci, val, b)
+            B.bj_op_apply(h, x)
+            B.bj_cond_estimate_ex(h, 6, reorth=bool(rep & 1))
+            B.bj_pcg_solve(h, x, max_iters=4, rtol=0.0)
+            if b in (3, 24):
+                B.bj_cond_estimate_batch(h, 2, 4)
+                B.bj_pcg_solve_batch(h, 2, x, max_iters=3, rtol=0.0)
+            B.bj_destroy(h)
+    torch_.cuda.synchronize()
+    torch_.cuda.empty_cache()
+    B.bj_release_cached_memory()
+    free1, _ = torch_.cuda.mem_get_info()
+    assert free0 - free1 <= 64 << 20, (free0, free1)
