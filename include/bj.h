@@ -194,22 +194,24 @@ int bj_profile_get(bj_handle_t h, int kind, double* ms_total_host, int64_t* laun
 
 /* many small independent systems in one launch (the paper's own sizes N = 2^10 .. 2^14,
  * PAPER.md:365, and its "solve each block separately" picture).  The handle's matrix is a batch of
- * `nsys` systems of equal size seg = n / nsys stored as ONE block-diagonal CSR (system s owns rows s*seg ..
- * (s+1)*seg - 1; the block size b must divide seg); bj_apply / bj_op_apply work on it unchanged.  This runs `iters`
+ * `nsys` systems stored as ONE block-diagonal CSR.  offsets_host == NULL: equal sizes seg = n / nsys (system s owns rows
+ * s*seg .. (s+1)*seg - 1; the block size b must divide seg).  Else offsets_host[0..nsys] (host, 0 = off[0] < .. < off[nsys] = n,
+ * every offset a multiple of b): systems of different sizes, e.g. the paper's 2^10, 2^12 and 2^14 mixed in one batch.
+ * bj_apply / bj_op_apply work on the batch unchanged.  This runs `iters`
  * Lanczos steps (no reorthogonalisation) on every system at once -- one CTA per system does the vector part of a step
  * with block-level reductions only -- and returns the extreme Ritz values per system: host arrays of nsys doubles
  * (kappa_s = lmax[s] / lmin[s]); iters_done_host (optional, nsys ints) is smaller than iters after a breakdown.
  * Start vector of system s: slice s of the seeded vector (bj_seeded_vector).  Synchronises. */
-int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, uint64_t seed, double* lmin_host, double* lmax_host,
-                           int32_t* iters_done_host);
+int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, const int64_t* offsets_host, int iters, uint64_t seed,
+                           double* lmin_host, double* lmax_host, int32_t* iters_done_host);
 
 /* NEXT-4, the solve side: PCG on every system of the batch at once (same layout rules as bj_cond_estimate_batch), each
  * system with its own step lengths and its own stopping test ||r_s|| / ||b_s|| <= rtol; a finished system is frozen
  * (its direction is zeroed) while the others go on.  b_dev / x_dev: device vectors of length n (x out).  Host outputs
  * (each optional, nsys entries): iterations taken, recurrence residual, and the paper's ||A x - b|| / ||b|| per system.
  * Synchronises. */
-int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_dev, double* x_dev, int max_iters, double rtol,
-                       int32_t* iters_host, double* relres_host, double* true_relres_host);
+int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const int64_t* offsets_host, const double* b_dev, double* x_dev,
+                       int max_iters, double rtol, int32_t* iters_host, double* relres_host, double* true_relres_host);
 
 /* Diagnostic (not on the operator path): the machine envelope that bounds the SpMV of matrices with random column
  * structure (config 3), which is limited by one L1 wavefront per 8-byte gather and not by HBM.  Measures, on the

@@ -92,8 +92,8 @@ def lib():
         L.bj_seeded_vector.argtypes = [vp, C.c_uint64, vp]
         L.bj_pcg_solve.argtypes = [vp, vp, vp, C.POINTER(bj_pcg_opts_t), C.POINTER(bj_pcg_result_t)]
         L.bj_release_cached_memory.argtypes = []
-        L.bj_cond_estimate_batch.argtypes = [vp, i64, i32, C.c_uint64, vp, vp, vp]
-        L.bj_pcg_solve_batch.argtypes = [vp, i64, vp, vp, i32, C.c_double, vp, vp, vp]
+        L.bj_cond_estimate_batch.argtypes = [vp, i64, vp, i32, C.c_uint64, vp, vp, vp]
+        L.bj_pcg_solve_batch.argtypes = [vp, i64, vp, vp, vp, i32, C.c_double, vp, vp, vp]
         L.bj_probe_gather_stream.argtypes = [i64, i64, i64] + [C.POINTER(C.c_double)] * 3
         L.bj_profile_enable.argtypes = [vp, i32]
         L.bj_profile_get.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
@@ -269,17 +269,29 @@ def bj_seeded_vector(h, seed: int, v=None):
     return v
 
 
-def bj_cond_estimate_batch(h, nsys: int, iters: int, seed: int = BJ_DEFAULT_SEED) -> dict:
-    """Per-system Lanczos extremes of a batch of `nsys` equal-size systems stored as one block-diagonal CSR."""
+def _offsets_arg(offsets, nsys):
+    import numpy as np
+    if offsets is None:
+        return None, None
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    if off.shape != (nsys + 1,):
+        raise ValueError("offsets must have nsys + 1 entries")
+    return off, off.ctypes.data_as(C.c_void_p)
+
+
+def bj_cond_estimate_batch(h, nsys: int, iters: int, seed: int = BJ_DEFAULT_SEED, offsets=None) -> dict:
+    """Per-system Lanczos extremes of a batch of `nsys` systems stored as one block-diagonal CSR (equal sizes, or
+    `offsets` = nsys + 1 row offsets)."""
     import numpy as np
     lmin, lmax = np.zeros(nsys), np.zeros(nsys)
     done = np.zeros(nsys, dtype=np.int32)
-    _check(lib().bj_cond_estimate_batch(h.ptr, int(nsys), int(iters), seed & 0xFFFFFFFFFFFFFFFF, lmin.ctypes.data_as(C.c_void_p),
+    keep, offp = _offsets_arg(offsets, nsys)
+    _check(lib().bj_cond_estimate_batch(h.ptr, int(nsys), offp, int(iters), seed & 0xFFFFFFFFFFFFFFFF, lmin.ctypes.data_as(C.c_void_p),
                                         lmax.ctypes.data_as(C.c_void_p), done.ctypes.data_as(C.c_void_p)))
     return {"lmin": lmin, "lmax": lmax, "kappa": lmax / lmin, "iters_done": done}
 
 
-def bj_pcg_solve_batch(h, nsys: int, b, x=None, max_iters: int = 1000, rtol: float = 1e-3) -> dict:
+def bj_pcg_solve_batch(h, nsys: int, b, x=None, max_iters: int = 1000, rtol: float = 1e-3, offsets=None) -> dict:
     """PCG on every system of a batch at once (per-system scalars and stopping tests)."""
     import numpy as np
     import torch
@@ -287,7 +299,8 @@ def bj_pcg_solve_batch(h, nsys: int, b, x=None, max_iters: int = 1000, rtol: flo
         x = torch.empty(h.n, dtype=torch.float64, device=b.device)
     it = np.zeros(nsys, dtype=np.int32)
     rel, trel = np.zeros(nsys), np.zeros(nsys)
-    _check(lib().bj_pcg_solve_batch(h.ptr, int(nsys), _dptr(b, torch.float64, h.n), _dptr(x, torch.float64, h.n), int(max_iters),
+    keep, offp = _offsets_arg(offsets, nsys)
+    _check(lib().bj_pcg_solve_batch(h.ptr, int(nsys), offp, _dptr(b, torch.float64, h.n), _dptr(x, torch.float64, h.n), int(max_iters),
                                     float(rtol), it.ctypes.data_as(C.c_void_p), rel.ctypes.data_as(C.c_void_p),
                                     trel.ctypes.data_as(C.c_void_p)))
     return {"x": x, "iters": it, "relres": rel, "true_relres": trel}

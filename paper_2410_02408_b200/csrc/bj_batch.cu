@@ -22,6 +22,13 @@ namespace {
 
 constexpr int kBatchThreads = 256;
 
+// rows of system s: equal sizes (off == nullptr) or explicit offsets off[0..nsys]
+__device__ __forceinline__ void batch_range(const int64_t* off, int64_t seg, int s, int64_t& base, int64_t& len)
+{
+    if (off) { base = off[s]; len = off[s + 1] - base; }
+    else { base = (int64_t)s * seg; len = seg; }
+}
+
 // sum over the CTA, valid on every thread
 __device__ __forceinline__ double block_sum_all(double v, double* sh)
 {
@@ -36,10 +43,11 @@ __device__ __forceinline__ double block_sum_all(double v, double* sh)
 
 // v_1 = v0 / ||v0|| per system
 __global__ void __launch_bounds__(kBatchThreads)
-lz_batch_start_kernel(int64_t seg, const double* __restrict__ v0, double* __restrict__ v)
+lz_batch_start_kernel(int64_t seg_, const int64_t* __restrict__ off, const double* __restrict__ v0, double* __restrict__ v)
 {
     __shared__ double sh[kBatchThreads / 32];
-    const int64_t base = (int64_t)blockIdx.x * seg;
+    int64_t base, seg;
+    batch_range(off, seg_, blockIdx.x, base, seg);
     double s = 0.0;
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
         const double x = v0[base + i];
@@ -53,7 +61,7 @@ lz_batch_start_kernel(int64_t seg, const double* __restrict__ v0, double* __rest
 // stop this system if beta_{j+1} <= tol max|alpha|;  v_{j+1} = w / beta_{j+1}.  alpha/beta: [nsys][m] (device).
 // A stopped system writes zeros into v_{j+1}, so the shared operator apply keeps producing zeros for it.
 __global__ void __launch_bounds__(kBatchThreads)
-lz_batch_step_kernel(int64_t seg, int m, int j, double tol, double* __restrict__ w, const double* vprev,
+lz_batch_step_kernel(int64_t seg_, const int64_t* __restrict__ off, int m, int j, double tol, double* __restrict__ w, const double* vprev,
                      const double* __restrict__ vcur, double* vnext,  // vprev and vnext share one buffer
                      double* __restrict__ alpha,
                      double* __restrict__ beta, double* __restrict__ amax, int* __restrict__ m_eff, int* __restrict__ stopped)
@@ -62,7 +70,8 @@ lz_batch_step_kernel(int64_t seg, int m, int j, double tol, double* __restrict__
     pdl_trigger();
     pdl_wait();
     const int s = blockIdx.x;
-    const int64_t base = (int64_t)s * seg;
+    int64_t base, seg;
+    batch_range(off, seg_, s, base, seg);
     if (stopped[s]) {
         if (vnext)
             for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) vnext[base + i] = 0.0;
@@ -143,12 +152,13 @@ batch_extremes_kernel(int64_t nsys, int m, const double* __restrict__ alpha, con
 // ---- batched PCG: per-system scalars, one CTA per system for the vector parts ------------------------------------
 // r = b, x = 0, bb[s] = ||b_s||^2 (a zero right-hand side stops its system at once)
 __global__ void __launch_bounds__(kBatchThreads)
-pcg_batch_init_kernel(int64_t seg, const double* __restrict__ b, double* __restrict__ r, double* __restrict__ x,
+pcg_batch_init_kernel(int64_t seg_, const int64_t* __restrict__ off, const double* __restrict__ b, double* __restrict__ r, double* __restrict__ x,
                       double* __restrict__ bb, int* __restrict__ stopped, int* __restrict__ nstopped)
 {
     __shared__ double sh[kBatchThreads / 32];
     const int s = blockIdx.x;
-    const int64_t base = (int64_t)s * seg;
+    int64_t base, seg;
+    batch_range(off, seg_, s, base, seg);
     double acc = 0.0;
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
         const double bi = b[base + i];
@@ -165,14 +175,15 @@ pcg_batch_init_kernel(int64_t seg, const double* __restrict__ b, double* __restr
 
 // first == 1: p = z, rho = r.z.   else: bt = (r.z) / rho, p = z + bt p, rho = r.z.   A stopped system keeps p = 0.
 __global__ void __launch_bounds__(kBatchThreads)
-pcg_batch_direction_kernel(int64_t seg, int first, const double* __restrict__ r, const double* __restrict__ z,
+pcg_batch_direction_kernel(int64_t seg_, const int64_t* __restrict__ off, int first, const double* __restrict__ r, const double* __restrict__ z,
                            double* __restrict__ p, double* __restrict__ rho, const int* __restrict__ stopped)
 {
     __shared__ double sh[kBatchThreads / 32];
     pdl_trigger();
     pdl_wait();
     const int s = blockIdx.x;
-    const int64_t base = (int64_t)s * seg;
+    int64_t base, seg;
+    batch_range(off, seg_, s, base, seg);
     if (stopped[s]) {
         for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) p[base + i] = 0.0;
         return;
@@ -187,7 +198,7 @@ pcg_batch_direction_kernel(int64_t seg, int first, const double* __restrict__ r,
 
 // a = rho / (p.q); x += a p; r -= a q; relres = ||r|| / ||b||; the system stops when relres <= rtol
 __global__ void __launch_bounds__(kBatchThreads)
-pcg_batch_update_kernel(int64_t seg, int k, double rtol, double* __restrict__ x, double* __restrict__ r,
+pcg_batch_update_kernel(int64_t seg_, const int64_t* __restrict__ off, int k, double rtol, double* __restrict__ x, double* __restrict__ r,
                         const double* __restrict__ p, const double* __restrict__ q, const double* __restrict__ rho,
                         const double* __restrict__ bb, double* __restrict__ relres, int* __restrict__ iters,
                         int* __restrict__ stopped, int* __restrict__ converged, int* __restrict__ nstopped)
@@ -197,7 +208,8 @@ pcg_batch_update_kernel(int64_t seg, int k, double rtol, double* __restrict__ x,
     pdl_wait();
     const int s = blockIdx.x;
     if (stopped[s]) return;
-    const int64_t base = (int64_t)s * seg;
+    int64_t base, seg;
+    batch_range(off, seg_, s, base, seg);
     double acc = 0.0;
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) acc = fma(p[base + i], q[base + i], acc);
     const double a = rho[s] / block_sum_all(acc, sh);
@@ -218,14 +230,15 @@ pcg_batch_update_kernel(int64_t seg, int k, double rtol, double* __restrict__ x,
 
 // true_relres[s] = ||q_s - b_s|| / ||b_s||  with q = A x
 __global__ void __launch_bounds__(kBatchThreads)
-pcg_batch_residual_kernel(int64_t seg, const double* __restrict__ q, const double* __restrict__ b,
+pcg_batch_residual_kernel(int64_t seg_, const int64_t* __restrict__ off, const double* __restrict__ q, const double* __restrict__ b,
                           const double* __restrict__ bb, double* __restrict__ out)
 {
     __shared__ double sh[kBatchThreads / 32];
     pdl_trigger();
     pdl_wait();
     const int s = blockIdx.x;
-    const int64_t base = (int64_t)s * seg;
+    int64_t base, seg;
+    batch_range(off, seg_, s, base, seg);
     double acc = 0.0;
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
         const double d = q[base + i] - b[base + i];
@@ -255,29 +268,56 @@ static void* batch_workspace(bj_handle_s* h, size_t bytes)
     h->workspace_bytes += (int64_t)bytes;
     return h->batch_ws;
 }
+// offsets_host == nullptr: nsys equal systems (n must divide).  Else offsets_host[0..nsys], 0 = off[0] < off[1] < .. = n,
+// every system a whole number of Jacobi blocks.  Uploads the offsets to `dst` (device, nsys + 1 entries); *seg = n / nsys
+// or 0.  Returns the device pointer to use (nullptr for equal sizes) through *off_dev.
+static int batch_layout(bj_handle_s* h, int64_t nsys, const int64_t* offsets_host, int64_t* dst, int64_t* seg,
+                        const int64_t** off_dev)
+{
+    *off_dev = nullptr;
+    *seg = 0;
+    if (!offsets_host) {
+        if (h->n % nsys) return BJ_ERR_INVALID_ARG;
+        *seg = h->n / nsys;
+        if (h->b > 0 && *seg % h->b) return BJ_ERR_INVALID_ARG;  // a Jacobi block must not straddle two systems
+        return BJ_OK;
+    }
+    if (offsets_host[0] != 0 || offsets_host[nsys] != h->n) return BJ_ERR_INVALID_ARG;
+    for (int64_t s = 0; s < nsys; ++s) {
+        if (offsets_host[s + 1] <= offsets_host[s]) return BJ_ERR_INVALID_ARG;
+        if (h->b > 0 && offsets_host[s] % h->b) return BJ_ERR_INVALID_ARG;
+    }
+    BJ_CUDA(cudaMemcpyAsync(dst, offsets_host, (size_t)(nsys + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, h->stream));
+    *off_dev = dst;
+    return BJ_OK;
+}
 }  // namespace bj
 
 using namespace bj;
 
-extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_dev, double* x_dev, int max_iters, double rtol,
-                                  int32_t* iters_host, double* relres_host, double* true_relres_host)
+extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const int64_t* offsets_host, const double* b_dev, double* x_dev,
+                                  int max_iters, double rtol, int32_t* iters_host, double* relres_host, double* true_relres_host)
 {
-    if (!h || h->failed || nsys < 1 || max_iters < 1 || !b_dev || !x_dev || b_dev == x_dev) return BJ_ERR_INVALID_ARG;
+    if (!h || h->failed || nsys < 1 || nsys > (1ll << 30) || max_iters < 1 || !b_dev || !x_dev || b_dev == x_dev) return BJ_ERR_INVALID_ARG;
     const int64_t n = h->n;
-    if (n % nsys) return BJ_ERR_INVALID_ARG;
-    const int64_t seg = n / nsys;
-    if (h->b > 0 && seg % h->b) return BJ_ERR_INVALID_ARG;
     cudaStream_t st = h->stream;
     // workspace: r, z, p, q; rho, bb, relres, true_relres [nsys each]; iters, stopped, converged [nsys each], nstopped
     const size_t vec_b = (size_t)4 * n * sizeof(double);
     const size_t scal_b = (size_t)4 * nsys * sizeof(double);
-    const size_t int_b = ((size_t)3 * nsys + 4) * sizeof(int);
-    char* ws = (char*)batch_workspace(h, vec_b + scal_b + int_b);
+    const size_t int_b = (((size_t)3 * nsys + 4) * sizeof(int) + 7) & ~(size_t)7;
+    const size_t off_b = (size_t)(nsys + 1) * sizeof(int64_t);
+    char* ws = (char*)batch_workspace(h, vec_b + scal_b + int_b + off_b);
     if (!ws) return BJ_ERR_ALLOC;
     double* vec = (double*)ws;
     double* scal = (double*)(ws + vec_b);
     int* ints = (int*)(ws + vec_b + scal_b);
     auto cleanup = [&]() {};
+    int64_t seg = 0;
+    const int64_t* off = nullptr;
+    {
+        const int lrc = batch_layout(h, nsys, offsets_host, (int64_t*)(ws + vec_b + scal_b + int_b), &seg, &off);
+        if (lrc != BJ_OK) return lrc;
+    }
     double *r = vec, *z = vec + n, *p = vec + 2 * n, *q = vec + 3 * n;
     double *rho = scal, *bb = scal + nsys, *relres = scal + 2 * nsys, *truerel = scal + 3 * nsys;
     int *iters = ints, *stopped = ints + nsys, *converged = ints + 2 * nsys, *nstopped = ints + 3 * nsys;
@@ -296,19 +336,19 @@ extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_d
         if (e != cudaSuccess) { set_cuda_error(e, #kernel); rc = BJ_ERR_CUDA; }                            \
         h->launches++;                                                                                     \
     } while (0)
-    pcg_batch_init_kernel<<<G, kBatchThreads, 0, st>>>(seg, b_dev, r, x_dev, bb, stopped, nstopped);
+    pcg_batch_init_kernel<<<G, kBatchThreads, 0, st>>>(seg, off, b_dev, r, x_dev, bb, stopped, nstopped);
     h->launches++;
     rc = launch_solve(h, 2, r, z);
-    if (rc == BJ_OK) BJ_BL(pcg_batch_direction_kernel, seg, 1, (const double*)r, (const double*)z, p, rho, (const int*)stopped);
+    if (rc == BJ_OK) BJ_BL(pcg_batch_direction_kernel, seg, off, 1, (const double*)r, (const double*)z, p, rho, (const int*)stopped);
     for (int k = 0; k < max_iters && rc == BJ_OK; ++k) {
         rc = spmv(p, q);
         if (rc != BJ_OK) break;
-        BJ_BL(pcg_batch_update_kernel, seg, k, rtol, x_dev, r, (const double*)p, (const double*)q, (const double*)rho,
+        BJ_BL(pcg_batch_update_kernel, seg, off, k, rtol, x_dev, r, (const double*)p, (const double*)q, (const double*)rho,
               (const double*)bb, relres, iters, stopped, converged, nstopped);
         if (rc != BJ_OK) break;
         rc = launch_solve(h, 2, r, z);
         if (rc != BJ_OK) break;
-        BJ_BL(pcg_batch_direction_kernel, seg, 0, (const double*)r, (const double*)z, p, rho, (const int*)stopped);
+        BJ_BL(pcg_batch_direction_kernel, seg, off, 0, (const double*)r, (const double*)z, p, rho, (const int*)stopped);
         if ((k + 1) % 16 == 0 && k + 1 < max_iters && rc == BJ_OK) {  // every system done?
             int ns = 0;
             e = cudaMemcpyAsync(&ns, nstopped, sizeof(int), cudaMemcpyDeviceToHost, st);
@@ -318,7 +358,7 @@ extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_d
         }
     }
     if (rc == BJ_OK) rc = spmv(x_dev, q);
-    if (rc == BJ_OK) BJ_BL(pcg_batch_residual_kernel, seg, (const double*)q, b_dev, (const double*)bb, truerel);
+    if (rc == BJ_OK) BJ_BL(pcg_batch_residual_kernel, seg, off, (const double*)q, b_dev, (const double*)bb, truerel);
 #undef BJ_BL
     if (rc == BJ_OK) {
         e = cudaSuccess;
@@ -332,14 +372,11 @@ extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const double* b_d
     return rc;
 }
 
-extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, uint64_t seed, double* lmin_host,
-                                      double* lmax_host, int32_t* iters_done_host)
+extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, const int64_t* offsets_host, int iters, uint64_t seed,
+                                      double* lmin_host, double* lmax_host, int32_t* iters_done_host)
 {
     if (!h || h->failed || nsys < 1 || iters < 1 || !lmin_host || !lmax_host) return BJ_ERR_INVALID_ARG;
     const int64_t n = h->n;
-    if (n % nsys) return BJ_ERR_INVALID_ARG;
-    const int64_t seg = n / nsys;
-    if (h->b > 0 && seg % h->b) return BJ_ERR_INVALID_ARG;  // a Jacobi block must not straddle two systems
     if (nsys > (1ll << 30)) return BJ_ERR_TOO_LARGE;
     const int m = iters;
     cudaStream_t st = h->stream;
@@ -348,13 +385,20 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
     // workspace: v_prev, v_cur (rotating), w; alpha/beta [nsys][m]; amax, lmin, lmax [nsys]; m_eff, stopped [nsys]
     const size_t vec_b = (size_t)3 * n * sizeof(double);
     const size_t scal_b = ((size_t)2 * nsys * m + 3 * nsys) * sizeof(double);
-    const size_t int_b = (size_t)2 * nsys * sizeof(int);
-    char* ws = (char*)batch_workspace(h, vec_b + scal_b + int_b);
+    const size_t int_b = ((size_t)2 * nsys * sizeof(int) + 7) & ~(size_t)7;
+    const size_t off_b = (size_t)(nsys + 1) * sizeof(int64_t);
+    char* ws = (char*)batch_workspace(h, vec_b + scal_b + int_b + off_b);
     if (!ws) return BJ_ERR_ALLOC;
     double* vec = (double*)ws;
     double* scal = (double*)(ws + vec_b);
     int* ints = (int*)(ws + vec_b + scal_b);
     auto cleanup = [&]() {};
+    int64_t seg = 0;
+    const int64_t* off = nullptr;
+    {
+        const int lrc = batch_layout(h, nsys, offsets_host, (int64_t*)(ws + vec_b + scal_b + int_b), &seg, &off);
+        if (lrc != BJ_OK) return lrc;
+    }
     double* V[2] = {vec, vec + n};
     double* w = vec + 2 * n;
     double* alpha = scal;
@@ -371,7 +415,7 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
 
     rc = launch_seeded_vector(h, seed, w);  // the start vector of system s is this vector's slice s
     if (rc == BJ_OK) {
-        lz_batch_start_kernel<<<(unsigned)nsys, kBatchThreads, 0, st>>>(seg, w, V[0]);
+        lz_batch_start_kernel<<<(unsigned)nsys, kBatchThreads, 0, st>>>(seg, off, w, V[0]);
         h->launches++;
     }
     for (int j = 0; j < m && rc == BJ_OK; ++j) {
@@ -379,7 +423,7 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, int iters, ui
         double* vn = V[(j + 1) & 1];
         rc = op_apply_device(h, vj, w);  // the whole batch at once: the matrix is block diagonal
         if (rc != BJ_OK) break;
-        e = launch_kernel(lz_batch_step_kernel, dim3((unsigned)nsys), dim3(kBatchThreads), 0, st, h->pdl, seg, m, j, tol, w,
+        e = launch_kernel(lz_batch_step_kernel, dim3((unsigned)nsys), dim3(kBatchThreads), 0, st, h->pdl, seg, off, m, j, tol, w,
                           (const double*)vn, (const double*)vj, j + 1 < m ? vn : (double*)nullptr, alpha, beta, amax, m_eff,
                           stopped);
         if (e != cudaSuccess) { set_cuda_error(e, "lz_batch_step_kernel"); rc = BJ_ERR_CUDA; break; }

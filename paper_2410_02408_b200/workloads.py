@@ -394,3 +394,32 @@ def batch_system(A: CSR, s: int) -> CSR:
     p0, p1 = int(A.row_ptr[r0]), int(A.row_ptr[r1])
     return CSR(seg, (A.row_ptr[r0:r1 + 1] - p0).astype(np.int32), (A.col_idx[p0:p1] - r0).astype(np.int32),
                A.val[p0:p1].copy(), {"kind": "batch_member", "s": s})
+
+
+def batch_poisson_mixed(grids, seed: int = SEED) -> CSR:
+    """A batch of systems of DIFFERENT sizes in one block-diagonal CSR: system s is config 1's construction on a
+    grids[s] x grids[s] grid (32, 64, 128 -> N = 2^10, 2^12, 2^14: the paper's three sizes), its diagonal draw
+    taken from one Philox stream in system order.  meta["offsets"]: row offsets, len(grids) + 1 entries."""
+    import scipy.sparse as sp
+    rng = _rng(1, seed)
+    mats, offsets = [], [0]
+    for n in grids:
+        a = laplacian((n, n))
+        rows = np.repeat(np.arange(a.n), np.diff(a.row_ptr.astype(np.int64)))
+        val = a.val.copy()
+        val[a.col_idx == rows] = 4.0 + rng.random(a.n)
+        mats.append(sp.csr_matrix((val, a.col_idx, a.row_ptr), shape=(a.n, a.n)))
+        offsets.append(offsets[-1] + a.n)
+    A = from_scipy(sp.block_diag(mats, format="csr"))
+    A.meta.update({"kind": "batch_mixed", "nsys": len(grids), "offsets": np.asarray(offsets, dtype=np.int64),
+                   "name": "batch_mixed_poisson2d_" + "_".join(str(g) for g in grids)})
+    return A
+
+
+def batch_member(A: CSR, s: int) -> CSR:
+    """System s of a batch with meta["offsets"] as a CSR of its own."""
+    off = A.meta["offsets"]
+    r0, r1 = int(off[s]), int(off[s + 1])
+    p0, p1 = int(A.row_ptr[r0]), int(A.row_ptr[r1])
+    return CSR(r1 - r0, (A.row_ptr[r0:r1 + 1] - p0).astype(np.int32), (A.col_idx[p0:p1] - r0).astype(np.int32),
+               A.val[p0:p1].copy(), {"kind": "batch_member", "s": s})

@@ -481,6 +481,30 @@ def test_batched_small_systems(B, torch_, rel):
         assert e2 <= 1e-7 and g["relres"][s] <= 1e-8 and g["true_relres"][s] <= 2e-8, (s, e2)
     assert len(set(g["iters"].tolist())) > 1                      # the systems really stop at different steps
     B.bj_destroy(h)
+    # systems of DIFFERENT sizes in one batch: the paper's three sizes N = 2^10, 2^12, 2^14 side by side
+    Am = W.batch_poisson_mixed([32, 64, 32, 128, 16])
+    off = Am.meta["offsets"]
+    ns = len(off) - 1
+    v0m = W.seeded_vector(B.BJ_DEFAULT_SEED, Am.n)
+    h, keep = B.setup_from_host(Am, 4)
+    g = B.bj_cond_estimate_batch(h, ns, 25, offsets=off)
+    rhs = W.seeded_vector(21, Am.n)
+    gp = B.bj_pcg_solve_batch(h, ns, dev(torch_, rhs), max_iters=300, rtol=1e-8, offsets=off)
+    xg = gp["x"].cpu().numpy()
+    for s in range(ns):
+        P = oracle.Precond(W.batch_member(Am, s), 4)
+        lo, hi = int(off[s]), int(off[s + 1])
+        c = P.cond_estimate(25, v0=v0m[lo:hi], reorth=False)
+        assert abs(g["kappa"][s] / c["kappa"] - 1) <= TOL_KAPPA, (s, g["kappa"][s], c["kappa"])
+        cp = P.pcg(rhs[lo:hi], 300, 1e-8)
+        assert abs(int(gp["iters"][s]) - cp["iters"]) <= 1
+        e2, ei = rel(xg[lo:hi], cp["x"])
+        assert e2 <= 1e-7, (s, e2)
+    with pytest.raises(B.BJError):
+        B.bj_cond_estimate_batch(h, ns, 5, offsets=np.r_[off[:-1], off[-1] - 4])      # offsets must end at n
+    with pytest.raises(B.BJError):
+        B.bj_cond_estimate_batch(h, ns, 5, offsets=np.r_[0, off[1] + 2, off[2:]])      # ... and fall on block boundaries
+    B.bj_destroy(h)
     # a system whose preconditioner is exact breaks down at step 1 while the others go on
     Ab = W.block_diagonal_spd(64, 8)
     h, keep = B.setup_from_host(Ab, 8)
