@@ -29,6 +29,10 @@ def main():
         out.append(f"b{b}_lmin_m50 {r['lmin']!r}")
         out.append(f"b{b}_lmax_m50 {r['lmax']!r}")
         out.append(f"b{b}_kappa_m50 {r['kappa']!r}")
+        pc = P.pcg(W.seeded_vector(17, A.n), 200, 1e-8)      # NEXT-1: PCG to 1e-8 from x0 = 0
+        out.append(f"b{b}_pcg_iters {pc['iters']!r}")
+        out.append(f"b{b}_pcg_alpha0 {float(pc['alpha'][0])!r}")
+        out.append(f"b{b}_pcg_x_norm2 {float(np.linalg.norm(pc['x']))!r}")
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_cfg1_fixture.txt")
     with open(path, "w") as fh:
         fh.write("# written by tests/golden/write_oracle_fixture.py (oracle only); config 1, seed %d\n" % W.SEED)

@@ -505,3 +505,28 @@ def test_pcg_terminates_in_as_many_steps_as_distinct_eigenvalues():
     dd, ee = oracle.cg_tridiag(rl["alpha"], rl["beta"][:11])
     ev = np.linalg.eigvalsh(np.diag(dd) + np.diag(ee, 1) + np.diag(ee, -1))
     assert np.allclose(ev, mu(12), rtol=1e-8, atol=0)
+
+
+def test_oracle_reproduces_its_committed_fixture():
+    """Regression guard for the oracle + generator pair: tests/golden/oracle_cfg1_fixture.txt was written by
+    tests/golden/write_oracle_fixture.py (oracle only, never the CUDA path); a change of the oracle's arithmetic or of the
+    config-1 generator shows up here and must be justified in the commit that rewrites the file."""
+    fix = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "oracle_cfg1_fixture.txt")) as fh:
+        for line in fh:
+            parts = line.split("#")[0].split()
+            if len(parts) == 2:
+                fix[parts[0]] = float(parts[1])
+    A = W.build(1, "full")
+    x = W.seeded_vector(12345, A.n)
+    for b in (0, 1, 4):
+        P = oracle.Precond(A, b)
+        y = P.op_apply(x)
+        r = P.cond_estimate(50)
+        pc = P.pcg(W.seeded_vector(17, A.n), 200, 1e-8)
+        got = {f"b{b}_op_apply_norm2": float(np.linalg.norm(y)), f"b{b}_op_apply_y0": float(y[0]), f"b{b}_lmin_m50": r["lmin"],
+               f"b{b}_lmax_m50": r["lmax"], f"b{b}_kappa_m50": r["kappa"], f"b{b}_pcg_iters": float(pc["iters"]),
+               f"b{b}_pcg_alpha0": float(pc["alpha"][0]), f"b{b}_pcg_x_norm2": float(np.linalg.norm(pc["x"]))}
+        for k, v in got.items():
+            assert k in fix, k
+            assert abs(v - fix[k]) <= 1e-11 * max(1.0, abs(fix[k])), (k, v, fix[k])
