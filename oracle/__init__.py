@@ -160,6 +160,49 @@ class Precond:
         return {"x": x, "iters": k, "alpha": alpha[:k].copy(), "beta": beta[:max(nb, 0)].copy(),
                 "relres": relres[:k].copy(), "true_relres": tr.value}
 
+    def lanczos_minv(self, m: int, r0=None, seed: int = DEFAULT_SEED, tol_bd: float = TOL_BREAKDOWN, return_basis: bool = False):
+        """Lanczos on M^-1 A in the M inner product ("the M^-1 A formulation (same spectrum)"): ONE pass
+        over the factor per step instead of the two of L^-1 A L^-T.  With u_j M-orthonormal and rh_j = M u_j the three-term
+        recurrence  M^-1 A u_j = bt_{j+1} u_{j+1} + al_j u_j + bt_j u_{j-1}  reads, multiplied by M,
+            r_{j+1} = A u_j - al_j rh_j - bt_j rh_{j-1},   al_j = u_j . A u_j,
+            z_{j+1} = M^-1 r_{j+1},   bt_{j+1} = sqrt(r_{j+1} . z_{j+1}),   u_{j+1} = z_{j+1} / bt_{j+1},  rh_{j+1} = r_{j+1} / bt_{j+1},
+        started from r_0 (seeded vector), z_0 = M^-1 r_0, bt_0 = sqrt(r_0 . z_0) (a normalisation, not an entry of T).
+        T = tridiag(bt_1..; al_0..) is the Lanczos matrix of L^-1 A L^-T started at L^-1 r_0 (same spectrum: A^ = L^-1 A L^-T
+        is similar to M^-1 A).  No reorthogonalisation.  Same breakdown rule as lanczos().  b = 0: M = I.
+        Returns (alpha[0..k-1], beta[0..k-1]) with beta[j] = bt_{j+1}, like lanczos()."""
+        r = seeded_vector(seed, self.n) if r0 is None else _f64(r0).copy()
+        minv = (lambda v: self.apply(v)) if self.b > 0 else (lambda v: v.copy())
+        z = minv(r)
+        bt = float(np.sqrt(np.dot(r, z)))
+        rh_prev = np.zeros(self.n)
+        bt_j = 0.0
+        alpha, beta, U = [], [], []
+        amax = 0.0
+        for j in range(m):
+            u = z / bt
+            rh = r / bt
+            if return_basis:
+                U.append(u)
+            p = spmv(self.A, u)
+            a = float(np.dot(u, p))
+            rn = p - a * rh - bt_j * rh_prev
+            zn = minv(rn)
+            bn = float(np.sqrt(max(np.dot(rn, zn), 0.0)))
+            alpha.append(a); beta.append(bn)
+            amax = max(amax, abs(a))
+            if not (bn > tol_bd * amax):
+                break
+            rh_prev, bt_j = rh, bn
+            r, z, bt = rn, zn, bn
+        out = (np.array(alpha), np.array(beta))
+        return out + (np.array(U).T,) if return_basis else out
+
+    def cond_estimate_minv(self, m: int, **kw):
+        alpha, beta = self.lanczos_minv(m, **kw)
+        tmin, tmax, rmin, rmax = tridiag_extremes(alpha, beta)
+        return {"lmin": tmin, "lmax": tmax, "kappa": tmax / tmin, "res_min": rmin, "res_max": rmax,
+                "iters_done": len(alpha), "alpha": alpha, "beta": beta}
+
     def cond_estimate(self, m: int, **kw):
         alpha, beta = self.lanczos(m, **kw)
         tmin, tmax, rmin, rmax = tridiag_extremes(alpha, beta)

@@ -530,3 +530,89 @@ def test_oracle_reproduces_its_committed_fixture():
         for k, v in got.items():
             assert k in fix, k
             assert abs(v - fix[k]) <= 1e-11 * max(1.0, abs(fix[k])), (k, v, fix[k])
+
+
+# ---------------------------------------------------------------- M-inner-product Lanczos (NEXT-2) ----
+def _dense_M(A, b):
+    """blockdiag(D_k) from the dense matrix by plain slicing (not through the oracle's extract)."""
+    Ad = A.to_dense()
+    M = np.zeros_like(Ad)
+    for lo in range(0, A.n, b):
+        hi = min(lo + b, A.n)
+        M[lo:hi, lo:hi] = Ad[lo:hi, lo:hi]
+    return Ad, M
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (4, 16), (5, 3), (3, 7)])
+def test_minv_lanczos_basis_is_M_orthonormal_and_projects_A_onto_T(cfg, b):
+    """What defines the method: U^T M U = I and U^T A U = T (a dropped term, a wrong sign or a missing 1/bt breaks one),
+    and the residual of the three-term relation A U = M U T + r_{m} e_m^T."""
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    m = 8
+    alpha, beta, U = P.lanczos_minv(m, return_basis=True)
+    assert len(alpha) == m and U.shape == (A.n, m)
+    Ad, M = _dense_M(A, b)
+    T = np.diag(alpha) + np.diag(beta[:-1], 1) + np.diag(beta[:-1], -1)
+    scale = np.abs(T).max()
+    assert np.abs(U.T @ M @ U - np.eye(m)).max() < 1e-10
+    assert np.abs(U.T @ Ad @ U - T).max() < 1e-10 * scale
+    Rm = Ad @ U - M @ U @ T                      # only the last column is non-zero: bt_m M u_m
+    assert np.abs(Rm[:, :-1]).max() < 1e-10 * scale
+    last = Rm[:, -1]
+    assert abs(np.sqrt(last @ np.linalg.solve(M, last)) - beta[-1]) < 1e-10 * scale
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (4, 16)])
+def test_minv_lanczos_full_run_gives_the_generalised_eigenvalues(cfg, b):
+    """Library routine for the same spectrum: scipy.linalg.eigh(A, M) (A x = lambda M x).  Small n, so the run without
+    reorthogonalisation is cut at 12 steps and checked through interlacing + Ritz residual bounds; the extremes it finds
+    must be eigenvalues to within the bound."""
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    Ad, M = _dense_M(A, b)
+    ev = sla.eigh(Ad, M, eigvals_only=True)
+    alpha, beta = P.lanczos_minv(12)
+    for m in (3, 6, 12):
+        tmin, tmax, rmin, rmax = oracle.tridiag_extremes(alpha[:m], beta[:m])
+        assert tmin >= ev[0] - 1e-10 and tmax <= ev[-1] + 1e-10
+        assert np.abs(ev - tmin).min() <= rmin + 1e-10
+        assert np.abs(ev - tmax).min() <= rmax + 1e-10
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (3, 32), (4, 16), (5, 24)])
+def test_minv_lanczos_equals_split_lanczos_started_at_Linv_r0(cfg, b):
+    """Same tridiagonal as Lanczos on L^-1 A L^-T from v_1 = L^-1 r_0 / ||.|| (similarity) for as many steps as
+    rounding keeps the two recurrences together."""
+    A = W.build(cfg, "tiny")
+    P = oracle.Precond(A, b)
+    r0 = W.seeded_vector(5, A.n)
+    a1, b1 = P.lanczos_minv(6, r0=r0)
+    a2, b2 = P.lanczos(6, v0=P.solve_L(r0), reorth=False)
+    assert np.abs(a1 - a2).max() < 1e-9 * np.abs(a2).max()
+    assert np.abs(b1 - b2).max() < 1e-9 * np.abs(a2).max()
+
+
+def test_minv_lanczos_special_cases():
+    A = W.build(1, "tiny")
+    # b = 0: M = I, the plain Lanczos recurrence on A from the same start
+    P0 = oracle.Precond(A, 0)
+    r0 = W.seeded_vector(9, A.n)
+    a1, b1 = P0.lanczos_minv(10, r0=r0)
+    a2, b2 = P0.lanczos(10, v0=r0, reorth=False)
+    assert np.abs(a1 - a2).max() < 1e-11 and np.abs(b1 - b2).max() < 1e-11
+    # exact preconditioner (one block = the matrix): M^-1 A = I, alpha_0 = 1 and breakdown after one step
+    Pn = oracle.Precond(A, A.n)
+    al, be = Pn.lanczos_minv(5)
+    assert len(al) == 1 and abs(al[0] - 1.0) < 1e-12 and be[0] < 1e-10
+    # first coefficient in closed form: al_0 = (z0 . A z0) / (r0 . z0), z0 = D^-1 r0 for b = 1
+    P1 = oracle.Precond(A, 1)
+    Ad = A.to_dense()
+    z0 = r0 / np.diag(Ad)
+    al, _ = P1.lanczos_minv(1, r0=r0)
+    assert abs(al[0] - (z0 @ Ad @ z0) / (r0 @ z0)) < 1e-12 * abs(al[0])
+    # M-Lanczos and the CG coefficients see the same Krylov space: T from PCG with right-hand side r0 is the same matrix
+    pc = P1.pcg(r0, 6, 0.0)
+    d, e = oracle.cg_tridiag(pc["alpha"], pc["beta"])
+    a6, b6 = P1.lanczos_minv(6, r0=r0)
+    assert np.abs(d - a6).max() < 1e-9 * np.abs(a6).max() and np.abs(e - b6[:5]).max() < 1e-9 * np.abs(a6).max()
