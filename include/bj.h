@@ -168,6 +168,18 @@ int bj_op_apply(bj_handle_t h, const double* x, double* y);
 int bj_cond_estimate(bj_handle_t h, int iters, double* lmin_host, double* lmax_host);
 int bj_cond_estimate_ex(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_lanczos_result_t* res_host);
 
+/* the same spectrum from Lanczos on M^-1 A in the M inner product -- ONE pass over the factor per step
+ * (z = M^-1 r, bj_apply) instead of the two of L^-1 A L^-T (A^ is similar to M^-1 A).  Three-term recurrence
+ *   r_{j+1} = A u_j - al_j rh_j - bt_j rh_{j-1},  al_j = u_j . A u_j,  z_{j+1} = M^-1 r_{j+1},  bt_{j+1} = sqrt(r_{j+1} . z_{j+1}),
+ *   u_j = z_j / bt_j,  rh_j = r_j / bt_j,
+ * started from r_0 = the seeded vector (or opts.v0, device, length n) -- T = tridiag(bt_1..; al_0..) equals the tridiagonal of
+ * bj_cond_estimate_ex started at v0 = L^-1 r_0.  opts.reorth is ignored (no reorthogonalisation: the fast-mode estimate);
+ * iters, seed, v0, breakdown_tol and every field of the result mean what they mean for bj_cond_estimate_ex.  Two kernels per
+ * step on the fused path (tile SpMV with a dot hook; block-solve pair with the combination built on the fly), vectors
+ * unnormalised, scalars on the device, one synchronisation at the end.  Workspace: the PCG workspace (4 n doubles, kept).
+ * A zero start vector returns BJ_ERR_INVALID_ARG.  Synchronises. */
+int bj_cond_estimate_minv(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_lanczos_result_t* res_host);
+
 /* preconditioned conjugate gradients for A x = b from x_0 = 0 with M = blockdiag(D_k)
  * (z = M^-1 r is bj_apply; b = 0 handle: plain CG), the classical stand-in for the solve stage that follows
  * the preconditioning path.  b_dev and x_dev are device vectors of length n (x_dev out).

@@ -23,7 +23,7 @@ EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_set_stream", "bj_set_option", "
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
            "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve",
-           "bj_probe_gather_stream", "bj_cond_estimate_batch", "bj_pcg_solve_batch"]
+           "bj_probe_gather_stream", "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv"]
 
 
 class bj_csr_t(C.Structure):
@@ -238,6 +238,21 @@ def bj_cond_estimate_ex(h, iters: int, reorth: bool = True, seed: int = BJ_DEFAU
                           _dptr(v0, torch.float64, h.n) if v0 is not None else None, breakdown_tol)
     r = bj_lanczos_result_t(0, 0.0, 0.0, 0.0, 0.0, alpha.ctypes.data_as(C.c_void_p), beta.ctypes.data_as(C.c_void_p))
     _check(lib().bj_cond_estimate_ex(h.ptr, C.byref(o), C.byref(r)))
+    k = r.iters_done
+    return {"iters_done": k, "lmin": r.lmin, "lmax": r.lmax, "kappa": r.lmax / r.lmin, "res_min": r.res_min,
+            "res_max": r.res_max, "alpha": alpha[:k].copy(), "beta": beta[:k].copy()}
+
+
+def bj_cond_estimate_minv(h, iters: int, seed: int = BJ_DEFAULT_SEED, r0=None, breakdown_tol: float = 0.0) -> dict:
+    """Lanczos on M^-1 A in the M inner product (one factor pass per step); same result fields as bj_cond_estimate_ex."""
+    import numpy as np
+    import torch
+    alpha = np.zeros(iters)
+    beta = np.zeros(iters)
+    o = bj_lanczos_opts_t(int(iters), 0, seed & 0xFFFFFFFFFFFFFFFF,
+                          _dptr(r0, torch.float64, h.n) if r0 is not None else None, breakdown_tol)
+    r = bj_lanczos_result_t(0, 0.0, 0.0, 0.0, 0.0, alpha.ctypes.data_as(C.c_void_p), beta.ctypes.data_as(C.c_void_p))
+    _check(lib().bj_cond_estimate_minv(h.ptr, C.byref(o), C.byref(r)))
     k = r.iters_done
     return {"iters_done": k, "lmin": r.lmin, "lmax": r.lmax, "kappa": r.lmax / r.lmin, "res_min": r.res_min,
             "res_max": r.res_max, "alpha": alpha[:k].copy(), "beta": beta[:k].copy()}

@@ -484,6 +484,13 @@ int bj_cond_estimate_ex(bj_handle_t h, const bj_lanczos_opts_t* o, bj_lanczos_re
     return lanczos_run(h, o, res);
 }
 
+int bj_cond_estimate_minv(bj_handle_t h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res)
+{
+    BJ_CHECK_H(h);
+    if (!o || !res || o->iters < 1 || o->iters > (1 << 20)) return BJ_ERR_INVALID_ARG;
+    return mlanczos_run(h, o, res);
+}
+
 int bj_cond_estimate(bj_handle_t h, int iters, double* lmin, double* lmax)
 {
     BJ_CHECK_H(h);

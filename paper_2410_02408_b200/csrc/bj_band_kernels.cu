@@ -201,7 +201,24 @@ solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
     } else if (LZ == 3) {
         double a;
         if (pcg_hook_begin(pcg, a)) return;  // uniform over the grid
-        if (act) {
+        if (pcg.mode) {  // three-term step of Lanczos on M^-1 A: r_{k+1} replaces r_{k-1} (uniform branch)
+            double cq, cr, cx;
+            mlz_hook_coeffs(pcg, cq, cr, cx);
+            if (act) {
+                double c[BMAX], xs[BMAX];
+                load_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
+                load_rows_rt<BMAX>(pcg.q, lo, n, b, vec, c);
+                load_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
+#pragma unroll
+                for (int i = 0; i < BMAX; ++i) {
+                    if (i < b) {
+                        v[i] = mlz_combine(cq, cr, cx, c[i], v[i], xs[i]);
+                        rin[i] = v[i];
+                    }
+                }
+                store_rows_rt<BMAX>(pcg.x, lo, n, b, vec, v);
+            }
+        } else if (act) {
             double c[BMAX];
             load_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
             load_rows_rt<BMAX>(pcg.q, lo, n, b, vec, c);

@@ -225,6 +225,9 @@ void lanczos_free(bj_handle_s* h);
 int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
 // k-th smallest eigenvalue (k = 0 .. m-1) of the symmetric tridiagonal (diag a[0..m-1], off-diagonal e[0..m-2]), bisection
 double tridiag_eig_k(int m, const double* a, const double* e, int k);
+void lanczos_fill_result(int me, const double* a, const double* b, bj_lanczos_result_t* res);
+// Lanczos on M^-1 A in the M inner product (bj_pcg.cu; shares the PCG workspace and the PCG hook of the solve kernels)
+int mlanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res);
 
 // preconditioned CG (bj_pcg.cu)
 int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* r);

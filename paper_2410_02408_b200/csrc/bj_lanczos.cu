@@ -455,14 +455,20 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     BJ_CUDA(cudaStreamSynchronize(st));
     const int me = done[1];
     if (me < 1) return BJ_ERR_CUDA;
-    res->iters_done = me;
-    res->lmin = tridiag_eig_k(me, a.data(), b.data(), 0);
-    res->lmax = tridiag_eig_k(me, a.data(), b.data(), me - 1);
-    res->res_min = fabs(b[me - 1]) * last_comp(me, a.data(), b.data(), res->lmin);
-    res->res_max = fabs(b[me - 1]) * last_comp(me, a.data(), b.data(), res->lmax);
-    if (res->alpha_host) std::copy(a.begin(), a.begin() + me, res->alpha_host);
-    if (res->beta_host) std::copy(b.begin(), b.begin() + me, res->beta_host);
+    lanczos_fill_result(me, a.data(), b.data(), res);
     return BJ_OK;
+}
+
+// extreme Ritz values, their residual bounds and the optional coefficient copies from alpha[0..me-1], beta[0..me-1]
+void lanczos_fill_result(int me, const double* a, const double* b, bj_lanczos_result_t* res)
+{
+    res->iters_done = me;
+    res->lmin = tridiag_eig_k(me, a, b, 0);
+    res->lmax = tridiag_eig_k(me, a, b, me - 1);
+    res->res_min = fabs(b[me - 1]) * last_comp(me, a, b, res->lmin);
+    res->res_max = fabs(b[me - 1]) * last_comp(me, a, b, res->lmax);
+    if (res->alpha_host) std::copy(a, a + me, res->alpha_host);
+    if (res->beta_host) std::copy(b, b + me, res->beta_host);
 }
 
 }  // namespace bj

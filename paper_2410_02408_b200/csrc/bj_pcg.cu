@@ -13,6 +13,7 @@
 #include <math.h>
 
 #include <algorithm>
+#include <cmath>
 #include <vector>
 
 #include "bj_device.cuh"
@@ -216,6 +217,68 @@ pcg_direction_fused_kernel(int64_t n, double* __restrict__ p, const double* __re
     for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) p[i] = fma(bt, p[i], z[i]);
 }
 
+// workspace of a run with up to m iterations: r, z, p, q (4 n doubles, kept by the handle); scalars, six partial arrays,
+// alpha / beta / relres, flags, three partial arrays of the fused path
+struct PcgWs {
+    double *r, *z, *p, *q, *scal, *P0, *PRa, *PRb, *PQ, *PRR, *PD, *alpha, *beta, *relres, *FP;
+    int* flags;  // 16 ints: [0..2] flags, [4..6] tickets of the fused path
+    size_t fcap;
+};
+
+int pcg_workspace(bj_handle_s* h, int m, PcgWs& w)
+{
+    const int64_t n = h->n;
+    w.fcap = (size_t)std::max<int64_t>(kMaxPartials, (h->nblocks + 127) / 128 + 1);
+    if (!h->pcg_vec) {
+        BJ_CUDA(cudaMalloc((void**)&h->pcg_vec, (size_t)4 * n * sizeof(double)));
+        h->workspace_bytes += (int64_t)4 * n * (int64_t)sizeof(double);
+    }
+    if (h->pcg_cap_iters < m) {
+        cudaFree(h->pcg_scal);
+        h->pcg_scal = nullptr;
+        h->pcg_cap_iters = 0;
+        BJ_CUDA(cudaMalloc((void**)&h->pcg_scal, sizeof(double) * (S_COUNT + 6 * (size_t)kMaxPartials + 3 * (size_t)m + 8 + 3 * w.fcap)));
+        h->pcg_cap_iters = m;
+    }
+    w.r = h->pcg_vec;
+    w.z = w.r + n;
+    w.p = w.z + n;
+    w.q = w.p + n;
+    w.scal = h->pcg_scal;
+    w.P0 = w.scal + S_COUNT;
+    w.PRa = w.P0 + kMaxPartials;
+    w.PRb = w.PRa + kMaxPartials;
+    w.PQ = w.PRb + kMaxPartials;
+    w.PRR = w.PQ + kMaxPartials;
+    w.PD = w.PRR + kMaxPartials;
+    w.alpha = w.PD + kMaxPartials;
+    w.beta = w.alpha + h->pcg_cap_iters;
+    w.relres = w.beta + h->pcg_cap_iters;
+    w.flags = reinterpret_cast<int*>(w.relres + h->pcg_cap_iters);
+    w.FP = w.relres + h->pcg_cap_iters + 8;
+    BJ_CUDA(cudaMemsetAsync(w.scal, 0, sizeof(double) * S_COUNT, h->stream));
+    BJ_CUDA(cudaMemsetAsync(w.alpha, 0, sizeof(double) * (3 * (size_t)h->pcg_cap_iters + 8), h->stream));
+    return BJ_OK;
+}
+
+// unfused step of Lanczos on M^-1 A (bj_pcg_fuse.cuh, mode 1): zp = sum PQ, the three coefficients, r_{k+1} written over r_{k-1}
+__global__ void __launch_bounds__(kReduceThreads)
+mlz_combine_kernel(int64_t n, const double* __restrict__ q, const double* __restrict__ r, double* __restrict__ x,
+                   const double* __restrict__ PQ, int nparts, const double* __restrict__ bsq, int k, double* __restrict__ alpha)
+{
+    __shared__ double sh[kReduceThreads / 32];
+    pdl_trigger();
+    pdl_wait();
+    const double zp = reduce_partials(PQ, nparts, sh);
+    const double b2 = bsq[k];
+    const double bt = sqrt(b2);
+    const double al = zp / b2;
+    const double cq = 1.0 / bt, cr = -al / bt, cx = k > 0 ? -bt / sqrt(bsq[k - 1]) : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) alpha[k] = al;
+    const Chunk c = my_chunk(n);
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) x[i] = mlz_combine(cq, cr, cx, q[i], r[i], x[i]);
+}
+
 }  // namespace
 
 void pcg_free(bj_handle_s* h)
@@ -235,42 +298,17 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     const double rtol = o->rtol > 0.0 ? o->rtol : 0.0;
     cudaStream_t st = h->stream;
 
-    // workspace: r, z, p, q; scalars, six partial arrays, alpha / beta / relres, flags, three partial arrays of the fused path
-    const size_t fcap = (size_t)std::max<int64_t>(kMaxPartials, (h->nblocks + 127) / 128 + 1);
-    if (!h->pcg_vec) {
-        BJ_CUDA(cudaMalloc((void**)&h->pcg_vec, (size_t)4 * n * sizeof(double)));
-        h->workspace_bytes += (int64_t)4 * n * (int64_t)sizeof(double);
-    }
-    if (h->pcg_cap_iters < m) {
-        cudaFree(h->pcg_scal);
-        h->pcg_scal = nullptr;
-        h->pcg_cap_iters = 0;
-        BJ_CUDA(cudaMalloc((void**)&h->pcg_scal, sizeof(double) * (S_COUNT + 6 * (size_t)kMaxPartials + 3 * (size_t)m + 8 + 3 * fcap)));
-        h->pcg_cap_iters = m;
-    }
-    double* r = h->pcg_vec;
-    double* z = r + n;
-    double* p = z + n;
-    double* q = p + n;
-    double* scal = h->pcg_scal;
-    double* P0 = scal + S_COUNT;
-    double* PRa = P0 + kMaxPartials;
-    double* PRb = PRa + kMaxPartials;
-    double* PQ = PRb + kMaxPartials;
-    double* PRR = PQ + kMaxPartials;
-    double* PD = PRR + kMaxPartials;
-    double* alpha = PD + kMaxPartials;
-    double* beta = alpha + h->pcg_cap_iters;
-    double* relres = beta + h->pcg_cap_iters;
-    int* flags = reinterpret_cast<int*>(relres + h->pcg_cap_iters);  // 16 ints: [0..2] flags, [4..6] tickets of the fused path
-    double* FP = relres + h->pcg_cap_iters + 8;                    // 3 x fcap partials of the fused path
-    BJ_CUDA(cudaMemsetAsync(scal, 0, sizeof(double) * S_COUNT, st));
-    BJ_CUDA(cudaMemsetAsync(alpha, 0, sizeof(double) * (3 * (size_t)h->pcg_cap_iters + 8), st));
+    PcgWs ws;
+    int rc = pcg_workspace(h, m, ws);
+    if (rc != BJ_OK) return rc;
+    double *r = ws.r, *z = ws.z, *p = ws.p, *q = ws.q, *scal = ws.scal, *P0 = ws.P0, *PRa = ws.PRa, *PRb = ws.PRb, *PQ = ws.PQ,
+           *PRR = ws.PRR, *PD = ws.PD, *alpha = ws.alpha, *beta = ws.beta, *relres = ws.relres, *FP = ws.FP;
+    int* flags = ws.flags;
+    const size_t fcap = ws.fcap;
 
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
     const bool pdl = h->pdl;
     cudaError_t e = cudaSuccess;
-    int rc = BJ_OK;
 #define BJ_LAUNCH(kernel, ...)                                                                  \
     do {                                                                                        \
         e = launch_kernel(kernel, dim3(G), dim3(kReduceThreads), 0, st, pdl, __VA_ARGS__);      \
@@ -292,7 +330,7 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     if (fused) {
         unsigned* tickets = reinterpret_cast<unsigned*>(flags + 4);
         LzReduce red_pq{FP, scal + S_PQ, tickets + 0, (int)fcap};
-        PcgHook hook;
+        PcgHook hook{};
         hook.x = x; hook.p = p; hook.r = r; hook.q = q; hook.pq = scal + S_PQ; hook.alpha = alpha; hook.flags = flags;
         hook.red_rr = LzReduce{FP + fcap, scal + S_RR, tickets + 1, (int)fcap};
         int rho_cur = S_RHO_A, rho_new = S_RHO_B;
@@ -376,6 +414,94 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     if (res->alpha_host) std::copy(ha.begin(), ha.begin() + it, res->alpha_host);
     if (res->beta_host) std::copy(hb.begin(), hb.begin() + std::max(nb, 0), res->beta_host);
     if (res->relres_host) std::copy(hr.begin(), hr.begin() + it, res->relres_host);
+    return BJ_OK;
+}
+
+// Lanczos on M^-1 A in the M inner product: one pass over the factor per step.  With z_k = M^-1 r_k,
+// bt_k^2 = r_k . z_k (bt_0 only normalises):
+//   q = A z_k;  al_k = (z_k . q) / bt_k^2;  r_{k+1} = q / bt_k - (al_k / bt_k) r_k - (bt_k / bt_{k-1}) r_{k-1};  z_{k+1} = M^-1 r_{k+1}
+// T = tridiag(bt_1..; al_0..) is the Lanczos matrix of L^-1 A L^-T started at L^-1 r_0.  Vectors stay unnormalised (the
+// scalars carry the scaling), so a step is TWO kernels on the fused path: the tile SpMV with its dot hook, and the solve
+// pair whose input is combined on the fly (PcgHook mode 1) and which finishes r_{k+1} . z_{k+1}.  No reorthogonalisation.
+int mlanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res)
+{
+    const int64_t n = h->n;
+    const int m = o->iters;
+    const double tol = o->breakdown_tol > 0.0 ? o->breakdown_tol : BJ_DEFAULT_BREAKDOWN_TOL;
+    cudaStream_t st = h->stream;
+    PcgWs ws;
+    int rc = pcg_workspace(h, m + 1, ws);
+    if (rc != BJ_OK) return rc;
+    double* rcur = ws.r;
+    double* rprev = ws.p;
+    double *z = ws.z, *q = ws.q, *alpha = ws.alpha, *bsq = ws.beta, *scal = ws.scal;  // bsq[0..m]
+    int* flags = ws.flags;
+    const size_t fcap = ws.fcap;
+    const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
+    const bool pdl = h->pdl;
+    cudaError_t e = cudaSuccess;
+#define BJ_LAUNCH(grid, kernel, ...)                                                            \
+    do {                                                                                        \
+        e = launch_kernel(kernel, dim3(grid), dim3(kReduceThreads), 0, st, pdl, __VA_ARGS__);   \
+        if (e != cudaSuccess) { set_cuda_error(e, #kernel); return BJ_ERR_CUDA; }               \
+        h->launches++;                                                                          \
+    } while (0)
+    if (o->v0) {
+        BJ_CUDA(cudaMemcpyAsync(rcur, o->v0, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    } else {
+        rc = launch_seeded_vector(h, o->seed, rcur);
+        if (rc != BJ_OK) return rc;
+    }
+    BJ_CUDA(cudaMemsetAsync(rprev, 0, sizeof(double) * n, st));
+    rc = launch_solve(h, 2, rcur, z);  // z_0 = M^-1 r_0  (b = 0: copy)
+    if (rc != BJ_OK) return rc;
+    BJ_LAUNCH(G, pcg_pq_kernel, n, (const double*)rcur, (const double*)z, ws.PRa, (const int*)flags);
+    BJ_LAUNCH(1, pcg_scalar_kernel, (const double*)ws.PRa, G, bsq, (const int*)flags);  // bt_0^2
+
+    const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && env_int("BJ_PCG_FUSE", 1) != 0;
+    unsigned* tickets = reinterpret_cast<unsigned*>(flags + 4);
+    LzReduce red_zp{ws.FP, scal + S_PQ, tickets + 0, (int)fcap};
+    PcgHook hook{};
+    hook.mode = 1; hook.q = q; hook.pq = scal + S_PQ; hook.alpha = alpha; hook.flags = flags; hook.bsq = bsq;
+    hook.red_rr = LzReduce{ws.FP + fcap, scal + S_RR, tickets + 1, (int)fcap};
+    for (int k = 0; k < m; ++k) {
+        if (fused) {
+            rc = launch_spmv_stream(h, z, q, false, nullptr, z, &red_zp);  // K1: q = A z_k, z_k . q
+            if (rc != BJ_OK) return rc;
+            hook.r = rcur; hook.x = rprev; hook.k = k;
+            hook.red_rz = LzReduce{ws.FP + 2 * fcap, bsq + k + 1, tickets + 2, (int)fcap};
+            rc = launch_solve(h, 2, nullptr, z, nullptr, nullptr, &hook);  // K2: r_{k+1}, z_{k+1}, bt_{k+1}^2
+            if (rc != BJ_OK) return rc;
+        } else {
+            rc = launch_spmv(h, z, q);
+            if (rc != BJ_OK) return rc;
+            BJ_LAUNCH(G, pcg_pq_kernel, n, (const double*)z, (const double*)q, ws.PQ, (const int*)flags);
+            BJ_LAUNCH(G, mlz_combine_kernel, n, (const double*)q, (const double*)rcur, rprev, (const double*)ws.PQ, G,
+                      (const double*)bsq, k, alpha);
+            rc = launch_solve(h, 2, rprev, z);
+            if (rc != BJ_OK) return rc;
+            BJ_LAUNCH(G, pcg_pq_kernel, n, (const double*)rprev, (const double*)z, ws.PRa, (const int*)flags);
+            BJ_LAUNCH(1, pcg_scalar_kernel, (const double*)ws.PRa, G, bsq + k + 1, (const int*)flags);
+        }
+        std::swap(rcur, rprev);  // r_{k+1} was written over r_{k-1}
+    }
+#undef BJ_LAUNCH
+    std::vector<double> a(m), b2(m + 1), b(m);
+    BJ_CUDA(cudaMemcpyAsync(a.data(), alpha, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(b2.data(), bsq, sizeof(double) * (m + 1), cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaStreamSynchronize(st));
+    if (!(b2[0] > 0.0) || !std::isfinite(b2[0])) return BJ_ERR_INVALID_ARG;  // r_0 = 0 (or not finite)
+    int me = 0;
+    double amax = 0.0;
+    for (int j = 0; j < m; ++j) {
+        if (!std::isfinite(a[j])) break;
+        b[j] = b2[j + 1] > 0.0 ? sqrt(b2[j + 1]) : 0.0;
+        amax = std::max(amax, fabs(a[j]));
+        me = j + 1;
+        if (!(b[j] > tol * amax)) break;  // breakdown: the steps after it computed nothing meaningful and are dropped
+    }
+    if (me < 1) return BJ_ERR_CUDA;
+    lanczos_fill_result(me, a.data(), b.data(), res);
     return BJ_OK;
 }
 

@@ -111,7 +111,22 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
     } else if (LZ == 3) {
         double a;
         if (pcg_hook_begin(pcg, a)) return;  // uniform over the grid
-        if (act) {
+        if (pcg.mode) {  // three-term step of Lanczos on M^-1 A: r_{k+1} replaces r_{k-1} (uniform branch)
+            double cq, cr, cx;
+            mlz_hook_coeffs(pcg, cq, cr, cx);
+            if (act) {
+                double c[B], xs[B];
+                load_rows<B, VEC>(pcg.r, lo, n, whole, v);
+                load_rows<B, VEC>(pcg.q, lo, n, whole, c);
+                load_rows<B, VEC>(pcg.x, lo, n, whole, xs);
+#pragma unroll
+                for (int i = 0; i < B; ++i) {
+                    v[i] = mlz_combine(cq, cr, cx, c[i], v[i], xs[i]);
+                    rin[i] = v[i];
+                }
+                store_rows<B, VEC>(pcg.x, lo, n, whole, v);
+            }
+        } else if (act) {
             double c[B];
             load_rows<B, VEC>(pcg.r, lo, n, whole, v);
             load_rows<B, VEC>(pcg.q, lo, n, whole, c);
@@ -402,6 +417,9 @@ solve_group_kernel(const GroupParams p)
     if (DIR == 0 && LZ == 2) stop = lz_epilogue_begin(p.epi, beta, inv_beta);
     double acc2 = 0.0;  // PCG: r.z
     if (DIR == 2 && LZ == 3) stop = pcg_hook_begin(p.pcg, alpha);  // alpha = the CG step length here
+    double mcq = 0.0, mcr = 0.0, mcx = 0.0;  // mode 1 (Lanczos on M^-1 A): coefficients of q, r, r_prev
+    const bool mlz = DIR == 2 && LZ == 3 && p.pcg.mode != 0;
+    if (mlz && !stop) mlz_hook_coeffs(p.pcg, mcq, mcr, mcx);
     if (stop) {  // uniform over the grid; the bulk copies already issued must land before the CTA may exit
         for (int s = 0; s < p.stages; ++s)
             if (first + s * stride < p.ntiles) mbar_wait(&full[s], 0u);
@@ -423,7 +441,7 @@ solve_group_kernel(const GroupParams p)
                 if (live) a[k] = p.pro.first ? p.pro.w0[row] : p.pro.w[row];
                 if (live && !p.pro.first) c[k] = p.pro.vcur[row];
             } else if (DIR == 2 && LZ == 3) {
-                if (live) { a[k] = p.pcg.r[row]; c[k] = p.pcg.q[row]; ew[k] = p.pcg.x[row]; ev[k] = p.pcg.p[row]; }
+                if (live) { a[k] = p.pcg.r[row]; c[k] = p.pcg.q[row]; ew[k] = p.pcg.x[row]; ev[k] = mlz ? 0.0 : p.pcg.p[row]; }
             } else {
                 if (live) a[k] = p.in[row];
                 if (DIR == 0 && LZ == 2) {  // the epilogue's own operands ride along one tile ahead
@@ -442,10 +460,14 @@ solve_group_kernel(const GroupParams p)
                 dst[k] = wi;
             } else if (DIR == 2 && LZ == 3) {  // r_new = r - a q (the solve's input, stored once), x += a p
                 const int64_t row = row0 + k * 32;
-                const double ri = a[k] - alpha * c[k];
+                const double ri = mlz ? mlz_combine(mcq, mcr, mcx, c[k], a[k], ew[k]) : a[k] - alpha * c[k];
                 if (tile < p.ntiles && row < p.n) {
-                    p.pcg.r[row] = ri;
-                    p.pcg.x[row] = fma(alpha, ev[k], ew[k]);
+                    if (mlz) {
+                        p.pcg.x[row] = ri;  // r_{k+1} takes the place of r_{k-1}
+                    } else {
+                        p.pcg.r[row] = ri;
+                        p.pcg.x[row] = fma(alpha, ev[k], ew[k]);
+                    }
                     acc = fma(ri, ri, acc);
                 }
                 dst[k] = (tile < p.ntiles && row < p.n) ? ri : 0.0;

@@ -784,3 +784,68 @@ def test_handles_release_their_device_memory(B, torch_, monkeypatch):
     B.bj_release_cached_memory()
     free1, _ = torch_.cuda.mem_get_info()
     assert free0 - free1 <= 64 << 20, (free0, free1)
+
+
+# ------------------------------------------------------------------ Lanczos on M^-1 A (NEXT-2) ----------
+@pytest.mark.parametrize("fuse", ["1", "0"])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_minv_lanczos_matches_oracle_small(B, torch_, monkeypatch, cfg, fuse):
+    """bj_cond_estimate_minv (one factor pass per step) against the oracle's M-inner-product Lanczos: the first coefficients
+    element by element, kappa at m = 50 to the bar of the north star.  fuse=1: two kernels per step where the solve kernel
+    carries the hook; fuse=0: the six-kernel step (also the path of b = 0 and of block sizes without a hooked kernel)."""
+    monkeypatch.setenv("BJ_PCG_FUSE", fuse)
+    A = mat(cfg, "small")
+    for b in ([0] if fuse == "0" else []) + W.BLOCK_SIZES[cfg]:
+        h, keep = B.setup_from_host(A, b)
+        P = oracle.Precond(A, b)
+        g = B.bj_cond_estimate_minv(h, 12)
+        c = P.cond_estimate_minv(12)
+        assert g["iters_done"] == c["iters_done"] == 12
+        sc = np.abs(c["alpha"]).max()
+        assert np.abs(g["alpha"] - c["alpha"]).max() <= 1e-9 * sc, (cfg, b)
+        assert np.abs(g["beta"] - c["beta"]).max() <= 1e-9 * sc, (cfg, b)
+        if b > 0:   # without reorthogonalisation kappa at m = 50 is reproducible on the preconditioned operators only
+            g = B.bj_cond_estimate_minv(h, 50)
+            c = P.cond_estimate_minv(50)
+            assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (cfg, b, g["kappa"], c["kappa"])
+            assert abs(g["res_min"] - c["res_min"]) <= 1e-6 * c["lmax"] and abs(g["res_max"] - c["res_max"]) <= 1e-6 * c["lmax"]
+        B.bj_destroy(h)
+
+
+def test_minv_lanczos_is_the_split_lanczos_from_Linv_r0(B, torch_):
+    """Both device estimates see one spectrum: T of bj_cond_estimate_minv from r_0 equals T of bj_cond_estimate_ex started at
+    v_0 = L^-1 r_0 (bj_solve_L) for the first steps, and a caller-supplied r_0 is honoured."""
+    A = mat(4, "small")
+    h, keep = B.setup_from_host(A, 16)
+    r0 = dev(torch_, W.seeded_vector(31, A.n))
+    g1 = B.bj_cond_estimate_minv(h, 8, r0=r0)
+    v0 = torch_.empty_like(r0)
+    B.bj_solve_L(h, r0, v0)
+    g2 = B.bj_cond_estimate_ex(h, 8, reorth=False, v0=v0)
+    sc = np.abs(g2["alpha"]).max()
+    assert np.abs(g1["alpha"] - g2["alpha"]).max() <= 1e-9 * sc and np.abs(g1["beta"] - g2["beta"]).max() <= 1e-9 * sc
+    c = oracle.Precond(A, 16).cond_estimate_minv(8, r0=r0.cpu().numpy())
+    assert np.abs(g1["alpha"] - c["alpha"]).max() <= 1e-9 * sc
+    B.bj_destroy(h)
+
+
+def test_minv_lanczos_degenerate_cases(B, torch_):
+    A = W.block_diagonal_spd(65, 8)     # M = A: M^-1 A = I, breakdown after one step, kappa = 1 (PAPER.md:80)
+    h, keep = B.setup_from_host(A, 8)
+    g = B.bj_cond_estimate_minv(h, 10)
+    assert g["iters_done"] == 1 and abs(g["alpha"][0] - 1) <= 1e-12 and abs(g["kappa"] - 1) <= 1e-12
+    z = torch_.zeros(A.n, dtype=torch_.float64, device="cuda")
+    with pytest.raises(B.BJError):
+        B.bj_cond_estimate_minv(h, 10, r0=z)
+    B.bj_destroy(h)
+
+
+def test_minv_lanczos_banded_factors(B, torch_, monkeypatch):
+    monkeypatch.setenv("BJ_BAND", "1")
+    A = mat(4, "small")
+    h, keep = B.setup_from_host(A, 16)
+    assert B.bj_get_info(h)["band_width"] >= 1
+    g = B.bj_cond_estimate_minv(h, 50)
+    c = oracle.Precond(A, 16).cond_estimate_minv(50)
+    assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
+    B.bj_destroy(h)
