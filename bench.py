@@ -487,6 +487,15 @@ def main():
             dt = time.perf_counter() - t0
             kap["fast_mode"] = {"kappa_est": r["kappa"], "iters": r["iters_done"], "seconds": dt,
                                 "lanczos_iters_per_s": r["iters_done"] / dt}
+            # the same spectrum from Lanczos on M^-1 A in the M inner product: one factor pass per step
+            r = B.bj_cond_estimate_minv(h, mf)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r = B.bj_cond_estimate_minv(h, mf)
+            dt = time.perf_counter() - t0
+            kap["minv_mode"] = {"kappa_est": r["kappa"], "iters": r["iters_done"], "seconds": dt,
+                                "lanczos_iters_per_s": r["iters_done"] / dt,
+                                "note": "start vector r_0 = seeded vector, i.e. v_0 = L^-1 r_0 in fast_mode's terms: same operator, another Krylov space"}
             # long runs (fast mode: the extreme Ritz values keep converging, ghosts only repeat them) so that
             # kappa(A) -> kappa(A^) is meaningful beyond the m-step lower bounds above (SURVEY 8(c) reading 13)
             ml = args.long_iters
@@ -498,6 +507,10 @@ def main():
                     r = B.bj_cond_estimate_ex(hh, ml, reorth=False)
                     long_run[name] = {"kappa_est": r["kappa"], "lmin": r["lmin"], "lmax": r["lmax"], "res_min": r["res_min"],
                                       "res_max": r["res_max"], "iters": r["iters_done"], "seconds": time.perf_counter() - t0}
+                t0 = time.perf_counter()
+                r = B.bj_cond_estimate_minv(h, ml)
+                long_run[f"bj{b}_minv"] = {"kappa_est": r["kappa"], "lmin": r["lmin"], "lmax": r["lmax"], "res_min": r["res_min"],
+                                           "res_max": r["res_max"], "iters": r["iters_done"], "seconds": time.perf_counter() - t0}
                 long_run["predicted_hhl_gain_kappa_sq"] = (long_run["A"]["kappa_est"] / long_run[f"bj{b}"]["kappa_est"]) ** 2
                 kap["long_run"] = long_run
                 B.bj_destroy(h0l)

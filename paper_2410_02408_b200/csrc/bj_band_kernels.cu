@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(128)
 solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ fac, const double* in, double* out,
                   const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg)
 {
-    __shared__ double lz_sh[4];
+    __shared__ double lz_sh[8];
     pdl_trigger();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool act = k < nblocks;
@@ -180,15 +180,18 @@ solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
     double acc = 0.0, acc2 = 0.0, beta = 0.0, inv_beta = 0.0;
     double rin[LZ == 3 ? BMAX : 1];
     if (LZ == 1) {
-        double alpha;
-        if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
-        if (act) {
+        double alpha, c[BMAX];
+        if (act) {  // operands first, the scalar (a dependent load) after them
             if (pro.first) {
                 load_rows_rt<BMAX>(pro.w0, lo, n, b, vec, v);
             } else {
-                double c[BMAX];
                 load_rows_rt<BMAX>(pro.w, lo, n, b, vec, v);
                 load_rows_rt<BMAX>(pro.vcur, lo, n, b, vec, c);
+            }
+        }
+        if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
+        if (act) {
+            if (!pro.first) {
 #pragma unroll
                 for (int i = 0; i < BMAX; ++i)
                     if (i < b) v[i] -= alpha * c[i];
@@ -199,16 +202,20 @@ solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
             store_rows_rt<BMAX>(pro.w, lo, n, b, vec, v);
         }
     } else if (LZ == 3) {
+        // vector operands are requested before the scalars are read (see solve_small_kernel)
+        double c[BMAX], xs[BMAX], pv[BMAX];
+        if (act) {
+            load_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
+            load_rows_rt<BMAX>(pcg.q, lo, n, b, vec, c);
+            load_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
+            if (!pcg.mode) load_rows_rt<BMAX>(pcg.p, lo, n, b, vec, pv);
+        }
         double a;
         if (pcg_hook_begin(pcg, a)) return;  // uniform over the grid
         if (pcg.mode) {  // three-term step of Lanczos on M^-1 A: r_{k+1} replaces r_{k-1} (uniform branch)
             double cq, cr, cx;
             mlz_hook_coeffs(pcg, cq, cr, cx);
             if (act) {
-                double c[BMAX], xs[BMAX];
-                load_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
-                load_rows_rt<BMAX>(pcg.q, lo, n, b, vec, c);
-                load_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
 #pragma unroll
                 for (int i = 0; i < BMAX; ++i) {
                     if (i < b) {
@@ -219,29 +226,21 @@ solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
                 store_rows_rt<BMAX>(pcg.x, lo, n, b, vec, v);
             }
         } else if (act) {
-            double c[BMAX];
-            load_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
-            load_rows_rt<BMAX>(pcg.q, lo, n, b, vec, c);
 #pragma unroll
             for (int i = 0; i < BMAX; ++i) {
                 if (i < b) {
                     v[i] = v[i] - a * c[i];
                     if (lo + i < n) acc = fma(v[i], v[i], acc);
                     rin[i] = v[i];
+                    xs[i] = fma(a, pv[i], xs[i]);
                 }
             }
             store_rows_rt<BMAX>(pcg.r, lo, n, b, vec, v);
-            double xs[BMAX];
-            load_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
-            load_rows_rt<BMAX>(pcg.p, lo, n, b, vec, c);
-#pragma unroll
-            for (int i = 0; i < BMAX; ++i)
-                if (i < b) xs[i] = fma(a, c[i], xs[i]);
             store_rows_rt<BMAX>(pcg.x, lo, n, b, vec, xs);
         }
     } else {
+        load_rows_rt<BMAX>(in, lo, n, b, vec, v);                       // before the scalars: independent of them
         if (LZ == 2 && lz_epilogue_begin(epi, beta, inv_beta)) return;  // uniform over the grid
-        load_rows_rt<BMAX>(in, lo, n, b, vec, v);
     }
     if (DIR == 0 || DIR == 2) {
 #pragma unroll
@@ -294,9 +293,7 @@ solve_band_kernel(int64_t n, int b, int64_t nblocks, const double* __restrict__ 
                 for (int i = 0; i < BMAX; ++i)
                     if (i < b && lo + i < n) acc2 = fma(rin[i], v[i], acc2);
             }
-            lz_reduce_finish(pcg.red_rr, acc, lz_sh);
-            __syncthreads();
-            lz_reduce_finish(pcg.red_rz, acc2, lz_sh);
+            lz_reduce_finish2(pcg.red_rr, acc, pcg.red_rz, acc2, lz_sh);  // one ticket for both sums
         }
     }
 }

@@ -149,4 +149,50 @@ __device__ __forceinline__ void lz_reduce_finish(const LzReduce& r, double p, do
     }
 }
 
+// Two reductions of one kernel closed by ONE ticket (one fence, one atomic, one round of barriers): ra's ticket and cap serve
+// both; rb.part / rb.out receive the second sum.  Same fixed order of additions as two calls of lz_reduce_finish.
+// sh: at least 2 * blockDim.x / 32 doubles.
+__device__ __forceinline__ void lz_reduce_finish2(const LzReduce& ra, double pa, const LzReduce& rb, double pb, double* sh)
+{
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        pa += __shfl_down_sync(0xffffffffu, pa, off);
+        pb += __shfl_down_sync(0xffffffffu, pb, off);
+    }
+    __syncthreads();
+    if (lane == 0) { sh[warp] = pa; sh[nw + warp] = pb; }
+    __syncthreads();
+    __shared__ int is_last2;
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int q = 0; q < nw; ++q) { a += sh[q]; b += sh[nw + q]; }
+        ra.part[blockIdx.x] = a;
+        rb.part[blockIdx.x] = b;
+        __threadfence();
+        const unsigned t = atomicAdd(ra.ticket, 1u);
+        is_last2 = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last2) return;
+    __threadfence();
+    double a = 0.0, b = 0.0;
+    for (unsigned q = threadIdx.x; q < gridDim.x; q += blockDim.x) { a += __ldcg(ra.part + q); b += __ldcg(rb.part + q); }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, off);
+        b += __shfl_down_sync(0xffffffffu, b, off);
+    }
+    __syncthreads();
+    if (lane == 0) { sh[warp] = a; sh[nw + warp] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double sa = 0.0, sb = 0.0;
+        for (int q = 0; q < nw; ++q) { sa += sh[q]; sb += sh[nw + q]; }
+        *ra.out = sa;
+        *rb.out = sb;
+        *ra.ticket = 0u;
+    }
+}
+
 }  // namespace bj

@@ -67,14 +67,18 @@ __device__ __forceinline__ void store_rows(double* dst, int64_t lo, int64_t n, b
 // LZ: 0 plain, 1 Lanczos prologue (DIR 1: the input is w built on the fly), 2 Lanczos epilogue (DIR 0),
 //     3 PCG update + apply (DIR 2: x += a p, r -= a q on the fly, z = M^-1 r, partials of r.r and r.z)
 //     TRI: tridiagonal blocks, compact bidiagonal factor of 2B - 1 elements, element (i, j) at slot i + j
+#ifndef BJ_SMALL_HOOK_MINB
+#define BJ_SMALL_HOOK_MINB 4
+#endif
+#define SMALL_MINB ((LZ == 3 && B >= 7 && !TRI) ? BJ_SMALL_HOOK_MINB : 1)
 template <int B, int DIR, bool VEC, int LZ, bool TRI>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, SMALL_MINB)
 solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                    const double* in, double* out,  // in == out allowed: a thread touches only its own block
                    const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg)
 {
     constexpr int P = TRI ? 2 * B - 1 : B * (B + 1) / 2;
-    __shared__ double lz_sh[4];
+    __shared__ double lz_sh[8];
     pdl_trigger();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool act = k < nblocks;
@@ -92,15 +96,18 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
     double rin[LZ == 3 ? B : 1];                   // PCG: the residual rows, kept for r.z
     double acc2 = 0.0;
     if (LZ == 1) {
-        double alpha;
-        if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
-        if (act) {
+        double alpha, c[B];
+        if (act) {  // operands first, the scalar (a dependent load) after them
             if (pro.first) {
                 load_rows<B, VEC>(pro.w0, lo, n, whole, v);
             } else {
-                double c[B];
                 load_rows<B, VEC>(pro.w, lo, n, whole, v);
                 load_rows<B, VEC>(pro.vcur, lo, n, whole, c);
+            }
+        }
+        if (lz_prologue_begin(pro, alpha)) return;  // uniform over the grid
+        if (act) {
+            if (!pro.first) {
 #pragma unroll
                 for (int i = 0; i < B; ++i) v[i] -= alpha * c[i];
             }
@@ -109,16 +116,21 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
             store_rows<B, VEC>(pro.w, lo, n, whole, v);
         }
     } else if (LZ == 3) {
+        // every vector operand is requested BEFORE the scalars are read: the step length / the three coefficients hang on
+        // a dependent load plus a division and a square root, and the loads do not depend on them
+        double c[B], xs[B], pv[B];
+        if (act) {
+            load_rows<B, VEC>(pcg.r, lo, n, whole, v);
+            load_rows<B, VEC>(pcg.q, lo, n, whole, c);
+            load_rows<B, VEC>(pcg.x, lo, n, whole, xs);
+            if (!pcg.mode) load_rows<B, VEC>(pcg.p, lo, n, whole, pv);
+        }
         double a;
         if (pcg_hook_begin(pcg, a)) return;  // uniform over the grid
         if (pcg.mode) {  // three-term step of Lanczos on M^-1 A: r_{k+1} replaces r_{k-1} (uniform branch)
             double cq, cr, cx;
             mlz_hook_coeffs(pcg, cq, cr, cx);
             if (act) {
-                double c[B], xs[B];
-                load_rows<B, VEC>(pcg.r, lo, n, whole, v);
-                load_rows<B, VEC>(pcg.q, lo, n, whole, c);
-                load_rows<B, VEC>(pcg.x, lo, n, whole, xs);
 #pragma unroll
                 for (int i = 0; i < B; ++i) {
                     v[i] = mlz_combine(cq, cr, cx, c[i], v[i], xs[i]);
@@ -127,26 +139,19 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                 store_rows<B, VEC>(pcg.x, lo, n, whole, v);
             }
         } else if (act) {
-            double c[B];
-            load_rows<B, VEC>(pcg.r, lo, n, whole, v);
-            load_rows<B, VEC>(pcg.q, lo, n, whole, c);
 #pragma unroll
             for (int i = 0; i < B; ++i) {
                 v[i] = v[i] - a * c[i];             // r_new
                 acc = fma(v[i], v[i], acc);
                 rin[i] = v[i];
+                xs[i] = fma(a, pv[i], xs[i]);
             }
             store_rows<B, VEC>(pcg.r, lo, n, whole, v);
-            double xs[B];
-            load_rows<B, VEC>(pcg.x, lo, n, whole, xs);
-            load_rows<B, VEC>(pcg.p, lo, n, whole, c);
-#pragma unroll
-            for (int i = 0; i < B; ++i) xs[i] = fma(a, c[i], xs[i]);
             store_rows<B, VEC>(pcg.x, lo, n, whole, xs);
         }
     } else {
+        load_rows<B, VEC>(in, lo, n, whole, v);                         // before the scalars: independent of them
         if (LZ == 2 && lz_epilogue_begin(epi, beta, inv_beta)) return;  // uniform over the grid
-        load_rows<B, VEC>(in, lo, n, whole, v);
     }
     if (DIR == 0 || DIR == 2) {
 #pragma unroll
@@ -200,9 +205,7 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
 #pragma unroll
                 for (int i = 0; i < B; ++i) acc2 = fma(rin[i], v[i], acc2);
             }
-            lz_reduce_finish(pcg.red_rr, acc, lz_sh);
-            __syncthreads();
-            lz_reduce_finish(pcg.red_rz, acc2, lz_sh);
+            lz_reduce_finish2(pcg.red_rr, acc, pcg.red_rz, acc2, lz_sh);  // one ticket for both sums
         }
     }
 }
@@ -410,7 +413,7 @@ solve_group_kernel(const GroupParams p)
 
     const int g = lane / LPB, l = lane % LPB;
     pdl_wait();  // `in` may come from the previous kernel
-    __shared__ double lz_sh[12];
+    __shared__ double lz_sh[24];
     double alpha = 0.0, beta = 0.0, inv_beta = 0.0, acc = 0.0;  // Lanczos scalars and this thread's dot product
     bool stop = false;
     if (DIR == 1 && LZ == 1) stop = lz_prologue_begin(p.pro, alpha);
@@ -534,9 +537,7 @@ solve_group_kernel(const GroupParams p)
     if (DIR == 1 && LZ == 1) lz_reduce_finish(p.pro.red, acc, lz_sh);
     if (DIR == 0 && LZ == 2) lz_reduce_finish(p.epi.red, acc, lz_sh);
     if (DIR == 2 && LZ == 3) {
-        lz_reduce_finish(p.pcg.red_rr, acc, lz_sh);
-        __syncthreads();
-        lz_reduce_finish(p.pcg.red_rz, acc2, lz_sh);
+        lz_reduce_finish2(p.pcg.red_rr, acc, p.pcg.red_rz, acc2, lz_sh);  // one ticket for both sums
     }
 }
 
