@@ -240,3 +240,85 @@ def tridiag_all(alpha, beta) -> np.ndarray:
     out = np.empty(len(alpha))
     _load().orc_tridiag_all(len(alpha), _p(alpha), _p(beta), _p(out))
     return out
+
+
+class PrecondBlocks:
+    """Block-Jacobi with diagonal blocks of DIFFERENT sizes ("variable-size / supervariable blocks").
+    block_ptr[0..nblocks] (0 = p_0 < p_1 < .. = n) delimits contiguous index ranges; block k is the dense diagonal slice
+    D_k = A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:254-263 with a per-block size), factored D_k = L_k L_k^T and
+    solved block by block -- every step is the uniform-size routine of bj_oracle.c called on ONE block (n = b = s_k), so
+    the arithmetic and its order are exactly those of Precond.  Slow (a Python loop over blocks): small cases only."""
+
+    def __init__(self, A, block_ptr):
+        self.A, self.n = A, A.n
+        p = np.asarray(block_ptr, dtype=np.int64)
+        if p[0] != 0 or p[-1] != A.n or np.any(np.diff(p) <= 0):
+            raise ValueError("block_ptr must increase strictly from 0 to n")
+        self.ptr = p
+        rp, ci, val = A.row_ptr, A.col_idx, A.val
+        self.L = []
+        for k in range(len(p) - 1):
+            lo, hi = int(p[k]), int(p[k + 1])
+            D = np.zeros((hi - lo, hi - lo))
+            for i in range(lo, hi):
+                for e in range(int(rp[i]), int(rp[i + 1])):
+                    c = int(ci[e])
+                    if lo <= c < hi:
+                        D[i - lo, c - lo] = val[e]
+            try:
+                self.L.append(factor(hi - lo, hi - lo, D.reshape(1, hi - lo, hi - lo)))
+            except NotSPD:
+                raise NotSPD(k)
+
+    def _blockwise(self, fn, v):
+        v = _f64(v); out = np.empty(self.n)
+        for k, L in enumerate(self.L):
+            lo, hi = int(self.ptr[k]), int(self.ptr[k + 1])
+            seg = np.ascontiguousarray(v[lo:hi]); res = np.empty(hi - lo)
+            fn(hi - lo, hi - lo, _p(L), _p(seg), _p(res))
+            out[lo:hi] = res
+        return out
+
+    def solve_L(self, r):
+        return self._blockwise(_load().orc_solve_L, r)
+
+    def solve_Lt(self, y):
+        return self._blockwise(_load().orc_solve_Lt, y)
+
+    def apply(self, r):
+        return self.solve_Lt(self.solve_L(r))
+
+    def op_apply(self, x):
+        return self.solve_L(spmv(self.A, self.solve_Lt(x)))
+
+    def lanczos(self, m: int, v0=None, reorth: bool = True, seed: int = DEFAULT_SEED, tol_bd: float = TOL_BREAKDOWN):
+        """The recurrence of orc_lanczos (bj_oracle.c), statement by statement, on this operator."""
+        v0 = seeded_vector(seed, self.n) if v0 is None else _f64(v0)
+        V = [v0 / np.sqrt(np.dot(v0, v0))]
+        alpha, beta = [], []
+        beta_j, amax = 0.0, 0.0
+        for j in range(m):
+            w = self.op_apply(V[j])
+            if j > 0:
+                w = w - beta_j * V[j - 1]
+            a = float(np.dot(V[j], w))
+            w = w - a * V[j]
+            if reorth:
+                for _ in range(2):
+                    c = [float(np.dot(V[q], w)) for q in range(j + 1)]
+                    for q in range(j + 1):
+                        w = w - c[q] * V[q]
+            bn = float(np.sqrt(np.dot(w, w)))
+            alpha.append(a); beta.append(bn)
+            amax = max(amax, abs(a))
+            if not (bn > tol_bd * amax):
+                break
+            V.append(w / bn)
+            beta_j = bn
+        return np.array(alpha), np.array(beta)
+
+    def cond_estimate(self, m: int, **kw):
+        alpha, beta = self.lanczos(m, **kw)
+        tmin, tmax, rmin, rmax = tridiag_extremes(alpha, beta)
+        return {"lmin": tmin, "lmax": tmax, "kappa": tmax / tmin, "res_min": rmin, "res_max": rmax,
+                "iters_done": len(alpha), "alpha": alpha, "beta": beta}

@@ -423,3 +423,28 @@ def batch_member(A: CSR, s: int) -> CSR:
     p0, p1 = int(A.row_ptr[r0]), int(A.row_ptr[r1])
     return CSR(r1 - r0, (A.row_ptr[r0:r1 + 1] - p0).astype(np.int32), (A.col_idx[p0:p1] - r0).astype(np.int32),
                A.val[p0:p1].copy(), {"kind": "batch_member", "s": s})
+
+
+def random_block_ptr(n: int, seed: int = SEED, smin: int = 1, smax: int = 32) -> np.ndarray:
+    """Variable-size Jacobi blocks (NEXT-3): consecutive sizes drawn from the seeded integer mixer, uniform in
+    [smin, smax], the last block cut at n.  int64 array p with p[0] = 0 < p[1] < .. < p[-1] = n."""
+    cnt = n // smin + 1
+    sizes = smin + (mix64(seed, np.arange(cnt, dtype=np.uint64)) % np.uint64(smax - smin + 1)).astype(np.int64)
+    ends = np.cumsum(sizes)
+    k = int(np.searchsorted(ends, n))          # first block whose end reaches n
+    ends = ends[:k + 1].copy()
+    ends[k] = n
+    return np.concatenate([[0], ends]).astype(np.int64)
+
+
+def direct_sum_spd(sizes, seed: int = SEED) -> CSR:
+    """Block-diagonal SPD matrix whose dense diagonal blocks have the given (different) sizes: the model M = A of
+    PAPER.md:76-82 for variable-size blocks.  Block k = G G^T / s + I with G drawn from the config-independent rng."""
+    import scipy.sparse as sp
+    rng = np.random.default_rng(seed + 77)
+    blocks = []
+    for s in sizes:
+        G = rng.standard_normal((s, s))
+        blocks.append(G @ G.T / s + np.eye(s))
+    import scipy.linalg as sla
+    return from_scipy(sp.csr_matrix(sla.block_diag(*blocks)), {"name": "direct_sum_spd", "sizes": list(map(int, sizes))})

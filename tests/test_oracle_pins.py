@@ -616,3 +616,58 @@ def test_minv_lanczos_special_cases():
     d, e = oracle.cg_tridiag(pc["alpha"], pc["beta"])
     a6, b6 = P1.lanczos_minv(6, r0=r0)
     assert np.abs(d - a6).max() < 1e-9 * np.abs(a6).max() and np.abs(e - b6[:5]).max() < 1e-9 * np.abs(a6).max()
+
+
+# ---------------------------------------------------------------- variable-size blocks (NEXT-3) ------
+def test_variable_blocks_with_equal_sizes_are_the_uniform_preconditioner():
+    A = W.build(2, "tiny")
+    for b in (3, 8, 16):
+        ptr = np.minimum(np.arange(0, A.n + b, b), A.n)
+        ptr = np.unique(ptr)
+        Pv, Pu = oracle.PrecondBlocks(A, ptr), oracle.Precond(A, b)
+        x = W.seeded_vector(3, A.n)
+        for f in ("solve_L", "solve_Lt", "apply", "op_apply"):
+            assert np.array_equal(getattr(Pv, f)(x), getattr(Pu, f)(x)), (b, f)
+        av, bv = Pv.lanczos(12, reorth=True)
+        au, bu = Pu.lanczos(12, reorth=True)
+        assert np.abs(av - au).max() < 1e-12 * np.abs(au).max() and np.abs(bv - bu).max() < 1e-12 * np.abs(au).max()
+
+
+@pytest.mark.parametrize("cfg", [1, 3, 4, 5])
+def test_variable_blocks_match_dense_numpy(cfg, rel):
+    """Independent restatement: per block np.linalg.solve / np.linalg.cholesky on dense slices."""
+    A = W.build(cfg, "tiny")
+    ptr = W.random_block_ptr(A.n, seed=cfg, smin=1, smax=32)
+    assert ptr[0] == 0 and ptr[-1] == A.n and np.diff(ptr).min() >= 1 and np.diff(ptr).max() <= 32
+    assert len(set(np.diff(ptr)[:-1].tolist())) > 3          # sizes really differ
+    P = oracle.PrecondBlocks(A, ptr)
+    Ad = A.to_dense()
+    x = W.seeded_vector(11, A.n)
+    z_ref = np.empty(A.n)
+    Linv = np.zeros((A.n, A.n))
+    for lo, hi in zip(ptr[:-1], ptr[1:]):
+        z_ref[lo:hi] = np.linalg.solve(Ad[lo:hi, lo:hi], x[lo:hi])
+        Lk = np.linalg.cholesky(Ad[lo:hi, lo:hi])
+        Linv[lo:hi, lo:hi] = sla.solve_triangular(Lk, np.eye(hi - lo), lower=True)
+    assert rel(P.apply(x), z_ref)[0] < 1e-10
+    assert rel(P.solve_L(x), Linv @ x)[0] < 1e-11 and rel(P.solve_Lt(x), Linv.T @ x)[0] < 1e-11
+    Mop = Linv @ Ad @ Linv.T
+    assert rel(P.op_apply(x), Mop @ x)[0] < 1e-11
+    ev = np.linalg.eigvalsh(0.5 * (Mop + Mop.T))
+    r = P.cond_estimate(min(A.n, 40), reorth=True)
+    assert r["lmin"] >= ev[0] - 1e-10 and r["lmax"] <= ev[-1] + 1e-10          # interlacing
+    assert np.abs(ev - r["lmin"]).min() <= r["res_min"] + 1e-10 and np.abs(ev - r["lmax"]).min() <= r["res_max"] + 1e-10
+
+
+def test_variable_blocks_equal_to_the_matrix_blocks_give_identity():
+    """M = A with blocks of different sizes: A^ = I, Lanczos breaks down after one step."""
+    sizes = [5, 1, 32, 7, 16, 2, 24]
+    A = W.direct_sum_spd(sizes)
+    ptr = np.concatenate([[0], np.cumsum(sizes)])
+    P = oracle.PrecondBlocks(A, ptr)
+    x = W.seeded_vector(2, A.n)
+    assert np.abs(P.op_apply(x) - x).max() < 1e-13
+    r = P.cond_estimate(10)
+    assert r["iters_done"] == 1 and abs(r["kappa"] - 1) < 1e-12
+    with pytest.raises(ValueError):
+        oracle.PrecondBlocks(A, [0, 5, 5, A.n])
