@@ -147,6 +147,14 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
  * bj_setup (block-size sweeps); this returns the cache to the driver.  Synchronises the device. */
 int bj_release_cached_memory(void);
 
+/* diagonal blocks of DIFFERENT sizes (supervariable blocks).  block_ptr_host[0..nblocks] (host, int64):
+ * 0 = p_0 < p_1 < .. < p_nblocks = n, every size p_{k+1} - p_k in 1..BJ_B_MAX; block k is the dense diagonal slice
+ * A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:254-263 with a per-block size).  The array is read during the call
+ * only.  Every other entry point works on the handle unchanged (bj_apply, bj_solve_L/Lt, bj_op_apply, bj_cond_estimate*,
+ * bj_pcg_solve; the Lanczos / PCG iterations run unfused); the batch entry points return BJ_ERR_INVALID_ARG.  One warp per
+ * block (lane = row), packed lower triangles back to back.  bj_get_info reports b = -1, solve_kernel = 4.  Errors as
+ * bj_setup; a layout that breaks the rules above is BJ_ERR_INVALID_ARG.  Synchronises. */
+int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out);
 int bj_set_stream(bj_handle_t h, void* cuda_stream);
 int bj_set_option(bj_handle_t h, int option, int value);
 int bj_destroy(bj_handle_t h);

@@ -23,7 +23,7 @@ EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_set_stream", "bj_set_option", "
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
            "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve",
-           "bj_probe_gather_stream", "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv"]
+           "bj_probe_gather_stream", "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv", "bj_setup_blocks"]
 
 
 class bj_csr_t(C.Structure):
@@ -150,6 +150,26 @@ def bj_setup(row_ptr, col_idx, val, b: int, stream=None) -> Handle:
     st = (stream or torch.cuda.current_stream()).cuda_stream
     out = C.c_void_p()
     code = lib().bj_setup_on_stream(C.byref(csr), int(b), C.c_void_p(st), C.byref(out))
+    if code == BJ_ERR_NOT_SPD and out.value:
+        info = bj_info_t()
+        lib().bj_get_info(out, C.byref(info))
+        lib().bj_destroy(out)
+        _check(code, int(info.bad_block))
+    _check(code)
+    return Handle(out, (row_ptr, col_idx, val), n)
+
+
+def bj_setup_blocks(row_ptr, col_idx, val, block_ptr, stream=None) -> Handle:
+    """Variable-size diagonal blocks: block_ptr = host int64 sequence 0 = p_0 < .. < p_nblocks = n, sizes 1..32."""
+    import numpy as np
+    import torch
+    n = row_ptr.numel() - 1
+    nnz = val.numel()
+    ptr = np.ascontiguousarray(np.asarray(block_ptr, dtype=np.int64))
+    csr = bj_csr_t(n, nnz, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32, nnz), _dptr(val, torch.float64))
+    st = (stream or torch.cuda.current_stream()).cuda_stream
+    out = C.c_void_p()
+    code = lib().bj_setup_blocks(C.byref(csr), ptr.ctypes.data_as(C.c_void_p), C.c_int64(len(ptr) - 1), C.c_void_p(st), C.byref(out))
     if code == BJ_ERR_NOT_SPD and out.value:
         info = bj_info_t()
         lib().bj_get_info(out, C.byref(info))

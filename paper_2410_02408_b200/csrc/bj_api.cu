@@ -151,6 +151,7 @@ static void free_handle(bj_handle_s* h)
         if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
         else cudaFree(h->slab);
     }
+    var_free(h);
     cudaFree(h->stage_in); cudaFree(h->stage_out);
     for (auto& s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
     for (auto e : h->event_pool) cudaEventDestroy(e);
@@ -364,6 +365,25 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
 
 int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out) { return bj_setup_on_stream(csr, b, nullptr, out); }
 
+int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out)
+{
+    if (!out) return BJ_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!csr || !block_ptr_host || nblocks < 1 || nblocks > csr->n) return BJ_ERR_INVALID_ARG;
+    if (block_ptr_host[0] != 0 || block_ptr_host[nblocks] != csr->n) return BJ_ERR_INVALID_ARG;
+    for (int64_t k = 0; k < nblocks; ++k) {
+        const int64_t s = block_ptr_host[k + 1] - block_ptr_host[k];
+        if (s < 1 || s > BJ_B_MAX) return BJ_ERR_INVALID_ARG;
+    }
+    bj_handle_t h = nullptr;
+    int rc = bj_setup_on_stream(csr, 0, cuda_stream, &h);  // validation and the SpMV plan of a b = 0 handle
+    if (rc != BJ_OK) return rc;
+    rc = var_setup(h, block_ptr_host, nblocks);
+    if (rc != BJ_OK && rc != BJ_ERR_NOT_SPD) { free_handle(h); return rc; }
+    *out = h;  // after BJ_ERR_NOT_SPD the handle only answers bj_get_info / bj_destroy, like bj_setup
+    return rc;
+}
+
 int bj_release_cached_memory(void)
 {
     int dev = 0;
@@ -411,14 +431,14 @@ int bj_get_info(bj_handle_t h, bj_info_t* info)
 {
     if (!h || !info) return BJ_ERR_INVALID_ARG;
     memset(info, 0, sizeof(*info));
-    info->n = h->n; info->nnz = h->nnz; info->b = h->b; info->nblocks = h->nblocks;
+    info->n = h->n; info->nnz = h->nnz; info->b = h->solve_kind == 4 ? -1 : h->b; info->nblocks = h->nblocks;
     info->bad_block = h->bad_block;
     info->factor_bytes = h->factor_bytes;
     info->workspace_bytes = h->workspace_bytes;
     info->kernel_launches = h->launches;
     info->spmv_kernel = h->spmv_kernel;
     info->spmv_lanes = h->spmv_lanes;
-    info->solve_kernel = h->solve_kind;
+    info->solve_kernel = h->solve_kind == 4 ? 4 : h->solve_kind;
     info->band_width = (h->solve_kind == 3 || h->tri) ? h->band : -1;
     info->col16 = h->col16 ? 1 : 0;
     info->fused_forward = (h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0 && h->solve_kind != 0) ? 1 : 0;

@@ -83,7 +83,11 @@ struct bj_handle_s {
     int64_t bad_block = -1;
 
     // factors
-    int solve_kind = 0;  // 0 none, 1 small (interleaved), 2 warp (fwd + bwd packed copies), 3 banded (interleaved band)
+    int solve_kind = 0;  // 0 none, 1 small (interleaved), 2 warp (fwd + bwd packed copies), 3 banded (interleaved band), 4 variable-size blocks
+    int32_t* var_bptr = nullptr;  // kind 4: block pointers (nblocks + 1), factor offsets (nblocks + 1), packed factors
+    int64_t* var_foff = nullptr;
+    double* var_fac = nullptr;
+    int var_smax = 0;
     int band = -1;       // kind 3: lower bandwidth w of every diagonal block (0..2)
     double* fac_band = nullptr;  // kind 3: aliases the dense factor storage of the slab
     bool tri = false;    // kind 1 with BJ_BAND=1: every block is (at most) tridiagonal, compact bidiagonal factors, packed = 2b - 1
@@ -230,6 +234,10 @@ void lanczos_fill_result(int me, const double* a, const double* b, bj_lanczos_re
 int mlanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res);
 
 // preconditioned CG (bj_pcg.cu)
+// variable-size blocks (bj_var_kernels.cu)
+int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks);
+void var_free(bj_handle_s* h);
+int launch_solve_var(bj_handle_s* h, int dir, const double* in, double* out);
 int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* r);
 void pcg_free(bj_handle_s* h);
 void batch_free(bj_handle_s* h);

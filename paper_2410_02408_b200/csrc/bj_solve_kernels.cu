@@ -865,7 +865,9 @@ int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const L
     const int kind = dir == 0 ? BJ_K_SOLVE_L : (dir == 1 ? BJ_K_SOLVE_LT : BJ_K_APPLY);
     {
         KernelScope scope(h, kind);
-        if (h->solve_kind == 3) {
+        if (h->solve_kind == 4) {
+            rc = launch_solve_var(h, dir, in, out);
+        } else if (h->solve_kind == 3) {
             rc = launch_solve_band(h, dir, in, out, pro, epi, pcg);
         } else if (h->solve_kind == 1) {
             rc = dir == 0   ? (epi ? launch_small<0, 2>(h, in, out, nullptr, epi) : launch_small<0, 0>(h, in, out, nullptr, nullptr))

@@ -1,0 +1,198 @@
+// Variable-size Jacobi blocks ("variable-size / supervariable blocks").
+// block_ptr[0..nblocks] delimits contiguous index ranges of 1..32 rows; block k is the dense diagonal slice
+// D_k = A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:254-263 with a per-block size), D_k = L_k L_k^T.
+// Storage: the lower triangles, column-major packed, back to back: block k starts at foff[k] = sum_{q<k} s_q (s_q+1)/2,
+// element (i, j), i >= j, at j s - j (j-1)/2 + (i - j); the diagonal slot holds 1 / l_jj.
+// One warp per block in both kernels (lane = row): the block sizes differ, so neither the 32-block interleave of the
+// b <= 8 kernels nor the fixed tile geometry of the group kernel applies; the packed factor of a block is one
+// contiguous range that the warp copies to shared memory with coalesced loads before the substitutions.
+#include <algorithm>
+#include <vector>
+
+#include "bj_device.cuh"
+#include "bj_internal.cuh"
+
+namespace bj {
+
+namespace {
+
+constexpr int kVarWarps = 4;
+constexpr int kVarMax = 32;
+constexpr int kVarPacked = kVarMax * (kVarMax + 1) / 2;  // 528
+
+__device__ __forceinline__ int var_col_start(int j, int s) { return j * s - (j * (j - 1)) / 2; }
+
+// a2-a4 for one block per warp: dense lower triangle out of the CSR rows, Cholesky (left-looking, column by column,
+// each sum in increasing k like the oracle's chol_block), packed store.  A non-positive or non-finite pivot flags
+// ST_NOT_SPD and records the smallest such block.
+__global__ void __launch_bounds__(kVarWarps * 32)
+extract_factor_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_t* __restrict__ foff,
+                          const int32_t* __restrict__ rp, const int32_t* __restrict__ ci, const double* __restrict__ val,
+                          double* __restrict__ fac, Status* __restrict__ status)
+{
+    __shared__ double Dsh[kVarWarps][kVarMax * (kVarMax + 1)];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t k = (int64_t)blockIdx.x * kVarWarps + warp;
+    if (k >= nblocks) return;
+    const int lo = bptr[k], s = bptr[k + 1] - lo;
+    double* D = Dsh[warp];  // row i at D + i * 33
+    if (lane < s) {
+        for (int j = 0; j < s; ++j) D[lane * (kVarMax + 1) + j] = 0.0;
+        const int row = lo + lane;
+        for (int e = rp[row]; e < rp[row + 1]; ++e) {
+            const int c = ci[e] - lo;
+            if (c >= 0 && c <= lane) D[lane * (kVarMax + 1) + c] = val[e];  // lower triangle only
+        }
+    }
+    __syncwarp();
+    bool bad = false;
+    for (int j = 0; j < s; ++j) {
+        double sum = 0.0;
+        if (lane >= j && lane < s) {
+            sum = D[lane * (kVarMax + 1) + j];
+            for (int q = 0; q < j; ++q) sum -= D[lane * (kVarMax + 1) + q] * D[j * (kVarMax + 1) + q];
+        }
+        const double piv = __shfl_sync(0xffffffffu, sum, j);
+        if (!(piv > 0.0) || !isfinite(piv)) { bad = true; break; }  // uniform over the warp
+        const double d = sqrt(piv);
+        __syncwarp();
+        if (lane == j) D[lane * (kVarMax + 1) + j] = d;
+        else if (lane > j && lane < s) D[lane * (kVarMax + 1) + j] = sum / d;
+        __syncwarp();
+    }
+    if (bad) {
+        if (lane == 0) {
+            atomicOr(&status->flags, ST_NOT_SPD);
+            atomicMin(&status->bad_block, (long long)k);
+        }
+        return;
+    }
+    double* f = fac + foff[k];
+    const int P = s * (s + 1) / 2;
+    // packed index e -> (i, j): walk the columns; each lane converts its own indices
+    for (int e = lane; e < P; e += 32) {
+        int j = 0, start = 0;
+        while (start + (s - j) <= e) { start += s - j; ++j; }
+        const int i = j + (e - start);
+        const double v = D[i * (kVarMax + 1) + j];
+        f[e] = (i == j) ? 1.0 / v : v;
+    }
+}
+
+// DIR 0: y = L^-1 r, 1: x = L^-T y, 2: z = L^-T L^-1 r.  One warp per block, lane = row, factor in shared memory.
+template <int DIR>
+__global__ void __launch_bounds__(kVarWarps * 32)
+solve_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_t* __restrict__ foff,
+                 const double* __restrict__ fac, const double* in, double* out)
+{
+    __shared__ double Fsh[kVarWarps][kVarPacked];
+    pdl_trigger();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t k = (int64_t)blockIdx.x * kVarWarps + warp;
+    if (k >= nblocks) return;
+    const int lo = bptr[k], s = bptr[k + 1] - lo;
+    const double* f = fac + foff[k];
+    double* F = Fsh[warp];
+    const int P = s * (s + 1) / 2;
+    for (int e = lane; e < P; e += 32) F[e] = ld_stream(f + e);  // factors never change after setup
+    pdl_wait();                                                  // `in` may come from the previous kernel
+    double v = lane < s ? in[lo + lane] : 0.0;
+    __syncwarp();
+    if (DIR == 0 || DIR == 2) {
+        for (int j = 0; j < s; ++j) {
+            const int cs = var_col_start(j, s);
+            if (lane == j) v *= F[cs];
+            const double yj = __shfl_sync(0xffffffffu, v, j);
+            if (lane > j && lane < s) v -= F[cs + (lane - j)] * yj;
+        }
+    }
+    if (DIR == 1 || DIR == 2) {
+        for (int j = s - 1; j >= 0; --j) {
+            if (lane == j) v *= F[var_col_start(j, s)];
+            const double xj = __shfl_sync(0xffffffffu, v, j);
+            if (lane < j) v -= F[var_col_start(lane, s) + (j - lane)] * xj;  // l_{j,lane}
+        }
+    }
+    if (lane < s) out[lo + lane] = v;
+}
+
+}  // namespace
+
+void var_free(bj_handle_s* h)
+{
+    if (h->var_fac) h->factor_bytes = 0;
+    cudaFree(h->var_bptr);
+    cudaFree(h->var_foff);
+    cudaFree(h->var_fac);
+    h->var_bptr = nullptr;
+    h->var_foff = nullptr;
+    h->var_fac = nullptr;
+}
+
+// Turns a b = 0 handle (validated matrix, SpMV plan) into a variable-block handle: uploads the block layout, extracts
+// and factors every block.  ptr_host was validated by the caller.
+int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks)
+{
+    std::vector<int32_t> bp((size_t)nblocks + 1);
+    std::vector<int64_t> fo((size_t)nblocks + 1);
+    int64_t off = 0;
+    int smax = 0;
+    for (int64_t k = 0; k < nblocks; ++k) {
+        const int64_t s = ptr_host[k + 1] - ptr_host[k];
+        bp[k] = (int32_t)ptr_host[k];
+        fo[k] = off;
+        off += s * (s + 1) / 2;
+        smax = std::max<int>(smax, (int)s);
+    }
+    bp[nblocks] = (int32_t)ptr_host[nblocks];
+    fo[nblocks] = off;
+    if (cudaMalloc((void**)&h->var_bptr, sizeof(int32_t) * bp.size()) != cudaSuccess ||
+        cudaMalloc((void**)&h->var_foff, sizeof(int64_t) * fo.size()) != cudaSuccess ||
+        cudaMalloc((void**)&h->var_fac, sizeof(double) * (size_t)off) != cudaSuccess) {
+        cudaGetLastError();
+        var_free(h);
+        return BJ_ERR_ALLOC;
+    }
+    cudaStream_t st = h->stream;
+    BJ_CUDA(cudaMemcpyAsync(h->var_bptr, bp.data(), sizeof(int32_t) * bp.size(), cudaMemcpyHostToDevice, st));
+    BJ_CUDA(cudaMemcpyAsync(h->var_foff, fo.data(), sizeof(int64_t) * fo.size(), cudaMemcpyHostToDevice, st));
+    h->nblocks = nblocks;
+    h->var_smax = smax;
+    h->solve_kind = 4;
+    h->factor_bytes = (int64_t)sizeof(double) * off + (int64_t)(sizeof(int32_t) * bp.size() + sizeof(int64_t) * fo.size());
+    const unsigned grid = (unsigned)((nblocks + kVarWarps - 1) / kVarWarps);
+    extract_factor_var_kernel<<<grid, kVarWarps * 32, 0, st>>>(nblocks, h->var_bptr, h->var_foff, h->row_ptr, h->col_idx, h->val,
+                                                               h->var_fac, h->status);
+    h->launches++;
+    BJ_CUDA(cudaGetLastError());
+    Status stt;
+    BJ_CUDA(cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaStreamSynchronize(st));  // also keeps bp / fo alive until the copies are done
+    if (stt.flags & ST_NOT_SPD) {
+        h->failed = true;
+        h->bad_block = (int64_t)stt.bad_block;
+        return BJ_ERR_NOT_SPD;
+    }
+    return BJ_OK;
+}
+
+int launch_solve_var(bj_handle_s* h, int dir, const double* in, double* out)
+{
+    const unsigned grid = (unsigned)((h->nblocks + kVarWarps - 1) / kVarWarps);
+    const bool pdl = h->pdl && !h->prof_on;
+    cudaError_t e;
+    if (dir == 0)
+        e = launch_kernel(solve_var_kernel<0>, dim3(grid), dim3(kVarWarps * 32), 0, h->stream, pdl, h->nblocks,
+                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out);
+    else if (dir == 1)
+        e = launch_kernel(solve_var_kernel<1>, dim3(grid), dim3(kVarWarps * 32), 0, h->stream, pdl, h->nblocks,
+                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out);
+    else
+        e = launch_kernel(solve_var_kernel<2>, dim3(grid), dim3(kVarWarps * 32), 0, h->stream, pdl, h->nblocks,
+                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out);
+    if (e != cudaSuccess) { set_cuda_error(e, "solve_var_kernel"); return BJ_ERR_CUDA; }
+    h->launches++;
+    return BJ_OK;
+}
+
+}  // namespace bj

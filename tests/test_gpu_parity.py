@@ -849,3 +849,79 @@ def test_minv_lanczos_banded_factors(B, torch_, monkeypatch):
     c = oracle.Precond(A, 16).cond_estimate_minv(50)
     assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
     B.bj_destroy(h)
+
+
+# ------------------------------------------------------------------ variable-size blocks (NEXT-3) --------
+def _setup_blocks(B, torch_, A, ptr):
+    rp, ci, val = dev(torch_, A.row_ptr), dev(torch_, A.col_idx), dev(torch_, A.val)
+    return B.bj_setup_blocks(rp, ci, val, ptr), (rp, ci, val)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_variable_blocks_match_oracle(B, torch_, rel, cfg):
+    """bj_setup_blocks with seeded block sizes 1..32 (several hundred blocks, ragged last block): every apply entry point
+    element by element against oracle.PrecondBlocks, kappa with full reorthogonalisation to the bar of the north star."""
+    A = mat(cfg, "tiny" if cfg != 1 else "full")
+    ptr = W.random_block_ptr(A.n, seed=40 + cfg, smin=1, smax=32)
+    h, keep = _setup_blocks(B, torch_, A, ptr)
+    info = B.bj_get_info(h)
+    assert info["b"] == -1 and info["solve_kernel"] == 4 and info["nblocks"] == len(ptr) - 1
+    P = oracle.PrecondBlocks(A, ptr)
+    for seed in (7, 8):
+        x = W.seeded_vector(seed, A.n)
+        xd = dev(torch_, x)
+        for name in ("bj_solve_L", "bj_solve_Lt", "bj_apply", "bj_op_apply"):
+            got = getattr(B, name)(h, xd).cpu().numpy()
+            want = getattr(P, name[3:])(x)
+            e2, ei = rel(got, want)
+            assert e2 <= TOL_APPLY, (cfg, name, e2)
+    g = B.bj_cond_estimate_ex(h, 30, reorth=True)
+    c = P.cond_estimate(30, reorth=True)
+    assert g["iters_done"] == c["iters_done"]
+    assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (cfg, g["kappa"], c["kappa"])
+    B.bj_destroy(h)
+
+
+def test_variable_blocks_equal_sizes_reproduce_the_uniform_handle(B, torch_, rel):
+    A = mat(2, "small")
+    x = dev(torch_, W.seeded_vector(5, A.n))
+    for b in (3, 8, 16, 32):
+        ptr = np.unique(np.minimum(np.arange(0, A.n + b, b), A.n))
+        hv, keep = _setup_blocks(B, torch_, A, ptr)
+        hu, keep2 = B.setup_from_host(A, b)
+        for name in ("bj_apply", "bj_op_apply"):
+            e2, ei = rel(getattr(B, name)(hv, x).cpu().numpy(), getattr(B, name)(hu, x).cpu().numpy())
+            assert e2 <= TOL_APPLY, (b, name, e2)
+        B.bj_destroy(hv); B.bj_destroy(hu)
+
+
+def test_variable_blocks_exact_preconditioner_pcg_and_errors(B, torch_, rel):
+    sizes = [5, 1, 32, 7, 16, 2, 24] * 9
+    A = W.direct_sum_spd(sizes)
+    ptr = np.concatenate([[0], np.cumsum(sizes)])
+    h, keep = _setup_blocks(B, torch_, A, ptr)
+    x = W.seeded_vector(2, A.n)
+    y = B.bj_op_apply(h, dev(torch_, x)).cpu().numpy()
+    assert np.abs(y - x).max() <= 1e-13                      # M = A: A^ = I (PAPER.md:76-82)
+    g = B.bj_cond_estimate_ex(h, 10, reorth=True)
+    assert g["iters_done"] == 1 and abs(g["kappa"] - 1) <= 1e-12
+    r = B.bj_pcg_solve(h, dev(torch_, x), max_iters=10, rtol=1e-12)
+    assert r["iters"] == 1 and r["true_relres"] <= 1e-13
+    gm = B.bj_cond_estimate_minv(h, 10)
+    assert gm["iters_done"] == 1 and abs(gm["kappa"] - 1) <= 1e-12
+    with pytest.raises(B.BJError):
+        B.bj_cond_estimate_batch(h, 9, 10, 1)
+    B.bj_destroy(h)
+    rp, ci, val = keep
+    for bad in ([0, 5, 5, A.n], [1, A.n], [0, 40, A.n], [0, A.n - 1]):
+        with pytest.raises(B.BJError):
+            B.bj_setup_blocks(rp, ci, val, bad)
+    # a block that is not positive definite is reported by index
+    A2 = W.direct_sum_spd([4, 6, 3])
+    v = A2.val.copy()
+    Ad = A2.to_dense()
+    d_idx = [e for i in range(4, 10) for e in range(A2.row_ptr[i], A2.row_ptr[i + 1]) if A2.col_idx[e] == i]
+    v[d_idx[2]] = -1.0
+    with pytest.raises(B.BJError) as ei:
+        B.bj_setup_blocks(dev(torch_, A2.row_ptr), dev(torch_, A2.col_idx), dev(torch_, v), [0, 4, 10, 13])
+    assert ei.value.bad_block == 1
