@@ -219,6 +219,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         t.group_smem_kb = env_int("BJ_GROUP_SMEM_KB", t.group_smem_kb);
         t.group_warps = env_int("BJ_GROUP_WARPS", t.group_warps);
         t.group_lanes = env_int("BJ_GROUP_LANES", t.group_lanes);
+        t.serp_keep_mb = env_int("BJ_SERP_KEEP_MB", t.serp_keep_mb);
         t.pdl_early = env_int("BJ_PDL_EARLY", t.pdl_early);
         t.ctas_per_sm = env_int("BJ_CTAS_PER_SM", t.ctas_per_sm);
         t.lanczos_fuse = env_int("BJ_LANCZOS_FUSE", t.lanczos_fuse);

@@ -14,6 +14,14 @@ __device__ __forceinline__ double ld_stream(const double* p)
     asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
+// streaming load with an explicit L2 eviction policy (createpolicy): evict_first for read-once data, evict_last for the
+// slice the next kernel starts with
+__device__ __forceinline__ double ld_stream_hint(const double* p, uint64_t pol)
+{
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
 // same load, but schedulable: the compiler may hoist it above unrelated arithmetic (the data never changes after setup)
 __device__ __forceinline__ double ld_const_stream(const double* p)
 {
@@ -91,6 +99,14 @@ __device__ __forceinline__ uint64_t policy_evict_first()
 {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// the slice of a read-once stream that the NEXT kernel starts with: ordinary LRU lines.  (evict_last was measured and
+// dropped: the lines outlive the chain of applies and take L2 away from the Lanczos vectors and from bj_apply's input.)
+__device__ __forceinline__ uint64_t policy_evict_normal()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol)

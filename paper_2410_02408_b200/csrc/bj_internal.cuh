@@ -38,6 +38,7 @@ struct Status {
 struct Tuning {
     int solve_warps = 8, solve_stage_kb = 32, solve_stages = 2, solve_ctas = 4, solve_pair = 1;  // solve_stream_kernel
     int solve_group = 1, group_stages = 2, group_smem_kb = 220, group_warps = 12, group_lanes = 0;  // solve_group_kernel
+    int serp_keep_mb = 48;  // BJ_SERP_KEEP_MB (0 = off): serpentine walk of the block solves, megabytes of factor kept in L2 per walk
     int pdl_early = 0;      // bit 0: stream solves, bit 1: stream SpMV release their dependents at entry
     int ctas_per_sm = 4;    // wanted CTAs per SM of the SpMV tile kernel
     int lanczos_fuse = 1;   // fast-mode Lanczos rides on the operator's kernels

@@ -75,19 +75,28 @@ template <int B, int DIR, bool VEC, int LZ, bool TRI>
 __global__ void __launch_bounds__(128, SMALL_MINB)
 solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                    const double* in, double* out,  // in == out allowed: a thread touches only its own block
-                   const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg)
+                   const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg,
+                   const int serp,                 // 1: serpentine walk (launch_small): CTA q takes the q-th LAST slice of blocks
+                   const unsigned serp_keep_from)  //    and CTAs q >= serp_keep_from load their factors as ordinary L2 lines instead of evict_first
 {
     constexpr int P = TRI ? 2 * B - 1 : B * (B + 1) / 2;
     __shared__ double lz_sh[8];
     pdl_trigger();
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned bid = serp ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int64_t k = (int64_t)bid * blockDim.x + threadIdx.x;
     const bool act = k < nblocks;
     if (LZ == 0 && !act) return;
     const int64_t kc = act ? k : 0;
     const double* f = fac + (kc >> 5) * (int64_t)(P * kInterleave) + (kc & 31);
     double l[P];
+    if (serp) {
+        const uint64_t pol = blockIdx.x >= serp_keep_from ? policy_evict_normal() : policy_evict_first();
 #pragma unroll
-    for (int e = 0; e < P; ++e) l[e] = ld_stream(f + e * kInterleave);   // factors never change after setup
+        for (int e = 0; e < P; ++e) l[e] = ld_stream_hint(f + e * kInterleave, pol);
+    } else {
+#pragma unroll
+        for (int e = 0; e < P; ++e) l[e] = ld_stream(f + e * kInterleave);   // factors never change after setup
+    }
     pdl_wait();                                                          // `in` may come from the previous kernel
     const int64_t lo = kc * B;
     double v[B];
@@ -356,6 +365,8 @@ struct GroupParams {
     int stages;
     int lz;              // 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0), 3 PCG update + apply (DIR 2)
     int bwd_from_fwd;    // DIR 1: run the backward substitution from the forward copy (fac0 = forward copy)
+    int reverse;         // serpentine: this launch walks the tiles from the last to the first (see launch_group_t)
+    int64_t keep_from;   // tiles at position >= keep_from of the walk are loaded as ordinary L2 lines instead of evict_first
     LzPrologue pro;
     LzEpilogue epi;
     PcgHook pcg;
@@ -397,10 +408,14 @@ solve_group_kernel(const GroupParams p)
 
     const int64_t stride = (int64_t)gridDim.x * nwarps;
     const int64_t first = (int64_t)blockIdx.x * nwarps + warp;
-    const uint64_t pol = policy_evict_first();
+    const uint64_t pol_stream = policy_evict_first();
+    const uint64_t pol_keep = policy_evict_normal();
+    // `tile` counts positions of the walk; phys() is the tile of the factor array that sits there
+    auto phys = [&](int64_t tile) { return p.reverse ? p.ntiles - 1 - tile : tile; };
     auto issue = [&](int64_t tile, int s) {  // lane 0 only: one bulk copy per block and copy
         if (tile >= p.ntiles) return;
-        const int64_t k0 = tile * NBW;
+        const uint64_t pol = tile >= p.keep_from ? pol_keep : pol_stream;
+        const int64_t k0 = phys(tile) * NBW;
         const int nb = (int)(k0 + NBW <= p.nblocks ? NBW : p.nblocks - k0);
         double* dst = ring + (size_t)s * kStageDoubles;
         mbar_expect_tx(&full[s], (uint32_t)nb * kBlockBytes * kCopies);
@@ -433,7 +448,7 @@ solve_group_kernel(const GroupParams p)
     // Loads of one tile are issued together (all rows, all vectors) before anything is stored: the Lanczos
     // vectors may alias as far as the compiler knows, so interleaved stores would serialise the loads.
     auto fetch = [&](int64_t tile, double (&dst)[RPL], double (&ew)[RPL], double (&ev)[RPL]) {
-        const int64_t row0 = tile * (NBW * B) + lane;
+        const int64_t row0 = phys(tile) * (NBW * B) + lane;
         double a[RPL], c[RPL];
 #pragma unroll
         for (int k = 0; k < RPL; ++k) {
@@ -509,7 +524,7 @@ solve_group_kernel(const GroupParams p)
 #pragma unroll
         for (int k = 0; k < RPL; ++k) xchg[g * XB + k * LPB + l] = r[k];
         __syncwarp();
-        const int64_t row0 = tile * (NBW * B) + lane;
+        const int64_t row0 = phys(tile) * (NBW * B) + lane;
 #pragma unroll
         for (int k = 0; k < RPL; ++k) {
             const int e = k * 32 + lane;
@@ -561,9 +576,16 @@ static int launch_small(bj_handle_s* h, const double* in, double* out, const LzP
     if (pcg && ((int)blocks > pcg->red_rr.cap || (int)blocks > pcg->red_rz.cap)) return BJ_ERR_INVALID_ARG;
     if ((epi && (int)blocks > epi->red.cap) || (pro && (int)blocks > pro->red.cap)) return BJ_ERR_INVALID_ARG;
     cudaError_t e = cudaSuccess;
+    // serpentine walk (see launch_group_t): the backward solve starts at the END of the factor array, where the fused
+    // SpMV + forward-solve kernel of the previous operator apply stopped, and keeps the head of the array for the next one
+    const int P = h->tri ? 2 * h->b - 1 : h->packed;
+    const int64_t cta_bytes = (int64_t)threads * P * 8;
+    const int64_t keep_ctas = std::min<int64_t>(blocks, (int64_t)h->tune.serp_keep_mb * 1000000 / cta_bytes);
+    const int serp = (DIR == 1 && LZ == 0 && keep_ctas > 0) ? 1 : 0;  // plain kernels only (see launch_group_t)
+    const unsigned serp_keep_from = (unsigned)(blocks - keep_ctas);
 #define BJ_LAUNCH_SMALL(B, V, T)                                                                                  \
     launch_kernel(solve_small_kernel<B, DIR, V, LZ, T>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,     \
-                  (const double*)h->fac_small, in, out, pr, ep, pc)
+                  (const double*)h->fac_small, in, out, pr, ep, pc, serp, serp_keep_from)
 #define BJ_CASE(B)                                                                         \
     case B:                                                                                \
         e = vec ? BJ_LAUNCH_SMALL(B, true, false) : BJ_LAUNCH_SMALL(B, false, false);      \
@@ -673,6 +695,18 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     gp.fac0 = (DIR == 1 && !gp.bwd_from_fwd) ? h->fac_bwd : h->fac_fwd;
     gp.fac1 = h->fac_bwd;
     gp.in = in; gp.out = out; gp.stages = stages;
+    // Serpentine walk (BJ_SERP_KEEP_MB > 0): the backward solve walks the factor array from its end to its start and the
+    // forward solve from start to end, and the last `keep` megabytes of each walk are loaded as ordinary L2 lines instead
+    // of evict_first.  In a chain of operator applies (back-to-back bj_op_apply, parity-mode Lanczos) the next backward
+    // solve then finds the tail of the array, and the forward solve its head, still in the 126 MB L2: those bytes are not
+    // read from HBM twice.  bj_apply (DIR 2) always walks forward and keeps nothing; the hooked kernels of the fused
+    // Lanczos / PCG steps keep nothing either (their vectors are worth more L2 than the factors: measured).
+    {
+        const int64_t tile_bytes = (int64_t)kGroupBlocksPerWarp * Geo::P * 8;
+        const int64_t keep_tiles = (DIR == 2 || pro || epi || pcg) ? 0 : std::min<int64_t>(gp.ntiles, (int64_t)h->tune.serp_keep_mb * 1000000 / tile_bytes);
+        gp.reverse = (DIR == 1 && keep_tiles > 0) ? 1 : 0;
+        gp.keep_from = gp.ntiles - keep_tiles;
+    }
     gp.lz = (DIR == 1 && pro) ? 1 : (DIR == 0 && epi) ? 2 : (DIR == 2 && pcg) ? 3 : 0;
     gp.pcg = pcg ? *pcg : PcgHook{};
     gp.pro = pro ? *pro : LzPrologue{};

@@ -119,6 +119,7 @@ struct StreamParams {
     LzEpilogue epi;
     const double* dot_with;  // lz == 2: per-CTA partials of dot_with . y go to dot_red (PCG: p . A p)
     LzReduce dot_red;
+    int64_t fac_keep_from;   // FUSE 1: tiles >= this load their factors as ordinary L2 lines (serpentine walk, launch_group_t)
 };
 
 __device__ __forceinline__ void consumer_bar_sync(int nthreads)
@@ -178,6 +179,7 @@ spmv_stream_kernel(const StreamParams p)
     if (warp == 0) {
         // ------------------------------ producer ------------------------------------------------
         const uint64_t pol = policy_evict_first();
+        const uint64_t pol_keep = policy_evict_normal();
         const int nnz4 = (int)(p.nnz & ~(long long)(Q - 1));
         int pb0 = 0, pb1 = 0;
         int it = 0;
@@ -246,7 +248,7 @@ spmv_stream_kernel(const StreamParams p)
                     else bulk_g2s(dc, p.ci + a0, (uint32_t)(a1 - a0) * 4u, &full[s], pol);
                 }
                 if (rq > 0) bulk_g2s(dr, p.rp + r0, (uint32_t)rq * 4u, &full[s], pol);
-                if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], pol);
+                if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], (FUSE == 1 && tile >= p.fac_keep_from) ? pol_keep : pol);
                 if (FUSE == 3)  // one copy per block, padded stride: the groups of a solving warp read different banks
                     for (int q = 0; q < gblk; ++q)
                         bulk_g2s(s_fac(s) + (size_t)q * Geo::STRIDE, p.fac + (r0 / GB + q) * (int64_t)Geo::P, (uint32_t)(Geo::P * 8),
@@ -605,6 +607,11 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the b > 8 fused paths have no hook
     if (epi && h->num_sms * 4 > epi->red.cap) return BJ_ERR_INVALID_ARG;
     sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
+    sp.fac_keep_from = sp.ntiles;
+    if (fuse && h->solve_kind == 1 && h->tune.serp_keep_mb > 0 && sp.lz == 0) {
+        const int64_t tile_bytes = (int64_t)(sp.R / sp.b) * sp.P * 8;
+        sp.fac_keep_from = sp.ntiles - std::min<int64_t>(sp.ntiles, (int64_t)h->tune.serp_keep_mb * 1000000 / tile_bytes);
+    }
     const int threads = 32 + 32 * h->stream_warps;
     const int grid = h->tune.ctas_per_sm;  // wanted CTAs per SM; clipped to the real occupancy at launch
     int rc = BJ_OK;
