@@ -154,6 +154,9 @@ int bj_release_cached_memory(void);
  * bj_pcg_solve; the Lanczos / PCG iterations run unfused); the batch entry points return BJ_ERR_INVALID_ARG.  One warp per
  * block (lane = row), packed lower triangles back to back.  bj_get_info reports b = -1, solve_kernel = 4.  Errors as
  * bj_setup; a layout that breaks the rules above is BJ_ERR_INVALID_ARG.  Synchronises. */
+/* (launch-shape knob read by bj_setup: BJ_SERP_KEEP_MB, default 48, 0 = off -- the plain backward solve walks the factor array from
+ * its end, the forward solve from its start, and the last that many megabytes of a walk stay ordinary L2 lines for the next kernel
+ * of a chain of operator applies; results are bit-identical either way.) */
 int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out);
 int bj_set_stream(bj_handle_t h, void* cuda_stream);
 int bj_set_option(bj_handle_t h, int option, int value);
