@@ -925,3 +925,37 @@ def test_variable_blocks_exact_preconditioner_pcg_and_errors(B, torch_, rel):
     with pytest.raises(B.BJError) as ei:
         B.bj_setup_blocks(dev(torch_, A2.row_ptr), dev(torch_, A2.col_idx), dev(torch_, v), [0, 4, 10, 13])
     assert ei.value.bad_block == 1
+
+
+def test_serpentine_walk_of_the_block_solves(B, torch_, rel, monkeypatch):
+    """BJ_SERP_KEEP_MB: the plain backward solve visits the blocks from the last to the first and the
+    last megabytes of every walk stay ordinary L2 lines.  Only the visiting order and the cache policy change, so every
+    output is bit-identical to the forward walk (keep = 0); sizes chosen so that keep = 1 MB covers PART of the factor array
+    (both policies and the reversed tail tile in one launch), with a ragged last block / tile.  Oracle parity at keep = 1."""
+    cases = ((W.config2(48), 8), (W.config2(47), 8), (W.config4(256), 16), (mat(3, "small"), 32), (W.config5(14), 24),
+             (W.config5(14), 3), (W.config4(250), 16))
+    for A, b in cases:
+        xs = [dev(torch_, W.seeded_vector(s, A.n)) for s in (11, 12)]
+        out = {}
+        for keep_mb in ("0", "1", "48"):
+            monkeypatch.setenv("BJ_SERP_KEEP_MB", keep_mb)
+            h, keep = B.setup_from_host(A, b)
+            res = []
+            for x in xs:   # a chain of applies, so that a walk really starts where the previous one stopped
+                y = B.bj_op_apply(h, x).clone()
+                y2 = B.bj_op_apply(h, y).clone()
+                res += [y.cpu().numpy(), y2.cpu().numpy(), B.bj_solve_Lt(h, x).cpu().numpy(), B.bj_solve_L(h, x).cpu().numpy(),
+                        B.bj_apply(h, x).cpu().numpy()]
+            out[keep_mb] = res
+            if keep_mb == "1":
+                P = oracle.Precond(A, b)
+                x = W.seeded_vector(11, A.n)
+                for got, ref in ((res[0], P.op_apply(x)), (res[2], P.solve_Lt(x)), (res[3], P.solve_L(x))):
+                    e2, ei = rel(got, ref)
+                    assert e2 <= TOL_APPLY and ei <= TOL_APPLY, f"n={A.n} b={b}: rel2={e2:.3e} relinf={ei:.3e}"
+                g = B.bj_cond_estimate_ex(h, 12, reorth=True)
+                assert abs(g["kappa"] / P.cond_estimate(12, reorth=True)["kappa"] - 1) <= TOL_KAPPA
+            B.bj_destroy(h)
+        for keep_mb in ("1", "48"):
+            for got, ref in zip(out[keep_mb], out["0"]):
+                assert np.array_equal(got, ref), f"n={A.n} b={b} keep={keep_mb}"
