@@ -386,6 +386,9 @@ def main():
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": A.meta.get("name"), "baseline_config": args.config, "n": n, "nnz": nnz, "block": b,
                        "l2": "inputs larger than L2 (%.0f MB per apply)" % (ab["op_apply"] / 1e6),
+                       # library default 48 (bj_internal.cuh Tuning::serp_keep_mb): consecutive applies may share up to
+                       # 2 x this many MB of factor lines in L2; the rate stays quoted on the full algorithmic bytes
+                       "serpentine_keep_mb": int(os.environ.get("BJ_SERP_KEEP_MB", "48")),
                        "parallelism": "replicas" if world > 1 else "single",
                        "spmv_kernel": info["spmv_kernel"], "fused_forward": info["fused_forward"],
                        "spmv_lanes": info["spmv_lanes"]},
