@@ -39,7 +39,10 @@ struct Tuning {
     int solve_warps = 8, solve_stage_kb = 32, solve_stages = 2, solve_ctas = 4, solve_pair = 1;  // solve_stream_kernel
     int solve_group = 1, group_stages = 2, group_smem_kb = 220, group_warps = 12, group_lanes = 0;  // solve_group_kernel
     int serp_keep_mb = 48;  // BJ_SERP_KEEP_MB (0 = off): serpentine walk of the block solves, megabytes of factor kept in L2 per walk
-    int pdl_early = 0;      // bit 0: stream solves, bit 1: stream SpMV release their dependents at entry
+    int pdl_early = 4;      // bit 0: stream solves, bit 1: stream SpMV release their dependents at entry; bit 2 (default): the
+                            // plain UNFUSED tile SpMV does (its dependent, the forward solve, then starts on the SMs the SpMV's
+                            // tail frees and prefetches its factors: cfg 3 131.8 -> 128.9 us, cfg 4 184.7 -> 182.7; the fused
+                            // SpMV + solve kernel measured 0.6 us slower with it and keeps the exit trigger)
     int ctas_per_sm = 4;    // wanted CTAs per SM of the SpMV tile kernel
     int lanczos_fuse = 1;   // fast-mode Lanczos rides on the operator's kernels
     int tiny = 0;           // BJ_TINY=1: launch-bound sizes run the whole operator apply in one single-CTA kernel

@@ -599,6 +599,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.ci16 = h->col16;
     sp.x = x; sp.y = y;
     sp.early_trigger = (h->tune.pdl_early >> 1) & 1;
+    if ((h->tune.pdl_early & 4) && !fuse && !epi && !dot_with) sp.early_trigger = 1;
     sp.lz = epi ? 1 : (dot_with && dot_red) ? 2 : 0;
     sp.dot_with = dot_with;
     sp.dot_red = dot_red ? *dot_red : LzReduce{};
