@@ -620,6 +620,32 @@ def test_full_size_configs(B, torch_, rel, cfg):
         c = P.cond_estimate(m, reorth=True)
         assert g["iters_done"] == c["iters_done"] == m
         assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (cfg, b, g["kappa"], c["kappa"])
+        # The FUSED fast mode on the default kernels -- the path bench.py times (`fast_mode`, `long_run`): at full size the
+        # hooked solve / SpMV kernels take several ring passes per warp and close their sums with many-CTA tickets, which the
+        # `small` matrices never reach.  Coefficients of the first 12 steps element by element, kappa at m = 50.
+        for name, gpu_fn, cpu_fn in (("split", lambda k: B.bj_cond_estimate_ex(h, k, reorth=False),
+                                      lambda k: P.cond_estimate(k, reorth=False)),
+                                     ("minv", lambda k: B.bj_cond_estimate_minv(h, k), lambda k: P.cond_estimate_minv(k))):
+            c50 = cpu_fn(50)
+            g12, g50 = gpu_fn(12), gpu_fn(50)
+            sc = np.abs(c50["alpha"]).max()
+            assert g12["iters_done"] == 12 and g50["iters_done"] == c50["iters_done"] == 50
+            assert np.abs(g12["alpha"] - c50["alpha"][:12]).max() <= 1e-9 * sc, (cfg, b, name)
+            assert np.abs(g12["beta"] - c50["beta"][:12]).max() <= 1e-9 * sc, (cfg, b, name)
+            assert np.abs(g50["alpha"][:12] - c50["alpha"][:12]).max() <= 1e-9 * sc, (cfg, b, name)
+            assert abs(g50["kappa"] / c50["kappa"] - 1) <= TOL_KAPPA, (cfg, b, name, g50["kappa"], c50["kappa"])
+        if cfg == 2:
+            lmin, lmax = B.bj_cond_estimate(h, 50)      # the 4-argument call of the north star, full size
+            assert abs((lmax / lmin) / c["kappa"] - 1) <= TOL_KAPPA
+        B.bj_destroy(h)
+        del h, keep
+    if cfg == 2:
+        # kappa(A) itself (b = 0, parity mode, m = 50): the value the bench line prints as kappa.A
+        h, keep = B.setup_from_host(A, 0)
+        g = B.bj_cond_estimate_ex(h, 50, reorth=True)
+        c = oracle.Precond(A, 0).cond_estimate(50, reorth=True)
+        assert g["iters_done"] == c["iters_done"] == 50
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (g["kappa"], c["kappa"])
         B.bj_destroy(h)
         del h, keep
     _MATS.pop((cfg, "full"), None)
