@@ -3,11 +3,13 @@
 
 A "step" is one application of the split-preconditioned operator y = L^-1 A L^-T x (bj_op_apply:
 backward block solve -> CSR SpMV -> forward block solve) on BASELINE.json configs[1]
-(3D 7-point variable-coefficient diffusion on 128^3, block-Jacobi b = 8, fp64), inputs resident in HBM.
-The same run also reports setup ms (extraction + batched Cholesky), bj_apply, the Lanczos kappa
-estimates kappa(A) -> kappa(A^), the roofline of the dominant kernel (CUDA events bracketed around
-each kernel by the library's profiling hooks), the end-to-end rate through the host-buffer entry
-point, and the CPU oracle timed on the host cores as a reported baseline.
+(3D 7-point variable-coefficient diffusion on 128^3, block-Jacobi b = 8, fp64), inputs resident in HBM,
+ROTATING over eight distinct x / y pairs so that no vector of a step is left in L2 by the previous one.
+The same run also reports: the roofline of the dominant kernel (CUDA events bracketed around each kernel by the
+library's profiling hooks; algorithmic AND ncu-measured DRAM bytes), an A/B of the serpentine factor walk, setup
+(wall clock, kernel-only, its own roofline), bj_apply, the Lanczos kappa estimates kappa(A) -> kappa(A^), PCG,
+the end-to-end rate through the host-buffer entry point, the CPU oracle timed on the host cores, and a `configs`
+section with the operator apply on the other four BASELINE.json configs.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--block B] [--impl reference]
 
@@ -33,6 +35,9 @@ from paper_2410_02408_b200 import workloads as W  # noqa: E402
 METRIC = "precond_operator_applies_per_s"
 UNIT = "applies/s"
 NOMINAL_HBM_GBS = 8000.0  # BASELINE.json north_star "~8 TB/s"
+L2_MB = 126.0
+PAIRS = 8                 # distinct x / y pairs the timed loops rotate over
+OTHER_CONFIGS = ((1, 4), (3, 32), (4, 16), (5, 3), (5, 24))
 
 
 def algorithmic_bytes(n: int, nnz: int, b: int, band: int = -1) -> dict:
@@ -46,9 +51,14 @@ def algorithmic_bytes(n: int, nnz: int, b: int, band: int = -1) -> dict:
             "spmv_solve_L": spmv + solve, "op_apply": spmv + 2 * solve}
 
 
+def setup_bytes(n: int, nnz: int, factor_bytes: int) -> int:
+    """read the CSR once, write the factors."""
+    return 12 * nnz + 4 * (n + 1) + factor_bytes
+
+
 def ncu_traffic(cfg: int, b: int, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary
-    (profiles/traffic.txt: JSON text, written by hand from profiles/*.md); None if that kernel was not captured."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel kind, from profiles/traffic.txt (JSON text
+    written by `python -m paper_2410_02408_b200.ncu_traffic` from the committed ncu raw exports); None if not captured."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.txt")) as fh:
             return json.load(fh).get(f"cfg{cfg}_b{b}", {}).get(kernel)
@@ -63,6 +73,15 @@ def measured_peaks() -> tuple[float, str]:
             return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def workload_config(A, cfg: int, b: int, world: int) -> dict:
+    """The `config` object: identical keys and values in both arms (ours and --impl reference)."""
+    ab = algorithmic_bytes(A.n, A.nnz, b)
+    return {"workload": A.meta.get("name"), "baseline_config": cfg, "n": A.n, "nnz": A.nnz, "block": b,
+            "l2": "working set %.0f MB per apply vs %.0f MB of L2; the timed loop rotates over %d distinct x / y pairs"
+                  % (ab["op_apply"] / 1e6, L2_MB, PAIRS),
+            "parallelism": "replicas" if world > 1 else "single"}
 
 
 class ClockSampler:
@@ -149,7 +168,7 @@ def run_reference(args, A, b: int):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": A.meta.get("name"), "n": A.n, "nnz": A.nnz, "block": b},
+            "config": workload_config(A, args.config, b, int(os.environ.get("WORLD_SIZE", "1"))),
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": f"{steps} full operator applies (whole vector, N={A.n})"},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -230,6 +249,212 @@ def aggregate_max(ms_local: float, world: int) -> float:
     return float(t.item())
 
 
+def byte_model(n: int, nnz: int, b: int, info: dict) -> dict:
+    """Algorithmic bytes of the layout this handle really uses (the opt-in variants have their own, smaller, models)."""
+    ab = algorithmic_bytes(n, nnz, b, info.get("band_width", -1))
+    if info.get("col16") and info["spmv_kernel"] == 1:  # 16-bit column deltas: 10 bytes per entry
+        spmv16 = ab["spmv"] - 2 * nnz
+        ab = dict(ab, spmv=spmv16, spmv_solve_L=spmv16 + ab["solve_L"], op_apply=spmv16 + 2 * ab["solve_L"])
+    if info["spmv_kernel"] == 2:  # BSR(3) copy: values + one block column per nine entries + block row pointers
+        spmv_bsr = 8 * nnz + 4 * (nnz // 9) + 4 * (n // 3 + 1) + 16 * n
+        ab = dict(ab, spmv=spmv_bsr, spmv_solve_L=spmv_bsr + ab["solve_L"], op_apply=spmv_bsr + 2 * ab["solve_L"])
+    return ab
+
+
+class Rotation:
+    """Eight distinct input / output pairs: consecutive timed calls never share a vector."""
+
+    def __init__(self, B, torch, h, n: int, pairs: int = PAIRS):
+        self.x = [B.bj_seeded_vector(h, 31 + k) for k in range(pairs)]
+        self.y = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(pairs)]
+        self.i = 0
+
+    def next(self):
+        k = self.i % len(self.x)
+        self.i += 1
+        return self.x[k], self.y[k]
+
+
+def time_calls(torch, fn, rot: Rotation, steps: int) -> float:
+    """milliseconds of `steps` back-to-back calls fn(x, y), CUDA events on the current stream."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        x, y = rot.next()
+        fn(x, y)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def kernel_profile(B, h, rot: Rotation, ab: dict, steps: int) -> dict:
+    """Per-kernel durations from the library's profiling hooks (CUDA events around every kernel on the launching stream)."""
+    B.bj_profile_enable(h, True)
+    for _ in range(steps):
+        x, y = rot.next()
+        B.bj_op_apply(h, x, y)
+    kinds = {B.KERNEL_KIND_NAMES[k]: B.bj_profile_get(h, k) for k in range(B.BJ_K_COUNT)}
+    B.bj_profile_enable(h, False)
+    return {k: {"avg_us": 1e3 * v[0] / v[1], "launches": v[1], "alg_bytes": ab[k],
+                "gbs": ab[k] / (1e-3 * v[0] / v[1]) / 1e9} for k, v in kinds.items() if v[1] > 0}
+
+
+def roofline_of(kern: dict, cfg: int, b: int, peak: float, peak_src: str) -> dict:
+    dom = max(kern, key=lambda k: kern[k]["avg_us"])
+    total_us = sum(v["avg_us"] for v in kern.values())
+    traffic = ncu_traffic(cfg, b, dom)
+    r = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
+         "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+         "algorithmic_bytes": kern[dom]["alg_bytes"], "avg_us": kern[dom]["avg_us"],
+         "share_of_step": kern[dom]["avg_us"] / total_us,
+         "frac_of_nominal_8TBs": kern[dom]["gbs"] / NOMINAL_HBM_GBS}
+    if traffic:
+        # the HBM roofline fraction proper: DRAM bytes of the ncu capture over the live kernel time.  `frac` is quoted on
+        # the ALGORITHMIC bytes and exceeds it when part of them is served by L2 (vectors, the serpentine factor slice)
+        r["achieved_dram"] = traffic / (kern[dom]["avg_us"] * 1e-6) / 1e9
+        r["frac_dram"] = r["achieved_dram"] / peak
+        r["l2_assisted"] = bool(traffic < 0.98 * kern[dom]["alg_bytes"])
+    return r
+
+
+def measure_operator(B, torch, h, cfg: int, n: int, nnz: int, b: int, steps: int, warmup: int, local: int,
+                     peak: float, peak_src: str) -> dict:
+    """The operator apply on one handle: rotating inputs, clocks sampled during the timed region, per-kernel profile."""
+    info = B.bj_get_info(h)
+    ab = byte_model(n, nnz, b, info)
+    rot = Rotation(B, torch, h, n)
+    fn = lambda x, y: B.bj_op_apply(h, x, y)  # noqa: E731
+    for _ in range(warmup):
+        fn(*rot.next())
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = B.bj_get_info(h)["kernel_launches"]
+    ms = time_calls(torch, fn, rot, steps)
+    launches = B.bj_get_info(h)["kernel_launches"] - l0
+    clocks = sampler.stop()
+    us = 1e3 * ms / steps
+    kern = kernel_profile(B, h, rot, ab, min(steps, 500))
+    gbs = ab["op_apply"] / us / 1e3
+    out = {"us_per_apply": us, "applies_per_s": 1e6 / us, "steps": steps, "alg_bytes": ab["op_apply"], "gbs": gbs,
+           "frac_of_measured": gbs / peak, "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS,
+           "kernels": kern, "roofline": roofline_of(kern, cfg, b, peak, peak_src), "clocks": clocks,
+           "gpu_launches": launches, "spmv_kernel": info["spmv_kernel"], "fused_forward": info["fused_forward"],
+           "solve_kernel": info["solve_kernel"]}
+    if ab["op_apply"] < 0.5 * L2_MB * 1e6:
+        out["note"] = "working set fits L2: launch-bound, the GB/s figures are not HBM figures"
+    return out
+
+
+def measure_setup(B, torch, rp, ci, val, b: int, peak: float, **opts):
+    """bj_setup: first call of the process (cold pool), wall-clock median of 3 warm calls (allocation included), device
+    time of the setup kernels alone and their roofline (CSR read once + factors written)."""
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    h = B.bj_setup(rp, ci, val, b, **opts)
+    torch.cuda.synchronize()
+    first = 1e3 * (time.perf_counter() - t0)
+    wall, kms = [], []
+    for _ in range(3):
+        B.bj_destroy(h)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h = B.bj_setup(rp, ci, val, b, **opts)
+        torch.cuda.synchronize()
+        wall.append(1e3 * (time.perf_counter() - t0))
+        kms.append(B.bj_get_setup_time(h)["kernel_ms"])
+    nb = B.bj_get_setup_time(h)["algorithmic_bytes"]
+    k = float(np.median(kms))
+    return h, {"first_call_ms": first, "wall_ms": float(np.median(wall)), "kernel_ms": k, "alg_bytes": nb,
+               "gbs": nb / (k * 1e-3) / 1e9 if k > 0 else None, "frac_of_measured": nb / (k * 1e-3) / 1e9 / peak if k > 0 else None}
+
+
+def graph_replay_us(B, torch, h, x, y, steps: int) -> dict:
+    """Launch-bound sizes: capture G back-to-back applies in a CUDA graph on a side stream and replay it -- the kernels,
+    their PDL chaining and their arguments are the library's own launches."""
+    G = 64
+    side = torch.cuda.Stream()
+    B.bj_set_stream(h, side)
+    with torch.cuda.stream(side):
+        for _ in range(3):
+            B.bj_op_apply(h, x, y)
+        side.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            for _ in range(G):
+                B.bj_op_apply(h, x, y)
+        graph.replay()
+        side.synchronize()
+        reps = max(1, steps // G)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(side)
+        for _ in range(reps):
+            graph.replay()
+        g1.record(side)
+        side.synchronize()
+        gus = 1e3 * g0.elapsed_time(g1) / (reps * G)
+    B.bj_set_stream(h, torch.cuda.current_stream())
+    del graph
+    return {"applies_per_graph": G, "replays": reps, "us_per_apply": gus, "applies_per_s": 1e6 / gus}
+
+
+def other_configs(B, torch, args, local: int, peak: float, peak_src: str) -> dict:
+    """The operator apply on the other BASELINE.json configs (1, 3, 4, 5 with b = 3 and 24) in the same run, so that every
+    rate quoted in profiles/ and DESIGN.md has a driver-run counterpart."""
+    out = {}
+    steps = max(50, args.steps)
+    mats = {}
+    for cfg, b in OTHER_CONFIGS:
+        t0 = time.perf_counter()
+        if cfg not in mats:
+            mats.clear()
+            torch.cuda.empty_cache()
+            A = W.build(cfg, "full")
+            mats[cfg] = (A, tuple(torch.from_numpy(a).cuda() for a in (A.row_ptr, A.col_idx, A.val)))
+        A, (rp, ci, val) = mats[cfg]
+        h, setup = measure_setup(B, torch, rp, ci, val, b, peak)
+        r = measure_operator(B, torch, h, cfg, A.n, A.nnz, b, steps if cfg != 1 else max(steps, 2000), max(args.warmup, 10),
+                             local, peak, peak_src)
+        r["workload"] = A.meta.get("name")
+        r["n"], r["nnz"], r["block"] = A.n, A.nnz, b
+        r["setup"] = setup
+        if cfg == 1:
+            # launch-bound: graph replay, and the whole 50-step kappa estimate beside the oracle's (SURVEY 8(d))
+            x = B.bj_seeded_vector(h, 31)
+            r["graph"] = graph_replay_us(B, torch, h, x, torch.empty_like(x), 2000)
+            m = args.lanczos_iters
+            lz = {}
+            for name, fn in (("parity_mode", lambda: B.bj_cond_estimate(h, m)),
+                             ("fast_mode", lambda: B.bj_cond_estimate_ex(h, m, reorth=False))):
+                fn()
+                ts = []
+                for _ in range(5):
+                    torch.cuda.synchronize()
+                    t1 = time.perf_counter()
+                    res = fn()
+                    ts.append(time.perf_counter() - t1)
+                lz[name] = {"seconds": float(np.median(ts)),
+                            "kappa_est": (res[1] / res[0]) if isinstance(res, tuple) else res["kappa"]}
+            import oracle
+            P = oracle.Precond(A, b)
+            P.cond_estimate(m)
+            ts = []
+            for _ in range(5):
+                t1 = time.perf_counter()
+                c = P.cond_estimate(m)
+                ts.append(time.perf_counter() - t1)
+            lz["oracle_parity_mode"] = {"seconds": float(np.median(ts)), "kappa_est": c["kappa"], "cores": oracle.num_threads()}
+            lz["iters"] = m
+            r["lanczos"] = lz
+        r["section_seconds"] = time.perf_counter() - t0
+        B.bj_destroy(h)
+        del h
+        out[f"cfg{cfg}_b{b}"] = r
+    mats.clear()
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -244,22 +469,23 @@ def main():
     ap.add_argument("--cpu-budget-s", type=float, default=10.0)
     ap.add_argument("--spmv-kernel", type=int, default=-1)
     ap.add_argument("--fuse", type=int, default=-1)
-    ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e (profiling runs)")
+    ap.add_argument("--no-extras", action="store_true", help="skip kappa / cpu_baseline / e2e / configs (profiling runs)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the section that runs the other four configs")
     ap.add_argument("--batch", type=int, default=0,
                     help="N > 0: second workload (SURVEY 8(f) NEXT-4): N independent 32x32 Poisson systems (the paper's N = 2^10) "
                          "in one block-diagonal CSR; prints one JSON line for it and exits")
     ap.add_argument("--band", type=int, default=0,
-                    help="1: banded block factors where the diagonal blocks are banded (b > 8; SURVEY 8(f) NEXT-2); "
+                    help="1: banded block factors where the diagonal blocks are banded (SURVEY 8(f) NEXT-2); "
                          "the byte model of the roofline then counts the band, the dense-packed count is given beside it")
     ap.add_argument("--col16", type=int, default=0,
                     help="1: 16-bit column deltas in the tile SpMV when the bandwidth allows (SURVEY 8(f) NEXT-2): 10 bytes per entry")
     ap.add_argument("--bsr", type=int, default=0,
                     help="1: keep a 3x3-blocked (BSR) copy of the matrix when its structure allows (config 5; SURVEY 8(f) NEXT-2); "
                          "the SpMV byte model then counts 8 nnz + 4 nnz/9, the CSR count is given beside it")
+    ap.add_argument("--spmv2d", type=int, default=0, help="bj_setup_opts_t.spmv2d: 0 automatic, 1 force, -1 never")
+    ap.add_argument("--serp-keep-mb", type=int, default=0, help="bj_setup_opts_t.serp_keep_mb: 0 default (48), < 0 off")
     ap.add_argument("--graph", type=int, default=-1,
                     help="1: also time the operator apply replayed from a CUDA graph (default: only config 1, launch-bound)")
-    ap.add_argument("--gather-envelope", type=int, default=-1,
-                    help="1: also measure the machine's gather+stream envelope for this matrix (default: only config 3)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -285,45 +511,23 @@ def main():
     if world > 1:
         dist.init_process_group("nccl")
     B.lib()  # fail loudly if the CUDA library is missing
-    if args.band:
-        os.environ["BJ_BAND"] = "1"  # read by bj_setup
-    if args.bsr:
-        os.environ["BJ_BSR"] = "1"   # read by bj_setup
-    if args.col16:
-        os.environ["BJ_COL16"] = "1"
+    opts = {"band": args.band, "col16": args.col16, "bsr": args.bsr, "spmv2d": args.spmv2d, "serp_keep_mb": args.serp_keep_mb}
+    peak, peak_src = measured_peaks()
 
     n, nnz = A.n, A.nnz
     rp = torch.from_numpy(A.row_ptr).cuda()
     ci = torch.from_numpy(A.col_idx).cuda()
     val = torch.from_numpy(A.val).cuda()
 
-    # ---- setup (a1-a4): wall-clock ms including allocation, median of 3 -----------------------------
-    setup_ms = []
-    h = None
-    for _ in range(3):
-        if h is not None:
-            B.bj_destroy(h)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        h = B.bj_setup(rp, ci, val, b)
-        torch.cuda.synchronize()
-        setup_ms.append(1e3 * (time.perf_counter() - t0))
+    # ---- setup (a1-a4): wall clock including allocation, kernel-only device time, roofline ---------------
+    h, setup = measure_setup(B, torch, rp, ci, val, b, peak, **opts)
     if args.spmv_kernel >= 0:
         B.bj_set_option(h, B.BJ_OPT_SPMV_KERNEL, args.spmv_kernel)
     if args.fuse >= 0:
         B.bj_set_option(h, B.BJ_OPT_FUSE_FORWARD, args.fuse)
     info = B.bj_get_info(h)
-
-    x = B.bj_seeded_vector(h, 31)
-    y = torch.empty_like(x)
-    ab = algorithmic_bytes(n, nnz, b, info.get("band_width", -1))
+    ab = byte_model(n, nnz, b, info)
     ab_dense = algorithmic_bytes(n, nnz, b)
-    if info.get("col16") and info["spmv_kernel"] == 1:  # 16-bit column deltas: 10 bytes per entry
-        spmv16 = ab["spmv"] - 2 * nnz
-        ab = dict(ab, spmv=spmv16, spmv_solve_L=spmv16 + ab["solve_L"], op_apply=spmv16 + 2 * ab["solve_L"])
-    if info["spmv_kernel"] == 2:  # BSR(3) copy: values + one block column per nine entries + block row pointers
-        spmv_bsr = 8 * nnz + 4 * (nnz // 9) + 4 * (n // 3 + 1) + 16 * n
-        ab = dict(ab, spmv=spmv_bsr, spmv_solve_L=spmv_bsr + ab["solve_L"], op_apply=spmv_bsr + 2 * ab["solve_L"])
 
     def barrier():
         torch.cuda.synchronize()
@@ -331,9 +535,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- timed region: K operator applies, inputs resident in HBM ------------------------------------
+    # ---- timed region: K operator applies, inputs resident in HBM, rotating over PAIRS x / y pairs ------------
+    rot = Rotation(B, torch, h, n)
     for _ in range(args.warmup):
-        B.bj_op_apply(h, x, y)
+        B.bj_op_apply(h, *rot.next())
     sampler = ClockSampler(local)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -341,7 +546,7 @@ def main():
     sampler.start()
     e0.record()
     for _ in range(args.steps):
-        B.bj_op_apply(h, x, y)
+        B.bj_op_apply(h, *rot.next())
     e1.record()
     barrier()
     clocks = sampler.stop()
@@ -350,109 +555,61 @@ def main():
     value = world * args.steps / (ms * 1e-3)
     ms_per_step = ms / args.steps
 
-    # ---- repeatability: five more timed regions of K/5 steps each (median of >= 5 repeats) ----
-    rep_us = []
+    # ---- repeatability: five more timed regions (median of >= 5 repeats) ----------------------
     kr = max(20, args.steps // 5)
-    for _ in range(5):
-        e0.record()
-        for _ in range(kr):
-            B.bj_op_apply(h, x, y)
-        e1.record()
-        torch.cuda.synchronize()
-        rep_us.append(1e3 * e0.elapsed_time(e1) / kr)
+    rep_us = [1e3 * time_calls(torch, lambda x, y: B.bj_op_apply(h, x, y), rot, kr) / kr for _ in range(5)]
     repeats = {"steps_each": kr, "us_median": float(np.median(rep_us)), "us_min": float(min(rep_us)), "us_max": float(max(rep_us))}
 
-    # ---- per-kernel durations (CUDA events around every kernel, on the launching stream) --------------
-    B.bj_profile_enable(h, True)
-    prof_steps = min(args.steps, 500)
-    for _ in range(prof_steps):
-        B.bj_op_apply(h, x, y)
-    kinds = {B.KERNEL_KIND_NAMES[k]: B.bj_profile_get(h, k) for k in range(B.BJ_K_COUNT)}
-    B.bj_profile_enable(h, False)
-    kern = {k: {"avg_us": 1e3 * v[0] / v[1], "launches": v[1], "alg_bytes": ab[k],
-                "gbs": ab[k] / (1e-3 * v[0] / v[1]) / 1e9} for k, v in kinds.items() if v[1] > 0}
-    peak, peak_src = measured_peaks()
-    dom = max(kern, key=lambda k: kern[k]["avg_us"])
-    total_us = sum(v["avg_us"] for v in kern.values())
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kern[dom]["gbs"] / peak, "traffic": ncu_traffic(args.config, b, dom), "peak_source": peak_src,
-                "algorithmic_bytes": kern[dom]["alg_bytes"],
-                "share_of_step": kern[dom]["avg_us"] / total_us,
-                "frac_of_nominal_8TBs": kern[dom]["gbs"] / NOMINAL_HBM_GBS}
+    # ---- per-kernel durations and the roofline of the dominant kernel ------------------------------------
+    kern = kernel_profile(B, h, rot, ab, min(max(args.steps, 50), 500))
+    roofline = roofline_of(kern, args.config, b, peak, peak_src)
     op_gbs = ab["op_apply"] / (ms_per_step * 1e-3) / 1e9
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": A.meta.get("name"), "baseline_config": args.config, "n": n, "nnz": nnz, "block": b,
-                       "l2": "inputs larger than L2 (%.0f MB per apply)" % (ab["op_apply"] / 1e6),
-                       # library default 48 (bj_internal.cuh Tuning::serp_keep_mb): consecutive applies may share up to
-                       # 2 x this many MB of factor lines in L2; the rate stays quoted on the full algorithmic bytes
-                       "serpentine_keep_mb": int(os.environ.get("BJ_SERP_KEEP_MB", "48")),
-                       "parallelism": "replicas" if world > 1 else "single",
-                       "spmv_kernel": info["spmv_kernel"], "fused_forward": info["fused_forward"],
-                       "spmv_lanes": info["spmv_lanes"]},
+            "config": workload_config(A, args.config, b, world),
+            "impl_config": {"spmv_kernel": info["spmv_kernel"], "fused_forward": info["fused_forward"],
+                            "solve_kernel": info["solve_kernel"], "spmv_lanes": info["spmv_lanes"],
+                            "serpentine_keep_mb": 48 if args.serp_keep_mb == 0 else max(args.serp_keep_mb, 0),
+                            "band_width": info.get("band_width", -1), "col16": bool(info.get("col16")),
+                            "bsr3": info["spmv_kernel"] == 2, "input_pairs": PAIRS},
             "clocks": clocks, "gpu_launches": launches, "repeats": repeats, "roofline": roofline,
             "op_apply": {"alg_bytes": ab["op_apply"], "gbs": op_gbs, "frac_of_measured": op_gbs / peak,
-                         "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS},
-            "band": {"width": info.get("band_width", -1), "bsr3": info["spmv_kernel"] == 2, "col16": bool(info.get("col16")), "op_apply_bytes_dense_packed": ab_dense["op_apply"],
-                     "gbs_vs_dense_packed_count": ab_dense["op_apply"] / (ms_per_step * 1e-3) / 1e9},
-            "kernels": kern, "setup_ms": float(np.median(setup_ms)),
-            "factor_bytes": info["factor_bytes"]}
+                         "frac_of_nominal_8TBs": op_gbs / NOMINAL_HBM_GBS,
+                         "bytes_dense_packed_csr_model": ab_dense["op_apply"],
+                         "note": "algorithmic bytes / time; part of them is served by L2 when frac_of_measured > 1 "
+                                 "(roofline.frac_dram is the HBM fraction proper)"},
+            "kernels": kern, "setup": setup, "setup_ms": setup["wall_ms"], "factor_bytes": info["factor_bytes"]}
 
     if args.graph == 1 or (args.graph < 0 and args.config == 1):
-        # Launch-bound sizes (config 1: 0.15 MB per apply): capture G back-to-back applies in a CUDA graph on a side
-        # stream and replay it -- the kernels, their PDL chaining and their arguments are the library's own launches.
-        G = 64
-        side = torch.cuda.Stream()
-        B.bj_set_stream(h, side)
-        with torch.cuda.stream(side):
-            for _ in range(3):
-                B.bj_op_apply(h, x, y)
-            side.synchronize()
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph, stream=side):
-                for _ in range(G):
-                    B.bj_op_apply(h, x, y)
-            graph.replay()
-            side.synchronize()
-            reps = max(1, args.steps // G)
-            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            g0.record(side)
-            for _ in range(reps):
-                graph.replay()
-            g1.record(side)
-            side.synchronize()
-            gus = 1e3 * g0.elapsed_time(g1) / (reps * G)
-        B.bj_set_stream(h, torch.cuda.current_stream())
-        line["graph"] = {"applies_per_graph": G, "replays": reps, "us_per_apply": gus, "applies_per_s": 1e6 / gus,
-                         "eager_us_per_apply": 1e3 * ms_per_step}
-        del graph
-
-    if args.gather_envelope == 1 or (args.gather_envelope < 0 and args.config == 3):
-        # The SpMV of a matrix with random column structure is bound by one L1 wavefront per 8-byte gather plus the
-        # matrix stream sharing the SM <-> L2 path, not by HBM: measure that envelope on this device for this mix.
-        env = B.bj_probe_gather_stream(n, nnz, 12 * nnz + 4 * (n + 1))
-        sp_us = kern.get("spmv", kern.get("spmv_solve_L", {})).get("avg_us")
-        env.update({"gathers": nnz, "stream_bytes": 12 * nnz + 4 * (n + 1), "vec_len": n, "spmv_us": sp_us,
-                    "spmv_frac_of_envelope": (env["us_both"] / sp_us) if sp_us else None,
-                    "gathers_per_clk_per_sm": nnz / (env["us_gather"] * 1e-6) / (clocks["sm_mhz"] * 1e6) / 148
-                    if clocks.get("sm_mhz") else None})
-        line["gather_envelope"] = env
+        x0, y0 = rot.next()
+        line["graph"] = dict(graph_replay_us(B, torch, h, x0, y0, max(args.steps, 640)), eager_us_per_apply=1e3 * ms_per_step)
 
     if not args.no_extras:
-        # ---- bj_apply (a5) -----------------------------------------------------------------------------
+        # ---- A/B: the serpentine factor walk off (what a consumer that evicts L2 between applies would see) -------
+        if b > 0 and not args.serp_keep_mb:
+            hb = B.bj_setup(rp, ci, val, b, **dict(opts, serp_keep_mb=-1))
+            for _ in range(args.warmup):
+                B.bj_op_apply(hb, *rot.next())
+            k_ab = max(50, min(args.steps, 1000))
+            us_off = 1e3 * time_calls(torch, lambda x, y: B.bj_op_apply(hb, x, y), rot, k_ab) / k_ab
+            us_on = 1e3 * time_calls(torch, lambda x, y: B.bj_op_apply(h, x, y), rot, k_ab) / k_ab
+            line["serpentine_ab"] = {"steps": k_ab, "keep48_us": us_on, "keep0_us": us_off,
+                                     "keep0_gbs": ab["op_apply"] / us_off / 1e3, "keep0_frac_of_measured": ab["op_apply"] / us_off / 1e3 / peak}
+            B.bj_destroy(hb)
+
+        # ---- bj_apply (a5), rotating inputs ------------------------------------------------------------------
         if b > 0:
+            fn = lambda x, y: B.bj_apply(h, x, y)  # noqa: E731
             for _ in range(10):
-                B.bj_apply(h, x, y)
+                fn(*rot.next())
             k_apply = max(50, args.steps // 10)
-            e0.record()
-            for _ in range(k_apply):
-                B.bj_apply(h, x, y)
-            e1.record()
-            torch.cuda.synchronize()
-            ams = e0.elapsed_time(e1) / k_apply
-            line["apply"] = {"applies_per_s": 1e3 / ams, "gbs": ab["apply"] / (ams * 1e-3) / 1e9}
+            ams = time_calls(torch, fn, rot, k_apply) / k_apply
+            a_gbs = ab["apply"] / (ams * 1e-3) / 1e9
+            line["apply"] = {"applies_per_s": 1e3 / ams, "us": 1e3 * ams, "alg_bytes": ab["apply"], "gbs": a_gbs,
+                             "frac_of_measured": a_gbs / peak, "input_pairs": PAIRS,
+                             "note": "eight distinct r / z pairs (268 MB of vectors on config 2): vectors come from HBM"}
 
         # ---- end to end through the host-buffer entry point (pinned host memory) -----------------------
         xh = torch.from_numpy(W.seeded_vector(31, n)).pin_memory()
@@ -476,6 +633,7 @@ def main():
             kap = {}
             h0 = B.bj_setup(rp, ci, val, 0)
             for name, hh in (("A", h0), (f"bj{b}", h)):
+                B.bj_cond_estimate_ex(hh, m, reorth=True)  # workspace allocation outside the timed call
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
                 r = B.bj_cond_estimate_ex(hh, m, reorth=True)
@@ -541,28 +699,18 @@ def main():
 
             # ---- NEXT-2 variant beside the headline: banded / compact factors (own byte model), same matrix and b ----
             if not args.band and b >= 4:
-                os.environ["BJ_BAND"] = "1"
-                os.environ["BJ_COL16"] = "1"
-                hb = B.bj_setup(rp, ci, val, b)
-                os.environ.pop("BJ_BAND", None)
-                os.environ.pop("BJ_COL16", None)
+                hb = B.bj_setup(rp, ci, val, b, band=1, col16=1)
                 ib = B.bj_get_info(hb)
                 if ib.get("band_width", -1) >= 0 or ib.get("col16"):
                     for _ in range(10):
-                        B.bj_op_apply(hb, x, y)
+                        B.bj_op_apply(hb, *rot.next())
                     kb = max(100, args.steps // 10)
-                    e0.record()
-                    for _ in range(kb):
-                        B.bj_op_apply(hb, x, y)
-                    e1.record()
-                    torch.cuda.synchronize()
-                    bus = 1e3 * e0.elapsed_time(e1) / kb
-                    abb = algorithmic_bytes(n, nnz, b, ib["band_width"])
-                    red_bytes = abb["op_apply"] - (2 * nnz if ib.get("col16") and ib["spmv_kernel"] == 1 else 0)
+                    bus = 1e3 * time_calls(torch, lambda x, y: B.bj_op_apply(hb, x, y), rot, kb) / kb
+                    red_bytes = byte_model(n, nnz, b, ib)["op_apply"]
                     line["banded_variant"] = {"band_width": ib["band_width"], "col16": bool(ib.get("col16")), "us_per_apply": bus,
                                               "applies_per_s": 1e6 / bus, "band_model_bytes": red_bytes,
                                               "gbs_band_model": red_bytes / bus / 1e3, "factor_bytes": ib["factor_bytes"],
-                                              "note": "opt-in (--band 1 --col16 1 / BJ_BAND=1 BJ_COL16=1): banded or compact "
+                                              "note": "opt-in (bj_setup_opts_t.band / .col16; --band 1 --col16 1): banded or compact "
                                                       "factors and 16-bit column deltas; fewer bytes than the counts of SURVEY 8(d), "
                                                       "own accounting"}
                 B.bj_destroy(hb)
@@ -573,6 +721,10 @@ def main():
                                     "sample": f"{reps} full operator applies (whole vector, N={n}) in ~{args.cpu_budget_s:.0f} s"}
 
     B.bj_destroy(h)
+    del h, rot, rp, ci, val
+    if rank == 0 and world == 1 and not args.no_extras and not args.no_configs and args.config == 2 and args.scale == "full":
+        torch.cuda.empty_cache()
+        line["configs"] = other_configs(B, torch, args, local, peak, peak_src)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

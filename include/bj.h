@@ -32,13 +32,12 @@
  *   - No CPU fallback exists: without a CUDA device every compute entry point fails with BJ_ERR_CUDA.
  *   - A handle is not thread-safe; different handles may be used concurrently on different streams.
  *
- * Opt-in storage variants, selected by environment variables that bj_setup reads ONCE (each moves fewer bytes than
- * the CSR / dense-block counts of SURVEY.md 8(d) and has its own byte accounting; each falls back
- * silently to the default layout when the matrix does not have the structure; results stay within the same tolerances):
- *     BJ_BAND=1   banded diagonal blocks (lower bandwidth <= 2; b <= 8: tridiagonal) keep banded Cholesky factors;
- *     BJ_COL16=1  the column stream of the tile SpMV as 16-bit deltas col - row when every |col - row| < 32768;
- *     BJ_BSR=1    a handle-owned BSR(3) copy of a 3x3-blocked matrix (three unknowns per node).
- * bj_get_info reports which are in use (band_width, col16, spmv_kernel == 2).  Launch-shape knobs: DESIGN.md section 5.
+ * Opt-in storage variants are ARGUMENTS (bj_setup_opts_t, bj_setup_ex), per handle: banded / compact factors, 16-bit
+ * column deltas, a BSR(3) copy of the matrix.  Each moves fewer bytes than the CSR / dense-block counts of SURVEY.md 8(d)
+ * and has its own byte accounting; each falls back silently to the default layout when the matrix
+ * does not have the structure; results stay within the same tolerances.  bj_get_info reports which are in use.
+ * Environment variables (BJ_*) only tune LAUNCH SHAPES (tile sizes, stages, warps per CTA); they
+ * never select a storage format or an algorithm, and every result is independent of them up to summation order.
  */
 #ifndef BJ_H_
 #define BJ_H_
@@ -72,6 +71,22 @@ typedef struct {
     const double* val;      /* device, nnz */
 } bj_csr_t;
 
+/* Per-handle setup options (bj_setup_ex).  Zero-initialise, then set fields: 0 / NULL is the default everywhere, so
+ * `bj_setup_opts_t o = {0};` reproduces bj_setup.  The three storage variants are SURVEY.md 8(f) NEXT-2: each is used
+ * only when the matrix has the structure (otherwise the default layout, silently) and has its own byte model. */
+typedef struct {
+    void* cuda_stream;      /* cudaStream_t the setup runs on and the handle keeps (NULL: the default stream)               */
+    int32_t band;           /* 1: banded diagonal blocks (lower bandwidth <= 2; b <= 8: tridiagonal) keep banded factors    */
+    int32_t col16;          /* 1: the tile SpMV streams 16-bit column deltas col - row when every |col - row| < 32768       */
+    int32_t bsr;            /* 1: a handle-owned BSR(3) copy of a 3x3-blocked matrix (three unknowns per node)              */
+    int32_t serp_keep_mb;   /* serpentine walk of the factor array in chains of applies: megabytes of each walk left as
+                               ordinary L2 lines for the next kernel (results bit-identical).  0: default (48); < 0: off   */
+    int32_t spmv2d;         /* 2-D blocked SpMV for matrices with incoherent columns (a handle-owned bucketed copy, x slabs
+                               and y tiles in shared memory).  0: automatic (from the column-coherence statistic of the
+                               validation pass), 1: always when the sizes allow, -1: never                                 */
+    int32_t reserved[7];    /* must be zero                                                                               */
+} bj_setup_opts_t;
+
 typedef struct {
     int32_t iters;        /* number of Lanczos steps = operator applies = dim of T (>= 1)           */
     int32_t reorth;       /* 0: none (fused fast mode), 1: full reorthogonalisation, twice (parity)  */
@@ -97,13 +112,13 @@ typedef struct {
     int64_t workspace_bytes;  /* device bytes held for temporaries and Lanczos workspace             */
     int64_t kernel_launches;  /* number of kernels this handle has launched so far                   */
     int32_t spmv_kernel;      /* 0: row-per-subwarp CSR-vector kernel, 1: TMA-streamed tile kernel,
-                                 2: TMA-streamed BSR(3) kernel (BJ_BSR=1)                              */
+                                 2: TMA-streamed BSR(3) kernel (opts.bsr), 3: 2-D blocked kernel (opts.spmv2d) */
     int32_t spmv_lanes;       /* lanes per row chosen at setup                                       */
     int32_t solve_kernel;     /* 0: none (b=0), 1: thread-per-block (b<=8), 2: group/subwarp-per-block, 3: banded */
     int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
-    int32_t band_width;       /* >= 0: banded factors in use (BJ_BAND=1 at setup, solve_kernel 3), the lower
-                                 bandwidth of every diagonal block; -1: dense packed factors              */
-    int32_t col16;            /* 1: the tile SpMV streams 16-bit column deltas (BJ_COL16=1 at setup)          */
+    int32_t band_width;       /* >= 0: banded factors in use (opts.band at setup), the lower bandwidth of every
+                                 diagonal block; -1: dense packed factors                                   */
+    int32_t col16;            /* 1: the tile SpMV streams 16-bit column deltas (opts.col16 at setup)            */
 } bj_info_t;
 
 typedef struct {
@@ -128,8 +143,10 @@ enum { BJ_K_SOLVE_LT = 0, BJ_K_SPMV = 1, BJ_K_SOLVE_L = 2, BJ_K_APPLY = 3, BJ_K_
 
 /* options for bj_set_option */
 enum {
-    BJ_OPT_SPMV_KERNEL = 1,   /* 0 / 1 as in bj_info_t.spmv_kernel; -1 = automatic (default)          */
-    BJ_OPT_FUSE_FORWARD = 2   /* 0: three kernels, 1: fuse forward solve into SpMV, -1 = automatic    */
+    BJ_OPT_SPMV_KERNEL = 1,   /* 0 / 1 / 3 as in bj_info_t.spmv_kernel (when built for the handle); -1 = automatic (default) */
+    BJ_OPT_FUSE_FORWARD = 2,  /* 0: three kernels, 1: fuse forward solve into SpMV, -1 = automatic    */
+    BJ_OPT_LANCZOS_FUSE = 3,  /* 0: fast-mode Lanczos runs the unfused vector kernels; 1 / -1: the fused step (default) */
+    BJ_OPT_PCG_FUSE = 4       /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
 };
 
 /* a1-a4. Validate the CSR, extract the diagonal b x b blocks, factor each
@@ -143,20 +160,26 @@ int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out);
  * torch.cuda.current_stream().cuda_stream) and keeps it as the handle's stream. */
 int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_t* out);
 
+/* Same as bj_setup with per-handle options (host struct, read during the call only; NULL = all defaults).  Two
+ * handles of one process may differ in every option.  A non-zero reserved field is BJ_ERR_INVALID_ARG. */
+int bj_setup_ex(const bj_csr_t* csr, int b, const bj_setup_opts_t* opts_host, bj_handle_t* out);
+
+/* Device time of the setup kernels of THIS handle (a1-a3: validation, plan, extraction + Cholesky; CUDA events on the
+ * handle's stream around the kernel sequence, host round trips between them excluded) and the bytes they must move
+ * (12 nnz + 4 (n + 1) read once + factor bytes written).  Host out-pointers, either may be NULL. */
+int bj_get_setup_time(bj_handle_t h, double* kernel_ms_host, int64_t* algorithmic_bytes_host);
+
 /* Handle memory comes from a private stream-ordered pool that keeps freed slabs cached for the next
  * bj_setup (block-size sweeps); this returns the cache to the driver.  Synchronises the device. */
 int bj_release_cached_memory(void);
 
 /* diagonal blocks of DIFFERENT sizes (supervariable blocks).  block_ptr_host[0..nblocks] (host, int64):
  * 0 = p_0 < p_1 < .. < p_nblocks = n, every size p_{k+1} - p_k in 1..BJ_B_MAX; block k is the dense diagonal slice
- * A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:254-263 with a per-block size).  The array is read during the call
+ * A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:191-197 with a per-block size).  The array is read during the call
  * only.  Every other entry point works on the handle unchanged (bj_apply, bj_solve_L/Lt, bj_op_apply, bj_cond_estimate*,
  * bj_pcg_solve; the Lanczos / PCG iterations run unfused); the batch entry points return BJ_ERR_INVALID_ARG.  One warp per
  * block (lane = row), packed lower triangles back to back.  bj_get_info reports b = -1, solve_kernel = 4.  Errors as
  * bj_setup; a layout that breaks the rules above is BJ_ERR_INVALID_ARG.  Synchronises. */
-/* (launch-shape knob read by bj_setup: BJ_SERP_KEEP_MB, default 48, 0 = off -- the plain backward solve walks the factor array from
- * its end, the forward solve from its start, and the last that many megabytes of a walk stay ordinary L2 lines for the next kernel
- * of a chain of operator applies; results are bit-identical either way.) */
 int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out);
 int bj_set_stream(bj_handle_t h, void* cuda_stream);
 int bj_set_option(bj_handle_t h, int option, int value);
@@ -235,14 +258,6 @@ int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, const int64_t* offsets_h
  * Synchronises. */
 int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const int64_t* offsets_host, const double* b_dev, double* x_dev,
                        int max_iters, double rtol, int32_t* iters_host, double* relres_host, double* true_relres_host);
-
-/* Diagnostic (not on the operator path): the machine envelope that bounds the SpMV of matrices with random column
- * structure (config 3), which is limited by one L1 wavefront per 8-byte gather and not by HBM.  Measures, on the
- * current device, the microseconds of (a) `gathers` random 8-byte loads from an L2-resident vector of `vec_len`
- * doubles, (b) `stream_bytes` streamed HBM -> shared memory by bulk async copies, (c) both in one kernel.
- * Host out-pointers; allocates and frees its own buffers; synchronises. */
-int bj_probe_gather_stream(int64_t vec_len, int64_t gathers, int64_t stream_bytes, double* us_gather_host,
-                           double* us_stream_host, double* us_both_host);
 
 #ifdef __cplusplus
 }

@@ -16,19 +16,24 @@ BJ_B_MAX = 32
 BJ_DEFAULT_SEED = 0x241002408
 BJ_OK, BJ_ERR_INVALID_ARG, BJ_ERR_NOT_CANONICAL, BJ_ERR_TOO_LARGE, BJ_ERR_NOT_SPD, BJ_ERR_ALLOC, BJ_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
 BJ_K_SOLVE_LT, BJ_K_SPMV, BJ_K_SOLVE_L, BJ_K_APPLY, BJ_K_SPMV_SOLVE_L, BJ_K_COUNT = 0, 1, 2, 3, 4, 5
-BJ_OPT_SPMV_KERNEL, BJ_OPT_FUSE_FORWARD = 1, 2
+BJ_OPT_SPMV_KERNEL, BJ_OPT_FUSE_FORWARD, BJ_OPT_LANCZOS_FUSE, BJ_OPT_PCG_FUSE = 1, 2, 3, 4
 KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
 
-EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",
+EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_setup_ex", "bj_get_setup_time", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
            "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve",
-           "bj_probe_gather_stream", "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv", "bj_setup_blocks"]
+           "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv", "bj_setup_blocks"]
 
 
 class bj_csr_t(C.Structure):
     _fields_ = [("n", C.c_int64), ("nnz", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
                 ("val", C.c_void_p)]
+
+
+class bj_setup_opts_t(C.Structure):
+    _fields_ = [("cuda_stream", C.c_void_p), ("band", C.c_int32), ("col16", C.c_int32), ("bsr", C.c_int32),
+                ("serp_keep_mb", C.c_int32), ("spmv2d", C.c_int32), ("reserved", C.c_int32 * 7)]
 
 
 class bj_lanczos_opts_t(C.Structure):
@@ -79,6 +84,10 @@ def lib():
         vp, i32, i64 = C.c_void_p, C.c_int, C.c_int64
         L.bj_setup.argtypes = [C.POINTER(bj_csr_t), i32, C.POINTER(vp)]
         L.bj_setup_on_stream.argtypes = [C.POINTER(bj_csr_t), i32, vp, C.POINTER(vp)]
+        L.bj_setup_ex.argtypes = [C.POINTER(bj_csr_t), i32, C.POINTER(bj_setup_opts_t), C.POINTER(vp)]
+        L.bj_get_setup_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
+        L.bj_cond_estimate_minv.argtypes = [vp, C.POINTER(bj_lanczos_opts_t), C.POINTER(bj_lanczos_result_t)]
+        L.bj_setup_blocks.argtypes = [C.POINTER(bj_csr_t), vp, i64, vp, C.POINTER(vp)]
         L.bj_set_stream.argtypes = [vp, vp]
         L.bj_set_option.argtypes = [vp, i32, i32]
         L.bj_destroy.argtypes = [vp]
@@ -94,7 +103,6 @@ def lib():
         L.bj_release_cached_memory.argtypes = []
         L.bj_cond_estimate_batch.argtypes = [vp, i64, vp, i32, C.c_uint64, vp, vp, vp]
         L.bj_pcg_solve_batch.argtypes = [vp, i64, vp, vp, vp, i32, C.c_double, vp, vp, vp]
-        L.bj_probe_gather_stream.argtypes = [i64, i64, i64] + [C.POINTER(C.c_double)] * 3
         L.bj_profile_enable.argtypes = [vp, i32]
         L.bj_profile_get.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
         for f in EXPORTS:
@@ -140,16 +148,18 @@ class Handle:
             self.ptr = None
 
 
-def bj_setup(row_ptr, col_idx, val, b: int, stream=None) -> Handle:
+def bj_setup(row_ptr, col_idx, val, b: int, stream=None, band: int = 0, col16: int = 0, bsr: int = 0,
+             serp_keep_mb: int = 0, spmv2d: int = 0) -> Handle:
     """row_ptr/col_idx: int32 CUDA tensors, val: float64 CUDA tensor (borrowed).  stream: a torch stream,
-    default the current one."""
+    default the current one.  The keyword options are the fields of bj_setup_opts_t (bj_setup_ex)."""
     import torch
     n = row_ptr.numel() - 1
     nnz = val.numel()
     csr = bj_csr_t(n, nnz, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32, nnz), _dptr(val, torch.float64))
     st = (stream or torch.cuda.current_stream()).cuda_stream
+    opts = bj_setup_opts_t(C.c_void_p(st), int(band), int(col16), int(bsr), int(serp_keep_mb), int(spmv2d))
     out = C.c_void_p()
-    code = lib().bj_setup_on_stream(C.byref(csr), int(b), C.c_void_p(st), C.byref(out))
+    code = lib().bj_setup_ex(C.byref(csr), int(b), C.byref(opts), C.byref(out))
     if code == BJ_ERR_NOT_SPD and out.value:
         info = bj_info_t()
         lib().bj_get_info(out, C.byref(info))
@@ -157,6 +167,13 @@ def bj_setup(row_ptr, col_idx, val, b: int, stream=None) -> Handle:
         _check(code, int(info.bad_block))
     _check(code)
     return Handle(out, (row_ptr, col_idx, val), n)
+
+
+def bj_get_setup_time(h: Handle) -> dict:
+    """Device milliseconds of this handle's setup kernels and the bytes they must move."""
+    ms, nb = C.c_double(), C.c_int64()
+    _check(lib().bj_get_setup_time(h.ptr, C.byref(ms), C.byref(nb)))
+    return {"kernel_ms": ms.value, "algorithmic_bytes": nb.value}
 
 
 def bj_setup_blocks(row_ptr, col_idx, val, block_ptr, stream=None) -> Handle:
@@ -341,13 +358,6 @@ def bj_pcg_solve_batch(h, nsys: int, b, x=None, max_iters: int = 1000, rtol: flo
     return {"x": x, "iters": it, "relres": rel, "true_relres": trel}
 
 
-def bj_probe_gather_stream(vec_len: int, gathers: int, stream_bytes: int) -> dict:
-    """Microseconds of random 8-byte gathers, of a TMA stream, and of both at once (see include/bj.h)."""
-    g, s_, b = C.c_double(), C.c_double(), C.c_double()
-    _check(lib().bj_probe_gather_stream(int(vec_len), int(gathers), int(stream_bytes), C.byref(g), C.byref(s_), C.byref(b)))
-    return {"us_gather": g.value, "us_stream": s_.value, "us_both": b.value}
-
-
 def bj_release_cached_memory():
     _check(lib().bj_release_cached_memory())
 
@@ -362,10 +372,11 @@ def bj_profile_get(h, kind: int):
     return ms.value, cnt.value
 
 
-def setup_from_host(A, b: int, device="cuda"):
-    """Convenience: copy a workloads.CSR to the device and set up.  Returns (handle, (rp, ci, val))."""
+def setup_from_host(A, b: int, device="cuda", **opts):
+    """Convenience: copy a workloads.CSR to the device and set up (opts: the keyword options of bj_setup).
+    Returns (handle, (rp, ci, val))."""
     import torch
     rp = torch.from_numpy(A.row_ptr).to(device)
     ci = torch.from_numpy(A.col_idx).to(device)
     val = torch.from_numpy(A.val).to(device)
-    return bj_setup(rp, ci, val, b), (rp, ci, val)
+    return bj_setup(rp, ci, val, b, **opts), (rp, ci, val)

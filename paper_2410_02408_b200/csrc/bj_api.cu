@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 
 #include "bj_internal.cuh"
@@ -68,7 +69,6 @@ int launch_spmv(bj_handle_s* h, const double* x, double* y)
 int op_apply_device(bj_handle_s* h, const double* x, double* y)
 {
     int rc;
-    if (tiny_op_usable(h)) return launch_tiny_op_apply(h, x, y);  // launch-bound sizes: one kernel
     if (h->solve_kind == 0) {  // identity preconditioner: A^ = A
         if (x == y) {
             BJ_CUDA(cudaMemcpyAsync(h->t, x, (size_t)h->n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
@@ -102,13 +102,12 @@ int op_apply_lanczos(bj_handle_s* h, const LzPrologue* pro, const LzEpilogue* ep
 // instead of a cudaMalloc each.  bj_release_cached_memory() returns the cache to the driver.
 // BJ_POOL=0 selects plain cudaMalloc.
 static cudaMemPool_t g_pool[64] = {};
-static bool g_pool_tried[64] = {};
+static std::once_flag g_pool_once[64];
 
 static cudaMemPool_t get_pool(int dev)
 {
     if (dev < 0 || dev >= 64 || env_int("BJ_POOL", 1) == 0) return nullptr;
-    if (!g_pool_tried[dev]) {
-        g_pool_tried[dev] = true;
+    std::call_once(g_pool_once[dev], [dev]() {  // two threads setting up at once create ONE pool
         cudaMemPoolProps props;
         memset(&props, 0, sizeof(props));
         props.allocType = cudaMemAllocationTypePinned;
@@ -123,7 +122,7 @@ static cudaMemPool_t get_pool(int dev)
         } else {
             cudaGetLastError();
         }
-    }
+    });
     return g_pool[dev];
 }
 
@@ -148,8 +147,13 @@ static void free_handle(bj_handle_s* h)
     bsr_free(h);
     col16_free(h);
     if (h->slab) {
-        if (h->slab_pooled) cudaFreeAsync(h->slab, h->stream);
-        else cudaFree(h->slab);
+        // stream-ordered free on the handle's stream; if that stream is gone (a destroyed torch side stream after
+        // bj_set_stream) fall back to a synchronous free so that the slab is not leaked
+        if (!h->slab_pooled || cudaFreeAsync(h->slab, h->stream) != cudaSuccess) {
+            cudaGetLastError();
+            cudaDeviceSynchronize();
+            cudaFree(h->slab);
+        }
     }
     var_free(h);
     cudaFree(h->stage_in); cudaFree(h->stage_out);
@@ -162,7 +166,7 @@ static void choose_spmv(bj_handle_s* h)
 {
     int k = 0;
     if (h->stream_ok) k = 1;
-    if (h->bsr_ok) k = 2;  // opt-in (BJ_BSR=1) and the matrix is 3x3-blocked: fewer bytes than either CSR kernel
+    if (h->bsr_ok) k = 2;  // opt-in (opts.bsr) and the matrix is 3x3-blocked: fewer bytes than either CSR kernel
     if (h->opt_spmv_kernel == 0) k = 0;
     if (h->opt_spmv_kernel == 1 && h->stream_ok) k = 1;
     h->spmv_kernel = k;
@@ -188,10 +192,29 @@ const char* bj_strerror(int code)
     }
 }
 
-int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_t* out)
+}  // extern "C"
+
+// CUDA events around the kernel sequences of bj_setup (the host round trips between them are not device time)
+struct SetupTimer {
+    cudaStream_t st;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> spans;
+    explicit SetupTimer(cudaStream_t s) : st(s) {}
+    void begin() { cudaEvent_t a = nullptr, b = nullptr; cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); spans.push_back({a, b}); }
+    void end() { if (!spans.empty()) cudaEventRecord(spans.back().second, st); }
+    double total_ms() {  // call after a stream synchronisation
+        double t = 0.0;
+        for (auto& sp : spans) { float ms = 0.f; if (cudaEventElapsedTime(&ms, sp.first, sp.second) == cudaSuccess) t += ms; else cudaGetLastError(); }
+        return t;
+    }
+    ~SetupTimer() { for (auto& sp : spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); } }
+};
+
+static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_handle_t* out)
 {
     if (!out) return BJ_ERR_INVALID_ARG;
     *out = nullptr;
+    for (int r : o.reserved) if (r != 0) return BJ_ERR_INVALID_ARG;
+    void* cuda_stream = o.cuda_stream;
     if (!csr || !csr->row_ptr || csr->n <= 0 || csr->nnz < 0 || b < 0 || b > BJ_B_MAX) return BJ_ERR_INVALID_ARG;
     if (csr->nnz > 0 && (!csr->col_idx || !csr->val)) return BJ_ERR_INVALID_ARG;
     if (csr->n >= (1ll << 31) - 64 || csr->nnz >= (1ll << 31) - 64) return BJ_ERR_TOO_LARGE;
@@ -206,24 +229,21 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     h->nblocks = b > 0 ? (csr->n + b - 1) / b : 0;
     h->packed = b * (b + 1) / 2;
     cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    h->opts = o;
     h->pdl = env_int("BJ_PDL", 1) != 0;
     {
-        Tuning& t = h->tune;
+        Tuning& t = h->tune;  // launch shapes only (see bj_internal.cuh)
         t.solve_warps = env_int("BJ_SOLVE_WARPS", t.solve_warps);
         t.solve_stage_kb = env_int("BJ_SOLVE_STAGE_KB", t.solve_stage_kb);
         t.solve_stages = env_int("BJ_SOLVE_STAGES", t.solve_stages);
         t.solve_ctas = env_int("BJ_SOLVE_CTAS", t.solve_ctas);
-        t.solve_pair = env_int("BJ_SOLVE_PAIR", t.solve_pair);
-        t.solve_group = env_int("BJ_SOLVE_GROUP", t.solve_group);
         t.group_stages = env_int("BJ_GROUP_STAGES", t.group_stages);
         t.group_smem_kb = env_int("BJ_GROUP_SMEM_KB", t.group_smem_kb);
         t.group_warps = env_int("BJ_GROUP_WARPS", t.group_warps);
         t.group_lanes = env_int("BJ_GROUP_LANES", t.group_lanes);
-        t.serp_keep_mb = env_int("BJ_SERP_KEEP_MB", t.serp_keep_mb);
         t.pdl_early = env_int("BJ_PDL_EARLY", t.pdl_early);
         t.ctas_per_sm = env_int("BJ_CTAS_PER_SM", t.ctas_per_sm);
-        t.lanczos_fuse = env_int("BJ_LANCZOS_FUSE", t.lanczos_fuse);
-        t.tiny = env_int("BJ_TINY", t.tiny);
+        if (o.serp_keep_mb != 0) t.serp_keep_mb = o.serp_keep_mb < 0 ? 0 : o.serp_keep_mb;
     }
 
     auto fail = [&](int code) { free_handle(h); return code; };
@@ -241,8 +261,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         h->lanes = b <= 16 ? 16 : 32;
         fac_a = fac_b = (size_t)h->nblocks * h->packed * sizeof(double) + 16;  // 16 B slack: bulk copies round up
         // the group kernel (b = 16, 24, 32) runs the backward substitution from the forward copy too: one copy is kept
-        h->single_copy = (b == 16 || b == 24 || b == 32) && h->tune.solve_group != 0 && env_int("BJ_SINGLE_COPY", 1) != 0 &&
-                         env_int("BJ_SETUP_WARP", 0) == 0;
+        h->single_copy = b == 16 || b == 24 || b == 32;
         if (h->single_copy) fac_b = 0;
     }
     const size_t total = 2 * vb + 256 + up256(fac_a) + up256(fac_b);
@@ -266,7 +285,10 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     if (ce != cudaSuccess) { set_cuda_error(ce, "status init"); return fail(BJ_ERR_CUDA); }
 
     // a1 validate (also longest row and the column-coherence statistic)
+    SetupTimer timer(h->stream);
+    timer.begin();
     int rc = launch_validate(h);
+    timer.end();
     if (rc != BJ_OK) return fail(rc);
     Status stt;
     ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
@@ -279,7 +301,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
 
     // NEXT-2, opt-in: banded diagonal blocks keep banded factors -- (w+1) b doubles per block instead of b(b+1)/2.
     // Only for b > 8 (the b <= 8 path fuses the forward solve into the SpMV kernel, which the band path does not).
-    if (h->solve_kind == 1 && b >= 4 && env_int("BJ_BAND", 0) != 0 && env_int("BJ_SETUP_WARP", 0) == 0) {
+    if (h->solve_kind == 1 && b >= 4 && o.band != 0) {
         // b <= 8: tridiagonal blocks keep bidiagonal factors, 2b - 1 doubles per block instead of b(b+1)/2; same kernels
         // (thread per block, fused into the SpMV tile kernel, Lanczos / PCG hooks), compile-time / uniform index switch
         rc = launch_band_width(h);
@@ -294,7 +316,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
             h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * h->packed * kInterleave * (int64_t)sizeof(double);
         }
     }
-    if (h->solve_kind == 2 && h->nblocks >= 64 && env_int("BJ_BAND", 0) != 0) {
+    if (h->solve_kind == 2 && h->nblocks >= 64 && o.band != 0) {
         rc = launch_band_width(h);
         if (rc != BJ_OK) return fail(rc);
         ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
@@ -308,6 +330,7 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
         }
     }
 
+    timer.begin();
     // lanes per row for the CSR-vector kernel: power of two near the mean row length
     {
         const double mean = (double)h->nnz / (double)h->n;
@@ -338,18 +361,20 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
 
     // SpMV plan for the streamed kernel: tile rows now, stage capacity once the fullest tile is known
     rc = spmv_stream_configure(h);
+    timer.end();
     if (rc != BJ_OK) return fail(rc);
 
     ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
     if (ce != cudaSuccess) { set_cuda_error(ce, "setup"); return fail(BJ_ERR_CUDA); }
+    h->setup_kernel_ms = timer.total_ms();
     rc = spmv_stream_finish(h, stt.max_tile_nnz);
     if (rc != BJ_OK) return fail(rc);
-    if (env_int("BJ_COL16", 0) != 0 && h->stream_ok) {  // NEXT-2, opt-in: 16-bit column deltas for the tile kernel
+    if (o.col16 != 0 && h->stream_ok) {  // NEXT-2, opt-in: 16-bit column deltas for the tile kernel
         rc = col16_build(h);
         if (rc != BJ_OK) return fail(rc);
     }
-    if (env_int("BJ_BSR", 0) != 0) {  // NEXT-2, opt-in: 3x3-blocked copy of the matrix when its structure allows
+    if (o.bsr != 0) {  // NEXT-2, opt-in: 3x3-blocked copy of the matrix when its structure allows
         h->bsr_max_row_nnz = stt.max_row_nnz;
         rc = bsr_build(h);
         if (rc != BJ_OK) return fail(rc);
@@ -364,7 +389,33 @@ int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_
     return BJ_OK;
 }
 
+extern "C" {
+
+int bj_setup_ex(const bj_csr_t* csr, int b, const bj_setup_opts_t* opts, bj_handle_t* out)
+{
+    bj_setup_opts_t o;
+    memset(&o, 0, sizeof(o));
+    if (opts) o = *opts;
+    return setup_impl(csr, b, o, out);
+}
+
+int bj_setup_on_stream(const bj_csr_t* csr, int b, void* cuda_stream, bj_handle_t* out)
+{
+    bj_setup_opts_t o;
+    memset(&o, 0, sizeof(o));
+    o.cuda_stream = cuda_stream;
+    return setup_impl(csr, b, o, out);
+}
+
 int bj_setup(const bj_csr_t* csr, int b, bj_handle_t* out) { return bj_setup_on_stream(csr, b, nullptr, out); }
+
+int bj_get_setup_time(bj_handle_t h, double* kernel_ms, int64_t* alg_bytes)
+{
+    if (!h) return BJ_ERR_INVALID_ARG;
+    if (kernel_ms) *kernel_ms = h->setup_kernel_ms;
+    if (alg_bytes) *alg_bytes = 12 * h->nnz + 4 * (h->n + 1) + h->factor_bytes;
+    return BJ_OK;
+}
 
 int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out)
 {
@@ -415,6 +466,14 @@ int bj_set_option(bj_handle_t h, int option, int value)
         case BJ_OPT_FUSE_FORWARD:
             if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
             h->opt_fuse = value;
+            return BJ_OK;
+        case BJ_OPT_LANCZOS_FUSE:
+            if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
+            h->opt_lanczos_fuse = value;
+            return BJ_OK;
+        case BJ_OPT_PCG_FUSE:
+            if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
+            h->opt_pcg_fuse = value;
             return BJ_OK;
         default: return BJ_ERR_INVALID_ARG;
     }

@@ -1,4 +1,4 @@
-// Banded block factors (opt-in with BJ_BAND=1 at setup), the b > 8 kernels.  (For b <= 8 the
+// Banded block factors (opt-in with bj_setup_opts_t.band), the b > 8 kernels.  (For b <= 8 the
 // same switch compacts tridiagonal blocks inside the existing thread-per-block kernels: see `tri` in bj_api.cu.)
 //
 // When every diagonal block D_k is banded with lower bandwidth w <= 2 (stencil matrices whose blocks follow a grid

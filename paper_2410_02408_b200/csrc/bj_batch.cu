@@ -41,6 +41,25 @@ __device__ __forceinline__ double block_sum_all(double v, double* sh)
     return r;
 }
 
+// The batch entry points treat the matrix as block diagonal with respect to the systems: SpMV and the operator run on the
+// whole matrix while every reduction is per system.  An entry that couples two systems would make every per-system result
+// silently wrong, so each call checks it: CTA s flags any column outside [base_s, base_s + len_s) in the rows of system s
+// (one coalesced pass over the column indices, 4 nnz bytes: microseconds beside the iterations that follow).
+__global__ void __launch_bounds__(kBatchThreads)
+batch_coupling_kernel(int64_t seg_, const int64_t* __restrict__ off, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
+                      int* __restrict__ flag)
+{
+    int64_t base, seg;
+    batch_range(off, seg_, blockIdx.x, base, seg);
+    const int p0 = rp[base], p1 = rp[base + seg];
+    bool bad = false;
+    for (int p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
+        const int64_t c = ci[p];
+        bad |= (c < base) | (c >= base + seg);
+    }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flag, 1);
+}
+
 // v_1 = v0 / ||v0|| per system
 __global__ void __launch_bounds__(kBatchThreads)
 lz_batch_start_kernel(int64_t seg_, const int64_t* __restrict__ off, const double* __restrict__ v0, double* __restrict__ v)
@@ -212,7 +231,15 @@ pcg_batch_update_kernel(int64_t seg_, const int64_t* __restrict__ off, int k, do
     batch_range(off, seg_, s, base, seg);
     double acc = 0.0;
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) acc = fma(p[base + i], q[base + i], acc);
-    const double a = rho[s] / block_sum_all(acc, sh);
+    const double pq = block_sum_all(acc, sh);
+    const double rh = rho[s];
+    if (!(pq > 0.0) || rh == 0.0) {
+        // p.Ap <= 0 (not SPD along p) or r.z = 0 (the residual is exactly zero although rtol = 0 kept the system going):
+        // a = rho / (p.q) would be 0/0 or a step in a wrong direction; freeze the system where it stands
+        if (threadIdx.x == 0) { stopped[s] = 1; converged[s] = rh == 0.0 ? 1 : 0; atomicAdd(nstopped, 1); }
+        return;
+    }
+    const double a = rh / pq;
     acc = 0.0;
     for (int64_t i = threadIdx.x; i < seg; i += blockDim.x) {
         x[base + i] = fma(a, p[base + i], x[base + i]);
@@ -292,6 +319,17 @@ static int batch_layout(bj_handle_s* h, int64_t nsys, const int64_t* offsets_hos
     *off_dev = dst;
     return BJ_OK;
 }
+// BJ_ERR_INVALID_ARG when an entry of the matrix couples two systems of the batch (see batch_coupling_kernel).  Synchronises.
+static int batch_check_decoupled(bj_handle_s* h, int64_t nsys, int64_t seg, const int64_t* off, int* flag_dev)
+{
+    BJ_CUDA(cudaMemsetAsync(flag_dev, 0, sizeof(int), h->stream));
+    batch_coupling_kernel<<<(unsigned)nsys, kBatchThreads, 0, h->stream>>>(seg, off, h->row_ptr, h->col_idx, flag_dev);
+    h->launches++;
+    int bad = 0;
+    BJ_CUDA(cudaMemcpyAsync(&bad, flag_dev, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    BJ_CUDA(cudaStreamSynchronize(h->stream));
+    return bad ? BJ_ERR_INVALID_ARG : BJ_OK;
+}
 }  // namespace bj
 
 using namespace bj;
@@ -322,6 +360,10 @@ extern "C" int bj_pcg_solve_batch(bj_handle_t h, int64_t nsys, const int64_t* of
     double *r = vec, *z = vec + n, *p = vec + 2 * n, *q = vec + 3 * n;
     double *rho = scal, *bb = scal + nsys, *relres = scal + 2 * nsys, *truerel = scal + 3 * nsys;
     int *iters = ints, *stopped = ints + nsys, *converged = ints + 2 * nsys, *nstopped = ints + 3 * nsys;
+    {
+        const int crc = batch_check_decoupled(h, nsys, seg, off, nstopped + 1);
+        if (crc != BJ_OK) return crc;
+    }
     cudaError_t e = cudaMemsetAsync(scal, 0, (size_t)4 * nsys * sizeof(double), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(ints, 0, ((size_t)3 * nsys + 4) * sizeof(int), st);
     if (e != cudaSuccess) { set_cuda_error(e, "batch memset"); cleanup(); return BJ_ERR_CUDA; }
@@ -399,6 +441,10 @@ extern "C" int bj_cond_estimate_batch(bj_handle_t h, int64_t nsys, const int64_t
     {
         const int lrc = batch_layout(h, nsys, offsets_host, (int64_t*)(ws + vec_b + scal_b + int_b), &seg, &off);
         if (lrc != BJ_OK) return lrc;
+    }
+    {
+        const int crc = batch_check_decoupled(h, nsys, seg, off, ints);
+        if (crc != BJ_OK) return crc;
     }
     double* V[2] = {vec, vec + n};
     double* w = vec + 2 * n;

@@ -1,4 +1,4 @@
-// 3x3-blocked storage of the matrix (opt-in with BJ_BSR=1 at setup).
+// 3x3-blocked storage of the matrix (opt-in with bj_setup_opts_t.bsr).
 //
 // A system with three unknowns per node (config 5: 3 dofs per node, 27-point node stencil) has a CSR whose rows come in
 // triples with identical column patterns made of dense 3-column groups.  Stored as BSR(3) a block costs 72 bytes of
@@ -210,7 +210,7 @@ void bsr_free(bj_handle_s* h)
     h->bsr_bytes = 0;
 }
 
-// Called by bj_setup when BJ_BSR=1: checks the structure, builds the copy.  Leaves bsr_ok false (no error) when the
+// Called by bj_setup when opts.bsr is set: checks the structure, builds the copy.  Leaves bsr_ok false (no error) when the
 // matrix is not 3x3-blocked.  Synchronises once.
 int bsr_build(bj_handle_s* h)
 {
@@ -261,7 +261,7 @@ int launch_spmv_bsr(bj_handle_s* h, const double* x, double* y)
     p.stage_bytes = (p.cap * 76 + (p.R + 4) * 4 + 15) & ~15;
     const size_t smem = 128 + (size_t)p.stages * p.stage_bytes;
     const int threads = 32 + 32 * kBsrConsumerWarps;
-    static bool configured[64] = {};
+    static std::atomic<bool> configured[64];
     {
         cudaError_t e = ensure_big_smem(spmv_bsr3_kernel, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_bsr3_kernel)"); return BJ_ERR_CUDA; }

@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace bj {
 
 // streaming (read-once) loads: bypass L1 allocation
@@ -147,45 +149,8 @@ __device__ __forceinline__ double subwarp_block_solve(const double* f, int b, in
     return r;
 }
 
-// Same solve with the block size known at compile time (B <= W): every factor address is the lane's base
-// plus an immediate and the step loop has no branches.  NB independent blocks are solved together: their
-// dependent chains (SHFL -> DFMA per step) interleave, and the step's lane predicate is shared.
-template <int W, int DIR, int B, int NB>
-__device__ __forceinline__ void subwarp_block_solve_ct(const double* const (&f)[NB], int i, double (&r)[NB])
-{
-    static_assert(B >= 2 && B <= W, "block size must fit the sub-warp");
-    const bool in = i < B;
-    const int dslot = DIR == 0 ? i * B - i * (i - 1) / 2 : i * (i + 1) / 2 + i;
-#pragma unroll
-    for (int q = 0; q < NB; ++q) r[q] *= in ? f[q][dslot] : 0.0;
-#pragma unroll
-    for (int jj = 0; jj < B - 1; ++jj) {
-        const int j = DIR == 0 ? jj : B - 1 - jj;
-        const bool on = DIR == 0 ? (i > j && in) : (i < j);
-        const int off = DIR == 0 ? j * B - j * (j - 1) / 2 - j : j * (j + 1) / 2;
-#pragma unroll
-        for (int q = 0; q < NB; ++q) {
-            const double lij = on ? f[q][i + off] : 0.0;
-            const double vj = __shfl_sync(0xffffffffu, r[q], j, W);
-            r[q] = fma(-lij, vj, r[q]);
-        }
-    }
-}
-
-// dispatch: compile-time instance for the block sizes of the paper-shaped workloads, runtime loop otherwise
-template <int W, int DIR, int B, int NB>
-__device__ __forceinline__ void subwarp_solve(const double* const (&f)[NB], int b, int i, double (&r)[NB])
-{
-    if constexpr (B > 0) {
-        subwarp_block_solve_ct<W, DIR, B, NB>(f, i, r);
-    } else {
-#pragma unroll
-        for (int q = 0; q < NB; ++q) r[q] = subwarp_block_solve<W, DIR>(f[q], b, i, r[q]);
-    }
-}
-
 // ---- group-per-block substitution (b = 16, 24, 32): LPB lanes per block, b / LPB rows per lane in registers ----
-// Used by solve_group_kernel (bj_solve_kernels.cu) and by the fused SpMV + forward solve (bj_spmv_kernels.cu).
+// Used by solve_group_kernel (bj_solve_kernels.cu).
 template <int B, int LPB>
 struct GroupGeom {
     static constexpr int P = B * (B + 1) / 2;
@@ -220,30 +185,6 @@ __device__ __forceinline__ void group_forward(const double* f, int l, double (&r
             double lij = col[k * LPB];
             if (k == kj) lij = (l > lj) ? lij : 0.0;
             r[k] = fma(-lij, vj, r[k]);
-        }
-    }
-}
-
-// backward substitution on the staged backward copy (row-major packed lower, columns scaled by 1/l_jj)
-template <int B, int LPB>
-__device__ __forceinline__ void group_backward(const double* f, int l, double (&r)[B / LPB])
-{
-    constexpr int RPL = B / LPB;
-#pragma unroll
-    for (int k = 0; k < RPL; ++k) {
-        const int i = k * LPB + l;
-        r[k] *= f[i * (i + 1) / 2 + i];
-    }
-#pragma unroll
-    for (int j = B - 1; j >= 1; --j) {
-        const int kj = j / LPB, lj = j % LPB;
-        const double vj = __shfl_sync(0xffffffffu, r[kj], lj, LPB);
-        const double* row = f + j * (j + 1) / 2 + l;  // element (j, i) at row[i - l]
-#pragma unroll
-        for (int k = 0; k <= kj; ++k) {
-            if (k == kj && lj == 0) continue;  // no row of this register row lies above j
-            double lji = (k < kj || l < lj) ? row[k * LPB] : 0.0;  // the guard also keeps the read inside row j
-            r[k] = fma(-lji, vj, r[k]);
         }
     }
 }
@@ -290,15 +231,15 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 
 // Opt-in to more than 48 KB of dynamic shared memory, once per kernel AND per device (the attribute is per device).
 template <typename K>
-inline cudaError_t ensure_big_smem(K kernel, bool (&done)[64])
+inline cudaError_t ensure_big_smem(K kernel, std::atomic<bool> (&done)[64])
 {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (done[dev]) return cudaSuccess;
+    if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;  // the attribute call is idempotent: a race only repeats it
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
-    if (e == cudaSuccess) done[dev] = true;
+    if (e == cudaSuccess) done[dev].store(true, std::memory_order_release);
     return e;
 }
 

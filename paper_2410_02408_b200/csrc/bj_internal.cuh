@@ -29,24 +29,22 @@ struct Status {
     unsigned long long compared;  // entries compared
     unsigned long long descents;        // entries with col[p] <= col[p-1]
     unsigned long long legal_descents;  // ... of which at the start of a non-empty row
-    int max_band;                       // largest lower bandwidth of a diagonal block (band_width_kernel, BJ_BAND=1)
+    int max_band;                       // largest lower bandwidth of a diagonal block (band_width_kernel, opts.band)
     int pad2;
 };
 
 // Launch-shape knobs: defaults are the measured best on B200; each can be overridden by the environment variable
-// BJ_<NAME>, read ONCE by bj_setup (sweeps re-run the setup).
+// BJ_<NAME>, read ONCE by bj_setup (sweeps re-run the setup).  They change launch geometry only -- never a storage
+// format or an algorithm (those are bj_setup_opts_t / bj_set_option).
 struct Tuning {
-    int solve_warps = 8, solve_stage_kb = 32, solve_stages = 2, solve_ctas = 4, solve_pair = 1;  // solve_stream_kernel
-    int solve_group = 1, group_stages = 2, group_smem_kb = 220, group_warps = 12, group_lanes = 0;  // solve_group_kernel
-    int serp_keep_mb = 48;  // BJ_SERP_KEEP_MB (0 = off): serpentine walk of the block solves, megabytes of factor kept in L2 per walk
+    int solve_warps = 8, solve_stage_kb = 32, solve_stages = 2, solve_ctas = 4;  // solve_stream_kernel
+    int group_stages = 2, group_smem_kb = 220, group_warps = 12, group_lanes = 0;  // solve_group_kernel
+    int serp_keep_mb = 48;  // bj_setup_opts_t.serp_keep_mb: serpentine walk of the block solves, megabytes of factor kept in L2 per walk
     int pdl_early = 4;      // bit 0: stream solves, bit 1: stream SpMV release their dependents at entry; bit 2 (default): the
                             // plain UNFUSED tile SpMV does (its dependent, the forward solve, then starts on the SMs the SpMV's
                             // tail frees and prefetches its factors: cfg 3 131.8 -> 128.9 us, cfg 4 184.7 -> 182.7; the fused
                             // SpMV + solve kernel measured 0.6 us slower with it and keeps the exit trigger)
     int ctas_per_sm = 4;    // wanted CTAs per SM of the SpMV tile kernel
-    int lanczos_fuse = 1;   // fast-mode Lanczos rides on the operator's kernels
-    int tiny = 0;           // BJ_TINY=1: launch-bound sizes run the whole operator apply in one single-CTA kernel
-                            // (eager 7.2 -> 5.9 us on config 1, but 5.2 vs 3.9 us when replayed from a CUDA graph: off)
 };
 
 struct ProfSpan {
@@ -69,6 +67,7 @@ struct LanczosWs {
     unsigned* lz_ticket = nullptr;
     int lz_cap = 0;
     int cap_iters = 0;
+    size_t cap_partial = 0;  // doubles held in `partial`
     int64_t bytes = 0;
 };
 
@@ -94,13 +93,13 @@ struct bj_handle_s {
     int var_smax = 0;
     int band = -1;       // kind 3: lower bandwidth w of every diagonal block (0..2)
     double* fac_band = nullptr;  // kind 3: aliases the dense factor storage of the slab
-    bool tri = false;    // kind 1 with BJ_BAND=1: every block is (at most) tridiagonal, compact bidiagonal factors, packed = 2b - 1
+    bool tri = false;    // kind 1 with opts.band: every block is (at most) tridiagonal, compact bidiagonal factors, packed = 2b - 1
     int lanes = 0;       // lanes per block for kind 2 (8, 16 or 32)
     int packed = 0;      // b(b+1)/2
     double* fac_small = nullptr;
     double* fac_fwd = nullptr;
     double* fac_bwd = nullptr;   // null when single_copy
-    bool single_copy = false;    // b = 16, 24, 32 with the group kernel: both substitutions run from the forward copy
+    bool single_copy = false;    // b = 16, 24, 32 (group kernel): both substitutions run from the forward copy, the only one kept
     int64_t factor_bytes = 0;
 
     // temporaries
@@ -119,13 +118,16 @@ struct bj_handle_s {
     int spmv_kernel = 0;      // chosen kernel: 0 CSR-vector, 1 TMA tile kernel, 2 BSR(3) copy
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;
+    int opt_lanczos_fuse = -1;  // BJ_OPT_LANCZOS_FUSE / BJ_OPT_PCG_FUSE: 0 selects the unfused iterations
+    int opt_pcg_fuse = -1;
+    bj_setup_opts_t opts = {};  // the options this handle was set up with
+    double setup_kernel_ms = 0.0;  // device time of the setup kernels (bj_get_setup_time)
     int tile_rows = 0;        // rows per tile of the streamed kernel (multiple of b)
     int tile_cap = 0;         // nnz capacity per stage
     int tile_stages = 0;
     int64_t ntiles = 0;
     bool stream_ok = false;   // streamed kernel usable (alignment, capacity)
     bool fuse_ok = false;
-    bool fuse_group = false;  // the fused forward solve is the group-per-block one (b = 16, 24, 32)
     int num_sms = 148;
     bool pdl = true;          // chain the library's kernels with programmatic dependent launch
     bj::Tuning tune;
@@ -138,9 +140,9 @@ struct bj_handle_s {
     double* pcg_scal = nullptr;
     int pcg_cap_iters = 0;
 
-    int16_t* col16 = nullptr;  // opt-in BJ_COL16=1: column stream as 16-bit deltas col - row (owned by the handle)
+    int16_t* col16 = nullptr;  // opt-in (opts.col16): column stream as 16-bit deltas col - row (owned by the handle)
 
-    // BSR(3) copy of the matrix (bj_bsr.cu), opt-in BJ_BSR=1: owned by the handle
+    // BSR(3) copy of the matrix (bj_bsr.cu), opt-in (opts.bsr): owned by the handle
     double* bsr_val = nullptr;
     int32_t* bsr_col = nullptr;
     int32_t* bsr_rp = nullptr;
@@ -210,8 +212,6 @@ int launch_solve_band(bj_handle_s* h, int dir, const double* in, double* out, co
 int launch_solve(bj_handle_s* h, int dir, const double* in, double* out, const LzPrologue* pro = nullptr,
                  const LzEpilogue* epi = nullptr, const PcgHook* pcg = nullptr);  // pcg: dir 2 only (bj_pcg_fuse.cuh)
 bool lanczos_fusable(const bj_handle_s* h);
-bool tiny_op_usable(const bj_handle_s* h);                          // n <= 8192, b <= 8: one-kernel operator apply
-int launch_tiny_op_apply(bj_handle_s* h, const double* x, double* y);  // the handle's solve / SpMV kernels carry the fused Lanczos hooks
 
 // SpMV (bj_spmv_kernels.cu)
 int launch_spmv_vector(bj_handle_s* h, const double* x, double* y);

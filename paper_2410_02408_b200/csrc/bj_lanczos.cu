@@ -63,6 +63,10 @@ scale_kernel(int64_t n, const double* __restrict__ in, double* __restrict__ out,
     pdl_wait();
     if (done[0]) return;
     const double bn = sqrt(reduce_partials(PB, nparts, sh));
+    if (mode == 0 && (!(bn > 0.0) || isinf(bn))) {  // zero or non-finite start vector: invalid argument, nothing is written
+        if (blockIdx.x == 0 && threadIdx.x == 0) { done[0] = 1; done[2] = 1; }
+        return;
+    }
     if (mode == 1) {
         const double a = fabs(alpha[j_prev]);
         const double prev = amax_buf[j_prev & 1];
@@ -258,10 +262,13 @@ void lanczos_free(bj_handle_s* h)
     z = LanczosWs();
 }
 
-static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec)
+static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec, bool reorth)
 {
     LanczosWs& z = h->lz;
-    if (z.cap_vectors >= nvec && z.cap_iters >= iters) return BJ_OK;
+    // partials: two rows for alpha / beta; the reorthogonalisation coefficients need kMaxPartials x (iters + 1) more,
+    // which only the parity mode touches (9.5 KB per iteration: not reserved for fast-mode runs of 10^5 steps)
+    const size_t want_partial = (size_t)kMaxPartials * (reorth ? (size_t)iters + 3 : 2);
+    if (z.cap_vectors >= nvec && z.cap_iters >= iters && z.cap_partial >= want_partial) return BJ_OK;
     lanczos_free(h);
     const size_t vb = (size_t)h->n * sizeof(double);
     int64_t bytes = 0;
@@ -269,7 +276,7 @@ static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec)
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = A((void**)&z.V, vb * nvec);
     if (e == cudaSuccess) e = A((void**)&z.w, vb);
-    if (e == cudaSuccess) e = A((void**)&z.partial, sizeof(double) * kMaxPartials * (size_t)(iters + 3));
+    if (e == cudaSuccess) e = A((void**)&z.partial, sizeof(double) * want_partial);
     if (e == cudaSuccess) e = A((void**)&z.coef, sizeof(double) * (size_t)(iters + 1));
     if (e == cudaSuccess) e = A((void**)&z.alpha, sizeof(double) * (size_t)iters);
     if (e == cudaSuccess) e = A((void**)&z.beta, sizeof(double) * (size_t)iters);
@@ -289,6 +296,7 @@ static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec)
     }
     z.cap_vectors = nvec;
     z.cap_iters = iters;
+    z.cap_partial = want_partial;
     return BJ_OK;
 }
 
@@ -355,7 +363,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     const double tol = o->breakdown_tol > 0.0 ? o->breakdown_tol : BJ_DEFAULT_BREAKDOWN_TOL;
     const int64_t n = h->n;
     const int64_t nvec = reorth ? m : 2;
-    int rc = lanczos_alloc(h, m, nvec);
+    int rc = lanczos_alloc(h, m, nvec, reorth);
     if (rc != BJ_OK) return rc;
     LanczosWs& z = h->lz;
     cudaStream_t st = h->stream;
@@ -388,7 +396,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         if (rc != BJ_OK) return rc;
         v0 = z.w;
     }
-    const bool fused_mode = !reorth && lanczos_fusable(h) && h->tune.lanczos_fuse != 0;
+    const bool fused_mode = !reorth && lanczos_fusable(h) && h->opt_lanczos_fuse != 0;
     if (!fused_mode) BJ_LAUNCH(dot_partial_kernel, G, kReduceThreads, n, v0, v0, PB);
     if (!fused_mode)
         BJ_LAUNCH(scale_kernel, G, kReduceThreads, n, v0, vcol(0), (const double*)PB, G, 0, 0, tol,
@@ -453,6 +461,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     BJ_CUDA(cudaMemcpyAsync(b.data(), z.beta, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
     BJ_CUDA(cudaMemcpyAsync(done, z.done, sizeof(int) * 4, cudaMemcpyDeviceToHost, st));
     BJ_CUDA(cudaStreamSynchronize(st));
+    if (done[2]) return BJ_ERR_INVALID_ARG;  // ||v0|| is zero or not finite
     const int me = done[1];
     if (me < 1) return BJ_ERR_CUDA;
     lanczos_fill_result(me, a.data(), b.data(), res);

@@ -50,7 +50,7 @@ struct LzEpilogue {
     const double* alpha;   // alpha[] (device)
     double* beta;          // beta[]  (device): entry j written by CTA 0
     double* amax;          // two slots, ping-pong: running max |alpha|
-    int* done;             // [0] stop flag, [1] m_eff
+    int* done;             // [0] stop flag, [1] m_eff, [2] invalid start vector
     LzReduce red;          // -> v_{j+1} . w'_new
     double tol;
     int j;                 // step whose beta is being closed (ignored when first)
@@ -86,7 +86,12 @@ __device__ __forceinline__ bool lz_epilogue_begin(const LzEpilogue& e, double& b
     const double s = *e.sum_b;
     beta = sqrt(s > 0.0 ? s : 0.0);
     inv_beta = 1.0 / beta;
-    if (e.first) return false;
+    if (e.first) {
+        // beta_1 = ||v0||: a zero or non-finite start vector is an invalid argument (done[2]), not a breakdown
+        const bool bad = !(beta > 0.0) || isinf(beta);
+        if (bad && blockIdx.x == 0 && threadIdx.x == 0) { e.done[0] = 1; e.done[2] = 1; }
+        return bad;
+    }
     const double a = fabs(e.alpha[e.j]);
     const double prev = e.amax[e.j & 1];
     const double amax = a > prev ? a : prev;

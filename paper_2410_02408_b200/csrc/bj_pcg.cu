@@ -326,7 +326,7 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
 
     int hflags[4] = {0, 0, 0, 0};
     // Fused iteration (bj_pcg_fuse.cuh): needs the tile SpMV (dot hook) and a solve kernel that carries the PCG hook
-    const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && env_int("BJ_PCG_FUSE", 1) != 0;
+    const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && h->opt_pcg_fuse != 0;
     if (fused) {
         unsigned* tickets = reinterpret_cast<unsigned*>(flags + 4);
         LzReduce red_pq{FP, scal + S_PQ, tickets + 0, (int)fcap};
@@ -458,7 +458,7 @@ int mlanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t
     BJ_LAUNCH(G, pcg_pq_kernel, n, (const double*)rcur, (const double*)z, ws.PRa, (const int*)flags);
     BJ_LAUNCH(1, pcg_scalar_kernel, (const double*)ws.PRa, G, bsq, (const int*)flags);  // bt_0^2
 
-    const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && env_int("BJ_PCG_FUSE", 1) != 0;
+    const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && h->opt_pcg_fuse != 0;
     unsigned* tickets = reinterpret_cast<unsigned*>(flags + 4);
     LzReduce red_zp{ws.FP, scal + S_PQ, tickets + 0, (int)fcap};
     PcgHook hook{};

@@ -130,93 +130,12 @@ int launch_spmv_plan(bj_handle_s* h)
     return BJ_OK;
 }
 
-// ------------------------------------------------------------------------------------------------
-// a2 + a3: one warp per diagonal block.
-//   D  : dense b x b tile, leading dimension b+1, warp-private shared memory
-//   rpl: the block's row pointers
-// Left-looking Cholesky in the textbook order: for each column j, s_i = d_ij - sum_{p<j} l_ip l_jp
-// for i >= j, l_jj = sqrt(s_j), l_ij = s_i / l_jj.  Only the lower triangle is read.
-// Rows past the end of a ragged last block are treated as identity rows.
-// Output layouts (diagonal entries stored as RECIPROCALS so the solves multiply instead of divide):
-//   KIND 1 (b <= 8)  fac_small[(k/32) * P * 32 + e * 32 + k % 32],  e = i(i+1)/2 + j  (row-major packed)
-//   KIND 2 (b  > 8)  fac_fwd[k * P + j*b - j(j-1)/2 + (i-j)] = l_ij / l_ii  (column-major packed lower, forward)
-//                    fac_bwd[k * P + i(i+1)/2 + j]           = l_ij / l_jj  (row-major packed lower, backward)
-// ------------------------------------------------------------------------------------------------
-constexpr int kSetupWarps = 4;
-
-template <int KIND>
-__global__ void __launch_bounds__(kSetupWarps * 32)
-extract_factor_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restrict__ rp,
-                      const int32_t* __restrict__ ci, const double* __restrict__ val,
-                      double* __restrict__ out0, double* __restrict__ out1, Status* st)
-{
-    extern __shared__ double smem[];
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    const int ld = b + 1;
-    const int per_warp = b * ld + ((b + 2 + 1) / 2);  // D + rpl (ints packed into doubles)
-    double* D = smem + (size_t)warp * per_warp;
-    int* rpl = reinterpret_cast<int*>(D + b * ld);
-
-    const int64_t k = (int64_t)blockIdx.x * kSetupWarps + warp;
-    if (k >= nblocks) return;
-    const int64_t lo = k * b;
-    const int64_t hi = lo + b < n ? lo + b : n;
-    const int nb = (int)(hi - lo);
-
-    for (int e = lane; e < b * ld; e += 32) D[e] = 0.0;
-    for (int i = lane; i <= nb; i += 32) rpl[i] = rp[lo + i];
-    __syncwarp();
-    for (int i = nb + lane; i < b; i += 32) D[i * ld + i] = 1.0;
-    const int s = rpl[0], e_ = rpl[nb];
-    for (int p = s + lane; p < e_; p += 32) {
-        const int64_t c = ci[p];
-        if (c >= lo && c < hi) {
-            int i = 0;
-            while (i + 1 < nb && rpl[i + 1] <= p) ++i;
-            const int j = (int)(c - lo);
-            if (j <= i) D[i * ld + j] = val[p];
-        }
-    }
-    __syncwarp();
-
-    bool bad = false;
-    for (int j = 0; j < b; ++j) {
-        for (int i = j + lane; i < b; i += 32) {
-            double acc = D[i * ld + j];
-            for (int p = 0; p < j; ++p) acc -= D[i * ld + p] * D[j * ld + p];
-            D[i * ld + j] = acc;
-        }
-        __syncwarp();
-        double sjj = D[j * ld + j];
-        if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
-        const double ljj = sqrt(sjj);
-        __syncwarp();
-        for (int i = j + 1 + lane; i < b; i += 32) D[i * ld + j] = D[i * ld + j] / ljj;
-        if (lane == 0) D[j * ld + j] = ljj;
-        __syncwarp();
-    }
-    if (bad && lane == 0) {
-        atomicOr(&st->flags, ST_NOT_SPD);
-        atomicMin(&st->bad_block, (long long)k);
-    }
-
-    const int P = b * (b + 1) / 2;
-    for (int idx = lane; idx < b * b; idx += 32) {
-        const int i = idx / b, j = idx - i * b;
-        if (j > i) continue;
-        const double v = D[i * ld + j];
-        if (KIND == 1) {
-            out0[(k >> 5) * (int64_t)P * kInterleave + (int64_t)(i * (i + 1) / 2 + j) * kInterleave + (k & 31)] =
-                (i == j) ? 1.0 / v : v;
-        } else {
-            // forward copy: row i scaled by 1/l_ii; backward copy: column j scaled by 1/l_jj
-            out0[k * P + (j * b - j * (j - 1) / 2 + (i - j))] = (i == j) ? 1.0 / v : v / D[i * ld + i];
-            out1[k * P + (i * (i + 1) / 2 + j)] = (i == j) ? 1.0 / v : v / D[j * ld + j];
-        }
-    }
-}
-
+// Output layouts of a2 + a3 (diagonal entries stored as RECIPROCALS so the solves multiply instead of divide):
+//   b <= 8  fac_small[(k/32) * P * 32 + e * 32 + k % 32],  e = i(i+1)/2 + j  (row-major packed, 32 blocks interleaved)
+//   b  > 8  fac_fwd[k * P + j*b - j(j-1)/2 + (i-j)] = l_ij / l_ii  (column-major packed lower, forward copy)
+//           fac_bwd[k * P + i(i+1)/2 + j]           = l_ij / l_jj  (row-major packed lower; not kept for b = 16, 24, 32)
+// Left-looking Cholesky in the textbook order; only the lower triangle is read; rows past the end of a ragged last
+// block are identity rows.
 // ------------------------------------------------------------------------------------------------
 // a2 + a3 for b <= 8: one THREAD per diagonal block, the block in registers (compile-time B).
 // A warp covers 32 consecutive blocks = 32 B consecutive rows, so its CSR reads stay inside one
@@ -286,7 +205,7 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
         atomicMin(&st->bad_block, (long long)k);
     }
     if (tri) {
-        // tridiagonal blocks (BJ_BAND=1): the factor is bidiagonal, only the 2B - 1 elements (i, i-1), (i, i) are kept,
+        // tridiagonal blocks (opts.band): the factor is bidiagonal, only the 2B - 1 elements (i, i-1), (i, i) are kept,
         // element (i, j) at slot i + j
         double* f = fac + (k >> 5) * (int64_t)((2 * B - 1) * kInterleave) + (k & 31);
 #pragma unroll
@@ -404,7 +323,7 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
 }
 
 // ------------------------------------------------------------------------------------------------
-// 16-bit column deltas (opt-in BJ_COL16=1): col - row fits int16 for stencil matrices whose bandwidth
+// 16-bit column deltas (opt-in: bj_setup_opts_t.col16): col - row fits int16 for stencil matrices whose bandwidth
 // is below 32768 (configs 2 and 4); the handle then owns a 2-byte-per-entry copy of the column stream.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
@@ -464,10 +383,7 @@ int col16_build(bj_handle_s* h)
 int launch_extract_factor(bj_handle_s* h)
 {
     const int b = h->b;
-    const int per_warp = b * (b + 1) + ((b + 2 + 1) / 2);
-    const size_t smem = (size_t)kSetupWarps * per_warp * sizeof(double);
-    const int64_t blocks = (h->nblocks + kSetupWarps - 1) / kSetupWarps;
-    if (h->solve_kind == 1 && env_int("BJ_SETUP_WARP", 0) == 0) {
+    if (h->solve_kind == 1) {
         const unsigned tb = (unsigned)((h->nblocks + 127) / 128);
 #define BJ_CASE(B)                                                                                          \
     case B:                                                                                                 \
@@ -480,10 +396,7 @@ int launch_extract_factor(bj_handle_s* h)
             default: return BJ_ERR_INVALID_ARG;
         }
 #undef BJ_CASE
-    } else if (h->solve_kind == 1) {
-        extract_factor_kernel<1><<<(unsigned)blocks, kSetupWarps * 32, smem, h->stream>>>(
-            h->n, b, h->nblocks, h->row_ptr, h->col_idx, h->val, h->fac_small, nullptr, h->status);
-    } else if (env_int("BJ_SETUP_WARP", 0) == 0) {
+    } else {
         const int W = h->lanes;
         const int nsub = 128 / W;
         const size_t sm = (size_t)nsub * W * (W + 1) * sizeof(double);
@@ -494,9 +407,6 @@ int launch_extract_factor(bj_handle_s* h)
         else
             extract_factor_subwarp_kernel<32><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
                                                                           h->val, h->fac_fwd, h->fac_bwd, h->status);
-    } else {
-        extract_factor_kernel<2><<<(unsigned)blocks, kSetupWarps * 32, smem, h->stream>>>(
-            h->n, b, h->nblocks, h->row_ptr, h->col_idx, h->val, h->fac_fwd, h->fac_bwd, h->status);
     }
     h->launches++;
     BJ_CUDA(cudaGetLastError());

@@ -12,6 +12,7 @@
 //            copies (TMA) in a persistent producer/consumer ring, so HBM streaming never waits for
 //            a block's dependent chain.
 #include <algorithm>
+#include <atomic>
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
@@ -220,7 +221,7 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
 }
 
 // ------------------------------------------------------------------------------------------------
-// b > 8: persistent CTAs, factors streamed through a shared-memory ring by the TMA engine.
+// 8 < b <= 32, b not in {16, 24, 32}: persistent CTAs, factors streamed through a shared-memory ring by the TMA engine.
 // A tile is G consecutive blocks; their packed factors are one contiguous byte range, moved by ONE
 // bulk async copy per stage (two when DIR == 2 needs both copies).  Each consumer sub-warp (W = 16
 // or 32 lanes, lane i owns row i) takes blocks of the tile round-robin: its right-hand sides are
@@ -244,7 +245,7 @@ struct SolveStreamParams {
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
 };
 
-template <int W, int DIR, int B, int NB>  // B: compile-time block size, 0 = runtime p.b; NB: blocks a sub-warp solves together
+template <int W, int DIR>
 __global__ void __launch_bounds__(32 + 256, BJ_SOLVE_MINB)
 solve_stream_kernel(const SolveStreamParams p)
 {
@@ -288,7 +289,7 @@ solve_stream_kernel(const SolveStreamParams p)
         const int nsub = (blockDim.x - 32) / W;
         const int sub = ctid / W;
         const int i = ctid & (W - 1);
-        const int b = B > 0 ? B : p.b;
+        const int b = p.b;
         pdl_wait();  // `in` may come from the previous kernel
         // right-hand sides are fetched one tile ahead: their HBM latency hides behind the current tile's solves
         auto fetch_rhs = [&](int64_t tile, double* dst) {
@@ -315,28 +316,17 @@ solve_stream_kernel(const SolveStreamParams p)
             mbar_wait(&full[s], ph);
             const double* f = stage0 + (size_t)s * stage_doubles;
 #pragma unroll
-            for (int q0 = 0; q0 < kMaxBlocksPerSub; q0 += NB) {
-                if (q0 * nsub < p.G) {  // uniform over the CTA
-                    const double* fq[NB];
-                    const double* gq[NB];
-                    double v[NB];
-#pragma unroll
-                    for (int d = 0; d < NB; ++d) {
-                        const int kb = sub + (q0 + d) * nsub;
-                        const int kc = kb < nb ? kb : 0;  // idle sub-warps read block 0 (valid memory), result dropped
-                        fq[d] = f + (size_t)kc * p.P;
-                        gq[d] = fq[d] + p.copy_doubles;
-                        v[d] = r[q0 + d];
-                    }
-                    if (DIR == 0 || DIR == 2) subwarp_solve<W, 0, B, NB>(fq, b, i, v);
-                    if (DIR == 1) subwarp_solve<W, 1, B, NB>(fq, b, i, v);
-                    if (DIR == 2) subwarp_solve<W, 1, B, NB>(gq, b, i, v);
-#pragma unroll
-                    for (int d = 0; d < NB; ++d) {
-                        const int kb = sub + (q0 + d) * nsub;
-                        const int64_t row = (k0 + kb) * b + i;
-                        if (kb < nb && i < b && row < p.n) p.out[row] = v[d];
-                    }
+            for (int q = 0; q < kMaxBlocksPerSub; ++q) {
+                if (q * nsub < p.G) {  // uniform over the CTA
+                    const int kb = sub + q * nsub;
+                    const int kc = kb < nb ? kb : 0;  // idle sub-warps read block 0 (valid memory), result dropped
+                    const double* fq = f + (size_t)kc * p.P;
+                    double v = r[q];
+                    if (DIR == 0 || DIR == 2) v = subwarp_block_solve<W, 0>(fq, b, i, v);
+                    if (DIR == 1) v = subwarp_block_solve<W, 1>(fq, b, i, v);
+                    if (DIR == 2) v = subwarp_block_solve<W, 1>(fq + p.copy_doubles, b, i, v);
+                    const int64_t row = (k0 + kb) * b + i;
+                    if (kb < nb && i < b && row < p.n) p.out[row] = v;
                 }
             }
             __syncwarp();
@@ -358,13 +348,11 @@ solve_stream_kernel(const SolveStreamParams p)
 // ------------------------------------------------------------------------------------------------
 struct GroupParams {
     int64_t n, nblocks, ntiles;  // a tile = the eight consecutive blocks one warp solves together
-    const double* fac0;          // forward copy (DIR 0, 2) or backward copy (DIR 1)
-    const double* fac1;          // backward copy (DIR 2 only)
+    const double* fac0;          // the forward copy: every direction runs from it (group_backward_fwdcopy)
     const double* in;
     double* out;
     int stages;
     int lz;              // 0 plain, 1 Lanczos prologue (DIR 1), 2 Lanczos epilogue (DIR 0), 3 PCG update + apply (DIR 2)
-    int bwd_from_fwd;    // DIR 1: run the backward substitution from the forward copy (fac0 = forward copy)
     int reverse;         // serpentine: this launch walks the tiles from the last to the first (see launch_group_t)
     int64_t keep_from;   // tiles at position >= keep_from of the walk are loaded as ordinary L2 lines instead of evict_first
     LzPrologue pro;
@@ -516,10 +504,7 @@ solve_group_kernel(const GroupParams p)
         mbar_wait(&full[s], ph);
         const double* f = ring + (size_t)s * kStageDoubles + g * Geo::STRIDE;
         if (DIR == 0 || DIR == 2) group_forward<B, LPB>(f, l, r);
-        if (DIR == 1) {
-            if (p.bwd_from_fwd) group_backward_fwdcopy<B, LPB>(f, l, r); else group_backward<B, LPB>(f, l, r);
-        }
-        if (DIR == 2) group_backward_fwdcopy<B, LPB>(f, l, r);
+        if (DIR == 1 || DIR == 2) group_backward_fwdcopy<B, LPB>(f, l, r);
         __syncwarp();
 #pragma unroll
         for (int k = 0; k < RPL; ++k) xchg[g * XB + k * LPB + l] = r[k];
@@ -606,19 +591,19 @@ static int launch_small(bj_handle_s* h, const double* in, double* out, const LzP
     return BJ_OK;
 }
 
-template <int W, int DIR, int B, int NB>
+template <int W, int DIR>
 static int launch_stream_solve(bj_handle_s* h, const SolveStreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
-    static bool configured[64] = {};
+    static std::atomic<bool> configured[64];
     {
-        cudaError_t e = ensure_big_smem(solve_stream_kernel<W, DIR, B, NB>, configured);
+        cudaError_t e = ensure_big_smem(solve_stream_kernel<W, DIR>, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(solve_stream_kernel)"); return BJ_ERR_CUDA; }
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR, B, NB>, threads, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_stream_kernel<W, DIR>, threads, smem);
     const int per_sm = std::max(1, std::min(occ, want_per_sm));
     const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
-    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR, B, NB>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
+    cudaError_t e = launch_kernel(solve_stream_kernel<W, DIR>, grid, threads, smem, h->stream, h->pdl && !h->prof_on, sp);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
 }
@@ -651,18 +636,7 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
     sp.stages = stages;
     const size_t smem = 128 + stages * stage_bytes;
     const int per_sm = h->tune.solve_ctas;
-    const bool pair = bps % 2 == 0 && h->tune.solve_pair != 0;  // two blocks per sub-warp at a time
-    switch (h->b) {  // compile-time instances for the workloads' block sizes
-        case 16: return pair ? launch_stream_solve<16, DIR, 16, 2>(h, sp, per_sm, threads, smem)
-                             : launch_stream_solve<16, DIR, 16, 1>(h, sp, per_sm, threads, smem);
-        case 24: return pair ? launch_stream_solve<32, DIR, 24, 2>(h, sp, per_sm, threads, smem)
-                             : launch_stream_solve<32, DIR, 24, 1>(h, sp, per_sm, threads, smem);
-        case 32: return pair ? launch_stream_solve<32, DIR, 32, 2>(h, sp, per_sm, threads, smem)
-                             : launch_stream_solve<32, DIR, 32, 1>(h, sp, per_sm, threads, smem);
-        default: break;
-    }
-    return W == 16 ? launch_stream_solve<16, DIR, 0, 1>(h, sp, per_sm, threads, smem)
-                   : launch_stream_solve<32, DIR, 0, 1>(h, sp, per_sm, threads, smem);
+    return W == 16 ? launch_stream_solve<16, DIR>(h, sp, per_sm, threads, smem) : launch_stream_solve<32, DIR>(h, sp, per_sm, threads, smem);
 }
 
 template <int B, int LPB, int DIR>
@@ -681,8 +655,8 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     int warps = (int)(budget / (stages * stage_bytes + 64 + xchg_bytes));
     warps = std::max(1, std::min(warps, h->tune.group_warps));
     const size_t smem = (size_t)warps * (64 + xchg_bytes + stages * stage_bytes);
-    static bool configured[64] = {};
-    static bool configured_hook[64] = {};
+    static std::atomic<bool> configured[64];
+    static std::atomic<bool> configured_hook[64];
     {
         cudaError_t e = ensure_big_smem(solve_group_kernel<B, LPB, DIR, 0>, configured);
         if (e == cudaSuccess) e = ensure_big_smem(solve_group_kernel<B, LPB, DIR, (DIR == 1 ? 1 : DIR == 0 ? 2 : 3)>, configured_hook);
@@ -691,9 +665,7 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
     GroupParams gp;
     gp.n = h->n; gp.nblocks = h->nblocks;
     gp.ntiles = (h->nblocks + kGroupBlocksPerWarp - 1) / kGroupBlocksPerWarp;
-    gp.bwd_from_fwd = h->single_copy ? 1 : 0;
-    gp.fac0 = (DIR == 1 && !gp.bwd_from_fwd) ? h->fac_bwd : h->fac_fwd;
-    gp.fac1 = h->fac_bwd;
+    gp.fac0 = h->fac_fwd;
     gp.in = in; gp.out = out; gp.stages = stages;
     // Serpentine walk (BJ_SERP_KEEP_MB > 0): the backward solve walks the factor array from its end to its start and the
     // forward solve from start to end, and the last `keep` megabytes of each walk are loaded as ordinary L2 lines instead
@@ -741,143 +713,7 @@ static int launch_group(bj_handle_s* h, const double* in, double* out, const LzP
 
 static bool use_group_kernel(const bj_handle_s* h)
 {
-    return (h->b == 16 || h->b == 24 || h->b == 32) && h->tune.solve_group != 0 &&
-           (((uintptr_t)h->fac_fwd | (uintptr_t)h->fac_bwd) & 15) == 0 && (h->single_copy || h->fac_bwd != nullptr);
-}
-
-// ------------------------------------------------------------------------------------------------
-// Launch-bound sizes (config 1: N = 1024, 0.15 MB per apply): the WHOLE operator y = L^-1 A L^-T x in ONE kernel of
-// one CTA -- backward block solves into shared memory, barrier, CSR rows out of shared memory, barrier, forward block
-// solves -- instead of two launches.  b <= 8 (thread per block, interleaved factors, same arithmetic and order as
-// solve_small_kernel and the CSR-vector kernel with one lane per row) or b = 0; n <= kTinyMaxN.
-// ------------------------------------------------------------------------------------------------
-constexpr int kTinyMaxN = 8192;
-constexpr int kTinyThreads = 1024;
-
-__global__ void __launch_bounds__(kTinyThreads)
-tiny_op_apply_kernel(int n, int b, int P, int tri, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
-                     const double* __restrict__ val, const double* __restrict__ fac, const double* x, double* y)
-{
-    extern __shared__ double tiny_sm[];
-    double* t = tiny_sm;
-    double* u = tiny_sm + n;
-    pdl_trigger();
-    pdl_wait();
-    const int nblocks = b > 0 ? (n + b - 1) / b : 0;
-    // the thread's first row: bounds and first eight entries, issued now so that their latency hides behind the solves
-    int pre_s = 0, pre_e = 0, pre_c[8];
-    double pre_a[8];
-    if ((int)threadIdx.x < n) {
-        pre_s = rp[threadIdx.x];
-        pre_e = rp[threadIdx.x + 1];
-    }
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        const bool live = pre_s + k < pre_e;
-        pre_c[k] = live ? ci[pre_s + k] : 0;
-        pre_a[k] = live ? val[pre_s + k] : 0.0;
-    }
-    // t = L^-T x
-    if (b == 0) {
-        for (int i = threadIdx.x; i < n; i += blockDim.x) t[i] = x[i];
-    }
-    for (int k = threadIdx.x; k < nblocks; k += blockDim.x) {
-        const double* f = fac + (size_t)(k >> 5) * P * kInterleave + (k & 31);
-        const int lo = k * b;
-        double v[kSmallMax];
-#pragma unroll
-        for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < n) ? x[lo + i] : 0.0;
-#pragma unroll
-        for (int i = kSmallMax - 1; i >= 0; --i) {
-            if (i < b) {
-                double s = v[i];
-                if (tri) {
-                    if (i + 1 < b) s -= f[(2 * i + 1) * kInterleave] * v[i + 1];
-                    v[i] = s * f[(2 * i) * kInterleave];
-                } else {
-#pragma unroll
-                    for (int j = i + 1; j < kSmallMax; ++j)
-                        if (j < b) s -= f[(j * (j + 1) / 2 + i) * kInterleave] * v[j];
-                    v[i] = s * f[(i * (i + 1) / 2 + i) * kInterleave];
-                }
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < kSmallMax; ++i)
-            if (i < b && lo + i < n) t[lo + i] = v[i];
-    }
-    __syncthreads();
-    // u = A t, left to right within a row (the oracle's order); eight entries per round, their loads in flight together;
-    // the first round of the thread's first row was loaded before the barrier (pre_*): it does not depend on t
-    for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        double acc = 0.0;
-        const bool first_row = i == (int)threadIdx.x;
-        const int s0 = first_row ? pre_s : rp[i];
-        const int e = first_row ? pre_e : rp[i + 1];
-        for (int q = s0; q < e; q += 8) {
-            int c[8];
-            double a[8];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const bool live = q + k < e;
-                const bool pre = first_row && q == s0;
-                c[k] = pre ? pre_c[k] : (live ? ci[q + k] : 0);
-                a[k] = pre ? pre_a[k] : (live ? val[q + k] : 0.0);
-            }
-#pragma unroll
-            for (int k = 0; k < 8; ++k) acc = fma(a[k], t[c[k]], acc);  // padded entries: a = 0, c = 0
-        }
-        u[i] = acc;
-    }
-    __syncthreads();
-    // y = L^-1 u
-    if (b == 0) {
-        for (int i = threadIdx.x; i < n; i += blockDim.x) y[i] = u[i];
-    }
-    for (int k = threadIdx.x; k < nblocks; k += blockDim.x) {
-        const double* f = fac + (size_t)(k >> 5) * P * kInterleave + (k & 31);
-        const int lo = k * b;
-        double v[kSmallMax];
-#pragma unroll
-        for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < n) ? u[lo + i] : 0.0;
-#pragma unroll
-        for (int i = 0; i < kSmallMax; ++i) {
-            if (i < b) {
-                double s = v[i];
-                if (tri) {
-                    if (i > 0) s -= f[(2 * i - 1) * kInterleave] * v[i - 1];
-                    v[i] = s * f[(2 * i) * kInterleave];
-                } else {
-#pragma unroll
-                    for (int j = 0; j < i; ++j) s -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
-                    v[i] = s * f[(i * (i + 1) / 2 + i) * kInterleave];
-                }
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < kSmallMax; ++i)
-            if (i < b && lo + i < n) y[lo + i] = v[i];
-    }
-}
-
-bool tiny_op_usable(const bj_handle_s* h)
-{
-    return h->n <= kTinyMaxN && h->solve_kind <= 1 && h->opt_spmv_kernel < 0 && h->opt_fuse < 0 && h->tune.tiny != 0;
-}
-
-int launch_tiny_op_apply(bj_handle_s* h, const double* x, double* y)
-{
-    KernelScope scope(h, h->solve_kind == 0 ? BJ_K_SPMV : BJ_K_SPMV_SOLVE_L);
-    const size_t smem = (size_t)2 * h->n * sizeof(double);
-    static bool configured[64] = {};
-    if (smem > 48 * 1024) {
-        cudaError_t e = ensure_big_smem(tiny_op_apply_kernel, configured);
-        if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(tiny_op_apply_kernel)"); return BJ_ERR_CUDA; }
-    }
-    cudaError_t e = launch_kernel(tiny_op_apply_kernel, 1, kTinyThreads, smem, h->stream, h->pdl && !h->prof_on, (int)h->n, h->b,
-                                  h->packed, h->tri ? 1 : 0, h->row_ptr, h->col_idx, h->val, (const double*)h->fac_small, x, y);
-    if (e != cudaSuccess) { set_cuda_error(e, "tiny_op_apply_kernel launch"); return BJ_ERR_CUDA; }
-    return BJ_OK;
+    return h->single_copy;  // b = 16, 24, 32: one (forward) copy of the factors, group of lanes per block
 }
 
 // kind 1 always carries the hooks; kind 2 only in the group kernel (b = 16, 24, 32); b = 0 has no solve to ride on

@@ -13,6 +13,7 @@
 #include <stdlib.h>
 
 #include <algorithm>
+#include <atomic>
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
@@ -127,25 +128,19 @@ __device__ __forceinline__ void consumer_bar_sync(int nthreads)
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
 
-// LPR lanes per row; BATCH entries per lane in flight per round;
-// FUSE: 0 = SpMV only, 1 = + forward solve, thread per block (b <= 8), 2 = + forward solve, sub-warp of W lanes per block,
-//           (W == 1 with FUSE 1: the blocks are tridiagonal and the factors compact, element (i, j) at slot i + j)
-//       3 = + forward solve, group of lanes per block (bj_device.cuh), W = the compile-time block size (16, 24, 32):
-//           the solving warps rotate from tile to tile and the other warps go on to the next tile meanwhile
+// LPR lanes per row; kBatch entries per lane in flight per round;
+// FUSE: 0 = SpMV only, 1 = + forward solve, thread per block (b <= 8);  TRI (FUSE 1 only): the blocks are tridiagonal and
+//       the factors compact, element (i, j) at slot i + j
 // LZ (compile time, so that the plain operator kernel carries none of it): 0 plain, 1 fused Lanczos epilogue, 2 dot hook,
-// 3 plain with 16-bit column deltas (BJ_COL16=1: the column stream is col - row in int16, 10 bytes per entry instead of 12)
-template <int LPR, int BATCH, int FUSE, int W, int LZ>
+// 3 plain with 16-bit column deltas (opts.col16: the column stream is col - row in int16, 10 bytes per entry instead of 12)
+constexpr int kBatch = 8;
+template <int LPR, int FUSE, bool TRI, int LZ>
 __global__ void __launch_bounds__(kMaxStreamThreads)
 spmv_stream_kernel(const StreamParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
     uint64_t* empty = full + p.stages;
-    // FUSE 3 geometry (unused otherwise): block size GB, GLPB lanes per block, NBW blocks per solving warp
-    constexpr int GB = FUSE == 3 ? W : 32;
-    constexpr int GLPB = GB == 32 ? 8 : 4;
-    using Geo = GroupGeom<GB, GLPB>;
-    constexpr int XB = GB + 2;  // padded block row of the su buffer
     double* su = reinterpret_cast<double*>(smem_raw + 128);               // su_bufs x su_doubles (fused only)
     unsigned char* stage0 = smem_raw + 128 + (size_t)p.su_bufs * p.su_doubles * sizeof(double);
     // per stage: val[cap] | fac[fac_bytes] | col[cap] | rp[rp_ints]
@@ -230,17 +225,6 @@ spmv_stream_kernel(const StreamParams p)
                     fsrc = p.fac + (r0 / p.b / kInterleave) * (int64_t)p.P * kInterleave;
                     bytes += fbytes;
                 }
-                if (FUSE == 2) {
-                    const int nblk = (rows + p.b - 1) / p.b;
-                    fbytes = (uint32_t)(((size_t)nblk * p.P * 8 + 15) & ~(size_t)15);  // factor arrays carry 16 B of slack
-                    fsrc = p.fac + (r0 / p.b) * (int64_t)p.P;
-                    bytes += fbytes;
-                }
-                int gblk = 0;
-                if (FUSE == 3) {
-                    gblk = (rows + GB - 1) / GB;
-                    bytes += (uint32_t)gblk * (uint32_t)(Geo::P * 8);
-                }
                 mbar_expect_tx(&full[s], bytes);
                 if (a1 > a0) {
                     bulk_g2s(dv, p.val + a0, (uint32_t)(a1 - a0) * 8u, &full[s], pol);
@@ -248,11 +232,7 @@ spmv_stream_kernel(const StreamParams p)
                     else bulk_g2s(dc, p.ci + a0, (uint32_t)(a1 - a0) * 4u, &full[s], pol);
                 }
                 if (rq > 0) bulk_g2s(dr, p.rp + r0, (uint32_t)rq * 4u, &full[s], pol);
-                if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], (FUSE == 1 && tile >= p.fac_keep_from) ? pol_keep : pol);
-                if (FUSE == 3)  // one copy per block, padded stride: the groups of a solving warp read different banks
-                    for (int q = 0; q < gblk; ++q)
-                        bulk_g2s(s_fac(s) + (size_t)q * Geo::STRIDE, p.fac + (r0 / GB + q) * (int64_t)Geo::P, (uint32_t)(Geo::P * 8),
-                                 &full[s], pol);
+                if (FUSE && fbytes) bulk_g2s(s_fac(s), fsrc, fbytes, &full[s], tile >= p.fac_keep_from ? pol_keep : pol);
             }
         }
     } else {
@@ -268,7 +248,7 @@ spmv_stream_kernel(const StreamParams p)
             const uint32_t ph = (uint32_t)((it / p.stages) & 1);
             const int64_t r0 = tile * R;
             const int rows = (int)(r0 + R <= p.n ? R : p.n - r0);
-            double* sub_u = su + (size_t)(FUSE == 3 ? it % p.su_bufs : (it & 1)) * p.su_doubles;
+            double* sub_u = su + (size_t)(it & 1) * p.su_doubles;
             mbar_wait(&full[s], ph);
             const double* sv = s_val(s);
             const int* sc = s_col(s);
@@ -283,24 +263,24 @@ spmv_stream_kernel(const StreamParams p)
                 if (valid) {
                     // BATCH entries per lane per round: all their gathers are in flight together
                     const int e = sr[i + 1] - a0;
-                    for (int q = sr[i] - a0 + sub; q < e; q += BATCH * LPR) {
-                        int c[BATCH];
-                        double xv[BATCH], av[BATCH];
+                    for (int q = sr[i] - a0 + sub; q < e; q += kBatch * LPR) {
+                        int c[kBatch];
+                        double xv[kBatch], av[kBatch];
 #pragma unroll
-                        for (int k = 0; k < BATCH; ++k) {
+                        for (int k = 0; k < kBatch; ++k) {
                             const int qq = q + k * LPR;
                             c[k] = C16 ? (int)(r0 + i) + (int)sc16[qq < e ? qq : q] : sc[qq < e ? qq : q];
                         }
 #pragma unroll
-                        for (int k = 0; k < BATCH; ++k)  // predicated: a masked lane costs no L1 wavefront
+                        for (int k = 0; k < kBatch; ++k)  // predicated: a masked lane costs no L1 wavefront
                             xv[k] = (q + k * LPR < e) ? __ldg(p.x + c[k]) : 0.0;
 #pragma unroll
-                        for (int k = 0; k < BATCH; ++k) {
+                        for (int k = 0; k < kBatch; ++k) {
                             const int qq = q + k * LPR;
                             av[k] = qq < e ? sv[qq] : 0.0;
                         }
 #pragma unroll
-                        for (int k = 0; k < BATCH; ++k) acc = fma(av[k], xv[k], acc);
+                        for (int k = 0; k < kBatch; ++k) acc = fma(av[k], xv[k], acc);
                     }
                 }
 #pragma unroll
@@ -309,11 +289,6 @@ spmv_stream_kernel(const StreamParams p)
                     if (FUSE == 1) {
                         const int k = (int)__umulhi((unsigned)i, p.b_magic);
                         sub_u[k * p.bs + (i - k * p.b)] = acc;
-                    } else if (FUSE == 2) {
-                        sub_u[i] = acc;
-                    } else if (FUSE == 3) {
-                        const int kb = i / GB;
-                        sub_u[kb * XB + (i - kb * GB)] = acc;
                     } else {
                         if (LZ == 1) {
                             lz_epilogue_elem(p.epi, beta, inv_beta, r0 + i, acc, pa);
@@ -322,64 +297,6 @@ spmv_stream_kernel(const StreamParams p)
                             p.y[r0 + i] = acc;
                         }
                     }
-                }
-            }
-            if (FUSE == 3) {
-                // (B) forward substitution y = L^-1 u by ROTATING solver warps: group gq (NBW blocks) of tile `it` belongs to
-                // consumer warp (it * ngmax + gq) mod ncw.  The other warps only signal that their rows are in the su
-                // buffer (bar.arrive) and go on to the next tile; a solver waits for all rows (bar.sync), solves, writes y
-                // coalesced, and only then hands the stage back.  The stage ring orders the reuse of the su buffers.
-                constexpr int NBW = Geo::NBW;
-                constexpr int RPL = Geo::RPL;
-                const int ncw = nct >> 5, cw = warp - 1;
-                const int nblk = (rows + GB - 1) / GB;
-                const int ngroups = (nblk + NBW - 1) / NBW;
-                const int ngmax = (R / GB + NBW - 1) / NBW;
-                int myg = -1;
-                for (int gq = 0; gq < ngroups; ++gq)
-                    if ((it * ngmax + gq) % ncw == cw) myg = gq;
-                const int bar_id = 2 + it % p.su_bufs;
-                if (myg < 0) {
-                    asm volatile("bar.arrive %0, %1;" ::"r"(bar_id), "r"(nct) : "memory");
-                } else {
-                    asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nct) : "memory");
-                    const int g = lane / GLPB, l = lane % GLPB;
-                    const int blk0 = myg * NBW;
-                    double* xu = sub_u + (blk0 + g) * XB;
-                    double r[RPL];
-#pragma unroll
-                    for (int k = 0; k < RPL; ++k) r[k] = xu[k * GLPB + l];
-                    group_forward<GB, GLPB>(s_fac(s) + (size_t)(blk0 + g) * Geo::STRIDE, l, r);
-#pragma unroll
-                    for (int k = 0; k < RPL; ++k) xu[k * GLPB + l] = r[k];
-                    __syncwarp();
-#pragma unroll
-                    for (int k = 0; k < RPL; ++k) {
-                        const int e = k * 32 + lane;
-                        const int i = blk0 * GB + e;
-                        if (i < rows) p.y[r0 + i] = sub_u[(blk0 + e / GB) * XB + e % GB];
-                    }
-                }
-            }
-            if (FUSE == 2) {
-                // (B) forward substitution y = L^-1 u, one sub-warp of W lanes per diagonal block
-                consumer_bar_sync(nct);
-                const int b = p.b;
-                const int nblk = (rows + b - 1) / b;
-                const int G = R / b;
-                const int nsub = nct / W;
-                const int sw = ctid / W;
-                const int li = ctid & (W - 1);
-                const double* sf = s_fac(s);
-                for (int q = 0; q * nsub < G; ++q) {
-                    const int kb = sw + q * nsub;
-                    const bool act = kb < nblk;
-                    const int kc = act ? kb : 0;  // idle sub-warps redo block 0, result dropped
-                    const int64_t row = r0 + (int64_t)kc * b + li;
-                    const bool live = act && li < b && row < p.n;
-                    double v = live ? sub_u[kc * b + li] : 0.0;
-                    v = subwarp_block_solve<W, 0>(sf + (size_t)kc * p.P, b, li, v);
-                    if (live) p.y[row] = v;
                 }
             }
             if (FUSE == 1) {
@@ -397,7 +314,7 @@ spmv_stream_kernel(const StreamParams p)
                     double v[kSmallMax];
 #pragma unroll
                     for (int i = 0; i < kSmallMax; ++i) v[i] = (i < b && lo + i < p.n) ? uk[i] : 0.0;
-                    if (FUSE == 1 && W == 1) {  // compact bidiagonal factors (tridiagonal blocks): compile-time variant, W == 1 marks it
+                    if (TRI) {  // compact bidiagonal factors (tridiagonal blocks): compile-time variant
 #pragma unroll
                         for (int i = 0; i < kSmallMax; ++i) {
                             if (i < b) {
@@ -439,19 +356,19 @@ spmv_stream_kernel(const StreamParams p)
     if (LZ == 2) lz_reduce_finish(p.dot_red, pa, lz_sh);
 }
 
-template <int LPR, int BATCH, int FUSE, int W, int LZ = 0>
+template <int LPR, int FUSE, bool TRI, int LZ>
 int launch_stream_t(bj_handle_s* h, const StreamParams& sp, int want_per_sm, int threads, size_t smem)
 {
-    static bool configured[64] = {};
+    static std::atomic<bool> configured[64];
     {
-        cudaError_t e = ensure_big_smem(spmv_stream_kernel<LPR, BATCH, FUSE, W, LZ>, configured);
+        cudaError_t e = ensure_big_smem(spmv_stream_kernel<LPR, FUSE, TRI, LZ>, configured);
         if (e != cudaSuccess) { set_cuda_error(e, "cudaFuncSetAttribute(spmv_stream_kernel)"); return BJ_ERR_CUDA; }
     }
     int occ = 1;  // persistent grid: exactly the CTAs that are resident at once
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_stream_kernel<LPR, BATCH, FUSE, W, LZ>, threads, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, spmv_stream_kernel<LPR, FUSE, TRI, LZ>, threads, smem);
     const int per_sm = std::max(1, std::min(occ, want_per_sm));
     const int grid = (int)std::min<int64_t>(sp.ntiles, (int64_t)h->num_sms * per_sm);
-    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, BATCH, FUSE, W, LZ>, grid, threads, smem, h->stream,
+    cudaError_t e = launch_kernel(spmv_stream_kernel<LPR, FUSE, TRI, LZ>, grid, threads, smem, h->stream,
                                   h->pdl && !h->prof_on, sp);
     if (e != cudaSuccess) { set_cuda_error(e, "spmv_stream_kernel launch"); return BJ_ERR_CUDA; }
     return BJ_OK;
@@ -472,20 +389,9 @@ void fill_layout(const bj_handle_s* h, bool fuse, StreamParams& sp, size_t& smem
     sp.stages = h->tile_stages;
     sp.ntiles = h->ntiles;
     sp.rp_ints = sp.R + 4;
-    const bool group = fuse && h->fuse_group;
-    sp.su_bufs = group ? sp.stages : 2;
-    if (group) {
-        // whole solver groups (NBW blocks of b rows, padded) so that idle lanes stay inside the buffers
-        const int lpb = sp.b == 32 ? 8 : 4, nbw = 32 / lpb;
-        const int pbytes = sp.P * 8, target = (lpb * 8) % 128;
-        const int stride = sp.P + (((target - pbytes % 128) + 128) % 128) / 8;  // GroupGeom<b, lpb>::STRIDE
-        const int slots = ((sp.R / sp.b + nbw - 1) / nbw) * nbw;
-        sp.fac_bytes = slots * stride * 8;
-        sp.su_doubles = slots * (sp.b + 2);
-    } else {
-        sp.fac_bytes = fuse ? (((sp.R / sp.b) * sp.P * 8 + 15) & ~15) : 0;
-        sp.su_doubles = !fuse ? 0 : (h->solve_kind == 1 ? (((sp.R / sp.b) * sp.bs + 1) & ~1) : ((sp.R + 1) & ~1));
-    }
+    sp.su_bufs = 2;
+    sp.fac_bytes = fuse ? (((sp.R / sp.b) * sp.P * 8 + 15) & ~15) : 0;
+    sp.su_doubles = !fuse ? 0 : (((sp.R / sp.b) * sp.bs + 1) & ~1);
     sp.stage_bytes = (sp.cap * (c16 ? 10 : 12) + sp.fac_bytes + sp.rp_ints * 4 + 15) & ~15;
     sp.b_magic = (unsigned)(((1ull << 32) + sp.b - 1) / sp.b);
     smem = 128 + (size_t)sp.su_bufs * sp.su_doubles * 8 + (size_t)sp.stages * sp.stage_bytes;
@@ -526,32 +432,9 @@ int spmv_stream_configure(bj_handle_s* h)
         if (Rf < unit) Rf = unit;
         if ((double)Rf * mean <= 1.6 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
     }
-    h->fuse_group = false;
-    const bool group_ok = h->solve_kind == 2 && (h->b == 16 || h->b == 24 || h->b == 32) && h->stream_lanes <= 4 &&
-                          (((uintptr_t)h->fac_fwd) & 15) == 0 && env_int("BJ_FUSE_GROUP", 0) != 0;
-    if (group_ok) {
-        // fused tiles hold whole solver groups (NBW blocks): the forward solve then rides on the SpMV kernel.
-        // Off by default: measured within 1 % of the unfused kernels on configs 3 and 4 (the stage is held for the
-        // solve, which costs the streaming what the saved u round trip gains).
-        const int unit = h->b * (h->b == 32 ? 4 : 8);
-        int Rf = ((R + unit / 2) / unit) * unit;
-        if (Rf < unit) Rf = unit;
-        if ((double)Rf * mean <= 2.0 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; h->fuse_group = true; }
-    }
-    if (!fuse && h->solve_kind == 2 && env_int("BJ_FUSE_WARP", 0)) {
-        // fused tiles hold whole blocks; with an odd packed size an even block count keeps every tile's factor
-        // range 16-byte aligned; row pointers need the tile start to be a multiple of 4 rows
-        int unit = h->b * ((h->packed % 2) ? 2 : 1);
-        while (unit % 4) unit += h->b * ((h->packed % 2) ? 2 : 1);
-        int Rf = ((R + unit / 2) / unit) * unit;
-        if (Rf < unit) Rf = unit;
-        if ((double)Rf * mean <= 2.0 * target_nnz && Rf <= 1024) { R = Rf; fuse = true; }
-    }
     if (!fuse) R = ((R + 31) / 32) * 32;
     R = env_int("BJ_TILE_ROWS", R);
-    if (fuse && h->solve_kind == 1 && (R % (kInterleave * h->b)) != 0) fuse = false;
-    if (fuse && h->solve_kind == 2 && !h->fuse_group && ((R % h->b) != 0 || (((R / h->b) * h->packed) % 2) != 0)) fuse = false;
-    if (fuse && h->fuse_group && (R % h->b) != 0) { fuse = false; h->fuse_group = false; }
+    if (fuse && (R % (kInterleave * h->b)) != 0) fuse = false;
     if (R % 4) return BJ_OK;
     h->tile_rows = R;
     h->ntiles = (h->n + R - 1) / R;
@@ -593,7 +476,7 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     StreamParams sp;
     size_t smem = 0;
     // 16-bit column deltas: plain operator kernels only (no hooks), thread-per-block fusion or none
-    const bool c16 = h->col16 != nullptr && !epi && !dot_with && (!fuse || h->solve_kind == 1);
+    const bool c16 = h->col16 != nullptr && !epi && !dot_with;
     fill_layout(h, fuse, sp, smem, c16);
     sp.n = h->n; sp.nnz = h->nnz; sp.rp = h->row_ptr; sp.ci = h->col_idx; sp.val = h->val;
     sp.ci16 = h->col16;
@@ -605,11 +488,10 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     sp.dot_red = dot_red ? *dot_red : LzReduce{};
     if (sp.lz == 2 && (fuse || h->num_sms * 4 > dot_red->cap)) return BJ_ERR_INVALID_ARG;
     sp.epi = epi ? *epi : LzEpilogue{};
-    if (epi && (h->solve_kind == 2 && fuse)) return BJ_ERR_INVALID_ARG;  // the b > 8 fused paths have no hook
     if (epi && h->num_sms * 4 > epi->red.cap) return BJ_ERR_INVALID_ARG;
-    sp.fac = !fuse ? nullptr : (h->solve_kind == 1 ? h->fac_small : h->fac_fwd);
+    sp.fac = fuse ? h->fac_small : nullptr;
     sp.fac_keep_from = sp.ntiles;
-    if (fuse && h->solve_kind == 1 && h->tune.serp_keep_mb > 0 && sp.lz == 0) {
+    if (fuse && h->tune.serp_keep_mb > 0 && sp.lz == 0) {
         const int64_t tile_bytes = (int64_t)(sp.R / sp.b) * sp.P * 8;
         sp.fac_keep_from = sp.ntiles - std::min<int64_t>(sp.ntiles, (int64_t)h->tune.serp_keep_mb * 1000000 / tile_bytes);
     }
@@ -618,40 +500,23 @@ int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_for
     int rc = BJ_OK;
     {
         KernelScope scope(h, fuse ? BJ_K_SPMV_SOLVE_L : BJ_K_SPMV);
-        const int mode = !fuse ? 0 : (h->solve_kind == 1 ? 1 : h->fuse_group ? (h->b == 16 ? 4 : h->b == 24 ? 5 : 6) : (h->lanes == 16 ? 2 : 3));
-#define BJ_CASE(L)                                                                               \
-    case L:                                                                                      \
-        rc = mode == 0   ? (sp.lz == 1   ? launch_stream_t<L, 8, 0, 32, 1>(h, sp, grid, threads, smem)  \
-                            : sp.lz == 2 ? launch_stream_t<L, 8, 0, 32, 2>(h, sp, grid, threads, smem)  \
-                            : c16        ? launch_stream_t<L, 8, 0, 32, 3>(h, sp, grid, threads, smem)  \
-                                         : launch_stream_t<L, 8, 0, 32, 0>(h, sp, grid, threads, smem)) \
-             : mode == 1 ? (h->tri ? (sp.lz == 1 ? launch_stream_t<L, 8, 1, 1, 1>(h, sp, grid, threads, smem)    \
-                                      : c16      ? launch_stream_t<L, 8, 1, 1, 3>(h, sp, grid, threads, smem)    \
-                                                 : launch_stream_t<L, 8, 1, 1, 0>(h, sp, grid, threads, smem))   \
-                                   : (sp.lz == 1 ? launch_stream_t<L, 8, 1, 32, 1>(h, sp, grid, threads, smem)   \
-                                      : c16      ? launch_stream_t<L, 8, 1, 32, 3>(h, sp, grid, threads, smem)   \
-                                                 : launch_stream_t<L, 8, 1, 32, 0>(h, sp, grid, threads, smem))) \
-             : mode == 2 ? launch_stream_t<L, 8, 2, 16>(h, sp, grid, threads, smem)               \
-                         : launch_stream_t<L, 8, 2, 32>(h, sp, grid, threads, smem);              \
+#define BJ_CASE(L)                                                                                 \
+    case L:                                                                                        \
+        rc = !fuse    ? (sp.lz == 1   ? launch_stream_t<L, 0, false, 1>(h, sp, grid, threads, smem)  \
+                         : sp.lz == 2 ? launch_stream_t<L, 0, false, 2>(h, sp, grid, threads, smem)  \
+                         : c16        ? launch_stream_t<L, 0, false, 3>(h, sp, grid, threads, smem)  \
+                                      : launch_stream_t<L, 0, false, 0>(h, sp, grid, threads, smem)) \
+             : h->tri ? (sp.lz == 1   ? launch_stream_t<L, 1, true, 1>(h, sp, grid, threads, smem)   \
+                         : c16        ? launch_stream_t<L, 1, true, 3>(h, sp, grid, threads, smem)   \
+                                      : launch_stream_t<L, 1, true, 0>(h, sp, grid, threads, smem))  \
+                      : (sp.lz == 1   ? launch_stream_t<L, 1, false, 1>(h, sp, grid, threads, smem)  \
+                         : c16        ? launch_stream_t<L, 1, false, 3>(h, sp, grid, threads, smem)  \
+                                      : launch_stream_t<L, 1, false, 0>(h, sp, grid, threads, smem)); \
         break;
-#define BJ_GCASE(L)                                                                              \
-    case L:                                                                                      \
-        rc = mode == 4   ? launch_stream_t<L, 8, 3, 16>(h, sp, grid, threads, smem)               \
-             : mode == 5 ? launch_stream_t<L, 8, 3, 24>(h, sp, grid, threads, smem)               \
-                         : launch_stream_t<L, 8, 3, 32>(h, sp, grid, threads, smem);              \
-        break;
-        if (mode >= 4) {
-            switch (h->stream_lanes) {
-                BJ_GCASE(1) BJ_GCASE(2) BJ_GCASE(4)
-                default: rc = BJ_ERR_INVALID_ARG;
-            }
-        } else {
-            switch (h->stream_lanes) {
-                BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
-                default: rc = BJ_ERR_INVALID_ARG;
-            }
+        switch (h->stream_lanes) {
+            BJ_CASE(1) BJ_CASE(2) BJ_CASE(4) BJ_CASE(8) BJ_CASE(16) BJ_CASE(32)
+            default: rc = BJ_ERR_INVALID_ARG;
         }
-#undef BJ_GCASE
 #undef BJ_CASE
     }
     if (rc != BJ_OK) return rc;

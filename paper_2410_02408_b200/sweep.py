@@ -3,7 +3,8 @@
 Stands in for the paper's ML tuner, which predicts a block size from (matrix size, sparsity)
 (sec 4.5): for each candidate b it runs the real path -- bj_setup, timed
 bj_op_apply, bj_cond_estimate_ex -- and picks the b that minimises the predicted HHL cost
-kappa_est(b)^2 (the paper's O(log n_b kappa^2)), ties broken by the cheaper apply.
+kappa_est(b)^2 (the paper's O(log n_b kappa^2)), ties (kappa within 1 % relative) broken by the
+cheaper apply (`pick_best`).
 Everything runs through the C ABI; nothing here touches the oracle.
 
     python -m paper_2410_02408_b200.sweep --config 2 [--scale full] [--iters 50] [--long-iters 0] [--pcg-rtol 1e-3]
@@ -15,6 +16,19 @@ import json
 import time
 
 DEFAULT_BLOCKS = (1, 2, 3, 4, 8, 16, 24, 32)
+TIE_REL = 0.01  # kappa estimates within 1 % of the smallest count as tied
+
+
+def pick_best(rows, key: str = "kappa_est", tie_rel: float = TIE_REL):
+    """a11's selection rule: minimise the predicted HHL cost kappa_est^2; candidates whose
+    kappa_est is within a RELATIVE `tie_rel` of the smallest are tied and the cheapest operator apply among them wins
+    (then the smaller b).  Rows with an "error" key are ignored.  Returns the winning row, or None."""
+    ok = [r for r in rows if "error" not in r]
+    if not ok:
+        return None
+    kmin = min(r[key] for r in ok)
+    tied = [r for r in ok if r[key] <= kmin * (1.0 + tie_rel)]
+    return min(tied, key=lambda r: (r["op_apply_us"], r["b"]))
 
 
 def sweep(rp, ci, val, blocks=DEFAULT_BLOCKS, iters: int = 50, reorth: bool = True, apply_steps: int = 200,
@@ -77,12 +91,11 @@ def sweep(rp, ci, val, blocks=DEFAULT_BLOCKS, iters: int = 50, reorth: bool = Tr
                         "pcg_true_relres": pr["true_relres"]})
         out["rows"].append(row)
         B.bj_destroy(h)
-    ok = [r for r in out["rows"] if "error" not in r]
-    if ok:
-        key = "kappa_est_long" if long_iters else "kappa_est"
-        best = min(ok, key=lambda r: (round(r[key] ** 2, 6), r["op_apply_us"]))
+    key = "kappa_est_long" if long_iters else "kappa_est"
+    best = pick_best(out["rows"], key)
+    if best is not None:
         out["best_b"] = best["b"]
-        out["criterion"] = f"argmin {key}^2, ties -> cheaper apply"
+        out["criterion"] = f"argmin {key}^2, ties (within {TIE_REL:.0%} relative) -> cheaper apply"
     return out
 
 

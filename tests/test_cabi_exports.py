@@ -28,6 +28,9 @@ def test_library_builds_and_exports_every_declared_symbol():
     for name in declared_symbols():
         assert hasattr(lib, name), f"{name} declared in include/bj.h but not exported"
     assert sorted(binding.EXPORTS) == declared_symbols()
+    L = binding.lib()
+    for name in binding.EXPORTS:      # every entry point has its argument types declared (a bare int would pass as 32 bits)
+        assert getattr(L, name).argtypes is not None, f"{name}: argtypes not set in binding.lib()"
     assert binding.lib().bj_strerror(0) == b"ok"
     assert binding.BJ_B_MAX == int(re.search(r"#define BJ_B_MAX (\d+)", open(os.path.join(ROOT, "include", "bj.h")).read()).group(1))
 

@@ -43,8 +43,8 @@ def dev(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def check_all_ops(B, torch, A, b, rel, seeds=(101, 202), tol=TOL_APPLY, kernels=(None,)):
-    h, keep = B.setup_from_host(A, b)
+def check_all_ops(B, torch, A, b, rel, seeds=(101, 202), tol=TOL_APPLY, kernels=(None,), **opts):
+    h, keep = B.setup_from_host(A, b, **opts)
     try:
         P = oracle.Precond(A, b)
         for kern in kernels:
@@ -170,6 +170,26 @@ def test_breakdown_is_not_an_error(B, torch_, rel):
         B.bj_destroy(h)
 
 
+def test_zero_or_nonfinite_start_vector_is_an_invalid_argument(B, torch_):
+    """beta_1 = ||v0|| = 0 (or NaN / inf) is not a breakdown: every estimator rejects it, fused and unfused alike."""
+    A = mat(2, "small")
+    z = torch_.zeros(A.n, dtype=torch_.float64, device="cuda")
+    nan = z.clone()
+    nan[5] = float("nan")
+    for b in (0, 8, 16, 12):              # no solve / thread-per-block / group / stream solve (unfused only)
+        h, keep = B.setup_from_host(A, b)
+        for fuse in (1, 0):
+            B.bj_set_option(h, B.BJ_OPT_LANCZOS_FUSE, fuse)
+            for v0 in (z, nan):
+                for reorth in (False, True):
+                    with pytest.raises(B.BJError) as e:
+                        B.bj_cond_estimate_ex(h, 10, reorth=reorth, v0=v0)
+                    assert e.value.code == B.BJ_ERR_INVALID_ARG, (b, fuse, reorth)
+            g = B.bj_cond_estimate_ex(h, 10, reorth=False)      # the handle is still usable afterwards
+            assert g["iters_done"] == 10 and np.isfinite(g["kappa"])
+        B.bj_destroy(h)
+
+
 def test_point_jacobi_is_the_papers_kernel(B, torch_):
     """PAPER.md:234: M[idx] = 1/A[idx*N+idx]."""
     A = mat(1, "full")
@@ -228,6 +248,36 @@ def test_error_codes(B, torch_):
     info = B.bj_get_info(h)
     assert info["n"] == A.n and info["nnz"] == A.nnz and info["b"] == 4 and info["nblocks"] == 256 and info["bad_block"] == -1
     B.bj_destroy(h)
+
+
+def test_setup_options_are_per_handle_arguments(B, torch_, rel):
+    """bj_setup_ex: storage variants are arguments of the call, not process state -- handles of one process differ."""
+    import ctypes as C
+    A = mat(4, "small")
+    rp, ci, val = dev(torch_, A.row_ptr), dev(torch_, A.col_idx), dev(torch_, A.val)
+    hs = {"default": B.bj_setup(rp, ci, val, 16), "band": B.bj_setup(rp, ci, val, 16, band=1),
+          "col16": B.bj_setup(rp, ci, val, 16, col16=1), "both": B.bj_setup(rp, ci, val, 16, band=1, col16=1)}
+    infos = {k: B.bj_get_info(h) for k, h in hs.items()}
+    assert [infos[k]["band_width"] for k in ("default", "band", "col16", "both")] == [-1, 1, -1, 1]
+    assert [infos[k]["col16"] for k in ("default", "band", "col16", "both")] == [0, 0, 1, 1]
+    assert infos["band"]["factor_bytes"] < infos["default"]["factor_bytes"]
+    x = W.seeded_vector(12, A.n)
+    ref = oracle.Precond(A, 16).op_apply(x)
+    for k, h in hs.items():       # interleaved use of all four
+        e2, ei = rel(B.bj_op_apply(h, dev(torch_, x)).cpu().numpy(), ref)
+        assert e2 <= TOL_APPLY and ei <= TOL_APPLY, k
+        t = B.bj_get_setup_time(h)
+        assert t["kernel_ms"] > 0 and t["algorithmic_bytes"] == 12 * A.nnz + 4 * (A.n + 1) + infos[k]["factor_bytes"]
+    for h in hs.values():
+        B.bj_destroy(h)
+    # a non-zero reserved field is rejected; NULL options are the defaults
+    csr = B.bj_csr_t(A.n, A.nnz, rp.data_ptr(), ci.data_ptr(), val.data_ptr())
+    o = B.bj_setup_opts_t()
+    o.reserved[3] = 1
+    out = C.c_void_p()
+    assert B.lib().bj_setup_ex(C.byref(csr), 16, C.byref(o), C.byref(out)) == B.BJ_ERR_INVALID_ARG and not out.value
+    assert B.lib().bj_setup_ex(C.byref(csr), 16, None, C.byref(out)) == B.BJ_OK
+    B.lib().bj_destroy(out)
 
 
 def test_tiny_and_degenerate_shapes(B, torch_, rel):
@@ -297,37 +347,6 @@ def test_runs_on_a_side_stream_and_profiling_counts(B, torch_, rel):
     B.bj_destroy(h)
 
 
-def test_fused_subwarp_forward_solve_path(B, torch_, rel, monkeypatch):
-    """The SpMV tile kernel can also run the b > 8 forward solve in its epilogue (off by default: not faster yet)."""
-    monkeypatch.setenv("BJ_FUSE_WARP", "1")
-    for cfg, b in ((4, 16), (3, 32), (5, 24), (2, 12)):
-        A = mat(cfg, "small")
-        h, keep = B.setup_from_host(A, b)
-        assert B.bj_get_info(h)["fused_forward"] == 1
-        B.bj_destroy(h)
-        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
-
-
-def test_single_kernel_operator_apply_for_tiny_sizes(B, torch_, rel, monkeypatch):
-    """BJ_TINY=1: n <= 8192 and b <= 8 run the whole operator in one single-CTA kernel (off by default: faster eagerly,
-    slower than the two PDL-chained kernels when replayed from a CUDA graph)."""
-    monkeypatch.setenv("BJ_TINY", "1")
-    for cfg, bs in ((1, (0, 1, 4, 7)), (5, (3, 8))):
-        A = mat(cfg, "small")
-        for b in bs:
-            h, keep = B.setup_from_host(A, b)
-            launches0 = B.bj_get_info(h)["kernel_launches"]
-            x = W.seeded_vector(11, A.n)
-            y = B.bj_op_apply(h, dev(torch_, x))
-            assert B.bj_get_info(h)["kernel_launches"] == launches0 + 1      # one kernel, not two or three
-            e2, ei = rel(y.cpu().numpy(), oracle.Precond(A, b).op_apply(x))
-            assert e2 <= TOL_APPLY and ei <= TOL_APPLY, (cfg, b, e2, ei)
-            z = dev(torch_, x).clone()
-            B.bj_op_apply(h, z, z)                                            # in place
-            assert np.array_equal(z.cpu().numpy(), y.cpu().numpy())
-            B.bj_destroy(h)
-
-
 def test_operator_apply_replays_from_a_cuda_graph(B, torch_, rel):
     """The library's launches (PDL-chained) can be captured on a side stream and replayed: bitwise the eager result."""
     for cfg, b in ((1, 4), (4, 16)):
@@ -356,31 +375,18 @@ def test_operator_apply_replays_from_a_cuda_graph(B, torch_, rel):
         B.bj_destroy(h)
 
 
-def test_fused_group_forward_solve_path(B, torch_, rel, monkeypatch):
-    """b = 16 / 24 / 32: the group-per-block forward solve can ride on the SpMV tile kernel with rotating solver warps
-    (off by default: within 1 % of the unfused kernels)."""
-    monkeypatch.setenv("BJ_FUSE_GROUP", "1")
-    for cfg, b in ((4, 16), (3, 32), (2, 24), (1, 16)):
-        A = mat(cfg, "small")
-        h, keep = B.setup_from_host(A, b)
-        assert B.bj_get_info(h)["fused_forward"] == 1
-        B.bj_destroy(h)
-        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 1),))
-
-
-def test_banded_factor_path(B, torch_, rel, monkeypatch):
-    """SURVEY 8(f) NEXT-2, opt-in (BJ_BAND=1): when every diagonal block is banded (w <= 2) the factor keeps the band and
+def test_banded_factor_path(B, torch_, rel):
+    """SURVEY 8(f) NEXT-2, opt-in (bj_setup_opts_t.band): when every diagonal block is banded (w <= 2) the factor keeps the band and
     only (w+1) b doubles per block are stored and streamed.  Same parity bar as the dense-packed path; blocks that are
     not banded fall back to it."""
     import scipy.sparse as sp
-    monkeypatch.setenv("BJ_BAND", "1")
     n = 5000
     T = sp.diags([-np.ones(n - 1), 2.5 * np.ones(n), -np.ones(n - 1)], [-1, 0, 1], format="csr")
     penta = W.from_scipy((T @ T).tocsr(), {"name": "pentadiagonal"})        # w = 2 inside every block
     cases = [(mat(4, "small"), 16, 1), (mat(2, "small"), 16, 1), (mat(4, "small"), 32, 1), (penta, 24, 2), (penta, 9, 2),
              (W.block_diagonal_spd(2000, 1), 16, 0), (mat(3, "small"), 32, None), (mat(5, "small"), 24, None)]
     for A, b, w in cases:
-        h, keep = B.setup_from_host(A, b)
+        h, keep = B.setup_from_host(A, b, band=1)
         info = B.bj_get_info(h)
         if w is None:
             assert info["solve_kernel"] == 2 and info["band_width"] == -1     # not banded: dense packed factors
@@ -388,8 +394,8 @@ def test_banded_factor_path(B, torch_, rel, monkeypatch):
             assert info["solve_kernel"] == 3 and info["band_width"] == w, (b, info)
             assert info["factor_bytes"] < 8 * A.n * (w + 1) + 8 * 32 * (w + 1) * b + 1
         B.bj_destroy(h)
-        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 0),))
-        h, keep = B.setup_from_host(A, b)
+        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=((1, 0),), band=1)
+        h, keep = B.setup_from_host(A, b, band=1)
         P = oracle.Precond(A, b)
         g = B.bj_cond_estimate_ex(h, 20, reorth=True)
         c = P.cond_estimate(20, reorth=True)
@@ -410,21 +416,20 @@ def test_banded_factor_path(B, torch_, rel, monkeypatch):
     bad = sp.diags([-np.ones(n - 1), np.r_[2.5 * np.ones(n - 40), -1.0, 2.5 * np.ones(39)], -np.ones(n - 1)], [-1, 0, 1], format="csr")
     Ab = W.from_scipy(bad, {"name": "indefinite tridiagonal"})
     with pytest.raises(B.BJError) as ei:
-        B.setup_from_host(Ab, 16)
+        B.setup_from_host(Ab, 16, band=1)
     assert ei.value.code == B.BJ_ERR_NOT_SPD and ei.value.bad_block == (n - 40) // 16
 
 
-def test_tridiagonal_compact_factors_small_blocks(B, torch_, rel, monkeypatch):
-    """BJ_BAND=1 with b <= 8: tridiagonal blocks keep 2b - 1 factor elements; the same kernels run (thread per block,
+def test_tridiagonal_compact_factors_small_blocks(B, torch_, rel):
+    """bj_setup_opts_t.band with b <= 8: tridiagonal blocks keep 2b - 1 factor elements; the same kernels run (thread per block,
     fused SpMV + solve, fused Lanczos and PCG hooks) with a compact index map."""
     import scipy.sparse as sp
-    monkeypatch.setenv("BJ_BAND", "1")
     n = 3001
     T = sp.diags([-np.ones(n - 1), 2.5 * np.ones(n), -np.ones(n - 1)], [-1, 0, 1], format="csr")
     penta = W.from_scipy((T @ T).tocsr(), {"name": "pentadiagonal"})
     for A, b, tri in ((mat(2, "small"), 8, True), (mat(4, "small"), 8, True), (mat(1, "small"), 4, True),
                       (mat(2, "small"), 5, True), (penta, 8, False), (mat(5, "small"), 3, False)):
-        h, keep = B.setup_from_host(A, b)
+        h, keep = B.setup_from_host(A, b, band=1)
         info = B.bj_get_info(h)
         assert info["solve_kernel"] == 1
         assert (info["band_width"] == 1) == tri, (b, info)
@@ -439,7 +444,7 @@ def test_tridiagonal_compact_factors_small_blocks(B, torch_, rel, monkeypatch):
         cp = P.pcg(rhs, 8, 0.0)
         assert np.allclose(gp["alpha"], cp["alpha"], rtol=1e-9, atol=0)
         B.bj_destroy(h)
-        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=KERNELS)
+        check_all_ops(B, torch_, A, b, rel, seeds=(3,), kernels=KERNELS, band=1)
 
 
 def test_batched_small_systems(B, torch_, rel):
@@ -505,6 +510,24 @@ def test_batched_small_systems(B, torch_, rel):
     with pytest.raises(B.BJError):
         B.bj_cond_estimate_batch(h, ns, 5, offsets=np.r_[0, off[1] + 2, off[2:]])      # ... and fall on block boundaries
     B.bj_destroy(h)
+    # a matrix with an entry that couples two systems is rejected (every per-system result would be silently wrong)
+    h, keep = B.setup_from_host(mat(1, "full"), 4)
+    with pytest.raises(B.BJError) as e:
+        B.bj_cond_estimate_batch(h, 2, 5)                  # one 32 x 32 grid cut in two halves: rows 15 | 16 are coupled
+    assert e.value.code == B.BJ_ERR_INVALID_ARG
+    with pytest.raises(B.BJError) as e:
+        B.bj_pcg_solve_batch(h, 2, dev(torch_, W.seeded_vector(3, 1024)), max_iters=5, rtol=0.0)
+    assert e.value.code == B.BJ_ERR_INVALID_ARG
+    B.bj_destroy(h)
+    # a system whose residual becomes EXACTLY zero while the stopping test cannot fire (rtol < 0) is frozen where it stands
+    # instead of taking the step length 0 / 0: A = 2 I, b = 1 makes every quantity of step 1 exact (a = 1, r = 0)
+    nd = 64
+    Ad = W.CSR(nd, np.arange(nd + 1, dtype=np.int32), np.arange(nd, dtype=np.int32), np.full(nd, 2.0))
+    h, keep = B.setup_from_host(Ad, 1)
+    rhs = W.seeded_vector(4, nd)
+    g = B.bj_pcg_solve_batch(h, 4, dev(torch_, rhs), max_iters=6, rtol=-1.0)
+    assert np.array_equal(g["x"].cpu().numpy(), rhs / 2.0) and (g["iters"] == 1).all() and (g["true_relres"] == 0.0).all()
+    B.bj_destroy(h)
     # a system whose preconditioner is exact breaks down at step 1 while the others go on
     Ab = W.block_diagonal_spd(64, 8)
     h, keep = B.setup_from_host(Ab, 8)
@@ -515,19 +538,17 @@ def test_batched_small_systems(B, torch_, rel):
     B.bj_destroy(h)
 
 
-def test_16_bit_column_deltas(B, torch_, rel, monkeypatch):
-    """SURVEY 8(f) NEXT-2, opt-in (BJ_COL16=1): when every |col - row| < 32768 the tile kernel streams the columns as
+def test_16_bit_column_deltas(B, torch_, rel):
+    """SURVEY 8(f) NEXT-2, opt-in (bj_setup_opts_t.col16): when every |col - row| < 32768 the tile kernel streams the columns as
     int16 deltas (10 bytes per entry instead of 12); bit-identical products (same values, same order)."""
     for cfg, b in ((2, 8), (4, 8), (1, 4), (3, 4), (4, 16), (5, 3)):
         A = mat(cfg, "small")
         x = dev(torch_, W.seeded_vector(6, A.n))
-        monkeypatch.delenv("BJ_COL16", raising=False)
-        h, keep = B.setup_from_host(A, b)
-        ref_spmv, ref_op = B.bj_spmv(h, x).clone(), B.bj_op_apply(h, x).clone()
-        B.bj_destroy(h)
-        monkeypatch.setenv("BJ_COL16", "1")
-        h, keep = B.setup_from_host(A, b)
-        assert B.bj_get_info(h)["col16"] == 1
+        h_ref, keep_ref = B.setup_from_host(A, b)
+        h, keep = B.setup_from_host(A, b, col16=1)          # two handles of one process, different options
+        assert B.bj_get_info(h)["col16"] == 1 and B.bj_get_info(h_ref)["col16"] == 0
+        ref_spmv, ref_op = B.bj_spmv(h_ref, x).clone(), B.bj_op_apply(h_ref, x).clone()
+        B.bj_destroy(h_ref)
         assert np.array_equal(B.bj_spmv(h, x).cpu().numpy(), ref_spmv.cpu().numpy())
         assert np.array_equal(B.bj_op_apply(h, x).cpu().numpy(), ref_op.cpu().numpy())
         P = oracle.Precond(A, b)
@@ -538,20 +559,19 @@ def test_16_bit_column_deltas(B, torch_, rel, monkeypatch):
     import scipy.sparse as sp
     n = 70000
     far = sp.diags([np.full(n, 4.0), np.full(n - 40000, -1.0), np.full(n - 40000, -1.0)], [0, 40000, -40000], format="csr")
-    h, keep = B.setup_from_host(W.from_scipy(far), 4)
+    h, keep = B.setup_from_host(W.from_scipy(far), 4, col16=1)
     assert B.bj_get_info(h)["col16"] == 0
     B.bj_destroy(h)
-    check_all_ops(B, torch_, mat(2, "small"), 8, rel, seeds=(3,), kernels=KERNELS)
+    check_all_ops(B, torch_, mat(2, "small"), 8, rel, seeds=(3,), kernels=KERNELS, col16=1)
 
 
-def test_bsr3_matrix_copy(B, torch_, rel, monkeypatch):
-    """SURVEY 8(f) NEXT-2, opt-in (BJ_BSR=1): a 3x3-blocked matrix (config 5: three dofs per node) is also kept as BSR(3)
+def test_bsr3_matrix_copy(B, torch_, rel):
+    """SURVEY 8(f) NEXT-2, opt-in (bj_setup_opts_t.bsr): a 3x3-blocked matrix (config 5: three dofs per node) is also kept as BSR(3)
     -- 8.44 bytes per entry instead of 12 -- and every product of the path runs from that copy; a matrix without the block
     structure keeps the CSR kernels."""
-    monkeypatch.setenv("BJ_BSR", "1")
     A = mat(5, "small")
     for b in (0, 3, 24, 6):
-        h, keep = B.setup_from_host(A, b)
+        h, keep = B.setup_from_host(A, b, bsr=1)
         assert B.bj_get_info(h)["spmv_kernel"] == 2
         P = oracle.Precond(A, b)
         for seed in (3, 4):
@@ -575,15 +595,15 @@ def test_bsr3_matrix_copy(B, torch_, rel, monkeypatch):
         assert B.bj_get_info(h)["spmv_kernel"] in (0, 1)
         B.bj_destroy(h)
     for cfg in (2, 3):                                         # no 3x3 block structure: CSR kernels
-        h, keep = B.setup_from_host(mat(cfg, "small"), 3)
+        h, keep = B.setup_from_host(mat(cfg, "small"), 3, bsr=1)
         assert B.bj_get_info(h)["spmv_kernel"] in (0, 1)
         B.bj_destroy(h)
     # a matrix whose size and entry count are multiples of 3 and 9 but whose pattern is not blocked
-    h, keep = B.setup_from_host(W.block_diagonal_spd(27, 9), 3)
+    h, keep = B.setup_from_host(W.block_diagonal_spd(27, 9), 3, bsr=1)
     info = B.bj_get_info(h)
     B.bj_destroy(h)
     assert info["spmv_kernel"] == 2                            # 9x9 dense blocks ARE 3x3-blocked
-    h, keep = B.setup_from_host(W.laplacian((9, 9, 9)), 3)
+    h, keep = B.setup_from_host(W.laplacian((9, 9, 9)), 3, bsr=1)
     assert B.bj_get_info(h)["spmv_kernel"] in (0, 1)
     B.bj_destroy(h)
 
@@ -601,7 +621,7 @@ def test_block_size_sweep_runs_the_real_path(B, torch_):
         assert r["applies_per_s"] > 0 and r["setup_ms"] > 0
     c0 = oracle.Precond(A, 0).cond_estimate(50)
     assert abs(res["kappa_A"]["kappa_est"] / c0["kappa"] - 1) <= TOL_KAPPA
-    assert res["best_b"] == min(res["rows"], key=lambda r: r["kappa_est"])["b"]
+    assert res["best_b"] == sweep.pick_best(res["rows"])["b"]
 
 
 # ------------------------------------------------------------------ BASELINE.json full sizes -------------
@@ -697,16 +717,16 @@ def test_pcg_matches_oracle_small(B, torch_, rel, cfg):
         B.bj_destroy(h)
 
 
-@pytest.mark.parametrize("fuse", ["0", "1"])
-def test_pcg_fused_and_unfused_iterations_agree(B, torch_, rel, monkeypatch, fuse):
-    """BJ_PCG_FUSE=0 runs the seven-kernel iteration of bj_pcg.cu, the default rides on the SpMV and solve kernels
+@pytest.mark.parametrize("fuse", [0, 1])
+def test_pcg_fused_and_unfused_iterations_agree(B, torch_, rel, fuse):
+    """BJ_OPT_PCG_FUSE = 0 runs the seven-kernel iteration of bj_pcg.cu, the default rides on the SpMV and solve kernels
     (three kernels per iteration): both follow the oracle, for every solve kernel (b = 3, 8: thread per block; 16, 24, 32:
     group per block; 12: no hook -> unfused either way)."""
-    monkeypatch.setenv("BJ_PCG_FUSE", fuse)
     A = mat(2, "small")
     rhs = W.seeded_vector(23, A.n)
     for b in (3, 8, 12, 16, 24, 32):
         h, keep = B.setup_from_host(A, b)
+        B.bj_set_option(h, B.BJ_OPT_PCG_FUSE, fuse)
         g = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=10, rtol=0.0, check_every=4)
         c = oracle.Precond(A, b).pcg(rhs, 10, 0.0)
         assert g["iters"] == 10
@@ -758,19 +778,16 @@ def test_pcg_full_size(B, torch_, rel, cfg):
     torch_.cuda.empty_cache()
 
 
-@pytest.mark.parametrize("cfg,b,env", [(2, 8, {"BJ_BAND": "1", "BJ_COL16": "1"}), (4, 16, {"BJ_BAND": "1", "BJ_COL16": "1"}),
-                                       (5, 3, {"BJ_BSR": "1"})])
-def test_full_size_opt_in_variants(B, torch_, rel, monkeypatch, cfg, b, env):
+@pytest.mark.parametrize("cfg,b,env", [(2, 8, {"band": 1, "col16": 1}), (4, 16, {"band": 1, "col16": 1}), (5, 3, {"bsr": 1})])
+def test_full_size_opt_in_variants(B, torch_, rel, cfg, b, env):
     """The byte-reducing variants at BASELINE.json's full sizes, in the launch configuration
-    `bench.py --band 1 --col16 1` / `--bsr 1` times: whole-vector parity of every op with the oracle, and a short kappa run."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+    `bench.py --band 1 --col16 1` / `--bsr 1` times (options of bj_setup_ex): whole-vector parity of every op with the oracle, and a short kappa run."""
     A = mat(cfg, "full")
-    h, keep = B.setup_from_host(A, b)
+    h, keep = B.setup_from_host(A, b, **env)
     info = B.bj_get_info(h)
-    if "BJ_BAND" in env:
+    if "band" in env:
         assert info["band_width"] == 1 and info["col16"] == 1
-    if "BJ_BSR" in env:
+    if "bsr" in env:
         assert info["spmv_kernel"] == 2
     P = oracle.Precond(A, b)
     g = B.bj_cond_estimate_ex(h, 12, reorth=False)
@@ -778,12 +795,12 @@ def test_full_size_opt_in_variants(B, torch_, rel, monkeypatch, cfg, b, env):
     assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA
     B.bj_destroy(h)
     del h, keep
-    check_all_ops(B, torch_, A, b, rel, seeds=(31,))
+    check_all_ops(B, torch_, A, b, rel, seeds=(31,), **env)
     _MATS.pop((cfg, "full"), None)
     torch_.cuda.empty_cache()
 
 
-def test_handles_release_their_device_memory(B, torch_, monkeypatch):
+def test_handles_release_their_device_memory(B, torch_):
     """Setup / Lanczos / PCG / batch / BSR / 16-bit-column workspaces all belong to the handle: after destroy and
     bj_release_cached_memory the free device memory is back where it started."""
     A = mat(5, "small")
@@ -792,12 +809,9 @@ def test_handles_release_their_device_memory(B, torch_, monkeypatch):
     torch_.cuda.synchronize()
     B.bj_release_cached_memory()
     free0, _ = torch_.cuda.mem_get_info()
-    monkeypatch.setenv("BJ_BSR", "1")
-    monkeypatch.setenv("BJ_COL16", "1")
-    monkeypatch.setenv("BJ_BAND", "1")
     for rep in range(12):
         for b in (0, 3, 8, 24):
-            h = B.bj_setup(rp, ci, val, b)
+            h = B.bj_setup(rp, ci, val, b, band=1, col16=1, bsr=1, spmv2d=1)
             B.bj_op_apply(h, x)
             B.bj_cond_estimate_ex(h, 6, reorth=bool(rep & 1))
             B.bj_pcg_solve(h, x, max_iters=4, rtol=0.0)
@@ -813,16 +827,16 @@ def test_handles_release_their_device_memory(B, torch_, monkeypatch):
 
 
 # ------------------------------------------------------------------ Lanczos on M^-1 A (NEXT-2) ----------
-@pytest.mark.parametrize("fuse", ["1", "0"])
+@pytest.mark.parametrize("fuse", [1, 0])
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
-def test_minv_lanczos_matches_oracle_small(B, torch_, monkeypatch, cfg, fuse):
+def test_minv_lanczos_matches_oracle_small(B, torch_, cfg, fuse):
     """bj_cond_estimate_minv (one factor pass per step) against the oracle's M-inner-product Lanczos: the first coefficients
     element by element, kappa at m = 50 to the bar of the north star.  fuse=1: two kernels per step where the solve kernel
     carries the hook; fuse=0: the six-kernel step (also the path of b = 0 and of block sizes without a hooked kernel)."""
-    monkeypatch.setenv("BJ_PCG_FUSE", fuse)
     A = mat(cfg, "small")
-    for b in ([0] if fuse == "0" else []) + W.BLOCK_SIZES[cfg]:
+    for b in ([0] if fuse == 0 else []) + W.BLOCK_SIZES[cfg]:
         h, keep = B.setup_from_host(A, b)
+        B.bj_set_option(h, B.BJ_OPT_PCG_FUSE, fuse)
         P = oracle.Precond(A, b)
         g = B.bj_cond_estimate_minv(h, 12)
         c = P.cond_estimate_minv(12)
@@ -866,10 +880,9 @@ def test_minv_lanczos_degenerate_cases(B, torch_):
     B.bj_destroy(h)
 
 
-def test_minv_lanczos_banded_factors(B, torch_, monkeypatch):
-    monkeypatch.setenv("BJ_BAND", "1")
+def test_minv_lanczos_banded_factors(B, torch_):
     A = mat(4, "small")
-    h, keep = B.setup_from_host(A, 16)
+    h, keep = B.setup_from_host(A, 16, band=1)
     assert B.bj_get_info(h)["band_width"] >= 1
     g = B.bj_cond_estimate_minv(h, 50)
     c = oracle.Precond(A, 16).cond_estimate_minv(50)
@@ -953,8 +966,8 @@ def test_variable_blocks_exact_preconditioner_pcg_and_errors(B, torch_, rel):
     assert ei.value.bad_block == 1
 
 
-def test_serpentine_walk_of_the_block_solves(B, torch_, rel, monkeypatch):
-    """BJ_SERP_KEEP_MB: the plain backward solve visits the blocks from the last to the first and the
+def test_serpentine_walk_of_the_block_solves(B, torch_, rel):
+    """bj_setup_opts_t.serp_keep_mb: the plain backward solve visits the blocks from the last to the first and the
     last megabytes of every walk stay ordinary L2 lines.  Only the visiting order and the cache policy change, so every
     output is bit-identical to the forward walk (keep = 0); sizes chosen so that keep = 1 MB covers PART of the factor array
     (both policies and the reversed tail tile in one launch), with a ragged last block / tile.  Oracle parity at keep = 1."""
@@ -964,8 +977,7 @@ def test_serpentine_walk_of_the_block_solves(B, torch_, rel, monkeypatch):
         xs = [dev(torch_, W.seeded_vector(s, A.n)) for s in (11, 12)]
         out = {}
         for keep_mb in ("0", "1", "48"):
-            monkeypatch.setenv("BJ_SERP_KEEP_MB", keep_mb)
-            h, keep = B.setup_from_host(A, b)
+            h, keep = B.setup_from_host(A, b, serp_keep_mb=int(keep_mb) or -1)     # -1: off, 0 would be the default (48)
             res = []
             for x in xs:   # a chain of applies, so that a walk really starts where the previous one stopped
                 y = B.bj_op_apply(h, x).clone()
