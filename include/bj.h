@@ -146,7 +146,9 @@ enum {
     BJ_OPT_SPMV_KERNEL = 1,   /* 0 / 1 / 3 as in bj_info_t.spmv_kernel (when built for the handle); -1 = automatic (default) */
     BJ_OPT_FUSE_FORWARD = 2,  /* 0: three kernels, 1: fuse forward solve into SpMV, -1 = automatic    */
     BJ_OPT_LANCZOS_FUSE = 3,  /* 0: fast-mode Lanczos runs the unfused vector kernels; 1 / -1: the fused step (default) */
-    BJ_OPT_PCG_FUSE = 4       /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
+    BJ_OPT_PCG_FUSE = 4,      /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
+    BJ_OPT_LANCZOS_SINGLE_LAUNCH = 5 /* 0: launch-bound sizes (vectors + factors fit one CTA's shared memory, b <= 8) keep the
+                                 multi-launch Lanczos; 1 / -1: the whole run is one single-CTA kernel (default)          */
 };
 
 /* a1-a4. Validate the CSR, extract the diagonal b x b blocks, factor each

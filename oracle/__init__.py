@@ -322,3 +322,63 @@ class PrecondBlocks:
         tmin, tmax, rmin, rmax = tridiag_extremes(alpha, beta)
         return {"lmin": tmin, "lmax": tmax, "kappa": tmax / tmin, "res_min": rmin, "res_max": rmax,
                 "iters_done": len(alpha), "alpha": alpha, "beta": beta}
+
+
+class _Csr:
+    """The four fields the routines above read from a matrix object."""
+
+    def __init__(self, n, row_ptr, col_idx, val):
+        self.n, self.row_ptr, self.col_idx, self.val = int(n), row_ptr, col_idx, val
+
+
+class PrecondPerm:
+    """Block-Jacobi after a symmetric permutation of the unknowns ("a permutation argument (RCM or
+    strong-coupling lines)"; the paper's partition into diagonal blocks, presupposes an ordering in which
+    contiguous index ranges are the intended blocks -- DESIGN.md reading 8).
+    perm[i] = original index of the unknown that sits at permuted position i, so (P v)[i] = v[perm[i]] and
+    (P A P^T)[i, j] = A[perm[i], perm[j]].  The diagonal blocks are those of P A P^T:
+        M = P^T blockdiag(D_k) P,   D_k = (P A P^T)[kb:(k+1)b, kb:(k+1)b] = L_k L_k^T,
+    and EVERY vector argument stays in the ORIGINAL ordering:
+        solve_L(r) = P^T L^-1 P r,  solve_Lt(y) = P^T L^-T P y,  apply = M^-1,  op_apply = solve_L . A . solve_Lt
+    (= P^T [L^-1 (P A P^T) L^-T] P: orthogonally similar to the split operator of the permuted matrix, same spectrum).
+    Written out as the definition: P A P^T is formed EXPLICITLY (scipy fancy indexing, a library primitive) and handed to
+    Precond / PrecondBlocks; vectors are permuted on the way in and out.  No arithmetic of its own."""
+
+    def __init__(self, A, perm, b: int | None = None, block_ptr=None):
+        import scipy.sparse as sp
+        p = np.asarray(perm, dtype=np.int64)
+        if p.shape != (A.n,) or not np.array_equal(np.sort(p), np.arange(A.n)):
+            raise ValueError("perm must be a permutation of 0..n-1")
+        self.A, self.n, self.perm = A, A.n, p
+        S = sp.csr_matrix((A.val, A.col_idx, A.row_ptr), shape=(A.n, A.n))
+        Sp = S[p][:, p].tocsr()
+        Sp.sum_duplicates()
+        Sp.sort_indices()
+        self.Ap = _Csr(A.n, Sp.indptr.astype(np.int32), Sp.indices.astype(np.int32), Sp.data.astype(np.float64))
+        self.P = PrecondBlocks(self.Ap, block_ptr) if block_ptr is not None else Precond(self.Ap, int(b))
+
+    def to_perm(self, v):
+        return _f64(v)[self.perm]
+
+    def from_perm(self, vp):
+        out = np.empty(self.n)
+        out[self.perm] = vp
+        return out
+
+    def solve_L(self, r):
+        return self.from_perm(self.P.solve_L(self.to_perm(r)))
+
+    def solve_Lt(self, y):
+        return self.from_perm(self.P.solve_Lt(self.to_perm(y)))
+
+    def apply(self, r):
+        return self.from_perm(self.P.apply(self.to_perm(r)))
+
+    def op_apply(self, x):
+        return self.from_perm(self.P.op_apply(self.to_perm(x)))
+
+    def cond_estimate(self, m: int, v0=None, seed: int = DEFAULT_SEED, **kw):
+        """Lanczos on the operator in the original ordering started at v0 (default: the seeded vector, original ordering)
+        = Lanczos on the split operator of P A P^T started at P v0: the same alpha, beta."""
+        v0 = seeded_vector(seed, self.n) if v0 is None else _f64(v0)
+        return self.P.cond_estimate(m, v0=self.to_perm(v0), **kw)

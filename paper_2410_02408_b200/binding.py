@@ -16,7 +16,7 @@ BJ_B_MAX = 32
 BJ_DEFAULT_SEED = 0x241002408
 BJ_OK, BJ_ERR_INVALID_ARG, BJ_ERR_NOT_CANONICAL, BJ_ERR_TOO_LARGE, BJ_ERR_NOT_SPD, BJ_ERR_ALLOC, BJ_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
 BJ_K_SOLVE_LT, BJ_K_SPMV, BJ_K_SOLVE_L, BJ_K_APPLY, BJ_K_SPMV_SOLVE_L, BJ_K_COUNT = 0, 1, 2, 3, 4, 5
-BJ_OPT_SPMV_KERNEL, BJ_OPT_FUSE_FORWARD, BJ_OPT_LANCZOS_FUSE, BJ_OPT_PCG_FUSE = 1, 2, 3, 4
+BJ_OPT_SPMV_KERNEL, BJ_OPT_FUSE_FORWARD, BJ_OPT_LANCZOS_FUSE, BJ_OPT_PCG_FUSE, BJ_OPT_LANCZOS_SINGLE_LAUNCH = 1, 2, 3, 4, 5
 KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
 
 EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_setup_ex", "bj_get_setup_time", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",

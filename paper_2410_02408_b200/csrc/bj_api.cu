@@ -194,21 +194,6 @@ const char* bj_strerror(int code)
 
 }  // extern "C"
 
-// CUDA events around the kernel sequences of bj_setup (the host round trips between them are not device time)
-struct SetupTimer {
-    cudaStream_t st;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> spans;
-    explicit SetupTimer(cudaStream_t s) : st(s) {}
-    void begin() { cudaEvent_t a = nullptr, b = nullptr; cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); spans.push_back({a, b}); }
-    void end() { if (!spans.empty()) cudaEventRecord(spans.back().second, st); }
-    double total_ms() {  // call after a stream synchronisation
-        double t = 0.0;
-        for (auto& sp : spans) { float ms = 0.f; if (cudaEventElapsedTime(&ms, sp.first, sp.second) == cudaSuccess) t += ms; else cudaGetLastError(); }
-        return t;
-    }
-    ~SetupTimer() { for (auto& sp : spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); } }
-};
-
 static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_handle_t* out)
 {
     if (!out) return BJ_ERR_INVALID_ARG;
@@ -284,53 +269,6 @@ static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_h
     cudaError_t ce = cudaMemcpyAsync(h->status, &init, sizeof(init), cudaMemcpyHostToDevice, h->stream);
     if (ce != cudaSuccess) { set_cuda_error(ce, "status init"); return fail(BJ_ERR_CUDA); }
 
-    // a1 validate (also longest row and the column-coherence statistic)
-    SetupTimer timer(h->stream);
-    timer.begin();
-    int rc = launch_validate(h);
-    timer.end();
-    if (rc != BJ_OK) return fail(rc);
-    Status stt;
-    ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
-    if (ce != cudaSuccess) { set_cuda_error(ce, "validate"); return fail(BJ_ERR_CUDA); }
-    if (stt.flags & (ST_BAD_ROWPTR | ST_BAD_COL | ST_UNSORTED)) return fail(BJ_ERR_NOT_CANONICAL);
-    if (stt.descents != stt.legal_descents) return fail(BJ_ERR_NOT_CANONICAL);  // a descent inside a row
-
-    h->coherence = stt.compared ? (double)stt.coherent / (double)stt.compared : 1.0;
-
-    // NEXT-2, opt-in: banded diagonal blocks keep banded factors -- (w+1) b doubles per block instead of b(b+1)/2.
-    // Only for b > 8 (the b <= 8 path fuses the forward solve into the SpMV kernel, which the band path does not).
-    if (h->solve_kind == 1 && b >= 4 && o.band != 0) {
-        // b <= 8: tridiagonal blocks keep bidiagonal factors, 2b - 1 doubles per block instead of b(b+1)/2; same kernels
-        // (thread per block, fused into the SpMV tile kernel, Lanczos / PCG hooks), compile-time / uniform index switch
-        rc = launch_band_width(h);
-        if (rc != BJ_OK) return fail(rc);
-        ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
-        if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
-        if (ce != cudaSuccess) { set_cuda_error(ce, "band width"); return fail(BJ_ERR_CUDA); }
-        if (stt.max_band >= 0 && stt.max_band <= 1) {
-            h->tri = true;
-            h->band = stt.max_band;
-            h->packed = 2 * b - 1;
-            h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * h->packed * kInterleave * (int64_t)sizeof(double);
-        }
-    }
-    if (h->solve_kind == 2 && h->nblocks >= 64 && o.band != 0) {
-        rc = launch_band_width(h);
-        if (rc != BJ_OK) return fail(rc);
-        ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
-        if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
-        if (ce != cudaSuccess) { set_cuda_error(ce, "band width"); return fail(BJ_ERR_CUDA); }
-        if (stt.max_band >= 0 && stt.max_band <= 2) {
-            h->solve_kind = 3;
-            h->band = stt.max_band;
-            h->fac_band = h->fac_fwd;  // (w+1) b <= 3 b < b(b+1)/2 for b > 8: fits the forward copy's storage
-            h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * kInterleave * (h->band + 1) * b * (int64_t)sizeof(double);
-        }
-    }
-
-    timer.begin();
     // lanes per row for the CSR-vector kernel: power of two near the mean row length
     {
         const double mean = (double)h->nnz / (double)h->n;
@@ -338,37 +276,86 @@ static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_h
         while (l < 32 && (double)l * 1.15 < mean) l *= 2;
         h->spmv_lanes = l;
     }
+    // only the padding the extraction kernels do not write needs zeroing
+    auto zero_padding = [&]() -> cudaError_t {
+        cudaError_t e = cudaSuccess;
+        if (h->solve_kind == 1) {
+            const size_t group_bytes = (size_t)h->packed * kInterleave * sizeof(double);
+            const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;  // (packed may be the compact tridiagonal size)
+            if (h->nblocks % kInterleave) e = cudaMemsetAsync((char*)h->fac_small + (size_t)(groups - 1) * group_bytes, 0, group_bytes, h->stream);
+        } else if (h->solve_kind == 3) {
+            // the last interleave group may be partly unused: zero it so that no lane ever reads an uninitialised factor
+            const size_t group_bytes = (size_t)(h->band + 1) * b * kInterleave * sizeof(double);
+            if (h->nblocks % kInterleave)
+                e = cudaMemsetAsync((char*)h->fac_band + (size_t)(h->nblocks / kInterleave) * group_bytes, 0, group_bytes, h->stream);
+        } else if (h->solve_kind == 2) {
+            e = cudaMemsetAsync((char*)h->fac_fwd + fac_a - 16, 0, 16, h->stream);
+            if (e == cudaSuccess && h->fac_bwd) e = cudaMemsetAsync((char*)h->fac_bwd + fac_b - 16, 0, 16, h->stream);
+        }
+        return e;
+    };
+    auto read_status = [&](Status& dst, const char* where) -> int {
+        cudaError_t e = cudaMemcpyAsync(&dst, h->status, sizeof(dst), cudaMemcpyDeviceToHost, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess) { set_cuda_error(e, where); return BJ_ERR_CUDA; }
+        return BJ_OK;
+    };
 
-    // a2-a4 extract + factor; only the padding the kernels do not write needs zeroing
-    if (h->solve_kind == 1) {
-        const size_t group_bytes = (size_t)h->packed * kInterleave * sizeof(double);
-        const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;  // (packed may be the compact tridiagonal size)
-        if (h->nblocks % kInterleave) ce = cudaMemsetAsync((char*)h->fac_small + (size_t)(groups - 1) * group_bytes, 0, group_bytes, h->stream);
-    } else if (h->solve_kind == 3) {
-        // the last interleave group may be partly unused: zero it so that no lane ever reads an uninitialised factor
-        const size_t group_bytes = (size_t)(h->band + 1) * b * kInterleave * sizeof(double);
-        if (h->nblocks % kInterleave)
-            ce = cudaMemsetAsync((char*)h->fac_band + (size_t)(h->nblocks / kInterleave) * group_bytes, 0, group_bytes, h->stream);
-    } else if (h->solve_kind == 2) {
-        ce = cudaMemsetAsync((char*)h->fac_fwd + fac_a - 16, 0, 16, h->stream);
-        if (ce == cudaSuccess && h->fac_bwd) ce = cudaMemsetAsync((char*)h->fac_bwd + fac_b - 16, 0, 16, h->stream);
+    SetupTimer timer(h->stream);
+    h->setup_timer = &timer;  // the launch helpers of the setup kernels bracket each kernel with events
+    struct TimerGuard { bj_handle_s* h; ~TimerGuard() { h->setup_timer = nullptr; } } timer_guard{h};
+    Status stt;
+    int rc = BJ_OK;
+    // opts.band: the factor layout depends on the band statistic, so the extraction follows the validation pass
+    const bool want_band = o.band != 0 && ((h->solve_kind == 1 && b >= 4) || (h->solve_kind == 2 && h->nblocks >= 64));
+
+    // a1 validate (also longest row and the column-coherence statistic)
+    rc = launch_validate(h);
+    if (rc != BJ_OK) return fail(rc);
+    rc = read_status(stt, "validate");
+    if (rc != BJ_OK) return fail(rc);
+    if (stt.flags & (ST_BAD_ROWPTR | ST_BAD_COL | ST_UNSORTED)) return fail(BJ_ERR_NOT_CANONICAL);
+    if (stt.descents != stt.legal_descents) return fail(BJ_ERR_NOT_CANONICAL);  // a descent inside a row
+
+    h->coherence = stt.compared ? (double)stt.coherent / (double)stt.compared : 1.0;
+    h->max_row_nnz = stt.max_row_nnz;
+
+    // NEXT-2, opt-in: banded diagonal blocks keep banded factors -- (w+1) b doubles per block instead of b(b+1)/2.
+    if (want_band) {
+        rc = launch_band_width(h);
+        if (rc != BJ_OK) return fail(rc);
+        rc = read_status(stt, "band width");
+        if (rc != BJ_OK) return fail(rc);
+        if (h->solve_kind == 1 && stt.max_band >= 0 && stt.max_band <= 1) {
+            // b <= 8: tridiagonal blocks keep bidiagonal factors, 2b - 1 doubles per block instead of b(b+1)/2; same kernels
+            // (thread per block, fused into the SpMV tile kernel, Lanczos / PCG hooks), compile-time / uniform index switch
+            h->tri = true;
+            h->band = stt.max_band;
+            h->packed = 2 * b - 1;
+            h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * h->packed * kInterleave * (int64_t)sizeof(double);
+        } else if (h->solve_kind == 2 && stt.max_band >= 0 && stt.max_band <= 2) {
+            h->solve_kind = 3;
+            h->band = stt.max_band;
+            h->fac_band = h->fac_fwd;  // (w+1) b <= 3 b < b(b+1)/2 for b > 8: fits the forward copy's storage
+            h->factor_bytes = (int64_t)((h->nblocks + kInterleave - 1) / kInterleave) * kInterleave * (h->band + 1) * b * (int64_t)sizeof(double);
+        }
     }
-    if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
+
     if (b > 0) {
+        // a2-a4 extract + factor
+        ce = zero_padding();
+        if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
         rc = h->solve_kind == 3 ? launch_extract_factor_band(h) : launch_extract_factor(h);
         if (rc != BJ_OK) return fail(rc);
     }
-
     // SpMV plan for the streamed kernel: tile rows now, stage capacity once the fullest tile is known
     rc = spmv_stream_configure(h);
-    timer.end();
     if (rc != BJ_OK) return fail(rc);
-
-    ce = cudaMemcpyAsync(&stt, h->status, sizeof(stt), cudaMemcpyDeviceToHost, h->stream);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
-    if (ce != cudaSuccess) { set_cuda_error(ce, "setup"); return fail(BJ_ERR_CUDA); }
+    rc = read_status(stt, "setup");
+    if (rc != BJ_OK) return fail(rc);
+    const int max_tile = stt.max_tile_nnz;
     h->setup_kernel_ms = timer.total_ms();
-    rc = spmv_stream_finish(h, stt.max_tile_nnz);
+    rc = spmv_stream_finish(h, max_tile);
     if (rc != BJ_OK) return fail(rc);
     if (o.col16 != 0 && h->stream_ok) {  // NEXT-2, opt-in: 16-bit column deltas for the tile kernel
         rc = col16_build(h);
@@ -474,6 +461,10 @@ int bj_set_option(bj_handle_t h, int option, int value)
         case BJ_OPT_PCG_FUSE:
             if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
             h->opt_pcg_fuse = value;
+            return BJ_OK;
+        case BJ_OPT_LANCZOS_SINGLE_LAUNCH:
+            if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
+            h->opt_lanczos_small = value;
             return BJ_OK;
         default: return BJ_ERR_INVALID_ARG;
     }

@@ -326,7 +326,7 @@ int launch_band_t(bj_handle_s* h, int dir, const double* in, double* out, const 
 int launch_band_width(bj_handle_s* h)
 {
     const unsigned blocks = (unsigned)((h->n + 255) / 256);
-    band_width_kernel<<<blocks, 256, 0, h->stream>>>(h->n, h->b, h->row_ptr, h->col_idx, h->status);
+    { SetupSpan span(h); band_width_kernel<<<blocks, 256, 0, h->stream>>>(h->n, h->b, h->row_ptr, h->col_idx, h->status); }
     h->launches++;
     BJ_CUDA(cudaGetLastError());
     return BJ_OK;
@@ -335,6 +335,7 @@ int launch_band_width(bj_handle_s* h)
 int launch_extract_factor_band(bj_handle_s* h)
 {
     const unsigned blocks = (unsigned)((h->nblocks + 127) / 128);
+    SetupSpan span(h);
 #define BJ_CASE(W)                                                                                                      \
     case W:                                                                                                             \
         extract_factor_band_kernel<W><<<blocks, 128, 0, h->stream>>>(h->n, h->b, h->nblocks, h->row_ptr, h->col_idx, h->val, \

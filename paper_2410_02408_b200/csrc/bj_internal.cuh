@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <utility>
 #include <vector>
 
 #include "bj.h"
@@ -45,6 +46,22 @@ struct Tuning {
                             // tail frees and prefetches its factors: cfg 3 131.8 -> 128.9 us, cfg 4 184.7 -> 182.7; the fused
                             // SpMV + solve kernel measured 0.6 us slower with it and keeps the exit trigger)
     int ctas_per_sm = 4;    // wanted CTAs per SM of the SpMV tile kernel
+};
+
+// CUDA events right around each kernel of bj_setup (bj_get_setup_time): host work between launches and the read-backs
+// between the phases are not device time
+struct SetupTimer {
+    cudaStream_t st;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> spans;
+    explicit SetupTimer(cudaStream_t s) : st(s) {}
+    void begin() { cudaEvent_t a = nullptr, b = nullptr; cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); spans.push_back({a, b}); }
+    void end() { if (!spans.empty()) cudaEventRecord(spans.back().second, st); }
+    double total_ms() {  // call after a stream synchronisation
+        double t = 0.0;
+        for (auto& sp : spans) { float ms = 0.f; if (cudaEventElapsedTime(&ms, sp.first, sp.second) == cudaSuccess) t += ms; else cudaGetLastError(); }
+        return t;
+    }
+    ~SetupTimer() { for (auto& sp : spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); } }
 };
 
 struct ProfSpan {
@@ -114,14 +131,17 @@ struct bj_handle_s {
     int spmv_lanes = 8;       // lanes per row, CSR-vector kernel
     int stream_lanes = 1;     // lanes per row, reduce phase of the tile kernel
     int stream_warps = 8;     // consumer warps of the tile kernel
+    int max_row_nnz = 0;      // longest row (validation pass)
     double coherence = 1.0;   // fraction of entries with |col(i+1, j) - col(i, j)| <= 16: ~1 banded/stencil, ~0 random
     int spmv_kernel = 0;      // chosen kernel: 0 CSR-vector, 1 TMA tile kernel, 2 BSR(3) copy
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;
     int opt_lanczos_fuse = -1;  // BJ_OPT_LANCZOS_FUSE / BJ_OPT_PCG_FUSE: 0 selects the unfused iterations
+    int opt_lanczos_small = -1; // BJ_OPT_LANCZOS_SINGLE_LAUNCH: 0 keeps launch-bound sizes on the multi-launch path
     int opt_pcg_fuse = -1;
     bj_setup_opts_t opts = {};  // the options this handle was set up with
     double setup_kernel_ms = 0.0;  // device time of the setup kernels (bj_get_setup_time)
+    bj::SetupTimer* setup_timer = nullptr;  // non-null while bj_setup runs
     int tile_rows = 0;        // rows per tile of the streamed kernel (multiple of b)
     int tile_cap = 0;         // nnz capacity per stage
     int tile_stages = 0;
@@ -169,6 +189,13 @@ struct bj_handle_s {
 
 namespace bj {
 
+// RAII bracket around ONE setup kernel launch (events only while bj_setup is timing)
+struct SetupSpan {
+    SetupTimer* t;
+    explicit SetupSpan(bj_handle_s* h) : t(h->setup_timer) { if (t) t->begin(); }
+    ~SetupSpan() { if (t) t->end(); }
+};
+
 // error plumbing -------------------------------------------------------------------------------
 void set_cuda_error(cudaError_t e, const char* where);
 #define BJ_CUDA(call)                                   \
@@ -193,7 +220,7 @@ struct KernelScope {
 // setup (bj_setup_kernels.cu)
 int launch_validate(bj_handle_s* h);
 int launch_extract_factor(bj_handle_s* h);
-int launch_spmv_plan(bj_handle_s* h);  // fills Status.max_tile_nnz / max_row_nnz
+int launch_spmv_plan(bj_handle_s* h, int tile_rows);  // Status.max_tile_nnz for tiles of tile_rows rows
 int col16_build(bj_handle_s* h);       // 16-bit column deltas when every |col - row| < 32768
 void col16_free(bj_handle_s* h);
 
@@ -224,7 +251,10 @@ struct LzReduce;
 // epi: fused Lanczos epilogue; dot_with / dot_red: per-CTA partials of dot_with . y finished into *dot_red->out (unfused only)
 int launch_spmv_stream(bj_handle_s* h, const double* x, double* y, bool fuse_forward, const LzEpilogue* epi = nullptr,
                        const double* dot_with = nullptr, const LzReduce* dot_red = nullptr);
-int spmv_stream_configure(bj_handle_s* h);  // decide tile rows / fusion, launch tile_nnz_kernel (async)
+struct StreamGeometry { int rows = 0; bool fuse = false; int lanes = 1, warps = 8; };
+StreamGeometry spmv_stream_geometry(const bj_handle_s* h, bool random_cols);  // tile rows / fusion / lanes for a column structure
+int spmv_stream_configure(bj_handle_s* h);  // geometry from h->coherence, launch tile_nnz_kernel (async)
+void spmv_stream_adopt(bj_handle_s* h, const StreamGeometry& g);  // take a geometry whose fullest tile was measured already
 int spmv_stream_finish(bj_handle_s* h, int max_tile);  // stage capacity and count, sets stream_ok
 
 // Lanczos (bj_lanczos.cu)
@@ -234,6 +264,10 @@ int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
 // k-th smallest eigenvalue (k = 0 .. m-1) of the symmetric tridiagonal (diag a[0..m-1], off-diagonal e[0..m-2]), bisection
 double tridiag_eig_k(int m, const double* a, const double* e, int k);
 void lanczos_fill_result(int me, const double* a, const double* b, bj_lanczos_result_t* res);
+// the whole run as one single-CTA kernel for launch-bound sizes (bj_lanczos_small.cu)
+bool lanczos_small_usable(const bj_handle_s* h, int m);
+int launch_lanczos_small(bj_handle_s* h, int m, bool reorth, double tol, const double* v0, double* V, double* alpha, double* beta,
+                         int* done);
 // Lanczos on M^-1 A in the M inner product (bj_pcg.cu; shares the PCG workspace and the PCG hook of the solve kernels)
 int mlanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res);
 

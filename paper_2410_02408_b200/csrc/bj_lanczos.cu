@@ -9,6 +9,7 @@
 // summation order (bitwise reproducible run to run).
 #include <math.h>
 #include <stdlib.h>
+#include <string.h>
 
 #include <algorithm>
 
@@ -256,7 +257,7 @@ void lanczos_free(bj_handle_s* h)
 {
     LanczosWs& z = h->lz;
     cudaFree(z.V); cudaFree(z.w); cudaFree(z.partial); cudaFree(z.coef);
-    cudaFree(z.alpha); cudaFree(z.beta); cudaFree(z.scal); cudaFree(z.done);
+    cudaFree(z.alpha);  // one block: done | scal | alpha | beta
     cudaFree(z.lz_part); cudaFree(z.lz_sums); cudaFree(z.lz_ticket);
     h->workspace_bytes -= z.bytes;
     z = LanczosWs();
@@ -278,10 +279,13 @@ static int lanczos_alloc(bj_handle_s* h, int iters, int64_t nvec, bool reorth)
     if (e == cudaSuccess) e = A((void**)&z.w, vb);
     if (e == cudaSuccess) e = A((void**)&z.partial, sizeof(double) * want_partial);
     if (e == cudaSuccess) e = A((void**)&z.coef, sizeof(double) * (size_t)(iters + 1));
-    if (e == cudaSuccess) e = A((void**)&z.alpha, sizeof(double) * (size_t)iters);
-    if (e == cudaSuccess) e = A((void**)&z.beta, sizeof(double) * (size_t)iters);
-    if (e == cudaSuccess) e = A((void**)&z.scal, sizeof(double) * 8);
-    if (e == cudaSuccess) e = A((void**)&z.done, sizeof(int) * 4);
+    // one block (one memset before a run, one copy back after it): alpha[iters] | beta[iters] | scal[8] | done[4 ints]
+    if (e == cudaSuccess) e = A((void**)&z.alpha, sizeof(double) * (2 * (size_t)iters + 8 + 2));
+    if (e == cudaSuccess) {
+        z.beta = z.alpha + iters;
+        z.scal = z.beta + iters;
+        z.done = reinterpret_cast<int*>(z.scal + 8);
+    }
     // fused fast mode: the epilogue kernel with the largest grid is the thread-per-block solve (nblocks / 128 CTAs)
     z.lz_cap = (int)std::max<int64_t>(kMaxPartials, (h->nblocks + 127) / 128 + 1);
     if (e == cudaSuccess) e = A((void**)&z.lz_part, sizeof(double) * 2 * (size_t)z.lz_cap);
@@ -355,6 +359,27 @@ static double last_comp(int m, const double* a, const double* e, double th)
     return fabs(z[m - 1]) / sqrt(nn);
 }
 
+// one D2H copy of alpha[], beta[] and the flags at the end of a run; extremes of T on the host
+static int lanczos_readback(bj_handle_s* h, int m, bj_lanczos_result_t* res)
+{
+    LanczosWs& z = h->lz;
+    cudaStream_t st = h->stream;
+    const size_t cap = (size_t)z.cap_iters, words = 2 * cap + 8 + 2;
+    std::vector<double> blk(words);
+    BJ_CUDA(cudaMemcpyAsync(blk.data(), z.alpha, sizeof(double) * words, cudaMemcpyDeviceToHost, st));  // one copy: alpha | beta | scal | done
+    BJ_CUDA(cudaStreamSynchronize(st));
+    const double* ap = blk.data();
+    const double* bp = blk.data() + cap;
+    int done[4];
+    memcpy(done, blk.data() + 2 * cap + 8, sizeof(done));
+    std::vector<double> a(ap, ap + m), b(bp, bp + m);
+    if (done[2]) return BJ_ERR_INVALID_ARG;  // ||v0|| is zero or not finite
+    const int me = done[1];
+    if (me < 1) return BJ_ERR_CUDA;
+    lanczos_fill_result(me, a.data(), b.data(), res);
+    return BJ_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t* res)
 {
@@ -370,10 +395,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     const int stride = m + 1;
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
 
-    BJ_CUDA(cudaMemsetAsync(z.scal, 0, sizeof(double) * 8, st));
-    BJ_CUDA(cudaMemsetAsync(z.done, 0, sizeof(int) * 4, st));
-    BJ_CUDA(cudaMemsetAsync(z.alpha, 0, sizeof(double) * m, st));
-    BJ_CUDA(cudaMemsetAsync(z.beta, 0, sizeof(double) * m, st));
+    BJ_CUDA(cudaMemsetAsync(z.alpha, 0, sizeof(double) * (2 * (size_t)z.cap_iters + 8 + 2), st));  // alpha, beta, scal, done
 
     auto vcol = [&](int j) { return z.V + (size_t)(reorth ? j : (j & 1)) * (size_t)n; };
     double* PA = z.partial;                 // per-CTA partials of v_j . w
@@ -395,6 +417,12 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         rc = launch_seeded_vector(h, o->seed, z.w);
         if (rc != BJ_OK) return rc;
         v0 = z.w;
+    }
+    if (h->opt_lanczos_small != 0 && lanczos_small_usable(h, m)) {
+        // launch-bound sizes: the whole run is ONE single-CTA kernel (bj_lanczos_small.cu)
+        rc = launch_lanczos_small(h, m, reorth, tol, v0, z.V, z.alpha, z.beta, z.done);
+        if (rc != BJ_OK) return rc;
+        return lanczos_readback(h, m, res);
     }
     const bool fused_mode = !reorth && lanczos_fusable(h) && h->opt_lanczos_fuse != 0;
     if (!fused_mode) BJ_LAUNCH(dot_partial_kernel, G, kReduceThreads, n, v0, v0, PB);
@@ -455,17 +483,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     }
 #undef BJ_LAUNCH
 
-    std::vector<double> a(m), b(m);
-    int done[4] = {0, 0, 0, 0};
-    BJ_CUDA(cudaMemcpyAsync(a.data(), z.alpha, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaMemcpyAsync(b.data(), z.beta, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaMemcpyAsync(done, z.done, sizeof(int) * 4, cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaStreamSynchronize(st));
-    if (done[2]) return BJ_ERR_INVALID_ARG;  // ||v0|| is zero or not finite
-    const int me = done[1];
-    if (me < 1) return BJ_ERR_CUDA;
-    lanczos_fill_result(me, a.data(), b.data(), res);
-    return BJ_OK;
+    return lanczos_readback(h, m, res);
 }
 
 // extreme Ritz values, their residual bounds and the optional coefficient copies from alpha[0..me-1], beta[0..me-1]

@@ -22,20 +22,25 @@ validate_rows_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ rp, con
                      Status* st)
 {
     __shared__ unsigned sh[3][8];
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int flags = 0, len = 0;
     unsigned coh = 0, cmp = 0, legal = 0;
-    if (i < n) {
+    // grid-stride over chunks of 256 rows: a few CTAs per SM, so that the same-address atomics at the end (which serialise
+    // in L2) number a few thousand, not one set per 256 rows
+    for (int64_t base = (int64_t)blockIdx.x * blockDim.x; base < n; base += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = base + threadIdx.x;
+        if (i >= n) continue;
         const int64_t s = rp[i], e = rp[i + 1];
         if (s > e || s < 0 || e > nnz || (i == 0 && s != 0) || (i == n - 1 && e != nnz)) {
             flags |= ST_BAD_ROWPTR;
         } else {
-            len = (int)(e - s);
-            if (len > 0 && s > 0) legal = ci[s] <= ci[s - 1];
-            if ((blockIdx.x & 7) == 0 && i + 1 < n) {
+            const int l = (int)(e - s);
+            len = l > len ? l : len;
+            if (l > 0 && s > 0) legal += ci[s] <= ci[s - 1];
+            if (((base >> 8) & 7) == 0 && i + 1 < n) {  // every eighth chunk also gathers the column-coherence statistic
                 const int64_t e2 = rp[i + 2];
                 if (e2 >= e && e2 <= nnz) {
-                    const int64_t m = (e2 - e) < (e - s) ? (e2 - e) : (e - s);
+                    int64_t m = (e2 - e) < (e - s) ? (e2 - e) : (e - s);
+                    if (m > 8) m = 8;  // a sample: the first entries of the two rows
                     for (int64_t q = 0; q < m; ++q) {
                         const int d = ci[e + q] - ci[s + q];
                         ++cmp;
@@ -92,13 +97,13 @@ validate_entries_kernel(int64_t n, int64_t nnz, const int32_t* __restrict__ ci, 
 
 int launch_validate(bj_handle_s* h)
 {
-    const int64_t blocks = (h->n + 255) / 256;
-    validate_rows_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->n, h->nnz, h->row_ptr, h->col_idx, h->status);
+    const int64_t blocks = std::min<int64_t>((h->n + 255) / 256, (int64_t)h->num_sms * 8);
+    { SetupSpan span(h); validate_rows_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->n, h->nnz, h->row_ptr, h->col_idx, h->status); }
     h->launches++;
     if (h->nnz > 0) {
         const int64_t want = (h->nnz + 256 * 8 - 1) / (256 * 8);
-        const unsigned eb = (unsigned)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * 32));
-        validate_entries_kernel<<<eb, 256, 0, h->stream>>>(h->n, h->nnz, h->col_idx, h->status);
+        const unsigned eb = (unsigned)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)h->num_sms * 8));
+        { SetupSpan span(h); validate_entries_kernel<<<eb, 256, 0, h->stream>>>(h->n, h->nnz, h->col_idx, h->status); }
         h->launches++;
     }
     BJ_CUDA(cudaGetLastError());
@@ -108,7 +113,7 @@ int launch_validate(bj_handle_s* h)
 // ------------------------------------------------------------------------------------------------
 // SpMV plan: nnz of the fullest tile of `tile_rows` consecutive rows
 // ------------------------------------------------------------------------------------------------
-__global__ void tile_nnz_kernel(int64_t n, int tile_rows, int64_t ntiles, const int32_t* __restrict__ rp, Status* st)
+__global__ void tile_nnz_kernel(int64_t n, int tile_rows, int64_t ntiles, const int32_t* __restrict__ rp, int* __restrict__ out)
 {
     int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int v = 0;
@@ -117,14 +122,17 @@ __global__ void tile_nnz_kernel(int64_t n, int tile_rows, int64_t ntiles, const 
         v = rp[r1] - rp[r0];
     }
     v = __reduce_max_sync(0xffffffffu, v);
-    if ((threadIdx.x & 31) == 0) atomicMax(&st->max_tile_nnz, v);
+    if ((threadIdx.x & 31) == 0) atomicMax(out, v);
 }
 
-int launch_spmv_plan(bj_handle_s* h)
+int launch_spmv_plan(bj_handle_s* h, int tile_rows)
 {
-    if (h->ntiles <= 0) return BJ_OK;
-    int64_t blocks = (h->ntiles + 255) / 256;
-    tile_nnz_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->n, h->tile_rows, h->ntiles, h->row_ptr, h->status);
+    if (tile_rows <= 0) return BJ_OK;
+    const int64_t ntiles = (h->n + tile_rows - 1) / tile_rows;
+    int64_t blocks = (ntiles + 255) / 256;
+    SetupSpan span(h);
+    tile_nnz_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->n, tile_rows, ntiles, h->row_ptr,
+                                                              &h->status->max_tile_nnz);
     h->launches++;
     BJ_CUDA(cudaGetLastError());
     return BJ_OK;
@@ -175,8 +183,8 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
                     const double v = val[p];
                     const int j = (int)(c - lo);
 #pragma unroll
-                    for (int jj = 0; jj <= i; ++jj)
-                        if (jj == j) d[i * (i + 1) / 2 + jj] = v;
+                    for (int jj = 0; jj < B; ++jj)
+                        if (jj <= i && jj == j) d[i * (i + 1) / 2 + jj] = v;
                 }
             }
         } else {
@@ -184,20 +192,25 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
         }
     }
     bool bad = false;
+    // every loop has the constant trip count B (triangular bounds as predicates): all of them unroll, d[] stays in registers
 #pragma unroll
     for (int j = 0; j < B; ++j) {
         double sjj = d[j * (j + 1) / 2 + j];
 #pragma unroll
-        for (int p = 0; p < j; ++p) sjj -= d[j * (j + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
+        for (int p = 0; p < B; ++p)
+            if (p < j) sjj -= d[j * (j + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
         if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
         const double ljj = sqrt(sjj);
         d[j * (j + 1) / 2 + j] = ljj;
 #pragma unroll
-        for (int i = j + 1; i < B; ++i) {
-            double t = d[i * (i + 1) / 2 + j];
+        for (int i = 0; i < B; ++i) {
+            if (i > j) {
+                double t = d[i * (i + 1) / 2 + j];
 #pragma unroll
-            for (int p = 0; p < j; ++p) t -= d[i * (i + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
-            d[i * (i + 1) / 2 + j] = t / ljj;
+                for (int p = 0; p < B; ++p)
+                    if (p < j) t -= d[i * (i + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
+                d[i * (i + 1) / 2 + j] = t / ljj;
+            }
         }
     }
     if (bad) {
@@ -383,6 +396,7 @@ int col16_build(bj_handle_s* h)
 int launch_extract_factor(bj_handle_s* h)
 {
     const int b = h->b;
+    SetupSpan span(h);
     if (h->solve_kind == 1) {
         const unsigned tb = (unsigned)((h->nblocks + 127) / 128);
 #define BJ_CASE(B)                                                                                          \

@@ -400,14 +400,13 @@ constexpr size_t kSmemTwoPerSm = 110 * 1024;
 constexpr size_t kSmemOnePerSm = 224 * 1024;
 }  // namespace
 
-// Decide the tile geometry (rows per tile, fusion) and launch the kernel that measures the fullest tile.
-int spmv_stream_configure(bj_handle_s* h)
+// Tile geometry (rows per tile, fusion, lanes per row) for a matrix whose columns are / are not coherent between
+// neighbouring rows.  rows == 0: the streamed kernel cannot be used.
+StreamGeometry spmv_stream_geometry(const bj_handle_s* h, bool random_cols)
 {
-    h->stream_ok = false;
-    h->fuse_ok = false;
-    h->ntiles = 0;
-    if (h->nnz == 0) return BJ_OK;
-    if (((uintptr_t)h->val & 15) || ((uintptr_t)h->col_idx & 15) || ((uintptr_t)h->row_ptr & 15)) return BJ_OK;
+    StreamGeometry g;
+    if (h->nnz == 0) return g;
+    if (((uintptr_t)h->val & 15) || ((uintptr_t)h->col_idx & 15) || ((uintptr_t)h->row_ptr & 15)) return g;
     const double mean = (double)h->nnz / (double)h->n;
     {
         // lanes per row in the tile kernel: rows come out of shared memory, so one thread per row
@@ -416,16 +415,14 @@ int spmv_stream_configure(bj_handle_s* h)
         while (l < 32 && (double)l * 12.0 < mean) l *= 2;
         // Random column structure (no coherence between neighbouring rows): the kernel is bound by the
         // L1/LSU gather rate, not by HBM; what helps is many warps with gathers in flight, one row per thread.
-        const bool random_cols = h->coherence < 0.25;
         if (random_cols && mean <= 48.0) l = 1;
-        h->stream_lanes = env_int("BJ_STREAM_LANES", l);
-        h->stream_warps = std::max(1, std::min(env_int("BJ_CONSUMER_WARPS", random_cols ? 16 : 8), kMaxConsumerThreads / 32));
+        g.lanes = env_int("BJ_STREAM_LANES", l);
+        g.warps = std::max(1, std::min(env_int("BJ_CONSUMER_WARPS", random_cols ? 16 : 8), kMaxConsumerThreads / 32));
     }
     const int target_nnz = env_int("BJ_TILE_NNZ", 2048);
     int R = (int)((double)target_nnz / (mean > 1.0 ? mean : 1.0));
     R = std::max(32, std::min(R, 1024));
     bool fuse = false;
-    const bool random_cols = h->coherence < 0.25;
     if (h->solve_kind == 1 && !random_cols) {
         const int unit = kInterleave * h->b;  // fused tiles must hold whole interleave groups
         int Rf = ((R + unit / 2) / unit) * unit;
@@ -435,12 +432,29 @@ int spmv_stream_configure(bj_handle_s* h)
     if (!fuse) R = ((R + 31) / 32) * 32;
     R = env_int("BJ_TILE_ROWS", R);
     if (fuse && (R % (kInterleave * h->b)) != 0) fuse = false;
-    if (R % 4) return BJ_OK;
-    h->tile_rows = R;
-    h->ntiles = (h->n + R - 1) / R;
-    h->fuse_ok = fuse;
+    if (R % 4) return g;
+    g.rows = R;
+    g.fuse = fuse;
+    return g;
+}
+
+void spmv_stream_adopt(bj_handle_s* h, const StreamGeometry& g)
+{
+    h->stream_ok = false;
+    h->fuse_ok = g.rows > 0 && g.fuse;
+    h->ntiles = g.rows > 0 ? (h->n + g.rows - 1) / g.rows : 0;
+    h->tile_rows = g.rows;
+    h->stream_lanes = g.lanes;
+    h->stream_warps = g.warps;
+}
+
+// Decide the tile geometry from the handle's coherence statistic and launch the kernel that measures the fullest tile.
+int spmv_stream_configure(bj_handle_s* h)
+{
+    const StreamGeometry g = spmv_stream_geometry(h, h->coherence < 0.25);
+    spmv_stream_adopt(h, g);
     // measure the fullest tile (result is read back with the rest of the setup status)
-    return launch_spmv_plan(h);
+    return launch_spmv_plan(h, g.rows);
 }
 
 // second half of the plan, once the fullest tile is known

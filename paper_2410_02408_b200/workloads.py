@@ -231,16 +231,24 @@ def config3_unscaled(N: int, seed: int = SEED, per_row: int = 8) -> CSR:
 # --------------------------------------------------------------------------------------
 # config 4: 2D anisotropic 9-point operator, y fastest
 # --------------------------------------------------------------------------------------
-def config4(n: int = 2048, eps: float = 1e-4, gamma_over_eps: float = 0.1) -> CSR:
+def config4(n: int = 2048, eps: float = 1e-4, gamma_over_eps: float = 0.1, x_fastest: bool = False) -> CSR:
+    """x_fastest = False: row p = y + n x (y fastest: contiguous blocks follow the strong coupling, the BASELINE.json
+    ordering).  x_fastest = True: the SAME operator numbered p = x + n y -- contiguous blocks then run along the weak
+    direction; `config4_line_permutation` maps it back (the permutation argument)."""
     gam = gamma_over_eps * eps
     N = n * n
-    xg, yg = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")  # index [x, y]; row p = y + n*x
+    if x_fastest:
+        yg, xg = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")  # index [y, x]; row p = x + n*y
+        sx, sy = 1, n
+    else:
+        xg, yg = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")  # index [x, y]; row p = y + n*x
+        sx, sy = n, 1
     x, y = xg.ravel(), yg.ravel()
-    idx = y + n * x
+    idx = sy * y + sx * x
     cols, vals, mask = [], [], []
     for dx in (-1, 0, 1):
         for dy in (-1, 0, 1):
-            cols.append(idx + dy + n * dx)
+            cols.append(idx + sy * dy + sx * dx)
             if dx == 0 and dy == 0:
                 v = 2.0 * eps + 2.0
             elif dx == 0:
@@ -255,7 +263,27 @@ def config4(n: int = 2048, eps: float = 1e-4, gamma_over_eps: float = 0.1) -> CS
             mask.append((x + dx >= 0) & (x + dx < n) & (y + dy >= 0) & (y + dy < n))
     return _from_masked(np.stack(cols, 1), np.stack(vals, 1), np.stack(mask, 1),
                         {"cfg": 4, "n": n, "b": [16], "iters": 50, "eps": eps, "gamma": gam,
-                         "name": f"aniso9pt_{n}^2_eps{eps:g}"})
+                         "name": f"aniso9pt_{n}^2_eps{eps:g}" + ("_xfastest" if x_fastest else "")})
+
+
+def config4_line_permutation(n: int) -> np.ndarray:
+    """perm[i] = index in the x-fastest numbering (x + n y) of the unknown that the y-fastest numbering calls i = y + n x:
+    P A_xfastest P^T = A_yfastest, where (P A P^T)[i, j] = A[perm[i], perm[j]]."""
+    i = np.arange(n * n, dtype=np.int64)
+    x, y = i // n, i % n
+    return (x + n * y).astype(np.int32)
+
+
+def random_permutation(n: int, seed: int = SEED) -> np.ndarray:
+    """A seeded permutation of 0..n-1 (int32), perm[i] = original index of the unknown at permuted position i."""
+    return np.random.Generator(np.random.Philox(key=seed + 977)).permutation(n).astype(np.int32)
+
+
+def permuted(A: CSR, perm: np.ndarray) -> CSR:
+    """P A P^T as canonical CSR, (P A P^T)[i, j] = A[perm[i], perm[j]] (an input generator: indexing only)."""
+    S = A.to_scipy()
+    p = np.asarray(perm, dtype=np.int64)
+    return from_scipy(S[p][:, p].tocsr(), dict(A.meta, name=str(A.meta.get("name")) + "_permuted"))
 
 
 # --------------------------------------------------------------------------------------

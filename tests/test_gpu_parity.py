@@ -170,9 +170,11 @@ def test_breakdown_is_not_an_error(B, torch_, rel):
         B.bj_destroy(h)
 
 
-def test_zero_or_nonfinite_start_vector_is_an_invalid_argument(B, torch_):
-    """beta_1 = ||v0|| = 0 (or NaN / inf) is not a breakdown: every estimator rejects it, fused and unfused alike."""
-    A = mat(2, "small")
+@pytest.mark.parametrize("which", ["multi_launch", "single_launch"])
+def test_zero_or_nonfinite_start_vector_is_an_invalid_argument(B, torch_, which):
+    """beta_1 = ||v0|| = 0 (or NaN / inf) is not a breakdown: every estimator rejects it, fused and unfused alike
+    (config 1 takes the single-launch kernel of bj_lanczos_small.cu, the 13 824-row matrix the multi-launch paths)."""
+    A = mat(2, "small") if which == "multi_launch" else mat(1, "full")
     z = torch_.zeros(A.n, dtype=torch_.float64, device="cuda")
     nan = z.clone()
     nan[5] = float("nan")
@@ -188,6 +190,42 @@ def test_zero_or_nonfinite_start_vector_is_an_invalid_argument(B, torch_):
             g = B.bj_cond_estimate_ex(h, 10, reorth=False)      # the handle is still usable afterwards
             assert g["iters_done"] == 10 and np.isfinite(g["kappa"])
         B.bj_destroy(h)
+
+
+def test_single_launch_lanczos_for_launch_bound_sizes(B, torch_):
+    """Config 1 (N = 1024, the paper's smallest size) and its relatives run the whole Lanczos estimate as ONE single-CTA
+    kernel: same recurrence as the multi-launch path and as the oracle, parity and fast mode, every b <= 8 and b = 0,
+    ragged last block, breakdown, caller's start vector; bj_set_option can switch it off."""
+    cases = [(mat(1, "full"), (0, 1, 3, 4, 7, 8)), (W.laplacian((37, 29)), (4, 5)), (mat(5, "tiny"), (3, 8))]
+    for A, blocks in cases:
+        for b in blocks:
+            h, keep = B.setup_from_host(A, b)
+            P = oracle.Precond(A, b)
+            l0 = B.bj_get_info(h)["kernel_launches"]
+            g = B.bj_cond_estimate_ex(h, 50, reorth=True)
+            assert B.bj_get_info(h)["kernel_launches"] - l0 <= 2          # seeded vector + the one kernel
+            c = P.cond_estimate(50, reorth=True)
+            assert g["iters_done"] == c["iters_done"]
+            assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (A.n, b, g["kappa"], c["kappa"])
+            assert np.allclose(g["alpha"], c["alpha"], rtol=1e-8, atol=1e-10 * abs(c["alpha"]).max())
+            assert np.allclose(g["beta"], c["beta"], rtol=1e-7, atol=1e-10 * abs(c["alpha"]).max())
+            g0 = B.bj_cond_estimate_ex(h, 30, reorth=False)
+            c0 = P.cond_estimate(30, reorth=False)
+            assert np.abs(g0["alpha"] - c0["alpha"]).max() <= 1e-8 * abs(c0["alpha"]).max(), (A.n, b)
+            v0 = W.seeded_vector(77, A.n)
+            gv = B.bj_cond_estimate_ex(h, 20, reorth=True, v0=dev(torch_, v0))
+            assert abs(gv["kappa"] / P.cond_estimate(20, v0=v0)["kappa"] - 1) <= TOL_KAPPA
+            B.bj_set_option(h, B.BJ_OPT_LANCZOS_SINGLE_LAUNCH, 0)           # the multi-launch path on the same handle
+            l0 = B.bj_get_info(h)["kernel_launches"]
+            gm = B.bj_cond_estimate_ex(h, 50, reorth=True)
+            assert B.bj_get_info(h)["kernel_launches"] - l0 > 50
+            assert abs(gm["kappa"] / g["kappa"] - 1) <= TOL_KAPPA
+            B.bj_destroy(h)
+    A = W.block_diagonal_spd(100, 8)          # M = A: breakdown at step 1 inside the single kernel
+    h, keep = B.setup_from_host(A, 8)
+    g = B.bj_cond_estimate_ex(h, 20, reorth=True)
+    assert g["iters_done"] == 1 and abs(g["kappa"] - 1) < 1e-12
+    B.bj_destroy(h)
 
 
 def test_point_jacobi_is_the_papers_kernel(B, torch_):
@@ -278,6 +316,41 @@ def test_setup_options_are_per_handle_arguments(B, torch_, rel):
     assert B.lib().bj_setup_ex(C.byref(csr), 16, C.byref(o), C.byref(out)) == B.BJ_ERR_INVALID_ARG and not out.value
     assert B.lib().bj_setup_ex(C.byref(csr), 16, None, C.byref(out)) == B.BJ_OK
     B.lib().bj_destroy(out)
+
+
+def test_setup_rejects_bad_inputs_in_the_middle_of_a_large_matrix(B, torch_):
+    """a1 / a3 on a matrix that spans many CTAs of the validation kernels: a negative pivot deep inside (first bad block
+    = the oracle's), swapped columns, a column out of range, row pointers that are not monotone or point far outside."""
+    A = mat(2, "small")
+    rp, ci, val = A.row_ptr, A.col_idx, A.val
+    rows = np.repeat(np.arange(A.n), np.diff(rp))
+    bad_val = val.copy()
+    for r in (4001, 9000):
+        bad_val[(rows == r) & (ci == r)] = -2.0
+    swapped = ci.copy()
+    s0 = rp[7000]
+    swapped[s0], swapped[s0 + 1] = swapped[s0 + 1], swapped[s0]
+    big = ci.copy()
+    big[12345] = A.n + 5
+    rp_bad = rp.copy()
+    rp_bad[5000] = rp_bad[5001] + 3          # not monotone in the middle
+    rp_wild = rp.copy()
+    rp_wild[6000:6100] = 2 ** 30             # far outside the arrays
+    for b in (8, 16):
+        with pytest.raises(B.BJError) as e:
+            B.bj_setup(dev(torch_, rp), dev(torch_, ci), dev(torch_, bad_val), b)
+        assert e.value.code == B.BJ_ERR_NOT_SPD and e.value.bad_block == 4001 // b, b
+        with pytest.raises(oracle.NotSPD) as eo:
+            oracle.Precond(W.CSR(A.n, rp, ci, bad_val), b)
+        assert eo.value.bad_block == e.value.bad_block
+        for bad_ci in (swapped, big):
+            with pytest.raises(B.BJError) as e:
+                B.bj_setup(dev(torch_, rp), dev(torch_, bad_ci), dev(torch_, val), b)
+            assert e.value.code == B.BJ_ERR_NOT_CANONICAL, b
+        for bad_rp in (rp_bad, rp_wild):
+            with pytest.raises(B.BJError) as e:
+                B.bj_setup(dev(torch_, bad_rp), dev(torch_, ci), dev(torch_, val), b)
+            assert e.value.code == B.BJ_ERR_NOT_CANONICAL, b
 
 
 def test_tiny_and_degenerate_shapes(B, torch_, rel):
@@ -520,10 +593,11 @@ def test_batched_small_systems(B, torch_, rel):
     assert e.value.code == B.BJ_ERR_INVALID_ARG
     B.bj_destroy(h)
     # a system whose residual becomes EXACTLY zero while the stopping test cannot fire (rtol < 0) is frozen where it stands
-    # instead of taking the step length 0 / 0: A = 2 I, b = 1 makes every quantity of step 1 exact (a = 1, r = 0)
+    # instead of taking the step length 0 / 0: A = 2 I without preconditioner makes every quantity of step 1 exact
+    # (z = r, a = 1/2, r_new = 0)
     nd = 64
     Ad = W.CSR(nd, np.arange(nd + 1, dtype=np.int32), np.arange(nd, dtype=np.int32), np.full(nd, 2.0))
-    h, keep = B.setup_from_host(Ad, 1)
+    h, keep = B.setup_from_host(Ad, 0)
     rhs = W.seeded_vector(4, nd)
     g = B.bj_pcg_solve_batch(h, 4, dev(torch_, rhs), max_iters=6, rtol=-1.0)
     assert np.array_equal(g["x"].cpu().numpy(), rhs / 2.0) and (g["iters"] == 1).all() and (g["true_relres"] == 0.0).all()
@@ -806,6 +880,9 @@ def test_handles_release_their_device_memory(B, torch_):
     A = mat(5, "small")
     rp, ci, val = (torch_.from_numpy(a).cuda() for a in (A.row_ptr, A.col_idx, A.val))
     x = dev(torch_, W.seeded_vector(1, A.n))
+    Ab = W.batch_poisson(4, 32)
+    rpb, cib, valb = (torch_.from_numpy(a).cuda() for a in (Ab.row_ptr, Ab.col_idx, Ab.val))
+    xb = dev(torch_, W.seeded_vector(2, Ab.n))
     torch_.cuda.synchronize()
     B.bj_release_cached_memory()
     free0, _ = torch_.cuda.mem_get_info()
@@ -815,10 +892,11 @@ def test_handles_release_their_device_memory(B, torch_):
             B.bj_op_apply(h, x)
             B.bj_cond_estimate_ex(h, 6, reorth=bool(rep & 1))
             B.bj_pcg_solve(h, x, max_iters=4, rtol=0.0)
-            if b in (3, 24):
-                B.bj_cond_estimate_batch(h, 2, 4)
-                B.bj_pcg_solve_batch(h, 2, x, max_iters=3, rtol=0.0)
             B.bj_destroy(h)
+        hb = B.bj_setup(rpb, cib, valb, 4, band=1)          # batch workspaces (a block-diagonal batch of four systems)
+        B.bj_cond_estimate_batch(hb, 4, 4)
+        B.bj_pcg_solve_batch(hb, 4, xb, max_iters=3, rtol=0.0)
+        B.bj_destroy(hb)
     torch_.cuda.synchronize()
     torch_.cuda.empty_cache()
     B.bj_release_cached_memory()
