@@ -671,3 +671,120 @@ def test_variable_blocks_equal_to_the_matrix_blocks_give_identity():
     assert r["iters_done"] == 1 and abs(r["kappa"] - 1) < 1e-12
     with pytest.raises(ValueError):
         oracle.PrecondBlocks(A, [0, 5, 5, A.n])
+
+
+# ---------------------------------------------------------------- permutation argument ------
+def _dense_perm_reference(A, perm, b):
+    """M = P^T blockdiag(D_k) P built by dense slicing of P A P^T (numpy only)."""
+    Ad = A.to_dense()
+    p = np.asarray(perm)
+    Ap = Ad[np.ix_(p, p)]
+    Mp = np.zeros_like(Ap)
+    for lo in range(0, A.n, b):
+        hi = min(lo + b, A.n)
+        Mp[lo:hi, lo:hi] = Ap[lo:hi, lo:hi]
+    M = np.zeros_like(Mp)
+    M[np.ix_(p, p)] = Mp          # M[perm[i], perm[j]] = Mp[i, j]
+    return Ad, M
+
+
+@pytest.mark.parametrize("cfg,b", [(1, 4), (2, 8), (3, 5), (4, 16), (5, 3)])
+def test_perm_apply_and_spectrum_match_dense_numpy(cfg, b, rel):
+    """oracle.PrecondPerm against the definition written densely: z = M^-1 r by numpy.linalg.solve with
+    M = P^T blockdiag(D_k) P, and the spectrum of the split operator = the generalised spectrum of (A, M)."""
+    A = W.build(cfg, "tiny")
+    perm = W.random_permutation(A.n, seed=100 + cfg)
+    Ad, M = _dense_perm_reference(A, perm, b)
+    P = oracle.PrecondPerm(A, perm, b)
+    r = W.seeded_vector(3, A.n)
+    e2, ei = rel(P.apply(r), np.linalg.solve(M, r))
+    assert e2 < 1e-12 and ei < 1e-12
+    # solve_Lt(solve_L(r)) is apply; op_apply = solve_L . A . solve_Lt, all in the ORIGINAL ordering
+    assert rel(P.solve_Lt(P.solve_L(r)), P.apply(r))[0] < 1e-14
+    assert rel(P.op_apply(r), P.solve_L(Ad @ P.solve_Lt(r)))[0] < 1e-13
+    cols = np.stack([P.op_apply(e) for e in np.eye(A.n)], axis=1)
+    assert np.abs(cols - cols.T).max() <= 1e-12 * np.abs(cols).max()      # symmetric operator
+    ev = np.linalg.eigvalsh(0.5 * (cols + cols.T))
+    gen = sla.eigh(Ad, M, eigvals_only=True)
+    assert np.abs(ev - gen).max() <= 1e-10 * np.abs(gen).max()
+    c = P.cond_estimate(A.n, reorth=True)                                    # m = N: Lanczos sees the whole spectrum
+    assert abs(c["lmin"] / gen[0] - 1) < 1e-8 and abs(c["lmax"] / gen[-1] - 1) < 1e-8
+
+
+def test_perm_identity_is_the_unpermuted_preconditioner_bit_for_bit():
+    A = W.build(2, "tiny")
+    P0, P1 = oracle.Precond(A, 8), oracle.PrecondPerm(A, np.arange(A.n), 8)
+    x = W.seeded_vector(5, A.n)
+    for name in ("solve_L", "solve_Lt", "apply", "op_apply"):
+        assert np.array_equal(getattr(P0, name)(x), getattr(P1, name)(x)), name
+    c0, c1 = P0.cond_estimate(20), P1.cond_estimate(20)
+    assert np.array_equal(c0["alpha"], c1["alpha"]) and np.array_equal(c0["beta"], c1["beta"])
+
+
+def test_point_jacobi_is_invariant_under_any_permutation():
+    """b = 1: M = diag(A) whatever the ordering, so the operator in the original ordering does not depend on P."""
+    A = W.build(3, "tiny")
+    x = W.seeded_vector(9, A.n)
+    ref = oracle.Precond(A, 1).op_apply(x)
+    for seed in (1, 2):
+        P = oracle.PrecondPerm(A, W.random_permutation(A.n, seed), 1)
+        assert np.abs(P.op_apply(x) - ref).max() <= 1e-14 * np.abs(ref).max()
+        k0, k1 = oracle.Precond(A, 1).cond_estimate(A.n)["kappa"], P.cond_estimate(A.n)["kappa"]
+        assert abs(k1 / k0 - 1) < 1e-9
+
+
+def test_line_permutation_turns_xfastest_config4_into_the_yfastest_one():
+    """Config 4 numbered x-fastest has its contiguous blocks along the WEAK direction; the line permutation
+    (workloads.config4_line_permutation) gives back exactly the y-fastest matrix of BASELINE.json: same factors, same
+    operator (in the permuted coordinates bit for bit), same kappa estimate -- and the natural blocks are far worse."""
+    n = 24
+    Ax, Ay = W.config4(n, x_fastest=True), W.config4(n)
+    perm = W.config4_line_permutation(n)
+    Pp, Py = oracle.PrecondPerm(Ax, perm, 8), oracle.Precond(Ay, 8)
+    assert np.array_equal(Pp.Ap.row_ptr, Ay.row_ptr) and np.array_equal(Pp.Ap.col_idx, Ay.col_idx)
+    assert np.array_equal(Pp.Ap.val, Ay.val)
+    assert np.array_equal(Pp.P.L, Py.L)
+    x = W.seeded_vector(2, Ax.n)
+    assert np.array_equal(Pp.op_apply(x)[perm], Py.op_apply(x[perm]))
+    kp = Pp.cond_estimate(Ax.n)["kappa"]
+    ky = Py.cond_estimate(Ax.n, v0=W.seeded_vector(oracle.DEFAULT_SEED, Ax.n)[perm])["kappa"]
+    assert abs(kp / ky - 1) < 1e-10
+    k_natural = oracle.Precond(Ax, 8).cond_estimate(Ax.n)["kappa"]
+    assert k_natural > 3 * kp          # blocks across the weak coupling barely help
+
+
+def test_rcm_restores_the_block_diagonal_model_after_a_shuffle():
+    """PAPER.md:80 (A = diag(A_1..A_k)) hidden by a random symmetric shuffle: reverse Cuthill-McKee (scipy) makes every
+    connected component contiguous again, the blocks match it, M = A and the preconditioned operator is the identity."""
+    from scipy.sparse.csgraph import reverse_cuthill_mckee
+    b = 6
+    A0 = W.block_diagonal_spd(40, b)
+    shuffle = W.random_permutation(A0.n, seed=7)
+    A = W.permuted(A0, shuffle)
+    x = W.seeded_vector(4, A.n)
+    assert np.abs(oracle.Precond(A, b).op_apply(x) - x).max() > 1e-3        # natural blocks of the shuffled matrix: not I
+    perm = reverse_cuthill_mckee(A.to_scipy(), symmetric_mode=True)
+    P = oracle.PrecondPerm(A, perm, b)
+    assert np.abs(P.op_apply(x) - x).max() <= 1e-13
+    c = P.cond_estimate(10)
+    assert c["iters_done"] == 1 and abs(c["kappa"] - 1) < 1e-12
+
+
+def test_perm_rejects_non_permutations_and_takes_variable_blocks():
+    A = W.build(1, "tiny")
+    with pytest.raises(ValueError):
+        oracle.PrecondPerm(A, np.zeros(A.n, dtype=np.int64), 4)
+    with pytest.raises(ValueError):
+        oracle.PrecondPerm(A, np.arange(A.n - 1), 4)
+    perm = W.random_permutation(A.n, 3)
+    ptr = W.random_block_ptr(A.n, seed=5, smin=1, smax=9)
+    P = oracle.PrecondPerm(A, perm, block_ptr=ptr)
+    Ad = A.to_dense()
+    Ap = Ad[np.ix_(perm, perm)]
+    Mp = np.zeros_like(Ap)
+    for k in range(len(ptr) - 1):
+        Mp[ptr[k]:ptr[k + 1], ptr[k]:ptr[k + 1]] = Ap[ptr[k]:ptr[k + 1], ptr[k]:ptr[k + 1]]
+    M = np.zeros_like(Mp)
+    M[np.ix_(perm, perm)] = Mp
+    r = W.seeded_vector(8, A.n)
+    assert np.abs(P.apply(r) - np.linalg.solve(M, r)).max() <= 1e-12 * np.abs(r).max()
