@@ -482,7 +482,6 @@ def main():
     ap.add_argument("--bsr", type=int, default=0,
                     help="1: keep a 3x3-blocked (BSR) copy of the matrix when its structure allows (config 5; SURVEY 8(f) NEXT-2); "
                          "the SpMV byte model then counts 8 nnz + 4 nnz/9, the CSR count is given beside it")
-    ap.add_argument("--spmv2d", type=int, default=0, help="bj_setup_opts_t.spmv2d: 0 automatic, 1 force, -1 never")
     ap.add_argument("--serp-keep-mb", type=int, default=0, help="bj_setup_opts_t.serp_keep_mb: 0 default (48), < 0 off")
     ap.add_argument("--graph", type=int, default=-1,
                     help="1: also time the operator apply replayed from a CUDA graph (default: only config 1, launch-bound)")
@@ -511,7 +510,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl")
     B.lib()  # fail loudly if the CUDA library is missing
-    opts = {"band": args.band, "col16": args.col16, "bsr": args.bsr, "spmv2d": args.spmv2d, "serp_keep_mb": args.serp_keep_mb}
+    opts = {"band": args.band, "col16": args.col16, "bsr": args.bsr, "serp_keep_mb": args.serp_keep_mb}
     peak, peak_src = measured_peaks()
 
     n, nnz = A.n, A.nnz

@@ -81,10 +81,7 @@ typedef struct {
     int32_t bsr;            /* 1: a handle-owned BSR(3) copy of a 3x3-blocked matrix (three unknowns per node)              */
     int32_t serp_keep_mb;   /* serpentine walk of the factor array in chains of applies: megabytes of each walk left as
                                ordinary L2 lines for the next kernel (results bit-identical).  0: default (48); < 0: off   */
-    int32_t spmv2d;         /* 2-D blocked SpMV for matrices with incoherent columns (a handle-owned bucketed copy, x slabs
-                               and y tiles in shared memory).  0: automatic (from the column-coherence statistic of the
-                               validation pass), 1: always when the sizes allow, -1: never                                 */
-    int32_t reserved[7];    /* must be zero                                                                               */
+    int32_t reserved[8];    /* must be zero                                                                               */
 } bj_setup_opts_t;
 
 typedef struct {
@@ -112,7 +109,7 @@ typedef struct {
     int64_t workspace_bytes;  /* device bytes held for temporaries and Lanczos workspace             */
     int64_t kernel_launches;  /* number of kernels this handle has launched so far                   */
     int32_t spmv_kernel;      /* 0: row-per-subwarp CSR-vector kernel, 1: TMA-streamed tile kernel,
-                                 2: TMA-streamed BSR(3) kernel (opts.bsr), 3: 2-D blocked kernel (opts.spmv2d) */
+                                 2: TMA-streamed BSR(3) kernel (opts.bsr)                              */
     int32_t spmv_lanes;       /* lanes per row chosen at setup                                       */
     int32_t solve_kernel;     /* 0: none (b=0), 1: thread-per-block (b<=8), 2: group/subwarp-per-block, 3: banded */
     int32_t fused_forward;    /* 1 if bj_op_apply fuses y = L^-1 u into the SpMV kernel               */
@@ -143,7 +140,7 @@ enum { BJ_K_SOLVE_LT = 0, BJ_K_SPMV = 1, BJ_K_SOLVE_L = 2, BJ_K_APPLY = 3, BJ_K_
 
 /* options for bj_set_option */
 enum {
-    BJ_OPT_SPMV_KERNEL = 1,   /* 0 / 1 / 3 as in bj_info_t.spmv_kernel (when built for the handle); -1 = automatic (default) */
+    BJ_OPT_SPMV_KERNEL = 1,   /* 0 / 1 as in bj_info_t.spmv_kernel; -1 = automatic (default) */
     BJ_OPT_FUSE_FORWARD = 2,  /* 0: three kernels, 1: fuse forward solve into SpMV, -1 = automatic    */
     BJ_OPT_LANCZOS_FUSE = 3,  /* 0: fast-mode Lanczos runs the unfused vector kernels; 1 / -1: the fused step (default) */
     BJ_OPT_PCG_FUSE = 4,      /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
@@ -183,6 +180,23 @@ int bj_release_cached_memory(void);
  * block (lane = row), packed lower triangles back to back.  bj_get_info reports b = -1, solve_kernel = 4.  Errors as
  * bj_setup; a layout that breaks the rules above is BJ_ERR_INVALID_ARG.  Synchronises. */
 int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out);
+
+/* SURVEY 8(f) NEXT-3, the permutation argument ("RCM or strong-coupling lines"): the paper's partition into diagonal blocks
+ * presupposes an ordering in which contiguous index ranges are the intended blocks.  perm_dev (device,
+ * n int32, read during the call only: the handle keeps its own copy) is a permutation of 0..n-1, perm[i] = ORIGINAL index of
+ * the unknown at permuted position i.  The diagonal blocks are those of P A P^T, (P A P^T)[i, j] = A[perm[i], perm[j]]:
+ *     M = P^T blockdiag(D_k) P,   D_k = (P A P^T)[kb:(k+1)b, kb:(k+1)b] = L_k L_k^T      (ragged last block as in bj_setup)
+ * and every vector of every entry point stays in the ORIGINAL ordering:
+ *     bj_solve_L: y = P^T L^-1 P r,  bj_solve_Lt: x = P^T L^-T P y,  bj_apply: z = M^-1 r,  bj_op_apply: y = (P^T L^-1 P) A (P^T L^-T P) x
+ * (orthogonally similar to the split operator of the permuted matrix: same spectrum, so bj_cond_estimate* report its
+ * kappa).  No permuted copy of A is made: the extraction looks columns up through the inverse permutation, the block solves
+ * gather and scatter through perm, the SpMV runs on A as it is.  Runs on the warp-per-block kernels of bj_setup_blocks
+ * (bj_get_info: b = -1, solve_kernel = 4; unfused Lanczos / PCG iterations; the batch entry points are INVALID_ARG).
+ * bj_setup_blocks_perm combines a permutation with block sizes 1..BJ_B_MAX given by block_ptr_host (positions in the PERMUTED
+ * ordering).  A sequence that is not a permutation is BJ_ERR_INVALID_ARG; other errors as bj_setup.  Synchronises. */
+int bj_setup_perm(const bj_csr_t* csr, int b, const int32_t* perm_dev, void* cuda_stream, bj_handle_t* out);
+int bj_setup_blocks_perm(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, const int32_t* perm_dev,
+                         void* cuda_stream, bj_handle_t* out);
 int bj_set_stream(bj_handle_t h, void* cuda_stream);
 int bj_set_option(bj_handle_t h, int option, int value);
 int bj_destroy(bj_handle_t h);

@@ -23,7 +23,8 @@ EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_setup_ex", "bj_get_setup_time",
            "bj_strerror", "bj_apply", "bj_spmv", "bj_solve_L", "bj_solve_Lt", "bj_op_apply", "bj_cond_estimate",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
            "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve",
-           "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv", "bj_setup_blocks"]
+           "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv", "bj_setup_blocks", "bj_setup_perm",
+           "bj_setup_blocks_perm"]
 
 
 class bj_csr_t(C.Structure):
@@ -33,7 +34,7 @@ class bj_csr_t(C.Structure):
 
 class bj_setup_opts_t(C.Structure):
     _fields_ = [("cuda_stream", C.c_void_p), ("band", C.c_int32), ("col16", C.c_int32), ("bsr", C.c_int32),
-                ("serp_keep_mb", C.c_int32), ("spmv2d", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("serp_keep_mb", C.c_int32), ("reserved", C.c_int32 * 8)]
 
 
 class bj_lanczos_opts_t(C.Structure):
@@ -88,6 +89,8 @@ def lib():
         L.bj_get_setup_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.bj_cond_estimate_minv.argtypes = [vp, C.POINTER(bj_lanczos_opts_t), C.POINTER(bj_lanczos_result_t)]
         L.bj_setup_blocks.argtypes = [C.POINTER(bj_csr_t), vp, i64, vp, C.POINTER(vp)]
+        L.bj_setup_perm.argtypes = [C.POINTER(bj_csr_t), i32, vp, vp, C.POINTER(vp)]
+        L.bj_setup_blocks_perm.argtypes = [C.POINTER(bj_csr_t), vp, i64, vp, vp, C.POINTER(vp)]
         L.bj_set_stream.argtypes = [vp, vp]
         L.bj_set_option.argtypes = [vp, i32, i32]
         L.bj_destroy.argtypes = [vp]
@@ -149,7 +152,7 @@ class Handle:
 
 
 def bj_setup(row_ptr, col_idx, val, b: int, stream=None, band: int = 0, col16: int = 0, bsr: int = 0,
-             serp_keep_mb: int = 0, spmv2d: int = 0) -> Handle:
+             serp_keep_mb: int = 0) -> Handle:
     """row_ptr/col_idx: int32 CUDA tensors, val: float64 CUDA tensor (borrowed).  stream: a torch stream,
     default the current one.  The keyword options are the fields of bj_setup_opts_t (bj_setup_ex)."""
     import torch
@@ -157,7 +160,7 @@ def bj_setup(row_ptr, col_idx, val, b: int, stream=None, band: int = 0, col16: i
     nnz = val.numel()
     csr = bj_csr_t(n, nnz, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32, nnz), _dptr(val, torch.float64))
     st = (stream or torch.cuda.current_stream()).cuda_stream
-    opts = bj_setup_opts_t(C.c_void_p(st), int(band), int(col16), int(bsr), int(serp_keep_mb), int(spmv2d))
+    opts = bj_setup_opts_t(C.c_void_p(st), int(band), int(col16), int(bsr), int(serp_keep_mb))
     out = C.c_void_p()
     code = lib().bj_setup_ex(C.byref(csr), int(b), C.byref(opts), C.byref(out))
     if code == BJ_ERR_NOT_SPD and out.value:
@@ -187,6 +190,33 @@ def bj_setup_blocks(row_ptr, col_idx, val, block_ptr, stream=None) -> Handle:
     st = (stream or torch.cuda.current_stream()).cuda_stream
     out = C.c_void_p()
     code = lib().bj_setup_blocks(C.byref(csr), ptr.ctypes.data_as(C.c_void_p), C.c_int64(len(ptr) - 1), C.c_void_p(st), C.byref(out))
+    if code == BJ_ERR_NOT_SPD and out.value:
+        info = bj_info_t()
+        lib().bj_get_info(out, C.byref(info))
+        lib().bj_destroy(out)
+        _check(code, int(info.bad_block))
+    _check(code)
+    return Handle(out, (row_ptr, col_idx, val), n)
+
+
+def bj_setup_perm(row_ptr, col_idx, val, b: int, perm, block_ptr=None, stream=None) -> Handle:
+    """Block-Jacobi after a symmetric permutation: perm = int32 CUDA tensor, perm[i] = original index of the unknown at
+    permuted position i; vectors stay in the original ordering.  block_ptr (host int64 sequence, optional): block sizes
+    1..32 in the permuted ordering instead of the uniform b."""
+    import numpy as np
+    import torch
+    n = row_ptr.numel() - 1
+    nnz = val.numel()
+    csr = bj_csr_t(n, nnz, _dptr(row_ptr, torch.int32), _dptr(col_idx, torch.int32, nnz), _dptr(val, torch.float64))
+    st = (stream or torch.cuda.current_stream()).cuda_stream
+    out = C.c_void_p()
+    pp = _dptr(perm, torch.int32, n)
+    if block_ptr is None:
+        code = lib().bj_setup_perm(C.byref(csr), int(b), pp, C.c_void_p(st), C.byref(out))
+    else:
+        ptr = np.ascontiguousarray(np.asarray(block_ptr, dtype=np.int64))
+        code = lib().bj_setup_blocks_perm(C.byref(csr), ptr.ctypes.data_as(C.c_void_p), C.c_int64(len(ptr) - 1), pp,
+                                          C.c_void_p(st), C.byref(out))
     if code == BJ_ERR_NOT_SPD and out.value:
         info = bj_info_t()
         lib().bj_get_info(out, C.byref(info))

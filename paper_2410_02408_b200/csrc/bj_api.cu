@@ -404,7 +404,8 @@ int bj_get_setup_time(bj_handle_t h, double* kernel_ms, int64_t* alg_bytes)
     return BJ_OK;
 }
 
-int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out)
+int bj_setup_blocks_perm(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, const int32_t* perm_dev,
+                         void* cuda_stream, bj_handle_t* out)
 {
     if (!out) return BJ_ERR_INVALID_ARG;
     *out = nullptr;
@@ -417,10 +418,27 @@ int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t 
     bj_handle_t h = nullptr;
     int rc = bj_setup_on_stream(csr, 0, cuda_stream, &h);  // validation and the SpMV plan of a b = 0 handle
     if (rc != BJ_OK) return rc;
-    rc = var_setup(h, block_ptr_host, nblocks);
+    rc = var_setup(h, block_ptr_host, nblocks, perm_dev);
     if (rc != BJ_OK && rc != BJ_ERR_NOT_SPD) { free_handle(h); return rc; }
     *out = h;  // after BJ_ERR_NOT_SPD the handle only answers bj_get_info / bj_destroy, like bj_setup
     return rc;
+}
+
+int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, void* cuda_stream, bj_handle_t* out)
+{
+    return bj_setup_blocks_perm(csr, block_ptr_host, nblocks, nullptr, cuda_stream, out);
+}
+
+int bj_setup_perm(const bj_csr_t* csr, int b, const int32_t* perm_dev, void* cuda_stream, bj_handle_t* out)
+{
+    if (!out) return BJ_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!csr || csr->n <= 0 || b < 1 || b > BJ_B_MAX || !perm_dev) return BJ_ERR_INVALID_ARG;
+    const int64_t nblocks = (csr->n + b - 1) / b;
+    std::vector<int64_t> ptr((size_t)nblocks + 1);
+    for (int64_t k = 0; k < nblocks; ++k) ptr[k] = k * b;
+    ptr[nblocks] = csr->n;  // ragged last block
+    return bj_setup_blocks_perm(csr, ptr.data(), nblocks, perm_dev, cuda_stream, out);
 }
 
 int bj_release_cached_memory(void)

@@ -1,6 +1,11 @@
 // Variable-size Jacobi blocks ("variable-size / supervariable blocks").
 // block_ptr[0..nblocks] delimits contiguous index ranges of 1..32 rows; block k is the dense diagonal slice
-// D_k = A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:254-263 with a per-block size), D_k = L_k L_k^T.
+// D_k = A[p_k:p_{k+1}, p_k:p_{k+1}] (the listing of PAPER.md:191-197 with a per-block size), D_k = L_k L_k^T.
+// Optional symmetric PERMUTATION ("a permutation argument (RCM or strong-coupling lines)"):
+// perm[i] = original index of the unknown at permuted position i; the blocks are those of P A P^T,
+// (P A P^T)[i, j] = A[perm[i], perm[j]], i.e. M = P^T blockdiag(D_k) P, and every vector stays in the ORIGINAL ordering:
+// the extraction looks columns up through the inverse permutation, the solves gather their right-hand side through perm
+// and scatter the result back through it.  No permuted copy of A is made; the SpMV runs on A as it is.
 // Storage: the lower triangles, column-major packed, back to back: block k starts at foff[k] = sum_{q<k} s_q (s_q+1)/2,
 // element (i, j), i >= j, at j s - j (j-1)/2 + (i - j); the diagonal slot holds 1 / l_jj.
 // One warp per block in both kernels (lane = row): the block sizes differ, so neither the 32-block interleave of the
@@ -28,7 +33,8 @@ __device__ __forceinline__ int var_col_start(int j, int s) { return j * s - (j *
 __global__ void __launch_bounds__(kVarWarps * 32)
 extract_factor_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_t* __restrict__ foff,
                           const int32_t* __restrict__ rp, const int32_t* __restrict__ ci, const double* __restrict__ val,
-                          double* __restrict__ fac, Status* __restrict__ status)
+                          double* __restrict__ fac, Status* __restrict__ status,
+                          const int32_t* __restrict__ perm, const int32_t* __restrict__ pinv)  // both null: no permutation
 {
     __shared__ double Dsh[kVarWarps][kVarMax * (kVarMax + 1)];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -38,9 +44,9 @@ extract_factor_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, con
     double* D = Dsh[warp];  // row i at D + i * 33
     if (lane < s) {
         for (int j = 0; j < s; ++j) D[lane * (kVarMax + 1) + j] = 0.0;
-        const int row = lo + lane;
+        const int row = perm ? perm[lo + lane] : lo + lane;
         for (int e = rp[row]; e < rp[row + 1]; ++e) {
-            const int c = ci[e] - lo;
+            const int c = (pinv ? pinv[ci[e]] : ci[e]) - lo;  // position of the column in the permuted ordering
             if (c >= 0 && c <= lane) D[lane * (kVarMax + 1) + c] = val[e];  // lower triangle only
         }
     }
@@ -83,7 +89,7 @@ extract_factor_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, con
 template <int DIR>
 __global__ void __launch_bounds__(kVarWarps * 32)
 solve_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_t* __restrict__ foff,
-                 const double* __restrict__ fac, const double* in, double* out)
+                 const double* __restrict__ fac, const double* in, double* out, const int32_t* __restrict__ perm)
 {
     __shared__ double Fsh[kVarWarps][kVarPacked];
     pdl_trigger();
@@ -96,7 +102,9 @@ solve_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_
     const int P = s * (s + 1) / 2;
     for (int e = lane; e < P; e += 32) F[e] = ld_stream(f + e);  // factors never change after setup
     pdl_wait();                                                  // `in` may come from the previous kernel
-    double v = lane < s ? in[lo + lane] : 0.0;
+    // row of this lane in the caller's (original) ordering: in == out stays safe, a lane reads and writes one index
+    const int row = lane < s ? (perm ? perm[lo + lane] : lo + lane) : 0;
+    double v = lane < s ? in[row] : 0.0;
     __syncwarp();
     if (DIR == 0 || DIR == 2) {
         for (int j = 0; j < s; ++j) {
@@ -113,7 +121,18 @@ solve_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_
             if (lane < j) v -= F[var_col_start(lane, s) + (j - lane)] * xj;  // l_{j,lane}
         }
     }
-    if (lane < s) out[lo + lane] = v;
+    if (lane < s) out[row] = v;
+}
+
+// pinv[perm[i]] = i; flag[0] |= 1 when an entry is out of range or occurs twice (pinv is preset to -1)
+__global__ void __launch_bounds__(256)
+perm_invert_kernel(int64_t n, const int32_t* __restrict__ perm, int32_t* __restrict__ pinv, int* __restrict__ flag)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int p = perm[i];
+    if (p < 0 || p >= n) { atomicOr(flag, 1); return; }
+    if (atomicExch(&pinv[p], (int)i) != -1) atomicOr(flag, 1);
 }
 
 }  // namespace
@@ -121,6 +140,10 @@ solve_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_
 void var_free(bj_handle_s* h)
 {
     if (h->var_fac) h->factor_bytes = 0;
+    cudaFree(h->var_perm);
+    cudaFree(h->var_pinv);
+    h->var_perm = nullptr;
+    h->var_pinv = nullptr;
     cudaFree(h->var_bptr);
     cudaFree(h->var_foff);
     cudaFree(h->var_fac);
@@ -131,8 +154,30 @@ void var_free(bj_handle_s* h)
 
 // Turns a b = 0 handle (validated matrix, SpMV plan) into a variable-block handle: uploads the block layout, extracts
 // and factors every block.  ptr_host was validated by the caller.
-int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks)
+int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks, const int32_t* perm_dev)
 {
+    cudaStream_t st = h->stream;
+    if (perm_dev) {
+        // the handle keeps its own copy of the permutation and of its inverse; a sequence that is not a permutation of
+        // 0..n-1 is an invalid argument
+        const size_t pb = sizeof(int32_t) * (size_t)h->n;
+        if (cudaMalloc((void**)&h->var_perm, pb) != cudaSuccess || cudaMalloc((void**)&h->var_pinv, pb) != cudaSuccess) {
+            cudaGetLastError();
+            var_free(h);
+            return BJ_ERR_ALLOC;
+        }
+        int* flag = &h->status->pad;
+        BJ_CUDA(cudaMemcpyAsync(h->var_perm, perm_dev, pb, cudaMemcpyDeviceToDevice, st));
+        BJ_CUDA(cudaMemsetAsync(h->var_pinv, 0xff, pb, st));
+        BJ_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
+        perm_invert_kernel<<<(unsigned)((h->n + 255) / 256), 256, 0, st>>>(h->n, h->var_perm, h->var_pinv, flag);
+        h->launches++;
+        int bad = 1;
+        BJ_CUDA(cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+        BJ_CUDA(cudaStreamSynchronize(st));
+        if (bad) { var_free(h); return BJ_ERR_INVALID_ARG; }
+        h->workspace_bytes += 2 * (int64_t)pb;
+    }
     std::vector<int32_t> bp((size_t)nblocks + 1);
     std::vector<int64_t> fo((size_t)nblocks + 1);
     int64_t off = 0;
@@ -153,7 +198,6 @@ int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks)
         var_free(h);
         return BJ_ERR_ALLOC;
     }
-    cudaStream_t st = h->stream;
     BJ_CUDA(cudaMemcpyAsync(h->var_bptr, bp.data(), sizeof(int32_t) * bp.size(), cudaMemcpyHostToDevice, st));
     BJ_CUDA(cudaMemcpyAsync(h->var_foff, fo.data(), sizeof(int64_t) * fo.size(), cudaMemcpyHostToDevice, st));
     h->nblocks = nblocks;
@@ -162,7 +206,7 @@ int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks)
     h->factor_bytes = (int64_t)sizeof(double) * off + (int64_t)(sizeof(int32_t) * bp.size() + sizeof(int64_t) * fo.size());
     const unsigned grid = (unsigned)((nblocks + kVarWarps - 1) / kVarWarps);
     extract_factor_var_kernel<<<grid, kVarWarps * 32, 0, st>>>(nblocks, h->var_bptr, h->var_foff, h->row_ptr, h->col_idx, h->val,
-                                                               h->var_fac, h->status);
+                                                               h->var_fac, h->status, h->var_perm, h->var_pinv);
     h->launches++;
     BJ_CUDA(cudaGetLastError());
     Status stt;
@@ -183,13 +227,16 @@ int launch_solve_var(bj_handle_s* h, int dir, const double* in, double* out)
     cudaError_t e;
     if (dir == 0)
         e = launch_kernel(solve_var_kernel<0>, dim3(grid), dim3(kVarWarps * 32), 0, h->stream, pdl, h->nblocks,
-                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out);
+                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out,
+                          (const int32_t*)h->var_perm);
     else if (dir == 1)
         e = launch_kernel(solve_var_kernel<1>, dim3(grid), dim3(kVarWarps * 32), 0, h->stream, pdl, h->nblocks,
-                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out);
+                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out,
+                          (const int32_t*)h->var_perm);
     else
         e = launch_kernel(solve_var_kernel<2>, dim3(grid), dim3(kVarWarps * 32), 0, h->stream, pdl, h->nblocks,
-                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out);
+                          (const int32_t*)h->var_bptr, (const int64_t*)h->var_foff, (const double*)h->var_fac, in, out,
+                          (const int32_t*)h->var_perm);
     if (e != cudaSuccess) { set_cuda_error(e, "solve_var_kernel"); return BJ_ERR_CUDA; }
     h->launches++;
     return BJ_OK;

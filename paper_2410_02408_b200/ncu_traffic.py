@@ -29,7 +29,7 @@ def kernel_kind(name: str):
     dirs = {0: "solve_L", 1: "solve_Lt", 2: "apply"}
     if base == "spmv_stream_kernel":
         return "spmv_solve_L" if arg(1) == 1 else "spmv"
-    if base in ("spmv_vector_kernel", "spmv_bsr3_kernel", "spmv2d_kernel"):
+    if base in ("spmv_vector_kernel", "spmv_bsr3_kernel"):
         return "spmv"
     if base == "solve_small_kernel":
         return dirs[arg(1)]

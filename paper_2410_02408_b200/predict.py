@@ -24,11 +24,16 @@ import numpy as np
 DEFAULT_BLOCKS = (1, 2, 3, 4, 8, 16, 24, 32)
 
 
-def coupling_captured(A, b: int) -> float:
+def coupling_captured(A, b: int, perm=None) -> float:
     """c(b): fraction of the off-diagonal absolute weight inside the diagonal b x b blocks (contiguous index ranges,
-    DESIGN.md reading 8)."""
+    DESIGN.md reading 8).  perm (optional, perm[i] = original index at permuted position i): the blocks are contiguous
+    ranges of the PERMUTED ordering (bj_setup_perm)."""
     rows = np.repeat(np.arange(A.n, dtype=np.int64), np.diff(A.row_ptr.astype(np.int64)))
     cols = A.col_idx.astype(np.int64)
+    if perm is not None:
+        pinv = np.empty(A.n, dtype=np.int64)
+        pinv[np.asarray(perm, dtype=np.int64)] = np.arange(A.n, dtype=np.int64)
+        rows, cols = pinv[rows], pinv[cols]
     w = np.abs(A.val)
     off = rows != cols
     total = float(w[off].sum())
@@ -56,6 +61,58 @@ def suggest_block(A, blocks=DEFAULT_BLOCKS, saturation: float = 0.98) -> dict:
         choice = min(b for b in blocks if c[b] >= saturation * best)
     f.update({"suggested_b": int(choice), "rule": f"smallest b with c(b) >= {saturation} max c; b = min when max c < 0.02"})
     return f
+
+
+def strong_coupling_lines(A, b: int) -> np.ndarray:
+    """An ordering for bj_setup_perm ("a permutation argument (RCM or strong-coupling lines)"): greedy
+    chains of up to b unknowns that follow the STRONGEST remaining coupling.  Starting from the lowest unvisited index, a
+    chain is extended by the unvisited neighbour with the largest |a_ij| of its last member until it has b members or no
+    unvisited neighbour is left; chains are laid out one after the other, so each fills one diagonal block (short chains
+    are padded by the start of the next one).  On a grid operator with one strong direction the chains are the grid
+    lines along it, whatever the numbering.  Returns perm (int32), perm[i] = original index at permuted position i.
+    Host-side, O(nnz) Python steps: meant for matrices up to ~10^6 entries."""
+    n = int(A.n)
+    rp = A.row_ptr.tolist()
+    ci = A.col_idx.tolist()
+    w = np.abs(A.val).tolist()
+    visited = bytearray(n)
+    perm = []
+    start = 0
+    while len(perm) < n:
+        while visited[start]:
+            start += 1
+        cur = start
+        visited[cur] = 1
+        perm.append(cur)
+        for _ in range(b - 1):
+            best, bw = -1, -1.0
+            for e in range(rp[cur], rp[cur + 1]):
+                c = ci[e]
+                if not visited[c] and w[e] > bw:   # ties: the first (lowest column) wins -- deterministic
+                    best, bw = c, w[e]
+            if best < 0:
+                break
+            visited[best] = 1
+            perm.append(best)
+            cur = best
+    return np.asarray(perm, dtype=np.int32)
+
+
+def rcm_permutation(A) -> np.ndarray:
+    """Reverse Cuthill-McKee ordering (scipy.sparse.csgraph, a library routine): makes every connected component -- and,
+    for banded structure, every neighbourhood -- contiguous.  perm[i] = original index at permuted position i."""
+    from scipy.sparse.csgraph import reverse_cuthill_mckee
+    return np.asarray(reverse_cuthill_mckee(A.to_scipy(), symmetric_mode=True), dtype=np.int32)
+
+
+def suggest_ordering(A, b: int) -> dict:
+    """Which of {natural, strong-coupling lines, RCM} captures the most coupling inside blocks of size b: the same
+    structural feature as suggest_block, applied to the ordering.  Returns the captured shares and the best perm
+    (None = keep the natural ordering)."""
+    cands = {"natural": None, "lines": strong_coupling_lines(A, b), "rcm": rcm_permutation(A)}
+    captured = {k: coupling_captured(A, b, p) for k, p in cands.items()}
+    best = max(captured, key=lambda k: (captured[k], k == "natural"))   # ties: keep the natural ordering
+    return {"captured": captured, "best": best, "perm": cands[best]}
 
 
 def main():

@@ -246,8 +246,10 @@ def config4(n: int = 2048, eps: float = 1e-4, gamma_over_eps: float = 0.1, x_fas
     x, y = xg.ravel(), yg.ravel()
     idx = sy * y + sx * x
     cols, vals, mask = [], [], []
-    for dx in (-1, 0, 1):
-        for dy in (-1, 0, 1):
+    # the offset along the slow index is the outer loop, so that the columns of a row ascend (canonical CSR)
+    for dslow in (-1, 0, 1):
+        for dfast in (-1, 0, 1):
+            dx, dy = (dfast, dslow) if x_fastest else (dslow, dfast)
             cols.append(idx + sy * dy + sx * dx)
             if dx == 0 and dy == 0:
                 v = 2.0 * eps + 2.0

@@ -888,7 +888,7 @@ def test_handles_release_their_device_memory(B, torch_):
     free0, _ = torch_.cuda.mem_get_info()
     for rep in range(12):
         for b in (0, 3, 8, 24):
-            h = B.bj_setup(rp, ci, val, b, band=1, col16=1, bsr=1, spmv2d=1)
+            h = B.bj_setup(rp, ci, val, b, band=1, col16=1, bsr=1)
             B.bj_op_apply(h, x)
             B.bj_cond_estimate_ex(h, 6, reorth=bool(rep & 1))
             B.bj_pcg_solve(h, x, max_iters=4, rtol=0.0)
@@ -1075,3 +1075,116 @@ def test_serpentine_walk_of_the_block_solves(B, torch_, rel):
         for keep_mb in ("1", "48"):
             for got, ref in zip(out[keep_mb], out["0"]):
                 assert np.array_equal(got, ref), f"n={A.n} b={b} keep={keep_mb}"
+
+
+# ------------------------------------------------------------------ permutation argument (NEXT-3) --------
+def _setup_perm(B, torch_, A, b, perm, block_ptr=None):
+    rp, ci, val = dev(torch_, A.row_ptr), dev(torch_, A.col_idx), dev(torch_, A.val)
+    pd = dev(torch_, np.asarray(perm, dtype=np.int32))
+    return B.bj_setup_perm(rp, ci, val, b, pd, block_ptr=block_ptr), (rp, ci, val, pd)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_permuted_blocks_match_oracle(B, torch_, rel, cfg):
+    """bj_setup_perm with a seeded random permutation (the hardest case for the gathers): every apply entry point, in the
+    ORIGINAL ordering, element by element against oracle.PrecondPerm (explicit P A P^T); kappa with full
+    reorthogonalisation to the bar of the north star; in-place calls; ragged last block."""
+    A = mat(cfg, "small" if cfg != 5 else "tiny")
+    for b in sorted(set(W.BLOCK_SIZES[cfg] + [7])):
+        perm = W.random_permutation(A.n, seed=60 + cfg + b)
+        h, keep = _setup_perm(B, torch_, A, b, perm)
+        info = B.bj_get_info(h)
+        assert info["solve_kernel"] == 4 and info["nblocks"] == (A.n + b - 1) // b
+        P = oracle.PrecondPerm(A, perm, b)
+        for seed in (7, 8):
+            x = W.seeded_vector(seed, A.n)
+            xd = dev(torch_, x)
+            for name in ("bj_solve_L", "bj_solve_Lt", "bj_apply", "bj_op_apply"):
+                got = getattr(B, name)(h, xd).cpu().numpy()
+                e2, ei = rel(got, getattr(P, name[3:])(x))
+                assert e2 <= TOL_APPLY and ei <= TOL_APPLY, (cfg, b, name, e2, ei)
+            y = xd.clone()
+            B.bj_op_apply(h, y, y)
+            assert rel(y.cpu().numpy(), P.op_apply(x))[0] <= TOL_APPLY
+        g = B.bj_cond_estimate_ex(h, 30, reorth=True)
+        c = P.cond_estimate(30, reorth=True)
+        assert g["iters_done"] == c["iters_done"]
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (cfg, b, g["kappa"], c["kappa"])
+        B.bj_destroy(h)
+
+
+def test_line_permutation_gives_xfastest_config4_the_yfastest_preconditioner(B, torch_, rel):
+    """Config 4 numbered along the weak direction: natural blocks of 16 are nearly useless; with the line permutation
+    (workloads.config4_line_permutation, and the one predict.strong_coupling_lines finds by itself) the handle reproduces
+    the y-fastest results: the operator equals the y-fastest handle's in permuted coordinates, kappa equals the oracle's."""
+    from paper_2410_02408_b200 import predict
+    n, b = 96, 16
+    Ax, Ay = W.config4(n, x_fastest=True), W.config4(n)
+    perm = W.config4_line_permutation(n)
+    hp, keep = _setup_perm(B, torch_, Ax, b, perm)
+    hy, keepy = B.setup_from_host(Ay, b)
+    x = W.seeded_vector(4, Ax.n)
+    yp = B.bj_op_apply(hp, dev(torch_, x)).cpu().numpy()          # original (x-fastest) ordering
+    yy = B.bj_op_apply(hy, dev(torch_, x[perm])).cpu().numpy()    # the y-fastest handle sees P x
+    e2, ei = rel(yp[perm], yy)
+    assert e2 <= TOL_APPLY and ei <= TOL_APPLY
+    P = oracle.PrecondPerm(Ax, perm, b)
+    g = B.bj_cond_estimate_ex(hp, 40, reorth=True)
+    assert abs(g["kappa"] / P.cond_estimate(40)["kappa"] - 1) <= TOL_KAPPA
+    hn, keepn = B.setup_from_host(Ax, b)                          # natural blocks of the badly numbered matrix
+    k_nat = B.bj_cond_estimate_ex(hn, 200, reorth=True)["kappa"]
+    k_perm = B.bj_cond_estimate_ex(hp, 200, reorth=True)["kappa"]
+    assert k_nat > 3 * k_perm
+    lines = predict.strong_coupling_lines(Ax, b)                   # found from the matrix alone
+    hl, keepl = _setup_perm(B, torch_, Ax, b, lines)
+    k_lines = B.bj_cond_estimate_ex(hl, 200, reorth=True)["kappa"]
+    assert abs(k_lines / k_perm - 1) < 0.05                        # same blocks in another order: same spectrum
+    rhs = dev(torch_, W.seeded_vector(17, Ax.n))
+    it_nat = B.bj_pcg_solve(hn, rhs, max_iters=3000, rtol=1e-3)["iters"]
+    r = B.bj_pcg_solve(hl, rhs, max_iters=3000, rtol=1e-3)
+    assert r["converged"] and r["true_relres"] <= 1.2e-3 and r["iters"] < 0.7 * it_nat
+    for h in (hp, hy, hn, hl):
+        B.bj_destroy(h)
+
+
+def test_rcm_restores_the_block_diagonal_model_on_the_device(B, torch_, rel):
+    """PAPER.md:80 hidden by a shuffle: with the RCM ordering (predict.rcm_permutation) M = A, the operator is the
+    identity, Lanczos stops at one step, PCG converges in one step; variable block sizes combine with the permutation;
+    a sequence that is not a permutation is rejected."""
+    from paper_2410_02408_b200 import predict
+    sizes = [5, 1, 32, 7, 16, 2, 24] * 6
+    A0 = W.direct_sum_spd(sizes)
+    A = W.permuted(A0, W.random_permutation(A0.n, seed=11))
+    # RCM keeps components contiguous but in its own order and with its own internal order: recover the component sizes
+    perm = predict.rcm_permutation(A)
+    import scipy.sparse.csgraph as csg
+    ncomp, label = csg.connected_components(A.to_scipy(), directed=False)
+    lab = label[perm]
+    cuts = np.flatnonzero(np.diff(lab)) + 1
+    ptr = np.concatenate([[0], cuts, [A.n]])
+    assert len(ptr) - 1 == len(sizes)
+    h, keep = _setup_perm(B, torch_, A, 0, perm, block_ptr=ptr)
+    x = W.seeded_vector(2, A.n)
+    y = B.bj_op_apply(h, dev(torch_, x)).cpu().numpy()
+    assert np.abs(y - x).max() <= 1e-13
+    g = B.bj_cond_estimate_ex(h, 10, reorth=True)
+    assert g["iters_done"] == 1 and abs(g["kappa"] - 1) <= 1e-12
+    r = B.bj_pcg_solve(h, dev(torch_, x), max_iters=10, rtol=1e-12)
+    assert r["iters"] == 1 and r["true_relres"] <= 1e-13
+    P = oracle.PrecondPerm(A, perm, block_ptr=ptr)
+    e2, ei = rel(B.bj_apply(h, dev(torch_, x)).cpu().numpy(), P.apply(x))
+    assert e2 <= TOL_APPLY
+    B.bj_destroy(h)
+    rp, ci, val, pd = keep
+    bad = perm.copy()
+    bad[3] = bad[4]
+    for seq in (bad, np.full(A.n, A.n, dtype=np.int32)):
+        with pytest.raises(B.BJError) as e:
+            B.bj_setup_perm(rp, ci, val, 4, dev(torch_, seq.astype(np.int32)))
+        assert e.value.code == B.BJ_ERR_INVALID_ARG
+    # identity permutation = bj_setup_blocks with equal sizes = the uniform handle (to the tolerance)
+    hi = B.bj_setup_perm(rp, ci, val, 8, dev(torch_, np.arange(A.n, dtype=np.int32)))
+    hu = B.bj_setup(rp, ci, val, 8)
+    e2, ei = rel(B.bj_op_apply(hi, dev(torch_, x)).cpu().numpy(), B.bj_op_apply(hu, dev(torch_, x)).cpu().numpy())
+    assert e2 <= TOL_APPLY
+    B.bj_destroy(hi); B.bj_destroy(hu)

@@ -97,3 +97,35 @@ def test_coupling_captured_properties_and_suggestions():
     # anisotropic operator ordered along the strong direction: long line blocks; the 2x2x2 node patch of config 5: b = 24
     assert predict.suggest_block(W.build(4, "small"))["suggested_b"] >= 16
     assert predict.suggest_block(W.build(5, "small"))["suggested_b"] == 24
+
+
+# ---------------------------------------------------------------- orderings for bj_setup_perm ------
+def test_orderings_recover_the_block_structure_that_the_numbering_hides():
+    import numpy as np
+    from paper_2410_02408_b200 import predict
+    from paper_2410_02408_b200 import workloads as W
+    # config 4 numbered along the WEAK direction: natural blocks capture almost nothing, the strong-coupling lines are
+    # exactly the y-lines of the BASELINE.json ordering (same blocks, another block order)
+    n, b = 48, 16
+    Ax, Ay = W.config4(n, x_fastest=True), W.config4(n)
+    for M in (Ax, Ay):   # canonical CSR in both numberings: columns strictly ascend inside every row
+        assert all(np.all(np.diff(M.col_idx[M.row_ptr[i]:M.row_ptr[i + 1]]) > 0) for i in range(M.n))
+    lines = predict.strong_coupling_lines(Ax, b)
+    assert sorted(lines.tolist()) == list(range(Ax.n))
+    c_nat, c_lines = predict.coupling_captured(Ax, b), predict.coupling_captured(Ax, b, lines)
+    c_y = predict.coupling_captured(Ay, b)
+    assert c_nat < 0.01 and abs(c_lines - c_y) < 1e-12 and c_y > 0.9
+    assert abs(predict.coupling_captured(Ax, b, W.config4_line_permutation(n)) - c_y) < 1e-12
+    blocks = {frozenset(int(v) for v in lines[k:k + b]) for k in range(0, Ax.n, b)}
+    want = {frozenset(int(x + n * y) for y in range(y0, y0 + b)) for x in range(n) for y0 in range(0, n, b)}
+    assert blocks == want
+    s = predict.suggest_ordering(Ax, b)
+    assert s["best"] == "lines" and predict.suggest_ordering(Ay, b)["best"] == "natural"
+    # a shuffled block-diagonal matrix: RCM makes the components contiguous again, everything is captured
+    A0 = W.block_diagonal_spd(30, 6)
+    A = W.permuted(A0, W.random_permutation(A0.n, 5))
+    assert predict.coupling_captured(A, 6) < 0.2
+    assert abs(predict.coupling_captured(A, 6, predict.rcm_permutation(A)) - 1.0) < 1e-15
+    assert abs(predict.coupling_captured(A, 6, predict.strong_coupling_lines(A, 6)) - 1.0) < 1e-15
+    # identity permutation = no permutation
+    assert predict.coupling_captured(Ay, b, np.arange(Ay.n)) == c_y
