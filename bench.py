@@ -317,11 +317,21 @@ def roofline_of(kern: dict, cfg: int, b: int, peak: float, peak_src: str) -> dic
     return r
 
 
+def var_block_bytes(n: int, nnz: int, info: dict, perm: bool) -> dict:
+    """Byte model of the warp-per-block kernels of bj_setup_blocks / bj_setup_perm (their own accounting): a solve pass
+    reads the packed factors with the block pointers and factor offsets (info.factor_bytes holds all three), the right-hand
+    side and, with a permutation, 4 N bytes of perm; it writes the result."""
+    spmv = 12 * nnz + 4 * (n + 1) + 16 * n
+    solve = info["factor_bytes"] + 16 * n + (4 * n if perm else 0)
+    return {"spmv": spmv, "solve_L": solve, "solve_Lt": solve, "apply": solve, "spmv_solve_L": spmv + solve,
+            "op_apply": spmv + 2 * solve}
+
+
 def measure_operator(B, torch, h, cfg: int, n: int, nnz: int, b: int, steps: int, warmup: int, local: int,
-                     peak: float, peak_src: str) -> dict:
+                     peak: float, peak_src: str, ab: dict | None = None) -> dict:
     """The operator apply on one handle: rotating inputs, clocks sampled during the timed region, per-kernel profile."""
     info = B.bj_get_info(h)
-    ab = byte_model(n, nnz, b, info)
+    ab = ab or byte_model(n, nnz, b, info)
     rot = Rotation(B, torch, h, n)
     fn = lambda x, y: B.bj_op_apply(h, x, y)  # noqa: E731
     for _ in range(warmup):
@@ -396,6 +406,43 @@ def graph_replay_us(B, torch, h, x, y, steps: int) -> dict:
     B.bj_set_stream(h, torch.cuda.current_stream())
     del graph
     return {"applies_per_graph": G, "replays": reps, "us_per_apply": gus, "applies_per_s": 1e6 / gus}
+
+
+def permutation_section(B, torch, args, local: int, peak: float, peak_src: str) -> dict:
+    """SURVEY 8(f) NEXT-3: config 4 numbered along the WEAK direction (x fastest).  Natural blocks of 16 are nearly useless;
+    bj_setup_perm with the line permutation gives back the y-fastest preconditioner without a permuted copy of A.  Reports
+    the kappa estimates (m steps, parity mode) and the operator apply of the warp-per-block kernels with their byte model."""
+    t0 = time.perf_counter()
+    A = W.config4(x_fastest=True)
+    n, nnz, b, m = A.n, A.nnz, 16, args.lanczos_iters
+    rp, ci, val = (torch.from_numpy(a).cuda() for a in (A.row_ptr, A.col_idx, A.val))
+    perm = torch.from_numpy(W.config4_line_permutation(A.meta["n"])).cuda()
+    out = {"workload": A.meta.get("name"), "n": n, "nnz": nnz, "block": b, "lanczos_iters": m}
+    hn = B.bj_setup(rp, ci, val, b)
+    r = B.bj_cond_estimate_ex(hn, m, reorth=True)
+    out["natural_blocks"] = {"kappa_est": r["kappa"], "res_min": r["res_min"], "res_max": r["res_max"]}
+    rhs = B.bj_seeded_vector(hn, 17)
+    pr = B.bj_pcg_solve(hn, rhs, max_iters=3000, rtol=1e-3)
+    out["natural_blocks"]["pcg_iters_to_1e-3"] = pr["iters"] if pr["converged"] else None
+    B.bj_destroy(hn)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    hp = B.bj_setup_perm(rp, ci, val, b, perm)
+    torch.cuda.synchronize()
+    setup_ms = 1e3 * (time.perf_counter() - t1)
+    r = B.bj_cond_estimate_ex(hp, m, reorth=True)
+    info = B.bj_get_info(hp)
+    ab = var_block_bytes(n, nnz, info, True)
+    op = measure_operator(B, torch, hp, 4, n, nnz, b, max(50, args.steps), max(args.warmup, 10), local, peak, peak_src, ab=ab)
+    pr = B.bj_pcg_solve(hp, rhs, max_iters=3000, rtol=1e-3)
+    out["line_permutation"] = {"kappa_est": r["kappa"], "res_min": r["res_min"], "res_max": r["res_max"],
+                               "pcg_iters_to_1e-3": pr["iters"] if pr["converged"] else None, "setup_wall_ms": setup_ms,
+                               "us_per_apply": op["us_per_apply"], "alg_bytes": op["alg_bytes"], "gbs": op["gbs"],
+                               "frac_of_measured": op["frac_of_measured"], "kernels": op["kernels"],
+                               "byte_model": "12 nnz + 4 (N + 1) + 16 N + 2 x (factor_bytes + 16 N + 4 N perm)"}
+    B.bj_destroy(hp)
+    out["section_seconds"] = time.perf_counter() - t0
+    return out
 
 
 def other_configs(B, torch, args, local: int, peak: float, peak_src: str) -> dict:
@@ -724,6 +771,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_extras and not args.no_configs and args.config == 2 and args.scale == "full":
         torch.cuda.empty_cache()
         line["configs"] = other_configs(B, torch, args, local, peak, peak_src)
+        line["permutation"] = permutation_section(B, torch, args, local, peak, peak_src)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -192,31 +192,56 @@ multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const d
     }
 }
 
-// w[i] -= c_0 V_0[i]; w[i] -= c_1 V_1[i]; ... in that order; optional partial of w . w
+// w[i] -= c_0 V_0[i]; w[i] -= c_1 V_1[i]; ... in that order; optional partial of w . w.
+// Same sweep structure as multidot_partial_kernel: eight columns at a time over the CTA's whole chunk of rows, so that every
+// column is read in one contiguous run per CTA (a first version walked all columns row by row: 50 interleaved 2 KB pieces per
+// CTA, 4.25 TB/s against the 6.3 TB/s of the dot kernel); the chunk of w waits in shared memory between the sweeps.
+constexpr int kAxpyRowsMax = 5888;  // rows of w a CTA holds at a time (46 KB of shared memory; longer chunks go piece by piece)
 __global__ void __launch_bounds__(kReduceThreads)
 multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w,
                  const double* __restrict__ coef, double* __restrict__ PB, int want_norm,
-                 const int* __restrict__ done)
+                 const int* __restrict__ done, int piece)
 {
+    extern __shared__ double wsh[];
     __shared__ double sh[kReduceThreads / 32];
     pdl_trigger();
     pdl_wait();
     if (done[0]) return;
     const Chunk c = my_chunk(n);
     double s = 0.0;
-    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) {
-        double wi = w[i];
-        int q = 0;
-        for (; q + kDotCols <= nv; q += kDotCols) {  // eight loads in flight, subtraction order unchanged
-            double vq[kDotCols];
+    for (int64_t lo = c.lo; lo < c.hi; lo += piece) {
+        const int rows = (int)(c.hi - lo < piece ? c.hi - lo : piece);
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) wsh[r] = w[lo + r];  // a thread re-reads only what it wrote
+        for (int q0 = 0; q0 < nv; q0 += kDotCols) {
+            const int live = nv - q0 < kDotCols ? nv - q0 : kDotCols;
+            double cq[kDotCols];
 #pragma unroll
-            for (int d = 0; d < kDotCols; ++d) vq[d] = V[(int64_t)(q + d) * n + i];
+            for (int d = 0; d < kDotCols; ++d) cq[d] = d < live ? coef[q0 + d] : 0.0;
+            if (live == kDotCols) {
+                for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+                    double vq[kDotCols];
 #pragma unroll
-            for (int d = 0; d < kDotCols; ++d) wi -= coef[q + d] * vq[d];
+                    for (int d = 0; d < kDotCols; ++d) vq[d] = V[(int64_t)(q0 + d) * n + lo + r];
+                    double wi = wsh[r];
+#pragma unroll
+                    for (int d = 0; d < kDotCols; ++d) wi -= cq[d] * vq[d];
+                    wsh[r] = wi;
+                }
+            } else {
+                for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+                    double wi = wsh[r];
+#pragma unroll
+                    for (int d = 0; d < kDotCols; ++d)
+                        if (d < live) wi -= cq[d] * V[(int64_t)(q0 + d) * n + lo + r];
+                    wsh[r] = wi;
+                }
+            }
         }
-        for (; q < nv; ++q) wi -= coef[q] * V[(int64_t)q * n + i];
-        w[i] = wi;
-        s = fma(wi, wi, s);
+        for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+            const double wi = wsh[r];
+            w[lo + r] = wi;
+            s = fma(wi, wi, s);
+        }
     }
     if (want_norm) {
         s = block_sum(s, sh);
@@ -224,23 +249,22 @@ multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __rest
     }
 }
 
-// one CTA: out[q] = sum_cta partial[cta * stride + q].  One WARP per coefficient: lane l adds the partials of CTAs
-// l, l + 32, .. (independent loads in flight), then a fixed shuffle tree -- a fixed order, bitwise reproducible.
+// out[q] = sum_cta partial[cta * stride + q]: one CTA per coefficient (a single CTA for all of them took 39 us at 50 vectors,
+// one tenth of a parity-mode step).  Thread t adds the partials of CTAs t, t + 256, .. in that order, then the fixed block
+// tree: bitwise reproducible.
 __global__ void __launch_bounds__(256)
 finalize_multi_kernel(int nparts, int nv, const double* __restrict__ partial, int stride,
                       double* __restrict__ out, const int* __restrict__ done)
 {
+    __shared__ double sh[8];
     pdl_trigger();
     pdl_wait();
     if (done[0]) return;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    for (int q = warp; q < nv; q += nw) {
-        double s = 0.0;
-        for (int p = lane; p < nparts; p += 32) s += partial[(int64_t)p * stride + q];
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
-        if (lane == 0) out[q] = s;
-    }
+    const int q = blockIdx.x;
+    double s = 0.0;
+    for (int p = threadIdx.x; p < nparts; p += blockDim.x) s += partial[(int64_t)p * stride + q];
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) out[q] = s;
 }
 
 int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v)
@@ -394,6 +418,9 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     cudaStream_t st = h->stream;
     const int stride = m + 1;
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
+    const int64_t chunk_rows = (n + G - 1) / G;  // rows per CTA of the vector kernels (my_chunk)
+    const int axpy_piece = (int)std::min<int64_t>(chunk_rows, kAxpyRowsMax);
+    const size_t axpy_smem = (size_t)axpy_piece * sizeof(double);
 
     BJ_CUDA(cudaMemsetAsync(z.alpha, 0, sizeof(double) * (2 * (size_t)z.cap_iters + 8 + 2), st));  // alpha, beta, scal, done
 
@@ -471,10 +498,13 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
             for (int pass = 0; pass < 2; ++pass) {
                 BJ_LAUNCH(multidot_partial_kernel, G, kReduceThreads, n, j + 1, (const double*)z.V,
                           (const double*)z.w, PM, stride, (const int*)z.done);
-                BJ_LAUNCH(finalize_multi_kernel, 1, 256, G, j + 1, (const double*)PM, stride, z.coef,
+                BJ_LAUNCH(finalize_multi_kernel, j + 1, 256, G, j + 1, (const double*)PM, stride, z.coef,
                           (const int*)z.done);
-                BJ_LAUNCH(multiaxpy_kernel, G, kReduceThreads, n, j + 1, (const double*)z.V, z.w,
-                          (const double*)z.coef, PB, pass == 1 ? 1 : 0, (const int*)z.done);
+                e = launch_kernel(multiaxpy_kernel, dim3(G), dim3(kReduceThreads), axpy_smem, st, pdl, n, j + 1,
+                                  (const double*)z.V, z.w, (const double*)z.coef, PB, pass == 1 ? 1 : 0, (const int*)z.done,
+                                  axpy_piece);
+                if (e != cudaSuccess) { set_cuda_error(e, "multiaxpy_kernel"); return BJ_ERR_CUDA; }
+                h->launches++;
             }
         }
         // beta_{j+2} = ||w||, bookkeeping, and v_{j+2} = w / beta (not needed after the last step)
