@@ -421,6 +421,9 @@ def permutation_section(B, torch, args, local: int, peak: float, peak_src: str) 
     hn = B.bj_setup(rp, ci, val, b)
     r = B.bj_cond_estimate_ex(hn, m, reorth=True)
     out["natural_blocks"] = {"kappa_est": r["kappa"], "res_min": r["res_min"], "res_max": r["res_max"]}
+    if args.long_iters > 0:  # m = 50 is far from converged on this operator: a long fast-mode run beside it
+        rl = B.bj_cond_estimate_ex(hn, args.long_iters, reorth=False)
+        out["natural_blocks"].update({"kappa_est_long": rl["kappa"], "long_iters": rl["iters_done"], "long_res_min": rl["res_min"]})
     rhs = B.bj_seeded_vector(hn, 17)
     pr = B.bj_pcg_solve(hn, rhs, max_iters=3000, rtol=1e-3)
     out["natural_blocks"]["pcg_iters_to_1e-3"] = pr["iters"] if pr["converged"] else None
@@ -435,7 +438,11 @@ def permutation_section(B, torch, args, local: int, peak: float, peak_src: str) 
     ab = var_block_bytes(n, nnz, info, True)
     op = measure_operator(B, torch, hp, 4, n, nnz, b, max(50, args.steps), max(args.warmup, 10), local, peak, peak_src, ab=ab)
     pr = B.bj_pcg_solve(hp, rhs, max_iters=3000, rtol=1e-3)
-    out["line_permutation"] = {"kappa_est": r["kappa"], "res_min": r["res_min"], "res_max": r["res_max"],
+    long_p = {}
+    if args.long_iters > 0:
+        rl = B.bj_cond_estimate_ex(hp, args.long_iters, reorth=False)
+        long_p = {"kappa_est_long": rl["kappa"], "long_iters": rl["iters_done"], "long_res_min": rl["res_min"]}
+    out["line_permutation"] = {**long_p, "kappa_est": r["kappa"], "res_min": r["res_min"], "res_max": r["res_max"],
                                "pcg_iters_to_1e-3": pr["iters"] if pr["converged"] else None, "setup_wall_ms": setup_ms,
                                "us_per_apply": op["us_per_apply"], "alg_bytes": op["alg_bytes"], "gbs": op["gbs"],
                                "frac_of_measured": op["frac_of_measured"], "kernels": op["kernels"],

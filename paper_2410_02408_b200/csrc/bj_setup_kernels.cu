@@ -163,52 +163,32 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
     double d[P];  // packed lower triangle, e = i(i+1)/2 + j
 #pragma unroll
     for (int e = 0; e < P; ++e) d[e] = 0.0;
-    // The B rows of the block are walked TOGETHER, entry k of every row in one round: the loads of a round are independent,
-    // so a thread has B of them in flight instead of one dependent chain of ~5 B loads (latency-bound: 111 us on config 2).
-    int rs[B], re[B];
 #pragma unroll
     for (int i = 0; i < B; ++i) {
         const int64_t row = lo + i;
-        rs[i] = re[i] = 0;
         if (row < n) {
-            rs[i] = rp[row];
-            re[i] = rp[row + 1];
-        } else {
-            d[i * (i + 1) / 2 + i] = 1.0;      // identity rows pad a ragged last block
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < B; ++i) {
-        if (re[i] - rs[i] > 16) {              // long row: binary search for the first column >= lo
-            int s = rs[i], hi = re[i];
-            while (s < hi) {
-                const int mid = (s + hi) >> 1;
-                if (ci[mid] < lo) s = mid + 1; else hi = mid;
+            int s = rp[row];
+            const int e_ = rp[row + 1];
+            if (e_ - s > 16) {                 // long row: binary search for the first column >= lo
+                int hi = e_;
+                while (s < hi) {
+                    const int mid = (s + hi) >> 1;
+                    if (ci[mid] < lo) s = mid + 1; else hi = mid;
+                }
             }
-            rs[i] = s;
-        }
-    }
-    bool any = true;
-    for (int k2 = 0; any; ++k2) {
-        any = false;
-        int c[B];
-#pragma unroll
-        for (int i = 0; i < B; ++i) c[i] = (rs[i] + k2 < re[i]) ? ci[rs[i] + k2] : 0x7fffffff;
-#pragma unroll
-        for (int i = 0; i < B; ++i) {
-            const int64_t row = lo + i;
-            if ((int64_t)c[i] > row) {         // columns ascend: nothing of the lower triangle is left (or the row is exhausted)
-                re[i] = rs[i];                 // retire the row
-            } else {
-                any = true;
-                if (c[i] >= lo) {
-                    const double v = val[rs[i] + k2];
-                    const int j = (int)(c[i] - lo);
+            for (int p = s; p < e_; ++p) {
+                const int64_t c = ci[p];
+                if (c > row) break;            // columns ascend: nothing of the lower triangle is left
+                if (c >= lo) {
+                    const double v = val[p];
+                    const int j = (int)(c - lo);
 #pragma unroll
                     for (int jj = 0; jj < B; ++jj)
                         if (jj <= i && jj == j) d[i * (i + 1) / 2 + jj] = v;
                 }
             }
+        } else {
+            d[i * (i + 1) / 2 + i] = 1.0;      // identity rows pad a ragged last block
         }
     }
     bool bad = false;

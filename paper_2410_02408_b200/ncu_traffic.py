@@ -7,6 +7,7 @@ operator path the script takes dram__bytes_read.sum + dram__bytes_write.sum per 
 captured launches of that kernel kind) -- the `traffic` figure of bench.py's roofline object.
 
     python -m paper_2410_02408_b200.ncu_traffic cfg2_b8=profiles/r2_ncu_raw_cfg2_b8.csv [cfg3_b32=...] > profiles/traffic.txt
+    python -m paper_2410_02408_b200.ncu_traffic --summary cfg2_b8=... [...] > profiles/r2_ncu_full.md     (the table of counters)
 """
 from __future__ import annotations
 
@@ -76,7 +77,72 @@ def read_export(path: str) -> dict:
     return acc
 
 
+SUMMARY_METRICS = [
+    ("gpu__time_duration.sum", "duration (us)", 1e-3), ("dram__bytes_read.sum", "DRAM read (MB)", 1e-6),
+    ("dram__bytes_write.sum", "DRAM write (MB)", 1e-6),
+    ("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "DRAM throughput (% of ncu peak)", 1),
+    ("l1tex__m_xbar2l1tex_read_bytes.sum", "L2 -> L1 bytes (MB)", 1e-6), ("l1tex__t_sector_hit_rate.pct", "L1 sector hit (%)", 1),
+    ("lts__t_sector_hit_rate.pct", "L2 sector hit (%)", 1), ("sm__warps_active.avg.pct_of_peak_sustained_active", "warps active (% of peak)", 1),
+    ("smsp__issue_active.avg.pct_of_peak_sustained_active", "issue active (%)", 1), ("launch__registers_per_thread", "registers / thread", 1),
+    ("launch__grid_size", "grid", 1), ("launch__block_size", "block", 1), ("launch__shared_mem_per_block_dynamic", "dynamic smem / CTA (KB)", 1e-3)]
+SHAPES = {"cfg2": (2097152, 14581760), "cfg3": (1048576, 17825676), "cfg4": (4194304, 37724164), "cfg5": (2654208, 210542904)}
+
+
+def algorithmic(key: str, kind: str) -> int:
+    """Byte count of DESIGN.md section 5 / SURVEY.md 8(d) for a kernel kind of `cfgC_bB`."""
+    cfg, b = key.split("_b")
+    n, nnz = SHAPES[cfg]
+    b = int(b)
+    spmv, solve = 12 * nnz + 4 * (n + 1) + 16 * n, 4 * n * (b + 1) + 16 * n
+    return {"spmv": spmv, "solve_L": solve, "solve_Lt": solve, "apply": solve, "spmv_solve_L": spmv + solve}[kind]
+
+
+def summary(argv):
+    """Markdown table of the counters per kernel kind (means over the captured launches) for each `key=path`."""
+    w = sys.stdout.write
+    w("# ncu `--set full`, the kernels of `bj_op_apply` (rotating inputs)\n\n")
+    w("Commands (per config C, block B; after the plain run of the same command exited 0 in the same call):\n\n```\n")
+    w("ncu --set full --clock-control none --import-source on -k regex:\"spmv_stream|solve_small|solve_group\" -s 40 -c 6 \\\n")
+    w("    -o prof python bench.py --config C --block B --steps 20 --warmup 5 --no-extras\n")
+    w("ncu -i prof.ncu-rep --page raw --csv --print-units base > profiles/r2_ncu_raw_cfgC_bB.csv\n")
+    w("python -m paper_2410_02408_b200.ncu_traffic --summary " + " ".join(argv) + "\n```\n\n")
+    w("Means over the captured launches of each kernel kind; the raw exports are beside this file.  `algorithmic` = the byte count of\n"
+      "DESIGN.md section 5 / SURVEY.md 8(d); `DRAM / algorithmic` < 1: vectors (and, in a chain of applies, the serpentine factor slice)\n"
+      "came from L2; `L2 -> L1 / algorithmic` > 1: sector over-fetch (config 3's 8-byte gathers pull 32-byte sectors).\n\n")
+    for item in argv:
+        key, path = item.split("=", 1)
+        with open(path, newline="") as fh:
+            rows = [r for r in csv.reader(fh) if r]
+        hdr = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+        col = {c: k for k, c in enumerate(rows[hdr])}
+        acc = {}
+        for r in rows[hdr + 2:]:
+            kind = kernel_kind(r[col["Kernel Name"]])
+            if kind is None:
+                continue
+            a = acc.setdefault(kind, {"name": r[col["Kernel Name"]].split("(")[0].replace("void ", "").replace("unnamed>::", ""), "n": 0})
+            a["n"] += 1
+            for m, _, _ in SUMMARY_METRICS:
+                a[m] = a.get(m, 0.0) + float(r[col[m]].replace(",", ""))
+        kinds = [k for k in ("solve_Lt", "spmv", "spmv_solve_L", "solve_L", "apply") if k in acc]
+        mean = lambda k, m: acc[k][m] / acc[k]["n"]  # noqa: E731
+        n, nnz = SHAPES[key.split("_b")[0]]
+        w(f"## {key}  (N = {n}, nnz = {nnz}, b = {key.split('_b')[1]})\n\n")
+        w("| metric | " + " | ".join(f"{k}: `{acc[k]['name']}`" for k in kinds) + " |\n|---|" + "---|" * len(kinds) + "\n")
+        for m, label, sc in SUMMARY_METRICS:
+            w(f"| {label} | " + " | ".join("%.1f" % (mean(k, m) * sc) for k in kinds) + " |\n")
+        w("| algorithmic bytes (MB) | " + " | ".join("%.1f" % (algorithmic(key, k) / 1e6) for k in kinds) + " |\n")
+        w("| DRAM / algorithmic | " + " | ".join(
+            "%.2f" % ((mean(k, "dram__bytes_read.sum") + mean(k, "dram__bytes_write.sum")) / algorithmic(key, k)) for k in kinds) + " |\n")
+        w("| L2 -> L1 / algorithmic | " + " | ".join(
+            "%.2f" % (mean(k, "l1tex__m_xbar2l1tex_read_bytes.sum") / algorithmic(key, k)) for k in kinds) + " |\n")
+        w("| algorithmic GB/s under ncu (cold, serialised) | " + " | ".join(
+            "%.0f" % (algorithmic(key, k) / mean(k, "gpu__time_duration.sum")) for k in kinds) + " |\n\n")
+
+
 def main(argv):
+    if argv and argv[0] == "--summary":
+        return summary(argv[1:])
     out = {"_comment": "dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes), written by "
                        "`python -m paper_2410_02408_b200.ncu_traffic` from the ncu raw exports named in _sources", "_sources": {}}
     for item in argv:
