@@ -435,7 +435,9 @@ def permutation_section(B, torch, args, local: int, peak: float, peak_src: str) 
     setup_ms = 1e3 * (time.perf_counter() - t1)
     r = B.bj_cond_estimate_ex(hp, m, reorth=True)
     info = B.bj_get_info(hp)
-    ab = var_block_bytes(n, nnz, info, True)
+    ab = algorithmic_bytes(n, nnz, b)   # the uniform-block kernels; each solve pass also reads 4 N bytes of perm
+    solve = ab["solve_L"] + 4 * n
+    ab = dict(ab, solve_L=solve, solve_Lt=solve, apply=solve, spmv_solve_L=ab["spmv"] + solve, op_apply=ab["spmv"] + 2 * solve)
     op = measure_operator(B, torch, hp, 4, n, nnz, b, max(50, args.steps), max(args.warmup, 10), local, peak, peak_src, ab=ab)
     pr = B.bj_pcg_solve(hp, rhs, max_iters=3000, rtol=1e-3)
     long_p = {}
@@ -446,7 +448,7 @@ def permutation_section(B, torch, args, local: int, peak: float, peak_src: str) 
                                "pcg_iters_to_1e-3": pr["iters"] if pr["converged"] else None, "setup_wall_ms": setup_ms,
                                "us_per_apply": op["us_per_apply"], "alg_bytes": op["alg_bytes"], "gbs": op["gbs"],
                                "frac_of_measured": op["frac_of_measured"], "kernels": op["kernels"],
-                               "byte_model": "12 nnz + 4 (N + 1) + 16 N + 2 x (factor_bytes + 16 N + 4 N perm)"}
+                               "byte_model": "SURVEY 8(d) count + 4 N bytes of perm per solve pass"}
     B.bj_destroy(hp)
     out["section_seconds"] = time.perf_counter() - t0
     return out
@@ -772,6 +774,26 @@ def main():
             v, reps, cores = time_oracle(A, b, args.cpu_budget_s)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{reps} full operator applies (whole vector, N={n}) in ~{args.cpu_budget_s:.0f} s"}
+            # the other rows of the path on the same cores (SURVEY 8(d) "oracle timing beside it"): setup, bj_apply, one
+            # Lanczos step with full reorthogonalisation (median of 3 each; a few seconds in all)
+            import oracle
+            xs = W.seeded_vector(31, n)
+
+            def med3(fn):
+                ts = []
+                for _ in range(3):
+                    t0 = time.perf_counter()
+                    fn()
+                    ts.append(time.perf_counter() - t0)
+                return float(np.median(ts))
+            P = oracle.Precond(A, b)
+            extras = {"setup_ms": 1e3 * med3(lambda: oracle.Precond(A, b)), "op_apply_ms": 1e3 / v}
+            if b > 0:
+                extras["apply_ms"] = 1e3 * med3(lambda: P.apply(xs))
+            t8 = med3(lambda: P.cond_estimate(8, reorth=True))
+            t4 = med3(lambda: P.cond_estimate(4, reorth=True))
+            extras["lanczos_step_ms_reorth"] = 1e3 * max(t8 - t4, 0.0) / 4.0
+            line["cpu_baseline"]["other_rows"] = extras
 
     B.bj_destroy(h)
     del h, rot, rp, ci, val

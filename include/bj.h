@@ -116,6 +116,7 @@ typedef struct {
     int32_t band_width;       /* >= 0: banded factors in use (opts.band at setup), the lower bandwidth of every
                                  diagonal block; -1: dense packed factors                                   */
     int32_t col16;            /* 1: the tile SpMV streams 16-bit column deltas (opts.col16 at setup)            */
+    int32_t permuted;         /* 1: the blocks are those of P A P^T (bj_setup_perm, bj_setup_blocks_perm)        */
 } bj_info_t;
 
 typedef struct {
@@ -190,10 +191,10 @@ int bj_setup_blocks(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t 
  *     bj_solve_L: y = P^T L^-1 P r,  bj_solve_Lt: x = P^T L^-T P y,  bj_apply: z = M^-1 r,  bj_op_apply: y = (P^T L^-1 P) A (P^T L^-T P) x
  * (orthogonally similar to the split operator of the permuted matrix: same spectrum, so bj_cond_estimate* report its
  * kappa).  No permuted copy of A is made: the extraction looks columns up through the inverse permutation, the block solves
- * gather and scatter through perm, the SpMV runs on A as it is.  Runs on the warp-per-block kernels of bj_setup_blocks
- * (bj_get_info: b = -1, solve_kernel = 4; unfused Lanczos / PCG iterations; the batch entry points are INVALID_ARG).
- * bj_setup_blocks_perm combines a permutation with block sizes 1..BJ_B_MAX given by block_ptr_host (positions in the PERMUTED
- * ordering).  A sequence that is not a permutation is BJ_ERR_INVALID_ARG; other errors as bj_setup.  Synchronises. */
+ * gather and scatter through perm, the SpMV runs on A as it is.  bj_setup_perm runs on the uniform-block kernels of bj_setup
+ * (bj_get_info: permuted = 1; plain solves and SpMV, unfused Lanczos / PCG iterations; the opt-in storage variants and the
+ * batch entry points do not apply).  bj_setup_blocks_perm combines a permutation with block sizes 1..BJ_B_MAX given by
+ * block_ptr_host (positions in the PERMUTED ordering) on the warp-per-block kernels of bj_setup_blocks (b = -1, solve_kernel = 4).  A sequence that is not a permutation is BJ_ERR_INVALID_ARG; other errors as bj_setup.  Synchronises. */
 int bj_setup_perm(const bj_csr_t* csr, int b, const int32_t* perm_dev, void* cuda_stream, bj_handle_t* out);
 int bj_setup_blocks_perm(const bj_csr_t* csr, const int64_t* block_ptr_host, int64_t nblocks, const int32_t* perm_dev,
                          void* cuda_stream, bj_handle_t* out);

@@ -61,7 +61,8 @@ class bj_info_t(C.Structure):
     _fields_ = [("n", C.c_int64), ("nnz", C.c_int64), ("b", C.c_int32), ("nblocks", C.c_int64),
                 ("bad_block", C.c_int64), ("factor_bytes", C.c_int64), ("workspace_bytes", C.c_int64),
                 ("kernel_launches", C.c_int64), ("spmv_kernel", C.c_int32), ("spmv_lanes", C.c_int32),
-                ("solve_kernel", C.c_int32), ("fused_forward", C.c_int32), ("band_width", C.c_int32), ("col16", C.c_int32)]
+                ("solve_kernel", C.c_int32), ("fused_forward", C.c_int32), ("band_width", C.c_int32), ("col16", C.c_int32),
+                ("permuted", C.c_int32)]
 
 
 class BJError(RuntimeError):

@@ -194,7 +194,7 @@ const char* bj_strerror(int code)
 
 }  // extern "C"
 
-static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_handle_t* out)
+static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_handle_t* out, const int32_t* perm_dev = nullptr)
 {
     if (!out) return BJ_ERR_INVALID_ARG;
     *out = nullptr;
@@ -307,7 +307,7 @@ static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_h
     Status stt;
     int rc = BJ_OK;
     // opts.band: the factor layout depends on the band statistic, so the extraction follows the validation pass
-    const bool want_band = o.band != 0 && ((h->solve_kind == 1 && b >= 4) || (h->solve_kind == 2 && h->nblocks >= 64));
+    const bool want_band = o.band != 0 && !perm_dev && ((h->solve_kind == 1 && b >= 4) || (h->solve_kind == 2 && h->nblocks >= 64));
 
     // a1 validate (also longest row and the column-coherence statistic)
     rc = launch_validate(h);
@@ -319,6 +319,10 @@ static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_h
 
     h->coherence = stt.compared ? (double)stt.coherent / (double)stt.compared : 1.0;
     h->max_row_nnz = stt.max_row_nnz;
+    if (perm_dev) {  // bj_setup_perm: blocks of P A P^T, vectors in the original ordering (reading 23)
+        rc = perm_install(h, perm_dev);
+        if (rc != BJ_OK) return fail(rc);
+    }
 
     // NEXT-2, opt-in: banded diagonal blocks keep banded factors -- (w+1) b doubles per block instead of b(b+1)/2.
     if (want_band) {
@@ -434,11 +438,10 @@ int bj_setup_perm(const bj_csr_t* csr, int b, const int32_t* perm_dev, void* cud
     if (!out) return BJ_ERR_INVALID_ARG;
     *out = nullptr;
     if (!csr || csr->n <= 0 || b < 1 || b > BJ_B_MAX || !perm_dev) return BJ_ERR_INVALID_ARG;
-    const int64_t nblocks = (csr->n + b - 1) / b;
-    std::vector<int64_t> ptr((size_t)nblocks + 1);
-    for (int64_t k = 0; k < nblocks; ++k) ptr[k] = k * b;
-    ptr[nblocks] = csr->n;  // ragged last block
-    return bj_setup_blocks_perm(csr, ptr.data(), nblocks, perm_dev, cuda_stream, out);
+    bj_setup_opts_t o;
+    memset(&o, 0, sizeof(o));
+    o.cuda_stream = cuda_stream;
+    return setup_impl(csr, b, o, out, perm_dev);  // the uniform-block kernels, vectors gathered / scattered through perm
 }
 
 int bj_release_cached_memory(void)
@@ -510,6 +513,7 @@ int bj_get_info(bj_handle_t h, bj_info_t* info)
     info->solve_kernel = h->solve_kind == 4 ? 4 : h->solve_kind;
     info->band_width = (h->solve_kind == 3 || h->tri) ? h->band : -1;
     info->col16 = h->col16 ? 1 : 0;
+    info->permuted = h->var_perm ? 1 : 0;
     info->fused_forward = (h->spmv_kernel == 1 && h->fuse_ok && h->opt_fuse != 0 && h->solve_kind != 0) ? 1 : 0;
     return BJ_OK;
 }

@@ -303,7 +303,7 @@ static int batch_layout(bj_handle_s* h, int64_t nsys, const int64_t* offsets_hos
 {
     *off_dev = nullptr;
     *seg = 0;
-    if (h->solve_kind == 4) return BJ_ERR_INVALID_ARG;  // variable-size blocks: alignment with the systems is not checked here
+    if (h->solve_kind == 4 || h->var_perm) return BJ_ERR_INVALID_ARG;  // variable-size / permuted blocks: alignment with the systems is not checked here
     if (!offsets_host) {
         if (h->n % nsys) return BJ_ERR_INVALID_ARG;
         *seg = h->n / nsys;

@@ -108,7 +108,7 @@ struct bj_handle_s {
     int64_t* var_foff = nullptr;
     double* var_fac = nullptr;
     int var_smax = 0;
-    int32_t* var_perm = nullptr;  // kind 4 with a permutation: perm and its inverse (handle-owned copies, n ints each)
+    int32_t* var_perm = nullptr;  // permuted handle (bj_setup_perm, bj_setup_blocks_perm): perm and its inverse (handle-owned, n ints each)
     int32_t* var_pinv = nullptr;
     int band = -1;       // kind 3: lower bandwidth w of every diagonal block (0..2)
     double* fac_band = nullptr;  // kind 3: aliases the dense factor storage of the slab
@@ -277,6 +277,8 @@ int mlanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t
 // variable-size blocks (bj_var_kernels.cu)
 int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks, const int32_t* perm_dev);  // perm_dev: device, or null
 void var_free(bj_handle_s* h);
+int perm_install(bj_handle_s* h, const int32_t* perm_dev);  // handle-owned copies of perm and its inverse; validates
+void perm_free(bj_handle_s* h);
 int launch_solve_var(bj_handle_s* h, int dir, const double* in, double* out);
 int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* r);
 void pcg_free(bj_handle_s* h);

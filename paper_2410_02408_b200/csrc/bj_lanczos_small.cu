@@ -280,7 +280,7 @@ size_t small_smem_bytes(const bj_handle_s* h, int m, bool mat)
 bool lanczos_small_usable(const bj_handle_s* h, int m)
 {
     if (env_int("BJ_LANCZOS_SMALL", 1) == 0) return false;
-    if (!(h->solve_kind == 0 || (h->solve_kind == 1 && !h->tri)) || m > 1024 || h->n > 16384 || h->nnz == 0) return false;
+    if (h->var_perm || !(h->solve_kind == 0 || (h->solve_kind == 1 && !h->tri)) || m > 1024 || h->n > 16384 || h->nnz == 0) return false;
     return small_smem_bytes(h, m, false) <= 200 * 1024;
 }
 

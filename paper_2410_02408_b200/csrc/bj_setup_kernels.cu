@@ -154,7 +154,8 @@ template <int B>
 __global__ void __launch_bounds__(128)
 extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restrict__ rp,
                             const int32_t* __restrict__ ci, const double* __restrict__ val,
-                            double* __restrict__ fac, Status* st, int tri)
+                            double* __restrict__ fac, Status* st, int tri,
+                            const int32_t* __restrict__ perm, const int32_t* __restrict__ pinv)  // both null: no permutation
 {
     constexpr int P = B * (B + 1) / 2;
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -163,6 +164,29 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
     double d[P];  // packed lower triangle, e = i(i+1)/2 + j
 #pragma unroll
     for (int e = 0; e < P; ++e) d[e] = 0.0;
+    if (perm) {
+        // permuted handle (reading 23): row lo + i of P A P^T is row perm[lo + i] of A, a column c sits at permuted
+        // position pinv[c]; positions are not sorted along the row, so the whole row is scanned
+#pragma unroll
+        for (int i = 0; i < B; ++i) {
+            if (lo + i < n) {
+                const int row = perm[lo + i];
+                const int e_ = rp[row + 1];
+                for (int p = rp[row]; p < e_; ++p) {
+                    const int64_t cp = pinv[ci[p]];
+                    if (cp >= lo && cp <= lo + i) {
+                        const double v = val[p];
+                        const int j = (int)(cp - lo);
+#pragma unroll
+                        for (int jj = 0; jj < B; ++jj)
+                            if (jj <= i && jj == j) d[i * (i + 1) / 2 + jj] = v;
+                    }
+                }
+            } else {
+                d[i * (i + 1) / 2 + i] = 1.0;
+            }
+        }
+    } else {
 #pragma unroll
     for (int i = 0; i < B; ++i) {
         const int64_t row = lo + i;
@@ -190,6 +214,7 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
         } else {
             d[i * (i + 1) / 2 + i] = 1.0;      // identity rows pad a ragged last block
         }
+    }
     }
     bool bad = false;
     // every loop has the constant trip count B (triangular bounds as predicates): all of them unroll, d[] stays in registers
@@ -252,7 +277,8 @@ template <int W>
 __global__ void __launch_bounds__(128)
 extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restrict__ rp,
                               const int32_t* __restrict__ ci, const double* __restrict__ val,
-                              double* __restrict__ out0, double* __restrict__ out1, Status* st)
+                              double* __restrict__ out0, double* __restrict__ out1, Status* st,
+                              const int32_t* __restrict__ perm, const int32_t* __restrict__ pinv)  // both null: no permutation
 {
     extern __shared__ double smem[];
     constexpr int LD = W + 1;
@@ -270,7 +296,15 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
 #pragma unroll
     for (int c = 0; c < W; ++c) D[i * LD + c] = 0.0;
     if (!rowlive) D[i * LD + i] = 1.0;  // identity rows pad ragged blocks and idle lanes
-    if (rowlive) {
+    if (rowlive && perm) {
+        // permuted handle: row lo + i of P A P^T is row perm[lo + i] of A; the whole row is scanned, columns through pinv
+        const int ro = perm[row];
+        const int e = rp[ro + 1];
+        for (int p = rp[ro]; p < e; ++p) {
+            const int64_t cp = pinv[ci[p]];
+            if (cp >= lo && cp <= row) D[i * LD + (int)(cp - lo)] = val[p];
+        }
+    } else if (rowlive) {
         int s = rp[row];
         const int e = rp[row + 1];
         int hi = e;
@@ -403,7 +437,7 @@ int launch_extract_factor(bj_handle_s* h)
     case B:                                                                                                 \
         extract_factor_small_kernel<B><<<tb, 128, 0, h->stream>>>(h->n, h->nblocks, h->row_ptr, h->col_idx,  \
                                                                   h->val, h->fac_small, h->status,          \
-                                                                  h->tri ? 1 : 0);                          \
+                                                                  h->tri ? 1 : 0, h->var_perm, h->var_pinv); \
         break;
         switch (b) {
             BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
@@ -417,10 +451,12 @@ int launch_extract_factor(bj_handle_s* h)
         const unsigned sb = (unsigned)((h->nblocks + nsub - 1) / nsub);
         if (W == 16)
             extract_factor_subwarp_kernel<16><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
-                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status);
+                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status,
+                                                                          h->var_perm, h->var_pinv);
         else
             extract_factor_subwarp_kernel<32><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
-                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status);
+                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status,
+                                                                          h->var_perm, h->var_pinv);
     }
     h->launches++;
     BJ_CUDA(cudaGetLastError());

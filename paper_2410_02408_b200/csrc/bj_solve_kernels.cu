@@ -65,6 +65,26 @@ __device__ __forceinline__ void store_rows(double* dst, int64_t lo, int64_t n, b
     }
 }
 
+// Permuted handles (bj_setup_perm, reading 23): the block's rows lo .. lo + B - 1 of the PERMUTED ordering live at
+// perm[lo + i] in the caller's vectors; the index loads are coalesced, the vector accesses are gathers / scatters.
+template <int B>
+__device__ __forceinline__ void load_rows_perm(const double* src, const int32_t* __restrict__ perm, int64_t lo, int64_t n, double (&v)[B])
+{
+    int idx[B];
+#pragma unroll
+    for (int i = 0; i < B; ++i) idx[i] = (lo + i < n) ? perm[lo + i] : -1;
+#pragma unroll
+    for (int i = 0; i < B; ++i) v[i] = idx[i] >= 0 ? src[idx[i]] : 0.0;
+}
+
+template <int B>
+__device__ __forceinline__ void store_rows_perm(double* dst, const int32_t* __restrict__ perm, int64_t lo, int64_t n, const double (&v)[B])
+{
+#pragma unroll
+    for (int i = 0; i < B; ++i)
+        if (lo + i < n) dst[perm[lo + i]] = v[i];
+}
+
 // LZ: 0 plain, 1 Lanczos prologue (DIR 1: the input is w built on the fly), 2 Lanczos epilogue (DIR 0),
 //     3 PCG update + apply (DIR 2: x += a p, r -= a q on the fly, z = M^-1 r, partials of r.r and r.z)
 //     TRI: tridiagonal blocks, compact bidiagonal factor of 2B - 1 elements, element (i, j) at slot i + j
@@ -78,7 +98,8 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
                    const double* in, double* out,  // in == out allowed: a thread touches only its own block
                    const LzPrologue pro, const LzEpilogue epi, const PcgHook pcg,
                    const int serp,                 // 1: serpentine walk (launch_small): CTA q takes the q-th LAST slice of blocks
-                   const unsigned serp_keep_from)  //    and CTAs q >= serp_keep_from load their factors as ordinary L2 lines instead of evict_first
+                   const unsigned serp_keep_from,  //    and CTAs q >= serp_keep_from load their factors as ordinary L2 lines instead of evict_first
+                   const int32_t* __restrict__ perm)  // plain solves only (LZ == 0): vectors are accessed through perm, or null
 {
     constexpr int P = TRI ? 2 * B - 1 : B * (B + 1) / 2;
     __shared__ double lz_sh[8];
@@ -160,7 +181,8 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
             store_rows<B, VEC>(pcg.x, lo, n, whole, xs);
         }
     } else {
-        load_rows<B, VEC>(in, lo, n, whole, v);                         // before the scalars: independent of them
+        if (LZ == 0 && perm) load_rows_perm<B>(in, perm, lo, n, v);
+        else load_rows<B, VEC>(in, lo, n, whole, v);                    // before the scalars: independent of them
         if (LZ == 2 && lz_epilogue_begin(epi, beta, inv_beta)) return;  // uniform over the grid
     }
     if (DIR == 0 || DIR == 2) {
@@ -208,7 +230,10 @@ solve_small_kernel(int64_t n, int64_t nblocks, const double* __restrict__ fac,
         }
         lz_reduce_finish(epi.red, acc, lz_sh);
     } else {
-        if (act) store_rows<B, VEC>(out, lo, n, whole, v);
+        if (act) {
+            if (LZ == 0 && perm) store_rows_perm<B>(out, perm, lo, n, v);
+            else store_rows<B, VEC>(out, lo, n, whole, v);
+        }
         if (LZ == 1) lz_reduce_finish(pro.red, acc, lz_sh);
         if (LZ == 3) {
             if (act) {
@@ -243,6 +268,7 @@ struct SolveStreamParams {
     int b, P, G, stages;
     int copy_doubles;    // doubles reserved per copy per stage (G * P rounded to even)
     int early_trigger;   // programmatic dependent launch: release the next kernel at entry (else at exit)
+    const int32_t* perm; // permuted handle: vectors are accessed through perm, or null
 };
 
 template <int W, int DIR>
@@ -298,7 +324,7 @@ solve_stream_kernel(const SolveStreamParams p)
             for (int q = 0; q < kMaxBlocksPerSub; ++q) {
                 const int64_t kb = k0 + sub + q * nsub;
                 const int64_t row = kb * b + i;
-                dst[q] = (tile < p.ntiles && q * nsub < p.G && kb < p.nblocks && i < b && row < p.n) ? p.in[row] : 0.0;
+                dst[q] = (tile < p.ntiles && q * nsub < p.G && kb < p.nblocks && i < b && row < p.n) ? p.in[p.perm ? p.perm[row] : row] : 0.0;
             }
         };
         double rn[kMaxBlocksPerSub];
@@ -326,7 +352,7 @@ solve_stream_kernel(const SolveStreamParams p)
                     if (DIR == 1) v = subwarp_block_solve<W, 1>(fq, b, i, v);
                     if (DIR == 2) v = subwarp_block_solve<W, 1>(fq + p.copy_doubles, b, i, v);
                     const int64_t row = (k0 + kb) * b + i;
-                    if (kb < nb && i < b && row < p.n) p.out[row] = v;
+                    if (kb < nb && i < b && row < p.n) p.out[p.perm ? p.perm[row] : row] = v;
                 }
             }
             __syncwarp();
@@ -358,6 +384,7 @@ struct GroupParams {
     LzPrologue pro;
     LzEpilogue epi;
     PcgHook pcg;
+    const int32_t* perm;  // plain solves of a permuted handle: vectors are accessed through perm, or null
 };
 
 __device__ __forceinline__ void fence_proxy_async()
@@ -449,7 +476,7 @@ solve_group_kernel(const GroupParams p)
             } else if (DIR == 2 && LZ == 3) {
                 if (live) { a[k] = p.pcg.r[row]; c[k] = p.pcg.q[row]; ew[k] = p.pcg.x[row]; ev[k] = mlz ? 0.0 : p.pcg.p[row]; }
             } else {
-                if (live) a[k] = p.in[row];
+                if (live) a[k] = p.in[(LZ == 0 && p.perm) ? p.perm[row] : row];
                 if (DIR == 0 && LZ == 2) {  // the epilogue's own operands ride along one tile ahead
                     ew[k] = live ? p.epi.w[row] : 0.0;
                     ev[k] = (live && p.epi.vprev) ? p.epi.vprev[row] : 0.0;
@@ -524,7 +551,7 @@ solve_group_kernel(const GroupParams p)
                     acc = fma(vn, wi, acc);
                 } else {
                     if (DIR == 2 && LZ == 3) acc2 = fma(ew[k], y, acc2);  // r_new . z
-                    p.out[row] = y;
+                    p.out[(LZ == 0 && p.perm) ? p.perm[row] : row] = y;
                 }
             }
         }
@@ -570,7 +597,7 @@ static int launch_small(bj_handle_s* h, const double* in, double* out, const LzP
     const unsigned serp_keep_from = (unsigned)(blocks - keep_ctas);
 #define BJ_LAUNCH_SMALL(B, V, T)                                                                                  \
     launch_kernel(solve_small_kernel<B, DIR, V, LZ, T>, blocks, threads, 0, h->stream, pdl, h->n, h->nblocks,     \
-                  (const double*)h->fac_small, in, out, pr, ep, pc, serp, serp_keep_from)
+                  (const double*)h->fac_small, in, out, pr, ep, pc, serp, serp_keep_from, (const int32_t*)(LZ == 0 ? h->var_perm : nullptr))
 #define BJ_CASE(B)                                                                         \
     case B:                                                                                \
         e = vec ? BJ_LAUNCH_SMALL(B, true, false) : BJ_LAUNCH_SMALL(B, false, false);      \
@@ -629,6 +656,7 @@ static int launch_warp(bj_handle_s* h, const double* in, double* out)
     sp.fac0 = DIR == 1 ? h->fac_bwd : h->fac_fwd;
     sp.fac1 = h->fac_bwd;
     sp.in = in; sp.out = out;
+    sp.perm = h->var_perm;
     sp.early_trigger = h->tune.pdl_early & 1;
     const size_t stage_bytes = (size_t)copies * sp.copy_doubles * 8;
     int stages = std::max(2, h->tune.solve_stages);
@@ -680,6 +708,7 @@ static int launch_group_t(bj_handle_s* h, const double* in, double* out, const L
         gp.keep_from = gp.ntiles - keep_tiles;
     }
     gp.lz = (DIR == 1 && pro) ? 1 : (DIR == 0 && epi) ? 2 : (DIR == 2 && pcg) ? 3 : 0;
+    gp.perm = h->var_perm;
     gp.pcg = pcg ? *pcg : PcgHook{};
     gp.pro = pro ? *pro : LzPrologue{};
     gp.epi = epi ? *epi : LzEpilogue{};
@@ -719,6 +748,7 @@ static bool use_group_kernel(const bj_handle_s* h)
 // kind 1 always carries the hooks; kind 2 only in the group kernel (b = 16, 24, 32); b = 0 has no solve to ride on
 bool lanczos_fusable(const bj_handle_s* h)
 {
+    if (h->var_perm) return false;  // the hooks address the vectors by block row: permuted handles run the unfused iterations
     return h->solve_kind == 1 || h->solve_kind == 3 || (h->solve_kind == 2 && use_group_kernel(h));
 }
 

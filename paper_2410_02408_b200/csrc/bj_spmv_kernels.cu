@@ -423,7 +423,7 @@ StreamGeometry spmv_stream_geometry(const bj_handle_s* h, bool random_cols)
     int R = (int)((double)target_nnz / (mean > 1.0 ? mean : 1.0));
     R = std::max(32, std::min(R, 1024));
     bool fuse = false;
-    if (h->solve_kind == 1 && !random_cols) {
+    if (h->solve_kind == 1 && !random_cols && !h->var_perm) {  // (a permuted handle's blocks are not row ranges of A)
         const int unit = kInterleave * h->b;  // fused tiles must hold whole interleave groups
         int Rf = ((R + unit / 2) / unit) * unit;
         if (Rf < unit) Rf = unit;

@@ -137,13 +137,18 @@ perm_invert_kernel(int64_t n, const int32_t* __restrict__ perm, int32_t* __restr
 
 }  // namespace
 
-void var_free(bj_handle_s* h)
+void perm_free(bj_handle_s* h)
 {
-    if (h->var_fac) h->factor_bytes = 0;
     cudaFree(h->var_perm);
     cudaFree(h->var_pinv);
     h->var_perm = nullptr;
     h->var_pinv = nullptr;
+}
+
+void var_free(bj_handle_s* h)
+{
+    if (h->var_fac) h->factor_bytes = 0;
+    perm_free(h);
     cudaFree(h->var_bptr);
     cudaFree(h->var_foff);
     cudaFree(h->var_fac);
@@ -154,29 +159,37 @@ void var_free(bj_handle_s* h)
 
 // Turns a b = 0 handle (validated matrix, SpMV plan) into a variable-block handle: uploads the block layout, extracts
 // and factors every block.  ptr_host was validated by the caller.
+// The handle's own copy of a permutation and of its inverse (bj_setup_perm, bj_setup_blocks_perm).  A sequence that is not
+// a permutation of 0..n-1 is BJ_ERR_INVALID_ARG.  Synchronises.
+int perm_install(bj_handle_s* h, const int32_t* perm_dev)
+{
+    cudaStream_t st = h->stream;
+    const size_t pb = sizeof(int32_t) * (size_t)h->n;
+    if (cudaMalloc((void**)&h->var_perm, pb) != cudaSuccess || cudaMalloc((void**)&h->var_pinv, pb) != cudaSuccess) {
+        cudaGetLastError();
+        perm_free(h);
+        return BJ_ERR_ALLOC;
+    }
+    int* flag = &h->status->pad;
+    BJ_CUDA(cudaMemcpyAsync(h->var_perm, perm_dev, pb, cudaMemcpyDeviceToDevice, st));
+    BJ_CUDA(cudaMemsetAsync(h->var_pinv, 0xff, pb, st));
+    BJ_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
+    perm_invert_kernel<<<(unsigned)((h->n + 255) / 256), 256, 0, st>>>(h->n, h->var_perm, h->var_pinv, flag);
+    h->launches++;
+    int bad = 1;
+    BJ_CUDA(cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaStreamSynchronize(st));
+    if (bad) { perm_free(h); return BJ_ERR_INVALID_ARG; }
+    h->workspace_bytes += 2 * (int64_t)pb;
+    return BJ_OK;
+}
+
 int var_setup(bj_handle_s* h, const int64_t* ptr_host, int64_t nblocks, const int32_t* perm_dev)
 {
     cudaStream_t st = h->stream;
     if (perm_dev) {
-        // the handle keeps its own copy of the permutation and of its inverse; a sequence that is not a permutation of
-        // 0..n-1 is an invalid argument
-        const size_t pb = sizeof(int32_t) * (size_t)h->n;
-        if (cudaMalloc((void**)&h->var_perm, pb) != cudaSuccess || cudaMalloc((void**)&h->var_pinv, pb) != cudaSuccess) {
-            cudaGetLastError();
-            var_free(h);
-            return BJ_ERR_ALLOC;
-        }
-        int* flag = &h->status->pad;
-        BJ_CUDA(cudaMemcpyAsync(h->var_perm, perm_dev, pb, cudaMemcpyDeviceToDevice, st));
-        BJ_CUDA(cudaMemsetAsync(h->var_pinv, 0xff, pb, st));
-        BJ_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
-        perm_invert_kernel<<<(unsigned)((h->n + 255) / 256), 256, 0, st>>>(h->n, h->var_perm, h->var_pinv, flag);
-        h->launches++;
-        int bad = 1;
-        BJ_CUDA(cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
-        BJ_CUDA(cudaStreamSynchronize(st));
-        if (bad) { var_free(h); return BJ_ERR_INVALID_ARG; }
-        h->workspace_bytes += 2 * (int64_t)pb;
+        const int prc = perm_install(h, perm_dev);
+        if (prc != BJ_OK) return prc;
     }
     std::vector<int32_t> bp((size_t)nblocks + 1);
     std::vector<int64_t> fo((size_t)nblocks + 1);

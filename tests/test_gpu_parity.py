@@ -1090,11 +1090,12 @@ def test_permuted_blocks_match_oracle(B, torch_, rel, cfg):
     ORIGINAL ordering, element by element against oracle.PrecondPerm (explicit P A P^T); kappa with full
     reorthogonalisation to the bar of the north star; in-place calls; ragged last block."""
     A = mat(cfg, "small" if cfg != 5 else "tiny")
-    for b in sorted(set(W.BLOCK_SIZES[cfg] + [7])):
+    for b in sorted(set(W.BLOCK_SIZES[cfg] + [7, 12])):   # thread-per-block, group, and stream solve kernels
         perm = W.random_permutation(A.n, seed=60 + cfg + b)
         h, keep = _setup_perm(B, torch_, A, b, perm)
         info = B.bj_get_info(h)
-        assert info["solve_kernel"] == 4 and info["nblocks"] == (A.n + b - 1) // b
+        assert info["permuted"] == 1 and info["b"] == b and info["nblocks"] == (A.n + b - 1) // b
+        assert info["solve_kernel"] in (1, 2) and info["fused_forward"] == 0          # the uniform-block kernels
         P = oracle.PrecondPerm(A, perm, b)
         for seed in (7, 8):
             x = W.seeded_vector(seed, A.n)
