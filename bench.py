@@ -454,6 +454,25 @@ def permutation_section(B, torch, args, local: int, peak: float, peak_src: str) 
     return out
 
 
+def variable_blocks_section(B, torch, args, A, rp, ci, val, local: int, peak: float, peak_src: str) -> dict:
+    """variable-size blocks (bj_setup_blocks) on the headline matrix with seeded sizes 1..32: the
+    warp-per-block kernels against their own byte model (packed factors + block pointers + factor offsets per pass)."""
+    ptr = W.random_block_ptr(A.n, seed=41, smin=1, smax=32)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    h = B.bj_setup_blocks(rp, ci, val, ptr)
+    torch.cuda.synchronize()
+    setup_ms = 1e3 * (time.perf_counter() - t0)
+    info = B.bj_get_info(h)
+    ab = var_block_bytes(A.n, A.nnz, info, False)
+    op = measure_operator(B, torch, h, 2, A.n, A.nnz, -1, max(50, args.steps), max(args.warmup, 10), local, peak, peak_src, ab=ab)
+    B.bj_destroy(h)
+    return {"nblocks": info["nblocks"], "mean_block": A.n / info["nblocks"], "factor_bytes": info["factor_bytes"],
+            "setup_wall_ms": setup_ms, "us_per_apply": op["us_per_apply"], "alg_bytes": op["alg_bytes"], "gbs": op["gbs"],
+            "frac_of_measured": op["frac_of_measured"], "kernels": op["kernels"],
+            "byte_model": "12 nnz + 4 (N + 1) + 16 N + 2 x (factor_bytes + 16 N), factor_bytes = packed factors + block pointers + offsets"}
+
+
 def other_configs(B, torch, args, local: int, peak: float, peak_src: str) -> dict:
     """The operator apply on the other BASELINE.json configs (1, 3, 4, 5 with b = 3 and 24) in the same run, so that every
     rate quoted in profiles/ and DESIGN.md has a driver-run counterpart."""
@@ -769,6 +788,9 @@ def main():
                                                       "factors and 16-bit column deltas; fewer bytes than the counts of SURVEY 8(d), "
                                                       "own accounting"}
                 B.bj_destroy(hb)
+
+            # ---- NEXT-3: variable-size blocks on the same matrix (warp-per-block kernels, own byte model) ------------
+            line["variable_blocks"] = variable_blocks_section(B, torch, args, A, rp, ci, val, local, peak, peak_src)
 
             # ---- CPU oracle on the host cores (reported baseline, not the target) -------------------------
             v, reps, cores = time_oracle(A, b, args.cpu_budget_s)
