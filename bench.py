@@ -79,8 +79,7 @@ def workload_config(A, cfg: int, b: int, world: int) -> dict:
     """The `config` object: identical keys and values in both arms (ours and --impl reference)."""
     ab = algorithmic_bytes(A.n, A.nnz, b)
     return {"workload": A.meta.get("name"), "baseline_config": cfg, "n": A.n, "nnz": A.nnz, "block": b,
-            "l2": "working set %.0f MB per apply vs %.0f MB of L2; the timed loop rotates over %d distinct x / y pairs"
-                  % (ab["op_apply"] / 1e6, L2_MB, PAIRS),
+            "l2": "working set %.0f MB per apply vs %.0f MB of L2" % (ab["op_apply"] / 1e6, L2_MB),
             "parallelism": "replicas" if world > 1 else "single"}
 
 
