@@ -593,6 +593,20 @@ def main():
     val = torch.from_numpy(A.val).cuda()
 
     # ---- setup (a1-a4): wall clock including allocation, kernel-only device time, roofline ---------------
+    if b < 0:
+        # --block -1 (profiling aid): seeded variable-size blocks 1..32 on the warp-per-block kernels, their own byte model
+        h = B.bj_setup_blocks(rp, ci, val, W.random_block_ptr(n, seed=41, smin=1, smax=32))
+        info = B.bj_get_info(h)
+        op = measure_operator(B, torch, h, args.config, n, nnz, -1, args.steps, args.warmup, local, peak, peak_src,
+                              ab=var_block_bytes(n, nnz, info, False))
+        B.bj_destroy(h)
+        print(json.dumps({"metric": METRIC, "value": op["applies_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": 1e-3 * op["us_per_apply"], "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": dict(workload_config(A, args.config, 0, world), block="variable 1..32 (seed 41)"),
+                          "variable_blocks": {k: v for k, v in op.items() if k != "roofline"}, "roofline": op["roofline"],
+                          "gpu_launches": op["gpu_launches"], "clocks": op["clocks"]}))
+        return
     h, setup = measure_setup(B, torch, rp, ci, val, b, peak, **opts)
     if args.spmv_kernel >= 0:
         B.bj_set_option(h, B.BJ_OPT_SPMV_KERNEL, args.spmv_kernel)

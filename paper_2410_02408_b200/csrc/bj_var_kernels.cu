@@ -85,6 +85,39 @@ extract_factor_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, con
     }
 }
 
+// The substitutions of one block by one warp (lane = row, all 32 lanes call): F = packed factor in shared memory.
+// The loops keep the packed index of this lane's entry as a running value (one add per step) and the lane's own
+// reciprocal diagonal in a register.
+template <int DIR>
+__device__ __forceinline__ double var_block_solve(const double* F, int s, int lane, double v)
+{
+    const bool act = lane < s;
+    const int csl = var_col_start(act ? lane : 0, s);
+    const double dinv = F[csl];
+    if (DIR == 0 || DIR == 2) {
+        int idx = lane, stride = s - 1;                  // l_{lane,j} at cs(j) + lane - j; cs(j + 1) - cs(j) = s - j
+#pragma unroll 4
+        for (int j = 0; j < s; ++j) {
+            if (lane == j) v *= dinv;
+            const double yj = __shfl_sync(0xffffffffu, v, j);
+            if (act && lane > j) v -= F[idx] * yj;
+            idx += stride;
+            --stride;
+        }
+    }
+    if (DIR == 1 || DIR == 2) {
+        int idb = csl + (s - 1 - lane);                  // l_{j,lane} at cs(lane) + j - lane, j = s - 1 first
+#pragma unroll 4
+        for (int j = s - 1; j >= 0; --j) {
+            if (lane == j) v *= dinv;
+            const double xj = __shfl_sync(0xffffffffu, v, j);
+            if (lane < j) v -= F[idb] * xj;
+            --idb;
+        }
+    }
+    return v;
+}
+
 // DIR 0: y = L^-1 r, 1: x = L^-T y, 2: z = L^-T L^-1 r.  One warp per block, lane = row, factor in shared memory.
 template <int DIR>
 __global__ void __launch_bounds__(kVarWarps * 32)
@@ -106,21 +139,7 @@ solve_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, const int64_
     const int row = lane < s ? (perm ? perm[lo + lane] : lo + lane) : 0;
     double v = lane < s ? in[row] : 0.0;
     __syncwarp();
-    if (DIR == 0 || DIR == 2) {
-        for (int j = 0; j < s; ++j) {
-            const int cs = var_col_start(j, s);
-            if (lane == j) v *= F[cs];
-            const double yj = __shfl_sync(0xffffffffu, v, j);
-            if (lane > j && lane < s) v -= F[cs + (lane - j)] * yj;
-        }
-    }
-    if (DIR == 1 || DIR == 2) {
-        for (int j = s - 1; j >= 0; --j) {
-            if (lane == j) v *= F[var_col_start(j, s)];
-            const double xj = __shfl_sync(0xffffffffu, v, j);
-            if (lane < j) v -= F[var_col_start(lane, s) + (j - lane)] * xj;  // l_{j,lane}
-        }
-    }
+    v = var_block_solve<DIR>(F, s, lane, v);
     if (lane < s) out[row] = v;
 }
 
