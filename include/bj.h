@@ -146,7 +146,9 @@ enum {
     BJ_OPT_LANCZOS_FUSE = 3,  /* 0: fast-mode Lanczos runs the unfused vector kernels; 1 / -1: the fused step (default) */
     BJ_OPT_PCG_FUSE = 4,      /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
     BJ_OPT_LANCZOS_SINGLE_LAUNCH = 5 /* 0: launch-bound sizes (vectors + factors fit one CTA's shared memory, b <= 8) keep the
-                                 multi-launch Lanczos; 1 / -1: the whole run is one single-CTA kernel (default)          */
+                                 multi-launch Lanczos; 1 / -1 (default): the whole run is ONE kernel -- of one eight-CTA
+                                 cluster with the basis distributed over their shared memory when a CTA's share fits,
+                                 else of one CTA; 2: always the single-CTA form                                         */
 };
 
 /* a1-a4. Validate the CSR, extract the diagonal b x b blocks, factor each

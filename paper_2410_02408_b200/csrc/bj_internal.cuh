@@ -266,6 +266,9 @@ int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
 // k-th smallest eigenvalue (k = 0 .. m-1) of the symmetric tridiagonal (diag a[0..m-1], off-diagonal e[0..m-2]), bisection
 double tridiag_eig_k(int m, const double* a, const double* e, int k);
 void lanczos_fill_result(int me, const double* a, const double* b, bj_lanczos_result_t* res);
+// the whole run as one kernel of one eight-CTA cluster, the basis distributed over their shared memory (bj_lanczos_cluster.cu)
+bool lanczos_cluster_usable(const bj_handle_s* h, int m, bool reorth);
+int launch_lanczos_cluster(bj_handle_s* h, int m, bool reorth, double tol, const double* v0, double* alpha, double* beta, int* done);
 // the whole run as one single-CTA kernel for launch-bound sizes (bj_lanczos_small.cu)
 bool lanczos_small_usable(const bj_handle_s* h, int m);
 int launch_lanczos_small(bj_handle_s* h, int m, bool reorth, double tol, const double* v0, double* V, double* alpha, double* beta,

@@ -1,0 +1,430 @@
+// Launch-bound sizes, second form: the whole m-step Lanczos run of bj_lanczos.cu as ONE kernel of ONE thread-block CLUSTER
+// of eight CTAs (bj_lanczos_small.cu runs it on one CTA: its reorthogonalisation re-reads the basis four times per step and
+// only ~20 basis vectors of N = 1024 fit beside the work vectors, the rest comes through one SM's L2 port: 17 us per step).
+// Here CTA r owns a contiguous range of diagonal blocks and their rows; its slice of EVERY basis vector stays in its
+// shared memory (8 x 200 KB for the basis), the operator's block solves and all vector updates are local, and the CTAs
+// exchange through distributed shared memory only
+//   * the slice of t = L^-T v_j (the SpMV reads arbitrary columns: every CTA keeps the full vector),
+//   * the partial sums of alpha_j, of the reorthogonalisation coefficients (two passes) and of beta_{j+1}:
+// each CTA pushes its partials into slot r of every CTA's exchange buffer, every CTA adds the eight slots in the same
+// order, so all CTAs hold bit-identical scalars and take the same branches.
+// Same recurrence, statement by statement, as lanczos_run (readings 10-13); the operator is the
+// arithmetic of solve_small_kernel (thread per block, interleaved packed factors) and of a row-per-thread CSR product
+// summed left to right.  Block sizes b <= 8 and b = 0.
+#include <cooperative_groups.h>
+#include <math.h>
+
+#include <algorithm>
+#include <atomic>
+
+#include "bj_device.cuh"
+#include "bj_internal.cuh"
+
+namespace cg = cooperative_groups;
+
+namespace bj {
+
+namespace {
+
+constexpr int kClusterSize = 8;
+constexpr int kClThreads = 256;
+constexpr int kClWarps = kClThreads / 32;
+constexpr int kClRowReg = 8;   // a thread keeps its row's entries in registers when no row is longer
+
+struct ClusterLzParams {
+    int n, nnz, nblocks, m, reorth;
+    int bpc;          // diagonal blocks per CTA (the last CTAs may own fewer, or none)
+    int nl_max;       // rows per CTA at most (bpc * b, or bpc for b = 0)
+    int ld;           // leading dimension of the basis slice Vt[row][vector] (odd: conflict-free in both passes)
+    int row_in_regs;  // nl_max <= kClThreads and no row longer than kClRowReg
+    int groups_max;   // interleave groups of factors a CTA copies at most
+    double tol;
+    const int32_t* rp;
+    const int32_t* ci;
+    const double* val;
+    const double* fac;  // fac_small (interleaved packed, reciprocal diagonals) or null
+    const double* v0;
+    double* alpha;      // [m] global
+    double* beta;       // [m] global
+    int* done;          // [0] stop flag, [1] m_eff, [2] invalid start vector
+};
+
+// sum over the CTA in a fixed order (shuffle tree per warp, pairwise tree over the warp sums), valid on every thread
+__device__ __forceinline__ double cl_cta_sum(double v, double* sh)
+{
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) sh[warp] = v;
+    __syncthreads();
+    double s[kClWarps];
+#pragma unroll
+    for (int q = 0; q < kClWarps; ++q) s[q] = sh[q];
+#pragma unroll
+    for (int w = kClWarps / 2; w > 0; w >>= 1)
+#pragma unroll
+        for (int q = 0; q < w; ++q) s[q] += s[q + w];
+    return s[0];
+}
+
+// Exchanges between the CTAs are one-way pushes: st.async writes 8 bytes into a peer's shared memory and counts them on
+// the PEER's mbarrier (complete_tx), the receiver arms that barrier with the bytes it expects and waits for the phase --
+// no cluster-wide barrier, no wait for store acknowledgements (a cluster barrier after remote stores measured ~1000
+// cycles per exchange, three to five times per step).  Exchange e uses barrier e & 1 and buffer e & 1: a CTA can be at
+// most one exchange ahead of a peer (it needs every peer's data of exchange e to finish e, and a peer sends e only after
+// it has read the buffer of e - 1), so two alternate.
+struct Exchange {
+    uint64_t* bar;  // [2]
+    int e;          // exchanges started so far (identical on every CTA)
+    int rank;
+};
+
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t saddr, int rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_async_f64(uint32_t raddr, double v, uint32_t rbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(raddr),
+                 "l"(__double_as_longlong(v)), "r"(rbar)
+                 : "memory");
+}
+
+// every CTA sends src[0..count) to dst_base[dst_off + 0..count) of EVERY CTA (itself included) and waits until the eight
+// contributions (total_doubles in all) have arrived in its own copy
+__device__ __forceinline__ void exchange_all(Exchange& x, const double* src, int count, double* dst_base, int dst_off, int total_doubles)
+{
+    uint64_t* bar = x.bar + (x.e & 1);
+    const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
+    if (threadIdx.x == 0) mbar_expect_tx(bar, (uint32_t)total_doubles * 8u);
+    const uint32_t bar_s = smem_u32(bar), dst_s = smem_u32(dst_base + dst_off);
+    for (int e = threadIdx.x; e < count * kClusterSize; e += kClThreads) {
+        const int dst = e & (kClusterSize - 1), q = e >> 3;
+        st_async_f64(mapa_u32(dst_s + 8u * (uint32_t)q, dst), src[q], mapa_u32(bar_s, dst));
+    }
+    mbar_wait(bar, parity);
+    ++x.e;
+}
+
+// All-reduce of `count` doubles: part[0..count) goes to slot `rank` of every CTA's exchange buffer; thread q then adds the
+// slots 0..7 in order into out[q] (the same bits on every CTA).
+__device__ __forceinline__ void cluster_allreduce(Exchange& x, const double* part, int count, double* xch2, int pm, double* out)
+{
+    double* xch = xch2 + (size_t)(x.e & 1) * kClusterSize * pm;
+    exchange_all(x, part, count, xch, x.rank * pm, count * kClusterSize);
+    for (int q = threadIdx.x; q < count; q += kClThreads) {
+        double s = 0.0;
+#pragma unroll
+        for (int r = 0; r < kClusterSize; ++r) s += xch[r * pm + q];
+        out[q] = s;
+    }
+    __syncthreads();
+}
+
+// x = L^-T y (DIR 1) or L^-1 y (DIR 0) on the CTA's own diagonal blocks k_lo .. k_hi, thread per block, factors in shared
+// memory (the interleave groups that cover the range, g_lo first); in / out are the CTA's local slices.
+// The arithmetic and its order are solve_small_kernel's.
+template <int B, int DIR>
+__device__ __forceinline__ void cluster_solve(int n, int k_lo, int k_hi, int g_lo, const double* sf, const double* in, double* out)
+{
+    if constexpr (B == 0) {
+        for (int i = threadIdx.x; i < k_hi - k_lo; i += kClThreads) out[i] = in[i];
+    } else {
+        constexpr int P = B * (B + 1) / 2;
+        for (int k = k_lo + threadIdx.x; k < k_hi; k += kClThreads) {
+            const double* f = sf + (size_t)((k >> 5) - g_lo) * (P * kInterleave) + (k & 31);
+            const int li = (k - k_lo) * B, lo = k * B;
+            double v[B];
+#pragma unroll
+            for (int i = 0; i < B; ++i) v[i] = (lo + i < n) ? in[li + i] : 0.0;
+            if (DIR == 0) {
+#pragma unroll
+                for (int i = 0; i < B; ++i) {
+                    double s = v[i];
+#pragma unroll
+                    for (int j = 0; j < B; ++j)
+                        if (j < i) s -= f[(i * (i + 1) / 2 + j) * kInterleave] * v[j];
+                    v[i] = s * f[(i * (i + 1) / 2 + i) * kInterleave];
+                }
+            } else {
+#pragma unroll
+                for (int i = B - 1; i >= 0; --i) {
+                    double s = v[i];
+#pragma unroll
+                    for (int j = 0; j < B; ++j)
+                        if (j > i) s -= f[(j * (j + 1) / 2 + i) * kInterleave] * v[j];
+                    v[i] = s * f[(i * (i + 1) / 2 + i) * kInterleave];
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < B; ++i)
+                if (lo + i < n) out[li + i] = v[i];
+        }
+    }
+}
+
+template <int B>
+__global__ void __cluster_dims__(kClusterSize, 1, 1) __launch_bounds__(kClThreads)
+lanczos_cluster_kernel(const ClusterLzParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cg::cluster_group cl = cg::this_cluster();
+    const int rank = (int)cl.block_rank();
+    const int n = p.n, tid = threadIdx.x;
+    constexpr int BB = B > 0 ? B : 1;                  // rows per unit (a "block" of the b = 0 handle is one row)
+    constexpr int P = B * (B + 1) / 2;
+    const int units = B > 0 ? p.nblocks : n;
+    const int k_lo = min(units, rank * p.bpc), k_hi = min(units, k_lo + p.bpc);
+    const int row_lo = k_lo * BB;
+    const int nl = min(n, k_hi * BB) - row_lo;          // rows of this CTA (0 for a CTA beyond the last block)
+    const int g_lo = k_lo >> 5;
+    const int pm = (p.m + 2) & ~1;
+    // red | dpart | part | c | xch[2][8][pm] | t_full[n] | tl | u | w | vc | vp (nl_max each) | fac | Vt[nl_max][ld] | 2 mbarriers
+    double* red = reinterpret_cast<double*>(smem_raw);
+    double* dpart = red + kClWarps;                     // (slice, vector) partials of a dot sweep
+    double* part = dpart + kClThreads;
+    double* c = part + pm;
+    double* xch = c + pm;
+    double* t_full = xch + 2 * kClusterSize * pm;
+    double* tl = t_full + ((n + 1) & ~1);
+    double* u = tl + p.nl_max;
+    double* w = u + p.nl_max;
+    double* vc = w + p.nl_max;
+    double* vp = vc + p.nl_max;
+    double* sf = vp + p.nl_max;
+    double* Vt = sf + (size_t)p.groups_max * P * kInterleave;
+    Exchange x;
+    x.bar = reinterpret_cast<uint64_t*>(Vt + (p.reorth ? (size_t)p.nl_max * p.ld : 0));
+    x.e = 0;
+    x.rank = rank;
+    if (tid == 0) {
+        mbar_init(&x.bar[0], 1);
+        mbar_init(&x.bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cl.sync();  // every CTA's barriers exist before a peer signals them
+    auto allreduce = [&](int count, double* out) { cluster_allreduce(x, part, count, xch, pm, out); };
+    if constexpr (B > 0) {
+        const int g_hi = k_hi > k_lo ? ((k_hi - 1) >> 5) + 1 : g_lo;
+        const double* src = p.fac + (size_t)g_lo * (P * kInterleave);
+        for (int e = tid; e < (g_hi - g_lo) * P * kInterleave; e += kClThreads) sf[e] = src[e];
+    }
+    // row `row_lo + tid` of the matrix in registers
+    double rv[kClRowReg];
+    int rc[kClRowReg];
+    int rlen = 0;
+#pragma unroll
+    for (int q = 0; q < kClRowReg; ++q) { rv[q] = 0.0; rc[q] = 0; }
+    if (p.row_in_regs && tid < nl) {
+        const int s0 = p.rp[row_lo + tid];
+        rlen = p.rp[row_lo + tid + 1] - s0;
+#pragma unroll
+        for (int q = 0; q < kClRowReg; ++q)
+            if (q < rlen) { rv[q] = p.val[s0 + q]; rc[q] = p.ci[s0 + q]; }
+    }
+    // v_1 = v0 / ||v0||
+    double s = 0.0;
+    for (int i = tid; i < nl; i += kClThreads) { const double x0 = p.v0[row_lo + i]; s = fma(x0, x0, s); }
+    s = cl_cta_sum(s, red);
+    if (tid == 0) part[0] = s;
+    __syncthreads();
+    allreduce(1, c);
+    const double nrm = sqrt(c[0]);
+    if (!(nrm > 0.0) || isinf(nrm)) {  // zero or non-finite start vector: invalid argument (uniform over the cluster)
+        if (rank == 0 && tid == 0) { p.done[0] = 1; p.done[2] = 1; }
+        cl.sync();
+        return;
+    }
+    for (int i = tid; i < nl; i += kClThreads) {
+        const double x0 = p.v0[row_lo + i] / nrm;
+        vc[i] = x0;
+        vp[i] = 0.0;
+        if (p.reorth) Vt[(size_t)i * p.ld] = x0;
+    }
+    double beta_j = 0.0, amax = 0.0;
+    __syncthreads();
+    for (int j = 0; j < p.m; ++j) {
+        // ---- t = L^-T v_j on the own blocks, then to every CTA (the SpMV reads arbitrary columns) ----
+        cluster_solve<B, 1>(n, k_lo, k_hi, g_lo, sf, vc, tl);
+        __syncthreads();
+        exchange_all(x, tl, nl, t_full, row_lo, n);
+        // ---- u = A t (own rows, left to right: the oracle's order), w = L^-1 u ----
+        if (p.row_in_regs) {
+            if (tid < nl) {
+                double acc = 0.0;
+#pragma unroll
+                for (int q = 0; q < kClRowReg; ++q)
+                    if (q < rlen) acc = fma(rv[q], t_full[rc[q]], acc);
+                u[tid] = acc;
+            }
+        } else {
+            for (int i = tid; i < nl; i += kClThreads) {
+                double acc = 0.0;
+                const int e = p.rp[row_lo + i + 1];
+                for (int q = p.rp[row_lo + i]; q < e; ++q) acc = fma(p.val[q], t_full[p.ci[q]], acc);
+                u[i] = acc;
+            }
+        }
+        __syncthreads();
+        cluster_solve<B, 0>(n, k_lo, k_hi, g_lo, sf, u, w);
+        __syncthreads();
+        // ---- w -= beta_j v_{j-1};  alpha_j = v_j . w;  w -= alpha_j v_j ----
+        double pa = 0.0;
+        for (int i = tid; i < nl; i += kClThreads) {
+            double wi = w[i];
+            if (j > 0) { wi -= beta_j * vp[i]; w[i] = wi; }
+            pa = fma(vc[i], wi, pa);
+        }
+        pa = cl_cta_sum(pa, red);
+        if (tid == 0) part[0] = pa;
+        __syncthreads();
+        allreduce(1, c);
+        const double a = c[0];
+        __syncthreads();  // c is rewritten by the reorthogonalisation
+        for (int i = tid; i < nl; i += kClThreads) w[i] -= a * vc[i];
+        __syncthreads();
+        // ---- full reorthogonalisation, classical Gram-Schmidt twice over v_1 .. v_j: c = V^T w, then w -= V c ----
+        if (p.reorth) {
+            const int nv = j + 1;
+            // dots: thread = (vector q, row slice): consecutive lanes read consecutive vectors of one row of Vt
+            // (conflict-free), w[row] is a broadcast; no shuffles.  `cols` vectors per sweep (a power of two that covers nv,
+            // at most 64), kClThreads / cols row slices; the partials of a vector are added in slice order.
+            int cols = 8;
+            while (cols < nv && cols < 64) cols <<= 1;
+            const int slices = kClThreads / cols;
+            const int per = (nl + slices - 1) / slices;
+            const int qc = tid & (cols - 1), sl = tid / cols;
+            const int i0 = min(nl, sl * per), i1 = min(nl, i0 + per);
+            for (int pass = 0; pass < 2; ++pass) {
+                for (int q0 = 0; q0 < nv; q0 += cols) {
+                    const int q = q0 + qc;
+                    double s0 = 0.0, s1 = 0.0;
+                    if (q < nv) {
+                        const double* col = Vt + q;
+                        int i = i0;
+                        for (; i + 1 < i1; i += 2) {
+                            s0 = fma(col[(size_t)i * p.ld], w[i], s0);
+                            s1 = fma(col[(size_t)(i + 1) * p.ld], w[i + 1], s1);
+                        }
+                        if (i < i1) s0 = fma(col[(size_t)i * p.ld], w[i], s0);
+                    }
+                    dpart[sl * cols + qc] = s0 + s1;
+                    __syncthreads();
+                    if (tid < cols && q0 + tid < nv) {
+                        double sq = dpart[tid];
+                        for (int r = 1; r < slices; ++r) sq += dpart[r * cols + tid];
+                        part[q0 + tid] = sq;
+                    }
+                    __syncthreads();
+                }
+                allreduce(nv, c);
+                // w -= V c: thread per row, the row of Vt is contiguous; lanes are ld (odd) doubles apart: conflict-free
+                for (int i = tid; i < nl; i += kClThreads) {
+                    const double* row = Vt + (size_t)i * p.ld;
+                    double wi = w[i];
+                    for (int q = 0; q < nv; ++q) wi -= c[q] * row[q];  // subtraction order q = 0, 1, .. (the oracle's)
+                    w[i] = wi;
+                }
+                __syncthreads();
+            }
+        }
+        // ---- beta_{j+1} = ||w||, bookkeeping, breakdown test ----
+        double pb = 0.0;
+        for (int i = tid; i < nl; i += kClThreads) pb = fma(w[i], w[i], pb);
+        pb = cl_cta_sum(pb, red);
+        if (tid == 0) part[0] = pb;
+        __syncthreads();
+        allreduce(1, c);
+        const double bn = sqrt(c[0]);
+        amax = fabs(a) > amax ? fabs(a) : amax;
+        const bool brk = !(bn > p.tol * amax);
+        if (rank == 0 && tid == 0) {
+            p.alpha[j] = a;
+            p.beta[j] = bn;
+            p.done[1] = j + 1;
+            if (brk) p.done[0] = 1;
+        }
+        if (brk || j + 1 == p.m) break;  // uniform over the cluster: every CTA holds the same bits
+        __syncthreads();
+        for (int i = tid; i < nl; i += kClThreads) {
+            const double x1 = w[i] / bn;
+            vp[i] = vc[i];
+            vc[i] = x1;
+            if (p.reorth) Vt[(size_t)i * p.ld + (j + 1)] = x1;
+        }
+        beta_j = bn;
+        __syncthreads();
+    }
+    cl.sync();  // no CTA leaves while another may still address its shared memory
+}
+
+struct ClusterGeom {
+    int bpc, nl_max, ld, groups_max;
+    size_t smem;
+};
+
+ClusterGeom cluster_geometry(const bj_handle_s* h, int m, bool reorth)
+{
+    ClusterGeom g;
+    const int bb = h->solve_kind == 1 ? h->b : 1;
+    const int64_t units = h->solve_kind == 1 ? h->nblocks : h->n;
+    g.bpc = (int)((units + kClusterSize - 1) / kClusterSize);
+    g.nl_max = g.bpc * bb;
+    g.ld = m | 1;
+    g.groups_max = h->solve_kind == 1 ? (g.bpc + kInterleave - 1) / kInterleave + 1 : 0;
+    const size_t pm = (size_t)((m + 2) & ~1);
+    size_t d = kClWarps + kClThreads + 2 * pm + 2 * kClusterSize * pm + (((size_t)h->n + 1) & ~(size_t)1) + 5 * (size_t)g.nl_max +
+               (size_t)g.groups_max * h->packed * kInterleave;
+    if (reorth) d += (size_t)g.nl_max * g.ld;
+    g.smem = d * 8 + 16 + 16;
+    return g;
+}
+
+}  // namespace
+
+// The cluster form is used when a CTA's share of the basis fits its shared memory beside the work vectors (N = 1024, m = 50:
+// 52 KB of basis per CTA); otherwise the single-CTA kernel (basis through L2) or the multi-launch path run.
+bool lanczos_cluster_usable(const bj_handle_s* h, int m, bool reorth)
+{
+    if (env_int("BJ_LANCZOS_CLUSTER", 1) == 0) return false;
+    if (h->var_perm || !(h->solve_kind == 0 || (h->solve_kind == 1 && !h->tri)) || m > 1024 || h->n > 16384 || h->n < kClusterSize ||
+        h->nnz == 0)
+        return false;
+    return cluster_geometry(h, m, reorth).smem <= 220 * 1024;
+}
+
+int launch_lanczos_cluster(bj_handle_s* h, int m, bool reorth, double tol, const double* v0, double* alpha, double* beta, int* done)
+{
+    const ClusterGeom g = cluster_geometry(h, m, reorth);
+    ClusterLzParams p;
+    p.n = (int)h->n; p.nnz = (int)h->nnz; p.nblocks = (int)h->nblocks; p.m = m;
+    p.reorth = reorth ? 1 : 0;
+    p.bpc = g.bpc; p.nl_max = g.nl_max; p.ld = g.ld; p.groups_max = g.groups_max;
+    p.row_in_regs = (g.nl_max <= kClThreads && h->max_row_nnz <= kClRowReg) ? 1 : 0;
+    p.tol = tol;
+    p.rp = h->row_ptr; p.ci = h->col_idx; p.val = h->val;
+    p.fac = h->solve_kind == 1 ? h->fac_small : nullptr;
+    p.v0 = v0; p.alpha = alpha; p.beta = beta; p.done = done;
+    cudaError_t e = cudaSuccess;
+#define BJ_CASE(B)                                                                                              \
+    case B: {                                                                                                   \
+        static std::atomic<bool> configured[64];                                                                \
+        e = ensure_big_smem(lanczos_cluster_kernel<B>, configured);                                             \
+        if (e == cudaSuccess) lanczos_cluster_kernel<B><<<kClusterSize, kClThreads, g.smem, h->stream>>>(p);    \
+        break;                                                                                                  \
+    }
+    switch (h->solve_kind == 1 ? h->b : 0) {
+        BJ_CASE(0) BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
+        default: return BJ_ERR_INVALID_ARG;
+    }
+#undef BJ_CASE
+    if (e != cudaSuccess) { set_cuda_error(e, "lanczos_cluster_kernel"); return BJ_ERR_CUDA; }
+    h->launches++;
+    BJ_CUDA(cudaGetLastError());
+    return BJ_OK;
+}
+
+}  // namespace bj

@@ -182,6 +182,7 @@ def test_zero_or_nonfinite_start_vector_is_an_invalid_argument(B, torch_, which)
         h, keep = B.setup_from_host(A, b)
         for fuse in (1, 0):
             B.bj_set_option(h, B.BJ_OPT_LANCZOS_FUSE, fuse)
+            B.bj_set_option(h, B.BJ_OPT_LANCZOS_SINGLE_LAUNCH, 1 if fuse else 2)   # cluster form / single-CTA form
             for v0 in (z, nan):
                 for reorth in (False, True):
                     with pytest.raises(B.BJError) as e:
@@ -201,20 +202,23 @@ def test_single_launch_lanczos_for_launch_bound_sizes(B, torch_):
         for b in blocks:
             h, keep = B.setup_from_host(A, b)
             P = oracle.Precond(A, b)
-            l0 = B.bj_get_info(h)["kernel_launches"]
-            g = B.bj_cond_estimate_ex(h, 50, reorth=True)
-            assert B.bj_get_info(h)["kernel_launches"] - l0 <= 2          # seeded vector + the one kernel
             c = P.cond_estimate(50, reorth=True)
-            assert g["iters_done"] == c["iters_done"]
-            assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (A.n, b, g["kappa"], c["kappa"])
-            assert np.allclose(g["alpha"], c["alpha"], rtol=1e-8, atol=1e-10 * abs(c["alpha"]).max())
-            assert np.allclose(g["beta"], c["beta"], rtol=1e-7, atol=1e-10 * abs(c["alpha"]).max())
-            g0 = B.bj_cond_estimate_ex(h, 30, reorth=False)
             c0 = P.cond_estimate(30, reorth=False)
-            assert np.abs(g0["alpha"] - c0["alpha"]).max() <= 1e-8 * abs(c0["alpha"]).max(), (A.n, b)
             v0 = W.seeded_vector(77, A.n)
-            gv = B.bj_cond_estimate_ex(h, 20, reorth=True, v0=dev(torch_, v0))
-            assert abs(gv["kappa"] / P.cond_estimate(20, v0=v0)["kappa"] - 1) <= TOL_KAPPA
+            cv = P.cond_estimate(20, v0=v0)
+            for form in (1, 2):      # 1: the eight-CTA cluster kernel where a CTA's share of the basis fits; 2: one CTA
+                B.bj_set_option(h, B.BJ_OPT_LANCZOS_SINGLE_LAUNCH, form)
+                l0 = B.bj_get_info(h)["kernel_launches"]
+                g = B.bj_cond_estimate_ex(h, 50, reorth=True)
+                assert B.bj_get_info(h)["kernel_launches"] - l0 <= 2          # seeded vector + the one kernel
+                assert g["iters_done"] == c["iters_done"]
+                assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (A.n, b, form, g["kappa"], c["kappa"])
+                assert np.allclose(g["alpha"], c["alpha"], rtol=1e-8, atol=1e-10 * abs(c["alpha"]).max())
+                assert np.allclose(g["beta"], c["beta"], rtol=1e-7, atol=1e-10 * abs(c["alpha"]).max())
+                g0 = B.bj_cond_estimate_ex(h, 30, reorth=False)
+                assert np.abs(g0["alpha"] - c0["alpha"]).max() <= 1e-8 * abs(c0["alpha"]).max(), (A.n, b, form)
+                gv = B.bj_cond_estimate_ex(h, 20, reorth=True, v0=dev(torch_, v0))
+                assert abs(gv["kappa"] / cv["kappa"] - 1) <= TOL_KAPPA
             B.bj_set_option(h, B.BJ_OPT_LANCZOS_SINGLE_LAUNCH, 0)           # the multi-launch path on the same handle
             l0 = B.bj_get_info(h)["kernel_launches"]
             gm = B.bj_cond_estimate_ex(h, 50, reorth=True)
@@ -223,9 +227,18 @@ def test_single_launch_lanczos_for_launch_bound_sizes(B, torch_):
             B.bj_destroy(h)
     A = W.block_diagonal_spd(100, 8)          # M = A: breakdown at step 1 inside the single kernel
     h, keep = B.setup_from_host(A, 8)
-    g = B.bj_cond_estimate_ex(h, 20, reorth=True)
-    assert g["iters_done"] == 1 and abs(g["kappa"] - 1) < 1e-12
+    for form in (1, 2):
+        B.bj_set_option(h, B.BJ_OPT_LANCZOS_SINGLE_LAUNCH, form)
+        g = B.bj_cond_estimate_ex(h, 20, reorth=True)
+        assert g["iters_done"] == 1 and abs(g["kappa"] - 1) < 1e-12
     B.bj_destroy(h)
+    # fewer blocks than CTAs, and a block count that leaves the last CTAs of the cluster without rows
+    for A, b in ((W.laplacian((5, 4)), 4), (W.laplacian((9, 9)), 8), (W.laplacian((3, 3)), 0)):
+        h, keep = B.setup_from_host(A, b)
+        g = B.bj_cond_estimate_ex(h, A.n, reorth=True)
+        c = oracle.Precond(A, b).cond_estimate(A.n, reorth=True)
+        assert g["iters_done"] == c["iters_done"] and abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (A.n, b)
+        B.bj_destroy(h)
 
 
 def test_point_jacobi_is_the_papers_kernel(B, torch_):
