@@ -59,7 +59,8 @@ typedef enum {
     BJ_ERR_TOO_LARGE = -3,     /* n or nnz >= 2^31                                                         */
     BJ_ERR_NOT_SPD = -4,       /* a diagonal block has a pivot <= 0 or non-finite; see bj_info_t.bad_block  */
     BJ_ERR_ALLOC = -5,         /* device or host allocation failed                                         */
-    BJ_ERR_CUDA = -6           /* CUDA runtime error (sticky text in bj_strerror)                           */
+    BJ_ERR_CUDA = -6,          /* CUDA runtime error (sticky text in bj_strerror)                           */
+    BJ_ERR_LIMIT = -7          /* bj_cond_estimate_noalloc: outside the limits of its fixed device scratch  */
 } bj_status;
 
 typedef struct bj_handle_s* bj_handle_t;
@@ -232,6 +233,21 @@ int bj_cond_estimate_ex(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_la
  * unnormalised, scalars on the device, one synchronisation at the end.  Workspace: the PCG workspace (4 n doubles, kept).
  * A zero start vector returns BJ_ERR_INVALID_ARG.  Synchronises. */
 int bj_cond_estimate_minv(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_lanczos_result_t* res_host);
+
+/* bj_cond_estimate_ex for callers that cannot allocate device memory at call time (CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same options, same result fields, the same single-launch cluster kernel
+ * (DESIGN.md section 5), but its device scratch (start vector, alpha, beta, status words) is ONE file-scope device array
+ * of fixed size, 147 488 bytes, which every GPU that loads the library holds until the process exits.  The call makes no
+ * cudaMalloc / cudaFree / pool call and no allocating library call.
+ * Limits: n <= BJ_NOALLOC_MAX_N, iters <= BJ_NOALLOC_MAX_ITERS, uniform blocks b <= 8 or b = 0 without permutation
+ * or band storage, and a CTA's share of the basis must fit its shared memory (8 CTAs; n (iters | 1) + ... <= 220 KB each);
+ * anything beyond returns BJ_ERR_LIMIT and does nothing.  The handle comes from bj_setup as usual (setup does allocate).
+ * Every call on a device shares the array, which keeps the previous call's contents (the call clears what must start at
+ * zero): calls that OVERLAP on the GPU -- two handles on two streams of one device -- race on it; serialise them.
+ * The device must be current.  Synchronises. */
+#define BJ_NOALLOC_MAX_N 16384
+#define BJ_NOALLOC_MAX_ITERS 1024
+int bj_cond_estimate_noalloc(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_lanczos_result_t* res_host);
 
 /* preconditioned conjugate gradients for A x = b from x_0 = 0 with M = blockdiag(D_k)
  * (z = M^-1 r is bj_apply; b = 0 handle: plain CG), the classical stand-in for the solve stage that follows

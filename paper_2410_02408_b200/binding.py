@@ -15,6 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libbj.so")
 BJ_B_MAX = 32
 BJ_DEFAULT_SEED = 0x241002408
 BJ_OK, BJ_ERR_INVALID_ARG, BJ_ERR_NOT_CANONICAL, BJ_ERR_TOO_LARGE, BJ_ERR_NOT_SPD, BJ_ERR_ALLOC, BJ_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
+BJ_ERR_LIMIT = -7
+BJ_NOALLOC_MAX_N, BJ_NOALLOC_MAX_ITERS = 16384, 1024
 BJ_K_SOLVE_LT, BJ_K_SPMV, BJ_K_SOLVE_L, BJ_K_APPLY, BJ_K_SPMV_SOLVE_L, BJ_K_COUNT = 0, 1, 2, 3, 4, 5
 BJ_OPT_SPMV_KERNEL, BJ_OPT_FUSE_FORWARD, BJ_OPT_LANCZOS_FUSE, BJ_OPT_PCG_FUSE, BJ_OPT_LANCZOS_SINGLE_LAUNCH = 1, 2, 3, 4, 5
 KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
@@ -24,7 +26,7 @@ EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_setup_ex", "bj_get_setup_time",
            "bj_cond_estimate_ex", "bj_seeded_vector", "bj_op_apply_host", "bj_apply_host", "bj_profile_enable",
            "bj_profile_get", "bj_release_cached_memory", "bj_pcg_solve",
            "bj_cond_estimate_batch", "bj_pcg_solve_batch", "bj_cond_estimate_minv", "bj_setup_blocks", "bj_setup_perm",
-           "bj_setup_blocks_perm"]
+           "bj_setup_blocks_perm", "bj_cond_estimate_noalloc"]
 
 
 class bj_csr_t(C.Structure):
@@ -89,6 +91,7 @@ def lib():
         L.bj_setup_ex.argtypes = [C.POINTER(bj_csr_t), i32, C.POINTER(bj_setup_opts_t), C.POINTER(vp)]
         L.bj_get_setup_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.bj_cond_estimate_minv.argtypes = [vp, C.POINTER(bj_lanczos_opts_t), C.POINTER(bj_lanczos_result_t)]
+        L.bj_cond_estimate_noalloc.argtypes = [vp, C.POINTER(bj_lanczos_opts_t), C.POINTER(bj_lanczos_result_t)]
         L.bj_setup_blocks.argtypes = [C.POINTER(bj_csr_t), vp, i64, vp, C.POINTER(vp)]
         L.bj_setup_perm.argtypes = [C.POINTER(bj_csr_t), i32, vp, vp, C.POINTER(vp)]
         L.bj_setup_blocks_perm.argtypes = [C.POINTER(bj_csr_t), vp, i64, vp, vp, C.POINTER(vp)]
@@ -306,6 +309,23 @@ def bj_cond_estimate_ex(h, iters: int, reorth: bool = True, seed: int = BJ_DEFAU
                           _dptr(v0, torch.float64, h.n) if v0 is not None else None, breakdown_tol)
     r = bj_lanczos_result_t(0, 0.0, 0.0, 0.0, 0.0, alpha.ctypes.data_as(C.c_void_p), beta.ctypes.data_as(C.c_void_p))
     _check(lib().bj_cond_estimate_ex(h.ptr, C.byref(o), C.byref(r)))
+    k = r.iters_done
+    return {"iters_done": k, "lmin": r.lmin, "lmax": r.lmax, "kappa": r.lmax / r.lmin, "res_min": r.res_min,
+            "res_max": r.res_max, "alpha": alpha[:k].copy(), "beta": beta[:k].copy()}
+
+
+def bj_cond_estimate_noalloc(h, iters: int, reorth: bool = True, seed: int = BJ_DEFAULT_SEED, v0=None,
+                             breakdown_tol: float = 0.0) -> dict:
+    """bj_cond_estimate_ex without any device allocation at call time (fixed file-scope device scratch; BJ_ERR_LIMIT beyond
+    n <= 16384, iters <= 1024, b <= 8).  Calls that overlap on one GPU race on the scratch."""
+    import numpy as np
+    import torch
+    alpha = np.zeros(iters)
+    beta = np.zeros(iters)
+    o = bj_lanczos_opts_t(int(iters), int(bool(reorth)), seed & 0xFFFFFFFFFFFFFFFF,
+                          _dptr(v0, torch.float64, h.n) if v0 is not None else None, breakdown_tol)
+    r = bj_lanczos_result_t(0, 0.0, 0.0, 0.0, 0.0, alpha.ctypes.data_as(C.c_void_p), beta.ctypes.data_as(C.c_void_p))
+    _check(lib().bj_cond_estimate_noalloc(h.ptr, C.byref(o), C.byref(r)))
     k = r.iters_done
     return {"iters_done": k, "lmin": r.lmin, "lmax": r.lmax, "kappa": r.lmax / r.lmin, "res_min": r.res_min,
             "res_max": r.res_max, "alpha": alpha[:k].copy(), "beta": beta[:k].copy()}

@@ -188,6 +188,8 @@ const char* bj_strerror(int code)
         case BJ_ERR_NOT_SPD: return "a diagonal block is not positive definite (see bj_get_info bad_block)";
         case BJ_ERR_ALLOC: return "allocation failed";
         case BJ_ERR_CUDA: return g_cuda_msg;
+        case BJ_ERR_LIMIT: return "bj_cond_estimate_noalloc: beyond the limits of the fixed device scratch (n <= 16384, iters <= 1024, "
+                                  "uniform blocks b <= 8 or b = 0 without permutation or band storage, basis share fits shared memory)";
         default: return "unknown bj status";
     }
 }
