@@ -7,12 +7,15 @@
 //   * the slice of t = L^-T v_j (the SpMV reads arbitrary columns: every CTA keeps the full vector),
 //   * the partial sums of alpha_j, of the reorthogonalisation coefficients (two passes) and of beta_{j+1}:
 // each CTA pushes its partials into slot r of every CTA's exchange buffer, every CTA adds the eight slots in the same
-// order, so all CTAs hold bit-identical scalars and take the same branches.
+// order, so all CTAs hold bit-identical scalars and take the same branches.  Per step: five exchanges of ~500 cycles and
+// about twenty __syncthreads-separated phases of a few hundred cycles each -- the kernel is a latency chain (5.5 us per
+// step with full reorthogonalisation over 25 vectors on average, 3.3 us without), not bandwidth-bound anywhere.
 // Same recurrence, statement by statement, as lanczos_run (readings 10-13); the operator is the
 // arithmetic of solve_small_kernel (thread per block, interleaved packed factors) and of a row-per-thread CSR product
 // summed left to right.  Block sizes b <= 8 and b = 0.
 #include <cooperative_groups.h>
 #include <math.h>
+#include <stdio.h>
 
 #include <algorithm>
 #include <atomic>
@@ -30,6 +33,7 @@ constexpr int kClusterSize = 8;
 constexpr int kClThreads = 256;
 constexpr int kClWarps = kClThreads / 32;
 constexpr int kClRowReg = 8;   // a thread keeps its row's entries in registers when no row is longer
+constexpr int kClDotCols = 64; // basis vectors per sweep of the dot pass
 
 struct ClusterLzParams {
     int n, nnz, nblocks, m, reorth;
@@ -109,19 +113,44 @@ __device__ __forceinline__ void exchange_all(Exchange& x, const double* src, int
     ++x.e;
 }
 
-// All-reduce of `count` doubles: part[0..count) goes to slot `rank` of every CTA's exchange buffer; thread q then adds the
-// slots 0..7 in order into out[q] (the same bits on every CTA).
-__device__ __forceinline__ void cluster_allreduce(Exchange& x, const double* part, int count, double* xch2, int pm, double* out)
+// The same exchange for a long slice (the CTA's rows of t): ONE bulk copy per peer through the async proxy instead of
+// count st.async per peer (1240 -> ~500 cycles for 128 rows), when the slice is 16-byte aligned and sized; the caller
+// has made src visible to the async proxy (fence.proxy.async before its __syncthreads).  src is not rewritten before
+// every peer has passed the next exchange, i.e. long after the copies have read it.
+__device__ __forceinline__ void exchange_all_bulk(Exchange& x, const double* src, int count, double* dst_base, int dst_off, int total_doubles)
+{
+    if (((count | dst_off) & 1) != 0) return exchange_all(x, src, count, dst_base, dst_off, total_doubles);
+    uint64_t* bar = x.bar + (x.e & 1);
+    const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
+    if (threadIdx.x == 0) mbar_expect_tx(bar, (uint32_t)total_doubles * 8u);
+    if (threadIdx.x < kClusterSize && count > 0) {
+        const uint32_t dst = mapa_u32(smem_u32(dst_base + dst_off), threadIdx.x), rbar = mapa_u32(smem_u32(bar), threadIdx.x);
+        asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                     "r"(smem_u32(src)), "r"((uint32_t)count * 8u), "r"(rbar)
+                     : "memory");
+    }
+    mbar_wait(bar, parity);
+    ++x.e;
+}
+
+// All-reduce of ONE double that every thread of the CTA already holds (cl_cta_sum): threads 0..7 push it straight from
+// the register to the eight CTAs, every thread adds the eight slots itself -- no staging store, no __syncthreads.
+// (The callers' next exchange is always behind a __syncthreads, so no thread still reads this buffer when a peer
+// refills it two exchanges later.)
+__device__ __forceinline__ double cluster_allreduce_scalar(Exchange& x, double v, double* xch2, int pm)
 {
     double* xch = xch2 + (size_t)(x.e & 1) * kClusterSize * pm;
-    exchange_all(x, part, count, xch, x.rank * pm, count * kClusterSize);
-    for (int q = threadIdx.x; q < count; q += kClThreads) {
-        double s = 0.0;
+    uint64_t* bar = x.bar + (x.e & 1);
+    const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
+    if (threadIdx.x == 0) mbar_expect_tx(bar, 8u * kClusterSize);
+    if (threadIdx.x < kClusterSize)
+        st_async_f64(mapa_u32(smem_u32(xch + x.rank * pm), threadIdx.x), v, mapa_u32(smem_u32(bar), threadIdx.x));
+    mbar_wait(bar, parity);
+    ++x.e;
+    double s = 0.0;
 #pragma unroll
-        for (int r = 0; r < kClusterSize; ++r) s += xch[r * pm + q];
-        out[q] = s;
-    }
-    __syncthreads();
+    for (int r = 0; r < kClusterSize; ++r) s += xch[r * pm];
+    return s;
 }
 
 // x = L^-T y (DIR 1) or L^-1 y (DIR 0) on the CTA's own diagonal blocks k_lo .. k_hi, thread per block, factors in shared
@@ -182,11 +211,10 @@ lanczos_cluster_kernel(const ClusterLzParams p)
     const int nl = min(n, k_hi * BB) - row_lo;          // rows of this CTA (0 for a CTA beyond the last block)
     const int g_lo = k_lo >> 5;
     const int pm = (p.m + 2) & ~1;
-    // red | dpart | part | c | xch[2][8][pm] | t_full[n] | tl | u | w | vc | vp (nl_max each) | fac | Vt[nl_max][ld] | 2 mbarriers
+    // red | dpart | c | xch[2][8][pm] | t_full[n] | tl | u | w | vc | vp (nl_max each) | fac | Vt[nl_max][ld] | 2 mbarriers
     double* red = reinterpret_cast<double*>(smem_raw);
     double* dpart = red + kClWarps;                     // (slice, vector) partials of a dot sweep
-    double* part = dpart + kClThreads;
-    double* c = part + pm;
+    double* c = dpart + kClThreads;
     double* xch = c + pm;
     double* t_full = xch + 2 * kClusterSize * pm;
     double* tl = t_full + ((n + 1) & ~1);
@@ -206,7 +234,6 @@ lanczos_cluster_kernel(const ClusterLzParams p)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cl.sync();  // every CTA's barriers exist before a peer signals them
-    auto allreduce = [&](int count, double* out) { cluster_allreduce(x, part, count, xch, pm, out); };
     if constexpr (B > 0) {
         const int g_hi = k_hi > k_lo ? ((k_hi - 1) >> 5) + 1 : g_lo;
         const double* src = p.fac + (size_t)g_lo * (P * kInterleave);
@@ -229,10 +256,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
     double s = 0.0;
     for (int i = tid; i < nl; i += kClThreads) { const double x0 = p.v0[row_lo + i]; s = fma(x0, x0, s); }
     s = cl_cta_sum(s, red);
-    if (tid == 0) part[0] = s;
-    __syncthreads();
-    allreduce(1, c);
-    const double nrm = sqrt(c[0]);
+    const double nrm = sqrt(cluster_allreduce_scalar(x, s, xch, pm));
     if (!(nrm > 0.0) || isinf(nrm)) {  // zero or non-finite start vector: invalid argument (uniform over the cluster)
         if (rank == 0 && tid == 0) { p.done[0] = 1; p.done[2] = 1; }
         cl.sync();
@@ -246,11 +270,20 @@ lanczos_cluster_kernel(const ClusterLzParams p)
     }
     double beta_j = 0.0, amax = 0.0;
     __syncthreads();
+#ifdef BJ_CL_PROF
+    long long tk[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, t0 = clock64(), t1;
+#define BJ_TICK(k) do { t1 = clock64(); tk[k] += t1 - t0; t0 = t1; } while (0)
+#else
+#define BJ_TICK(k) do { } while (0)
+#endif
     for (int j = 0; j < p.m; ++j) {
         // ---- t = L^-T v_j on the own blocks, then to every CTA (the SpMV reads arbitrary columns) ----
         cluster_solve<B, 1>(n, k_lo, k_hi, g_lo, sf, vc, tl);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // tl is read by the async proxy (bulk copies)
         __syncthreads();
-        exchange_all(x, tl, nl, t_full, row_lo, n);
+        BJ_TICK(0);
+        exchange_all_bulk(x, tl, nl, t_full, row_lo, n);
+        BJ_TICK(1);
         // ---- u = A t (own rows, left to right: the oracle's order), w = L^-1 u ----
         if (p.row_in_regs) {
             if (tid < nl) {
@@ -271,6 +304,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
         __syncthreads();
         cluster_solve<B, 0>(n, k_lo, k_hi, g_lo, sf, u, w);
         __syncthreads();
+        BJ_TICK(2);
         // ---- w -= beta_j v_{j-1};  alpha_j = v_j . w;  w -= alpha_j v_j ----
         double pa = 0.0;
         for (int i = tid; i < nl; i += kClThreads) {
@@ -279,26 +313,30 @@ lanczos_cluster_kernel(const ClusterLzParams p)
             pa = fma(vc[i], wi, pa);
         }
         pa = cl_cta_sum(pa, red);
-        if (tid == 0) part[0] = pa;
-        __syncthreads();
-        allreduce(1, c);
-        const double a = c[0];
-        __syncthreads();  // c is rewritten by the reorthogonalisation
+        BJ_TICK(3);
+        const double a = cluster_allreduce_scalar(x, pa, xch, pm);
+        BJ_TICK(4);
         for (int i = tid; i < nl; i += kClThreads) w[i] -= a * vc[i];
         __syncthreads();
         // ---- full reorthogonalisation, classical Gram-Schmidt twice over v_1 .. v_j: c = V^T w, then w -= V c ----
         if (p.reorth) {
             const int nv = j + 1;
             // dots: thread = (vector q, row slice): consecutive lanes read consecutive vectors of one row of Vt
-            // (conflict-free), w[row] is a broadcast; no shuffles.  `cols` vectors per sweep (a power of two that covers nv,
-            // at most 64), kClThreads / cols row slices; the partials of a vector are added in slice order.
-            int cols = 8;
-            while (cols < nv && cols < 64) cols <<= 1;
-            const int slices = kClThreads / cols;
+            // (conflict-free), w[row] is a broadcast; no shuffles.  64 vectors per sweep, four row slices whose partials
+            // are added in slice order.  (Measured and dropped: narrower sweeps with more slices for few vectors, four
+            // accumulators with eight loads in flight, 512 threads -- all slower; the pass is a latency chain.)
+            constexpr int cols = kClDotCols, slices = kClThreads / kClDotCols;
             const int per = (nl + slices - 1) / slices;
             const int qc = tid & (cols - 1), sl = tid / cols;
             const int i0 = min(nl, sl * per), i1 = min(nl, i0 + per);
+            BJ_TICK(5);
             for (int pass = 0; pass < 2; ++pass) {
+                // the coefficient exchange is armed first; the thread that finishes a vector's CTA sum pushes it straight
+                // from its register into slot `rank` of the eight CTAs
+                double* xb = xch + (size_t)(x.e & 1) * kClusterSize * pm;
+                uint64_t* bar = x.bar + (x.e & 1);
+                const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
+                if (tid == 0) mbar_expect_tx(bar, (uint32_t)nv * 8u * kClusterSize);
                 for (int q0 = 0; q0 < nv; q0 += cols) {
                     const int q = q0 + qc;
                     double s0 = 0.0, s1 = 0.0;
@@ -311,34 +349,48 @@ lanczos_cluster_kernel(const ClusterLzParams p)
                         }
                         if (i < i1) s0 = fma(col[(size_t)i * p.ld], w[i], s0);
                     }
+                    if (q0 > 0) __syncthreads();  // dpart is reused by the next sweep (more than 64 vectors)
                     dpart[sl * cols + qc] = s0 + s1;
                     __syncthreads();
-                    if (tid < cols && q0 + tid < nv) {
+                    if (tid < cols && q < nv) {
                         double sq = dpart[tid];
+#pragma unroll
                         for (int r = 1; r < slices; ++r) sq += dpart[r * cols + tid];
-                        part[q0 + tid] = sq;
+                        const uint32_t dst = smem_u32(xb + rank * pm + q), bar_s = smem_u32(bar);
+#pragma unroll
+                        for (int r = 0; r < kClusterSize; ++r) st_async_f64(mapa_u32(dst, r), sq, mapa_u32(bar_s, r));
                     }
-                    __syncthreads();
                 }
-                allreduce(nv, c);
+                BJ_TICK(6);
+                mbar_wait(bar, parity);
+                ++x.e;
+                for (int q = tid; q < nv; q += kClThreads) {
+                    double sc = 0.0;
+#pragma unroll
+                    for (int r = 0; r < kClusterSize; ++r) sc += xb[r * pm + q];
+                    c[q] = sc;
+                }
+                __syncthreads();
+                BJ_TICK(7);
                 // w -= V c: thread per row, the row of Vt is contiguous; lanes are ld (odd) doubles apart: conflict-free
                 for (int i = tid; i < nl; i += kClThreads) {
                     const double* row = Vt + (size_t)i * p.ld;
                     double wi = w[i];
-                    for (int q = 0; q < nv; ++q) wi -= c[q] * row[q];  // subtraction order q = 0, 1, .. (the oracle's)
+                    int q = 0;
+                    for (; q < nv; ++q) wi -= c[q] * row[q];
                     w[i] = wi;
                 }
                 __syncthreads();
+                BJ_TICK(8);
             }
         }
         // ---- beta_{j+1} = ||w||, bookkeeping, breakdown test ----
         double pb = 0.0;
         for (int i = tid; i < nl; i += kClThreads) pb = fma(w[i], w[i], pb);
         pb = cl_cta_sum(pb, red);
-        if (tid == 0) part[0] = pb;
-        __syncthreads();
-        allreduce(1, c);
-        const double bn = sqrt(c[0]);
+        BJ_TICK(9);
+        const double bn = sqrt(cluster_allreduce_scalar(x, pb, xch, pm));
+        BJ_TICK(10);
         amax = fabs(a) > amax ? fabs(a) : amax;
         const bool brk = !(bn > p.tol * amax);
         if (rank == 0 && tid == 0) {
@@ -357,7 +409,14 @@ lanczos_cluster_kernel(const ClusterLzParams p)
         }
         beta_j = bn;
         __syncthreads();
+        BJ_TICK(11);
     }
+#ifdef BJ_CL_PROF
+    if (tid == 0 && rank == 0)
+        printf("solveT %lld xchT %lld spmv+solve %lld asum %lld axch %lld axpy %lld | dot %lld cxch %lld upd %lld | bsum %lld bxch %lld norm %lld (cycles/step)\n",
+               tk[0] / p.m, tk[1] / p.m, tk[2] / p.m, tk[3] / p.m, tk[4] / p.m, tk[5] / p.m, tk[6] / p.m, tk[7] / p.m, tk[8] / p.m, tk[9] / p.m,
+               tk[10] / p.m, tk[11] / p.m);
+#endif
     cl.sync();  // no CTA leaves while another may still address its shared memory
 }
 
@@ -376,7 +435,7 @@ ClusterGeom cluster_geometry(const bj_handle_s* h, int m, bool reorth)
     g.ld = m | 1;
     g.groups_max = h->solve_kind == 1 ? (g.bpc + kInterleave - 1) / kInterleave + 1 : 0;
     const size_t pm = (size_t)((m + 2) & ~1);
-    size_t d = kClWarps + kClThreads + 2 * pm + 2 * kClusterSize * pm + (((size_t)h->n + 1) & ~(size_t)1) + 5 * (size_t)g.nl_max +
+    size_t d = kClWarps + kClThreads + pm + 2 * kClusterSize * pm + (((size_t)h->n + 1) & ~(size_t)1) + 5 * (size_t)g.nl_max +
                (size_t)g.groups_max * h->packed * kInterleave;
     if (reorth) d += (size_t)g.nl_max * g.ld;
     g.smem = d * 8 + 16 + 16;
