@@ -151,7 +151,12 @@ multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const d
     if (done[0]) return;
     const Chunk c = my_chunk(n);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int q0 = 0; q0 < nv; q0 += kDotCols) {
+    // The sweeps run from the LAST eight columns to the first (each dot product is independent: same bits in any order):
+    // the kernel ends on the columns multiaxpy_kernel starts with, and starts on the ones it ended with in the previous
+    // pass: a few columns per kernel come out of L2 (parity mode, m = 50, config 2: 21.5 -> 21.25 ms).  Explicit L2 policies
+    // on top (keep the 2..6 boundary columns as ordinary lines, everything else evict_first) were measured and dropped:
+    // the hinted loads run the two kernels 25 % slower (26.2 ms).
+    for (int q0 = ((nv - 1) / kDotCols) * kDotCols; q0 >= 0; q0 -= kDotCols) {
         double s[kDotCols];
 #pragma unroll
         for (int d = 0; d < kDotCols; ++d) s[d] = 0.0;
@@ -196,51 +201,60 @@ multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const d
 // Same sweep structure as multidot_partial_kernel: eight columns at a time over the CTA's whole chunk of rows, so that every
 // column is read in one contiguous run per CTA (a first version walked all columns row by row: 50 interleaved 2 KB pieces per
 // CTA, 4.25 TB/s against the 6.3 TB/s of the dot kernel); the chunk of w waits in shared memory between the sweeps.
-constexpr int kAxpyRowsMax = 5888;  // rows of w a CTA holds at a time (46 KB of shared memory; longer chunks go piece by piece)
+constexpr int kAxpyRowsPerThread = 8;                               // rows of w a thread holds in registers at a time
+constexpr int kAxpyRowsMax = kAxpyRowsPerThread * kReduceThreads;   // rows of a piece (longer chunks go piece by piece)
 __global__ void __launch_bounds__(kReduceThreads)
 multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w,
                  const double* __restrict__ coef, double* __restrict__ PB, int want_norm,
                  const int* __restrict__ done, int piece)
 {
-    extern __shared__ double wsh[];
     __shared__ double sh[kReduceThreads / 32];
     pdl_trigger();
     pdl_wait();
     if (done[0]) return;
     const Chunk c = my_chunk(n);
     double s = 0.0;
-    for (int64_t lo = c.lo; lo < c.hi; lo += piece) {
-        const int rows = (int)(c.hi - lo < piece ? c.hi - lo : piece);
-        for (int r = threadIdx.x; r < rows; r += blockDim.x) wsh[r] = w[lo + r];  // a thread re-reads only what it wrote
+    for (int64_t lo = c.lo; lo < c.hi; lo += kAxpyRowsMax) {
+        // the thread's rows lo + tid + k * 256 of the piece wait in registers between the sweeps (a first version kept the
+        // piece in shared memory: one LDS + STS per row and sweep, 5.5 TB/s against the 6.3 TB/s of the dot kernel)
+        double wr[kAxpyRowsPerThread];
+        const int64_t base = lo + threadIdx.x;
+#pragma unroll
+        for (int k = 0; k < kAxpyRowsPerThread; ++k) wr[k] = base + k * kReduceThreads < c.hi ? w[base + k * kReduceThreads] : 0.0;
         for (int q0 = 0; q0 < nv; q0 += kDotCols) {
             const int live = nv - q0 < kDotCols ? nv - q0 : kDotCols;
             double cq[kDotCols];
 #pragma unroll
             for (int d = 0; d < kDotCols; ++d) cq[d] = d < live ? coef[q0 + d] : 0.0;
+            const double* Vq = V + (int64_t)q0 * n + base;
             if (live == kDotCols) {
-                for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-                    double vq[kDotCols];
 #pragma unroll
-                    for (int d = 0; d < kDotCols; ++d) vq[d] = V[(int64_t)(q0 + d) * n + lo + r];
-                    double wi = wsh[r];
+                for (int k = 0; k < kAxpyRowsPerThread; ++k) {
+                    if (base + k * kReduceThreads < c.hi) {
+                        double vq[kDotCols];
 #pragma unroll
-                    for (int d = 0; d < kDotCols; ++d) wi -= cq[d] * vq[d];
-                    wsh[r] = wi;
+                        for (int d = 0; d < kDotCols; ++d) vq[d] = Vq[(int64_t)d * n + k * kReduceThreads];
+#pragma unroll
+                        for (int d = 0; d < kDotCols; ++d) wr[k] -= cq[d] * vq[d];
+                    }
                 }
             } else {
-                for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-                    double wi = wsh[r];
 #pragma unroll
-                    for (int d = 0; d < kDotCols; ++d)
-                        if (d < live) wi -= cq[d] * V[(int64_t)(q0 + d) * n + lo + r];
-                    wsh[r] = wi;
+                for (int k = 0; k < kAxpyRowsPerThread; ++k) {
+                    if (base + k * kReduceThreads < c.hi) {
+#pragma unroll
+                        for (int d = 0; d < kDotCols; ++d)
+                            if (d < live) wr[k] -= cq[d] * Vq[(int64_t)d * n + k * kReduceThreads];
+                    }
                 }
             }
         }
-        for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-            const double wi = wsh[r];
-            w[lo + r] = wi;
-            s = fma(wi, wi, s);
+#pragma unroll
+        for (int k = 0; k < kAxpyRowsPerThread; ++k) {
+            if (base + k * kReduceThreads < c.hi) {
+                w[base + k * kReduceThreads] = wr[k];
+                s = fma(wr[k], wr[k], s);
+            }
         }
     }
     if (want_norm) {
@@ -420,7 +434,7 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>(kMaxPartials, (n + 1023) / 1024));
     const int64_t chunk_rows = (n + G - 1) / G;  // rows per CTA of the vector kernels (my_chunk)
     const int axpy_piece = (int)std::min<int64_t>(chunk_rows, kAxpyRowsMax);
-    const size_t axpy_smem = (size_t)axpy_piece * sizeof(double);
+    const size_t axpy_smem = 0;
 
     BJ_CUDA(cudaMemsetAsync(z.alpha, 0, sizeof(double) * (2 * (size_t)z.cap_iters + 8 + 2), st));  // alpha, beta, scal, done
 
