@@ -155,7 +155,9 @@ multidot_partial_kernel(int64_t n, int nv, const double* __restrict__ V, const d
     // the kernel ends on the columns multiaxpy_kernel starts with, and starts on the ones it ended with in the previous
     // pass: a few columns per kernel come out of L2 (parity mode, m = 50, config 2: 21.5 -> 21.25 ms).  Explicit L2 policies
     // on top (keep the 2..6 boundary columns as ordinary lines, everything else evict_first) were measured and dropped:
-    // the hinted loads run the two kernels 25 % slower (26.2 ms).
+    // the hinted loads run the two kernels 25 % slower (26.2 ms).  Also measured and dropped: alpha_j and w -= alpha_j v_j folded
+    // into the first sweep of the first pass (saves the axpy_norm_kernel launch, but w then needs coherent loads and a
+    // write-back inside the sweep: 20.9 -> 21.1 ms).
     for (int q0 = ((nv - 1) / kDotCols) * kDotCols; q0 >= 0; q0 -= kDotCols) {
         double s[kDotCols];
 #pragma unroll
