@@ -268,20 +268,33 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
 //   extraction : each lane binary-searches its (sorted) row for the first column >= kb and copies the
 //                entries up to the diagonal into its row of a small shared-memory tile;
 //   Cholesky   : right-looking in registers -- column j: l_jj = sqrt(a_jj) (broadcast from lane j),
-//                l_ij = a_ij / l_jj, then a_ik -= l_ij l_kj for k in (j, i] with l_kj fetched by shuffle.
-//                Updates hit a_ik in the order j = 0, 1, ..: the same subtraction order as the oracle's
-//                left-looking sum.  No shared memory, no barriers inside the factorisation.
+//                l_ij = a_ij / l_jj, then a_ik -= l_ij l_kj for k in (j, i] with column j passed between the
+//                lanes through shared memory (broadcast loads).  Updates hit a_ik in the order j = 0, 1, ..:
+//                the same subtraction order as the oracle's left-looking sum.
 //   output     : both scaled packed copies, written with consecutive lanes on consecutive addresses.
 // ------------------------------------------------------------------------------------------------
-template <int W>
-__global__ void __launch_bounds__(128)
+// a / l with r = RN(1 / l): one multiplication and one residual correction (Markstein) give the correctly rounded
+// quotient.  The library division takes its ~55-instruction slow path for the whole warp as soon as ONE lane divides a
+// zero or tiny numerator -- which a sparse block does in every column.
+__device__ __forceinline__ double div_by(double a, double l, double r)
+{
+    const double q = a * r;
+    return fma(fma(-l, q, a), r, q);
+}
+
+// BM: compile-time bound on the block size (b <= BM <= W): the unrolled loops of the factorisation run to BM with no
+// runtime guard -- rows and columns b .. BM-1 are identity padding (l = 1, zeros), whose arithmetic is harmless.
+// The factorisation is a dependent chain per column (shuffle, sqrt, reciprocal, store, barrier, loads, FMAs): resident warps
+// hide it, so registers are capped for 4 / 5 / 6 CTAs per SM (measured best per variant; a few spilled bytes cost less).
+template <int W, int BM>
+__global__ void __launch_bounds__(128, BM == 32 ? 4 : (BM == 24 ? 5 : 6))
 extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* __restrict__ rp,
                               const int32_t* __restrict__ ci, const double* __restrict__ val,
                               double* __restrict__ out0, double* __restrict__ out1, Status* st,
                               const int32_t* __restrict__ perm, const int32_t* __restrict__ pinv)  // both null: no permutation
 {
-    extern __shared__ double smem[];
-    constexpr int LD = W + 1;
+    extern __shared__ __align__(16) double smem[];
+    constexpr int LD = BM + 1;
     const int nsub = blockDim.x / W;
     const int sub = threadIdx.x / W;
     const int i = threadIdx.x & (W - 1);
@@ -294,8 +307,8 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
     const bool rowlive = i < b && row < n;
 
 #pragma unroll
-    for (int c = 0; c < W; ++c) D[i * LD + c] = 0.0;
-    if (!rowlive) D[i * LD + i] = 1.0;  // identity rows pad ragged blocks and idle lanes
+    for (int c = 0; c < BM; ++c) D[i * LD + c] = 0.0;
+    if (!rowlive && i < BM) D[i * LD + i] = 1.0;  // identity rows pad ragged blocks and idle lanes
     if (rowlive && perm) {
         // permuted handle: row lo + i of P A P^T is row perm[lo + i] of A; the whole row is scanned, columns through pinv
         const int ro = perm[row];
@@ -327,25 +340,36 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
         }
     }
     __syncwarp();
-    double a[W];
+    double a[BM];
 #pragma unroll
-    for (int c = 0; c < W; ++c) a[c] = D[i * LD + c];
+    for (int c = 0; c < BM; ++c) a[c] = D[i * LD + c];
 
+    // Column j of L goes from the lanes to the lanes through shared memory (the tile D is free while the rows sit in
+    // registers): every lane stores its l_ij, then all lanes read l_kj for k > j as BROADCAST 128-bit loads, two k per
+    // instruction.  A shuffle per (j, k) pair -- b^2 / 2 64-bit shuffles = 1024 SHFL per 32 x 32 block -- made the kernel
+    // shuffle-bound.  Two column buffers alternate: one __syncwarp per column.  The update a_ik -= l_ij l_kj runs on every
+    // lane for every k > j: entries above the diagonal (k > i) collect garbage that nothing reads.
+    __syncwarp();  // every lane has its row of D in registers
+    const double2* Lc2 = reinterpret_cast<const double2*>(D);  // [2][W / 2]
     bool bad = false;
+    double inv = 1.0;  // 1 / l_ii of this lane's row
 #pragma unroll
-    for (int j = 0; j < W; ++j) {
-        if (j < b) {
-            double ajj = __shfl_sync(0xffffffffu, a[j], j, W);
-            if (!(ajj > 0.0) || isinf(ajj)) { bad = true; ajj = 1.0; }
-            const double ljj = sqrt(ajj);
-            const double lij = (i > j) ? a[j] / ljj : (i == j ? ljj : 0.0);
-            a[j] = lij;
+    for (int j = 0; j < BM; ++j) {
+        double ajj = __shfl_sync(0xffffffffu, a[j], j, W);
+        if (!(ajj > 0.0) || isinf(ajj)) { bad = true; ajj = 1.0; }
+        const double ljj = sqrt(ajj);
+        const double rjj = __drcp_rn(ljj);
+        const double lij = (i > j) ? div_by(a[j], ljj, rjj) : (i == j ? ljj : 0.0);
+        if (i == j) inv = rjj;
+        a[j] = lij;
+        if (j + 1 < BM) {
+            D[(j & 1) * W + i] = lij;
+            __syncwarp();
 #pragma unroll
-            for (int k2 = j + 1; k2 < W; ++k2) {
-                if (k2 < b) {
-                    const double lkj = __shfl_sync(0xffffffffu, lij, k2, W);
-                    if (i >= k2) a[k2] = fma(-lij, lkj, a[k2]);
-                }
+            for (int pp = (j + 1) / 2; pp < BM / 2; ++pp) {
+                const double2 t = Lc2[(j & 1) * (W / 2) + pp];
+                if (2 * pp > j) a[2 * pp] = fma(-lij, t.x, a[2 * pp]);
+                a[2 * pp + 1] = fma(-lij, t.y, a[2 * pp + 1]);
             }
         }
     }
@@ -353,20 +377,26 @@ extract_factor_subwarp_kernel(int64_t n, int b, int64_t nblocks, const int32_t* 
         atomicOr(&st->flags, ST_NOT_SPD);
         atomicMin(&st->bad_block, (long long)k);
     }
-    __syncwarp();
-#pragma unroll
-    for (int c = 0; c < W; ++c) D[i * LD + c] = a[c];
-    __syncwarp();
-    if (!act) return;
     const int P = b * (b + 1) / 2;
-    const double inv = 1.0 / D[i * LD + i];  // one division per lane; the scalings below multiply by it
-    // forward copy: column-major packed, row i scaled by 1/l_ii
-    for (int j = 0; j < b; ++j)
-        if (i >= j && i < b) out0[k * P + (j * b - j * (j - 1) / 2) + (i - j)] = (i == j) ? inv : D[i * LD + j] * inv;
-    // backward copy: row-major packed, column i scaled by 1/l_ii (not kept when the solves use the forward copy for both)
-    if (out1)
-        for (int r = 0; r < b; ++r)
-            if (i <= r) out1[k * P + r * (r + 1) / 2 + i] = (i == r) ? inv : D[r * LD + i] * inv;
+    // forward copy straight from the registers: column-major packed, row i scaled by 1 / l_ii, consecutive lanes on
+    // consecutive addresses
+    if (act && i < b) {
+        double* o = out0 + k * P;
+#pragma unroll
+        for (int j = 0; j < BM; ++j)
+            if (j < b && i >= j) o[(j * b - j * (j - 1) / 2) + (i - j)] = (i == j) ? inv : a[j] * inv;
+    }
+    // backward copy: row-major packed, column i scaled by 1 / l_ii (not kept when the solves use the forward copy for both):
+    // through the tile, read transposed
+    if (out1) {
+        __syncwarp();  // the column buffers in D are dead
+#pragma unroll
+        for (int c = 0; c < BM; ++c) D[i * LD + c] = a[c];
+        __syncwarp();
+        if (act)
+            for (int r = 0; r < b; ++r)
+                if (i <= r) out1[k * P + r * (r + 1) / 2 + i] = (i == r) ? inv : D[r * LD + i] * inv;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -446,17 +476,17 @@ int launch_extract_factor(bj_handle_s* h)
 #undef BJ_CASE
     } else {
         const int W = h->lanes;
+        const int BM = W == 16 ? 16 : (b <= 24 ? 24 : 32);  // compile-time loop bound of the factorisation
         const int nsub = 128 / W;
-        const size_t sm = (size_t)nsub * W * (W + 1) * sizeof(double);
+        const size_t sm = (size_t)nsub * W * (BM + 1) * sizeof(double);
         const unsigned sb = (unsigned)((h->nblocks + nsub - 1) / nsub);
-        if (W == 16)
-            extract_factor_subwarp_kernel<16><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
-                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status,
-                                                                          h->var_perm, h->var_pinv);
-        else
-            extract_factor_subwarp_kernel<32><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx,
-                                                                          h->val, h->fac_fwd, h->fac_bwd, h->status,
-                                                                          h->var_perm, h->var_pinv);
+#define BJ_SUBWARP(WW, BB)                                                                                             \
+    extract_factor_subwarp_kernel<WW, BB><<<sb, 128, sm, h->stream>>>(h->n, b, h->nblocks, h->row_ptr, h->col_idx, h->val, \
+                                                                      h->fac_fwd, h->fac_bwd, h->status, h->var_perm, h->var_pinv)
+        if (BM == 16) BJ_SUBWARP(16, 16);
+        else if (BM == 24) BJ_SUBWARP(32, 24);
+        else BJ_SUBWARP(32, 32);
+#undef BJ_SUBWARP
     }
     h->launches++;
     BJ_CUDA(cudaGetLastError());
