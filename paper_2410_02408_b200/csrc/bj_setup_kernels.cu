@@ -150,6 +150,15 @@ int launch_spmv_plan(bj_handle_s* h, int tile_rows)
 // contiguous range (L1 absorbs the per-thread strides) and its interleaved factor writes are whole
 // 256-byte lines.  Same left-looking Cholesky order as above.
 // ------------------------------------------------------------------------------------------------
+// a / l with r = RN(1 / l): one multiplication and one residual correction (Markstein) give the correctly rounded
+// quotient.  The library division takes its ~55-instruction slow path for the whole warp as soon as ONE lane divides a
+// zero or tiny numerator -- which a sparse block does in every column.
+__device__ __forceinline__ double div_by(double a, double l, double r)
+{
+    const double q = a * r;
+    return fma(fma(-l, q, a), r, q);
+}
+
 template <int B>
 __global__ void __launch_bounds__(128)
 extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restrict__ rp,
@@ -217,6 +226,7 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
     }
     }
     bool bad = false;
+    double rinv[B];
     // every loop has the constant trip count B (triangular bounds as predicates): all of them unroll, d[] stays in registers
 #pragma unroll
     for (int j = 0; j < B; ++j) {
@@ -226,6 +236,8 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
             if (p < j) sjj -= d[j * (j + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
         if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
         const double ljj = sqrt(sjj);
+        const double rjj = __drcp_rn(ljj);  // also the stored diagonal slot 1 / l_jj
+        rinv[j] = rjj;
         d[j * (j + 1) / 2 + j] = ljj;
 #pragma unroll
         for (int i = 0; i < B; ++i) {
@@ -234,7 +246,7 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
 #pragma unroll
                 for (int p = 0; p < B; ++p)
                     if (p < j) t -= d[i * (i + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
-                d[i * (i + 1) / 2 + j] = t / ljj;
+                d[i * (i + 1) / 2 + j] = div_by(t, ljj, rjj);  // (the library division: ~55 instructions whenever a lane's t is 0)
             }
         }
     }
@@ -249,7 +261,7 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
 #pragma unroll
         for (int i = 0; i < B; ++i) {
             if (i > 0) f[(2 * i - 1) * kInterleave] = d[i * (i + 1) / 2 + i - 1];
-            f[(2 * i) * kInterleave] = 1.0 / d[i * (i + 1) / 2 + i];
+            f[(2 * i) * kInterleave] = rinv[i];
         }
         return;
     }
@@ -259,7 +271,7 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
 #pragma unroll
         for (int j = 0; j <= i; ++j) {
             const double v = d[i * (i + 1) / 2 + j];
-            f[(i * (i + 1) / 2 + j) * kInterleave] = (i == j) ? 1.0 / v : v;
+            f[(i * (i + 1) / 2 + j) * kInterleave] = (i == j) ? rinv[i] : v;
         }
 }
 
@@ -273,15 +285,6 @@ extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restric
 //                the same subtraction order as the oracle's left-looking sum.
 //   output     : both scaled packed copies, written with consecutive lanes on consecutive addresses.
 // ------------------------------------------------------------------------------------------------
-// a / l with r = RN(1 / l): one multiplication and one residual correction (Markstein) give the correctly rounded
-// quotient.  The library division takes its ~55-instruction slow path for the whole warp as soon as ONE lane divides a
-// zero or tiny numerator -- which a sparse block does in every column.
-__device__ __forceinline__ double div_by(double a, double l, double r)
-{
-    const double q = a * r;
-    return fma(fma(-l, q, a), r, q);
-}
-
 // BM: compile-time bound on the block size (b <= BM <= W): the unrolled loops of the factorisation run to BM with no
 // runtime guard -- rows and columns b .. BM-1 are identity padding (l = 1, zeros), whose arithmetic is harmless.
 // The factorisation is a dependent chain per column (shuffle, sqrt, reciprocal, store, barrier, loads, FMAs): resident warps
