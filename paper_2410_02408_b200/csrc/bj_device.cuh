@@ -52,6 +52,15 @@ __device__ __forceinline__ int ld_stream(const int* p)
     return v;
 }
 
+// a / l with r = RN(1 / l): one multiplication and one residual correction (Markstein) give the correctly rounded
+// quotient.  The library division takes its ~55-instruction slow path for the whole warp as soon as ONE lane divides a
+// zero or tiny numerator -- which a sparse block does in every column.
+__device__ __forceinline__ double div_by(double a, double l, double r)
+{
+    const double q = a * r;
+    return fma(fma(-l, q, a), r, q);
+}
+
 // 256-bit / 128-bit vector accesses (LDG.E.256 / STG.E.256 on sm_100); pointers must be 32 / 16 byte aligned
 __device__ __forceinline__ void ld_v4(const double* p, double* v)
 {

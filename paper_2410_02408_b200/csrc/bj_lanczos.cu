@@ -83,7 +83,8 @@ scale_kernel(int64_t n, const double* __restrict__ in, double* __restrict__ out,
     }
     if (!out) return;
     const Chunk c = my_chunk(n);
-    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) out[i] = in[i] / bn;
+    const double rb = __drcp_rn(bn);  // in / bn as one multiplication and a residual correction (div_by): the correctly rounded quotient
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += blockDim.x) out[i] = div_by(in[i], bn, rb);
 }
 
 // w -= beta_j v_{j-1} (j > 0);  PA[cta] = partial of v_j . w

@@ -5,6 +5,7 @@
 // shared memory, factors it there and writes the layouts the solve kernels want.
 #include <algorithm>
 
+#include "bj_device.cuh"
 #include "bj_internal.cuh"
 
 namespace bj {
@@ -150,15 +151,6 @@ int launch_spmv_plan(bj_handle_s* h, int tile_rows)
 // contiguous range (L1 absorbs the per-thread strides) and its interleaved factor writes are whole
 // 256-byte lines.  Same left-looking Cholesky order as above.
 // ------------------------------------------------------------------------------------------------
-// a / l with r = RN(1 / l): one multiplication and one residual correction (Markstein) give the correctly rounded
-// quotient.  The library division takes its ~55-instruction slow path for the whole warp as soon as ONE lane divides a
-// zero or tiny numerator -- which a sparse block does in every column.
-__device__ __forceinline__ double div_by(double a, double l, double r)
-{
-    const double q = a * r;
-    return fma(fma(-l, q, a), r, q);
-}
-
 template <int B>
 __global__ void __launch_bounds__(128)
 extract_factor_small_kernel(int64_t n, int64_t nblocks, const int32_t* __restrict__ rp,
