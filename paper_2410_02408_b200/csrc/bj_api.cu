@@ -594,10 +594,13 @@ int bj_cond_estimate(bj_handle_t h, int iters, double* lmin, double* lmax)
     memset(&o, 0, sizeof(o));
     o.iters = iters;
     o.seed = BJ_DEFAULT_SEED;
-    size_t free_b = 0, total_b = 0;
-    BJ_CUDA(cudaMemGetInfo(&free_b, &total_b));
-    const double need = ((double)iters + 2.0) * (double)h->n * 8.0;
-    o.reorth = (h->lz.cap_vectors >= iters || need < 0.8 * (double)free_b) ? 1 : 0;
+    o.reorth = 1;
+    if (h->lz.cap_vectors < iters) {  // the basis is not there yet: full reorthogonalisation only if it fits (the query costs ~50 us)
+        size_t free_b = 0, total_b = 0;
+        BJ_CUDA(cudaMemGetInfo(&free_b, &total_b));
+        const double need = ((double)iters + 2.0) * (double)h->n * 8.0;
+        o.reorth = need < 0.8 * (double)free_b ? 1 : 0;
+    }
     bj_lanczos_result_t r;
     memset(&r, 0, sizeof(r));
     int rc = lanczos_run(h, &o, &r);
