@@ -147,8 +147,8 @@ enum {
     BJ_OPT_LANCZOS_FUSE = 3,  /* 0: fast-mode Lanczos runs the unfused vector kernels; 1 / -1: the fused step (default) */
     BJ_OPT_PCG_FUSE = 4,      /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
     BJ_OPT_LANCZOS_SINGLE_LAUNCH = 5 /* 0: launch-bound sizes (vectors + factors fit one CTA's shared memory, b <= 8) keep the
-                                 multi-launch Lanczos; 1 / -1 (default): the whole run is ONE kernel -- of one eight-CTA
-                                 cluster with the basis distributed over their shared memory when a CTA's share fits,
+                                 multi-launch Lanczos; 1 / -1 (default): the whole run is ONE kernel -- of one cluster of 8
+                                 (or 16) CTAs with the basis distributed over their shared memory when a CTA's share fits,
                                  else of one CTA; 2: always the single-CTA form                                         */
 };
 
@@ -240,7 +240,8 @@ int bj_cond_estimate_minv(bj_handle_t h, const bj_lanczos_opts_t* opts_host, bj_
  * of fixed size, 147 488 bytes, which every GPU that loads the library holds until the process exits.  The call makes no
  * cudaMalloc / cudaFree / pool call and no allocating library call.
  * Limits: n <= BJ_NOALLOC_MAX_N, iters <= BJ_NOALLOC_MAX_ITERS, uniform blocks b <= 8 or b = 0 without permutation
- * or band storage, and a CTA's share of the basis must fit its shared memory (8 CTAs; n (iters | 1) + ... <= 220 KB each);
+ * or band storage, and a CTA's share of the basis must fit its shared memory (a cluster of 8 CTAs, or of 16 when the rows fit registers:
+ * N = 1024 and N = 4096 at iters = 50 do, N = 16384 does not);
  * anything beyond returns BJ_ERR_LIMIT and does nothing.  The handle comes from bj_setup as usual (setup does allocate).
  * Every call on a device shares the array, which keeps the previous call's contents (the call clears what must start at
  * zero): calls that OVERLAP on the GPU -- two handles on two streams of one device -- race on it; serialise them.

@@ -139,6 +139,7 @@ struct bj_handle_s {
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;
     int opt_lanczos_fuse = -1;  // BJ_OPT_LANCZOS_FUSE / BJ_OPT_PCG_FUSE: 0 selects the unfused iterations
+    int cl_m = -1, cl_reorth = -1, cl_cs = 0;  // last answer of the cluster-size choice of bj_lanczos_cluster.cu
     int opt_lanczos_small = -1; // BJ_OPT_LANCZOS_SINGLE_LAUNCH: 0 keeps launch-bound sizes on the multi-launch path
     int opt_pcg_fuse = -1;
     bj_setup_opts_t opts = {};  // the options this handle was set up with
@@ -267,7 +268,7 @@ int launch_seeded_vector(bj_handle_s* h, uint64_t seed, double* v);
 double tridiag_eig_k(int m, const double* a, const double* e, int k);
 void lanczos_fill_result(int me, const double* a, const double* b, bj_lanczos_result_t* res);
 // the whole run as one kernel of one eight-CTA cluster, the basis distributed over their shared memory (bj_lanczos_cluster.cu)
-bool lanczos_cluster_usable(const bj_handle_s* h, int m, bool reorth);
+bool lanczos_cluster_usable(bj_handle_s* h, int m, bool reorth);
 int launch_lanczos_cluster(bj_handle_s* h, int m, bool reorth, double tol, const double* v0, double* alpha, double* beta, int* done);
 // the whole run as one single-CTA kernel for launch-bound sizes (bj_lanczos_small.cu)
 bool lanczos_small_usable(const bj_handle_s* h, int m);

@@ -462,10 +462,11 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         if (rc != BJ_OK) return rc;
         v0 = z.w;
     }
-    if (h->opt_lanczos_small != 0 && lanczos_small_usable(h, m)) {
+    const bool cluster_ok = h->opt_lanczos_small != 0 && h->opt_lanczos_small != 2 && lanczos_cluster_usable(h, m, reorth);
+    if (h->opt_lanczos_small != 0 && (cluster_ok || lanczos_small_usable(h, m))) {
         // launch-bound sizes: the whole run is ONE single-CTA kernel (bj_lanczos_small.cu)
         // (option value 2 keeps the single-CTA form; by default the eight-CTA cluster form runs when a CTA's share of the basis fits)
-        if (h->opt_lanczos_small != 2 && lanczos_cluster_usable(h, m, reorth))
+        if (cluster_ok)
             rc = launch_lanczos_cluster(h, m, reorth, tol, v0, z.alpha, z.beta, z.done);
         else
             rc = launch_lanczos_small(h, m, reorth, tol, v0, z.V, z.alpha, z.beta, z.done);

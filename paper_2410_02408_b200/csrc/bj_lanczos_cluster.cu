@@ -1,5 +1,5 @@
 // Launch-bound sizes, second form: the whole m-step Lanczos run of bj_lanczos.cu as ONE kernel of ONE thread-block CLUSTER
-// of eight CTAs (bj_lanczos_small.cu runs it on one CTA: its reorthogonalisation re-reads the basis four times per step and
+// of eight CTAs -- sixteen when eight cannot hold the basis (N = 4096 at m = 50) -- (bj_lanczos_small.cu runs it on one CTA: its reorthogonalisation re-reads the basis four times per step and
 // only ~20 basis vectors of N = 1024 fit beside the work vectors, the rest comes through one SM's L2 port: 17 us per step).
 // Here CTA r owns a contiguous range of diagonal blocks and their rows; its slice of EVERY basis vector stays in its
 // shared memory (8 x 200 KB for the basis), the operator's block solves and all vector updates are local, and the CTAs
@@ -29,7 +29,7 @@ namespace bj {
 
 namespace {
 
-constexpr int kClusterSize = 8;
+constexpr int kClusterMax = 16;  // eight CTAs (portable) or sixteen (opt-in: one GPC of a B200 holds them)
 constexpr int kClThreads = 256;
 constexpr int kClWarps = kClThreads / 32;
 constexpr int kClRowReg = 8;   // a thread keeps its row's entries in registers when no row is longer
@@ -99,14 +99,15 @@ __device__ __forceinline__ void st_async_f64(uint32_t raddr, double v, uint32_t 
 
 // every CTA sends src[0..count) to dst_base[dst_off + 0..count) of EVERY CTA (itself included) and waits until the eight
 // contributions (total_doubles in all) have arrived in its own copy
+template <int CS>
 __device__ __forceinline__ void exchange_all(Exchange& x, const double* src, int count, double* dst_base, int dst_off, int total_doubles)
 {
     uint64_t* bar = x.bar + (x.e & 1);
     const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
     if (threadIdx.x == 0) mbar_expect_tx(bar, (uint32_t)total_doubles * 8u);
     const uint32_t bar_s = smem_u32(bar), dst_s = smem_u32(dst_base + dst_off);
-    for (int e = threadIdx.x; e < count * kClusterSize; e += kClThreads) {
-        const int dst = e & (kClusterSize - 1), q = e >> 3;
+    for (int e = threadIdx.x; e < count * CS; e += kClThreads) {
+        const int dst = e % CS, q = e / CS;
         st_async_f64(mapa_u32(dst_s + 8u * (uint32_t)q, dst), src[q], mapa_u32(bar_s, dst));
     }
     mbar_wait(bar, parity);
@@ -117,13 +118,14 @@ __device__ __forceinline__ void exchange_all(Exchange& x, const double* src, int
 // count st.async per peer (1240 -> ~500 cycles for 128 rows), when the slice is 16-byte aligned and sized; the caller
 // has made src visible to the async proxy (fence.proxy.async before its __syncthreads).  src is not rewritten before
 // every peer has passed the next exchange, i.e. long after the copies have read it.
+template <int CS>
 __device__ __forceinline__ void exchange_all_bulk(Exchange& x, const double* src, int count, double* dst_base, int dst_off, int total_doubles)
 {
-    if (((count | dst_off) & 1) != 0) return exchange_all(x, src, count, dst_base, dst_off, total_doubles);
+    if (((count | dst_off) & 1) != 0) return exchange_all<CS>(x, src, count, dst_base, dst_off, total_doubles);
     uint64_t* bar = x.bar + (x.e & 1);
     const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
     if (threadIdx.x == 0) mbar_expect_tx(bar, (uint32_t)total_doubles * 8u);
-    if (threadIdx.x < kClusterSize && count > 0) {
+    if (threadIdx.x < CS && count > 0) {
         const uint32_t dst = mapa_u32(smem_u32(dst_base + dst_off), threadIdx.x), rbar = mapa_u32(smem_u32(bar), threadIdx.x);
         asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                      "r"(smem_u32(src)), "r"((uint32_t)count * 8u), "r"(rbar)
@@ -137,19 +139,20 @@ __device__ __forceinline__ void exchange_all_bulk(Exchange& x, const double* src
 // the register to the eight CTAs, every thread adds the eight slots itself -- no staging store, no __syncthreads.
 // (The callers' next exchange is always behind a __syncthreads, so no thread still reads this buffer when a peer
 // refills it two exchanges later.)
+template <int CS>
 __device__ __forceinline__ double cluster_allreduce_scalar(Exchange& x, double v, double* xch2, int pm)
 {
-    double* xch = xch2 + (size_t)(x.e & 1) * kClusterSize * pm;
+    double* xch = xch2 + (size_t)(x.e & 1) * CS * pm;
     uint64_t* bar = x.bar + (x.e & 1);
     const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
-    if (threadIdx.x == 0) mbar_expect_tx(bar, 8u * kClusterSize);
-    if (threadIdx.x < kClusterSize)
+    if (threadIdx.x == 0) mbar_expect_tx(bar, 8u * CS);
+    if (threadIdx.x < CS)
         st_async_f64(mapa_u32(smem_u32(xch + x.rank * pm), threadIdx.x), v, mapa_u32(smem_u32(bar), threadIdx.x));
     mbar_wait(bar, parity);
     ++x.e;
     double s = 0.0;
 #pragma unroll
-    for (int r = 0; r < kClusterSize; ++r) s += xch[r * pm];
+    for (int r = 0; r < CS; ++r) s += xch[r * pm];
     return s;
 }
 
@@ -195,9 +198,9 @@ __device__ __forceinline__ void cluster_solve(int n, int k_lo, int k_hi, int g_l
     }
 }
 
-template <int B>
-__global__ void __cluster_dims__(kClusterSize, 1, 1) __launch_bounds__(kClThreads)
-lanczos_cluster_kernel(const ClusterLzParams p)
+template <int B, int CS>
+__global__ void __launch_bounds__(kClThreads)
+lanczos_cluster_kernel(const ClusterLzParams p)  // launched as clusters of CS CTAs (launch attribute)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cg::cluster_group cl = cg::this_cluster();
@@ -216,7 +219,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
     double* dpart = red + kClWarps;                     // (slice, vector) partials of a dot sweep
     double* c = dpart + kClThreads;
     double* xch = c + pm;
-    double* t_full = xch + 2 * kClusterSize * pm;
+    double* t_full = xch + 2 * CS * pm;
     double* tl = t_full + ((n + 1) & ~1);
     double* u = tl + p.nl_max;
     double* w = u + p.nl_max;
@@ -256,7 +259,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
     double s = 0.0;
     for (int i = tid; i < nl; i += kClThreads) { const double x0 = p.v0[row_lo + i]; s = fma(x0, x0, s); }
     s = cl_cta_sum(s, red);
-    const double nrm = sqrt(cluster_allreduce_scalar(x, s, xch, pm));
+    const double nrm = sqrt(cluster_allreduce_scalar<CS>(x, s, xch, pm));
     if (!(nrm > 0.0) || isinf(nrm)) {  // zero or non-finite start vector: invalid argument (uniform over the cluster)
         if (rank == 0 && tid == 0) { p.done[0] = 1; p.done[2] = 1; }
         cl.sync();
@@ -282,7 +285,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // tl is read by the async proxy (bulk copies)
         __syncthreads();
         BJ_TICK(0);
-        exchange_all_bulk(x, tl, nl, t_full, row_lo, n);
+        exchange_all_bulk<CS>(x, tl, nl, t_full, row_lo, n);
         BJ_TICK(1);
         // ---- u = A t (own rows, left to right: the oracle's order), w = L^-1 u ----
         if (p.row_in_regs) {
@@ -314,7 +317,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
         }
         pa = cl_cta_sum(pa, red);
         BJ_TICK(3);
-        const double a = cluster_allreduce_scalar(x, pa, xch, pm);
+        const double a = cluster_allreduce_scalar<CS>(x, pa, xch, pm);
         BJ_TICK(4);
         for (int i = tid; i < nl; i += kClThreads) w[i] -= a * vc[i];
         __syncthreads();
@@ -333,10 +336,10 @@ lanczos_cluster_kernel(const ClusterLzParams p)
             for (int pass = 0; pass < 2; ++pass) {
                 // the coefficient exchange is armed first; the thread that finishes a vector's CTA sum pushes it straight
                 // from its register into slot `rank` of the eight CTAs
-                double* xb = xch + (size_t)(x.e & 1) * kClusterSize * pm;
+                double* xb = xch + (size_t)(x.e & 1) * CS * pm;
                 uint64_t* bar = x.bar + (x.e & 1);
                 const uint32_t parity = (uint32_t)((x.e >> 1) & 1);
-                if (tid == 0) mbar_expect_tx(bar, (uint32_t)nv * 8u * kClusterSize);
+                if (tid == 0) mbar_expect_tx(bar, (uint32_t)nv * 8u * CS);
                 for (int q0 = 0; q0 < nv; q0 += cols) {
                     const int q = q0 + qc;
                     double s0 = 0.0, s1 = 0.0;
@@ -358,7 +361,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
                         for (int r = 1; r < slices; ++r) sq += dpart[r * cols + tid];
                         const uint32_t dst = smem_u32(xb + rank * pm + q), bar_s = smem_u32(bar);
 #pragma unroll
-                        for (int r = 0; r < kClusterSize; ++r) st_async_f64(mapa_u32(dst, r), sq, mapa_u32(bar_s, r));
+                        for (int r = 0; r < CS; ++r) st_async_f64(mapa_u32(dst, r), sq, mapa_u32(bar_s, r));
                     }
                 }
                 BJ_TICK(6);
@@ -367,7 +370,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
                 for (int q = tid; q < nv; q += kClThreads) {
                     double sc = 0.0;
 #pragma unroll
-                    for (int r = 0; r < kClusterSize; ++r) sc += xb[r * pm + q];
+                    for (int r = 0; r < CS; ++r) sc += xb[r * pm + q];
                     c[q] = sc;
                 }
                 __syncthreads();
@@ -389,7 +392,7 @@ lanczos_cluster_kernel(const ClusterLzParams p)
         for (int i = tid; i < nl; i += kClThreads) pb = fma(w[i], w[i], pb);
         pb = cl_cta_sum(pb, red);
         BJ_TICK(9);
-        const double bn = sqrt(cluster_allreduce_scalar(x, pb, xch, pm));
+        const double bn = sqrt(cluster_allreduce_scalar<CS>(x, pb, xch, pm));
         BJ_TICK(10);
         amax = fabs(a) > amax ? fabs(a) : amax;
         const bool brk = !(bn > p.tol * amax);
@@ -425,39 +428,109 @@ struct ClusterGeom {
     size_t smem;
 };
 
-ClusterGeom cluster_geometry(const bj_handle_s* h, int m, bool reorth)
+ClusterGeom cluster_geometry(const bj_handle_s* h, int m, bool reorth, int cs)
 {
     ClusterGeom g;
     const int bb = h->solve_kind == 1 ? h->b : 1;
     const int64_t units = h->solve_kind == 1 ? h->nblocks : h->n;
-    g.bpc = (int)((units + kClusterSize - 1) / kClusterSize);
+    g.bpc = (int)((units + cs - 1) / cs);
     g.nl_max = g.bpc * bb;
     g.ld = m | 1;
     g.groups_max = h->solve_kind == 1 ? (g.bpc + kInterleave - 1) / kInterleave + 1 : 0;
     const size_t pm = (size_t)((m + 2) & ~1);
-    size_t d = kClWarps + kClThreads + pm + 2 * kClusterSize * pm + (((size_t)h->n + 1) & ~(size_t)1) + 5 * (size_t)g.nl_max +
+    size_t d = kClWarps + kClThreads + pm + 2 * (size_t)cs * pm + (((size_t)h->n + 1) & ~(size_t)1) + 5 * (size_t)g.nl_max +
                (size_t)g.groups_max * h->packed * kInterleave;
     if (reorth) d += (size_t)g.nl_max * g.ld;
     g.smem = d * 8 + 16 + 16;
     return g;
 }
 
+template <int B, int CS>
+cudaError_t cluster_prepare(size_t smem, int* max_clusters)
+{
+    static std::atomic<bool> configured[64];
+    cudaError_t e = ensure_big_smem(lanczos_cluster_kernel<B, CS>, configured);
+    if (e == cudaSuccess && CS > 8) e = cudaFuncSetAttribute(lanczos_cluster_kernel<B, CS>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess || !max_clusters) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(CS);
+    cfg.blockDim = dim3(kClThreads);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CS;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaOccupancyMaxActiveClusters(max_clusters, lanczos_cluster_kernel<B, CS>, &cfg);
+}
+
+template <int B, int CS>
+cudaError_t cluster_launch(const ClusterLzParams& p, size_t smem, cudaStream_t st)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(CS);
+    cfg.blockDim = dim3(kClThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CS;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, lanczos_cluster_kernel<B, CS>, p);
+}
+
+// which cluster size serves (h, m, reorth): 8 when a CTA's share fits its shared memory, else 16 (opt-in size: half the
+// share per CTA) when that fits and the device can place such a cluster, else 0.  The answer is kept in the handle.
+int cluster_pick(bj_handle_s* h, int m, bool reorth)
+{
+    if (env_int("BJ_LANCZOS_CLUSTER", 1) == 0) return 0;
+    if (h->var_perm || !(h->solve_kind == 0 || (h->solve_kind == 1 && !h->tri)) || m > 1024 || h->n > 16384 || h->n < kClusterMax ||
+        h->nnz == 0)
+        return 0;
+    if (h->cl_m == m && h->cl_reorth == (reorth ? 1 : 0)) return h->cl_cs;
+    int cs = 0;
+    constexpr size_t kBudget = 220 * 1024;
+    if (cluster_geometry(h, m, reorth, 8).smem <= kBudget) {
+        cs = 8;
+    } else if (cluster_geometry(h, m, reorth, 16).smem <= kBudget && cluster_geometry(h, m, reorth, 16).nl_max <= kClThreads &&
+               h->max_row_nnz <= kClRowReg && env_int("BJ_LANCZOS_CLUSTER16", 1) != 0) {
+        // (only with the CTA's rows of the matrix in registers: N = 16384 without them measured 0.82 ms for 50 steps
+        // against 0.67 ms on the multi-launch path)
+        const size_t smem = cluster_geometry(h, m, reorth, 16).smem;
+        int nc = 0;
+        cudaError_t e = cudaSuccess;
+#define BJ_CASE(B) case B: e = cluster_prepare<B, 16>(smem, &nc); break;
+        switch (h->solve_kind == 1 ? h->b : 0) {
+            BJ_CASE(0) BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
+            default: break;
+        }
+#undef BJ_CASE
+        if (e != cudaSuccess) cudaGetLastError();  // the device cannot place it: not an error of the call
+        cs = (e == cudaSuccess && nc >= 1) ? 16 : 0;
+    }
+    h->cl_m = m;
+    h->cl_reorth = reorth ? 1 : 0;
+    h->cl_cs = cs;
+    return cs;
+}
+
 }  // namespace
 
 // The cluster form is used when a CTA's share of the basis fits its shared memory beside the work vectors (N = 1024, m = 50:
-// 52 KB of basis per CTA); otherwise the single-CTA kernel (basis through L2) or the multi-launch path run.
-bool lanczos_cluster_usable(const bj_handle_s* h, int m, bool reorth)
-{
-    if (env_int("BJ_LANCZOS_CLUSTER", 1) == 0) return false;
-    if (h->var_perm || !(h->solve_kind == 0 || (h->solve_kind == 1 && !h->tri)) || m > 1024 || h->n > 16384 || h->n < kClusterSize ||
-        h->nnz == 0)
-        return false;
-    return cluster_geometry(h, m, reorth).smem <= 220 * 1024;
-}
+// 52 KB of basis per CTA of an eight-CTA cluster; N = 4096: 104 KB per CTA of a sixteen-CTA cluster); otherwise the
+// single-CTA kernel (basis through L2) or the multi-launch path run.
+bool lanczos_cluster_usable(bj_handle_s* h, int m, bool reorth) { return cluster_pick(h, m, reorth) != 0; }
 
 int launch_lanczos_cluster(bj_handle_s* h, int m, bool reorth, double tol, const double* v0, double* alpha, double* beta, int* done)
 {
-    const ClusterGeom g = cluster_geometry(h, m, reorth);
+    const int cs = cluster_pick(h, m, reorth);
+    if (cs == 0) return BJ_ERR_INVALID_ARG;
+    const ClusterGeom g = cluster_geometry(h, m, reorth, cs);
     ClusterLzParams p;
     p.n = (int)h->n; p.nnz = (int)h->nnz; p.nblocks = (int)h->nblocks; p.m = m;
     p.reorth = reorth ? 1 : 0;
@@ -468,13 +541,16 @@ int launch_lanczos_cluster(bj_handle_s* h, int m, bool reorth, double tol, const
     p.fac = h->solve_kind == 1 ? h->fac_small : nullptr;
     p.v0 = v0; p.alpha = alpha; p.beta = beta; p.done = done;
     cudaError_t e = cudaSuccess;
-#define BJ_CASE(B)                                                                                              \
-    case B: {                                                                                                   \
-        static std::atomic<bool> configured[64];                                                                \
-        e = ensure_big_smem(lanczos_cluster_kernel<B>, configured);                                             \
-        if (e == cudaSuccess) lanczos_cluster_kernel<B><<<kClusterSize, kClThreads, g.smem, h->stream>>>(p);    \
-        break;                                                                                                  \
-    }
+#define BJ_CASE(B)                                                                                  \
+    case B:                                                                                         \
+        if (cs == 8) {                                                                              \
+            e = cluster_prepare<B, 8>(g.smem, nullptr);                                             \
+            if (e == cudaSuccess) e = cluster_launch<B, 8>(p, g.smem, h->stream);                   \
+        } else {                                                                                    \
+            e = cluster_prepare<B, 16>(g.smem, nullptr);                                            \
+            if (e == cudaSuccess) e = cluster_launch<B, 16>(p, g.smem, h->stream);                  \
+        }                                                                                           \
+        break;
     switch (h->solve_kind == 1 ? h->b : 0) {
         BJ_CASE(0) BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
         default: return BJ_ERR_INVALID_ARG;
@@ -482,7 +558,6 @@ int launch_lanczos_cluster(bj_handle_s* h, int m, bool reorth, double tol, const
 #undef BJ_CASE
     if (e != cudaSuccess) { set_cuda_error(e, "lanczos_cluster_kernel"); return BJ_ERR_CUDA; }
     h->launches++;
-    BJ_CUDA(cudaGetLastError());
     return BJ_OK;
 }
 

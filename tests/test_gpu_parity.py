@@ -241,6 +241,29 @@ def test_single_launch_lanczos_for_launch_bound_sizes(B, torch_):
         B.bj_destroy(h)
 
 
+def test_single_launch_lanczos_on_the_papers_larger_sizes(B, torch_):
+    """N = 2^12: a sixteen-CTA cluster holds what an eight-CTA one cannot -- the basis of N = 4096 at m = 50
+    with full reorthogonalisation.  N = 2^14 stays on the multi-launch path (checked against the oracle all the same).
+    Same bar as everywhere: kappa to 1e-6, alpha / beta against the oracle."""
+    for grid, b, reorth in ((64, 4, True), (64, 8, True), (64, 0, False), (64, 3, False), (128, 4, False), (128, 4, True)):
+        A = W.config1(grid)
+        h, keep = B.setup_from_host(A, b)
+        l0 = B.bj_get_info(h)["kernel_launches"]
+        g = B.bj_cond_estimate_ex(h, 50, reorth=reorth)
+        if grid == 64:
+            assert B.bj_get_info(h)["kernel_launches"] - l0 <= 2, (grid, b, reorth)  # seeded vector + the one kernel
+        c = oracle.Precond(A, b).cond_estimate(50, reorth=reorth)
+        assert g["iters_done"] == c["iters_done"]
+        scale = abs(c["alpha"]).max()
+        assert np.abs(g["alpha"] - c["alpha"]).max() <= 1e-8 * scale and np.abs(g["beta"] - c["beta"]).max() <= 1e-7 * scale
+        if reorth:
+            assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (grid, b, g["kappa"], c["kappa"])
+        B.bj_set_option(h, B.BJ_OPT_LANCZOS_SINGLE_LAUNCH, 0)                        # the multi-launch path agrees
+        gm = B.bj_cond_estimate_ex(h, 50, reorth=reorth)
+        assert np.abs(gm["alpha"] - g["alpha"]).max() <= 1e-8 * scale
+        B.bj_destroy(h)
+
+
 def test_point_jacobi_is_the_papers_kernel(B, torch_):
     """PAPER.md:234: M[idx] = 1/A[idx*N+idx]."""
     A = mat(1, "full")
