@@ -146,6 +146,8 @@ enum {
     BJ_OPT_FUSE_FORWARD = 2,  /* 0: three kernels, 1: fuse forward solve into SpMV, -1 = automatic    */
     BJ_OPT_LANCZOS_FUSE = 3,  /* 0: fast-mode Lanczos runs the unfused vector kernels; 1 / -1: the fused step (default) */
     BJ_OPT_PCG_FUSE = 4,      /* 0: PCG / M^-1 A Lanczos run the unfused iteration; 1 / -1: the fused one (default)     */
+    BJ_OPT_PCG_SINGLE_LAUNCH = 6, /* 0: launch-bound sizes keep the multi-launch PCG iteration; 1 / -1 (default): bj_pcg_solve runs as ONE
+                                 kernel of one cluster of 8 (or 16) CTAs when the vectors fit their shared memory (b <= 8 or 0) */
     BJ_OPT_LANCZOS_SINGLE_LAUNCH = 5 /* 0: launch-bound sizes (vectors + factors fit one CTA's shared memory, b <= 8) keep the
                                  multi-launch Lanczos; 1 / -1 (default): the whole run is ONE kernel -- of one cluster of 8
                                  (or 16) CTAs with the basis distributed over their shared memory when a CTA's share fits,

@@ -19,6 +19,7 @@ BJ_ERR_LIMIT = -7
 BJ_NOALLOC_MAX_N, BJ_NOALLOC_MAX_ITERS = 16384, 1024
 BJ_K_SOLVE_LT, BJ_K_SPMV, BJ_K_SOLVE_L, BJ_K_APPLY, BJ_K_SPMV_SOLVE_L, BJ_K_COUNT = 0, 1, 2, 3, 4, 5
 BJ_OPT_SPMV_KERNEL, BJ_OPT_FUSE_FORWARD, BJ_OPT_LANCZOS_FUSE, BJ_OPT_PCG_FUSE, BJ_OPT_LANCZOS_SINGLE_LAUNCH = 1, 2, 3, 4, 5
+BJ_OPT_PCG_SINGLE_LAUNCH = 6
 KERNEL_KIND_NAMES = ["solve_Lt", "spmv", "solve_L", "apply", "spmv_solve_L"]
 
 EXPORTS = ["bj_setup", "bj_setup_on_stream", "bj_setup_ex", "bj_get_setup_time", "bj_set_stream", "bj_set_option", "bj_destroy", "bj_get_info",

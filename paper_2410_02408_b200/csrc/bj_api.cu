@@ -485,6 +485,10 @@ int bj_set_option(bj_handle_t h, int option, int value)
             if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
             h->opt_pcg_fuse = value;
             return BJ_OK;
+        case BJ_OPT_PCG_SINGLE_LAUNCH:
+            if (value < -1 || value > 1) return BJ_ERR_INVALID_ARG;
+            h->opt_pcg_small = value;
+            return BJ_OK;
         case BJ_OPT_LANCZOS_SINGLE_LAUNCH:
             if (value < -1 || value > 2) return BJ_ERR_INVALID_ARG;
             h->opt_lanczos_small = value;

@@ -139,6 +139,8 @@ struct bj_handle_s {
     int opt_spmv_kernel = -1; // user override
     int opt_fuse = -1;
     int opt_lanczos_fuse = -1;  // BJ_OPT_LANCZOS_FUSE / BJ_OPT_PCG_FUSE: 0 selects the unfused iterations
+    int pcg_cl_cs = -1;  // cluster size of the single-launch PCG (bj_pcg_cluster.cu): -1 not asked yet, 0 not usable
+    int opt_pcg_small = -1;  // BJ_OPT_PCG_SINGLE_LAUNCH: 0 keeps launch-bound sizes on the multi-launch iteration
     int cl_m = -1, cl_reorth = -1, cl_cs = 0;  // last answer of the cluster-size choice of bj_lanczos_cluster.cu
     int opt_lanczos_small = -1; // BJ_OPT_LANCZOS_SINGLE_LAUNCH: 0 keeps launch-bound sizes on the multi-launch path
     int opt_pcg_fuse = -1;
@@ -285,6 +287,10 @@ int perm_install(bj_handle_s* h, const int32_t* perm_dev);  // handle-owned copi
 void perm_free(bj_handle_s* h);
 int launch_solve_var(bj_handle_s* h, int dir, const double* in, double* out);
 int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, bj_pcg_result_t* r);
+// the whole run as one kernel of one cluster for launch-bound sizes (bj_pcg_cluster.cu)
+bool pcg_cluster_usable(bj_handle_s* h);
+int launch_pcg_cluster(bj_handle_s* h, const double* b, double* x, int m, double rtol, double* alpha, double* beta, double* relres,
+                       double* scal, double* pd, int* flags);
 void pcg_free(bj_handle_s* h);
 void batch_free(bj_handle_s* h);
 

@@ -12,6 +12,8 @@
 // extreme Ritz values of M^-1 A from the CG coefficients (CG-Lanczos equivalence).
 #include <math.h>
 
+#include <string.h>
+
 #include <algorithm>
 #include <cmath>
 #include <vector>
@@ -319,12 +321,21 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
         return launch_spmv(h, in, out);
     };
 
+    // launch-bound sizes: the whole run is ONE kernel of one cluster (bj_pcg_cluster.cu)
+    const bool single = h->opt_pcg_small != 0 && pcg_cluster_usable(h);
+    int G_read = G;  // partials of ||A x - b||^2 to add on the host
+    if (single) {
+        rc = launch_pcg_cluster(h, b, x, m, rtol, alpha, beta, relres, scal, PD, flags);
+        if (rc != BJ_OK) return rc;
+        G_read = 1;
+    }
+    int hflags[4] = {0, 0, 0, 0};
+    if (!single) {
     BJ_LAUNCH(pcg_init_kernel, n, b, r, x, P0);
     rc = launch_solve(h, 2, r, z);  // z = M^-1 r  (b = 0: copy)
     if (rc != BJ_OK) return rc;
     BJ_LAUNCH(pcg_start_kernel, n, (const double*)r, (const double*)z, p, (const double*)P0, G, scal, PRa, flags);
 
-    int hflags[4] = {0, 0, 0, 0};
     // Fused iteration (bj_pcg_fuse.cuh): needs the tile SpMV (dot hook) and a solve kernel that carries the PCG hook
     const bool fused = h->spmv_kernel == 1 && lanczos_fusable(h) && h->opt_pcg_fuse != 0;
     if (fused) {
@@ -381,24 +392,26 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
     rc = spmv(x, q);
     if (rc != BJ_OK) return rc;
     BJ_LAUNCH(pcg_residual_kernel, n, (const double*)q, b, PD);
+    }  // !single
 #undef BJ_LAUNCH
 
-    std::vector<double> ha(m), hb(m), hr(m), hpd(G);
+    // alpha | beta | relres | flags are one block of the workspace: one copy (a copy costs ~10 us of host time)
+    const size_t cap = (size_t)h->pcg_cap_iters;
+    std::vector<double> hblk(3 * cap + 8), hpd(G_read);
     double hscal[S_COUNT];
-    BJ_CUDA(cudaMemcpyAsync(ha.data(), alpha, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaMemcpyAsync(hb.data(), beta, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaMemcpyAsync(hr.data(), relres, sizeof(double) * m, cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaMemcpyAsync(hpd.data(), PD, sizeof(double) * G, cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hblk.data(), alpha, sizeof(double) * hblk.size(), cudaMemcpyDeviceToHost, st));
+    BJ_CUDA(cudaMemcpyAsync(hpd.data(), PD, sizeof(double) * G_read, cudaMemcpyDeviceToHost, st));
     BJ_CUDA(cudaMemcpyAsync(hscal, scal, sizeof(hscal), cudaMemcpyDeviceToHost, st));
-    BJ_CUDA(cudaMemcpyAsync(hflags, flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
     BJ_CUDA(cudaStreamSynchronize(st));
+    const double *ha = hblk.data(), *hb = hblk.data() + cap, *hr = hblk.data() + 2 * cap;
+    memcpy(hflags, hblk.data() + 3 * cap, sizeof(hflags));
 
     const int it = hflags[1];
     res->iters = it;
     res->converged = hflags[2];
     res->relres = it > 0 ? hr[it - 1] : 0.0;
     double dd = 0.0;
-    for (int g = 0; g < G; ++g) dd += hpd[g];
+    for (int g = 0; g < G_read; ++g) dd += hpd[g];
     res->true_relres = hscal[S_BB] > 0.0 ? sqrt(dd / hscal[S_BB]) : 0.0;
     res->lmin = res->lmax = 0.0;
     // CG-Lanczos: T = tridiag(e; d) with d_0 = 1/a_0, d_j = 1/a_j + bt_{j-1}/a_{j-1}, e_j = sqrt(bt_j)/a_j
@@ -411,9 +424,9 @@ int pcg_run(bj_handle_s* h, const double* b, double* x, const bj_pcg_opts_t* o, 
         res->lmin = tridiag_eig_k(kt, d.data(), off.data(), 0);
         res->lmax = tridiag_eig_k(kt, d.data(), off.data(), kt - 1);
     }
-    if (res->alpha_host) std::copy(ha.begin(), ha.begin() + it, res->alpha_host);
-    if (res->beta_host) std::copy(hb.begin(), hb.begin() + std::max(nb, 0), res->beta_host);
-    if (res->relres_host) std::copy(hr.begin(), hr.begin() + it, res->relres_host);
+    if (res->alpha_host) std::copy(ha, ha + it, res->alpha_host);
+    if (res->beta_host) std::copy(hb, hb + std::max(nb, 0), res->beta_host);
+    if (res->relres_host) std::copy(hr, hr + it, res->relres_host);
     return BJ_OK;
 }
 

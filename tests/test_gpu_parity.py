@@ -850,6 +850,50 @@ def test_pcg_fused_and_unfused_iterations_agree(B, torch_, rel, fuse):
         B.bj_destroy(h)
 
 
+def test_pcg_single_launch_on_the_papers_sizes(B, torch_, rel):
+    """N = 2^10 and 2^12: bj_pcg_solve runs as ONE kernel of one cluster (8 / 16 CTAs).  Against the oracle's
+    textbook PCG and against the multi-launch iteration on the same handle: coefficients, residual history, x, the paper's
+    residual; zero right-hand side; exact preconditioner; ragged last block."""
+    import scipy.sparse as sp
+    for A, blocks in ((W.config1(32), (0, 1, 4, 7, 8)), (W.config1(64), (4, 8)), (W.laplacian((37, 29)), (5,))):
+        S = sp.csr_matrix((A.val, A.col_idx, A.row_ptr), shape=(A.n, A.n))
+        rhs = W.seeded_vector(23, A.n)
+        rd = dev(torch_, rhs)
+        for b in blocks:
+            h, keep = B.setup_from_host(A, b)
+            P = oracle.Precond(A, b)
+            l0 = B.bj_get_info(h)["kernel_launches"]
+            g = B.bj_pcg_solve(h, rd, max_iters=10, rtol=0.0)
+            assert B.bj_get_info(h)["kernel_launches"] - l0 == 1, (A.n, b)
+            c = P.pcg(rhs, 10, 0.0)
+            assert g["iters"] == c["iters"] == 10 and not g["converged"]
+            assert np.allclose(g["alpha"], c["alpha"], rtol=1e-9, atol=0) and np.allclose(g["beta"], c["beta"], rtol=1e-9, atol=0)
+            assert np.allclose(g["relres_hist"], c["relres"], rtol=1e-9, atol=0)
+            xg = g["x"].cpu().numpy()
+            e2, ei = rel(xg, c["x"])
+            assert e2 <= 1e-10 and ei <= 1e-9, (A.n, b, e2, ei)
+            tr = np.linalg.norm(S @ xg - rhs) / np.linalg.norm(rhs)
+            assert abs(g["true_relres"] - tr) <= 1e-10 * tr
+            g = B.bj_pcg_solve(h, rd, max_iters=400, rtol=1e-8)
+            c = P.pcg(rhs, 400, 1e-8)
+            assert g["converged"] and abs(g["iters"] - c["iters"]) <= 1 and g["true_relres"] <= 2e-8, (A.n, b, g["iters"], c["iters"])
+            B.bj_set_option(h, B.BJ_OPT_PCG_SINGLE_LAUNCH, 0)      # the multi-launch iteration on the same handle
+            l0 = B.bj_get_info(h)["kernel_launches"]
+            gm = B.bj_pcg_solve(h, rd, max_iters=400, rtol=1e-8)
+            assert B.bj_get_info(h)["kernel_launches"] - l0 > 20
+            assert gm["iters"] == g["iters"] and rel(g["x"].cpu().numpy(), gm["x"].cpu().numpy())[0] <= 1e-10
+            B.bj_set_option(h, B.BJ_OPT_PCG_SINGLE_LAUNCH, 1)
+            z = B.bj_pcg_solve(h, torch_.zeros_like(rd), max_iters=5, rtol=1e-3)
+            assert z["iters"] == 0 and float(z["x"].abs().max()) == 0.0
+            B.bj_destroy(h)
+    A = W.block_diagonal_spd(100, 8)          # M = A: one step
+    h, keep = B.setup_from_host(A, 8)
+    rhs = W.seeded_vector(5, A.n)
+    g = B.bj_pcg_solve(h, dev(torch_, rhs), max_iters=20, rtol=1e-10)
+    assert g["iters"] == 1 and g["converged"] and g["true_relres"] <= 1e-12
+    B.bj_destroy(h)
+
+
 def test_pcg_degenerate_cases(B, torch_, rel):
     A = W.block_diagonal_spd(65, 8)     # M = A: one step (PAPER.md:80)
     h, keep = B.setup_from_host(A, 8)
