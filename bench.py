@@ -520,6 +520,17 @@ def other_configs(B, torch, args, local: int, peak: float, peak_src: str) -> dic
             lz["oracle_parity_mode"] = {"seconds": float(np.median(ts)), "kappa_est": c["kappa"], "cores": oracle.num_threads()}
             lz["iters"] = m
             r["lanczos"] = lz
+            # the solve-stage stand-in on the paper's size: PCG to the paper's bar, one launch of one cluster
+            rhs = B.bj_seeded_vector(h, 17)
+            B.bj_pcg_solve(h, rhs, max_iters=200, rtol=1e-3)
+            ts = []
+            for _ in range(5):
+                torch.cuda.synchronize()
+                t1 = time.perf_counter()
+                pr = B.bj_pcg_solve(h, rhs, max_iters=200, rtol=1e-3)
+                ts.append(time.perf_counter() - t1)
+            r["pcg"] = {"rtol": 1e-3, "seconds": float(np.median(ts)), "iters": int(pr["iters"]), "converged": bool(pr["converged"]),
+                        "true_relres": float(pr["true_relres"])}
         r["section_seconds"] = time.perf_counter() - t0
         B.bj_destroy(h)
         del h
