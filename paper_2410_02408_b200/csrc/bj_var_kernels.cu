@@ -61,9 +61,11 @@ extract_factor_var_kernel(int64_t nblocks, const int32_t* __restrict__ bptr, con
         const double piv = __shfl_sync(0xffffffffu, sum, j);
         if (!(piv > 0.0) || !isfinite(piv)) { bad = true; break; }  // uniform over the warp
         const double d = sqrt(piv);
+        const double rd = __drcp_rn(d);  // sum / d below = one multiplication + a residual correction (div_by): the library
+                                         // division takes its slow path for the whole warp whenever one lane's sum is 0
         __syncwarp();
         if (lane == j) D[lane * (kVarMax + 1) + j] = d;
-        else if (lane > j && lane < s) D[lane * (kVarMax + 1) + j] = sum / d;
+        else if (lane > j && lane < s) D[lane * (kVarMax + 1) + j] = div_by(sum, d, rd);
         __syncwarp();
     }
     if (bad) {
