@@ -12,6 +12,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <atomic>
 
 #include "bj_device.cuh"
 #include "bj_internal.cuh"
@@ -266,6 +267,112 @@ multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __rest
     }
 }
 
+// Reorthogonalisation, middle of a step: w -= V c (the first pass' update) AND the second pass' dot products c2 = V^T w in
+// ONE pass over the basis.  Four kernels per step read V four times (dot, axpy, dot, axpy: 4 x 16.8 MB x j on config 2);
+// the update of one pass and the dots of the next need the same tile of V and nothing global in between, so a persistent
+// CTA brings a tile of R rows of every column into shared memory ONCE (one bulk async copy per column and stage, two
+// stages: ~100 KB in flight per SM), updates its rows of w (thread per row, subtraction order q = 0, 1, ..: the oracle's),
+// writes them back, and adds the tile's contribution to its running c2 (warp per column, fixed order).  Three reads of V
+// per step instead of four.  Partials: partial[cta * stride + q], closed by finalize_multi_kernel as before.
+constexpr int kFuseThreads = 512;
+constexpr int kFuseWarps = kFuseThreads / 32;
+constexpr int kFuseSlots = 13;                 // columns per warp at most: nv <= kFuseWarps * kFuseSlots = 208
+constexpr int kFuseStageBytes = 100 * 1024;
+__global__ void __launch_bounds__(kFuseThreads, 1)
+reorth_axpy_dot_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w, const double* __restrict__ coef,
+                       double* __restrict__ partial, int stride, const int* __restrict__ done, int R, int64_t ntiles)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);            // [2]
+    double* cs = reinterpret_cast<double*>(smem_raw + 64);              // coefficients of the update, nv (<= 208)
+    double* w1 = cs + 208;                                              // the tile's updated rows, R (<= 512)
+    double* stage0 = w1 + 512;                                          // [2][(nv + 1) * R]: columns 0..nv-1, then w
+    const size_t stage_doubles = (size_t)(nv + 1) * R;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    pdl_trigger();
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    pdl_wait();  // w and the coefficients come from the previous kernels
+    if (done[0]) return;
+    for (int q = tid; q < nv; q += kFuseThreads) cs[q] = coef[q];
+    // a full tile (R rows) arrives by bulk copies; the ragged last tile is read with ordinary loads
+    auto issue = [&](int64_t tile, int s) {  // warp 0
+        const int64_t r0 = tile * R;
+        if (r0 + R > n) return;
+        double* dst = stage0 + (size_t)s * stage_doubles;
+        const uint32_t bytes = (uint32_t)R * 8u;
+        if (lane == 0) mbar_expect_tx(&full[s], bytes * (uint32_t)(nv + 1));
+        __syncwarp();
+        const uint64_t pol = policy_evict_first();
+        for (int q = lane; q <= nv; q += 32)
+            bulk_g2s(dst + (size_t)q * R, q < nv ? V + (int64_t)q * n + r0 : w + r0, bytes, &full[s], pol);
+    };
+    double acc[kFuseSlots];
+#pragma unroll
+    for (int k = 0; k < kFuseSlots; ++k) acc[k] = 0.0;
+    if (warp == 0) {
+        issue(blockIdx.x, 0);
+        if ((int64_t)blockIdx.x + gridDim.x < ntiles) issue((int64_t)blockIdx.x + gridDim.x, 1);
+    }
+    __syncthreads();  // cs is complete
+    int it = 0;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+        const int s = it & 1;
+        const int64_t r0 = tile * R;
+        const int rows = (int)(r0 + R <= n ? R : n - r0);
+        double* Vs = stage0 + (size_t)s * stage_doubles;
+        if (rows == R) {
+            mbar_wait(&full[s], (uint32_t)((it >> 1) & 1));
+        } else {
+            for (int e = tid; e < (nv + 1) * rows; e += kFuseThreads) {
+                const int q = e / rows, r = e - q * rows;
+                Vs[(size_t)q * R + r] = q < nv ? V[(int64_t)q * n + r0 + r] : w[r0 + r];
+            }
+            __syncthreads();
+        }
+        // ---- w -= V c on the tile's rows (thread per row) ----
+        if (tid < rows) {
+            double wi = Vs[(size_t)nv * R + tid];
+            for (int q = 0; q < nv; ++q) wi -= cs[q] * Vs[(size_t)q * R + tid];
+            w1[tid] = wi;
+            w[r0 + tid] = wi;
+        }
+        __syncthreads();
+        // ---- c2 += V^T w1 over the tile (warp per column, lanes stride the rows, fixed shuffle tree) ----
+#pragma unroll
+        for (int k = 0; k < kFuseSlots; ++k) {
+            const int q = warp + k * kFuseWarps;
+            if (q < nv) {
+                const double* col = Vs + (size_t)q * R;
+                double s0 = 0.0, s1 = 0.0;
+                int r = lane;
+                for (; r + 32 < rows; r += 64) {
+                    s0 = fma(col[r], w1[r], s0);
+                    s1 = fma(col[r + 32], w1[r + 32], s1);
+                }
+                if (r < rows) s0 = fma(col[r], w1[r], s0);
+                double sq = s0 + s1;
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) sq += __shfl_down_sync(0xffffffffu, sq, off);
+                acc[k] += sq;  // (meaningful on lane 0)
+            }
+        }
+        __syncthreads();  // the stage and w1 are free
+        if (warp == 0 && tile + 2 * (int64_t)gridDim.x < ntiles) issue(tile + 2 * (int64_t)gridDim.x, s);
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < kFuseSlots; ++k) {
+            const int q = warp + k * kFuseWarps;
+            if (q < nv) partial[(int64_t)blockIdx.x * stride + q] = acc[k];
+        }
+    }
+}
+
 // out[q] = sum_cta partial[cta * stride + q]: one CTA per coefficient (a single CTA for all of them took 39 us at 50 vectors,
 // one tenth of a parity-mode step).  Thread t adds the partials of CTAs t, t + 256, .. in that order, then the fixed block
 // tree: bitwise reproducible.
@@ -438,6 +545,11 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     const int64_t chunk_rows = (n + G - 1) / G;  // rows per CTA of the vector kernels (my_chunk)
     const int axpy_piece = (int)std::min<int64_t>(chunk_rows, kAxpyRowsMax);
     const size_t axpy_smem = 0;
+    bool fuse_reorth = reorth && env_int("BJ_REORTH_FUSE", 1) != 0;
+    if (fuse_reorth) {
+        static std::atomic<bool> configured[64];
+        if (ensure_big_smem(reorth_axpy_dot_kernel, configured) != cudaSuccess) { cudaGetLastError(); fuse_reorth = false; }
+    }
 
     BJ_CUDA(cudaMemsetAsync(z.alpha, 0, sizeof(double) * (2 * (size_t)z.cap_iters + 8 + 2), st));  // alpha, beta, scal, done
 
@@ -517,12 +629,33 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         BJ_LAUNCH(axpy_norm_kernel, G, kReduceThreads, n, z.w, (const double*)vj, (const double*)PA, G, j, z.alpha,
                   PB, reorth ? 0 : 1, (const int*)z.done);
         if (reorth) {
+            const int nv = j + 1;
+            // the first pass' update and the second pass' dots in one pass over V (reorth_axpy_dot_kernel) when a tile of
+            // at least 64 rows of all nv columns fits a stage and the arrays are 16-byte aligned for the bulk copies
+            int R = (int)((kFuseStageBytes / ((size_t)(nv + 1) * 8)) & ~(size_t)31);
+            if (R > 512) R = 512;
+            const bool fuse_mid = fuse_reorth && R >= 64 && nv <= kFuseWarps * kFuseSlots && n % 2 == 0 &&
+                                  ((uintptr_t)z.V % 16) == 0 && ((uintptr_t)z.w % 16) == 0;
             for (int pass = 0; pass < 2; ++pass) {
-                BJ_LAUNCH(multidot_partial_kernel, G, kReduceThreads, n, j + 1, (const double*)z.V,
-                          (const double*)z.w, PM, stride, (const int*)z.done);
-                BJ_LAUNCH(finalize_multi_kernel, j + 1, 256, G, j + 1, (const double*)PM, stride, z.coef,
-                          (const int*)z.done);
-                e = launch_kernel(multiaxpy_kernel, dim3(G), dim3(kReduceThreads), axpy_smem, st, pdl, n, j + 1,
+                if (pass == 0 || !fuse_mid) {
+                    BJ_LAUNCH(multidot_partial_kernel, G, kReduceThreads, n, nv, (const double*)z.V,
+                              (const double*)z.w, PM, stride, (const int*)z.done);
+                    BJ_LAUNCH(finalize_multi_kernel, nv, 256, G, nv, (const double*)PM, stride, z.coef,
+                              (const int*)z.done);
+                }
+                if (pass == 0 && fuse_mid) {
+                    const int64_t ntiles = (n + R - 1) / R;
+                    const int grid = (int)std::min<int64_t>(ntiles, h->num_sms);
+                    const size_t smem = 64 + (208 + 512) * sizeof(double) + 2 * (size_t)(nv + 1) * R * sizeof(double);
+                    e = launch_kernel(reorth_axpy_dot_kernel, dim3(grid), dim3(kFuseThreads), smem, st, pdl, n, nv,
+                                      (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done, R, ntiles);
+                    if (e != cudaSuccess) { set_cuda_error(e, "reorth_axpy_dot_kernel"); return BJ_ERR_CUDA; }
+                    h->launches++;
+                    BJ_LAUNCH(finalize_multi_kernel, nv, 256, grid, nv, (const double*)PM, stride, z.coef,
+                              (const int*)z.done);
+                    continue;
+                }
+                e = launch_kernel(multiaxpy_kernel, dim3(G), dim3(kReduceThreads), axpy_smem, st, pdl, n, nv,
                                   (const double*)z.V, z.w, (const double*)z.coef, PB, pass == 1 ? 1 : 0, (const int*)z.done,
                                   axpy_piece);
                 if (e != cudaSuccess) { set_cuda_error(e, "multiaxpy_kernel"); return BJ_ERR_CUDA; }
