@@ -271,28 +271,32 @@ multiaxpy_kernel(int64_t n, int nv, const double* __restrict__ V, double* __rest
 // ONE pass over the basis.  Four kernels per step read V four times (dot, axpy, dot, axpy: 4 x 16.8 MB x j on config 2);
 // the update of one pass and the dots of the next need the same tile of V and nothing global in between, so a persistent
 // CTA brings a tile of R rows of every column into shared memory ONCE (one bulk async copy per column and stage, two
-// stages: ~100 KB in flight per SM), updates its rows of w (thread per row, subtraction order q = 0, 1, ..: the oracle's),
+// stages of 100 KB), updates its rows of w (thread per row, subtraction order q = 0, 1, ..: the oracle's),
 // writes them back, and adds the tile's contribution to its running c2 (warp per column, fixed order).  Three reads of V
 // per step instead of four.  Partials: partial[cta * stride + q], closed by finalize_multi_kernel as before.
 constexpr int kFuseThreads = 512;
+constexpr int kFuseCtasPerSm = 1;
 constexpr int kFuseWarps = kFuseThreads / 32;
-constexpr int kFuseSlots = 13;                 // columns per warp at most: nv <= kFuseWarps * kFuseSlots = 208
+constexpr int kFuseSlots = 208 / kFuseWarps;   // columns per warp at most: nv <= 208
+constexpr int kFuseStages = 2;                 // measured on config 2, m = 50 (BJ_REORTH_STAGES / BJ_REORTH_STAGE_KB): 2 x 100 KB 19.4 ms,
+                                               // 3 x 66 KB 21.4, 4 x 50 KB 23.4, two 256-thread CTAs per SM 22.3: a tile costs ~1 us
+                                               // whatever its height (barriers, the nv-step update chain, the shuffle trees), so
+                                               // tall tiles win although two stages keep only one tile in flight
 constexpr int kFuseStageBytes = 100 * 1024;
-__global__ void __launch_bounds__(kFuseThreads, 1)
+__global__ void __launch_bounds__(kFuseThreads, kFuseCtasPerSm)
 reorth_axpy_dot_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w, const double* __restrict__ coef,
-                       double* __restrict__ partial, int stride, const int* __restrict__ done, int R, int64_t ntiles)
+                       double* __restrict__ partial, int stride, const int* __restrict__ done, int R, int64_t ntiles, int S)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);            // [2]
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);            // [kFuseStages]
     double* cs = reinterpret_cast<double*>(smem_raw + 64);              // coefficients of the update, nv (<= 208)
     double* w1 = cs + 208;                                              // the tile's updated rows, R (<= 512)
-    double* stage0 = w1 + 512;                                          // [2][(nv + 1) * R]: columns 0..nv-1, then w
+    double* stage0 = w1 + 512;                                          // [kFuseStages][(nv + 1) * R]: columns 0..nv-1, then w
     const size_t stage_doubles = (size_t)(nv + 1) * R;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     pdl_trigger();
     if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
+        for (int q = 0; q < S; ++q) mbar_init(&full[q], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -315,18 +319,18 @@ reorth_axpy_dot_kernel(int64_t n, int nv, const double* __restrict__ V, double* 
 #pragma unroll
     for (int k = 0; k < kFuseSlots; ++k) acc[k] = 0.0;
     if (warp == 0) {
-        issue(blockIdx.x, 0);
-        if ((int64_t)blockIdx.x + gridDim.x < ntiles) issue((int64_t)blockIdx.x + gridDim.x, 1);
+        for (int q = 0; q < S; ++q)
+            if ((int64_t)blockIdx.x + (int64_t)q * gridDim.x < ntiles) issue((int64_t)blockIdx.x + (int64_t)q * gridDim.x, q);
     }
     __syncthreads();  // cs is complete
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-        const int s = it & 1;
+        const int s = it % S;
         const int64_t r0 = tile * R;
         const int rows = (int)(r0 + R <= n ? R : n - r0);
         double* Vs = stage0 + (size_t)s * stage_doubles;
         if (rows == R) {
-            mbar_wait(&full[s], (uint32_t)((it >> 1) & 1));
+            mbar_wait(&full[s], (uint32_t)((it / S) & 1));
         } else {
             for (int e = tid; e < (nv + 1) * rows; e += kFuseThreads) {
                 const int q = e / rows, r = e - q * rows;
@@ -362,7 +366,7 @@ reorth_axpy_dot_kernel(int64_t n, int nv, const double* __restrict__ V, double* 
             }
         }
         __syncthreads();  // the stage and w1 are free
-        if (warp == 0 && tile + 2 * (int64_t)gridDim.x < ntiles) issue(tile + 2 * (int64_t)gridDim.x, s);
+        if (warp == 0 && tile + S * (int64_t)gridDim.x < ntiles) issue(tile + S * (int64_t)gridDim.x, s);
     }
     if (lane == 0) {
 #pragma unroll
@@ -546,6 +550,8 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
     const int axpy_piece = (int)std::min<int64_t>(chunk_rows, kAxpyRowsMax);
     const size_t axpy_smem = 0;
     bool fuse_reorth = reorth && env_int("BJ_REORTH_FUSE", 1) != 0;
+    const int fuse_stages = std::max(2, std::min(8, env_int("BJ_REORTH_STAGES", kFuseStages)));
+    const int fuse_stage_bytes = std::min(env_int("BJ_REORTH_STAGE_KB", kFuseStageBytes / 1024) * 1024, 200 * 1024 / fuse_stages) / kFuseCtasPerSm;
     if (fuse_reorth) {
         static std::atomic<bool> configured[64];
         if (ensure_big_smem(reorth_axpy_dot_kernel, configured) != cudaSuccess) { cudaGetLastError(); fuse_reorth = false; }
@@ -631,10 +637,10 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
         if (reorth) {
             const int nv = j + 1;
             // the first pass' update and the second pass' dots in one pass over V (reorth_axpy_dot_kernel) when a tile of
-            // at least 64 rows of all nv columns fits a stage and the arrays are 16-byte aligned for the bulk copies
-            int R = (int)((kFuseStageBytes / ((size_t)(nv + 1) * 8)) & ~(size_t)31);
-            if (R > 512) R = 512;
-            const bool fuse_mid = fuse_reorth && R >= 64 && nv <= kFuseWarps * kFuseSlots && n % 2 == 0 &&
+            // at least 32 rows of all nv columns fits a stage and the arrays are 16-byte aligned for the bulk copies
+            int R = (int)(((size_t)fuse_stage_bytes / ((size_t)(nv + 1) * 8)) & ~(size_t)31);
+            if (R > kFuseThreads) R = kFuseThreads;  // a thread per row of the tile
+            const bool fuse_mid = fuse_reorth && R >= 32 && nv <= kFuseWarps * kFuseSlots && n % 2 == 0 &&
                                   ((uintptr_t)z.V % 16) == 0 && ((uintptr_t)z.w % 16) == 0;
             for (int pass = 0; pass < 2; ++pass) {
                 if (pass == 0 || !fuse_mid) {
@@ -645,10 +651,10 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
                 }
                 if (pass == 0 && fuse_mid) {
                     const int64_t ntiles = (n + R - 1) / R;
-                    const int grid = (int)std::min<int64_t>(ntiles, h->num_sms);
-                    const size_t smem = 64 + (208 + 512) * sizeof(double) + 2 * (size_t)(nv + 1) * R * sizeof(double);
+                    const int grid = (int)std::min<int64_t>(ntiles, (int64_t)h->num_sms * kFuseCtasPerSm);
+                    const size_t smem = 64 + (208 + 512) * sizeof(double) + fuse_stages * (size_t)(nv + 1) * R * sizeof(double);
                     e = launch_kernel(reorth_axpy_dot_kernel, dim3(grid), dim3(kFuseThreads), smem, st, pdl, n, nv,
-                                      (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done, R, ntiles);
+                                      (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done, R, ntiles, fuse_stages);
                     if (e != cudaSuccess) { set_cuda_error(e, "reorth_axpy_dot_kernel"); return BJ_ERR_CUDA; }
                     h->launches++;
                     BJ_LAUNCH(finalize_multi_kernel, nv, 256, grid, nv, (const double*)PM, stride, z.coef,
