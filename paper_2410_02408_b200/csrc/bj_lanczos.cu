@@ -377,6 +377,56 @@ reorth_axpy_dot_kernel(int64_t n, int nv, const double* __restrict__ V, double* 
     }
 }
 
+// The same fused pass with the tile in REGISTERS (nv <= NVMAX <= 52): a thread takes one row at a time, requests its nv basis
+// entries together (coalesced across the warp: consecutive threads, consecutive rows; ~100 KB in flight per SM), updates
+// w_r in the oracle's order, writes it back, and adds V_qr w_r to its nv private accumulators; one reduction at the very
+// end (shuffle tree per column inside each warp, then the warp sums in order).  No shared-memory tile, no bulk copies (a
+// 1.8 KB copy per column and tile is what holds the kernel above at 3.4 TB/s), no barrier inside the stream.
+constexpr int kRegFuseThreads = 256;
+template <int NVMAX>
+__global__ void __launch_bounds__(kRegFuseThreads, 1)
+reorth_axpy_dot_reg_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w, const double* __restrict__ coef,
+                           double* __restrict__ partial, int stride, const int* __restrict__ done)
+{
+    __shared__ double cs[NVMAX];
+    __shared__ double sh[kRegFuseThreads / 32][NVMAX];
+    pdl_trigger();
+    pdl_wait();
+    if (done[0]) return;
+    for (int q = threadIdx.x; q < NVMAX; q += kRegFuseThreads) cs[q] = q < nv ? coef[q] : 0.0;
+    __syncthreads();
+    double acc[NVMAX];
+#pragma unroll
+    for (int q = 0; q < NVMAX; ++q) acc[q] = 0.0;
+    const Chunk c = my_chunk(n);
+    for (int64_t i = c.lo + threadIdx.x; i < c.hi; i += kRegFuseThreads) {
+        double v[NVMAX];
+#pragma unroll
+        for (int q = 0; q < NVMAX; ++q) v[q] = q < nv ? V[(int64_t)q * n + i] : 0.0;
+        double wi = w[i];
+#pragma unroll
+        for (int q = 0; q < NVMAX; ++q) wi -= cs[q] * v[q];  // (columns past nv: c = v = 0, exact)
+        w[i] = wi;
+#pragma unroll
+        for (int q = 0; q < NVMAX; ++q) acc[q] = fma(v[q], wi, acc[q]);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int q = 0; q < NVMAX; ++q) {
+        double sq = acc[q];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) sq += __shfl_down_sync(0xffffffffu, sq, off);
+        if (lane == 0) sh[warp][q] = sq;
+    }
+    __syncthreads();
+    if (threadIdx.x < nv) {
+        double r = 0.0;
+#pragma unroll
+        for (int k = 0; k < kRegFuseThreads / 32; ++k) r += sh[k][threadIdx.x];
+        partial[(int64_t)blockIdx.x * stride + threadIdx.x] = r;
+    }
+}
+
 // out[q] = sum_cta partial[cta * stride + q]: one CTA per coefficient (a single CTA for all of them took 39 us at 50 vectors,
 // one tenth of a parity-mode step).  Thread t adds the partials of CTAs t, t + 256, .. in that order, then the fixed block
 // tree: bitwise reproducible.
@@ -643,11 +693,30 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
             const bool fuse_mid = fuse_reorth && R >= 32 && nv <= kFuseWarps * kFuseSlots && n % 2 == 0 &&
                                   ((uintptr_t)z.V % 16) == 0 && ((uintptr_t)z.w % 16) == 0;
             for (int pass = 0; pass < 2; ++pass) {
-                if (pass == 0 || !fuse_mid) {
+                const bool fused_before = pass == 1 && (fuse_mid || (fuse_reorth && nv <= 52 && env_int("BJ_REORTH_REG", 1) != 0));
+                if (!fused_before) {
                     BJ_LAUNCH(multidot_partial_kernel, G, kReduceThreads, n, nv, (const double*)z.V,
                               (const double*)z.w, PM, stride, (const int*)z.done);
                     BJ_LAUNCH(finalize_multi_kernel, nv, 256, G, nv, (const double*)PM, stride, z.coef,
                               (const int*)z.done);
+                }
+                if (pass == 0 && fuse_reorth && nv <= 52 && env_int("BJ_REORTH_REG", 1) != 0) {
+                    // the tile in registers (no alignment condition: ordinary loads)
+                    const int grid = (int)std::min<int64_t>((n + kRegFuseThreads - 1) / kRegFuseThreads, h->num_sms);
+                    if (nv <= 16)
+                        e = launch_kernel(reorth_axpy_dot_reg_kernel<16>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,
+                                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);
+                    else if (nv <= 32)
+                        e = launch_kernel(reorth_axpy_dot_reg_kernel<32>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,
+                                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);
+                    else
+                        e = launch_kernel(reorth_axpy_dot_reg_kernel<52>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,
+                                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);
+                    if (e != cudaSuccess) { set_cuda_error(e, "reorth_axpy_dot_reg_kernel"); return BJ_ERR_CUDA; }
+                    h->launches++;
+                    BJ_LAUNCH(finalize_multi_kernel, nv, 256, grid, nv, (const double*)PM, stride, z.coef,
+                              (const int*)z.done);
+                    continue;
                 }
                 if (pass == 0 && fuse_mid) {
                     const int64_t ntiles = (n + R - 1) / R;
