@@ -383,8 +383,8 @@ reorth_axpy_dot_kernel(int64_t n, int nv, const double* __restrict__ V, double* 
 // end (shuffle tree per column inside each warp, then the warp sums in order).  No shared-memory tile, no bulk copies (a
 // 1.8 KB copy per column and tile is what holds the kernel above at 3.4 TB/s), no barrier inside the stream.
 constexpr int kRegFuseThreads = 256;
-template <int NVMAX>
-__global__ void __launch_bounds__(kRegFuseThreads, 1)
+template <int NVMAX, int MINB>
+__global__ void __launch_bounds__(kRegFuseThreads, MINB)
 reorth_axpy_dot_reg_kernel(int64_t n, int nv, const double* __restrict__ V, double* __restrict__ w, const double* __restrict__ coef,
                            double* __restrict__ partial, int stride, const int* __restrict__ done)
 {
@@ -702,16 +702,22 @@ int lanczos_run(bj_handle_s* h, const bj_lanczos_opts_t* o, bj_lanczos_result_t*
                 }
                 if (pass == 0 && fuse_reorth && nv <= 52 && env_int("BJ_REORTH_REG", 1) != 0) {
                     // the tile in registers (no alignment condition: ordinary loads)
-                    const int grid = (int)std::min<int64_t>((n + kRegFuseThreads - 1) / kRegFuseThreads, h->num_sms);
-                    if (nv <= 16)
-                        e = launch_kernel(reorth_axpy_dot_reg_kernel<16>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,
-                                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);
-                    else if (nv <= 32)
-                        e = launch_kernel(reorth_axpy_dot_reg_kernel<32>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,
-                                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);
-                    else
-                        e = launch_kernel(reorth_axpy_dot_reg_kernel<52>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,
-                                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);
+                    // the kernel's cost follows NVMAX (padding columns are multiplied by zeros) and, for few columns, the
+                    // memory latency of a row: narrower variants run more CTAs per SM
+                    int grid = 0;
+#define BJ_REG_FUSE(NVM, MB)                                                                                                   \
+    do {                                                                                                                       \
+        grid = (int)std::min<int64_t>((n + kRegFuseThreads - 1) / kRegFuseThreads, (int64_t)h->num_sms * MB);                  \
+        e = launch_kernel(reorth_axpy_dot_reg_kernel<NVM, MB>, dim3(grid), dim3(kRegFuseThreads), 0, st, pdl, n, nv,           \
+                          (const double*)z.V, z.w, (const double*)z.coef, PM, stride, (const int*)z.done);                     \
+    } while (0)
+                    if (nv <= 8) BJ_REG_FUSE(8, 4);
+                    else if (nv <= 16) BJ_REG_FUSE(16, 3);
+                    else if (nv <= 24) BJ_REG_FUSE(24, 2);
+                    else if (nv <= 32) BJ_REG_FUSE(32, 1);
+                    else if (nv <= 40) BJ_REG_FUSE(40, 1);
+                    else BJ_REG_FUSE(52, 1);
+#undef BJ_REG_FUSE
                     if (e != cudaSuccess) { set_cuda_error(e, "reorth_axpy_dot_reg_kernel"); return BJ_ERR_CUDA; }
                     h->launches++;
                     BJ_LAUNCH(finalize_multi_kernel, nv, 256, grid, nv, (const double*)PM, stride, z.coef,
