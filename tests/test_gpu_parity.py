@@ -264,6 +264,22 @@ def test_single_launch_lanczos_on_the_papers_larger_sizes(B, torch_):
         B.bj_destroy(h)
 
 
+@pytest.mark.parametrize("m", [60, 120, 230])
+def test_parity_mode_reorthogonalisation_kernels_beyond_52_vectors(B, torch_, m):
+    """Full reorthogonalisation on the multi-launch path: up to 52 basis vectors the fused update + dot pass keeps its tile in
+    registers, up to 199 in shared memory (bulk copies), beyond that the four unfused kernels run; odd n takes the unfused
+    kernels too.  kappa and the coefficients against the oracle in every regime."""
+    for A, b in ((mat(2, "small"), 8), (W.laplacian((113, 97)), 4)):     # n = 13 824 (even), n = 10 961 (odd)
+        h, keep = B.setup_from_host(A, b)
+        g = B.bj_cond_estimate_ex(h, m, reorth=True)
+        c = oracle.Precond(A, b).cond_estimate(m, reorth=True)
+        assert g["iters_done"] == c["iters_done"] == m
+        assert abs(g["kappa"] / c["kappa"] - 1) <= TOL_KAPPA, (A.n, m, g["kappa"], c["kappa"])
+        scale = abs(c["alpha"]).max()
+        assert np.abs(g["alpha"] - c["alpha"]).max() <= 1e-8 * scale and np.abs(g["beta"] - c["beta"]).max() <= 1e-7 * scale
+        B.bj_destroy(h)
+
+
 def test_point_jacobi_is_the_papers_kernel(B, torch_):
     """PAPER.md:234: M[idx] = 1/A[idx*N+idx]."""
     A = mat(1, "full")
