@@ -1,0 +1,254 @@
+// Setup for b <= 8 without a permutation or band detection: TWO kernels instead of three passes over the CSR.
+//   tile_validate_extract_kernel<B>   a1 + a2, ENTRY-parallel: a CTA takes a tile of consecutive rows (a multiple of b, at most
+//       256) -- whose entries are one contiguous range of col_idx / val -- keeps the tile's row pointers in shared memory, and
+//       walks the range with consecutive threads on consecutive entries (coalesced; eight entries per thread requested
+//       together).  Per entry: its row by binary search in the shared row pointers, the checks of a1 (column range, strictly
+//       ascending inside the row), and, if it lies in the lower triangle of the row's diagonal block, one store into the factor
+//       array in a row-friendly raw layout (block k at k * P, packed by rows; the tile's blocks are zero-filled first).  The
+//       row-pointer checks, the longest row and the column-coherence statistic of the SpMV plan ride on the threads that load
+//       the row pointers.  The thread-per-BLOCK extraction it replaces walked b rows per thread with ~100 registers (16 warps
+//       per SM, 31 sectors per warp load): 90 us on config 2 at 14 % issue utilisation.
+//   factor_small_inplace_kernel<B>    a3, one thread per block: 36 independent loads of the raw block, Cholesky in registers
+//       (the arithmetic of extract_factor_small_kernel), then the interleaved layout of solve_small_kernel written over the
+//       SAME 32-block group (a warp owns a group: all lanes load, __syncwarp, all lanes store).
+// The CSR is read once, and one host synchronisation goes away.  An invalid CSR is flagged in the status word and reported
+// as BJ_ERR_NOT_CANONICAL by bj_setup; reads stay in bounds (a tile with a bad row pointer is skipped), the factorisation
+// then runs on garbage and its result is discarded.
+#include <algorithm>
+
+#include "bj_device.cuh"
+#include "bj_internal.cuh"
+
+namespace bj {
+
+namespace {
+
+constexpr int kTileThreads = 256;
+constexpr int kTileUnroll = 8;   // entries per thread requested together
+
+template <int B>
+__global__ void __launch_bounds__(kTileThreads)
+tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
+                             const double* __restrict__ val, double* __restrict__ raw, Status* st)
+{
+    constexpr int P = B * (B + 1) / 2;
+    constexpr int TR = (kTileThreads / B) * B;  // rows per tile: whole blocks only, so that a block belongs to ONE CTA
+    __shared__ int rps[TR + 1];
+    __shared__ unsigned sh[2][kTileThreads / 32];
+    __shared__ int tile_bad;
+    int flags = 0, len = 0;
+    unsigned coh = 0, cmp = 0;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool vec_ok = (reinterpret_cast<uintptr_t>(ci) & 15) == 0;  // 16-byte loads of the columns
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t r0 = tile * TR;
+        const int rows = (int)(r0 + TR <= n ? TR : n - r0);
+        __syncthreads();  // the previous tile's readers of rps / tile_bad are done
+        if (tid == 0) tile_bad = 0;
+        __syncthreads();
+        // ---- row pointers of the tile; a1 for them ----
+        if (tid < rows) {
+            const int64_t i = r0 + tid;
+            const int64_t s = rp[i];
+            rps[tid] = (int)s;
+            {
+                const int64_t e = rp[i + 1];
+                if (tid == rows - 1) rps[rows] = (int)e;
+                if (s > e || s < 0 || e > nnz || (i == 0 && s != 0) || (i == n - 1 && e != nnz)) {
+                    flags |= ST_BAD_ROWPTR;
+                    tile_bad = 1;
+                } else {
+                    const int l = (int)(e - s);
+                    len = l > len ? l : len;
+                    if ((tile & 7) == 0 && i + 1 < n) {  // every eighth tile also gathers the column-coherence statistic
+                        const int64_t e2 = rp[i + 2];
+                        if (e2 >= e && e2 <= nnz) {
+                            int64_t m = (e2 - e) < (e - s) ? (e2 - e) : (e - s);
+                            if (m > 8) m = 8;  // a sample: the first entries of the two rows
+                            for (int64_t q = 0; q < m; ++q) {
+                                const int d = ci[e + q] - ci[s + q];
+                                ++cmp;
+                                coh += (d >= -16 && d <= 16);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        // ---- zero the raw blocks of the tile (TR is a multiple of B: they are this CTA's alone) ----
+        const int64_t kb0 = r0 / B, kb1 = (r0 + rows + B - 1) / B;
+        for (int64_t e = kb0 * P + tid; e < kb1 * P; e += kTileThreads) raw[e] = 0.0;
+        __syncthreads();
+        if (tile_bad) continue;  // uniform: nothing of this tile is read through its row pointers
+        // ---- the entries of the tile: one contiguous range; a thread takes EIGHT CONSECUTIVE entries (two 16-byte loads of
+        // columns; a warp covers 1 KB), finds the row of the first by binary search and walks the row pointers from there ----
+        const int e0 = rps[0], e1 = rps[rows];
+        for (int base = e0 & ~7; base < e1; base += kTileThreads * kTileUnroll) {
+            const int p0 = base + tid * kTileUnroll;
+            int c[kTileUnroll];
+            if (vec_ok && p0 >= e0 && p0 + kTileUnroll <= e1) {
+                const int4 a4 = *reinterpret_cast<const int4*>(ci + p0);
+                const int4 b4 = *reinterpret_cast<const int4*>(ci + p0 + 4);
+                c[0] = a4.x; c[1] = a4.y; c[2] = a4.z; c[3] = a4.w;
+                c[4] = b4.x; c[5] = b4.y; c[6] = b4.z; c[7] = b4.w;
+            } else {
+#pragma unroll
+                for (int u = 0; u < kTileUnroll; ++u) c[u] = (p0 + u >= e0 && p0 + u < e1) ? ci[p0 + u] : -1;
+            }
+            int cprev = __shfl_up_sync(0xffffffffu, c[kTileUnroll - 1], 1);  // entry p0 - 1 is the last one of the lane below
+            if (lane == 0 && p0 > e0 && p0 < e1) cprev = ci[p0 - 1];
+            // the row of the first entry: the last r with rps[r] <= p (rows <= 256: eight steps)
+            int r = 0;
+            {
+                const int pf = p0 < e0 ? e0 : p0;
+                int lo = 0, hi = rows;
+                while (hi - lo > 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if (rps[mid] <= pf) lo = mid; else hi = mid;
+                }
+                r = lo;
+            }
+            int next = rps[r + 1], start = rps[r];
+            // everything below is 32-bit and tile-local: block kl = r / B of the tile, row rr of it, first column of the block lob
+            int kl = r / B, rr = r - kl * B;
+            const int r0i = (int)r0;
+            int lob = r0i + kl * B;
+            int dst[kTileUnroll];  // offset of the entry in the tile's raw blocks, or -1
+#pragma unroll
+            for (int u = 0; u < kTileUnroll; ++u) {
+                const int p = p0 + u;
+                dst[u] = -1;
+                if (p >= e0 && p < e1) {
+                    while (p >= next) {  // next row (empty rows are stepped over)
+                        ++r;
+                        start = next;
+                        next = rps[r + 1];
+                        if (++rr == B) { rr = 0; ++kl; lob += B; }
+                    }
+                    const int cc = c[u];
+                    if ((unsigned)cc >= (unsigned)n) flags |= ST_BAD_COL;
+                    if (p != start && cc <= cprev) flags |= ST_UNSORTED;  // columns ascend strictly inside a row
+                    const unsigned d = (unsigned)(cc - lob);                 // in the block's lower triangle: 0 <= d <= rr
+                    if (cc >= lob && d <= (unsigned)rr) dst[u] = kl * P + rr * (rr + 1) / 2 + (int)d;
+                }
+                cprev = c[u];
+            }
+            double* rawt = raw + kb0 * P;
+            double v[kTileUnroll];  // the values of the entries inside the blocks, requested together
+#pragma unroll
+            for (int u = 0; u < kTileUnroll; ++u) v[u] = dst[u] >= 0 ? val[p0 + u] : 0.0;
+#pragma unroll
+            for (int u = 0; u < kTileUnroll; ++u)
+                if (dst[u] >= 0) rawt[dst[u]] = v[u];
+        }
+    }
+    flags = __reduce_or_sync(0xffffffffu, flags);
+    len = __reduce_max_sync(0xffffffffu, len);
+    coh = __reduce_add_sync(0xffffffffu, coh);
+    cmp = __reduce_add_sync(0xffffffffu, cmp);
+    const int warp = tid >> 5;
+    if (lane == 0) {
+        if (flags) atomicOr(&st->flags, flags);
+        if (len > *(volatile int*)&st->max_row_nnz) atomicMax(&st->max_row_nnz, len);
+        sh[0][warp] = coh; sh[1][warp] = cmp;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        unsigned a = 0, c2 = 0;
+        for (int w = 0; w < kTileThreads / 32; ++w) { a += sh[0][w]; c2 += sh[1][w]; }
+        if (c2) { atomicAdd(&st->coherent, (unsigned long long)a); atomicAdd(&st->compared, (unsigned long long)c2); }
+    }
+}
+
+// One thread per block, a warp per interleave group of 32 blocks, in place (see the header).  Blocks past the last one of
+// a partly filled group are written as zeros; rows past n of a ragged last block are identity rows.
+template <int B>
+__global__ void __launch_bounds__(128)
+factor_small_inplace_kernel(int64_t n, int64_t nblocks, double* fac, Status* st)
+{
+    constexpr int P = B * (B + 1) / 2;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // the grid covers whole groups
+    const bool act = k < nblocks;
+    const int64_t lo = k * B;
+    double d[P];  // packed lower triangle, e = i(i+1)/2 + j
+    {
+        const double* src = fac + k * P;
+#pragma unroll
+        for (int e = 0; e < P; ++e) d[e] = act ? src[e] : 0.0;
+    }
+#pragma unroll
+    for (int i = 0; i < B; ++i) {
+        if (lo + i >= n) {  // (also every row of an inactive lane: nothing of it is stored)
+#pragma unroll
+            for (int j = 0; j < B; ++j)
+                if (j <= i) d[i * (i + 1) / 2 + j] = (j == i) ? 1.0 : 0.0;
+        }
+    }
+    __syncwarp();  // every lane of the group holds its raw block: the group's storage may be overwritten
+    bool bad = false;
+    double rinv[B];
+    // every loop has the constant trip count B (triangular bounds as predicates): all of them unroll, d[] stays in registers
+#pragma unroll
+    for (int j = 0; j < B; ++j) {
+        double sjj = d[j * (j + 1) / 2 + j];
+#pragma unroll
+        for (int p = 0; p < B; ++p)
+            if (p < j) sjj -= d[j * (j + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
+        if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
+        const double ljj = sqrt(sjj);
+        const double rjj = __drcp_rn(ljj);  // also the stored diagonal slot 1 / l_jj
+        rinv[j] = rjj;
+        d[j * (j + 1) / 2 + j] = ljj;
+#pragma unroll
+        for (int i = 0; i < B; ++i) {
+            if (i > j) {
+                double t = d[i * (i + 1) / 2 + j];
+#pragma unroll
+                for (int p = 0; p < B; ++p)
+                    if (p < j) t -= d[i * (i + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
+                d[i * (i + 1) / 2 + j] = div_by(t, ljj, rjj);
+            }
+        }
+    }
+    if (bad && act) {
+        atomicOr(&st->flags, ST_NOT_SPD);
+        atomicMin(&st->bad_block, (long long)k);
+    }
+    double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
+#pragma unroll
+    for (int i = 0; i < B; ++i)
+#pragma unroll
+        for (int j = 0; j <= i; ++j) {
+            const double v = d[i * (i + 1) / 2 + j];
+            f[(i * (i + 1) / 2 + j) * kInterleave] = act ? ((i == j) ? rinv[i] : v) : 0.0;
+        }
+}
+
+}  // namespace
+
+// a1-a3 for solve_kind 1 without permutation and without band detection (see the header); the caller reads the status back
+int launch_setup_rows(bj_handle_s* h)
+{
+    const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;
+    const unsigned fb = (unsigned)((groups * kInterleave + 127) / 128);
+#define BJ_CASE(B)                                                                                                          \
+    case B: {                                                                                                               \
+        const int64_t tr = (kTileThreads / B) * B;                                                                          \
+        const int64_t ntiles = (h->n + tr - 1) / tr;                                                                        \
+        const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)h->num_sms * 8);                                 \
+        { SetupSpan span(h); tile_validate_extract_kernel<B><<<grid, kTileThreads, 0, h->stream>>>(h->n, h->nnz, ntiles, h->row_ptr, \
+                                                                     h->col_idx, h->val, h->fac_small, h->status); }        \
+        { SetupSpan span(h); factor_small_inplace_kernel<B><<<fb, 128, 0, h->stream>>>(h->n, h->nblocks, h->fac_small, h->status); } \
+        break;                                                                                                              \
+    }
+    switch (h->b) {
+        BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
+        default: return BJ_ERR_INVALID_ARG;
+    }
+#undef BJ_CASE
+    h->launches += 2;
+    BJ_CUDA(cudaGetLastError());
+    return BJ_OK;
+}
+
+}  // namespace bj
