@@ -313,13 +313,17 @@ static int setup_impl(const bj_csr_t* csr, int b, const bj_setup_opts_t& o, bj_h
 
     // b <= 8, short rows, no permutation, no band detection: validation rides on the entry-parallel extraction
     // (bj_setup_rows.cu) and the factorisation follows without a host round trip.  Its cost follows nnz (6.5 ns per entry and
-    // SM-microsecond): measured against the three passes it wins for up to 8 entries per row (config 2 b = 8 0.140 -> 0.127 ms,
-    // b = 7 0.148 -> 0.127, config 1 0.031 -> 0.024) and loses beyond (config 4 b = 8, 9 per row: 0.30 vs 0.26 ms; config 5
+    // SM-microsecond): measured against the three passes it wins for up to 8 entries per row (config 2 b = 8 0.140 -> 0.120 ms,
+    // b = 7 0.148 -> 0.122, config 1 0.031 -> 0.016) and loses beyond (config 4 b = 8, 9 per row: 0.30 vs 0.26 ms; config 5
     // b = 3, 81 per row: 0.59 vs 0.44), except for incoherent columns (config 3 b = 8: 0.12 vs 0.22 ms), which setup cannot
-    // know before it has read them.  BJ_SETUP_ROWWISE = 0 / 2 forces the three passes / the two kernels.
+    // know before it has read them.  BJ_SETUP_ROWWISE = 0 / 2 forces the three passes / the one kernel.
     const int rowwise_env = env_int("BJ_SETUP_ROWWISE", 1);
     const bool rowwise = h->solve_kind == 1 && !perm_dev && !want_band && rowwise_env != 0 && (rowwise_env == 2 || h->nnz <= 8 * h->n);
     // a1 validate (also longest row and the column-coherence statistic)
+    if (rowwise) {  // (the unused slots of a partly filled last interleave group are zeroed first)
+        ce = zero_padding();
+        if (ce != cudaSuccess) { set_cuda_error(ce, "factor memset"); return fail(BJ_ERR_CUDA); }
+    }
     rc = rowwise ? launch_setup_rows(h) : launch_validate(h);
     if (rc != BJ_OK) return fail(rc);
     rc = read_status(stt, "validate");

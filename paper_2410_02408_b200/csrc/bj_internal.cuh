@@ -225,7 +225,7 @@ struct KernelScope {
 // setup (bj_setup_kernels.cu)
 int launch_validate(bj_handle_s* h);
 int launch_extract_factor(bj_handle_s* h);
-int launch_setup_rows(bj_handle_s* h);  // a1-a3 in two kernels for b <= 8 without permutation / band detection (bj_setup_rows.cu)
+int launch_setup_rows(bj_handle_s* h);  // a1-a3 in one kernel for b <= 8, short rows, no permutation / band detection (bj_setup_rows.cu)
 int launch_spmv_plan(bj_handle_s* h, int tile_rows);  // Status.max_tile_nnz for tiles of tile_rows rows
 int col16_build(bj_handle_s* h);       // 16-bit column deltas when every |col - row| < 32768
 void col16_free(bj_handle_s* h);

@@ -1,19 +1,18 @@
-// Setup for b <= 8 without a permutation or band detection: TWO kernels instead of three passes over the CSR.
-//   tile_validate_extract_kernel<B>   a1 + a2, ENTRY-parallel: a CTA takes a tile of consecutive rows (a multiple of b, at most
-//       256) -- whose entries are one contiguous range of col_idx / val -- keeps the tile's row pointers in shared memory, and
-//       walks the range with consecutive threads on consecutive entries (coalesced; eight entries per thread requested
-//       together).  Per entry: its row by binary search in the shared row pointers, the checks of a1 (column range, strictly
-//       ascending inside the row), and, if it lies in the lower triangle of the row's diagonal block, one store into the factor
-//       array in a row-friendly raw layout (block k at k * P, packed by rows; the tile's blocks are zero-filled first).  The
-//       row-pointer checks, the longest row and the column-coherence statistic of the SpMV plan ride on the threads that load
-//       the row pointers.  The thread-per-BLOCK extraction it replaces walked b rows per thread with ~100 registers (16 warps
-//       per SM, 31 sectors per warp load): 90 us on config 2 at 14 % issue utilisation.
-//   factor_small_inplace_kernel<B>    a3, one thread per block: 36 independent loads of the raw block, Cholesky in registers
-//       (the arithmetic of extract_factor_small_kernel), then the interleaved layout of solve_small_kernel written over the
-//       SAME 32-block group (a warp owns a group: all lanes load, __syncwarp, all lanes store).
-// The CSR is read once, and one host synchronisation goes away.  An invalid CSR is flagged in the status word and reported
-// as BJ_ERR_NOT_CANONICAL by bj_setup; reads stay in bounds (a tile with a bad row pointer is skipped), the factorisation
-// then runs on garbage and its result is discarded.
+// Setup for b <= 8 and short rows, without a permutation or band detection: ONE kernel instead of three passes over the CSR.
+// tile_validate_extract_kernel<B> (a1 + a2 + a3): a CTA takes a tile of consecutive rows (a multiple of b, at most 256) --
+// whose entries are one contiguous range of col_idx / val -- and keeps the tile's row pointers and its diagonal blocks
+// (packed lower triangles, zero-filled) in shared memory.
+//   * ENTRY-parallel walk: a thread takes eight consecutive entries (two 16-byte loads of columns; a warp covers 1 KB), finds
+//     the row of the first by binary search in the shared row pointers and walks them from there; per entry the checks of a1
+//     (column range, strictly ascending inside the row) and, if it lies in the lower triangle of the row's diagonal block, one
+//     store into the shared tile.  The row-pointer checks, the longest row and the column-coherence statistic of the SpMV plan
+//     ride on the threads that load the row pointers.
+//   * then thread t factors block t of the tile in place in shared memory (the arithmetic of extract_factor_small_kernel)
+//     and writes it in the interleaved layout of solve_small_kernel.
+// The CSR is read once, nothing intermediate goes through global memory, and one host synchronisation goes away.  The
+// thread-per-BLOCK extraction it replaces walked b rows per thread with ~100 registers (16 warps per SM, 31 sectors per warp
+// load): 90 us on config 2 at 14 % issue utilisation.  An invalid CSR is flagged in the status word and reported as
+// BJ_ERR_NOT_CANONICAL by bj_setup; reads stay in bounds (a tile with a bad row pointer is skipped).
 #include <algorithm>
 
 #include "bj_device.cuh"
@@ -26,14 +25,19 @@ namespace {
 constexpr int kTileThreads = 256;
 constexpr int kTileUnroll = 8;   // entries per thread requested together
 
+// (four CTAs per SM: the entry walk needs the warps, the factorisation -- one warp per tile -- pays a few spilled bytes;
+// measured on config 2 b = 8: 2 / 3 / 4 / 5 / 6 CTAs per SM 0.189 / 0.163 / 0.120 / 0.129 / 0.134 ms)
 template <int B>
-__global__ void __launch_bounds__(kTileThreads)
-tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, const int32_t* __restrict__ rp, const int32_t* __restrict__ ci,
-                             const double* __restrict__ val, double* __restrict__ raw, Status* st)
+__global__ void __launch_bounds__(kTileThreads, 4)
+tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nblocks, const int32_t* __restrict__ rp,
+                             const int32_t* __restrict__ ci, const double* __restrict__ val, double* __restrict__ fac, Status* st)
 {
     constexpr int P = B * (B + 1) / 2;
+    constexpr int PS = P | 1;                   // odd stride of a block in the shared tile: thread-per-block accesses hit different banks
     constexpr int TR = (kTileThreads / B) * B;  // rows per tile: whole blocks only, so that a block belongs to ONE CTA
+    constexpr int NB = TR / B;                  // blocks per tile
     __shared__ int rps[TR + 1];
+    __shared__ double raws[NB * PS];            // the tile's diagonal blocks, packed lower triangles by rows
     __shared__ unsigned sh[2][kTileThreads / 32];
     __shared__ int tile_bad;
     int flags = 0, len = 0;
@@ -75,9 +79,9 @@ tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, const int32
                 }
             }
         }
-        // ---- zero the raw blocks of the tile (TR is a multiple of B: they are this CTA's alone) ----
+        // ---- zero the tile's blocks (TR is a multiple of B: they are this CTA's alone) ----
         const int64_t kb0 = r0 / B, kb1 = (r0 + rows + B - 1) / B;
-        for (int64_t e = kb0 * P + tid; e < kb1 * P; e += kTileThreads) raw[e] = 0.0;
+        for (int e = tid; e < NB * PS; e += kTileThreads) raws[e] = 0.0;
         __syncthreads();
         if (tile_bad) continue;  // uniform: nothing of this tile is read through its row pointers
         // ---- the entries of the tile: one contiguous range; a thread takes EIGHT CONSECUTIVE entries (two 16-byte loads of
@@ -129,17 +133,60 @@ tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, const int32
                     if ((unsigned)cc >= (unsigned)n) flags |= ST_BAD_COL;
                     if (p != start && cc <= cprev) flags |= ST_UNSORTED;  // columns ascend strictly inside a row
                     const unsigned d = (unsigned)(cc - lob);                 // in the block's lower triangle: 0 <= d <= rr
-                    if (cc >= lob && d <= (unsigned)rr) dst[u] = kl * P + rr * (rr + 1) / 2 + (int)d;
+                    if (cc >= lob && d <= (unsigned)rr) dst[u] = kl * PS + rr * (rr + 1) / 2 + (int)d;
                 }
                 cprev = c[u];
             }
-            double* rawt = raw + kb0 * P;
             double v[kTileUnroll];  // the values of the entries inside the blocks, requested together
 #pragma unroll
             for (int u = 0; u < kTileUnroll; ++u) v[u] = dst[u] >= 0 ? val[p0 + u] : 0.0;
 #pragma unroll
             for (int u = 0; u < kTileUnroll; ++u)
-                if (dst[u] >= 0) rawt[dst[u]] = v[u];
+                if (dst[u] >= 0) raws[dst[u]] = v[u];
+        }
+        __syncthreads();
+        // ---- a3: thread t factors block kb0 + t in place in the shared tile (the arithmetic of extract_factor_small_kernel)
+        // and writes it in the interleaved layout of solve_small_kernel ----
+        if (tid < (int)(kb1 - kb0)) {
+            const int64_t k = kb0 + tid;
+            double* D = raws + tid * PS;  // packed lower triangle, e = i (i + 1) / 2 + j
+            const int64_t lo = k * B;
+#pragma unroll
+            for (int i = 0; i < B; ++i) {
+                if (lo + i >= n) {  // identity rows pad a ragged last block
+#pragma unroll
+                    for (int j = 0; j <= i; ++j) D[i * (i + 1) / 2 + j] = (j == i) ? 1.0 : 0.0;
+                }
+            }
+            bool bad = false;
+            double rinv[B];
+#pragma unroll
+            for (int j = 0; j < B; ++j) {
+                double sjj = D[j * (j + 1) / 2 + j];
+#pragma unroll
+                for (int q = 0; q < j; ++q) sjj -= D[j * (j + 1) / 2 + q] * D[j * (j + 1) / 2 + q];
+                if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
+                const double ljj = sqrt(sjj);
+                const double rjj = __drcp_rn(ljj);  // also the stored diagonal slot 1 / l_jj
+                rinv[j] = rjj;
+                D[j * (j + 1) / 2 + j] = ljj;
+#pragma unroll
+                for (int i = j + 1; i < B; ++i) {
+                    double t = D[i * (i + 1) / 2 + j];
+#pragma unroll
+                    for (int q = 0; q < j; ++q) t -= D[i * (i + 1) / 2 + q] * D[j * (j + 1) / 2 + q];
+                    D[i * (i + 1) / 2 + j] = div_by(t, ljj, rjj);
+                }
+            }
+            if (bad) {
+                atomicOr(&st->flags, ST_NOT_SPD);
+                atomicMin(&st->bad_block, (long long)k);
+            }
+            double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
+#pragma unroll
+            for (int i = 0; i < B; ++i)
+#pragma unroll
+                for (int j = 0; j <= i; ++j) f[(i * (i + 1) / 2 + j) * kInterleave] = (i == j) ? rinv[i] : D[i * (i + 1) / 2 + j];
         }
     }
     flags = __reduce_or_sync(0xffffffffu, flags);
@@ -160,85 +207,18 @@ tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, const int32
     }
 }
 
-// One thread per block, a warp per interleave group of 32 blocks, in place (see the header).  Blocks past the last one of
-// a partly filled group are written as zeros; rows past n of a ragged last block are identity rows.
-template <int B>
-__global__ void __launch_bounds__(128)
-factor_small_inplace_kernel(int64_t n, int64_t nblocks, double* fac, Status* st)
-{
-    constexpr int P = B * (B + 1) / 2;
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // the grid covers whole groups
-    const bool act = k < nblocks;
-    const int64_t lo = k * B;
-    double d[P];  // packed lower triangle, e = i(i+1)/2 + j
-    {
-        const double* src = fac + k * P;
-#pragma unroll
-        for (int e = 0; e < P; ++e) d[e] = act ? src[e] : 0.0;
-    }
-#pragma unroll
-    for (int i = 0; i < B; ++i) {
-        if (lo + i >= n) {  // (also every row of an inactive lane: nothing of it is stored)
-#pragma unroll
-            for (int j = 0; j < B; ++j)
-                if (j <= i) d[i * (i + 1) / 2 + j] = (j == i) ? 1.0 : 0.0;
-        }
-    }
-    __syncwarp();  // every lane of the group holds its raw block: the group's storage may be overwritten
-    bool bad = false;
-    double rinv[B];
-    // every loop has the constant trip count B (triangular bounds as predicates): all of them unroll, d[] stays in registers
-#pragma unroll
-    for (int j = 0; j < B; ++j) {
-        double sjj = d[j * (j + 1) / 2 + j];
-#pragma unroll
-        for (int p = 0; p < B; ++p)
-            if (p < j) sjj -= d[j * (j + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
-        if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
-        const double ljj = sqrt(sjj);
-        const double rjj = __drcp_rn(ljj);  // also the stored diagonal slot 1 / l_jj
-        rinv[j] = rjj;
-        d[j * (j + 1) / 2 + j] = ljj;
-#pragma unroll
-        for (int i = 0; i < B; ++i) {
-            if (i > j) {
-                double t = d[i * (i + 1) / 2 + j];
-#pragma unroll
-                for (int p = 0; p < B; ++p)
-                    if (p < j) t -= d[i * (i + 1) / 2 + p] * d[j * (j + 1) / 2 + p];
-                d[i * (i + 1) / 2 + j] = div_by(t, ljj, rjj);
-            }
-        }
-    }
-    if (bad && act) {
-        atomicOr(&st->flags, ST_NOT_SPD);
-        atomicMin(&st->bad_block, (long long)k);
-    }
-    double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
-#pragma unroll
-    for (int i = 0; i < B; ++i)
-#pragma unroll
-        for (int j = 0; j <= i; ++j) {
-            const double v = d[i * (i + 1) / 2 + j];
-            f[(i * (i + 1) / 2 + j) * kInterleave] = act ? ((i == j) ? rinv[i] : v) : 0.0;
-        }
-}
-
 }  // namespace
 
 // a1-a3 for solve_kind 1 without permutation and without band detection (see the header); the caller reads the status back
 int launch_setup_rows(bj_handle_s* h)
 {
-    const int64_t groups = (h->nblocks + kInterleave - 1) / kInterleave;
-    const unsigned fb = (unsigned)((groups * kInterleave + 127) / 128);
 #define BJ_CASE(B)                                                                                                          \
     case B: {                                                                                                               \
         const int64_t tr = (kTileThreads / B) * B;                                                                          \
         const int64_t ntiles = (h->n + tr - 1) / tr;                                                                        \
         const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)h->num_sms * 8);                                 \
-        { SetupSpan span(h); tile_validate_extract_kernel<B><<<grid, kTileThreads, 0, h->stream>>>(h->n, h->nnz, ntiles, h->row_ptr, \
-                                                                     h->col_idx, h->val, h->fac_small, h->status); }        \
-        { SetupSpan span(h); factor_small_inplace_kernel<B><<<fb, 128, 0, h->stream>>>(h->n, h->nblocks, h->fac_small, h->status); } \
+        { SetupSpan span(h); tile_validate_extract_kernel<B><<<grid, kTileThreads, 0, h->stream>>>(h->n, h->nnz, ntiles, h->nblocks, \
+                                                          h->row_ptr, h->col_idx, h->val, h->fac_small, h->status); }       \
         break;                                                                                                              \
     }
     switch (h->b) {
@@ -246,7 +226,7 @@ int launch_setup_rows(bj_handle_s* h)
         default: return BJ_ERR_INVALID_ARG;
     }
 #undef BJ_CASE
-    h->launches += 2;
+    h->launches += 1;
     BJ_CUDA(cudaGetLastError());
     return BJ_OK;
 }
