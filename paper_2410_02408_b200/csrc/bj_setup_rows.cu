@@ -207,25 +207,249 @@ tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nbl
     }
 }
 
+// The same kernel with the factorisation taken off the critical path: warps 0..6 (224 threads) are the EXTRACT group and
+// walk tile after tile, warp 7 is the FACTOR group and factors the blocks of the previous tile meanwhile (in the one-group
+// form a third of the warp time was seven warps waiting at the barrier while one factored).  Two shared tiles alternate;
+// the groups hand them over through two pairs of mbarriers (full: 7 arrivals, one per extract warp; empty: 1 arrival).
+constexpr int kExtractThreads = kTileThreads - 32;
+__device__ __forceinline__ void bar_extract() { asm volatile("bar.sync 1, %0;" ::"n"(kExtractThreads) : "memory"); }
+
+template <int B>
+__global__ void __launch_bounds__(kTileThreads, 4)
+tile_setup_ws_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nblocks, const int32_t* __restrict__ rp,
+                     const int32_t* __restrict__ ci, const double* __restrict__ val, double* __restrict__ fac, Status* st)
+{
+    constexpr int P = B * (B + 1) / 2;
+    constexpr int PS = P | 1;
+    constexpr int TR = (kTileThreads / B) * B;
+    constexpr int NB = TR / B;
+    __shared__ __align__(8) uint64_t full[2], empty[2];
+    __shared__ int rps[TR + 1];
+    __shared__ double raws[2][NB * PS];
+    __shared__ unsigned sh[2][kTileThreads / 32];
+    __shared__ int tile_bad, bad_buf[2];
+    int flags = 0, len = 0;
+    unsigned coh = 0, cmp = 0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool vec_ok = (reinterpret_cast<uintptr_t>(ci) & 15) == 0;
+    if (tid == 0) {
+        mbar_init(&full[0], kExtractThreads / 32);
+        mbar_init(&full[1], kExtractThreads / 32);
+        mbar_init(&empty[0], 1);
+        mbar_init(&empty[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == kExtractThreads / 32) {
+        // ================= FACTOR group: one warp, thread per block, in place in the shared tile =================
+        int it = 0;
+        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+            const int buf = it & 1;
+            mbar_wait(&full[buf], (uint32_t)((it >> 1) & 1));
+            const int64_t r0 = tile * TR;
+            const int rows = (int)(r0 + TR <= n ? TR : n - r0);
+            const int64_t kb0 = r0 / B, kb1 = (r0 + rows + B - 1) / B;
+            if (!bad_buf[buf]) {
+                for (int t = lane; t < (int)(kb1 - kb0); t += 32) {
+                    const int64_t k = kb0 + t;
+                    double* D = raws[buf] + t * PS;  // packed lower triangle, e = i (i + 1) / 2 + j
+                    const int64_t lo = k * B;
+#pragma unroll
+                    for (int i = 0; i < B; ++i) {
+                        if (lo + i >= n) {  // identity rows pad a ragged last block
+#pragma unroll
+                            for (int j = 0; j <= i; ++j) D[i * (i + 1) / 2 + j] = (j == i) ? 1.0 : 0.0;
+                        }
+                    }
+                    bool bad = false;
+                    double rinv[B];
+#pragma unroll
+                    for (int j = 0; j < B; ++j) {
+                        double sjj = D[j * (j + 1) / 2 + j];
+#pragma unroll
+                        for (int q = 0; q < j; ++q) sjj -= D[j * (j + 1) / 2 + q] * D[j * (j + 1) / 2 + q];
+                        if (!(sjj > 0.0) || isinf(sjj)) { bad = true; sjj = 1.0; }
+                        const double ljj = sqrt(sjj);
+                        const double rjj = __drcp_rn(ljj);
+                        rinv[j] = rjj;
+                        D[j * (j + 1) / 2 + j] = ljj;
+#pragma unroll
+                        for (int i = j + 1; i < B; ++i) {
+                            double tt = D[i * (i + 1) / 2 + j];
+#pragma unroll
+                            for (int q = 0; q < j; ++q) tt -= D[i * (i + 1) / 2 + q] * D[j * (j + 1) / 2 + q];
+                            D[i * (i + 1) / 2 + j] = div_by(tt, ljj, rjj);
+                        }
+                    }
+                    if (bad) {
+                        atomicOr(&st->flags, ST_NOT_SPD);
+                        atomicMin(&st->bad_block, (long long)k);
+                    }
+                    double* f = fac + (k >> 5) * (int64_t)(P * kInterleave) + (k & 31);
+#pragma unroll
+                    for (int i = 0; i < B; ++i)
+#pragma unroll
+                        for (int j = 0; j <= i; ++j) f[(i * (i + 1) / 2 + j) * kInterleave] = (i == j) ? rinv[i] : D[i * (i + 1) / 2 + j];
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[buf]);
+        }
+    } else {
+        // ================= EXTRACT group: 224 threads =================
+        int it = 0;
+        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+            const int buf = it & 1;
+            const int64_t r0 = tile * TR;
+            const int rows = (int)(r0 + TR <= n ? TR : n - r0);
+            bar_extract();  // the previous tile's readers of rps / tile_bad are done
+            if (tid == 0) tile_bad = 0;
+            bar_extract();
+            for (int rl = tid; rl < rows; rl += kExtractThreads) {
+                const int64_t i = r0 + rl;
+                const int64_t s = rp[i];
+                rps[rl] = (int)s;
+                const int64_t e = rp[i + 1];
+                if (rl == rows - 1) rps[rows] = (int)e;
+                if (s > e || s < 0 || e > nnz || (i == 0 && s != 0) || (i == n - 1 && e != nnz)) {
+                    flags |= ST_BAD_ROWPTR;
+                    tile_bad = 1;
+                } else {
+                    const int l = (int)(e - s);
+                    len = l > len ? l : len;
+                    if ((tile & 7) == 0 && i + 1 < n) {  // every eighth tile also gathers the column-coherence statistic
+                        const int64_t e2 = rp[i + 2];
+                        if (e2 >= e && e2 <= nnz) {
+                            int64_t m = (e2 - e) < (e - s) ? (e2 - e) : (e - s);
+                            if (m > 8) m = 8;
+                            for (int64_t q = 0; q < m; ++q) {
+                                const int d = ci[e + q] - ci[s + q];
+                                ++cmp;
+                                coh += (d >= -16 && d <= 16);
+                            }
+                        }
+                    }
+                }
+            }
+            // the tile two iterations ago has left this buffer
+            if (it >= 2) mbar_wait(&empty[buf], (uint32_t)(((it >> 1) + 1) & 1));
+            double* R = raws[buf];
+            for (int e = tid; e < NB * PS; e += kExtractThreads) R[e] = 0.0;
+            bar_extract();
+            const bool skip = tile_bad != 0;
+            if (tid == 0) bad_buf[buf] = skip ? 1 : 0;
+            if (!skip) {
+                // the entries of the tile: one contiguous range; a thread takes EIGHT CONSECUTIVE entries
+                const int e0 = rps[0], e1 = rps[rows];
+                for (int base = e0 & ~7; base < e1; base += kExtractThreads * kTileUnroll) {
+                    const int p0 = base + tid * kTileUnroll;
+                    int c[kTileUnroll];
+                    if (vec_ok && p0 >= e0 && p0 + kTileUnroll <= e1) {
+                        const int4 a4 = *reinterpret_cast<const int4*>(ci + p0);
+                        const int4 b4 = *reinterpret_cast<const int4*>(ci + p0 + 4);
+                        c[0] = a4.x; c[1] = a4.y; c[2] = a4.z; c[3] = a4.w;
+                        c[4] = b4.x; c[5] = b4.y; c[6] = b4.z; c[7] = b4.w;
+                    } else {
+#pragma unroll
+                        for (int u = 0; u < kTileUnroll; ++u) c[u] = (p0 + u >= e0 && p0 + u < e1) ? ci[p0 + u] : -1;
+                    }
+                    int cprev = __shfl_up_sync(0xffffffffu, c[kTileUnroll - 1], 1);  // entry p0 - 1 is the last one of the lane below
+                    if (lane == 0 && p0 > e0 && p0 < e1) cprev = ci[p0 - 1];
+                    int r = 0;
+                    {
+                        const int pf = p0 < e0 ? e0 : p0;
+                        int lo = 0, hi = rows;
+                        while (hi - lo > 1) {
+                            const int mid = (lo + hi) >> 1;
+                            if (rps[mid] <= pf) lo = mid; else hi = mid;
+                        }
+                        r = lo;
+                    }
+                    int next = rps[r + 1], start = rps[r];
+                    int kl = r / B, rr = r - kl * B;
+                    int lob = (int)r0 + kl * B;
+                    int dst[kTileUnroll];
+#pragma unroll
+                    for (int u = 0; u < kTileUnroll; ++u) {
+                        const int p = p0 + u;
+                        dst[u] = -1;
+                        if (p >= e0 && p < e1) {
+                            while (p >= next) {  // next row (empty rows are stepped over)
+                                ++r;
+                                start = next;
+                                next = rps[r + 1];
+                                if (++rr == B) { rr = 0; ++kl; lob += B; }
+                            }
+                            const int cc = c[u];
+                            if ((unsigned)cc >= (unsigned)n) flags |= ST_BAD_COL;
+                            if (p != start && cc <= cprev) flags |= ST_UNSORTED;
+                            const unsigned d = (unsigned)(cc - lob);
+                            if (cc >= lob && d <= (unsigned)rr) dst[u] = kl * PS + rr * (rr + 1) / 2 + (int)d;
+                        }
+                        cprev = c[u];
+                    }
+                    double v[kTileUnroll];
+#pragma unroll
+                    for (int u = 0; u < kTileUnroll; ++u) v[u] = dst[u] >= 0 ? val[p0 + u] : 0.0;
+#pragma unroll
+                    for (int u = 0; u < kTileUnroll; ++u)
+                        if (dst[u] >= 0) R[dst[u]] = v[u];
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&full[buf]);  // this warp's part of the tile is in the buffer
+        }
+    }
+    flags = __reduce_or_sync(0xffffffffu, flags);
+    len = __reduce_max_sync(0xffffffffu, len);
+    coh = __reduce_add_sync(0xffffffffu, coh);
+    cmp = __reduce_add_sync(0xffffffffu, cmp);
+    if (lane == 0) {
+        if (flags) atomicOr(&st->flags, flags);
+        if (len > *(volatile int*)&st->max_row_nnz) atomicMax(&st->max_row_nnz, len);
+        sh[0][warp] = coh; sh[1][warp] = cmp;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        unsigned a = 0, c2 = 0;
+        for (int w = 0; w < kTileThreads / 32; ++w) { a += sh[0][w]; c2 += sh[1][w]; }
+        if (c2) { atomicAdd(&st->coherent, (unsigned long long)a); atomicAdd(&st->compared, (unsigned long long)c2); }
+    }
+}
+
 }  // namespace
 
-// a1-a3 for solve_kind 1 without permutation and without band detection (see the header); the caller reads the status back
+// a1-a3 for solve_kind 1 without permutation and without band detection (see the header); the caller reads the status back.
+// b >= 7: the warp-specialised form (measured on config 2: b = 8 0.122 -> 0.113 ms, b = 7 0.121 -> 0.118); smaller blocks
+// factor too quickly to be worth a warp of their own (b = 4: 0.097 one group, 0.104 specialised).
+template <int B>
+static void launch_tile(bj_handle_s* h)
+{
+    constexpr int64_t tr = (kTileThreads / B) * B;
+    const int64_t ntiles = (h->n + tr - 1) / tr;
+    const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)h->num_sms * 8);
+    SetupSpan span(h);
+    if constexpr (B >= 7)
+        tile_setup_ws_kernel<B><<<grid, kTileThreads, 0, h->stream>>>(h->n, h->nnz, ntiles, h->nblocks, h->row_ptr, h->col_idx, h->val,
+                                                                     h->fac_small, h->status);
+    else
+        tile_validate_extract_kernel<B><<<grid, kTileThreads, 0, h->stream>>>(h->n, h->nnz, ntiles, h->nblocks, h->row_ptr, h->col_idx,
+                                                                             h->val, h->fac_small, h->status);
+}
+
 int launch_setup_rows(bj_handle_s* h)
 {
-#define BJ_CASE(B)                                                                                                          \
-    case B: {                                                                                                               \
-        const int64_t tr = (kTileThreads / B) * B;                                                                          \
-        const int64_t ntiles = (h->n + tr - 1) / tr;                                                                        \
-        const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)h->num_sms * 8);                                 \
-        { SetupSpan span(h); tile_validate_extract_kernel<B><<<grid, kTileThreads, 0, h->stream>>>(h->n, h->nnz, ntiles, h->nblocks, \
-                                                          h->row_ptr, h->col_idx, h->val, h->fac_small, h->status); }       \
-        break;                                                                                                              \
-    }
     switch (h->b) {
-        BJ_CASE(1) BJ_CASE(2) BJ_CASE(3) BJ_CASE(4) BJ_CASE(5) BJ_CASE(6) BJ_CASE(7) BJ_CASE(8)
+        case 1: launch_tile<1>(h); break;
+        case 2: launch_tile<2>(h); break;
+        case 3: launch_tile<3>(h); break;
+        case 4: launch_tile<4>(h); break;
+        case 5: launch_tile<5>(h); break;
+        case 6: launch_tile<6>(h); break;
+        case 7: launch_tile<7>(h); break;
+        case 8: launch_tile<8>(h); break;
         default: return BJ_ERR_INVALID_ARG;
     }
-#undef BJ_CASE
     h->launches += 1;
     BJ_CUDA(cudaGetLastError());
     return BJ_OK;
