@@ -212,6 +212,7 @@ tile_validate_extract_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nbl
 // form a third of the warp time was seven warps waiting at the barrier while one factored).  Two shared tiles alternate;
 // the groups hand them over through two pairs of mbarriers (full: 7 arrivals, one per extract warp; empty: 1 arrival).
 constexpr int kExtractThreads = kTileThreads - 32;
+constexpr int kStageCap = 4096;  // entries of a tile staged in shared memory
 __device__ __forceinline__ void bar_extract() { asm volatile("bar.sync 1, %0;" ::"n"(kExtractThreads) : "memory"); }
 
 template <int B>
@@ -228,6 +229,7 @@ tile_setup_ws_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nblocks, co
     __shared__ double raws[2][NB * PS];
     __shared__ unsigned sh[2][kTileThreads / 32];
     __shared__ int tile_bad, bad_buf[2];
+    __shared__ int cis[kStageCap];              // the columns of the tile
     int flags = 0, len = 0;
     unsigned coh = 0, cmp = 0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -339,61 +341,29 @@ tile_setup_ws_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nblocks, co
             const bool skip = tile_bad != 0;
             if (tid == 0) bad_buf[buf] = skip ? 1 : 0;
             if (!skip) {
-                // the entries of the tile: one contiguous range; a thread takes EIGHT CONSECUTIVE entries
+                // The columns of the tile -- one contiguous range -- are staged in shared memory with coalesced loads; then a
+                // thread takes a ROW: it scans the row's columns out of shared memory (checks of a1: range, strictly
+                // ascending) and fetches the value of an entry only if it lies in the lower triangle of the row's diagonal
+                // block.  (An entry-parallel walk with a binary search per eight entries cost ~80 instructions per entry.)
                 const int e0 = rps[0], e1 = rps[rows];
-                for (int base = e0 & ~7; base < e1; base += kExtractThreads * kTileUnroll) {
-                    const int p0 = base + tid * kTileUnroll;
-                    int c[kTileUnroll];
-                    if (vec_ok && p0 >= e0 && p0 + kTileUnroll <= e1) {
-                        const int4 a4 = *reinterpret_cast<const int4*>(ci + p0);
-                        const int4 b4 = *reinterpret_cast<const int4*>(ci + p0 + 4);
-                        c[0] = a4.x; c[1] = a4.y; c[2] = a4.z; c[3] = a4.w;
-                        c[4] = b4.x; c[5] = b4.y; c[6] = b4.z; c[7] = b4.w;
-                    } else {
-#pragma unroll
-                        for (int u = 0; u < kTileUnroll; ++u) c[u] = (p0 + u >= e0 && p0 + u < e1) ? ci[p0 + u] : -1;
+                const bool staged = e1 - e0 <= kStageCap;  // (a tile of very long rows reads its columns from global memory)
+                if (staged)
+                    for (int q = tid; q < e1 - e0; q += kExtractThreads) cis[q] = ci[e0 + q];
+                bar_extract();
+                for (int rl = tid; rl < rows; rl += kExtractThreads) {
+                    const int sr = rps[rl], er = rps[rl + 1];
+                    const int kl = rl / B, rr = rl - kl * B;
+                    const int lob = (int)r0 + kl * B;
+                    double* Rr = R + kl * PS + rr * (rr + 1) / 2;
+                    int prev = -1;
+                    for (int p = sr; p < er; ++p) {
+                        const int cc = staged ? cis[p - e0] : ci[p];
+                        if ((unsigned)cc >= (unsigned)n) flags |= ST_BAD_COL;
+                        if (cc <= prev) flags |= ST_UNSORTED;
+                        prev = cc;
+                        const unsigned d = (unsigned)(cc - lob);
+                        if (cc >= lob && d <= (unsigned)rr) Rr[d] = val[p];
                     }
-                    int cprev = __shfl_up_sync(0xffffffffu, c[kTileUnroll - 1], 1);  // entry p0 - 1 is the last one of the lane below
-                    if (lane == 0 && p0 > e0 && p0 < e1) cprev = ci[p0 - 1];
-                    int r = 0;
-                    {
-                        const int pf = p0 < e0 ? e0 : p0;
-                        int lo = 0, hi = rows;
-                        while (hi - lo > 1) {
-                            const int mid = (lo + hi) >> 1;
-                            if (rps[mid] <= pf) lo = mid; else hi = mid;
-                        }
-                        r = lo;
-                    }
-                    int next = rps[r + 1], start = rps[r];
-                    int kl = r / B, rr = r - kl * B;
-                    int lob = (int)r0 + kl * B;
-                    int dst[kTileUnroll];
-#pragma unroll
-                    for (int u = 0; u < kTileUnroll; ++u) {
-                        const int p = p0 + u;
-                        dst[u] = -1;
-                        if (p >= e0 && p < e1) {
-                            while (p >= next) {  // next row (empty rows are stepped over)
-                                ++r;
-                                start = next;
-                                next = rps[r + 1];
-                                if (++rr == B) { rr = 0; ++kl; lob += B; }
-                            }
-                            const int cc = c[u];
-                            if ((unsigned)cc >= (unsigned)n) flags |= ST_BAD_COL;
-                            if (p != start && cc <= cprev) flags |= ST_UNSORTED;
-                            const unsigned d = (unsigned)(cc - lob);
-                            if (cc >= lob && d <= (unsigned)rr) dst[u] = kl * PS + rr * (rr + 1) / 2 + (int)d;
-                        }
-                        cprev = c[u];
-                    }
-                    double v[kTileUnroll];
-#pragma unroll
-                    for (int u = 0; u < kTileUnroll; ++u) v[u] = dst[u] >= 0 ? val[p0 + u] : 0.0;
-#pragma unroll
-                    for (int u = 0; u < kTileUnroll; ++u)
-                        if (dst[u] >= 0) R[dst[u]] = v[u];
                 }
             }
             __syncwarp();
