@@ -299,33 +299,72 @@ tile_setup_ws_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nblocks, co
         }
     } else {
         // ================= EXTRACT group: 224 threads =================
+        // The row pointers and the columns of the NEXT tile are requested while this tile is worked on and wait in
+        // registers: a tile is then one global latency (the values) instead of a chain of three.
+        constexpr int kPfRp = (TR + kExtractThreads) / kExtractThreads;  // row pointers per thread (TR + 1 in all)
+        constexpr int kPfCi = 9;                                          // columns per thread: tiles of up to 2016 entries
+        int pf_rp[kPfRp], pf_ci[kPfCi], pf_e0 = 0, pf_ne = -1;            // pf_ne < 0: the columns were not prefetched
+        auto prefetch = [&](int64_t tnext) {
+            pf_ne = -1;
+            if (tnext >= ntiles) return;
+            const int64_t r0n = tnext * TR;
+            const int rowsn = (int)(r0n + TR <= n ? TR : n - r0n);
+#pragma unroll
+            for (int u = 0; u < kPfRp; ++u) {
+                const int rl = tid + u * kExtractThreads;
+                pf_rp[u] = rl <= rowsn ? rp[r0n + rl] : 0;
+            }
+            const int64_t e0n = rp[r0n], e1n = rp[r0n + rowsn];
+            if (e0n >= 0 && e0n <= e1n && e1n <= nnz && e1n - e0n <= (int64_t)kExtractThreads * kPfCi) {
+                pf_e0 = (int)e0n;
+                pf_ne = (int)(e1n - e0n);
+#pragma unroll
+                for (int u = 0; u < kPfCi; ++u) {
+                    const int q = tid + u * kExtractThreads;
+                    pf_ci[u] = q < pf_ne ? ci[e0n + q] : 0;
+                }
+            }
+        };
+        prefetch(blockIdx.x);
         int it = 0;
         for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
             const int buf = it & 1;
             const int64_t r0 = tile * TR;
             const int rows = (int)(r0 + TR <= n ? TR : n - r0);
-            bar_extract();  // the previous tile's readers of rps / tile_bad are done
+            bar_extract();  // the previous tile's readers of rps / cis / tile_bad are done
             if (tid == 0) tile_bad = 0;
+#pragma unroll
+            for (int u = 0; u < kPfRp; ++u) {
+                const int rl = tid + u * kExtractThreads;
+                if (rl <= rows) rps[rl] = pf_rp[u];
+            }
+            const int st_e0 = pf_e0, st_ne = pf_ne;  // what the staged columns cover (uniform over the group)
+            if (st_ne >= 0) {
+#pragma unroll
+                for (int u = 0; u < kPfCi; ++u) {
+                    const int q = tid + u * kExtractThreads;
+                    if (q < st_ne) cis[q] = pf_ci[u];
+                }
+            }
             bar_extract();
+            prefetch(tile + gridDim.x);  // in flight during this tile's work
+            // ---- a1 for the row pointers; longest row; coherence sample ----
             for (int rl = tid; rl < rows; rl += kExtractThreads) {
                 const int64_t i = r0 + rl;
-                const int64_t s = rp[i];
-                rps[rl] = (int)s;
-                const int64_t e = rp[i + 1];
-                if (rl == rows - 1) rps[rows] = (int)e;
-                if (s > e || s < 0 || e > nnz || (i == 0 && s != 0) || (i == n - 1 && e != nnz)) {
+                const int64_t sR = rps[rl], eR = rps[rl + 1];
+                if (sR > eR || sR < 0 || eR > nnz || (i == 0 && sR != 0) || (i == n - 1 && eR != nnz)) {
                     flags |= ST_BAD_ROWPTR;
                     tile_bad = 1;
                 } else {
-                    const int l = (int)(e - s);
+                    const int l = (int)(eR - sR);
                     len = l > len ? l : len;
                     if ((tile & 7) == 0 && i + 1 < n) {  // every eighth tile also gathers the column-coherence statistic
                         const int64_t e2 = rp[i + 2];
-                        if (e2 >= e && e2 <= nnz) {
-                            int64_t m = (e2 - e) < (e - s) ? (e2 - e) : (e - s);
+                        if (e2 >= eR && e2 <= nnz) {
+                            int64_t m = (e2 - eR) < (eR - sR) ? (e2 - eR) : (eR - sR);
                             if (m > 8) m = 8;
                             for (int64_t q = 0; q < m; ++q) {
-                                const int d = ci[e + q] - ci[s + q];
+                                const int d = ci[eR + q] - ci[sR + q];
                                 ++cmp;
                                 coh += (d >= -16 && d <= 16);
                             }
@@ -341,15 +380,16 @@ tile_setup_ws_kernel(int64_t n, int64_t nnz, int64_t ntiles, int64_t nblocks, co
             const bool skip = tile_bad != 0;
             if (tid == 0) bad_buf[buf] = skip ? 1 : 0;
             if (!skip) {
-                // The columns of the tile -- one contiguous range -- are staged in shared memory with coalesced loads; then a
-                // thread takes a ROW: it scans the row's columns out of shared memory (checks of a1: range, strictly
+                // A thread takes a ROW: it scans the row's columns out of shared memory (checks of a1: range, strictly
                 // ascending) and fetches the value of an entry only if it lies in the lower triangle of the row's diagonal
                 // block.  (An entry-parallel walk with a binary search per eight entries cost ~80 instructions per entry.)
                 const int e0 = rps[0], e1 = rps[rows];
-                const bool staged = e1 - e0 <= kStageCap;  // (a tile of very long rows reads its columns from global memory)
-                if (staged)
+                bool staged = st_ne >= 0 && st_e0 == e0 && st_ne == e1 - e0;  // (always, for a valid tile that was prefetched)
+                if (!staged && e1 - e0 <= kStageCap) {  // a longer tile: staged now
                     for (int q = tid; q < e1 - e0; q += kExtractThreads) cis[q] = ci[e0 + q];
-                bar_extract();
+                    bar_extract();
+                    staged = true;
+                }
                 for (int rl = tid; rl < rows; rl += kExtractThreads) {
                     const int sr = rps[rl], er = rps[rl + 1];
                     const int kl = rl / B, rr = rl - kl * B;
